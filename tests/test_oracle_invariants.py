@@ -1,0 +1,222 @@
+"""Bookkeeping and geometry pins for the oracle (CPU only).
+
+Fixed from outside the oracle: the disk count is conserved and ids stay a permutation,
+n <= n_max = 4 (L152), every local coordinate lies in (0, w] (Alg. 4 lines 10/21), every configuration is
+overlap-free — checked here with an independent periodic KD-tree in double on the unpacked global
+coordinates — a pure grid shift leaves every global position where it was (L350), and a disk only moves
+when its move was accepted.
+"""
+import math
+
+import numpy as np
+import pytest
+from scipy.spatial import cKDTree
+
+from paper_1211_1646_b200 import inputs as I
+
+
+def min_pair_distance(xy, L):
+    xy = np.mod(xy, np.asarray(L))
+    xy = np.minimum(xy, np.nextafter(np.asarray(L), 0))
+    tree = cKDTree(xy, boxsize=np.asarray(L))
+    d, _ = tree.query(xy, k=2)
+    return d[:, 1].min()
+
+
+def periodic_delta(a, b, L):
+    d = a - b
+    return d - np.asarray(L) * np.round(d / np.asarray(L))
+
+
+def check_state(o, st):
+    n = st["counts"]
+    assert n.sum() == o.N
+    assert n.max() <= 4
+    used = np.arange(4)[None, :] < n[:, None]
+    ids = st["ids"][used]
+    assert np.array_equal(np.sort(ids), np.arange(o.N, dtype=np.uint32))
+    assert np.all(st["ids"][~used] == 0xFFFFFFFF)
+    lx = st["slab"][..., 0][used]
+    ly = st["slab"][..., 1][used]
+    assert np.all(lx > 0) and np.all(lx <= o.real(o.wx))
+    assert np.all(ly > 0) and np.all(ly <= o.real(o.wy))
+
+
+@pytest.mark.parametrize("fp32", [False, True])
+def test_c1_invariants_every_sweep(oracle_mod, fp32):
+    w = I.CONFIGS["C1"]
+    xy, box = I.workload_inputs(w)
+    o = oracle_mod.Oracle(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=fp32)
+    assert (o.mx, o.my) == (86, 74)
+    assert o.wx >= w.sigma and o.wy >= w.sigma
+    o.load_positions(xy)
+    eps = 6e-8 if fp32 else 1.2e-16
+    got = o.get_positions()
+    assert np.abs(periodic_delta(got, xy, o.L_eff)).max() < (2e-4 if fp32 else 1e-12)
+    last = o.acceptance()
+    for sweep in range(30):
+        o.sweep(1)
+        st = o.debug_state()
+        assert st["sweep"] == sweep + 1
+        check_state(o, st)
+        a = o.acceptance()
+        assert a[0] == a[1] + a[2] + a[3]
+        # attempted = n_s per non-empty active cell (reading A10): every non-empty cell once per sweep...
+        assert 0 < a[0] - last[0] <= w.n_s * o.M
+        last = a
+        pos = o.get_positions()
+        assert np.all(pos >= 0) and np.all(pos[:, 0] < o.L_eff[0]) and np.all(pos[:, 1] < o.L_eff[1])
+        assert min_pair_distance(pos, o.L_eff) >= w.sigma * (1 - 4 * eps) - (1e-4 if fp32 else 0)
+    assert last[1] > 0 and last[2] > 0 and last[3] > 0
+
+
+def test_attempted_counts_nonempty_active_cells(oracle_mod):
+    w = I.CONFIGS["C1"]
+    xy, box = I.workload_inputs(w)
+    o = oracle_mod.Oracle(w.N, box, w.sigma, w.d, w.n_s, w.seed)
+    o.load_positions(xy)
+    total = 0
+    for q in range(4):
+        n = o.debug_state()["counts"].reshape(o.my, o.mx)
+        active = n[(q >> 1)::2, (q & 1)::2]
+        total += w.n_s * int((active > 0).sum())
+        o.sub_sweep(q)
+        assert o.acceptance()[0] == total
+
+
+def test_only_accepted_moves_move_disks(oracle_mod):
+    w = I.CONFIGS["C1"]
+    xy, box = I.workload_inputs(w)
+    o = oracle_mod.Oracle(w.N, box, w.sigma, w.d, w.n_s, w.seed)
+    o.load_positions(xy)
+    before = o.debug_state()
+    o.sub_sweep(0)
+    after = o.debug_state()
+    assert np.array_equal(before["ids"], after["ids"]) and np.array_equal(before["counts"], after["counts"])
+    moved_cells = np.any(before["slab"] != after["slab"], axis=(1, 2))
+    x = np.arange(o.M) % o.mx
+    y = np.arange(o.M) // o.mx
+    in_set_a = (x % 2 == 0) & (y % 2 == 0)
+    assert not np.any(moved_cells & ~in_set_a)               # eq. 1: only set a is active
+    assert np.array_equal(moved_cells, after["accept_mask"] != 0)
+    assert np.all(after["accept_mask"] < (1 << w.n_s))
+    acc = o.acceptance()
+    assert acc[1] == sum(bin(int(m)).count("1") for m in after["accept_mask"])
+    # no displacement exceeds d per coordinate times the number of moves of that disk
+    disp = np.abs(after["slab"] - before["slab"])
+    assert disp.max() <= w.d * w.n_s
+
+
+@pytest.mark.parametrize("fp32", [False, True])
+@pytest.mark.parametrize("direction", [0, 1, 2, 3])
+def test_shift_keeps_global_positions(oracle_mod, fp32, direction):
+    w = I.CONFIGS["C1"]
+    xy, box = I.workload_inputs(w)
+    o = oracle_mod.Oracle(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=fp32)
+    o.load_positions(xy)
+    p0 = o.get_positions()
+    s0 = o.debug_state()
+    delta = 0.37 * (o.wx if direction < 2 else o.wy)
+    o.shift(direction, delta)
+    s1 = o.debug_state()
+    check_state(o, s1)
+    p1 = o.get_positions()
+    assert np.abs(periodic_delta(p1, p0, o.L_eff)).max() < (1e-5 if fp32 else 1e-13)
+    axis = 0 if direction < 2 else 1
+    sign = 1.0 if direction % 2 == 0 else -1.0
+    expect = (sign * float(o.real(delta))) % o.L_eff[axis]
+    assert s1["origin"][axis] == pytest.approx(expect, abs=1e-15)
+    assert s1["origin"][1 - axis] == 0.0
+    # some disks changed cell, and the cell counts moved accordingly
+    assert not np.array_equal(s0["counts"], s1["counts"])
+    # +f shift: local coordinates of stayers decrease by delta (disks are translated by -f*delta, L303/L350)
+    c = np.flatnonzero((s0["counts"] == 1) & (s1["counts"] == 1) & (s0["ids"][:, 0] == s1["ids"][:, 0]))
+    assert len(c) > 100
+    dl = s1["slab"][c, 0, axis].astype(np.float64) - s0["slab"][c, 0, axis].astype(np.float64)
+    assert np.allclose(dl, -sign * float(o.real(delta)), atol=2e-6 if fp32 else 1e-15)
+
+
+def test_slot_order_after_shift_is_stayers_then_entrants(oracle_mod):
+    # 4x4 cells of width 1.1; all four disks sit in cell row 0.  A +x shift by 0.3 makes A (cell 1, local
+    # 0.05) and C (cell 2, local 0.10) leave to the cell on their left; B and D stay.  Reading A13 / Alg. 4
+    # lines 7-27: new slot order = stayers (old slot order) then entrants — NOT ascending id.
+    box = (4.4, 4.4)
+    xy = np.array([[1.15, 0.05],    # id 0 = A
+                   [0.70, 1.00],    # id 1 = B
+                   [2.30, 0.05],    # id 2 = C
+                   [1.90, 1.00]])   # id 3 = D
+    o = oracle_mod.Oracle(4, box, 1.0, 0.1, 4, 7)
+    assert (o.mx, o.my) == (4, 4)
+    o.load_positions(xy)
+    st = o.debug_state()
+    assert list(st["ids"].reshape(4, 4, 4)[0, 1][:2]) == [0, 3]      # load order: ascending id
+    o.shift(0, 0.3)
+    st = o.debug_state()
+    ids = st["ids"].reshape(4, 4, 4)
+    cnt = st["counts"].reshape(4, 4)
+    assert cnt[0, 0] == 2 and list(ids[0, 0][:2]) == [1, 0]          # B stays, then A enters
+    assert cnt[0, 1] == 2 and list(ids[0, 1][:2]) == [3, 2]          # D stays, then C enters
+    assert cnt.sum() == 4
+    slab = st["slab"].reshape(4, 4, 4, 2)
+    assert slab[0, 0, 1, 0] == pytest.approx(0.05 - 0.3 + 1.1, abs=1e-12)   # A: l' = l - delta, then + w
+    assert slab[0, 0, 0, 0] == pytest.approx(0.70 - 0.3, abs=1e-12)
+    assert np.allclose(o.get_positions(), xy, atol=1e-14)
+    # and back: a -x shift by the same amount
+    o.shift(1, 0.3)
+    st = o.debug_state()
+    ids = st["ids"].reshape(4, 4, 4)
+    assert list(ids[0, 0][:1]) == [1] and list(ids[0, 1][:2]) == [3, 0] and list(ids[0, 2][:1]) == [2]
+    assert np.allclose(o.get_positions(), xy, atol=1e-14)
+
+
+def test_load_rejects_overlap_and_out_of_box(oracle_mod):
+    box = (4.4, 4.4)
+    o = oracle_mod.Oracle(2, box, 1.0, 0.1, 4, 1)
+    with pytest.raises(oracle_mod.OracleError) as e:
+        o.load_positions(np.array([[1.0, 1.0], [1.5, 1.0]]))
+    assert e.value.code == -4
+    with pytest.raises(oracle_mod.OracleError):
+        o.load_positions(np.array([[1.0, 1.0], [5.5, 1.0]]))
+    with pytest.raises(oracle_mod.OracleError):
+        o.load_positions(np.array([[1.0, 1.0], [float("nan"), 1.0]]))
+    # touching across the periodic boundary is an overlap too
+    with pytest.raises(oracle_mod.OracleError):
+        o.load_positions(np.array([[0.1, 1.0], [4.3, 1.0]]))
+    o.load_positions(np.array([[1.0, 1.0], [2.0, 1.0]]))          # r = sigma exactly: not an overlap (A4)
+    with pytest.raises(oracle_mod.OracleError):
+        oracle_mod.Oracle(2, (1.9, 4.4), 1.0, 0.1, 4, 1)          # mx < 2
+    with pytest.raises(oracle_mod.OracleError):
+        oracle_mod.Oracle(2, box, 1.0, 0.1, 4, 1).sweep(1)        # nothing loaded
+
+
+def test_geometry_of_baseline_configs(oracle_mod):
+    # (mx, my) per config
+    want = {"C1": (86, 74), "C2": (290, 252), "C3": (1152, 998), "C4": (4596, 3980), "C5": (1780, 1540)}
+    for name, (mx, my) in want.items():
+        w = I.CONFIGS[name]
+        box = I.box_for(w.n_side, w.phi, w.sigma)
+        m = [2 * math.floor(box[a] / 2.0) for a in range(2)]
+        assert (m[0], m[1]) == (mx, my)
+        if w.N <= 65536:
+            o = oracle_mod.Oracle(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=w.fp32)
+            assert (o.mx, o.my) == (mx, my)
+            assert 1.0 <= o.wx < math.sqrt(2) and 1.0 <= o.wy < math.sqrt(2)
+
+
+def test_deterministic_and_seed_dependent(oracle_mod):
+    w = I.CONFIGS["C1"]
+    xy, box = I.workload_inputs(w)
+    runs = []
+    for seed in (1, 1, 2):
+        o = oracle_mod.Oracle(w.N, box, w.sigma, w.d, w.n_s, seed)
+        o.load_positions(xy)
+        o.sweep(5)
+        runs.append((o.get_positions(), o.acceptance(), o.debug_state()["digest"]))
+    assert np.array_equal(runs[0][0], runs[1][0]) and runs[0][1:] == runs[1][1:]
+    assert not np.array_equal(runs[0][0], runs[2][0]) and runs[0][2] != runs[2][2]
+    # k sweeps at once == k single sweeps
+    o = oracle_mod.Oracle(w.N, box, w.sigma, w.d, w.n_s, 1)
+    o.load_positions(xy)
+    for _ in range(5):
+        o.sweep(1)
+    assert np.array_equal(o.get_positions(), runs[0][0])
