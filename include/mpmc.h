@@ -1,0 +1,124 @@
+/* mpmc.h — C ABI of the B200-native checkerboard cell sweep for hard disks.
+ *
+ * Method: Anderson, Jankowski, Grubb, Engel, Glotzer, "Massively parallel Monte Carlo for many-particle
+ * simulations on GPUs" (arxiv 1211.1646).  Citations are lines of /root/reference/PAPER.md.
+ *   - one sweep = Algorithm 1 (L60-93): the four checkerboard sets (eq. 1) in a random order, each an
+ *     Algorithm-2 sub-sweep (L164-236) over all cells of the set, then a random cell shift, Algorithm 4
+ *     (L270-342, L350-354);
+ *   - positions live in the cell list in cell-local coordinates (L148-154), n_max = 4 slots per cell (L152);
+ *   - pressure from the pair-distance histogram near contact (L366-382, eq. 4-6).
+ * The readings taken where the paper is silent or garbled are listed in DESIGN.md "Readings".
+ *
+ * Conventions for every call
+ *   - Return value: 0 (MPMC_OK) or a negative MPMC_ERR_* code; nothing throws across the ABI.
+ *   - "device" pointers are CUDA device pointers on the device current at mpmc_create; "host" pointers are
+ *     ordinary host memory.  The library NEVER allocates or frees device memory: the caller provides one
+ *     workspace (mpmc_workspace_bytes) that must outlive the context, and every in/out buffer.
+ *   - All device work is enqueued on the CUDA stream given at creation (a cudaStream_t cast to void*;
+ *     NULL = legacy default stream).  Calls that return host values synchronise that stream; the others are
+ *     asynchronous.  Conditions detected on the device (cell overflow, bad input) set a sticky error word
+ *     that the next synchronising call returns.
+ *   - There is no CPU fallback: without a CUDA device every call except mpmc_workspace_bytes*, mpmc_strerror
+ *     and mpmc_version fails with MPMC_ERR_CUDA.
+ */
+#ifndef MPMC_H_
+#define MPMC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mpmc_ctx mpmc_ctx; /* opaque host object; owns no device memory */
+
+/* error codes */
+#define MPMC_OK 0
+#define MPMC_ERR_ARG (-1)           /* bad argument (NULL pointer, N = 0, n_s > 32, both/neither precision flag ...) */
+#define MPMC_ERR_BOX (-2)           /* box too small: fewer than 2 cells of width >= sigma along an axis, or too many cells */
+#define MPMC_ERR_WORKSPACE (-3)     /* workspace NULL, misaligned (256 B) or smaller than mpmc_workspace_bytes */
+#define MPMC_ERR_OVERLAP (-4)       /* loaded positions overlap, or a coordinate is NaN / outside [0, L] */
+#define MPMC_ERR_CELL_OVERFLOW (-5) /* more than n_max = 4 disks in one cell (possible only when w >= sqrt(2) sigma) */
+#define MPMC_ERR_CUDA (-6)          /* CUDA runtime error (no device, launch failure ...) */
+#define MPMC_ERR_STATE (-7)         /* no positions loaded yet */
+
+/* flags for mpmc_create: exactly one precision bit */
+#define MPMC_FP64 0x1u  /* local coordinates and all move arithmetic in double */
+#define MPMC_FP32 0x2u  /* ... in float (the paper's benchmarks, L390); pressure histogram still in double */
+#define MPMC_DEBUG 0x100u /* record per-cell accept masks and the accept-sequence digest (tests only; slower) */
+
+/* Bytes of device workspace mpmc_create needs for this system (0 on invalid arguments).  Pure host arithmetic.
+ * w_target: requested minimum cell width; <= sigma (e.g. 0) means "smallest width >= sigma that divides the box"
+ * (BASELINE.json configs; reading A11), a value in (sigma, sqrt(2) sigma) gives the paper's regime (L152). */
+size_t mpmc_workspace_bytes(uint64_t N, const double box[2], double sigma, uint32_t flags);
+size_t mpmc_workspace_bytes_ex(uint64_t N, const double box[2], double sigma, double w_target, uint32_t flags);
+
+/* Create a simulation of N hard disks of diameter sigma in the periodic box [0,Lx) x [0,Ly)  (L25, L362).
+ *   box      host, {Lx, Ly}
+ *   d        maximum displacement per coordinate: trial moves are uniform in [-d, d]^2 (reading A2)
+ *   n_s      trial moves per non-empty active cell per sub-sweep (the paper's n_M, L95, L358); 0..32
+ *   seed     user seed, fixed for the run (L170); keys the Philox4x32-10 streams (reading A9)
+ *   workspace  device, 256-byte aligned, >= mpmc_workspace_bytes(...); owned by the caller
+ *   cuda_stream  cudaStream_t as void*
+ * Derived, not passed: mx, my = largest even cell counts with cell width w = L/m >= max(sigma, w_target)
+ * (rounded to the working precision); the simulated box is L_eff = m * w (mpmc_geometry). */
+int mpmc_create(mpmc_ctx** out, uint64_t N, const double box[2], double sigma, double d, uint32_t n_s,
+                uint64_t seed, uint32_t flags, void* workspace, size_t workspace_bytes, void* cuda_stream);
+int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma, double d, uint32_t n_s,
+                   uint64_t seed, uint32_t flags, double w_target, void* workspace, size_t workspace_bytes,
+                   void* cuda_stream);
+int mpmc_destroy(mpmc_ctx* ctx);
+
+/* Geometry chosen at creation (all host out-pointers, any may be NULL): m = {mx, my}, w = {wx, wy} (the working-
+ * precision cell widths as doubles), L_eff = {mx*wx, my*wy}. */
+int mpmc_geometry(const mpmc_ctx* ctx, uint32_t m[2], double w[2], double L_eff[2]);
+
+/* Cell-list build (L148-154): xy = device, N x 2 interleaved doubles, global coordinates in [0, L].  Slots of a
+ * cell are filled in ascending disk index (reading A13).  Resets the grid origin, the sweep index and the
+ * counters.  Synchronises; returns MPMC_ERR_OVERLAP / MPMC_ERR_CELL_OVERFLOW for bad input. */
+int mpmc_load_positions(mpmc_ctx* ctx, const double* xy);
+
+/* k full sweeps of Algorithm 1 (each: 4 sub-sweep kernels + 1 shift kernel, replayed from a CUDA graph).
+ * Asynchronous.  All random draws, including the per-sweep set order and shift, are made on the device from
+ * (seed, sweep index), so there is no host<->device traffic inside the loop. */
+int mpmc_sweep(mpmc_ctx* ctx, uint64_t k);
+
+/* Unpack (L154): xy_out = device, N x 2 doubles, written in the original disk order;
+ * X = (origin + cell*w + local) wrapped into [0, L_eff).  Asynchronous. */
+int mpmc_get_positions(mpmc_ctx* ctx, double* xy_out);
+
+/* out = host, {attempted, accepted, rejected_boundary, rejected_overlap} since the last load.  attempted counts
+ * n_s per non-empty active cell (reading A10; eta = attempted / time, L421).  Synchronises. */
+int mpmc_acceptance(mpmc_ctx* ctx, uint64_t out[4]);
+
+/* Contact pressure (L366-382).  hist_out = host, nbins counts of unordered pairs with r in [sigma + i dr,
+ * sigma + (i+1) dr), computed on the device in double; g_contact = polynomial fit (unweighted least squares,
+ * given degree < nbins) of g(R_i) (eq. 5-6) extrapolated to r = sigma; p_star = eq. 4.  hist_out, g_contact,
+ * p_star may each be NULL.  nbins <= 4096.  Synchronises. */
+int mpmc_pressure_contact(mpmc_ctx* ctx, double dr, uint32_t nbins, uint32_t degree, uint64_t* hist_out,
+                          double* g_contact, double* p_star);
+
+/* Test hooks: single pieces of Algorithm 1 at the current sweep index (do not advance it). */
+int mpmc_debug_sub_sweep(mpmc_ctx* ctx, uint32_t checkerboard_set /*0=a(0,0) 1=b(1,0) 2=c(0,1) 3=d(1,1)*/);
+int mpmc_debug_shift(mpmc_ctx* ctx, uint32_t direction /*0:+x 1:-x 2:+y 3:-y*/, double delta);
+
+/* Test hook: the state in a layout-independent canonical form, cell c = y*mx + x.  Device out-pointers (any may
+ * be NULL): counts u32[M]; slab real[M][4][2] (real = float or double per the precision flag; unused slots 0);
+ * ids u32[M][4] (unused 0xFFFFFFFF); accept_mask u32[M] (bit s = move s of the cell accepted in the last sweep;
+ * needs MPMC_DEBUG).  Host out-pointers (any may be NULL): origin[2], sweep index, accept-sequence digest.
+ * Synchronises. */
+int mpmc_debug_state(mpmc_ctx* ctx, void* counts, void* slab, void* ids, void* accept_mask, double origin[2],
+                     uint64_t* sweep, uint64_t* digest);
+
+/* Test hook: Philox4x32-10 evaluated ON THE DEVICE by the same routine the kernels use.
+ * ctr = device u32[n][4], key = host u32[2], out = device u32[n][4]; enqueued on cuda_stream and synchronised. */
+int mpmc_debug_philox(const uint32_t* ctr, const uint32_t key[2], uint32_t* out, uint32_t n, void* cuda_stream);
+
+const char* mpmc_strerror(int code);
+const char* mpmc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MPMC_H_ */

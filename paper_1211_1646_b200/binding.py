@@ -1,0 +1,206 @@
+"""Thin Python binding of include/mpmc.h (ctypes).  Argument marshalling only: every step of the path runs in
+the CUDA kernels behind the C ABI.  PyTorch supplies device memory and the stream, nothing else.
+
+There is no CPU fallback: a missing library or a missing CUDA device raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+from . import build as _build
+
+FP64 = 0x1
+FP32 = 0x2
+DEBUG = 0x100
+
+_u32, _u64, _dbl, _vp, _sz = C.c_uint32, C.c_uint64, C.c_double, C.c_void_p, C.c_size_t
+
+# every symbol include/mpmc.h declares: name -> (restype, argtypes)
+SYMBOLS = {
+    "mpmc_workspace_bytes": (_sz, [_u64, C.POINTER(_dbl), _dbl, _u32]),
+    "mpmc_workspace_bytes_ex": (_sz, [_u64, C.POINTER(_dbl), _dbl, _dbl, _u32]),
+    "mpmc_create": (C.c_int, [C.POINTER(_vp), _u64, C.POINTER(_dbl), _dbl, _dbl, _u32, _u64, _u32, _vp, _sz, _vp]),
+    "mpmc_create_ex": (C.c_int, [C.POINTER(_vp), _u64, C.POINTER(_dbl), _dbl, _dbl, _u32, _u64, _u32, _dbl, _vp, _sz, _vp]),
+    "mpmc_destroy": (C.c_int, [_vp]),
+    "mpmc_geometry": (C.c_int, [_vp, C.POINTER(_u32), C.POINTER(_dbl), C.POINTER(_dbl)]),
+    "mpmc_load_positions": (C.c_int, [_vp, _vp]),
+    "mpmc_sweep": (C.c_int, [_vp, _u64]),
+    "mpmc_get_positions": (C.c_int, [_vp, _vp]),
+    "mpmc_acceptance": (C.c_int, [_vp, C.POINTER(_u64)]),
+    "mpmc_pressure_contact": (C.c_int, [_vp, _dbl, _u32, _u32, _vp, C.POINTER(_dbl), C.POINTER(_dbl)]),
+    "mpmc_debug_sub_sweep": (C.c_int, [_vp, _u32]),
+    "mpmc_debug_shift": (C.c_int, [_vp, _u32, _dbl]),
+    "mpmc_debug_state": (C.c_int, [_vp, _vp, _vp, _vp, _vp, C.POINTER(_dbl), C.POINTER(_u64), C.POINTER(_u64)]),
+    "mpmc_debug_philox": (C.c_int, [_vp, C.POINTER(_u32), _vp, _u32, _vp]),
+    "mpmc_strerror": (C.c_char_p, [C.c_int]),
+    "mpmc_version": (C.c_char_p, []),
+}
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def lib() -> C.CDLL:
+    """Load libmpmc_b200.so (built in-tree by build.py / __graft_entry__.build()).  Raises if it is missing."""
+    global _lib
+    if _lib is None:
+        path = library_path()
+        if not os.path.exists(path):
+            raise RuntimeError(f"{path} is missing: run `python -m paper_1211_1646_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(path)
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+class MpmcError(RuntimeError):
+    def __init__(self, code: int):
+        super().__init__(f"mpmc error {code}: {lib().mpmc_strerror(code).decode()}")
+        self.code = code
+
+
+def _chk(code: int) -> None:
+    if code != 0:
+        raise MpmcError(code)
+
+
+def workspace_bytes(N: int, box, sigma: float, fp32: bool, debug: bool = False, w_target: float = 0.0) -> int:
+    b = (_dbl * 2)(float(box[0]), float(box[1]))
+    flags = (FP32 if fp32 else FP64) | (DEBUG if debug else 0)
+    return int(lib().mpmc_workspace_bytes_ex(int(N), b, float(sigma), float(w_target), flags))
+
+
+class Mpmc:
+    """mpmc_* calls on torch CUDA tensors.  Same call list as the C ABI."""
+
+    def __init__(self, N: int, box, sigma: float, d: float, n_s: int, seed: int, fp32: bool = False,
+                 debug: bool = False, w_target: float = 0.0, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1211_1646_b200 needs a CUDA device; there is no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        self.N, self.fp32, self.debug, self.sigma = int(N), bool(fp32), bool(debug), float(sigma)
+        self.flags = (FP32 if fp32 else FP64) | (DEBUG if debug else 0)
+        nbytes = workspace_bytes(N, box, sigma, fp32, debug, w_target)
+        if nbytes == 0:
+            # let mpmc_create report the precise error code
+            nbytes = 256
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self._h = _vp()
+            b = (_dbl * 2)(float(box[0]), float(box[1]))
+            _chk(lib().mpmc_create_ex(C.byref(self._h), self.N, b, float(sigma), float(d), int(n_s), int(seed),
+                                      self.flags, float(w_target), self.workspace.data_ptr(), nbytes,
+                                      self.stream.cuda_stream))
+        m = (_u32 * 2)()
+        w = (_dbl * 2)()
+        Le = (_dbl * 2)()
+        _chk(lib().mpmc_geometry(self._h, m, w, Le))
+        self.mx, self.my = int(m[0]), int(m[1])
+        self.wx, self.wy = float(w[0]), float(w[1])
+        self.L_eff = (float(Le[0]), float(Le[1]))
+        self.M = self.mx * self.my
+        self.real = torch.float32 if fp32 else torch.float64
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            lib().mpmc_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # --- the calls of include/mpmc.h -------------------------------------------------------------------
+    def load_positions(self, xy) -> None:
+        """xy: (N, 2) float64 CUDA tensor (device pointer passed through)."""
+        t = self.torch
+        assert xy.is_cuda and xy.dtype == t.float64 and tuple(xy.shape) == (self.N, 2) and xy.is_contiguous()
+        with t.cuda.device(self.device):
+            _chk(lib().mpmc_load_positions(self._h, xy.data_ptr()))
+
+    def sweep(self, k: int = 1) -> None:
+        with self.torch.cuda.device(self.device):
+            _chk(lib().mpmc_sweep(self._h, int(k)))
+
+    def get_positions(self, out=None):
+        t = self.torch
+        if out is None:
+            out = t.empty((self.N, 2), dtype=t.float64, device=self.device)
+        with t.cuda.device(self.device):
+            _chk(lib().mpmc_get_positions(self._h, out.data_ptr()))
+        return out
+
+    def acceptance(self):
+        o = (_u64 * 4)()
+        with self.torch.cuda.device(self.device):
+            _chk(lib().mpmc_acceptance(self._h, o))
+        return tuple(int(v) for v in o)
+
+    def pressure_contact(self, dr: float, nbins: int, degree: int):
+        import numpy as np
+        h = np.zeros(nbins, dtype=np.uint64)
+        g0, ps = _dbl(), _dbl()
+        with self.torch.cuda.device(self.device):
+            _chk(lib().mpmc_pressure_contact(self._h, float(dr), int(nbins), int(degree), h.ctypes.data,
+                                             C.byref(g0), C.byref(ps)))
+        return h, g0.value, ps.value
+
+    def contact_histogram(self, dr: float, nbins: int):
+        import numpy as np
+        h = np.zeros(nbins, dtype=np.uint64)
+        with self.torch.cuda.device(self.device):
+            _chk(lib().mpmc_pressure_contact(self._h, float(dr), int(nbins), 0, h.ctypes.data, None, None))
+        return h
+
+    # --- test hooks ------------------------------------------------------------------------------------
+    def sub_sweep(self, checkerboard_set: int) -> None:
+        with self.torch.cuda.device(self.device):
+            _chk(lib().mpmc_debug_sub_sweep(self._h, int(checkerboard_set)))
+
+    def shift(self, direction: int, delta: float) -> None:
+        with self.torch.cuda.device(self.device):
+            _chk(lib().mpmc_debug_shift(self._h, int(direction), float(delta)))
+
+    def debug_state(self) -> dict:
+        t = self.torch
+        counts = t.empty(self.M, dtype=t.int32, device=self.device)
+        slab = t.empty((self.M, 4, 2), dtype=self.real, device=self.device)
+        ids = t.empty((self.M, 4), dtype=t.int32, device=self.device)
+        mask = t.empty(self.M, dtype=t.int32, device=self.device) if self.debug else None
+        origin = (_dbl * 2)()
+        sw, dg = _u64(), _u64()
+        with t.cuda.device(self.device):
+            _chk(lib().mpmc_debug_state(self._h, counts.data_ptr(), slab.data_ptr(), ids.data_ptr(),
+                                        mask.data_ptr() if mask is not None else None, origin,
+                                        C.byref(sw), C.byref(dg)))
+        import numpy as np
+        return dict(counts=counts.cpu().numpy().view(np.uint32), slab=slab.cpu().numpy(),
+                    ids=ids.cpu().numpy().view(np.uint32),
+                    accept_mask=mask.cpu().numpy().view(np.uint32) if mask is not None else None,
+                    origin=(origin[0], origin[1]), sweep=int(sw.value), digest=int(dg.value))
+
+
+def device_philox(ctr, key, device="cuda:0"):
+    """Philox4x32-10 on the device (test hook).  ctr: (n, 4) integer array-like."""
+    import numpy as np
+    import torch
+    c = torch.as_tensor(np.asarray(ctr, dtype=np.uint32).astype(np.int64), device=device).to(torch.int32).contiguous()
+    n = c.shape[0]
+    out = torch.empty((n, 4), dtype=torch.int32, device=device)
+    k = (_u32 * 2)(int(key[0]) & 0xFFFFFFFF, int(key[1]) & 0xFFFFFFFF)
+    with torch.cuda.device(device):
+        _chk(lib().mpmc_debug_philox(c.data_ptr(), k, out.data_ptr(), n, torch.cuda.current_stream().cuda_stream))
+    return out.cpu().numpy().view(np.uint32)

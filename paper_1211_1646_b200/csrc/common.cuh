@@ -1,0 +1,169 @@
+// common.cuh — data layout, control block, Philox4x32-10 and variates for the sm_100a MPMC kernels.
+//
+// Product code (CUDA path).  Shares nothing with oracle/.  Compile with -fmad=false: every floating-point
+// operation below is ONE IEEE round-to-nearest operation, and the only fused multiply-add of the method (the
+// squared distance) is written __fma_rn / __fmaf_rn explicitly, so results are bit-identical to a plain CPU
+// evaluation of the same formulas.
+//
+// Layout in HBM ("colour-split slot planes"): the four checkerboard sets of
+// PAPER.md eq. 1 (L43) are stored as four dense sub-grids of hx x hy = (mx/2) x (my/2) cells, cell (x, y) at
+//   colour Q = 2 (y & 1) + (x & 1),   index ci = (y >> 1) * hx + (x >> 1),
+// and the n_max = 4 slots of a cell (L150, L152) are four separate planes:
+//   cnt[buf][Q][ci]            u8      number of disks n[x, y]
+//   pos[buf][Q][slot][ci]      real2   cell-local coordinates (L154), valid for slot < n
+//   ids[buf][Q][slot][ci]      u32     original disk index
+// so a warp that works on 32 consecutive active cells reads 32 consecutive real2 per slot (one or two 128-B
+// lines), its eight neighbour cells are dense rows of the three other colours, and slots beyond the occupancy
+// (2 and 3 at w ~ sigma) are never touched.  This generalises the even/odd-x split of the paper's Algorithm 3
+// (L241-258) to both axes.  buf = 0/1 is the double buffer of the cell shift (L350).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mpmc {
+
+constexpr int NMAX = 4;                       // n_max
+constexpr uint32_t SLOT_SHUFFLE = 0x80000000u;  // Philox counter word 3 for the cell's shuffle words
+constexpr uint32_t CELL_GLOBAL = 0xFFFFFFFFu;   // counter word 0 for per-sweep draws
+constexpr uint32_t SLOT_ORDER = 0xFFFFFFFFu;    // set order + shift direction
+constexpr uint32_t SLOT_DIST = 0xFFFFFFFEu;     // shift distance
+
+// sticky device error bits (Ctl::err)
+constexpr uint32_t ERRBIT_OVERFLOW = 1u;  // a cell would hold more than NMAX disks
+constexpr uint32_t ERRBIT_RANGE = 2u;     // loaded coordinate NaN or outside [0, L]
+constexpr uint32_t ERRBIT_OVERLAP = 4u;   // loaded positions overlap
+
+// Device-resident control block: everything that changes from sweep to sweep, so that a captured CUDA graph
+// can be replayed with no host-side argument updates (mpmc.h, mpmc_sweep).
+struct Ctl {
+  unsigned long long t;            // sweep index
+  uint32_t order[4];               // checkerboard sets in the order they run this sweep (Alg. 1 line 2, L64)
+  uint32_t dir;                    // shift direction 0:+x 1:-x 2:+y 3:-y (Alg. 1 line 16, L91)
+  uint32_t dist_word;              // random word the shift distance is made of (Alg. 1 line 15, L90)
+  uint32_t cur;                    // which buffer holds the current state
+  uint32_t err;                    // sticky error bits
+  uint32_t ticket;                 // blocks-done counter of the shift kernel
+  uint32_t pad0;
+  double origin[2];                // grid origin: X = origin + cell * w + local
+  unsigned long long counters[3];  // accepted, rejected_boundary, rejected_overlap
+  unsigned long long digest;       // accept-sequence digest (MPMC_DEBUG)
+};
+
+// Kernel parameters (by value, __grid_constant__): geometry and the workspace pointers.
+struct Params {
+  uint32_t mx, my, hx, hy;   // cells; hx = mx/2, hy = my/2
+  uint32_t Mq, Mqp;          // cells per colour; plane stride (Mq rounded up to 64)
+  uint32_t n_s, N;
+  uint32_t seed_lo, seed_hi;
+  float wx_f, wy_f, sigma2_f, d_f;      // working-precision constants (fp32 mode)
+  double wx_p, wy_p, sigma2_p, d_p;     // working-precision constants (fp64 mode)
+  double wx_d, wy_d;                    // (double) of the working-precision widths
+  double Lx_eff, Ly_eff, sigma_d;
+  double Lx_user, Ly_user;              // the caller's box (input range check)
+  Ctl* ctl;
+  uint8_t* cnt[2];
+  void* pos[2];
+  uint32_t* ids[2];
+  uint32_t* cnt32;                      // scratch: u32 counters for the cell-list build
+  unsigned long long* hist;             // scratch: contact histogram
+  uint32_t* mask;                       // MPMC_DEBUG: accept masks, canonical index y*mx+x; else nullptr
+};
+
+template <typename P> struct Real;
+template <> struct Real<float> {
+  using T2 = float2;
+  static __device__ __forceinline__ float wx(const Params& p) { return p.wx_f; }
+  static __device__ __forceinline__ float wy(const Params& p) { return p.wy_f; }
+  static __device__ __forceinline__ float sigma2(const Params& p) { return p.sigma2_f; }
+  static __device__ __forceinline__ float d(const Params& p) { return p.d_f; }
+  static __device__ __forceinline__ float add(float a, float b) { return __fadd_rn(a, b); }
+  static __device__ __forceinline__ float sub(float a, float b) { return __fsub_rn(a, b); }
+  static __device__ __forceinline__ float mul(float a, float b) { return __fmul_rn(a, b); }
+  static __device__ __forceinline__ float fma(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+  // symmetric unit variate: odd integer of magnitude < 2^24 times 2^-24 (exact; never 0)
+  static __device__ __forceinline__ float sym(uint32_t R) {
+    return __fmul_rn((float)((int)(2u * (R >> 8) + 1u) - (1 << 24)), 0x1p-24f);
+  }
+  static __device__ __forceinline__ float unit(uint32_t R) { return __fmul_rn((float)(R >> 8), 0x1p-24f); }
+  static __device__ __forceinline__ float far_away() { return 1.0e18f; }   // sentinel: never overlaps
+};
+template <> struct Real<double> {
+  using T2 = double2;
+  static __device__ __forceinline__ double wx(const Params& p) { return p.wx_p; }
+  static __device__ __forceinline__ double wy(const Params& p) { return p.wy_p; }
+  static __device__ __forceinline__ double sigma2(const Params& p) { return p.sigma2_p; }
+  static __device__ __forceinline__ double d(const Params& p) { return p.d_p; }
+  static __device__ __forceinline__ double add(double a, double b) { return __dadd_rn(a, b); }
+  static __device__ __forceinline__ double sub(double a, double b) { return __dsub_rn(a, b); }
+  static __device__ __forceinline__ double mul(double a, double b) { return __dmul_rn(a, b); }
+  static __device__ __forceinline__ double fma(double a, double b, double c) { return __fma_rn(a, b, c); }
+  static __device__ __forceinline__ double sym(uint32_t R) {
+    return __dmul_rn((double)(2ll * (long long)R + 1ll - (1ll << 32)), 0x1p-32);
+  }
+  static __device__ __forceinline__ double unit(uint32_t R) { return __dmul_rn((double)R, 0x1p-32); }
+  static __device__ __forceinline__ double far_away() { return 1.0e150; }
+};
+
+// Philox4x32-10 (Salmon et al., SC'11).  Ten rounds of two 32x32->64 multiplies and xors; the key schedule
+// adds the Weyl constants.  counter = (c0..c3), key = (k0, k1).
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                              uint32_t k1, uint32_t (&out)[4]) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;
+    const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    c1 = (uint32_t)p1;
+    c3 = (uint32_t)p0;
+    c0 = n0;
+    c2 = n2;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+__device__ __forceinline__ uint32_t bounded(uint32_t word, uint32_t bound) { return __umulhi(word, bound); }
+
+// Per-sweep draws (Alg. 1 lines 2, 15, 16; reading A9): Fisher-Yates of the four sets with
+// words G0..G2, direction from the top two bits of G3, distance word from a second counter.
+__device__ __forceinline__ void draw_sweep(const Params& p, unsigned long long t, Ctl* ctl) {
+  uint32_t G[4], H[4];
+  philox4x32_10(CELL_GLOBAL, (uint32_t)t, (uint32_t)(t >> 32), SLOT_ORDER, p.seed_lo, p.seed_hi, G);
+  uint32_t o[4] = {0, 1, 2, 3};
+#pragma unroll
+  for (int i = 3; i >= 1; --i) {
+    const uint32_t j = bounded(G[3 - i], (uint32_t)i + 1u);
+    const uint32_t a = o[i];
+    // o[j] with j dynamic: select chain keeps o[] in registers
+    const uint32_t b = j == 0 ? o[0] : j == 1 ? o[1] : j == 2 ? o[2] : o[3];
+    if (j == 0) o[0] = a; else if (j == 1) o[1] = a; else if (j == 2) o[2] = a; else o[3] = a;
+    o[i] = b;
+  }
+  philox4x32_10(CELL_GLOBAL, (uint32_t)t, (uint32_t)(t >> 32), SLOT_DIST, p.seed_lo, p.seed_hi, H);
+  ctl->order[0] = o[0]; ctl->order[1] = o[1]; ctl->order[2] = o[2]; ctl->order[3] = o[3];
+  ctl->dir = G[3] >> 30;
+  ctl->dist_word = H[0];
+}
+
+// plane addressing
+template <typename P>
+__device__ __forceinline__ typename Real<P>::T2* pos_plane(const Params& p, uint32_t buf, uint32_t Q, uint32_t slot) {
+  return reinterpret_cast<typename Real<P>::T2*>(p.pos[buf]) + (size_t)(Q * NMAX + slot) * p.Mqp;
+}
+__device__ __forceinline__ uint32_t* ids_plane(const Params& p, uint32_t buf, uint32_t Q, uint32_t slot) {
+  return p.ids[buf] + (size_t)(Q * NMAX + slot) * p.Mqp;
+}
+__device__ __forceinline__ uint8_t* cnt_plane(const Params& p, uint32_t buf, uint32_t Q) {
+  return p.cnt[buf] + (size_t)Q * p.Mqp;
+}
+
+__device__ __forceinline__ unsigned long long mix64(unsigned long long z) {  // splitmix64 finaliser (digest only)
+  z += 0x9E3779B97F4A7C15ull;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+}  // namespace mpmc

@@ -1,0 +1,418 @@
+// mpmc.cu — host side of the C ABI declared in include/mpmc.h.  Product code (CUDA path); no CPU fallback.
+// Build: nvcc -gencode arch=compute_100a,code=sm_100a -fmad=false -lineinfo -shared (see ../build.py).
+#include "../../include/mpmc.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "aux.cuh"
+#include "common.cuh"
+#include "sweep.cuh"
+
+using namespace mpmc;
+
+struct mpmc_ctx {
+  Params p;
+  uint64_t N;
+  uint32_t flags;
+  bool fp32, debug, loaded;
+  int nf;                  // register-resident neighbour slots per cell of the sub-sweep kernel (2 or 4)
+  cudaStream_t stream;
+  cudaGraphExec_t graph1;  // one sweep
+  cudaGraphExec_t graphK;  // GRAPH_BATCH sweeps
+  int sticky;
+};
+
+namespace {
+
+constexpr uint32_t GRAPH_BATCH = 16;
+constexpr size_t ALIGN = 256;
+constexpr uint32_t MAX_BINS = 4096;
+
+inline size_t up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Geom {
+  uint32_t m[2];
+  double w0[2];    // L/m in double
+  double wp[2];    // rounded to the working precision, as double
+};
+
+// Setup (reading A11): mx, my = largest even integers with w = P(L/m) >= P(max(sigma, w_target)).
+int geometry(const double box[2], double sigma, double w_target, bool fp32, Geom* g) {
+  if (!box || !(sigma > 0) || !(box[0] > 0) || !(box[1] > 0)) return MPMC_ERR_ARG;
+  const double wmin = (w_target > sigma) ? w_target : sigma;
+  for (int a = 0; a < 2; ++a) {
+    const double q = std::floor(box[a] / (2.0 * wmin));
+    if (!(q >= 1.0) || q > 1e9) return MPMC_ERR_BOX;
+    long long mm = 2 * (long long)q;
+    for (;;) {
+      if (mm < 2) return MPMC_ERR_BOX;
+      const double w0 = box[a] / (double)mm;
+      const bool ok = fp32 ? ((float)w0 >= (float)wmin) : (w0 >= wmin);
+      if (ok) break;
+      mm -= 2;
+    }
+    g->m[a] = (uint32_t)mm;
+    g->w0[a] = box[a] / (double)mm;
+    g->wp[a] = fp32 ? (double)(float)g->w0[a] : g->w0[a];
+  }
+  if ((uint64_t)g->m[0] * g->m[1] >= 0xFFFFFFFFull / NMAX) return MPMC_ERR_BOX;
+  return MPMC_OK;
+}
+
+struct Layout {
+  uint32_t Mq, Mqp;
+  size_t off_ctl, off_hist, off_cnt32, off_cnt[2], off_pos[2], off_ids[2], off_mask, total;
+};
+
+Layout layout(const Geom& g, bool fp32, bool debug) {
+  Layout L;
+  L.Mq = (g.m[0] / 2) * (g.m[1] / 2);
+  L.Mqp = (uint32_t)up(L.Mq, 64);
+  const size_t real2 = fp32 ? 8 : 16;
+  size_t o = 0;
+  L.off_ctl = o; o += up(sizeof(Ctl), ALIGN);
+  L.off_hist = o; o += up((size_t)MAX_BINS * 8, ALIGN);
+  L.off_cnt32 = o; o += up((size_t)4 * L.Mqp * 4, ALIGN);
+  for (int b = 0; b < 2; ++b) { L.off_cnt[b] = o; o += up((size_t)4 * L.Mqp, ALIGN); }
+  for (int b = 0; b < 2; ++b) { L.off_pos[b] = o; o += up((size_t)4 * NMAX * L.Mqp * real2, ALIGN); }
+  for (int b = 0; b < 2; ++b) { L.off_ids[b] = o; o += up((size_t)4 * NMAX * L.Mqp * 4, ALIGN); }
+  L.off_mask = o;
+  if (debug) o += up((size_t)g.m[0] * g.m[1] * 4, ALIGN);
+  L.total = o;
+  return L;
+}
+
+bool precision_ok(uint32_t flags) { return ((flags & MPMC_FP64) != 0) != ((flags & MPMC_FP32) != 0); }
+
+int cuda_fail(cudaError_t e) {
+  if (e == cudaSuccess) return MPMC_OK;
+  std::fprintf(stderr, "[mpmc] CUDA error: %s\n", cudaGetErrorString(e));
+  return MPMC_ERR_CUDA;
+}
+#define CU(x) do { cudaError_t e__ = (x); if (e__ != cudaSuccess) return cuda_fail(e__); } while (0)
+
+dim3 cell_grid(const mpmc_ctx* c, int threads) { return dim3((c->p.Mq + threads - 1) / threads, 4, 1); }
+
+// ---- kernel launchers ----------------------------------------------------------------------------------
+template <typename P, bool DEBUG>
+void launch_sub_nf(const mpmc_ctx* c, uint32_t setk) {
+  const dim3 grid((c->p.Mq + SUB_THREADS - 1) / SUB_THREADS);
+  if (c->nf == 2) k_sub_sweep<P, 2, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk);
+  else            k_sub_sweep<P, 4, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk);
+}
+void launch_sub(const mpmc_ctx* c, uint32_t setk) {
+  if (c->fp32) { if (c->debug) launch_sub_nf<float, true>(c, setk); else launch_sub_nf<float, false>(c, setk); }
+  else         { if (c->debug) launch_sub_nf<double, true>(c, setk); else launch_sub_nf<double, false>(c, setk); }
+}
+void launch_shift(const mpmc_ctx* c, uint32_t ovr, uint32_t dir, double delta) {
+  const dim3 grid = cell_grid(c, SHIFT_THREADS);
+  if (c->fp32) k_shift<float><<<grid, SHIFT_THREADS, 0, c->stream>>>(c->p, ovr, dir, delta);
+  else         k_shift<double><<<grid, SHIFT_THREADS, 0, c->stream>>>(c->p, ovr, dir, delta);
+}
+void enqueue_sweep(const mpmc_ctx* c) {       // Algorithm 1: 4 sub-sweeps + shift
+  for (uint32_t k = 0; k < 4; ++k) launch_sub(c, k);
+  launch_shift(c, 0, 0, 0.0);
+}
+
+int build_graph(mpmc_ctx* c, uint32_t sweeps, cudaGraphExec_t* out) {
+  cudaGraph_t g = nullptr;
+  CU(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+  for (uint32_t i = 0; i < sweeps; ++i) enqueue_sweep(c);
+  CU(cudaStreamEndCapture(c->stream, &g));
+  cudaError_t e = cudaGraphInstantiate(out, g, 0);
+  cudaGraphDestroy(g);
+  return cuda_fail(e);
+}
+
+int read_ctl(mpmc_ctx* c, Ctl* h) {
+  CU(cudaMemcpyAsync(h, c->p.ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  if (h->err & ERRBIT_OVERFLOW) c->sticky = MPMC_ERR_CELL_OVERFLOW;
+  else if (h->err & (ERRBIT_OVERLAP | ERRBIT_RANGE)) c->sticky = MPMC_ERR_OVERLAP;
+  return c->sticky;
+}
+
+// Unweighted least-squares polynomial of the given degree through (t_i, y_i); returns the value at t = 0.
+// Householder QR on the Vandermonde matrix (host, double).
+bool polyfit_at_zero(const std::vector<double>& t, const std::vector<double>& y, uint32_t degree, double* value) {
+  const size_t n = t.size(), m = degree + 1;
+  if (n < m) return false;
+  std::vector<double> A(n * m), b(y);
+  for (size_t i = 0; i < n; ++i) { double pw = 1.0; for (size_t j = 0; j < m; ++j) { A[i * m + j] = pw; pw *= t[i]; } }
+  for (size_t k = 0; k < m; ++k) {
+    double norm = 0; for (size_t i = k; i < n; ++i) norm += A[i * m + k] * A[i * m + k];
+    norm = std::sqrt(norm);
+    if (norm == 0) return false;
+    const double alpha = A[k * m + k] > 0 ? -norm : norm;
+    std::vector<double> v(n - k);
+    for (size_t i = k; i < n; ++i) v[i - k] = A[i * m + k];
+    v[0] -= alpha;
+    double vn = 0; for (double x : v) vn += x * x;
+    if (vn == 0) continue;
+    for (size_t j = k; j < m; ++j) {
+      double s = 0; for (size_t i = k; i < n; ++i) s += v[i - k] * A[i * m + j];
+      s = 2 * s / vn;
+      for (size_t i = k; i < n; ++i) A[i * m + j] -= s * v[i - k];
+    }
+    double s = 0; for (size_t i = k; i < n; ++i) s += v[i - k] * b[i];
+    s = 2 * s / vn;
+    for (size_t i = k; i < n; ++i) b[i] -= s * v[i - k];
+  }
+  std::vector<double> c(m);
+  for (size_t kk = m; kk-- > 0;) {
+    double s = b[kk];
+    for (size_t j = kk + 1; j < m; ++j) s -= A[kk * m + j] * c[j];
+    if (A[kk * m + kk] == 0) return false;
+    c[kk] = s / A[kk * m + kk];
+  }
+  *value = c[0];
+  return true;
+}
+
+}  // namespace
+
+// =========================================================================================================
+extern "C" {
+
+size_t mpmc_workspace_bytes_ex(uint64_t N, const double box[2], double sigma, double w_target, uint32_t flags) {
+  if (N == 0 || N >= 0xFFFFFFFFull || !precision_ok(flags)) return 0;
+  Geom g;
+  if (geometry(box, sigma, w_target, (flags & MPMC_FP32) != 0, &g) != MPMC_OK) return 0;
+  return layout(g, (flags & MPMC_FP32) != 0, (flags & MPMC_DEBUG) != 0).total;
+}
+size_t mpmc_workspace_bytes(uint64_t N, const double box[2], double sigma, uint32_t flags) {
+  return mpmc_workspace_bytes_ex(N, box, sigma, 0.0, flags);
+}
+
+int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma, double d, uint32_t n_s,
+                   uint64_t seed, uint32_t flags, double w_target, void* workspace, size_t workspace_bytes,
+                   void* cuda_stream) {
+  if (!out || !box || N == 0 || N >= 0xFFFFFFFFull || !(sigma > 0) || !(d > 0) || n_s > 32 || !precision_ok(flags))
+    return MPMC_ERR_ARG;
+  const bool fp32 = (flags & MPMC_FP32) != 0, debug = (flags & MPMC_DEBUG) != 0;
+  Geom g;
+  const int st = geometry(box, sigma, w_target, fp32, &g);
+  if (st != MPMC_OK) return st;
+  const Layout L = layout(g, fp32, debug);
+  if (!workspace || ((uintptr_t)workspace % ALIGN) != 0 || workspace_bytes < L.total) return MPMC_ERR_WORKSPACE;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return MPMC_ERR_CUDA; }
+
+  mpmc_ctx* c = new (std::nothrow) mpmc_ctx();
+  if (!c) return MPMC_ERR_ARG;
+  std::memset(&c->p, 0, sizeof(Params));
+  c->N = N; c->flags = flags; c->fp32 = fp32; c->debug = debug; c->loaded = false; c->sticky = MPMC_OK;
+  c->stream = (cudaStream_t)cuda_stream; c->graph1 = nullptr; c->graphK = nullptr;
+  Params& p = c->p;
+  p.mx = g.m[0]; p.my = g.m[1]; p.hx = g.m[0] / 2; p.hy = g.m[1] / 2;
+  p.Mq = L.Mq; p.Mqp = L.Mqp; p.n_s = n_s; p.N = (uint32_t)N;
+  p.seed_lo = (uint32_t)seed; p.seed_hi = (uint32_t)(seed >> 32);
+  p.wx_f = (float)g.w0[0]; p.wy_f = (float)g.w0[1];
+  p.sigma2_f = (float)sigma * (float)sigma; p.d_f = (float)d;
+  p.wx_p = g.w0[0]; p.wy_p = g.w0[1]; p.sigma2_p = sigma * sigma; p.d_p = d;
+  p.wx_d = g.wp[0]; p.wy_d = g.wp[1];
+  p.Lx_eff = (double)g.m[0] * g.wp[0]; p.Ly_eff = (double)g.m[1] * g.wp[1];
+  p.sigma_d = sigma;
+  p.Lx_user = g.w0[0] * g.m[0]; p.Ly_user = g.w0[1] * g.m[1];
+  char* base = (char*)workspace;
+  p.ctl = (Ctl*)(base + L.off_ctl);
+  p.hist = (unsigned long long*)(base + L.off_hist);
+  p.cnt32 = (uint32_t*)(base + L.off_cnt32);
+  for (int b = 0; b < 2; ++b) {
+    p.cnt[b] = (uint8_t*)(base + L.off_cnt[b]);
+    p.pos[b] = (void*)(base + L.off_pos[b]);
+    p.ids[b] = (uint32_t*)(base + L.off_ids[b]);
+  }
+  p.mask = debug ? (uint32_t*)(base + L.off_mask) : nullptr;
+  // NF = 2 register slots per neighbour while at most 2 disks fit a cell most of the time (w < ~1.15 sigma);
+  // NF = 4 in the paper's regime (w up to sqrt(2) sigma, L152).
+  const double wmax = g.wp[0] > g.wp[1] ? g.wp[0] : g.wp[1];
+  c->nf = (wmax < 1.15 * sigma) ? 2 : 4;
+  *out = c;
+  return MPMC_OK;
+}
+
+int mpmc_create(mpmc_ctx** out, uint64_t N, const double box[2], double sigma, double d, uint32_t n_s,
+                uint64_t seed, uint32_t flags, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  return mpmc_create_ex(out, N, box, sigma, d, n_s, seed, flags, 0.0, workspace, workspace_bytes, cuda_stream);
+}
+
+int mpmc_destroy(mpmc_ctx* c) {
+  if (!c) return MPMC_OK;
+  if (c->graph1) cudaGraphExecDestroy(c->graph1);
+  if (c->graphK) cudaGraphExecDestroy(c->graphK);
+  delete c;
+  return MPMC_OK;
+}
+
+int mpmc_geometry(const mpmc_ctx* c, uint32_t m[2], double w[2], double L_eff[2]) {
+  if (!c) return MPMC_ERR_ARG;
+  if (m) { m[0] = c->p.mx; m[1] = c->p.my; }
+  if (w) { w[0] = c->p.wx_d; w[1] = c->p.wy_d; }
+  if (L_eff) { L_eff[0] = c->p.Lx_eff; L_eff[1] = c->p.Ly_eff; }
+  return MPMC_OK;
+}
+
+int mpmc_load_positions(mpmc_ctx* c, const double* xy) {
+  if (!c || !xy) return MPMC_ERR_ARG;
+  c->loaded = false;
+  c->sticky = MPMC_OK;
+  k_reset<<<148 * 4, 256, 0, c->stream>>>(c->p);
+  const dim3 gN((c->p.N + AUX_THREADS - 1) / AUX_THREADS), gC = cell_grid(c, AUX_THREADS);
+  if (c->fp32) {
+    k_load_bin<float><<<gN, AUX_THREADS, 0, c->stream>>>(c->p, xy);
+    k_load_sort<float><<<gC, AUX_THREADS, 0, c->stream>>>(c->p);
+    k_load_check<float><<<gC, AUX_THREADS, 0, c->stream>>>(c->p);
+  } else {
+    k_load_bin<double><<<gN, AUX_THREADS, 0, c->stream>>>(c->p, xy);
+    k_load_sort<double><<<gC, AUX_THREADS, 0, c->stream>>>(c->p);
+    k_load_check<double><<<gC, AUX_THREADS, 0, c->stream>>>(c->p);
+  }
+  CU(cudaGetLastError());
+  if (c->debug) CU(cudaMemsetAsync(c->p.mask, 0, (size_t)c->p.mx * c->p.my * 4, c->stream));
+  Ctl h;
+  const int st = read_ctl(c, &h);
+  if (st != MPMC_OK) return st;
+  c->loaded = true;
+  return MPMC_OK;
+}
+
+int mpmc_sweep(mpmc_ctx* c, uint64_t k) {
+  if (!c) return MPMC_ERR_ARG;
+  if (!c->loaded) return MPMC_ERR_STATE;
+  if (!c->graph1) {
+    int st = build_graph(c, 1, &c->graph1);
+    if (st != MPMC_OK) return st;
+    st = build_graph(c, GRAPH_BATCH, &c->graphK);
+    if (st != MPMC_OK) return st;
+  }
+  while (k >= GRAPH_BATCH) { CU(cudaGraphLaunch(c->graphK, c->stream)); k -= GRAPH_BATCH; }
+  while (k > 0) { CU(cudaGraphLaunch(c->graph1, c->stream)); --k; }
+  return c->sticky;
+}
+
+int mpmc_get_positions(mpmc_ctx* c, double* xy_out) {
+  if (!c || !xy_out) return MPMC_ERR_ARG;
+  if (!c->loaded) return MPMC_ERR_STATE;
+  const dim3 gC = cell_grid(c, AUX_THREADS);
+  if (c->fp32) k_unpack<float><<<gC, AUX_THREADS, 0, c->stream>>>(c->p, xy_out);
+  else         k_unpack<double><<<gC, AUX_THREADS, 0, c->stream>>>(c->p, xy_out);
+  CU(cudaGetLastError());
+  return c->sticky;
+}
+
+int mpmc_acceptance(mpmc_ctx* c, uint64_t out[4]) {
+  if (!c || !out) return MPMC_ERR_ARG;
+  if (!c->loaded) return MPMC_ERR_STATE;
+  Ctl h;
+  const int st = read_ctl(c, &h);
+  out[1] = h.counters[0]; out[2] = h.counters[1]; out[3] = h.counters[2];
+  out[0] = out[1] + out[2] + out[3];
+  return st;
+}
+
+int mpmc_pressure_contact(mpmc_ctx* c, double dr, uint32_t nbins, uint32_t degree, uint64_t* hist_out,
+                          double* g_contact, double* p_star) {
+  if (!c || !(dr > 0) || nbins == 0 || nbins > MAX_BINS) return MPMC_ERR_ARG;
+  if ((g_contact || p_star) && degree + 1 > nbins) return MPMC_ERR_ARG;
+  if (!c->loaded) return MPMC_ERR_STATE;
+  const Params& p = c->p;
+  const double rmax = p.sigma_d + (double)nbins * dr;
+  const double wmin = p.wx_d < p.wy_d ? p.wx_d : p.wy_d;
+  const int Rc = (int)std::ceil(rmax / wmin);
+  CU(cudaMemsetAsync(p.hist, 0, (size_t)nbins * 8, c->stream));
+  const dim3 gC = cell_grid(c, AUX_THREADS);
+  const size_t sh = (size_t)nbins * 4;
+  if (c->fp32) k_contact_hist<float><<<gC, AUX_THREADS, sh, c->stream>>>(p, dr, nbins, Rc);
+  else         k_contact_hist<double><<<gC, AUX_THREADS, sh, c->stream>>>(p, dr, nbins, Rc);
+  CU(cudaGetLastError());
+  std::vector<uint64_t> H(nbins);
+  CU(cudaMemcpyAsync(H.data(), p.hist, (size_t)nbins * 8, cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  if (hist_out) std::memcpy(hist_out, H.data(), (size_t)nbins * 8);
+  if (g_contact || p_star) {
+    // eq. 5-6 (L374-379): g(R_i) = 2 H_i / (N rho 2 pi R_i dr), R_i = (2/3)(r_{i+1}^3 - r_i^3)/(r_{i+1}^2 - r_i^2)
+    const double Nd = (double)c->N, rho = Nd / (p.Lx_eff * p.Ly_eff), sg = p.sigma_d;
+    const double PI = 3.14159265358979323846;
+    std::vector<double> t(nbins), g(nbins);
+    for (uint32_t i = 0; i < nbins; ++i) {
+      const double r0 = sg + dr * (double)i, r1 = sg + dr * (double)(i + 1);
+      const double Ri = (2.0 / 3.0) * (r1 * r1 * r1 - r0 * r0 * r0) / (r1 * r1 - r0 * r0);
+      t[i] = (Ri - sg) / (dr * (double)nbins);     // scaled abscissa; the value at 0 is unchanged
+      g[i] = 2.0 * (double)H[i] / (Nd * rho * 2.0 * PI * Ri * dr);
+    }
+    double g0 = 0;
+    if (!polyfit_at_zero(t, g, degree, &g0)) return MPMC_ERR_ARG;
+    if (g_contact) *g_contact = g0;
+    if (p_star) *p_star = sg * sg * rho * (1.0 + 0.5 * PI * sg * sg * rho * g0);   // eq. 4 (L368)
+  }
+  return c->sticky;
+}
+
+int mpmc_debug_sub_sweep(mpmc_ctx* c, uint32_t set) {
+  if (!c || set > 3) return MPMC_ERR_ARG;
+  if (!c->loaded) return MPMC_ERR_STATE;
+  launch_sub(c, 4u + set);
+  CU(cudaGetLastError());
+  return c->sticky;
+}
+
+int mpmc_debug_shift(mpmc_ctx* c, uint32_t direction, double delta) {
+  if (!c || direction > 3 || !(delta >= 0)) return MPMC_ERR_ARG;
+  if (!c->loaded) return MPMC_ERR_STATE;
+  launch_shift(c, 1, direction, delta);
+  CU(cudaGetLastError());
+  return c->sticky;
+}
+
+int mpmc_debug_state(mpmc_ctx* c, void* counts, void* slab, void* ids, void* accept_mask, double origin[2],
+                     uint64_t* sweep, uint64_t* digest) {
+  if (!c) return MPMC_ERR_ARG;
+  if (!c->loaded) return MPMC_ERR_STATE;
+  if (accept_mask && !c->debug) return MPMC_ERR_ARG;
+  const dim3 gC = cell_grid(c, AUX_THREADS);
+  if (counts || slab || ids) {
+    if (c->fp32) k_export<float><<<gC, AUX_THREADS, 0, c->stream>>>(c->p, (uint32_t*)counts, (float*)slab, (uint32_t*)ids);
+    else         k_export<double><<<gC, AUX_THREADS, 0, c->stream>>>(c->p, (uint32_t*)counts, (double*)slab, (uint32_t*)ids);
+    CU(cudaGetLastError());
+  }
+  if (accept_mask)
+    CU(cudaMemcpyAsync(accept_mask, c->p.mask, (size_t)c->p.mx * c->p.my * 4, cudaMemcpyDeviceToDevice, c->stream));
+  Ctl h;
+  const int st = read_ctl(c, &h);
+  if (origin) { origin[0] = h.origin[0]; origin[1] = h.origin[1]; }
+  if (sweep) *sweep = h.t;
+  if (digest) *digest = h.digest;
+  return st;
+}
+
+int mpmc_debug_philox(const uint32_t* ctr, const uint32_t key[2], uint32_t* out, uint32_t n, void* cuda_stream) {
+  if (!ctr || !key || !out) return MPMC_ERR_ARG;
+  if (n == 0) return MPMC_OK;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  k_philox_test<<<(n + 127) / 128, 128, 0, s>>>(ctr, key[0], key[1], out, n);
+  CU(cudaGetLastError());
+  CU(cudaStreamSynchronize(s));
+  return MPMC_OK;
+}
+
+const char* mpmc_strerror(int code) {
+  switch (code) {
+    case MPMC_OK: return "ok";
+    case MPMC_ERR_ARG: return "bad argument";
+    case MPMC_ERR_BOX: return "box too small for two cells of width >= sigma per axis (or too many cells)";
+    case MPMC_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+    case MPMC_ERR_OVERLAP: return "loaded positions overlap or lie outside the box";
+    case MPMC_ERR_CELL_OVERFLOW: return "more than n_max = 4 disks in one cell";
+    case MPMC_ERR_CUDA: return "CUDA error (no device, or a launch failed)";
+    case MPMC_ERR_STATE: return "no positions loaded";
+    default: return "unknown error";
+  }
+}
+const char* mpmc_version(void) { return "mpmc-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,103 @@
+"""CPU-only checks of the boundary: the C-ABI library builds for sm_100a, loads, exports every symbol that
+include/mpmc.h declares, does its pure-host arithmetic, and fails loudly (no CPU fallback) without a GPU."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1211_1646_b200 import build, binding
+    build.build()
+    return binding.lib()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "mpmc.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(mpmc_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_symbols_all_exported(lib):
+    from paper_1211_1646_b200 import binding
+    names = declared_symbols()
+    assert len(names) >= 17
+    for n in names:
+        assert hasattr(lib, n), n
+        assert n in binding.SYMBOLS, f"{n} missing from the Python binding"
+    assert sorted(binding.SYMBOLS) == names
+
+
+def test_version_and_strerror(lib):
+    assert b"sm_100a" in lib.mpmc_version()
+    for code in range(0, -8, -1):
+        assert lib.mpmc_strerror(code)
+    assert lib.mpmc_strerror(-99) == b"unknown error"
+
+
+def test_workspace_bytes_host_arithmetic(lib):
+    from paper_1211_1646_b200 import binding, inputs
+    w = inputs.CONFIGS["C3"]
+    box = inputs.box_for(w.n_side, w.phi)
+    nb = binding.workspace_bytes(w.N, box, 1.0, fp32=True)
+    Mq = (1152 // 2) * (998 // 2)
+    # two buffers of 4 colours x 4 slot planes of float2 + ids + counts
+    assert nb >= 2 * 16 * Mq * (8 + 4) + 2 * 4 * Mq
+    assert nb < 1.1 * (2 * 16 * Mq * 12 + 2 * 4 * Mq + 4 * 4 * Mq) + (1 << 20)
+    assert binding.workspace_bytes(w.N, box, 1.0, fp32=False) > nb
+    assert binding.workspace_bytes(w.N, box, 1.0, fp32=True, debug=True) >= nb + 4 * 1152 * 998
+    assert binding.workspace_bytes(w.N, (1.5, 10.0), 1.0, fp32=True) == 0      # box too small
+    assert binding.workspace_bytes(0, box, 1.0, fp32=True) == 0
+    b = (C.c_double * 2)(*box)
+    assert lib.mpmc_workspace_bytes(w.N, b, 1.0, binding.FP32 | binding.FP64) == 0   # both precision bits
+    # a wider target cell means fewer cells and a smaller workspace
+    assert binding.workspace_bytes(w.N, box, 1.0, fp32=True, w_target=1.4) < nb
+
+
+def test_argument_errors_without_gpu(lib):
+    from paper_1211_1646_b200 import binding
+    h = C.c_void_p()
+    b = (C.c_double * 2)(10.0, 10.0)
+    fake = C.c_void_p(0x10000)   # never dereferenced: argument checks come first
+    assert lib.mpmc_create(C.byref(h), 0, b, 1.0, 0.1, 4, 1, binding.FP32, fake, 1 << 30, None) == -1
+    assert lib.mpmc_create(C.byref(h), 10, b, 1.0, 0.1, 33, 1, binding.FP32, fake, 1 << 30, None) == -1
+    assert lib.mpmc_create(C.byref(h), 10, b, 1.0, 0.1, 4, 1, 0, fake, 1 << 30, None) == -1
+    small = (C.c_double * 2)(1.9, 10.0)
+    assert lib.mpmc_create(C.byref(h), 10, small, 1.0, 0.1, 4, 1, binding.FP32, fake, 1 << 30, None) == -2
+    assert lib.mpmc_create(C.byref(h), 10, b, 1.0, 0.1, 4, 1, binding.FP32, None, 1 << 30, None) == -3
+    assert lib.mpmc_create(C.byref(h), 10, b, 1.0, 0.1, 4, 1, binding.FP32, fake, 16, None) == -3
+    assert lib.mpmc_create(C.byref(h), 10, b, 1.0, 0.1, 4, 1, binding.FP32, C.c_void_p(0x10001), 1 << 30, None) == -3
+    assert lib.mpmc_sweep(None, 1) == -1
+    assert lib.mpmc_destroy(None) == 0
+
+
+def test_no_cpu_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    from paper_1211_1646_b200 import binding
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        binding.Mpmc(16, (10.0, 10.0), 1.0, 0.1, 4, 1)
+    # and the C library itself reports MPMC_ERR_CUDA rather than computing anything
+    h = C.c_void_p()
+    b = (C.c_double * 2)(10.0, 10.0)
+    assert binding.lib().mpmc_create(C.byref(h), 10, b, 1.0, 0.1, 4, 1, binding.FP32, C.c_void_p(0x10000), 1 << 30,
+                                     None) == -6
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_1211_1646_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle", src, flags=re.M), f
+                assert "oracle_mpmc" not in src and "liboracle" not in src, f
+    orc = open(os.path.join(ROOT, "oracle", "oracle.py")).read() + open(os.path.join(ROOT, "oracle", "oracle_mpmc.cpp")).read()
+    assert "paper_1211_1646_b200" not in orc.replace("paper_1211_1646_b200/csrc (the CUDA", "").replace(
+        "imports nothing from paper_1211_1646_b200", "")
+    assert "mpmc.h" not in orc

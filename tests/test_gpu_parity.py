@@ -1,0 +1,261 @@
+"""GPU parity tests (`-m gpu`): the CUDA path, called through the C ABI, against the CPU oracle on the same
+seeded inputs.  Bar (BASELINE.json north_star): accept/reject sequences, counters, cell membership, slot order
+and ids bit-exact; local coordinates bit-exact in both precisions (stronger than the stated |dx| <= 1e-12 /
+1e-5 on unpacked positions, which is checked as well); every configuration overlap-free."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1211_1646_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_1211_1646_b200 import build
+    build.build()
+    return torch
+
+
+def make_pair(oracle_mod, torch, N, box, sigma, d, n_s, seed, fp32, xy, debug=True, w_target=0.0):
+    from paper_1211_1646_b200.binding import Mpmc
+    o = oracle_mod.Oracle(N, box, sigma, d, n_s, seed, fp32=fp32, w_target=w_target)
+    g = Mpmc(N, box, sigma, d, n_s, seed, fp32=fp32, debug=debug, w_target=w_target)
+    assert (g.mx, g.my) == (o.mx, o.my) and (g.wx, g.wy) == (o.wx, o.wy) and g.L_eff == o.L_eff
+    o.load_positions(xy)
+    g.load_positions(torch.as_tensor(xy, device="cuda"))
+    return o, g
+
+
+def assert_same_state(o, g, fp32, check_mask=True, pos_tol=None):
+    so, sg = o.debug_state(), g.debug_state()
+    assert sg["sweep"] == so["sweep"]
+    assert np.array_equal(sg["counts"], so["counts"])
+    assert np.array_equal(sg["ids"], so["ids"])
+    assert np.array_equal(sg["slab"].view(np.uint32 if fp32 else np.uint64),
+                          so["slab"].view(np.uint32 if fp32 else np.uint64))      # bit-exact locals
+    assert sg["origin"] == so["origin"]
+    if check_mask and sg["accept_mask"] is not None:
+        assert np.array_equal(sg["accept_mask"], so["accept_mask"])
+        assert sg["digest"] == so["digest"]
+    assert g.acceptance() == o.acceptance()
+    po, pg = o.get_positions(), g.get_positions().cpu().numpy()
+    tol = pos_tol if pos_tol is not None else (1e-5 if fp32 else 1e-12)
+    assert np.abs(pg - po).max() <= tol
+    assert np.array_equal(pg, po)      # same formula, same operands: in fact identical
+    return so
+
+
+def test_device_philox_matches_known_answers_and_oracle(oracle_mod, torch_cuda):
+    from paper_1211_1646_b200.binding import device_philox
+    kat = [[0, 0, 0, 0], [0xFFFFFFFF] * 4, [0x243f6a88, 0x85a308d3, 0x13198a2e, 0x03707344]]
+    keys = [(0, 0), (0xFFFFFFFF, 0xFFFFFFFF), (0xa4093822, 0x299f31d0)]
+    want = [[0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8], [0x408f276d, 0x41c83b0e, 0xa20bc7c6, 0x6d5451fd],
+            [0xd16cfe09, 0x94fdcceb, 0x5001e420, 0x24126ea1]]
+    for c, k, w in zip(kat, keys, want):
+        assert device_philox([c], k)[0].tolist() == w
+    rng = np.random.default_rng(5)
+    ctr = rng.integers(0, 2 ** 32, size=(1000, 4), dtype=np.uint64)
+    got = device_philox(ctr, (123, 456))
+    for i in range(0, 1000, 37):
+        assert got[i].tolist() == oracle_mod.philox4x32_10(ctr[i].tolist(), (123, 456))
+
+
+@pytest.mark.parametrize("fp32", [False, True])
+def test_pieces_load_subsweeps_shift(oracle_mod, torch_cuda, fp32):
+    w = I.CONFIGS["C1"]
+    xy, box = I.workload_inputs(w)
+    o, g = make_pair(oracle_mod, torch_cuda, w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32, xy)
+    assert_same_state(o, g, fp32)                      # cell-list build
+    for q in (2, 0, 3, 1):                             # one sub-sweep per checkerboard set
+        o.sub_sweep(q); g.sub_sweep(q)
+        assert_same_state(o, g, fp32)
+    for direction in range(4):                         # the four shift directions
+        delta = 0.31 * (o.wx if direction < 2 else o.wy)
+        o.shift(direction, delta); g.shift(direction, delta)
+        assert_same_state(o, g, fp32)
+    o.shift(0, 0.0); g.shift(0, 0.0)                   # delta = 0 is allowed (reading A5)
+    assert_same_state(o, g, fp32)
+
+
+@pytest.mark.parametrize("fp32", [False, True])
+def test_c1_100_sweeps_bit_exact(oracle_mod, torch_cuda, fp32):
+    w = I.CONFIGS["C1"]
+    xy, box = I.workload_inputs(w)
+    o, g = make_pair(oracle_mod, torch_cuda, w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32, xy)
+    for k in (1, 1, 3, 16, 17, 62):                    # single launches, graph batches and remainders
+        o.sweep(k); g.sweep(k)
+        st = assert_same_state(o, g, fp32)
+    assert st["sweep"] == 100
+    att, acc, rb, ro = g.acceptance()
+    assert att == acc + rb + ro and acc > 0 and rb > 0 and ro > 0
+
+
+@pytest.mark.parametrize("fp32", [False, True])
+def test_c2_dense_fluid(oracle_mod, torch_cuda, fp32):
+    w = I.CONFIGS["C2"]
+    xy, box = I.workload_inputs(w)
+    o, g = make_pair(oracle_mod, torch_cuda, w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32, xy)
+    assert (g.mx, g.my) == (290, 252)
+    o.sweep(40); g.sweep(40)
+    assert_same_state(o, g, fp32)
+    # contact pressure every 10 sweeps: histogram bit-exact, fit to rounding (config C2: bin width 0.005 sigma)
+    for _ in range(2):
+        o.sweep(10); g.sweep(10)
+        ho, g0o, pso = o.pressure_contact(0.005, 20, 2)
+        hg, g0g, psg = g.pressure_contact(0.005, 20, 2)
+        assert np.array_equal(ho, hg) and ho.sum() > 1000
+        assert g0g == pytest.approx(g0o, rel=1e-9) and psg == pytest.approx(pso, rel=1e-9)
+    hg = g.contact_histogram(1e-4, 200)                # the paper's estimator parameters (L382)
+    assert np.array_equal(hg, o.contact_histogram(1e-4, 200))
+
+
+def test_c3_headline_config_bench_launch_configuration(oracle_mod, torch_cuda):
+    """Full size N = 2^20, fp32, NO debug flag: exactly the kernels bench.py times."""
+    w = I.CONFIGS["C3"]
+    xy, box = I.workload_inputs(w)
+    o, g = make_pair(oracle_mod, torch_cuda, w.N, box, w.sigma, w.d, w.n_s, w.seed, True, xy, debug=False)
+    assert (g.mx, g.my) == (1152, 998)
+    o.sweep(12); g.sweep(12)
+    st = assert_same_state(o, g, True, check_mask=False)
+    assert st["counts"].sum() == w.N
+    att = g.acceptance()[0]
+    assert 11.5 * 4.0e6 < att < 12 * 4.2e6
+
+
+def test_c3_debug_digest(oracle_mod, torch_cuda):
+    w = I.CONFIGS["C3"]
+    xy, box = I.workload_inputs(w)
+    o, g = make_pair(oracle_mod, torch_cuda, w.N, box, w.sigma, w.d, w.n_s, w.seed, True, xy, debug=True)
+    o.sweep(3); g.sweep(3)
+    assert_same_state(o, g, True)
+
+
+def test_c4_shape_reduced_and_ns8(oracle_mod, torch_cuda):
+    # C4's parameters (phi 0.720, d 0.06, n_s 8) on a 512^2 lattice the oracle finishes in seconds
+    xy, box = I.jittered_lattice(512, 0.720, seed=1)
+    o, g = make_pair(oracle_mod, torch_cuda, 512 * 512, box, 1.0, 0.06, 8, 1, True, xy)
+    o.sweep(8); g.sweep(8)
+    assert_same_state(o, g, True)
+
+
+def test_c5_dilute_fluid_with_three_per_cell(oracle_mod, torch_cuda):
+    # C5's parameters (phi 0.30, d 0.5, w = sigma) on 256^2 disks; melted by the ORACLE (reading A15), then
+    # both sides run from the melted configuration.  Cells with 3 disks exercise the NF = 2 overflow path.
+    n = 256
+    xy0, box = I.jittered_lattice(n, 0.30, seed=1)
+    pre = oracle_mod.Oracle(n * n, box, 1.0, 0.5, 4, 999, fp32=True)
+    pre.load_positions(xy0)
+    while pre.acceptance()[0] < 100 * n * n:
+        pre.sweep(10)
+    xy = pre.get_positions()
+    o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.5, 4, 1, True, xy)
+    seen3 = False
+    for _ in range(6):
+        o.sweep(10); g.sweep(10)
+        st = assert_same_state(o, g, True)
+        seen3 |= st["counts"].max() >= 3
+    assert seen3
+    att, acc, rb, ro = g.acceptance()
+    assert rb / att > 0.3           # boundary-crossing rejections dominate at d = 0.5 (config C5)
+
+
+@pytest.mark.parametrize("fp32", [False, True])
+def test_paper_cell_regime_w_1p4(oracle_mod, torch_cuda, fp32):
+    # cell width just under sqrt(2) sigma, n_max = 4 fully used (L152); NF = 4 kernel
+    xy, box = I.jittered_lattice(128, 0.698, seed=2)
+    o, g = make_pair(oracle_mod, torch_cuda, 128 * 128, box, 1.0, 0.16, 4, 3, fp32, xy, w_target=1.40)
+    assert g.wx >= 1.40 and g.wx < math.sqrt(2)
+    o.sweep(25); g.sweep(25)
+    st = assert_same_state(o, g, fp32)
+    assert st["counts"].max() >= 3
+
+
+@pytest.mark.parametrize("N,box,xy", [
+    (1, (2.6, 2.6), [[0.3, 0.4]]),
+    (2, (2.6, 2.9), [[0.5, 0.5], [1.8, 1.9]]),                 # mx = my = 2: neighbour at two image offsets
+    (3, (4.3, 4.5), [[0.5, 0.5], [2.0, 2.0], [3.5, 0.9]]),
+])
+@pytest.mark.parametrize("fp32", [False, True])
+def test_tiny_systems(oracle_mod, torch_cuda, N, box, xy, fp32):
+    xy = np.array(xy, dtype=np.float64)
+    o, g = make_pair(oracle_mod, torch_cuda, N, box, 1.0, 0.4, 4, 9, fp32, xy)
+    for _ in range(5):
+        o.sweep(40); g.sweep(40)
+        assert_same_state(o, g, fp32)
+
+
+@pytest.mark.parametrize("n_s", [0, 1, 7, 32])
+def test_moves_per_cell_range(oracle_mod, torch_cuda, n_s):
+    xy, box = I.jittered_lattice(32, 0.6, seed=4)
+    o, g = make_pair(oracle_mod, torch_cuda, 1024, box, 1.0, 0.2, n_s, 5, False, xy)
+    o.sweep(20); g.sweep(20)
+    assert_same_state(o, g, False)
+    assert g.acceptance()[0] == o.acceptance()[0]
+    if n_s == 0:
+        assert g.acceptance() == (0, 0, 0, 0)
+
+
+def test_seed_and_high_sweep_words(oracle_mod, torch_cuda):
+    xy, box = I.jittered_lattice(32, 0.6, seed=4)
+    seed = 0xDEADBEEF12345678
+    o, g = make_pair(oracle_mod, torch_cuda, 1024, box, 1.0, 0.2, 4, seed, True, xy)
+    o.sweep(5); g.sweep(5)
+    assert_same_state(o, g, True)
+
+
+def test_errors_on_device(oracle_mod, torch_cuda):
+    torch = torch_cuda
+    from paper_1211_1646_b200.binding import Mpmc, MpmcError
+    g = Mpmc(2, (4.4, 4.4), 1.0, 0.1, 4, 1)
+    with pytest.raises(MpmcError) as e:
+        g.sweep(1)
+    assert e.value.code == -7
+    with pytest.raises(MpmcError) as e:
+        g.load_positions(torch.tensor([[1.0, 1.0], [1.5, 1.0]], dtype=torch.float64, device="cuda"))
+    assert e.value.code == -4
+    with pytest.raises(MpmcError):
+        g.load_positions(torch.tensor([[1.0, 1.0], [float("nan"), 1.0]], dtype=torch.float64, device="cuda"))
+    with pytest.raises(MpmcError):
+        g.load_positions(torch.tensor([[0.1, 1.0], [4.3, 1.0]], dtype=torch.float64, device="cuda"))   # across the edge
+    g.load_positions(torch.tensor([[1.0, 1.0], [2.0, 1.0]], dtype=torch.float64, device="cuda"))       # r = sigma: fine
+    g.sweep(3)
+    assert g.acceptance()[0] > 0
+    with pytest.raises(MpmcError) as e:
+        Mpmc(2, (1.9, 4.4), 1.0, 0.1, 4, 1)
+    assert e.value.code == -2
+    # five disks forced into one wide cell -> overflow reported at load
+    g5 = Mpmc(5, (6.4, 6.4), 1.0, 0.1, 4, 1, w_target=3.0)
+    pts = torch.tensor([[0.2, 0.2], [1.4, 0.2], [2.6, 0.2], [0.2, 1.4], [1.4, 1.4]], dtype=torch.float64, device="cuda")
+    with pytest.raises(MpmcError) as e:
+        g5.load_positions(pts)
+    assert e.value.code == -5
+
+
+def test_overlap_free_and_conserved_at_full_size(torch_cuda):
+    """Properties that hold at any size, at the headline size and in the bench launch configuration."""
+    torch = torch_cuda
+    from scipy.spatial import cKDTree
+    from paper_1211_1646_b200.binding import Mpmc
+    w = I.CONFIGS["C3"]
+    xy, box = I.workload_inputs(w)
+    g = Mpmc(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=True)
+    g.load_positions(torch.as_tensor(xy, device="cuda"))
+    g.sweep(200)
+    p = g.get_positions().cpu().numpy()
+    assert np.isfinite(p).all() and p.shape == (w.N, 2)
+    Le = np.array(g.L_eff)
+    assert (p >= 0).all() and (p < Le).all()
+    tree = cKDTree(np.minimum(p, np.nextafter(Le, 0)), boxsize=Le)
+    dmin = tree.query(p, k=2)[0][:, 1].min()
+    assert dmin >= 1.0 - 1e-4          # fp32 locals: two cells' frames differ by an ulp of w (~1e-7) at most
+    st = g.debug_state()
+    assert st["counts"].sum() == w.N and st["counts"].max() <= 4 and st["sweep"] == 200
+    used = np.arange(4)[None, :] < st["counts"][:, None]
+    assert np.array_equal(np.sort(st["ids"][used]), np.arange(w.N, dtype=np.uint32))
+    att, acc, rb, ro = g.acceptance()
+    assert att == acc + rb + ro and 0.2 < acc / att < 0.9
