@@ -213,6 +213,9 @@ def main():
             moves += att
         return total_ms, moves
 
+    # everything below is enqueued on the library's own stream, so torch.cuda.Event times that stream
+    torch.cuda.synchronize(dev)
+    torch.cuda.set_stream(sim.stream)
     for _ in range(args.warmup):
         step_resident()
     if dist:

@@ -96,7 +96,9 @@ class Mpmc:
             nbytes = 256
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
-            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            # The library's stream: a dedicated side stream by default (the legacy default stream cannot be
+            # captured into a CUDA graph).  _enter/_exit order it against torch's current stream.
+            self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
             self._h = _vp()
             b = (_dbl * 2)(float(box[0]), float(box[1]))
             _chk(lib().mpmc_create_ex(C.byref(self._h), self.N, b, float(sigma), float(d), int(n_s), int(seed),
@@ -123,30 +125,48 @@ class Mpmc:
         except Exception:
             pass
 
+    def _enter(self):
+        cur = self.torch.cuda.current_stream(self.device)
+        if cur != self.stream:
+            self.stream.wait_stream(cur)
+
+    def _exit(self):
+        cur = self.torch.cuda.current_stream(self.device)
+        if cur != self.stream:
+            cur.wait_stream(self.stream)
+
     # --- the calls of include/mpmc.h -------------------------------------------------------------------
     def load_positions(self, xy) -> None:
         """xy: (N, 2) float64 CUDA tensor (device pointer passed through)."""
         t = self.torch
         assert xy.is_cuda and xy.dtype == t.float64 and tuple(xy.shape) == (self.N, 2) and xy.is_contiguous()
         with t.cuda.device(self.device):
+            self._enter()
             _chk(lib().mpmc_load_positions(self._h, xy.data_ptr()))
+            self._exit()
 
     def sweep(self, k: int = 1) -> None:
         with self.torch.cuda.device(self.device):
+            self._enter()
             _chk(lib().mpmc_sweep(self._h, int(k)))
+            self._exit()
 
     def get_positions(self, out=None):
         t = self.torch
         if out is None:
             out = t.empty((self.N, 2), dtype=t.float64, device=self.device)
         with t.cuda.device(self.device):
+            self._enter()
             _chk(lib().mpmc_get_positions(self._h, out.data_ptr()))
+            self._exit()
         return out
 
     def acceptance(self):
         o = (_u64 * 4)()
         with self.torch.cuda.device(self.device):
+            self._enter()
             _chk(lib().mpmc_acceptance(self._h, o))
+            self._exit()
         return tuple(int(v) for v in o)
 
     def pressure_contact(self, dr: float, nbins: int, degree: int):
@@ -154,25 +174,33 @@ class Mpmc:
         h = np.zeros(nbins, dtype=np.uint64)
         g0, ps = _dbl(), _dbl()
         with self.torch.cuda.device(self.device):
+            self._enter()
             _chk(lib().mpmc_pressure_contact(self._h, float(dr), int(nbins), int(degree), h.ctypes.data,
                                              C.byref(g0), C.byref(ps)))
+            self._exit()
         return h, g0.value, ps.value
 
     def contact_histogram(self, dr: float, nbins: int):
         import numpy as np
         h = np.zeros(nbins, dtype=np.uint64)
         with self.torch.cuda.device(self.device):
+            self._enter()
             _chk(lib().mpmc_pressure_contact(self._h, float(dr), int(nbins), 0, h.ctypes.data, None, None))
+            self._exit()
         return h
 
     # --- test hooks ------------------------------------------------------------------------------------
     def sub_sweep(self, checkerboard_set: int) -> None:
         with self.torch.cuda.device(self.device):
+            self._enter()
             _chk(lib().mpmc_debug_sub_sweep(self._h, int(checkerboard_set)))
+            self._exit()
 
     def shift(self, direction: int, delta: float) -> None:
         with self.torch.cuda.device(self.device):
+            self._enter()
             _chk(lib().mpmc_debug_shift(self._h, int(direction), float(delta)))
+            self._exit()
 
     def debug_state(self) -> dict:
         t = self.torch
@@ -183,9 +211,11 @@ class Mpmc:
         origin = (_dbl * 2)()
         sw, dg = _u64(), _u64()
         with t.cuda.device(self.device):
+            self._enter()
             _chk(lib().mpmc_debug_state(self._h, counts.data_ptr(), slab.data_ptr(), ids.data_ptr(),
                                         mask.data_ptr() if mask is not None else None, origin,
                                         C.byref(sw), C.byref(dg)))
+            self._exit()
         import numpy as np
         return dict(counts=counts.cpu().numpy().view(np.uint32), slab=slab.cpu().numpy(),
                     ids=ids.cpu().numpy().view(np.uint32),

@@ -284,6 +284,12 @@ int mpmc_load_positions(mpmc_ctx* c, const double* xy) {
 int mpmc_sweep(mpmc_ctx* c, uint64_t k) {
   if (!c) return MPMC_ERR_ARG;
   if (!c->loaded) return MPMC_ERR_STATE;
+  if (c->stream == nullptr) {
+    // the legacy default stream cannot be captured: plain launches (same kernels, same order)
+    for (; k > 0; --k) enqueue_sweep(c);
+    CU(cudaGetLastError());
+    return c->sticky;
+  }
   if (!c->graph1) {
     int st = build_graph(c, 1, &c->graph1);
     if (st != MPMC_OK) return st;

@@ -145,7 +145,7 @@ def test_c4_shape_reduced_and_ns8(oracle_mod, torch_cuda):
 
 def test_c5_dilute_fluid_with_three_per_cell(oracle_mod, torch_cuda):
     # C5's parameters (phi 0.30, d 0.5, w = sigma) on 256^2 disks; melted by the ORACLE (reading A15), then
-    # both sides run from the melted configuration.  Cells with 3 disks exercise the NF = 2 overflow path.
+    # both sides run from the melted configuration.
     n = 256
     xy0, box = I.jittered_lattice(n, 0.30, seed=1)
     pre = oracle_mod.Oracle(n * n, box, 1.0, 0.5, 4, 999, fp32=True)
@@ -154,14 +154,27 @@ def test_c5_dilute_fluid_with_three_per_cell(oracle_mod, torch_cuda):
         pre.sweep(10)
     xy = pre.get_positions()
     o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.5, 4, 1, True, xy)
-    seen3 = False
     for _ in range(6):
         o.sweep(10); g.sweep(10)
         st = assert_same_state(o, g, True)
-        seen3 |= st["counts"].max() >= 3
-    assert seen3
+    assert st["counts"].max() >= 2 and (st["counts"] == 0).mean() > 0.5
     att, acc, rb, ro = g.acceptance()
     assert rb / att > 0.3           # boundary-crossing rejections dominate at d = 0.5 (config C5)
+
+
+@pytest.mark.parametrize("fp32", [False, True])
+def test_three_per_cell_with_two_register_slots(oracle_mod, torch_cuda, fp32):
+    # w ~ 1.13 sigma keeps the NF = 2 kernel (w < 1.15 sigma) while cells with 3 disks do occur: exercises the
+    # path that re-reads slots 2, 3 of crowded neighbours inside the move loop
+    xy, box = I.jittered_lattice(64, 0.50, seed=6)
+    o, g = make_pair(oracle_mod, torch_cuda, 4096, box, 1.0, 0.3, 4, 8, fp32, xy, w_target=1.12)
+    assert 1.12 <= g.wx < 1.15 and 1.12 <= g.wy < 1.15
+    seen3 = False
+    for _ in range(10):
+        o.sweep(20); g.sweep(20)
+        st = assert_same_state(o, g, fp32)
+        seen3 |= st["counts"].max() >= 3
+    assert seen3
 
 
 @pytest.mark.parametrize("fp32", [False, True])
