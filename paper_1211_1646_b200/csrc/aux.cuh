@@ -102,7 +102,7 @@ __global__ void __launch_bounds__(AUX_THREADS) k_load_check(const __grid_constan
   if (ci >= p.Mq) return;
   const uint32_t n = cnt_plane(p, 0, Q)[ci];
   if (n == 0) return;
-  const uint32_t ya = ci / p.hx, xa = ci - ya * p.hx;
+  const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
   const uint32_t x = 2u * xa + (Q & 1u), y = 2u * ya + (Q >> 1);
   const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p);
   bool bad = false;
@@ -134,7 +134,7 @@ __global__ void __launch_bounds__(AUX_THREADS) k_unpack(const __grid_constant__ 
   if (ci >= p.Mq) return;
   const uint32_t cur = p.ctl->cur;
   const uint32_t n = cnt_plane(p, cur, Q)[ci];
-  const uint32_t ya = ci / p.hx, xa = ci - ya * p.hx;
+  const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
   const double bx = __fma_rn((double)(2u * xa + (Q & 1u)), p.wx_d, p.ctl->origin[0]);
   const double by = __fma_rn((double)(2u * ya + (Q >> 1)), p.wy_d, p.ctl->origin[1]);
   for (uint32_t i = 0; i < n; ++i) {
@@ -156,7 +156,7 @@ __global__ void __launch_bounds__(AUX_THREADS) k_export(const __grid_constant__ 
   if (ci >= p.Mq) return;
   const uint32_t cur = p.ctl->cur;
   const uint32_t n = cnt_plane(p, cur, Q)[ci];
-  const uint32_t ya = ci / p.hx, xa = ci - ya * p.hx;
+  const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
   const size_t c = (size_t)(2u * ya + (Q >> 1)) * p.mx + (2u * xa + (Q & 1u));
   if (counts) counts[c] = n;
   for (uint32_t i = 0; i < (uint32_t)NMAX; ++i) {
@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(AUX_THREADS) k_contact_hist(const __grid_const
   if (ci < p.Mq) {
     const uint32_t cur = p.ctl->cur;
     const uint32_t n = cnt_plane(p, cur, Q)[ci];
-    const uint32_t ya = ci / p.hx, xa = ci - ya * p.hx;
+    const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
     const uint32_t x = 2u * xa + (Q & 1u), y = 2u * ya + (Q >> 1);
     for (uint32_t i = 0; i < n; ++i) {
       const P2 a = pos_plane<P>(p, cur, Q, i)[ci];

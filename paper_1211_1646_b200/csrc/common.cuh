@@ -54,6 +54,7 @@ struct Params {
   uint32_t mx, my, hx, hy;   // cells; hx = mx/2, hy = my/2
   uint32_t Mq, Mqp;          // cells per colour; plane stride (Mq rounded up to 64)
   uint32_t n_s, N;
+  uint32_t hx_magic, hx_sh1, hx_sh2;  // ci / hx without a divide (Granlund-Montgomery; host: div_magic)
   uint32_t seed_lo, seed_hi;
   float wx_f, wy_f, sigma2_f, d_f;      // working-precision constants (fp32 mode)
   double wx_p, wy_p, sigma2_p, d_p;     // working-precision constants (fp64 mode)
@@ -86,6 +87,12 @@ template <> struct Real<float> {
   }
   static __device__ __forceinline__ float unit(uint32_t R) { return __fmul_rn((float)(R >> 8), 0x1p-24f); }
   static __device__ __forceinline__ float far_away() { return 1.0e18f; }   // sentinel: never overlaps
+  // Two lanes at once: sm_100a packed fp32x2 instructions (FADD2 / FMUL2 / FFMA2), each lane one IEEE rn op.
+  using Pair = float2;
+  static __device__ __forceinline__ Pair pair(float a, float b) { return make_float2(a, b); }
+  static __device__ __forceinline__ Pair padd(Pair a, Pair b) { return __fadd2_rn(a, b); }
+  static __device__ __forceinline__ Pair pmul(Pair a, Pair b) { return __fmul2_rn(a, b); }
+  static __device__ __forceinline__ Pair pfma(Pair a, Pair b, Pair c) { return __ffma2_rn(a, b, c); }
 };
 template <> struct Real<double> {
   using T2 = double2;
@@ -102,6 +109,11 @@ template <> struct Real<double> {
   }
   static __device__ __forceinline__ double unit(uint32_t R) { return __dmul_rn((double)R, 0x1p-32); }
   static __device__ __forceinline__ double far_away() { return 1.0e150; }
+  struct Pair { double x, y; };             // no packed fp64 instruction: two scalar ops
+  static __device__ __forceinline__ Pair pair(double a, double b) { Pair r; r.x = a; r.y = b; return r; }
+  static __device__ __forceinline__ Pair padd(Pair a, Pair b) { return pair(__dadd_rn(a.x, b.x), __dadd_rn(a.y, b.y)); }
+  static __device__ __forceinline__ Pair pmul(Pair a, Pair b) { return pair(__dmul_rn(a.x, b.x), __dmul_rn(a.y, b.y)); }
+  static __device__ __forceinline__ Pair pfma(Pair a, Pair b, Pair c) { return pair(__fma_rn(a.x, b.x, c.x), __fma_rn(a.y, b.y, c.y)); }
 };
 
 // Philox4x32-10 (Salmon et al., SC'11).  Ten rounds of two 32x32->64 multiplies and xors; the key schedule
@@ -145,6 +157,12 @@ __device__ __forceinline__ void draw_sweep(const Params& p, unsigned long long t
   ctl->order[0] = o[0]; ctl->order[1] = o[1]; ctl->order[2] = o[2]; ctl->order[3] = o[3];
   ctl->dir = G[3] >> 30;
   ctl->dist_word = H[0];
+}
+
+// ya = ci / hx, xa = ci - ya * hx with the precomputed magic numbers of Params
+__device__ __forceinline__ uint32_t div_hx(const Params& p, uint32_t ci) {
+  const uint32_t t = __umulhi(p.hx_magic, ci);
+  return (t + ((ci - t) >> p.hx_sh1)) >> p.hx_sh2;
 }
 
 // plane addressing

@@ -86,6 +86,16 @@ Layout layout(const Geom& g, bool fp32, bool debug) {
   return L;
 }
 
+// unsigned division by an invariant d >= 1 (Granlund & Montgomery 1994): q = (t + ((n - t) >> sh1)) >> sh2,
+// t = mulhi(magic, n)
+void div_magic(uint32_t d, uint32_t* magic, uint32_t* sh1, uint32_t* sh2) {
+  uint32_t l = 0;
+  while ((1ull << l) < d) ++l;
+  *magic = (uint32_t)(((1ull << 32) * ((1ull << l) - d)) / d + 1);
+  *sh1 = l < 1 ? l : 1;
+  *sh2 = l < 1 ? 0 : l - 1;
+}
+
 bool precision_ok(uint32_t flags) { return ((flags & MPMC_FP64) != 0) != ((flags & MPMC_FP32) != 0); }
 
 int cuda_fail(cudaError_t e) {
@@ -98,11 +108,19 @@ int cuda_fail(cudaError_t e) {
 dim3 cell_grid(const mpmc_ctx* c, int threads) { return dim3((c->p.Mq + threads - 1) / threads, 4, 1); }
 
 // ---- kernel launchers ----------------------------------------------------------------------------------
+template <typename P, int NF, bool DEBUG>
+void launch_sub_ns(const mpmc_ctx* c, uint32_t setk) {
+  const dim3 grid((c->p.Mq + SUB_THREADS - 1) / SUB_THREADS);
+  switch (c->p.n_s) {      // n_s = 4 and 8 (the BASELINE configs) are compile-time instantiations
+    case 4: k_sub_sweep<P, NF, 4, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); break;
+    case 8: k_sub_sweep<P, NF, 8, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); break;
+    default: k_sub_sweep<P, NF, 0, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); break;
+  }
+}
 template <typename P, bool DEBUG>
 void launch_sub_nf(const mpmc_ctx* c, uint32_t setk) {
-  const dim3 grid((c->p.Mq + SUB_THREADS - 1) / SUB_THREADS);
-  if (c->nf == 2) k_sub_sweep<P, 2, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk);
-  else            k_sub_sweep<P, 4, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk);
+  if (c->nf == 2) launch_sub_ns<P, 2, DEBUG>(c, setk);
+  else            launch_sub_ns<P, 4, DEBUG>(c, setk);
 }
 void launch_sub(const mpmc_ctx* c, uint32_t setk) {
   if (c->fp32) { if (c->debug) launch_sub_nf<float, true>(c, setk); else launch_sub_nf<float, false>(c, setk); }
@@ -210,6 +228,7 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   Params& p = c->p;
   p.mx = g.m[0]; p.my = g.m[1]; p.hx = g.m[0] / 2; p.hy = g.m[1] / 2;
   p.Mq = L.Mq; p.Mqp = L.Mqp; p.n_s = n_s; p.N = (uint32_t)N;
+  div_magic(p.hx, &p.hx_magic, &p.hx_sh1, &p.hx_sh2);
   p.seed_lo = (uint32_t)seed; p.seed_hi = (uint32_t)(seed >> 32);
   p.wx_f = (float)g.w0[0]; p.wy_f = (float)g.w0[1];
   p.sigma2_f = (float)sigma * (float)sigma; p.d_f = (float)d;

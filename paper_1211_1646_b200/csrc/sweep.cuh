@@ -13,21 +13,30 @@ constexpr int SHIFT_THREADS = 256;
 // over the dense colour plane so that a warp's 32 cells are contiguous.
 //
 //  * the cell's own <= 4 disks and the first NF disks of each of the 8 neighbour cells are loaded ONCE into
-//    registers (neighbours already translated into the active cell's frame, q = l_j + s, L154/L196) and
+//    registers, neighbours already translated into the active cell's frame (q = l_j + s, L154/L196), and are
 //    reused by all n_s moves; empty entries hold a far-away sentinel so the overlap loop has a fixed trip
 //    count and no divergence (the paper's (-10,-10) trick, L295/L346);
+//  * entries are kept NEGATED and in pairs, so that one overlap test of two disks is four packed fp32x2
+//    instructions of sm_100a (FADD2, FADD2, FMUL2, FFMA2: D = M + (-q), r^2 = fma(Dx, Dx, Dy*Dy)) and two
+//    compares; every lane of a packed instruction is one IEEE rn operation, so results are unchanged
+//    (-(a+b) = (-a)+(-b) exactly under round-to-nearest-even).  fp64 uses the same code with scalar pairs;
 //  * NF = 2 covers every neighbour at w ~ sigma except a rare few (occupancy 0/1/2); neighbours with more
 //    than NF disks set a bit in `big` and their remaining slots are re-read from L1/L2 inside the move loop;
 //    NF = 4 is the instantiation for the paper's own regime w ~ 1.4 sigma (L152);
 //  * Philox4x32-10 keyed on (seed; cell, sweep, move) replaces the per-thread Saru stream (L180, L262);
 //  * accept/reject is computed without early exit: all lanes run the same instruction stream.
+//  * NS > 0 fixes n_s at compile time (4 and 8, the BASELINE configs): the n_s Philox calls, which depend
+//    only on (seed, sweep, cell, s), are issued up front and interleaved (4-8 independent dependency chains
+//    instead of one), and the move loop is fully unrolled; NS = 0 is the generic run-time loop;
 // SETK: index into Ctl::order (0..3) or, for the test hook, 4 + explicit set.
 // ---------------------------------------------------------------------------------------------------------
-template <typename P, int NF, bool DEBUG>
+template <typename P, int NF, int NS, bool DEBUG>
 __global__ void __launch_bounds__(SUB_THREADS)
 k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
   using R = Real<P>;
   using P2 = typename R::T2;
+  using Pair = typename R::Pair;
+  constexpr int NPN = 8 * NF / 2;        // neighbour pairs
   const Ctl* __restrict__ ctl = p.ctl;
   const uint32_t Q = setk < 4 ? ctl->order[setk] : (setk & 3u);
   const unsigned long long t = ctl->t;
@@ -35,23 +44,35 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
   const uint32_t offx = Q & 1u, offy = Q >> 1;
   const uint32_t ci = blockIdx.x * SUB_THREADS + threadIdx.x;
   const bool valid = ci < p.Mq;
+  const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
+
+  // base pointers of the current buffer; planes are addressed with 32-bit element indices
+  const uint8_t* __restrict__ cntb = p.cnt[cur];
+  P2* __restrict__ posb = reinterpret_cast<P2*>(p.pos[cur]);
+  const uint32_t Mqp = p.Mqp;
 
   uint32_t n_acc = 0, n_rb = 0, n_ro = 0;
   uint32_t n = 0;
-  if (valid) n = cnt_plane(p, cur, Q)[ci];
+  if (valid) n = cntb[Q * Mqp + ci];
 
   if (n > 0) {
-    const uint32_t ya = ci / p.hx, xa = ci - ya * p.hx;
+    const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
     const uint32_t cell = (2u * ya + offy) * p.mx + (2u * xa + offx);   // canonical cell id y*mx + x
     const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p), dmax = R::d(p);
-    const P FAR = R::far_away();
+    const P NFAR = -R::far_away();
+    const Pair MINUS1 = R::pair((P)-1, (P)-1);
 
-    // ---- own cell (Alg. 2 line 8, L186) ----
-    P ox_[NMAX], oy_[NMAX];
+    // ---- own cell (Alg. 2 line 8, L186), negated, as pairs (slot 0,1) and (slot 2,3) ----
+    Pair nox[2], noy[2];
+    {
+      P vx[NMAX], vy[NMAX];
 #pragma unroll
-    for (int i = 0; i < NMAX; ++i) {
-      ox_[i] = FAR; oy_[i] = FAR;
-      if ((uint32_t)i < n) { const P2 v = pos_plane<P>(p, cur, Q, i)[ci]; ox_[i] = v.x; oy_[i] = v.y; }
+      for (int i = 0; i < NMAX; ++i) {
+        vx[i] = NFAR; vy[i] = NFAR;
+        if ((uint32_t)i < n) { const P2 v = posb[(Q * NMAX + i) * Mqp + ci]; vx[i] = -v.x; vy[i] = -v.y; }
+      }
+      nox[0] = R::pair(vx[0], vx[1]); nox[1] = R::pair(vx[2], vx[3]);
+      noy[0] = R::pair(vy[0], vy[1]); noy[1] = R::pair(vy[2], vy[3]);
     }
 
     // ---- neighbour cells: index in their colour plane, with periodic wrap ----
@@ -59,38 +80,31 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
     const uint32_t xr = offx ? (xa + 1 == p.hx ? 0 : xa + 1) : xa;        // ... of cell x+1
     const uint32_t yd = offy ? ya : (ya == 0 ? p.hy - 1 : ya - 1);
     const uint32_t yu = offy ? (ya + 1 == p.hy ? 0 : ya + 1) : ya;
+    const uint32_t rowd = yd * p.hx, rowa = ya * p.hx, rowu = yu * p.hx;
 
-    P qx[8 * NF], qy[8 * NF];
+    Pair nqx[NPN], nqy[NPN];
     uint32_t big = 0;          // bit e set: neighbour e holds more than NF disks
     uint32_t ncnt = 0;         // 4 bits per neighbour: its count
-    {
-      int e = 0;
 #pragma unroll
-      for (int oy = -1; oy <= 1; ++oy) {
+    for (int idx = 0; idx < 9; ++idx) {
+      if (idx == 4) continue;
+      const int e = idx < 4 ? idx : idx - 1;
+      const int ox = idx % 3 - 1, oy = idx / 3 - 1;
+      const uint32_t qn = ((offy ^ (uint32_t)(oy & 1)) << 1) | (offx ^ (uint32_t)(ox & 1));
+      const uint32_t cn = (oy < 0 ? rowd : oy > 0 ? rowu : rowa) + (ox < 0 ? xl : ox > 0 ? xr : xa);
+      const uint32_t nj = cntb[qn * Mqp + cn];
+      ncnt |= nj << (4 * e);
+      if (nj > (uint32_t)NF) big |= 1u << e;
+      // translation s (L154, L196); entries are stored as -(l_j + s) = fma(l_j, -1, -s), one rn operation
+      const P nsx = ox < 0 ? wx : ox > 0 ? -wx : (P)0;
+      const P nsy = oy < 0 ? wy : oy > 0 ? -wy : (P)0;
 #pragma unroll
-        for (int ox = -1; ox <= 1; ++ox) {
-          if (ox == 0 && oy == 0) continue;
-          const uint32_t qn = ((offy ^ (uint32_t)(oy & 1)) << 1) | (offx ^ (uint32_t)(ox & 1));
-          const uint32_t xn = ox < 0 ? xl : ox > 0 ? xr : xa;
-          const uint32_t yn = oy < 0 ? yd : oy > 0 ? yu : ya;
-          const uint32_t cn = yn * p.hx + xn;
-          const uint32_t nj = cnt_plane(p, cur, qn)[cn];
-          ncnt |= nj << (4 * e);
-          if (nj > (uint32_t)NF) big |= 1u << e;
-          const P sx = ox < 0 ? -wx : ox > 0 ? wx : (P)0;     // translation s (L154, L196)
-          const P sy = oy < 0 ? -wy : oy > 0 ? wy : (P)0;
-#pragma unroll
-          for (int i = 0; i < NF; ++i) {
-            P ax = FAR, ay = FAR;
-            if ((uint32_t)i < nj) {
-              const P2 v = pos_plane<P>(p, cur, qn, i)[cn];
-              ax = R::add(v.x, sx);                              // q = rn(l_j + s)
-              ay = R::add(v.y, sy);
-            }
-            qx[e * NF + i] = ax; qy[e * NF + i] = ay;
-          }
-          ++e;
-        }
+      for (int h = 0; h < NF / 2; ++h) {
+        P ax = R::far_away(), ay = R::far_away(), bx = R::far_away(), by = R::far_away();
+        if ((uint32_t)(2 * h) < nj) { const P2 v = posb[(qn * NMAX + 2 * h) * Mqp + cn]; ax = v.x; ay = v.y; }
+        if ((uint32_t)(2 * h + 1) < nj) { const P2 v = posb[(qn * NMAX + 2 * h + 1) * Mqp + cn]; bx = v.x; by = v.y; }
+        nqx[e * (NF / 2) + h] = R::pfma(R::pair(ax, bx), MINUS1, R::pair(nsx, nsx));
+        nqy[e * (NF / 2) + h] = R::pfma(R::pair(ay, by), MINUS1, R::pair(nsy, nsy));
       }
     }
 
@@ -98,7 +112,7 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
     uint32_t perm = 0x3210u;
     if (n >= 2) {
       uint32_t S[4];
-      philox4x32_10(cell, (uint32_t)t, (uint32_t)(t >> 32), SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
+      philox4x32_10(cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
 #pragma unroll
       for (int step = 0; step < NMAX - 1; ++step) {
         if ((uint32_t)step + 1u < n) {
@@ -113,54 +127,57 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
 
     // ---- n_s trial moves (Alg. 2 lines 11-32, L189-230) ----
     uint32_t amask = 0, vi = 0;
-    bool changed = false;
-    for (uint32_t s = 0; s < p.n_s; ++s) {
+    // displacement of move s: (d u(R0), d u(R1)), R = Philox(seed; cell, sweep, s)   (line 12, L190; A2, A9)
+    auto displacement = [&](uint32_t s, P& ddx, P& ddy) {
+      uint32_t Rw[4];
+      philox4x32_10(cell, t_lo, t_hi, s, p.seed_lo, p.seed_hi, Rw);
+      ddx = R::mul(dmax, R::sym(Rw[0]));
+      ddy = R::mul(dmax, R::sym(Rw[1]));
+    };
+    auto trial_move = [&](const uint32_t s, const P ddx, const P ddy) {
       const uint32_t k = (perm >> (4u * vi)) & 3u;               // p <- particles[s mod n]  (L75)
       vi = (vi + 1u == n) ? 0u : vi + 1u;                        // lines 28-32 (L224-230)
-      uint32_t Rw[4];
-      philox4x32_10(cell, (uint32_t)t, (uint32_t)(t >> 32), s, p.seed_lo, p.seed_hi, Rw);
-      const P lx = k == 0 ? ox_[0] : k == 1 ? ox_[1] : k == 2 ? ox_[2] : ox_[3];
-      const P ly = k == 0 ? oy_[0] : k == 1 ? oy_[1] : k == 2 ? oy_[2] : oy_[3];
-      const P Mx = R::add(lx, R::mul(dmax, R::sym(Rw[0])));      // line 12 (L190); square proposal (A2)
-      const P My = R::add(ly, R::mul(dmax, R::sym(Rw[1])));
+      const P nlx = k == 0 ? nox[0].x : k == 1 ? nox[0].y : k == 2 ? nox[1].x : nox[1].y;
+      const P nly = k == 0 ? noy[0].x : k == 1 ? noy[0].y : k == 2 ? noy[1].x : noy[1].y;
+      const P Mx = R::sub(ddx, nlx);                             // D_move = l + displacement
+      const P My = R::sub(ddy, nly);
       const bool inside = (Mx > (P)0) && (Mx <= wx) && (My > (P)0) && (My <= wy);   // (0, w]  (A3)
+      const Pair MMx = R::pair(Mx, Mx), MMy = R::pair(My, My);
       bool ov = false;
       // the other disks of the own cell (line 17 skips i = j, L201); s = 0 so q = l_j
 #pragma unroll
-      for (int j = 0; j < NMAX; ++j) {
-        const P Dx = R::sub(Mx, ox_[j]), Dy = R::sub(My, oy_[j]);
-        const P r2 = R::fma(Dx, Dx, R::mul(Dy, Dy));
-        ov |= (r2 < sigma2) && ((uint32_t)j != k);
+      for (int h = 0; h < 2; ++h) {
+        const Pair Dx = R::padd(MMx, nox[h]), Dy = R::padd(MMy, noy[h]);
+        const Pair r2 = R::pfma(Dx, Dx, R::pmul(Dy, Dy));
+        ov |= (r2.x < sigma2) && ((uint32_t)(2 * h) != k);
+        ov |= (r2.y < sigma2) && ((uint32_t)(2 * h + 1) != k);
       }
-      // neighbour disks held in registers
+      // neighbour disks held in registers: |D_move - (D + s)|^2 < sigma^2 (line 19, L204)
 #pragma unroll
-      for (int e = 0; e < 8 * NF; ++e) {
-        const P Dx = R::sub(Mx, qx[e]), Dy = R::sub(My, qy[e]);
-        const P r2 = R::fma(Dx, Dx, R::mul(Dy, Dy));             // |D_move - (D + s)|^2 < sigma^2 (line 19, L204)
-        ov |= r2 < sigma2;
+      for (int e = 0; e < NPN; ++e) {
+        const Pair Dx = R::padd(MMx, nqx[e]), Dy = R::padd(MMy, nqy[e]);
+        const Pair r2 = R::pfma(Dx, Dx, R::pmul(Dy, Dy));
+        ov |= (r2.x < sigma2) || (r2.y < sigma2);
       }
       if (NF < NMAX && big != 0 && inside && !ov) {              // rare: neighbours with more than NF disks
-        int e = 0;
-        for (int oy = -1; oy <= 1; ++oy)
-          for (int ox = -1; ox <= 1; ++ox) {
-            if (ox == 0 && oy == 0) continue;
-            if ((big >> e) & 1u) {
-              const uint32_t qn = ((offy ^ (uint32_t)(oy & 1)) << 1) | (offx ^ (uint32_t)(ox & 1));
-              const uint32_t xn = ox < 0 ? xl : ox > 0 ? xr : xa;
-              const uint32_t yn = oy < 0 ? yd : oy > 0 ? yu : ya;
-              const uint32_t cn = yn * p.hx + xn;
-              const uint32_t nj = (ncnt >> (4 * e)) & 15u;
-              const P sx = ox < 0 ? -wx : ox > 0 ? wx : (P)0;
-              const P sy = oy < 0 ? -wy : oy > 0 ? wy : (P)0;
-              for (uint32_t i = NF; i < nj; ++i) {
-                const P2 v = pos_plane<P>(p, cur, qn, i)[cn];
-                const P Dx = R::sub(Mx, R::add(v.x, sx)), Dy = R::sub(My, R::add(v.y, sy));
-                const P r2 = R::fma(Dx, Dx, R::mul(Dy, Dy));
-                ov |= r2 < sigma2;
-              }
-            }
-            ++e;
+#pragma unroll 1
+        for (int idx = 0; idx < 9; ++idx) {
+          if (idx == 4) continue;
+          const int e = idx < 4 ? idx : idx - 1;
+          if (!((big >> e) & 1u)) continue;
+          const int ox = idx % 3 - 1, oy = idx / 3 - 1;
+          const uint32_t qn = ((offy ^ (uint32_t)(oy & 1)) << 1) | (offx ^ (uint32_t)(ox & 1));
+          const uint32_t cn = (oy < 0 ? rowd : oy > 0 ? rowu : rowa) + (ox < 0 ? xl : ox > 0 ? xr : xa);
+          const uint32_t nj = (ncnt >> (4 * e)) & 15u;
+          const P sx = ox < 0 ? -wx : ox > 0 ? wx : (P)0;
+          const P sy = oy < 0 ? -wy : oy > 0 ? wy : (P)0;
+          for (uint32_t i = NF; i < nj; ++i) {
+            const P2 v = posb[(qn * NMAX + i) * Mqp + cn];
+            const P Dx = R::sub(Mx, R::add(v.x, sx)), Dy = R::sub(My, R::add(v.y, sy));
+            const P r2 = R::fma(Dx, Dx, R::mul(Dy, Dy));
+            ov |= r2 < sigma2;
           }
+        }
       }
       if (!inside) {
         ++n_rb;                                                  // leaves the cell: rejected (L79, L118)
@@ -169,25 +186,41 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
       } else {                                                   // lines 24-27 (L215-222)
         ++n_acc;
         amask |= 1u << (s & 31u);
-        changed = true;
+        const P nMx = -Mx, nMy = -My;
+        if (k == 0) { nox[0].x = nMx; noy[0].x = nMy; }
+        if (k == 1) { nox[0].y = nMx; noy[0].y = nMy; }
+        if (k == 2) { nox[1].x = nMx; noy[1].x = nMy; }
+        if (k == 3) { nox[1].y = nMx; noy[1].y = nMy; }
+      }
+    };
+    if (NS > 0) {
+      P ddx[NS > 0 ? NS : 1], ddy[NS > 0 ? NS : 1];
 #pragma unroll
-        for (int j = 0; j < NMAX; ++j)
-          if ((uint32_t)j == k) { ox_[j] = Mx; oy_[j] = My; }
+      for (int s = 0; s < NS; ++s) displacement((uint32_t)s, ddx[s], ddy[s]);
+#pragma unroll
+      for (int s = 0; s < NS; ++s) trial_move((uint32_t)s, ddx[s], ddy[s]);
+    } else {
+      for (uint32_t s = 0; s < p.n_s; ++s) {
+        P ddx, ddy;
+        displacement(s, ddx, ddy);
+        trial_move(s, ddx, ddy);
       }
     }
 
     // ---- write back (line 34, L234) ----
-    if (changed) {
+    if (amask != 0) {
+      const P vx[NMAX] = {nox[0].x, nox[0].y, nox[1].x, nox[1].y};
+      const P vy[NMAX] = {noy[0].x, noy[0].y, noy[1].x, noy[1].y};
 #pragma unroll
       for (int i = 0; i < NMAX; ++i)
-        if ((uint32_t)i < n) { P2 v; v.x = ox_[i]; v.y = oy_[i]; pos_plane<P>(p, cur, Q, i)[ci] = v; }
+        if ((uint32_t)i < n) { P2 v; v.x = -vx[i]; v.y = -vy[i]; posb[(Q * NMAX + i) * Mqp + ci] = v; }
     }
     if (DEBUG) {
       p.mask[cell] = amask;
       atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)cell << 32) | amask)));
     }
   } else if (DEBUG && valid) {
-    const uint32_t ya = ci / p.hx, xa = ci - ya * p.hx;
+    const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
     p.mask[(2u * ya + offy) * p.mx + (2u * xa + offx)] = 0u;
   }
 
@@ -216,11 +249,79 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
 // order and shift, so a sweep needs no host involvement.
 // ovr: 0 = use Ctl's draws and advance the sweep; 1 = test hook (explicit dir/delta, sweep index unchanged).
 // ---------------------------------------------------------------------------------------------------------
+// one new cell; ALONG_X and POSITIVE are uniform across the grid, so the caller branches once
+template <typename P, bool ALONG_X, bool POSITIVE>
+__device__ __forceinline__ void shift_cell(const Params& p, Ctl* ctl, const uint32_t cur, const uint32_t Q,
+                                           const uint32_t ci, const P delta) {
+  using R = Real<P>;
+  using P2 = typename R::T2;
+  const uint32_t nxt = cur ^ 1u, Mqp = p.Mqp;
+  const uint8_t* __restrict__ cntc = p.cnt[cur];
+  const P2* __restrict__ posc = reinterpret_cast<const P2*>(p.pos[cur]);
+  const uint32_t* __restrict__ idsc = p.ids[cur];
+  P2* __restrict__ posn = reinterpret_cast<P2*>(p.pos[nxt]);
+  uint32_t* __restrict__ idsn = p.ids[nxt];
+  const P w = ALONG_X ? R::wx(p) : R::wy(p);
+  const P step = POSITIVE ? -delta : delta;     // l' = l - f*delta   (L303)
+  const P back = POSITIVE ? w : -w;             // entrant translation (L332)
+  const uint32_t offx = Q & 1u, offy = Q >> 1;
+  // the old neighbour in direction f (lines 15-16, L314-317)
+  uint32_t qn, cn;
+  if (ALONG_X) {
+    const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
+    qn = Q ^ 1u;
+    const uint32_t xn = POSITIVE ? (offx ? (xa + 1 == p.hx ? 0 : xa + 1) : xa)
+                                 : (offx ? xa : (xa == 0 ? p.hx - 1 : xa - 1));
+    cn = ci - xa + xn;
+  } else {
+    qn = Q ^ 2u;
+    // one row up or down in the other colour: +-hx with wrap over the Mq = hx*hy cells of the plane
+    if (POSITIVE) cn = offy ? (ci + p.hx >= p.Mq ? ci + p.hx - p.Mq : ci + p.hx) : ci;
+    else          cn = offy ? ci : (ci < p.hx ? ci + p.Mq - p.hx : ci - p.hx);
+  }
+  const uint32_t own0 = Q * NMAX * Mqp + ci, nb0 = qn * NMAX * Mqp + cn;
+  const uint32_t n0 = cntc[Q * Mqp + ci], n1 = cntc[qn * Mqp + cn];
+  uint32_t nn = 0;
+  // lines 7-14 (L299-312): own disks that stay, in slot order
+#pragma unroll
+  for (int i = 0; i < NMAX; ++i) {
+    if ((uint32_t)i < n0) {
+      P2 v = posc[own0 + i * Mqp];
+      const uint32_t id = idsc[own0 + i * Mqp];
+      const P a = R::add(ALONG_X ? v.x : v.y, step);
+      if (a > (P)0 && a <= w) {
+        if (ALONG_X) v.x = a; else v.y = a;
+        posn[own0 + nn * Mqp] = v;
+        idsn[own0 + nn * Mqp] = id;
+        ++nn;
+      }
+    }
+  }
+  // lines 17-27 (L319-339): disks of the neighbour that left it enter here
+#pragma unroll
+  for (int i = 0; i < NMAX; ++i) {
+    if ((uint32_t)i < n1) {
+      P2 v = posc[nb0 + i * Mqp];
+      const P a = R::add(ALONG_X ? v.x : v.y, step);
+      if (!(a > (P)0 && a <= w)) {              // else: stays in the neighbour (L326-328)
+        const P b = R::add(a, back);            // L332: a separate operation after the test (L352)
+        if (nn < (uint32_t)NMAX) {
+          if (ALONG_X) v.x = b; else v.y = b;
+          posn[own0 + nn * Mqp] = v;
+          idsn[own0 + nn * Mqp] = idsc[nb0 + i * Mqp];
+        }
+        ++nn;
+      }
+    }
+  }
+  if (nn > (uint32_t)NMAX) { atomicOr(&ctl->err, ERRBIT_OVERFLOW); nn = NMAX; }
+  p.cnt[nxt][Q * Mqp + ci] = (uint8_t)nn;        // L280, L342
+}
+
 template <typename P>
 __global__ void __launch_bounds__(SHIFT_THREADS)
 k_shift(const __grid_constant__ Params p, const uint32_t ovr, const uint32_t ovr_dir, const double ovr_delta) {
   using R = Real<P>;
-  using P2 = typename R::T2;
   Ctl* ctl = p.ctl;
   const uint32_t cur = ctl->cur, nxt = cur ^ 1u;
   const uint32_t dir = ovr ? ovr_dir : ctl->dir;
@@ -228,56 +329,18 @@ k_shift(const __grid_constant__ Params p, const uint32_t ovr, const uint32_t ovr
   const P w = along_x ? R::wx(p) : R::wy(p);
   // Alg. 1 line 15 (L90): delta = uniform(0, w/2) = rn(rn(0.5 w) * u01)
   const P delta = ovr ? (P)ovr_delta : R::mul(R::mul((P)0.5, w), R::unit(ctl->dist_word));
-  const P step = positive ? -delta : delta;     // l' = l - f*delta   (L303)
-  const P back = positive ? w : -w;             // entrant translation (L332)
   const unsigned long long t = ctl->t;
 
   const uint32_t Q = blockIdx.y;
   const uint32_t ci = blockIdx.x * SHIFT_THREADS + threadIdx.x;
   if (ci < p.Mq) {
-    const uint32_t offx = Q & 1u, offy = Q >> 1;
-    const uint32_t ya = ci / p.hx, xa = ci - ya * p.hx;
-    uint32_t nn = 0;
-    // lines 7-14 (L299-312): own disks that stay
-    const uint32_t n0 = cnt_plane(p, cur, Q)[ci];
-    for (uint32_t i = 0; i < n0; ++i) {
-      P2 v = pos_plane<P>(p, cur, Q, i)[ci];
-      P a = R::add(along_x ? v.x : v.y, step);
-      if (a > (P)0 && a <= w) {
-        if (along_x) v.x = a; else v.y = a;
-        pos_plane<P>(p, nxt, Q, nn)[ci] = v;
-        ids_plane(p, nxt, Q, nn)[ci] = ids_plane(p, cur, Q, i)[ci];
-        ++nn;
-      }
-    }
-    // lines 15-27 (L314-339): the neighbour in direction f
-    uint32_t qn, cn;
     if (along_x) {
-      qn = Q ^ 1u;
-      const uint32_t xn = positive ? (offx ? (xa + 1 == p.hx ? 0 : xa + 1) : xa)
-                                   : (offx ? xa : (xa == 0 ? p.hx - 1 : xa - 1));
-      cn = ya * p.hx + xn;
+      if (positive) shift_cell<P, true, true>(p, ctl, cur, Q, ci, delta);
+      else          shift_cell<P, true, false>(p, ctl, cur, Q, ci, delta);
     } else {
-      qn = Q ^ 2u;
-      const uint32_t yn = positive ? (offy ? (ya + 1 == p.hy ? 0 : ya + 1) : ya)
-                                   : (offy ? ya : (ya == 0 ? p.hy - 1 : ya - 1));
-      cn = yn * p.hx + xa;
+      if (positive) shift_cell<P, false, true>(p, ctl, cur, Q, ci, delta);
+      else          shift_cell<P, false, false>(p, ctl, cur, Q, ci, delta);
     }
-    const uint32_t n1 = cnt_plane(p, cur, qn)[cn];
-    for (uint32_t i = 0; i < n1; ++i) {
-      P2 v = pos_plane<P>(p, cur, qn, i)[cn];
-      P a = R::add(along_x ? v.x : v.y, step);
-      if (a > (P)0 && a <= w) continue;         // stays in the neighbour (L326-328)
-      a = R::add(a, back);                      // L332
-      if (nn < (uint32_t)NMAX) {
-        if (along_x) v.x = a; else v.y = a;
-        pos_plane<P>(p, nxt, Q, nn)[ci] = v;
-        ids_plane(p, nxt, Q, nn)[ci] = ids_plane(p, cur, qn, i)[cn];
-      }
-      ++nn;
-    }
-    if (nn > (uint32_t)NMAX) { atomicOr(&ctl->err, ERRBIT_OVERFLOW); nn = NMAX; }
-    cnt_plane(p, nxt, Q)[ci] = (uint8_t)nn;      // L280, L342
   }
 
   // ---- last block done: advance the control block ----
