@@ -41,7 +41,7 @@ _lib = None
 
 
 def library_path() -> str:
-    return _build.LIB
+    return os.environ.get("MPMC_B200_LIB") or _build.LIB
 
 
 def lib() -> C.CDLL:

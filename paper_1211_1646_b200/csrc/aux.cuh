@@ -16,7 +16,8 @@ __global__ void k_reset(const __grid_constant__ Params p) {
     Ctl* c = p.ctl;
     c->t = 0; c->cur = 0; c->err = 0; c->ticket = 0; c->pad0 = 0;
     c->origin[0] = 0.0; c->origin[1] = 0.0;
-    c->counters[0] = c->counters[1] = c->counters[2] = 0; c->digest = 0;
+    c->digest = 0;
+    for (uint32_t r = 0; r < CTR_SLOTS; ++r) c->counters[r][0] = c->counters[r][1] = c->counters[r][2] = c->counters[r][3] = 0;
     draw_sweep(p, 0ull, c);
   }
 }

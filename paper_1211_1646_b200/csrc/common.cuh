@@ -32,6 +32,7 @@ constexpr uint32_t SLOT_DIST = 0xFFFFFFFEu;     // shift distance
 constexpr uint32_t ERRBIT_OVERFLOW = 1u;  // a cell would hold more than NMAX disks
 constexpr uint32_t ERRBIT_RANGE = 2u;     // loaded coordinate NaN or outside [0, L]
 constexpr uint32_t ERRBIT_OVERLAP = 4u;   // loaded positions overlap
+constexpr uint32_t CTR_SLOTS = 64;        // rows of move counters (summed on read)
 
 // Device-resident control block: everything that changes from sweep to sweep, so that a captured CUDA graph
 // can be replayed with no host-side argument updates (mpmc.h, mpmc_sweep).
@@ -45,8 +46,8 @@ struct Ctl {
   uint32_t ticket;                 // blocks-done counter of the shift kernel
   uint32_t pad0;
   double origin[2];                // grid origin: X = origin + cell * w + local
-  unsigned long long counters[3];  // accepted, rejected_boundary, rejected_overlap
   unsigned long long digest;       // accept-sequence digest (MPMC_DEBUG)
+  unsigned long long counters[CTR_SLOTS][4];  // per row: accepted, rejected_boundary, rejected_overlap, -
 };
 
 // Kernel parameters (by value, __grid_constant__): geometry and the workspace pointers.
@@ -163,6 +164,24 @@ __device__ __forceinline__ void draw_sweep(const Params& p, unsigned long long t
 __device__ __forceinline__ uint32_t div_hx(const Params& p, uint32_t ci) {
   const uint32_t t = __umulhi(p.hx_magic, ci);
   return (t + ((ci - t) >> p.hx_sh1)) >> p.hx_sh2;
+}
+
+// Prefetching loads.  `asm volatile` keeps the compiler from sinking them into the branch that consumes them,
+// so they are issued up front and their latency overlaps the Philox arithmetic (sweep.cuh, level-1 loads).
+__device__ __forceinline__ uint32_t ld_u8_early(const uint8_t* ptr) {
+  uint32_t v;
+  asm volatile("ld.global.u8 %0, [%1];" : "=r"(v) : "l"(ptr));
+  return v;
+}
+__device__ __forceinline__ float2 ld_pos_early(const float2* ptr) {
+  float2 v;
+  asm volatile("ld.global.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(ptr));
+  return v;
+}
+__device__ __forceinline__ double2 ld_pos_early(const double2* ptr) {
+  double2 v;
+  asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(ptr));
+  return v;
 }
 
 // plane addressing

@@ -335,7 +335,8 @@ int mpmc_acceptance(mpmc_ctx* c, uint64_t out[4]) {
   if (!c->loaded) return MPMC_ERR_STATE;
   Ctl h;
   const int st = read_ctl(c, &h);
-  out[1] = h.counters[0]; out[2] = h.counters[1]; out[3] = h.counters[2];
+  out[1] = out[2] = out[3] = 0;
+  for (uint32_t r = 0; r < CTR_SLOTS; ++r) { out[1] += h.counters[r][0]; out[2] += h.counters[r][1]; out[3] += h.counters[r][2]; }
   out[0] = out[1] + out[2] + out[3];
   return st;
 }

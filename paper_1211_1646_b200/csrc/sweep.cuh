@@ -5,7 +5,14 @@
 
 namespace mpmc {
 
-constexpr int SUB_THREADS = 128;
+#ifndef MPMC_SUB_THREADS
+#define MPMC_SUB_THREADS 128
+#endif
+#ifndef MPMC_SUB_MINB
+#define MPMC_SUB_MINB 1
+#endif
+constexpr int SUB_THREADS = MPMC_SUB_THREADS;
+constexpr int SUB_MINB = MPMC_SUB_MINB;      // minimum resident blocks per SM asked of ptxas (register cap)
 constexpr int SHIFT_THREADS = 256;
 
 // ---------------------------------------------------------------------------------------------------------
@@ -31,7 +38,7 @@ constexpr int SHIFT_THREADS = 256;
 // SETK: index into Ctl::order (0..3) or, for the test hook, 4 + explicit set.
 // ---------------------------------------------------------------------------------------------------------
 template <typename P, int NF, int NS, bool DEBUG>
-__global__ void __launch_bounds__(SUB_THREADS)
+__global__ void __launch_bounds__(SUB_THREADS, SUB_MINB)
 k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
   using R = Real<P>;
   using P2 = typename R::T2;
@@ -42,8 +49,9 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
   const unsigned long long t = ctl->t;
   const uint32_t cur = ctl->cur;
   const uint32_t offx = Q & 1u, offy = Q >> 1;
-  const uint32_t ci = blockIdx.x * SUB_THREADS + threadIdx.x;
-  const bool valid = ci < p.Mq;
+  const uint32_t ci_raw = blockIdx.x * SUB_THREADS + threadIdx.x;
+  const bool valid = ci_raw < p.Mq;
+  const uint32_t ci = valid ? ci_raw : p.Mq - 1u;      // clamped: every lane may prefetch
   const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
 
   // base pointers of the current buffer; planes are addressed with 32-bit element indices
@@ -51,96 +59,128 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
   P2* __restrict__ posb = reinterpret_cast<P2*>(p.pos[cur]);
   const uint32_t Mqp = p.Mqp;
 
-  uint32_t n_acc = 0, n_rb = 0, n_ro = 0;
-  uint32_t n = 0;
-  if (valid) n = cntb[Q * Mqp + ci];
+  // ---- cell and neighbour indices in the colour planes, with periodic wrap ----
+  const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
+  const uint32_t cell = (2u * ya + offy) * p.mx + (2u * xa + offx);   // canonical cell id y*mx + x
+  const uint32_t xl = offx ? xa : (xa == 0 ? p.hx - 1 : xa - 1);        // plane column of cell x-1
+  const uint32_t xr = offx ? (xa + 1 == p.hx ? 0 : xa + 1) : xa;        // ... of cell x+1
+  const uint32_t yd = offy ? ya : (ya == 0 ? p.hy - 1 : ya - 1);
+  const uint32_t yu = offy ? (ya + 1 == p.hy ? 0 : ya + 1) : ya;
+  const uint32_t rowd = yd * p.hx, rowa = ya * p.hx, rowu = yu * p.hx;
 
-  if (n > 0) {
-    const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
-    const uint32_t cell = (2u * ya + offy) * p.mx + (2u * xa + offx);   // canonical cell id y*mx + x
-    const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p), dmax = R::d(p);
-    const P NFAR = -R::far_away();
+  // ---- level-1 loads, all independent: count and slot 0 of the 3x3 cells (idx 4 = own cell) ----
+  uint32_t cidx[9], cj[9];
+  P2 v0[9];
+#pragma unroll
+  for (int idx = 0; idx < 9; ++idx) {
+    const int ox = idx % 3 - 1, oy = idx / 3 - 1;
+    const uint32_t qn = ((offy ^ (uint32_t)(oy & 1)) << 1) | (offx ^ (uint32_t)(ox & 1));
+    const uint32_t cn = (oy < 0 ? rowd : oy > 0 ? rowu : rowa) + (ox < 0 ? xl : ox > 0 ? xr : xa);
+    cidx[idx] = qn * Mqp + cn;                       // count index; slot s of the cell is at 4*qn*Mqp + s*Mqp + cn
+    cj[idx] = ld_u8_early(cntb + cidx[idx]);
+    v0[idx] = ld_pos_early(posb + (cidx[idx] + 3u * qn * Mqp));
+  }
+
+  // ---- arithmetic that needs no memory, issued while the loads are in flight: the Philox words of the
+  //      shuffle (Alg. 2 line 9) and of the first half of the displacements (line 12, L190; A2, A9) ----
+  const P dmax = R::d(p);
+  auto displacement = [&](uint32_t s, P& ddx, P& ddy) {
+    uint32_t Rw[4];
+    philox4x32_10(cell, t_lo, t_hi, s, p.seed_lo, p.seed_hi, Rw);
+    ddx = R::mul(dmax, R::sym(Rw[0]));
+    ddy = R::mul(dmax, R::sym(Rw[1]));
+  };
+  uint32_t S[4];
+  philox4x32_10(cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
+  constexpr int NSA = NS > 0 ? NS : 1;
+  P ddx[NSA], ddy[NSA];
+  if (NS > 0) {
+#pragma unroll
+    for (int s = 0; s < NS / 2; ++s) displacement((uint32_t)s, ddx[s], ddy[s]);
+  }
+
+  uint32_t n_acc = 0, n_rb = 0, n_ro = 0;
+  // Empty cells (and the clamped lanes past the end) run the same instruction stream on sentinels and are
+  // masked out of the counters and the write-back: no lane-dependent branch stands between the loads above
+  // and their first use, so the loads are issued before the Philox arithmetic and overlap it.  (Skipping an
+  // empty cell saves nothing unless all 32 cells of a warp are empty; Alg. 2 lines 4-7, L181-185.)
+  if (!valid) cj[4] = 0u;
+  const uint32_t n = cj[4];
+  const uint32_t nv = n > 0u ? n : 1u;                 // visiting modulus; an empty cell "visits" a sentinel
+
+  {
+    const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p);
+    const P FAR = R::far_away();
     const Pair MINUS1 = R::pair((P)-1, (P)-1);
+
+    // ---- level-2 loads: the occupied higher slots (rare at w ~ sigma) ----
+    P2 v1[9], v2[9], v3[9];
+    uint32_t big = 0;          // bit idx set: neighbour idx holds more than NF disks
+#pragma unroll
+    for (int idx = 0; idx < 9; ++idx) {
+      const int ox = idx % 3 - 1, oy = idx / 3 - 1;
+      const uint32_t qn = ((offy ^ (uint32_t)(oy & 1)) << 1) | (offx ^ (uint32_t)(ox & 1));
+      const uint32_t s0 = cidx[idx] + 3u * qn * Mqp;
+      v1[idx].x = FAR; v1[idx].y = FAR; v2[idx] = v1[idx]; v3[idx] = v1[idx];
+      if (cj[idx] > 1u) v1[idx] = posb[s0 + Mqp];
+      if (idx == 4 || NF == 4) {
+        if (cj[idx] > 2u) v2[idx] = posb[s0 + 2u * Mqp];
+        if (cj[idx] > 3u) v3[idx] = posb[s0 + 3u * Mqp];
+      } else if (cj[idx] > (uint32_t)NF) {
+        big |= 1u << idx;
+      }
+      if (cj[idx] == 0u) { v0[idx].x = FAR; v0[idx].y = FAR; }
+    }
+    if (NS > 0) {
+#pragma unroll
+      for (int s = NS / 2; s < NS; ++s) displacement((uint32_t)s, ddx[s], ddy[s]);
+    }
 
     // ---- own cell (Alg. 2 line 8, L186), negated, as pairs (slot 0,1) and (slot 2,3) ----
     Pair nox[2], noy[2];
-    {
-      P vx[NMAX], vy[NMAX];
-#pragma unroll
-      for (int i = 0; i < NMAX; ++i) {
-        vx[i] = NFAR; vy[i] = NFAR;
-        if ((uint32_t)i < n) { const P2 v = posb[(Q * NMAX + i) * Mqp + ci]; vx[i] = -v.x; vy[i] = -v.y; }
-      }
-      nox[0] = R::pair(vx[0], vx[1]); nox[1] = R::pair(vx[2], vx[3]);
-      noy[0] = R::pair(vy[0], vy[1]); noy[1] = R::pair(vy[2], vy[3]);
-    }
+    nox[0] = R::pair(-v0[4].x, -v1[4].x); nox[1] = R::pair(-v2[4].x, -v3[4].x);
+    noy[0] = R::pair(-v0[4].y, -v1[4].y); noy[1] = R::pair(-v2[4].y, -v3[4].y);
 
-    // ---- neighbour cells: index in their colour plane, with periodic wrap ----
-    const uint32_t xl = offx ? xa : (xa == 0 ? p.hx - 1 : xa - 1);        // plane column of cell x-1
-    const uint32_t xr = offx ? (xa + 1 == p.hx ? 0 : xa + 1) : xa;        // ... of cell x+1
-    const uint32_t yd = offy ? ya : (ya == 0 ? p.hy - 1 : ya - 1);
-    const uint32_t yu = offy ? (ya + 1 == p.hy ? 0 : ya + 1) : ya;
-    const uint32_t rowd = yd * p.hx, rowa = ya * p.hx, rowu = yu * p.hx;
-
+    // ---- neighbours, translated into this cell's frame (s = (ox wx, oy wy), L154, L196), negated:
+    //      -(l_j + s) = fma(l_j, -1, -s), one rn operation ----
     Pair nqx[NPN], nqy[NPN];
-    uint32_t big = 0;          // bit e set: neighbour e holds more than NF disks
-    uint32_t ncnt = 0;         // 4 bits per neighbour: its count
 #pragma unroll
     for (int idx = 0; idx < 9; ++idx) {
       if (idx == 4) continue;
       const int e = idx < 4 ? idx : idx - 1;
       const int ox = idx % 3 - 1, oy = idx / 3 - 1;
-      const uint32_t qn = ((offy ^ (uint32_t)(oy & 1)) << 1) | (offx ^ (uint32_t)(ox & 1));
-      const uint32_t cn = (oy < 0 ? rowd : oy > 0 ? rowu : rowa) + (ox < 0 ? xl : ox > 0 ? xr : xa);
-      const uint32_t nj = cntb[qn * Mqp + cn];
-      ncnt |= nj << (4 * e);
-      if (nj > (uint32_t)NF) big |= 1u << e;
-      // translation s (L154, L196); entries are stored as -(l_j + s) = fma(l_j, -1, -s), one rn operation
       const P nsx = ox < 0 ? wx : ox > 0 ? -wx : (P)0;
       const P nsy = oy < 0 ? wy : oy > 0 ? -wy : (P)0;
-#pragma unroll
-      for (int h = 0; h < NF / 2; ++h) {
-        P ax = R::far_away(), ay = R::far_away(), bx = R::far_away(), by = R::far_away();
-        if ((uint32_t)(2 * h) < nj) { const P2 v = posb[(qn * NMAX + 2 * h) * Mqp + cn]; ax = v.x; ay = v.y; }
-        if ((uint32_t)(2 * h + 1) < nj) { const P2 v = posb[(qn * NMAX + 2 * h + 1) * Mqp + cn]; bx = v.x; by = v.y; }
-        nqx[e * (NF / 2) + h] = R::pfma(R::pair(ax, bx), MINUS1, R::pair(nsx, nsx));
-        nqy[e * (NF / 2) + h] = R::pfma(R::pair(ay, by), MINUS1, R::pair(nsy, nsy));
+      nqx[e * (NF / 2)] = R::pfma(R::pair(v0[idx].x, v1[idx].x), MINUS1, R::pair(nsx, nsx));
+      nqy[e * (NF / 2)] = R::pfma(R::pair(v0[idx].y, v1[idx].y), MINUS1, R::pair(nsy, nsy));
+      if (NF == 4) {
+        nqx[e * (NF / 2) + NF / 2 - 1] = R::pfma(R::pair(v2[idx].x, v3[idx].x), MINUS1, R::pair(nsx, nsx));
+        nqy[e * (NF / 2) + NF / 2 - 1] = R::pfma(R::pair(v2[idx].y, v3[idx].y), MINUS1, R::pair(nsy, nsy));
       }
     }
 
     // ---- shuffle (Alg. 2 line 9, L187), kept as a visiting permutation packed in nibbles ----
     uint32_t perm = 0x3210u;
-    if (n >= 2) {
-      uint32_t S[4];
-      philox4x32_10(cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
 #pragma unroll
-      for (int step = 0; step < NMAX - 1; ++step) {
-        if ((uint32_t)step + 1u < n) {
-          const uint32_t i = n - 1u - (uint32_t)step;
-          const uint32_t j = bounded(S[step], i + 1u);
-          const uint32_t a = (perm >> (4u * i)) & 15u, b = (perm >> (4u * j)) & 15u;
-          const uint32_t x = a ^ b;
-          perm ^= (x << (4u * i)) ^ (x << (4u * j));
-        }
+    for (int step = 0; step < NMAX - 1; ++step) {
+      if ((uint32_t)step + 1u < n) {
+        const uint32_t i = n - 1u - (uint32_t)step;
+        const uint32_t j = bounded(S[step], i + 1u);
+        const uint32_t a = (perm >> (4u * i)) & 15u, b = (perm >> (4u * j)) & 15u;
+        const uint32_t x = a ^ b;
+        perm ^= (x << (4u * i)) ^ (x << (4u * j));
       }
     }
 
     // ---- n_s trial moves (Alg. 2 lines 11-32, L189-230) ----
     uint32_t amask = 0, vi = 0;
-    // displacement of move s: (d u(R0), d u(R1)), R = Philox(seed; cell, sweep, s)   (line 12, L190; A2, A9)
-    auto displacement = [&](uint32_t s, P& ddx, P& ddy) {
-      uint32_t Rw[4];
-      philox4x32_10(cell, t_lo, t_hi, s, p.seed_lo, p.seed_hi, Rw);
-      ddx = R::mul(dmax, R::sym(Rw[0]));
-      ddy = R::mul(dmax, R::sym(Rw[1]));
-    };
-    auto trial_move = [&](const uint32_t s, const P ddx, const P ddy) {
+    auto trial_move = [&](const uint32_t s, const P dx, const P dy) {
       const uint32_t k = (perm >> (4u * vi)) & 3u;               // p <- particles[s mod n]  (L75)
-      vi = (vi + 1u == n) ? 0u : vi + 1u;                        // lines 28-32 (L224-230)
+      vi = (vi + 1u == nv) ? 0u : vi + 1u;                       // lines 28-32 (L224-230)
       const P nlx = k == 0 ? nox[0].x : k == 1 ? nox[0].y : k == 2 ? nox[1].x : nox[1].y;
       const P nly = k == 0 ? noy[0].x : k == 1 ? noy[0].y : k == 2 ? noy[1].x : noy[1].y;
-      const P Mx = R::sub(ddx, nlx);                             // D_move = l + displacement
-      const P My = R::sub(ddy, nly);
+      const P Mx = R::sub(dx, nlx);                              // D_move = l + displacement
+      const P My = R::sub(dy, nly);
       const bool inside = (Mx > (P)0) && (Mx <= wx) && (My > (P)0) && (My <= wy);   // (0, w]  (A3)
       const Pair MMx = R::pair(Mx, Mx), MMy = R::pair(My, My);
       bool ov = false;
@@ -162,13 +202,11 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
       if (NF < NMAX && big != 0 && inside && !ov) {              // rare: neighbours with more than NF disks
 #pragma unroll 1
         for (int idx = 0; idx < 9; ++idx) {
-          if (idx == 4) continue;
-          const int e = idx < 4 ? idx : idx - 1;
-          if (!((big >> e) & 1u)) continue;
+          if (!((big >> idx) & 1u)) continue;
           const int ox = idx % 3 - 1, oy = idx / 3 - 1;
           const uint32_t qn = ((offy ^ (uint32_t)(oy & 1)) << 1) | (offx ^ (uint32_t)(ox & 1));
           const uint32_t cn = (oy < 0 ? rowd : oy > 0 ? rowu : rowa) + (ox < 0 ? xl : ox > 0 ? xr : xa);
-          const uint32_t nj = (ncnt >> (4 * e)) & 15u;
+          const uint32_t nj = cntb[qn * Mqp + cn];
           const P sx = ox < 0 ? -wx : ox > 0 ? wx : (P)0;
           const P sy = oy < 0 ? -wy : oy > 0 ? wy : (P)0;
           for (uint32_t i = NF; i < nj; ++i) {
@@ -194,16 +232,13 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
       }
     };
     if (NS > 0) {
-      P ddx[NS > 0 ? NS : 1], ddy[NS > 0 ? NS : 1];
-#pragma unroll
-      for (int s = 0; s < NS; ++s) displacement((uint32_t)s, ddx[s], ddy[s]);
 #pragma unroll
       for (int s = 0; s < NS; ++s) trial_move((uint32_t)s, ddx[s], ddy[s]);
     } else {
       for (uint32_t s = 0; s < p.n_s; ++s) {
-        P ddx, ddy;
-        displacement(s, ddx, ddy);
-        trial_move(s, ddx, ddy);
+        P dx, dy;
+        displacement(s, dx, dy);
+        trial_move(s, dx, dy);
       }
     }
 
@@ -215,29 +250,24 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
       for (int i = 0; i < NMAX; ++i)
         if ((uint32_t)i < n) { P2 v; v.x = -vx[i]; v.y = -vy[i]; posb[(Q * NMAX + i) * Mqp + ci] = v; }
     }
-    if (DEBUG) {
+    if (DEBUG && valid) {
       p.mask[cell] = amask;
-      atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)cell << 32) | amask)));
+      if (n > 0u) atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)cell << 32) | amask)));
     }
-  } else if (DEBUG && valid) {
-    const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
-    p.mask[(2u * ya + offy) * p.mx + (2u * xa + offx)] = 0u;
   }
+  if (n == 0u) n_rb = 0u;        // a sentinel never passes the in-cell test; empty cells attempt nothing (A10)
 
-  // ---- counters: warp reduce, one shared atomic per warp, three global atomics per block ----
-  __shared__ uint32_t sh[3];
-  if (threadIdx.x < 3) sh[threadIdx.x] = 0;
-  __syncthreads();
+  // ---- counters: warp reduce, then three fire-and-forget 64-bit reductions per warp into one of CTR_SLOTS
+  //      counter rows (spread so that same-address atomics do not serialise); no block barrier ----
   n_acc = __reduce_add_sync(0xFFFFFFFFu, n_acc);
   n_rb = __reduce_add_sync(0xFFFFFFFFu, n_rb);
   n_ro = __reduce_add_sync(0xFFFFFFFFu, n_ro);
   if ((threadIdx.x & 31) == 0) {
-    if (n_acc) atomicAdd(&sh[0], n_acc);
-    if (n_rb) atomicAdd(&sh[1], n_rb);
-    if (n_ro) atomicAdd(&sh[2], n_ro);
+    unsigned long long* row = p.ctl->counters[(blockIdx.x * (SUB_THREADS / 32) + (threadIdx.x >> 5)) % CTR_SLOTS];
+    if (n_acc) atomicAdd(&row[0], (unsigned long long)n_acc);
+    if (n_rb) atomicAdd(&row[1], (unsigned long long)n_rb);
+    if (n_ro) atomicAdd(&row[2], (unsigned long long)n_ro);
   }
-  __syncthreads();
-  if (threadIdx.x < 3 && sh[threadIdx.x]) atomicAdd(&p.ctl->counters[threadIdx.x], (unsigned long long)sh[threadIdx.x]);
 }
 
 // ---------------------------------------------------------------------------------------------------------
