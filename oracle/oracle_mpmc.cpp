@@ -68,7 +68,8 @@ void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]
 }
 
 // Counter layout (reading A9): counter = (cell_id, t_lo, t_hi, slot), key = (seed_lo, seed_hi).
-//   slot s in [0, n_s)      : the two displacement words of trial move s
+//   slot q in [0, ceil(n_s/2)): the displacement words of trial moves 2q (words 0, 1 = x, y) and
+//                             2q + 1 (words 2, 3 = x, y) — all four words of a Philox block are used
 //   slot 0x80000000         : the shuffle words of the cell
 //   cell 0xFFFFFFFF, slot 0xFFFFFFFF : per-sweep set order + shift direction
 //   cell 0xFFFFFFFF, slot 0xFFFFFFFE : per-sweep shift distance
@@ -207,10 +208,11 @@ struct Sim : Base {
     for (uint32_t s = 0; s < n_s; ++s) {                        // line 11 (L189)
       const uint32_t k = visit(perm, nc, s);
       uint32_t R[4];
-      draw(seed, (uint32_t)c, t, s, R);
+      draw(seed, (uint32_t)c, t, s >> 1, R);                    // reading A9: block s/2 serves moves 2q, 2q+1
+      const uint32_t h = 2u * (s & 1u);
       // line 12 (L190); reading A2: uniform in the square [-d, d]^2
-      const P ddx = d * Variate<P>::sym(R[0]);
-      const P ddy = d * Variate<P>::sym(R[1]);
+      const P ddx = d * Variate<P>::sym(R[h]);
+      const P ddy = d * Variate<P>::sym(R[h + 1]);
       const P Mx = lx[c * NMAX + k] + ddx;
       const P My = ly[c * NMAX + k] + ddy;
       counters[0] += 1;

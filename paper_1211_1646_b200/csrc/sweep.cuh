@@ -84,19 +84,21 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
   // ---- arithmetic that needs no memory, issued while the loads are in flight: the Philox words of the
   //      shuffle (Alg. 2 line 9) and of the first half of the displacements (line 12, L190; A2, A9) ----
   const P dmax = R::d(p);
-  auto displacement = [&](uint32_t s, P& ddx, P& ddy) {
+  // Philox block q serves moves 2q (words 0, 1) and 2q + 1 (words 2, 3)  (reading A9)
+  auto displacement2 = [&](uint32_t q, P& ax, P& ay, P& bx, P& by) {
     uint32_t Rw[4];
-    philox4x32_10(cell, t_lo, t_hi, s, p.seed_lo, p.seed_hi, Rw);
-    ddx = R::mul(dmax, R::sym(Rw[0]));
-    ddy = R::mul(dmax, R::sym(Rw[1]));
+    philox4x32_10(cell, t_lo, t_hi, q, p.seed_lo, p.seed_hi, Rw);
+    ax = R::mul(dmax, R::sym(Rw[0])); ay = R::mul(dmax, R::sym(Rw[1]));
+    bx = R::mul(dmax, R::sym(Rw[2])); by = R::mul(dmax, R::sym(Rw[3]));
   };
   uint32_t S[4];
   philox4x32_10(cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
-  constexpr int NSA = NS > 0 ? NS : 1;
+  static_assert(NS % 4 == 0, "compile-time n_s must be a multiple of 4");
+  constexpr int NSA = NS > 0 ? NS : 2;
   P ddx[NSA], ddy[NSA];
   if (NS > 0) {
 #pragma unroll
-    for (int s = 0; s < NS / 2; ++s) displacement((uint32_t)s, ddx[s], ddy[s]);
+    for (int q = 0; q < NS / 4; ++q) displacement2((uint32_t)q, ddx[2 * q], ddy[2 * q], ddx[2 * q + 1], ddy[2 * q + 1]);
   }
 
   uint32_t n_acc = 0, n_rb = 0, n_ro = 0;
@@ -133,7 +135,7 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
     }
     if (NS > 0) {
 #pragma unroll
-      for (int s = NS / 2; s < NS; ++s) displacement((uint32_t)s, ddx[s], ddy[s]);
+      for (int q = NS / 4; q < NS / 2; ++q) displacement2((uint32_t)q, ddx[2 * q], ddy[2 * q], ddx[2 * q + 1], ddy[2 * q + 1]);
     }
 
     // ---- own cell (Alg. 2 line 8, L186), negated, as pairs (slot 0,1) and (slot 2,3) ----
@@ -235,10 +237,10 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
 #pragma unroll
       for (int s = 0; s < NS; ++s) trial_move((uint32_t)s, ddx[s], ddy[s]);
     } else {
-      for (uint32_t s = 0; s < p.n_s; ++s) {
-        P dx, dy;
-        displacement(s, dx, dy);
-        trial_move(s, dx, dy);
+      for (uint32_t s = 0; s < p.n_s; s += 2) {
+        displacement2(s >> 1, ddx[0], ddy[0], ddx[1], ddy[1]);
+        trial_move(s, ddx[0], ddy[0]);
+        if (s + 1 < p.n_s) trial_move(s + 1, ddx[1], ddy[1]);
       }
     }
 
