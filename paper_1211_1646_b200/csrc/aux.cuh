@@ -38,10 +38,9 @@ __device__ __forceinline__ void to_local(double X, double w_d, P w, uint32_t m, 
 }
 
 // Cell-list build, pass 1: one thread per disk appends to its cell with an atomic slot
-// counter (arrival order); pass 2 puts each cell's slots in ascending disk index (reading A13).
+// counter (arrival order); pass 2 (k_load_sort) puts each cell's slots in ascending disk index (reading A13).
 template <typename P>
 __global__ void __launch_bounds__(AUX_THREADS) k_load_bin(const __grid_constant__ Params p, const double* __restrict__ xy) {
-  using P2 = typename Real<P>::T2;
   const uint32_t i = blockIdx.x * AUX_THREADS + threadIdx.x;
   if (i >= p.N) return;
   const double X = xy[2 * (size_t)i], Y = xy[2 * (size_t)i + 1];
@@ -56,33 +55,34 @@ __global__ void __launch_bounds__(AUX_THREADS) k_load_bin(const __grid_constant_
   const uint32_t ci = (cy >> 1) * p.hx + (cx >> 1);
   const uint32_t slot = atomicAdd(&p.cnt32[Q * p.Mqp + ci], 1u);
   if (slot >= (uint32_t)NMAX) { atomicOr(&p.ctl->err, ERRBIT_OVERFLOW); return; }
-  P2 v; v.x = lx; v.y = ly;
-  pos_plane<P>(p, 0, Q, slot)[ci] = v;
-  ids_plane(p, 0, Q, slot)[ci] = i;
+  st_slot<P>(p, 0, Q, slot, ci, lx, ly);
+  st_id(p, 0, Q, slot, ci, i);
 }
 
+// Pass 2: one thread per cell sorts its <= 4 (id, position) by id and writes the cell in its final form: u8
+// count, slots ascending by id, empty slots of half 0 (and of half 1 when n > 2) = the far-away sentinel.
 template <typename P>
 __global__ void __launch_bounds__(AUX_THREADS) k_load_sort(const __grid_constant__ Params p) {
-  using P2 = typename Real<P>::T2;
+  using R = Real<P>;
+  using P2 = typename R::T2;
   const uint32_t Q = blockIdx.y;
   const uint32_t ci = blockIdx.x * AUX_THREADS + threadIdx.x;
   if (ci >= p.Mq) return;
   uint32_t n = p.cnt32[Q * p.Mqp + ci];
   if (n > (uint32_t)NMAX) n = NMAX;
   cnt_plane(p, 0, Q)[ci] = (uint8_t)n;
-  if (n < 2) return;
   uint32_t id[NMAX]; P2 v[NMAX];
 #pragma unroll
   for (int i = 0; i < NMAX; ++i) {
-    id[i] = 0xFFFFFFFFu; v[i].x = 0; v[i].y = 0;
-    if ((uint32_t)i < n) { id[i] = ids_plane(p, 0, Q, i)[ci]; v[i] = pos_plane<P>(p, 0, Q, i)[ci]; }
+    id[i] = 0xFFFFFFFFu; v[i].x = R::far_away(); v[i].y = R::far_away();
+    if ((uint32_t)i < n) { id[i] = ld_id(p, 0, Q, i, ci); v[i] = ld_slot<P>(p, 0, Q, i, ci); }
   }
 #define MPMC_CSWAP(a, b) if (id[a] > id[b]) { uint32_t ti = id[a]; id[a] = id[b]; id[b] = ti; P2 tv = v[a]; v[a] = v[b]; v[b] = tv; }
   MPMC_CSWAP(0, 1) MPMC_CSWAP(2, 3) MPMC_CSWAP(0, 2) MPMC_CSWAP(1, 3) MPMC_CSWAP(1, 2)
 #undef MPMC_CSWAP
 #pragma unroll
   for (int i = 0; i < NMAX; ++i)
-    if ((uint32_t)i < n) { ids_plane(p, 0, Q, i)[ci] = id[i]; pos_plane<P>(p, 0, Q, i)[ci] = v[i]; }
+    if (i < 2 || n > 2u) { st_id(p, 0, Q, i, ci, id[i]); st_slot<P>(p, 0, Q, i, ci, v[i].x, v[i].y); }
 }
 
 // colour-plane location of the cell (x + ox, y + oy) with periodic wrap, for arbitrary small offsets
@@ -108,7 +108,7 @@ __global__ void __launch_bounds__(AUX_THREADS) k_load_check(const __grid_constan
   const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p);
   bool bad = false;
   for (uint32_t k = 0; k < n; ++k) {
-    const P2 m = pos_plane<P>(p, 0, Q, k)[ci];
+    const P2 m = ld_slot<P>(p, 0, Q, k, ci);
     for (int oy = -1; oy <= 1; ++oy)
       for (int ox = -1; ox <= 1; ++ox) {
         uint32_t qn, cn;
@@ -117,7 +117,7 @@ __global__ void __launch_bounds__(AUX_THREADS) k_load_check(const __grid_constan
         const P sx = R::mul((P)ox, wx), sy = R::mul((P)oy, wy);
         for (uint32_t j = 0; j < nj; ++j) {
           if (ox == 0 && oy == 0 && j == k) continue;
-          const P2 v = pos_plane<P>(p, 0, qn, j)[cn];
+          const P2 v = ld_slot<P>(p, 0, qn, j, cn);
           const P Dx = R::sub(m.x, R::add(v.x, sx)), Dy = R::sub(m.y, R::add(v.y, sy));
           if (R::fma(Dx, Dx, R::mul(Dy, Dy)) < sigma2) bad = true;
         }
@@ -139,11 +139,11 @@ __global__ void __launch_bounds__(AUX_THREADS) k_unpack(const __grid_constant__ 
   const double bx = __fma_rn((double)(2u * xa + (Q & 1u)), p.wx_d, p.ctl->origin[0]);
   const double by = __fma_rn((double)(2u * ya + (Q >> 1)), p.wy_d, p.ctl->origin[1]);
   for (uint32_t i = 0; i < n; ++i) {
-    const P2 v = pos_plane<P>(p, cur, Q, i)[ci];
+    const P2 v = ld_slot<P>(p, cur, Q, i, ci);
     double X = __dadd_rn(bx, (double)v.x), Y = __dadd_rn(by, (double)v.y);
     if (X >= p.Lx_eff) X = __dsub_rn(X, p.Lx_eff);
     if (Y >= p.Ly_eff) Y = __dsub_rn(Y, p.Ly_eff);
-    const uint32_t who = ids_plane(p, cur, Q, i)[ci];
+    const uint32_t who = ld_id(p, cur, Q, i, ci);
     reinterpret_cast<double2*>(xy)[who] = make_double2(X, Y);
   }
 }
@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(AUX_THREADS) k_export(const __grid_constant__ 
   if (counts) counts[c] = n;
   for (uint32_t i = 0; i < (uint32_t)NMAX; ++i) {
     P2 v; v.x = 0; v.y = 0; uint32_t id = 0xFFFFFFFFu;
-    if (i < n) { v = pos_plane<P>(p, cur, Q, i)[ci]; id = ids_plane(p, cur, Q, i)[ci]; }
+    if (i < n) { v = ld_slot<P>(p, cur, Q, i, ci); id = ld_id(p, cur, Q, i, ci); }
     if (slab) { slab[(c * NMAX + i) * 2] = v.x; slab[(c * NMAX + i) * 2 + 1] = v.y; }
     if (ids) ids[c * NMAX + i] = id;
   }
@@ -186,16 +186,16 @@ __global__ void __launch_bounds__(AUX_THREADS) k_contact_hist(const __grid_const
     const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
     const uint32_t x = 2u * xa + (Q & 1u), y = 2u * ya + (Q >> 1);
     for (uint32_t i = 0; i < n; ++i) {
-      const P2 a = pos_plane<P>(p, cur, Q, i)[ci];
-      const uint32_t ida = ids_plane(p, cur, Q, i)[ci];
+      const P2 a = ld_slot<P>(p, cur, Q, i, ci);
+      const uint32_t ida = ld_id(p, cur, Q, i, ci);
       for (int oy = -Rc; oy <= Rc; ++oy)
         for (int ox = -Rc; ox <= Rc; ++ox) {
           uint32_t qn, cn;
           locate(p, x, y, ox, oy, qn, cn);
           const uint32_t nj = cnt_plane(p, cur, qn)[cn];
           for (uint32_t j = 0; j < nj; ++j) {
-            if (!(ida < ids_plane(p, cur, qn, j)[cn])) continue;     // each unordered pair image once
-            const P2 b = pos_plane<P>(p, cur, qn, j)[cn];
+            if (!(ida < ld_id(p, cur, qn, j, cn))) continue;     // each unordered pair image once
+            const P2 b = ld_slot<P>(p, cur, qn, j, cn);
             const double Dx = __dsub_rn(__dadd_rn((double)b.x, __dmul_rn((double)ox, p.wx_d)), (double)a.x);
             const double Dy = __dsub_rn(__dadd_rn((double)b.y, __dmul_rn((double)oy, p.wy_d)), (double)a.y);
             const double r = sqrt(__dadd_rn(__dmul_rn(Dx, Dx), __dmul_rn(Dy, Dy)));

@@ -5,16 +5,18 @@
 // squared distance) is written __fma_rn / __fmaf_rn explicitly, so results are bit-identical to a plain CPU
 // evaluation of the same formulas.
 //
-// Layout in HBM ("colour-split slot planes"): the four checkerboard sets of
+// Layout in HBM ("colour-split slot-pair planes"): the four checkerboard sets of
 // PAPER.md eq. 1 (L43) are stored as four dense sub-grids of hx x hy = (mx/2) x (my/2) cells, cell (x, y) at
 //   colour Q = 2 (y & 1) + (x & 1),   index ci = (y >> 1) * hx + (x >> 1),
-// and the n_max = 4 slots of a cell (L150, L152) are four separate planes:
-//   cnt[buf][Q][ci]            u8      number of disks n[x, y]
-//   pos[buf][Q][slot][ci]      real2   cell-local coordinates (L154), valid for slot < n
-//   ids[buf][Q][slot][ci]      u32     original disk index
-// so a warp that works on 32 consecutive active cells reads 32 consecutive real2 per slot (one or two 128-B
-// lines), its eight neighbour cells are dense rows of the three other colours, and slots beyond the occupancy
-// (2 and 3 at w ~ sigma) are never touched.  This generalises the even/odd-x split of the paper's Algorithm 3
+// and the n_max = 4 slots of a cell (L150, L152) are two planes of slot PAIRS (half h = slots 2h, 2h+1):
+//   cnt[buf][Q][ci]            u8        number of disks n[x, y]
+//   pos[buf][Q][h][ci]         real x 4  {x_a, x_b, y_a, y_b}: cell-local coordinates (L154) of slots a = 2h, b = 2h+1
+//   ids[buf][Q][h][ci]         u32 x 2   original disk indices of the two slots
+// Invariant: an EMPTY slot of half 0 holds the far-away sentinel (the paper's (-10,-10) trick, L295/L346), so
+// a neighbour cell is ONE 128-bit load (fp32) whose two register pairs are directly the operands of the packed
+// fp32x2 overlap test, with no count-dependent select.  Half 1 is valid (and sentinel-filled) only while
+// n > 2; it is never touched at w ~ sigma.  A warp that works on 32 consecutive active cells reads 512
+// contiguous bytes per neighbour cell row.  This generalises the even/odd-x split of the paper's Algorithm 3
 // (L241-258) to both axes.  buf = 0/1 is the double buffer of the cell shift (L350).
 #pragma once
 #include <cuda_runtime.h>
@@ -59,6 +61,7 @@ struct Params {
   uint32_t seed_lo, seed_hi;
   float wx_f, wy_f, sigma2_f, d_f;      // working-precision constants (fp32 mode)
   double wx_p, wy_p, sigma2_p, d_p;     // working-precision constants (fp64 mode)
+  float dsc_f; double dsc_p;            // d 2^-24 (fp32) / d 2^-32 (fp64): displacement = dsc * odd integer
   double wx_d, wy_d;                    // (double) of the working-precision widths
   double Lx_eff, Ly_eff, sigma_d;
   double Lx_user, Ly_user;              // the caller's box (input range check)
@@ -87,6 +90,11 @@ template <> struct Real<float> {
     return __fmul_rn((float)((int)(2u * (R >> 8) + 1u) - (1 << 24)), 0x1p-24f);
   }
   static __device__ __forceinline__ float unit(uint32_t R) { return __fmul_rn((float)(R >> 8), 0x1p-24f); }
+  // d * sym(R) as (d 2^-24) * integer: the same real product, so the same rounded value (host checks d 2^-24 is normal)
+  static __device__ __forceinline__ float scaled_sym(const Params& p, uint32_t R) {
+    return __fmul_rn((float)((int)(2u * (R >> 8) + 1u) - (1 << 24)), p.dsc_f);
+  }
+  static __device__ __forceinline__ float min3(float a, float b, float c) { return fminf(fminf(a, b), c); }
   static __device__ __forceinline__ float far_away() { return 1.0e18f; }   // sentinel: never overlaps
   // Two lanes at once: sm_100a packed fp32x2 instructions (FADD2 / FMUL2 / FFMA2), each lane one IEEE rn op.
   using Pair = float2;
@@ -109,6 +117,10 @@ template <> struct Real<double> {
     return __dmul_rn((double)(2ll * (long long)R + 1ll - (1ll << 32)), 0x1p-32);
   }
   static __device__ __forceinline__ double unit(uint32_t R) { return __dmul_rn((double)R, 0x1p-32); }
+  static __device__ __forceinline__ double scaled_sym(const Params& p, uint32_t R) {
+    return __dmul_rn((double)(2ll * (long long)R + 1ll - (1ll << 32)), p.dsc_p);
+  }
+  static __device__ __forceinline__ double min3(double a, double b, double c) { return fmin(fmin(a, b), c); }
   static __device__ __forceinline__ double far_away() { return 1.0e150; }
   struct Pair { double x, y; };             // no packed fp64 instruction: two scalar ops
   static __device__ __forceinline__ Pair pair(double a, double b) { Pair r; r.x = a; r.y = b; return r; }
@@ -173,24 +185,60 @@ __device__ __forceinline__ uint32_t ld_u8_early(const uint8_t* ptr) {
   asm volatile("ld.global.u8 %0, [%1];" : "=r"(v) : "l"(ptr));
   return v;
 }
-__device__ __forceinline__ float2 ld_pos_early(const float2* ptr) {
-  float2 v;
-  asm volatile("ld.global.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(ptr));
-  return v;
+
+// ---- slot-pair planes: wide accessors for the hot kernels (index i = (Q*2 + h)*Mqp + ci, in cells) ----
+template <typename P> struct Half { typename Real<P>::Pair x, y; };   // (x_a, x_b), (y_a, y_b)
+
+// `asm volatile` keeps the compiler from sinking the load into a branch that consumes it: it is issued up front
+__device__ __forceinline__ Half<float> ld_half_early(const float* pos, uint32_t i) {
+  Half<float> h;
+  asm volatile("ld.global.v4.f32 {%0, %1, %2, %3}, [%4];"
+               : "=f"(h.x.x), "=f"(h.x.y), "=f"(h.y.x), "=f"(h.y.y) : "l"(reinterpret_cast<const float4*>(pos) + i));
+  return h;
 }
-__device__ __forceinline__ double2 ld_pos_early(const double2* ptr) {
-  double2 v;
-  asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(ptr));
-  return v;
+__device__ __forceinline__ Half<double> ld_half_early(const double* pos, uint32_t i) {
+  Half<double> h;
+  const double2* q = reinterpret_cast<const double2*>(pos) + 2 * (size_t)i;
+  asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(h.x.x), "=d"(h.x.y) : "l"(q));
+  asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(h.y.x), "=d"(h.y.y) : "l"(q + 1));
+  return h;
+}
+__device__ __forceinline__ Half<float> ld_half(const float* pos, uint32_t i) {
+  const float4 v = reinterpret_cast<const float4*>(pos)[i];
+  Half<float> h; h.x.x = v.x; h.x.y = v.y; h.y.x = v.z; h.y.y = v.w; return h;
+}
+__device__ __forceinline__ Half<double> ld_half(const double* pos, uint32_t i) {
+  const double2* q = reinterpret_cast<const double2*>(pos) + 2 * (size_t)i;
+  const double2 a = q[0], b = q[1];
+  Half<double> h; h.x.x = a.x; h.x.y = a.y; h.y.x = b.x; h.y.y = b.y; return h;
+}
+__device__ __forceinline__ void st_half(float* pos, uint32_t i, const Half<float>& h) {
+  reinterpret_cast<float4*>(pos)[i] = make_float4(h.x.x, h.x.y, h.y.x, h.y.y);
+}
+__device__ __forceinline__ void st_half(double* pos, uint32_t i, const Half<double>& h) {
+  double2* q = reinterpret_cast<double2*>(pos) + 2 * (size_t)i;
+  q[0] = make_double2(h.x.x, h.x.y); q[1] = make_double2(h.y.x, h.y.y);
 }
 
-// plane addressing
-template <typename P>
-__device__ __forceinline__ typename Real<P>::T2* pos_plane(const Params& p, uint32_t buf, uint32_t Q, uint32_t slot) {
-  return reinterpret_cast<typename Real<P>::T2*>(p.pos[buf]) + (size_t)(Q * NMAX + slot) * p.Mqp;
+// ---- scalar accessors (kernels off the per-sweep path, and the rare generic paths) ----
+__device__ __forceinline__ size_t slot_index(const Params& p, uint32_t Q, uint32_t slot, uint32_t ci) {
+  return (size_t)((Q * 2u + (slot >> 1)) * p.Mqp + ci);       // in slot pairs
 }
-__device__ __forceinline__ uint32_t* ids_plane(const Params& p, uint32_t buf, uint32_t Q, uint32_t slot) {
-  return p.ids[buf] + (size_t)(Q * NMAX + slot) * p.Mqp;
+template <typename P>
+__device__ __forceinline__ typename Real<P>::T2 ld_slot(const Params& p, uint32_t buf, uint32_t Q, uint32_t slot, uint32_t ci) {
+  const P* b = reinterpret_cast<const P*>(p.pos[buf]) + (slot_index(p, Q, slot, ci) * 4 + (slot & 1u));
+  typename Real<P>::T2 v; v.x = b[0]; v.y = b[2]; return v;
+}
+template <typename P>
+__device__ __forceinline__ void st_slot(const Params& p, uint32_t buf, uint32_t Q, uint32_t slot, uint32_t ci, P x, P y) {
+  P* b = reinterpret_cast<P*>(p.pos[buf]) + (slot_index(p, Q, slot, ci) * 4 + (slot & 1u));
+  b[0] = x; b[2] = y;
+}
+__device__ __forceinline__ uint32_t ld_id(const Params& p, uint32_t buf, uint32_t Q, uint32_t slot, uint32_t ci) {
+  return p.ids[buf][slot_index(p, Q, slot, ci) * 2 + (slot & 1u)];
+}
+__device__ __forceinline__ void st_id(const Params& p, uint32_t buf, uint32_t Q, uint32_t slot, uint32_t ci, uint32_t id) {
+  p.ids[buf][slot_index(p, Q, slot, ci) * 2 + (slot & 1u)] = id;
 }
 __device__ __forceinline__ uint8_t* cnt_plane(const Params& p, uint32_t buf, uint32_t Q) {
   return p.cnt[buf] + (size_t)Q * p.Mqp;

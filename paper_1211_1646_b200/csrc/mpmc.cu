@@ -19,7 +19,7 @@ struct mpmc_ctx {
   uint64_t N;
   uint32_t flags;
   bool fp32, debug, loaded;
-  int nf;                  // register-resident neighbour slots per cell of the sub-sweep kernel (2 or 4)
+  int nf;                  // 2: w < 1.15 sigma, cells hold 0/1/2 disks -> fast sub-sweep kernel; 4: general kernel
   cudaStream_t stream;
   cudaGraphExec_t graph1;  // one sweep
   cudaGraphExec_t graphK;  // GRAPH_BATCH sweeps
@@ -108,23 +108,21 @@ int cuda_fail(cudaError_t e) {
 dim3 cell_grid(const mpmc_ctx* c, int threads) { return dim3((c->p.Mq + threads - 1) / threads, 4, 1); }
 
 // ---- kernel launchers ----------------------------------------------------------------------------------
-template <typename P, int NF, bool DEBUG>
-void launch_sub_ns(const mpmc_ctx* c, uint32_t setk) {
+// fast = the w ~ sigma kernel (occupancy 0/1/2, compile-time n_s in {4, 8}); otherwise the general kernel
+template <typename P, bool DEBUG>
+void launch_sub_t(const mpmc_ctx* c, uint32_t setk) {
   const dim3 grid((c->p.Mq + SUB_THREADS - 1) / SUB_THREADS);
-  switch (c->p.n_s) {      // n_s = 4 and 8 (the BASELINE configs) are compile-time instantiations
-    case 4: k_sub_sweep<P, NF, 4, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); break;
-    case 8: k_sub_sweep<P, NF, 8, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); break;
-    default: k_sub_sweep<P, NF, 0, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); break;
+  if (c->nf == 2 && c->p.n_s == 4) { k_sub_fast<P, 4, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); return; }
+  if (c->nf == 2 && c->p.n_s == 8) { k_sub_fast<P, 8, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); return; }
+  switch (c->p.n_s) {      // n_s = 4 and 8 are compile-time instantiations
+    case 4: k_sub_sweep<P, 4, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); break;
+    case 8: k_sub_sweep<P, 8, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); break;
+    default: k_sub_sweep<P, 0, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); break;
   }
 }
-template <typename P, bool DEBUG>
-void launch_sub_nf(const mpmc_ctx* c, uint32_t setk) {
-  if (c->nf == 2) launch_sub_ns<P, 2, DEBUG>(c, setk);
-  else            launch_sub_ns<P, 4, DEBUG>(c, setk);
-}
 void launch_sub(const mpmc_ctx* c, uint32_t setk) {
-  if (c->fp32) { if (c->debug) launch_sub_nf<float, true>(c, setk); else launch_sub_nf<float, false>(c, setk); }
-  else         { if (c->debug) launch_sub_nf<double, true>(c, setk); else launch_sub_nf<double, false>(c, setk); }
+  if (c->fp32) { if (c->debug) launch_sub_t<float, true>(c, setk); else launch_sub_t<float, false>(c, setk); }
+  else         { if (c->debug) launch_sub_t<double, true>(c, setk); else launch_sub_t<double, false>(c, setk); }
 }
 void launch_shift(const mpmc_ctx* c, uint32_t ovr, uint32_t dir, double delta) {
   const dim3 grid = cell_grid(c, SHIFT_THREADS);
@@ -215,6 +213,8 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   Geom g;
   const int st = geometry(box, sigma, w_target, fp32, &g);
   if (st != MPMC_OK) return st;
+  // displacement = (d 2^-k) * odd integer must equal d * (integer 2^-k): the scaled d has to be a normal number
+  if (fp32 ? !((float)d * 0x1p-24f >= 1.17549435e-38f) : !(d * 0x1p-32 >= 2.2250738585072014e-308)) return MPMC_ERR_ARG;
   const Layout L = layout(g, fp32, debug);
   if (!workspace || ((uintptr_t)workspace % ALIGN) != 0 || workspace_bytes < L.total) return MPMC_ERR_WORKSPACE;
   int ndev = 0;
@@ -232,6 +232,7 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   p.seed_lo = (uint32_t)seed; p.seed_hi = (uint32_t)(seed >> 32);
   p.wx_f = (float)g.w0[0]; p.wy_f = (float)g.w0[1];
   p.sigma2_f = (float)sigma * (float)sigma; p.d_f = (float)d;
+  p.dsc_f = p.d_f * 0x1p-24f; p.dsc_p = d * 0x1p-32;
   p.wx_p = g.w0[0]; p.wy_p = g.w0[1]; p.sigma2_p = sigma * sigma; p.d_p = d;
   p.wx_d = g.wp[0]; p.wy_d = g.wp[1];
   p.Lx_eff = (double)g.m[0] * g.wp[0]; p.Ly_eff = (double)g.m[1] * g.wp[1];
@@ -247,8 +248,8 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
     p.ids[b] = (uint32_t*)(base + L.off_ids[b]);
   }
   p.mask = debug ? (uint32_t*)(base + L.off_mask) : nullptr;
-  // NF = 2 register slots per neighbour while at most 2 disks fit a cell most of the time (w < ~1.15 sigma);
-  // NF = 4 in the paper's regime (w up to sqrt(2) sigma, L152).
+  // fast kernel while at most 2 disks fit a cell nearly always (w < ~1.15 sigma; rarer cells take its generic
+  // path); general kernel in the paper's regime (w up to sqrt(2) sigma, L152).
   const double wmax = g.wp[0] > g.wp[1] ? g.wp[0] : g.wp[1];
   c->nf = (wmax < 1.15 * sigma) ? 2 : 4;
   *out = c;

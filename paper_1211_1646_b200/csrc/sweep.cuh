@@ -1,5 +1,5 @@
-// sweep.cuh — the two hot kernels: the active-cell sub-sweep (Algorithm 2) and the cell
-// shift / re-bin (Algorithm 4), re-designed for sm_100a.  See DESIGN.md "Kernels".
+// sweep.cuh — the hot kernels: the active-cell sub-sweep (Algorithm 2) in two forms and the
+// cell shift / re-bin (Algorithm 4), re-designed for sm_100a.  See DESIGN.md "Kernels".
 #pragma once
 #include "common.cuh"
 
@@ -11,261 +11,120 @@ namespace mpmc {
 #ifndef MPMC_SUB_MINB
 #define MPMC_SUB_MINB 1
 #endif
+#ifndef MPMC_FAST_MINB
+#define MPMC_FAST_MINB 6
+#endif
 constexpr int SUB_THREADS = MPMC_SUB_THREADS;
 constexpr int SUB_MINB = MPMC_SUB_MINB;      // minimum resident blocks per SM asked of ptxas (register cap)
+constexpr int FAST_MINB = MPMC_FAST_MINB;
 constexpr int SHIFT_THREADS = 256;
 
 // ---------------------------------------------------------------------------------------------------------
-// Sub-sweep kernel.  One thread per cell of the active checkerboard set (the paper's mapping, L158/L260),
-// over the dense colour plane so that a warp's 32 cells are contiguous.
-//
-//  * the cell's own <= 4 disks and the first NF disks of each of the 8 neighbour cells are loaded ONCE into
-//    registers, neighbours already translated into the active cell's frame (q = l_j + s, L154/L196), and are
-//    reused by all n_s moves; empty entries hold a far-away sentinel so the overlap loop has a fixed trip
-//    count and no divergence (the paper's (-10,-10) trick, L295/L346);
-//  * entries are kept NEGATED and in pairs, so that one overlap test of two disks is four packed fp32x2
-//    instructions of sm_100a (FADD2, FADD2, FMUL2, FFMA2: D = M + (-q), r^2 = fma(Dx, Dx, Dy*Dy)) and two
-//    compares; every lane of a packed instruction is one IEEE rn operation, so results are unchanged
-//    (-(a+b) = (-a)+(-b) exactly under round-to-nearest-even).  fp64 uses the same code with scalar pairs;
-//  * NF = 2 covers every neighbour at w ~ sigma except a rare few (occupancy 0/1/2); neighbours with more
-//    than NF disks set a bit in `big` and their remaining slots are re-read from L1/L2 inside the move loop;
-//    NF = 4 is the instantiation for the paper's own regime w ~ 1.4 sigma (L152);
-//  * Philox4x32-10 keyed on (seed; cell, sweep, move) replaces the per-thread Saru stream (L180, L262);
-//  * accept/reject is computed without early exit: all lanes run the same instruction stream.
-//  * NS > 0 fixes n_s at compile time (4 and 8, the BASELINE configs): the n_s Philox calls, which depend
-//    only on (seed, sweep, cell, s), are issued up front and interleaved (4-8 independent dependency chains
-//    instead of one), and the move loop is fully unrolled; NS = 0 is the generic run-time loop;
-// SETK: index into Ctl::order (0..3) or, for the test hook, 4 + explicit set.
+// Where an active cell and its 3x3 neighbourhood live in the colour planes (periodic wrap).
 // ---------------------------------------------------------------------------------------------------------
-template <typename P, int NF, int NS, bool DEBUG>
-__global__ void __launch_bounds__(SUB_THREADS, SUB_MINB)
-k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
+struct Where {
+  uint32_t Q, offx, offy, ci, cell;
+  uint32_t xl, xa, xr, rowd, rowa, rowu;
+  bool valid;
+};
+__device__ __forceinline__ Where locate_active(const Params& p, const uint32_t Q, const uint32_t ci_raw) {
+  Where w;
+  w.Q = Q; w.offx = Q & 1u; w.offy = Q >> 1;
+  w.valid = ci_raw < p.Mq;
+  w.ci = w.valid ? ci_raw : p.Mq - 1u;             // clamped: every lane may prefetch
+  const uint32_t ya = div_hx(p, w.ci);
+  w.xa = w.ci - ya * p.hx;
+  w.cell = (2u * ya + w.offy) * p.mx + (2u * w.xa + w.offx);        // canonical cell id y*mx + x
+  w.xl = w.offx ? w.xa : (w.xa == 0 ? p.hx - 1 : w.xa - 1);          // plane column of cell x-1
+  w.xr = w.offx ? (w.xa + 1 == p.hx ? 0 : w.xa + 1) : w.xa;          // ... of cell x+1
+  const uint32_t yd = w.offy ? ya : (ya == 0 ? p.hy - 1 : ya - 1);
+  const uint32_t yu = w.offy ? (ya + 1 == p.hy ? 0 : ya + 1) : ya;
+  w.rowd = yd * p.hx; w.rowa = ya * p.hx; w.rowu = yu * p.hx;
+  return w;
+}
+// colour and in-plane index of the neighbour at offset (ox, oy), ox, oy in {-1, 0, 1}
+__device__ __forceinline__ void neighbour(const Where& w, int ox, int oy, uint32_t& qn, uint32_t& cn) {
+  qn = ((w.offy ^ (uint32_t)(oy & 1)) << 1) | (w.offx ^ (uint32_t)(ox & 1));
+  cn = (oy < 0 ? w.rowd : oy > 0 ? w.rowu : w.rowa) + (ox < 0 ? w.xl : ox > 0 ? w.xr : w.xa);
+}
+
+// Fisher-Yates of the cell's n disks (Alg. 2 line 9, L187) as a visiting permutation packed in nibbles
+__device__ __forceinline__ uint32_t visiting_permutation(const uint32_t n, const uint32_t (&S)[4]) {
+  uint32_t perm = 0x3210u;
+#pragma unroll
+  for (int step = 0; step < NMAX - 1; ++step) {
+    if ((uint32_t)step + 1u < n) {
+      const uint32_t i = n - 1u - (uint32_t)step;
+      const uint32_t j = bounded(S[step], i + 1u);
+      const uint32_t a = (perm >> (4u * i)) & 15u, b = (perm >> (4u * j)) & 15u;
+      const uint32_t x = a ^ b;
+      perm ^= (x << (4u * i)) ^ (x << (4u * j));
+    }
+  }
+  return perm;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Generic cell update: Algorithm 2 line by line on the slots in global memory, any occupancy up to n_max.
+// Used by the fast kernel for the rare cells whose 3x3 neighbourhood holds a cell with more than 2 disks.
+// Deliberately compact (rolled loops, scalar arithmetic): it runs for a handful of lanes.
+// ---------------------------------------------------------------------------------------------------------
+template <typename P>
+__device__ __forceinline__ void cell_update_generic(const Params& p, const Where& w, const uint8_t* cntb, P* posb,
+                                                    const uint32_t n, const uint32_t n_s, const uint32_t t_lo,
+                                                    const uint32_t t_hi, uint32_t& n_acc, uint32_t& n_rb,
+                                                    uint32_t& n_ro, uint32_t& amask) {
   using R = Real<P>;
-  using P2 = typename R::T2;
-  using Pair = typename R::Pair;
-  constexpr int NPN = 8 * NF / 2;        // neighbour pairs
-  const Ctl* __restrict__ ctl = p.ctl;
-  const uint32_t Q = setk < 4 ? ctl->order[setk] : (setk & 3u);
-  const unsigned long long t = ctl->t;
-  const uint32_t cur = ctl->cur;
-  const uint32_t offx = Q & 1u, offy = Q >> 1;
-  const uint32_t ci_raw = blockIdx.x * SUB_THREADS + threadIdx.x;
-  const bool valid = ci_raw < p.Mq;
-  const uint32_t ci = valid ? ci_raw : p.Mq - 1u;      // clamped: every lane may prefetch
-  const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
-
-  // base pointers of the current buffer; planes are addressed with 32-bit element indices
-  const uint8_t* __restrict__ cntb = p.cnt[cur];
-  P2* __restrict__ posb = reinterpret_cast<P2*>(p.pos[cur]);
   const uint32_t Mqp = p.Mqp;
-
-  // ---- cell and neighbour indices in the colour planes, with periodic wrap ----
-  const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
-  const uint32_t cell = (2u * ya + offy) * p.mx + (2u * xa + offx);   // canonical cell id y*mx + x
-  const uint32_t xl = offx ? xa : (xa == 0 ? p.hx - 1 : xa - 1);        // plane column of cell x-1
-  const uint32_t xr = offx ? (xa + 1 == p.hx ? 0 : xa + 1) : xa;        // ... of cell x+1
-  const uint32_t yd = offy ? ya : (ya == 0 ? p.hy - 1 : ya - 1);
-  const uint32_t yu = offy ? (ya + 1 == p.hy ? 0 : ya + 1) : ya;
-  const uint32_t rowd = yd * p.hx, rowa = ya * p.hx, rowu = yu * p.hx;
-
-  // ---- level-1 loads, all independent: count and slot 0 of the 3x3 cells (idx 4 = own cell) ----
-  uint32_t cidx[9], cj[9];
-  P2 v0[9];
-#pragma unroll
-  for (int idx = 0; idx < 9; ++idx) {
-    const int ox = idx % 3 - 1, oy = idx / 3 - 1;
-    const uint32_t qn = ((offy ^ (uint32_t)(oy & 1)) << 1) | (offx ^ (uint32_t)(ox & 1));
-    const uint32_t cn = (oy < 0 ? rowd : oy > 0 ? rowu : rowa) + (ox < 0 ? xl : ox > 0 ? xr : xa);
-    cidx[idx] = qn * Mqp + cn;                       // count index; slot s of the cell is at 4*qn*Mqp + s*Mqp + cn
-    cj[idx] = ld_u8_early(cntb + cidx[idx]);
-    v0[idx] = ld_pos_early(posb + (cidx[idx] + 3u * qn * Mqp));
+  const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p), dmax = R::d(p);
+  uint32_t perm = 0x3210u;
+  if (n >= 2u) {
+    uint32_t S[4];
+    philox4x32_10(w.cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
+    perm = visiting_permutation(n, S);
   }
-
-  // ---- arithmetic that needs no memory, issued while the loads are in flight: the Philox words of the
-  //      shuffle (Alg. 2 line 9) and of the first half of the displacements (line 12, L190; A2, A9) ----
-  const P dmax = R::d(p);
-  // Philox block q serves moves 2q (words 0, 1) and 2q + 1 (words 2, 3)  (reading A9)
-  auto displacement2 = [&](uint32_t q, P& ax, P& ay, P& bx, P& by) {
-    uint32_t Rw[4];
-    philox4x32_10(cell, t_lo, t_hi, q, p.seed_lo, p.seed_hi, Rw);
-    ax = R::mul(dmax, R::sym(Rw[0])); ay = R::mul(dmax, R::sym(Rw[1]));
-    bx = R::mul(dmax, R::sym(Rw[2])); by = R::mul(dmax, R::sym(Rw[3]));
-  };
-  uint32_t S[4];
-  philox4x32_10(cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
-  static_assert(NS % 4 == 0, "compile-time n_s must be a multiple of 4");
-  constexpr int NSA = NS > 0 ? NS : 2;
-  P ddx[NSA], ddy[NSA];
-  if (NS > 0) {
-#pragma unroll
-    for (int q = 0; q < NS / 4; ++q) displacement2((uint32_t)q, ddx[2 * q], ddy[2 * q], ddx[2 * q + 1], ddy[2 * q + 1]);
-  }
-
-  uint32_t n_acc = 0, n_rb = 0, n_ro = 0;
-  // Empty cells (and the clamped lanes past the end) run the same instruction stream on sentinels and are
-  // masked out of the counters and the write-back: no lane-dependent branch stands between the loads above
-  // and their first use, so the loads are issued before the Philox arithmetic and overlap it.  (Skipping an
-  // empty cell saves nothing unless all 32 cells of a warp are empty; Alg. 2 lines 4-7, L181-185.)
-  if (!valid) cj[4] = 0u;
-  const uint32_t n = cj[4];
-  const uint32_t nv = n > 0u ? n : 1u;                 // visiting modulus; an empty cell "visits" a sentinel
-
-  {
-    const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p);
-    const P FAR = R::far_away();
-    const Pair MINUS1 = R::pair((P)-1, (P)-1);
-
-    // ---- level-2 loads: the occupied higher slots (rare at w ~ sigma) ----
-    P2 v1[9], v2[9], v3[9];
-    uint32_t big = 0;          // bit idx set: neighbour idx holds more than NF disks
-#pragma unroll
-    for (int idx = 0; idx < 9; ++idx) {
-      const int ox = idx % 3 - 1, oy = idx / 3 - 1;
-      const uint32_t qn = ((offy ^ (uint32_t)(oy & 1)) << 1) | (offx ^ (uint32_t)(ox & 1));
-      const uint32_t s0 = cidx[idx] + 3u * qn * Mqp;
-      v1[idx].x = FAR; v1[idx].y = FAR; v2[idx] = v1[idx]; v3[idx] = v1[idx];
-      if (cj[idx] > 1u) v1[idx] = posb[s0 + Mqp];
-      if (idx == 4 || NF == 4) {
-        if (cj[idx] > 2u) v2[idx] = posb[s0 + 2u * Mqp];
-        if (cj[idx] > 3u) v3[idx] = posb[s0 + 3u * Mqp];
-      } else if (cj[idx] > (uint32_t)NF) {
-        big |= 1u << idx;
-      }
-      if (cj[idx] == 0u) { v0[idx].x = FAR; v0[idx].y = FAR; }
-    }
-    if (NS > 0) {
-#pragma unroll
-      for (int q = NS / 4; q < NS / 2; ++q) displacement2((uint32_t)q, ddx[2 * q], ddy[2 * q], ddx[2 * q + 1], ddy[2 * q + 1]);
-    }
-
-    // ---- own cell (Alg. 2 line 8, L186), negated, as pairs (slot 0,1) and (slot 2,3) ----
-    Pair nox[2], noy[2];
-    nox[0] = R::pair(-v0[4].x, -v1[4].x); nox[1] = R::pair(-v2[4].x, -v3[4].x);
-    noy[0] = R::pair(-v0[4].y, -v1[4].y); noy[1] = R::pair(-v2[4].y, -v3[4].y);
-
-    // ---- neighbours, translated into this cell's frame (s = (ox wx, oy wy), L154, L196), negated:
-    //      -(l_j + s) = fma(l_j, -1, -s), one rn operation ----
-    Pair nqx[NPN], nqy[NPN];
-#pragma unroll
-    for (int idx = 0; idx < 9; ++idx) {
-      if (idx == 4) continue;
-      const int e = idx < 4 ? idx : idx - 1;
-      const int ox = idx % 3 - 1, oy = idx / 3 - 1;
-      const P nsx = ox < 0 ? wx : ox > 0 ? -wx : (P)0;
-      const P nsy = oy < 0 ? wy : oy > 0 ? -wy : (P)0;
-      nqx[e * (NF / 2)] = R::pfma(R::pair(v0[idx].x, v1[idx].x), MINUS1, R::pair(nsx, nsx));
-      nqy[e * (NF / 2)] = R::pfma(R::pair(v0[idx].y, v1[idx].y), MINUS1, R::pair(nsy, nsy));
-      if (NF == 4) {
-        nqx[e * (NF / 2) + NF / 2 - 1] = R::pfma(R::pair(v2[idx].x, v3[idx].x), MINUS1, R::pair(nsx, nsx));
-        nqy[e * (NF / 2) + NF / 2 - 1] = R::pfma(R::pair(v2[idx].y, v3[idx].y), MINUS1, R::pair(nsy, nsy));
-      }
-    }
-
-    // ---- shuffle (Alg. 2 line 9, L187), kept as a visiting permutation packed in nibbles ----
-    uint32_t perm = 0x3210u;
-#pragma unroll
-    for (int step = 0; step < NMAX - 1; ++step) {
-      if ((uint32_t)step + 1u < n) {
-        const uint32_t i = n - 1u - (uint32_t)step;
-        const uint32_t j = bounded(S[step], i + 1u);
-        const uint32_t a = (perm >> (4u * i)) & 15u, b = (perm >> (4u * j)) & 15u;
-        const uint32_t x = a ^ b;
-        perm ^= (x << (4u * i)) ^ (x << (4u * j));
-      }
-    }
-
-    // ---- n_s trial moves (Alg. 2 lines 11-32, L189-230) ----
-    uint32_t amask = 0, vi = 0;
-    auto trial_move = [&](const uint32_t s, const P dx, const P dy) {
-      const uint32_t k = (perm >> (4u * vi)) & 3u;               // p <- particles[s mod n]  (L75)
-      vi = (vi + 1u == nv) ? 0u : vi + 1u;                       // lines 28-32 (L224-230)
-      const P nlx = k == 0 ? nox[0].x : k == 1 ? nox[0].y : k == 2 ? nox[1].x : nox[1].y;
-      const P nly = k == 0 ? noy[0].x : k == 1 ? noy[0].y : k == 2 ? noy[1].x : noy[1].y;
-      const P Mx = R::sub(dx, nlx);                              // D_move = l + displacement
-      const P My = R::sub(dy, nly);
-      const bool inside = (Mx > (P)0) && (Mx <= wx) && (My > (P)0) && (My <= wy);   // (0, w]  (A3)
-      const Pair MMx = R::pair(Mx, Mx), MMy = R::pair(My, My);
-      bool ov = false;
-      // the other disks of the own cell (line 17 skips i = j, L201); s = 0 so q = l_j
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        const Pair Dx = R::padd(MMx, nox[h]), Dy = R::padd(MMy, noy[h]);
-        const Pair r2 = R::pfma(Dx, Dx, R::pmul(Dy, Dy));
-        ov |= (r2.x < sigma2) && ((uint32_t)(2 * h) != k);
-        ov |= (r2.y < sigma2) && ((uint32_t)(2 * h + 1) != k);
-      }
-      // neighbour disks held in registers: |D_move - (D + s)|^2 < sigma^2 (line 19, L204)
-#pragma unroll
-      for (int e = 0; e < NPN; ++e) {
-        const Pair Dx = R::padd(MMx, nqx[e]), Dy = R::padd(MMy, nqy[e]);
-        const Pair r2 = R::pfma(Dx, Dx, R::pmul(Dy, Dy));
-        ov |= (r2.x < sigma2) || (r2.y < sigma2);
-      }
-      if (NF < NMAX && big != 0 && inside && !ov) {              // rare: neighbours with more than NF disks
+  const uint32_t own = 2u * w.Q * Mqp + w.ci;           // half-0 index of the own cell
+  uint32_t vi = 0;
+  uint32_t Rw[4] = {0, 0, 0, 0};
 #pragma unroll 1
-        for (int idx = 0; idx < 9; ++idx) {
-          if (!((big >> idx) & 1u)) continue;
-          const int ox = idx % 3 - 1, oy = idx / 3 - 1;
-          const uint32_t qn = ((offy ^ (uint32_t)(oy & 1)) << 1) | (offx ^ (uint32_t)(ox & 1));
-          const uint32_t cn = (oy < 0 ? rowd : oy > 0 ? rowu : rowa) + (ox < 0 ? xl : ox > 0 ? xr : xa);
-          const uint32_t nj = cntb[qn * Mqp + cn];
-          const P sx = ox < 0 ? -wx : ox > 0 ? wx : (P)0;
-          const P sy = oy < 0 ? -wy : oy > 0 ? wy : (P)0;
-          for (uint32_t i = NF; i < nj; ++i) {
-            const P2 v = posb[(qn * NMAX + i) * Mqp + cn];
-            const P Dx = R::sub(Mx, R::add(v.x, sx)), Dy = R::sub(My, R::add(v.y, sy));
-            const P r2 = R::fma(Dx, Dx, R::mul(Dy, Dy));
-            ov |= r2 < sigma2;
-          }
-        }
-      }
-      if (!inside) {
-        ++n_rb;                                                  // leaves the cell: rejected (L79, L118)
-      } else if (ov) {
-        ++n_ro;
-      } else {                                                   // lines 24-27 (L215-222)
-        ++n_acc;
-        amask |= 1u << (s & 31u);
-        const P nMx = -Mx, nMy = -My;
-        if (k == 0) { nox[0].x = nMx; noy[0].x = nMy; }
-        if (k == 1) { nox[0].y = nMx; noy[0].y = nMy; }
-        if (k == 2) { nox[1].x = nMx; noy[1].x = nMy; }
-        if (k == 3) { nox[1].y = nMx; noy[1].y = nMy; }
-      }
-    };
-    if (NS > 0) {
-#pragma unroll
-      for (int s = 0; s < NS; ++s) trial_move((uint32_t)s, ddx[s], ddy[s]);
-    } else {
-      for (uint32_t s = 0; s < p.n_s; s += 2) {
-        displacement2(s >> 1, ddx[0], ddy[0], ddx[1], ddy[1]);
-        trial_move(s, ddx[0], ddy[0]);
-        if (s + 1 < p.n_s) trial_move(s + 1, ddx[1], ddy[1]);
+  for (uint32_t s = 0; s < n_s; ++s) {
+    if ((s & 1u) == 0u) philox4x32_10(w.cell, t_lo, t_hi, s >> 1, p.seed_lo, p.seed_hi, Rw);
+    const uint32_t k = (perm >> (4u * vi)) & 3u;                 // p <- particles[s mod n]  (L75)
+    vi = (vi + 1u == n) ? 0u : vi + 1u;                          // lines 28-32 (L224-230)
+    const uint32_t r0 = (s & 1u) ? Rw[2] : Rw[0], r1 = (s & 1u) ? Rw[3] : Rw[1];
+    P* slot_k = posb + ((size_t)(own + (k >> 1) * Mqp) * 4 + (k & 1u));
+    const P Mx = R::add(slot_k[0], R::mul(dmax, R::sym(r0)));    // D_move = l + displacement (line 12, L190)
+    const P My = R::add(slot_k[2], R::mul(dmax, R::sym(r1)));
+    if (!((Mx > (P)0) && (Mx <= wx) && (My > (P)0) && (My <= wy))) { ++n_rb; continue; }   // (0, w]  (A3; L79)
+    bool ov = false;
+#pragma unroll 1
+    for (int idx = 0; idx < 9; ++idx) {
+      const int ox = idx % 3 - 1, oy = idx / 3 - 1;
+      uint32_t qn, cn;
+      neighbour(w, ox, oy, qn, cn);
+      const uint32_t nj = cntb[qn * Mqp + cn];
+      const P sx = ox < 0 ? -wx : ox > 0 ? wx : (P)0;            // s = (ox wx, oy wy)  (L154, L196)
+      const P sy = oy < 0 ? -wy : oy > 0 ? wy : (P)0;
+      for (uint32_t j = 0; j < nj; ++j) {
+        if (idx == 4 && j == k) continue;                        // line 17 (L201)
+        const P* sj = posb + ((size_t)(2u * qn * Mqp + (j >> 1) * Mqp + cn) * 4 + (j & 1u));
+        const P Dx = R::sub(Mx, R::add(sj[0], sx)), Dy = R::sub(My, R::add(sj[2], sy));
+        ov |= R::fma(Dx, Dx, R::mul(Dy, Dy)) < sigma2;           // line 19 (L204), strict (A4)
       }
     }
-
-    // ---- write back (line 34, L234) ----
-    if (amask != 0) {
-      const P vx[NMAX] = {nox[0].x, nox[0].y, nox[1].x, nox[1].y};
-      const P vy[NMAX] = {noy[0].x, noy[0].y, noy[1].x, noy[1].y};
-#pragma unroll
-      for (int i = 0; i < NMAX; ++i)
-        if ((uint32_t)i < n) { P2 v; v.x = -vx[i]; v.y = -vy[i]; posb[(Q * NMAX + i) * Mqp + ci] = v; }
-    }
-    if (DEBUG && valid) {
-      p.mask[cell] = amask;
-      if (n > 0u) atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)cell << 32) | amask)));
-    }
+    if (ov) { ++n_ro; }
+    else { ++n_acc; amask |= 1u << (s & 31u); slot_k[0] = Mx; slot_k[2] = My; }   // lines 24-27 (L215-222)
   }
-  if (n == 0u) n_rb = 0u;        // a sentinel never passes the in-cell test; empty cells attempt nothing (A10)
+}
 
-  // ---- counters: warp reduce, then three fire-and-forget 64-bit reductions per warp into one of CTR_SLOTS
-  //      counter rows (spread so that same-address atomics do not serialise); no block barrier ----
+// counters: warp reduce, then three fire-and-forget 64-bit reductions per warp into one of CTR_SLOTS counter
+// rows (spread so that same-address atomics do not serialise); no block barrier
+__device__ __forceinline__ void add_counters(const Params& p, uint32_t n_acc, uint32_t n_rb, uint32_t n_ro) {
   n_acc = __reduce_add_sync(0xFFFFFFFFu, n_acc);
   n_rb = __reduce_add_sync(0xFFFFFFFFu, n_rb);
   n_ro = __reduce_add_sync(0xFFFFFFFFu, n_ro);
   if ((threadIdx.x & 31) == 0) {
-    unsigned long long* row = p.ctl->counters[(blockIdx.x * (SUB_THREADS / 32) + (threadIdx.x >> 5)) % CTR_SLOTS];
+    unsigned long long* row = p.ctl->counters[(blockIdx.x * (blockDim.x / 32) + (threadIdx.x >> 5)) % CTR_SLOTS];
     if (n_acc) atomicAdd(&row[0], (unsigned long long)n_acc);
     if (n_rb) atomicAdd(&row[1], (unsigned long long)n_rb);
     if (n_ro) atomicAdd(&row[2], (unsigned long long)n_ro);
@@ -273,29 +132,330 @@ k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// Fast sub-sweep kernel for cell widths w ~ sigma (the BASELINE configs: occupancy 0/1/2 per cell).
+// One thread per cell of the active checkerboard set (the paper's mapping, L158/L260) over the dense colour
+// plane, so a warp's 32 cells are contiguous.
+//
+//  * each of the 3x3 cells is ONE load of its slot pair {x0, x1, y0, y1} (128 bit in fp32), issued up front and
+//    unconditionally; empty slots hold the far-away sentinel (the paper's (-10,-10) trick, L295/L346), so the
+//    two register pairs of a neighbour are, after one packed fma that translates them into this cell's frame and
+//    negates them (-(l_j + s), s = (ox wx, oy wy), L154/L196), directly the operands of the packed fp32x2
+//    overlap test (FADD2, FADD2, FMUL2, FFMA2: D = M + (-q), r^2 = fma(Dx, Dx, Dy*Dy)); every lane of a packed
+//    instruction is one IEEE rn operation and -(a+b) = (-a)+(-b) exactly, so results are those of the scalar
+//    formula.  No count-dependent select, no branch, no divergence: the verdict of a move is min r^2 < sigma^2;
+//  * the two own disks are kept in VISITING order (A = the disk the next move acts on, B = the other one or the
+//    sentinel): the shuffle (Alg. 2 line 9, L187) swaps them once up front, and after every move they swap iff
+//    n = 2 (the s mod n cycling, L75, L224-230) — no dynamic slot index anywhere;
+//  * Philox4x32-10 keyed on (seed; cell, sweep, block) replaces the per-thread Saru stream (L180, L262); the
+//    NS/2 blocks depend on nothing loaded and are computed while the loads are in flight; d*u is evaluated as
+//    (d 2^-24) * integer, the same real product, hence the same rounding;
+//  * the rare cell with more than 2 disks in its 3x3 neighbourhood takes cell_update_generic (lane-divergent).
+// SETK: index into Ctl::order (0..3) or, for the test hook, 4 + explicit set.
+// ---------------------------------------------------------------------------------------------------------
+template <typename P, int NS, bool DEBUG>
+__global__ void __launch_bounds__(SUB_THREADS, sizeof(P) == 4 ? FAST_MINB : FAST_MINB / 2)
+k_sub_fast(const __grid_constant__ Params p, const uint32_t setk) {
+  using R = Real<P>;
+  using Pair = typename R::Pair;
+  static_assert(NS > 0 && NS % 2 == 0, "compile-time n_s must be even");
+  const Ctl* __restrict__ ctl = p.ctl;
+  const uint32_t Q = setk < 4 ? ctl->order[setk] : (setk & 3u);
+  const unsigned long long t = ctl->t;
+  const uint32_t cur = ctl->cur;
+  const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
+  const Where w = locate_active(p, Q, blockIdx.x * SUB_THREADS + threadIdx.x);
+  const uint8_t* cntb = p.cnt[cur];
+  P* posb = reinterpret_cast<P*>(p.pos[cur]);
+  const uint32_t Mqp = p.Mqp;
+
+  // ---- all loads, independent and unconditional: count and slot pair 0 of the 3x3 cells (idx 4 = own) ----
+  uint32_t cj[9];
+  Half<P> h[9];
+#pragma unroll
+  for (int idx = 0; idx < 9; ++idx) {
+    uint32_t qn, cn;
+    neighbour(w, idx % 3 - 1, idx / 3 - 1, qn, cn);
+    cj[idx] = ld_u8_early(cntb + (qn * Mqp + cn));
+    h[idx] = ld_half_early(posb, 2u * qn * Mqp + cn);
+  }
+
+  // ---- arithmetic that needs no memory: the displacements of all NS moves (line 12, L190; A2, A9) ----
+  P ddx[NS], ddy[NS];
+#pragma unroll
+  for (int q = 0; q < NS / 2; ++q) {
+    uint32_t Rw[4];
+    philox4x32_10(w.cell, t_lo, t_hi, (uint32_t)q, p.seed_lo, p.seed_hi, Rw);
+    ddx[2 * q] = R::scaled_sym(p, Rw[0]); ddy[2 * q] = R::scaled_sym(p, Rw[1]);
+    ddx[2 * q + 1] = R::scaled_sym(p, Rw[2]); ddy[2 * q + 1] = R::scaled_sym(p, Rw[3]);
+  }
+
+  uint32_t n_acc = 0, n_rb = 0, n_ro = 0, amask = 0;
+  const uint32_t n = w.valid ? cj[4] : 0u;
+  // largest count in the neighbourhood: above 2 the slot pair does not hold the whole cell
+  uint32_t cmax = cj[0];
+#pragma unroll
+  for (int idx = 1; idx < 9; ++idx) cmax = max(cmax, cj[idx]);
+
+  if (cmax > 2u) {
+    if (n > 0u) cell_update_generic<P>(p, w, cntb, posb, n, (uint32_t)NS, t_lo, t_hi, n_acc, n_rb, n_ro, amask);
+  } else {
+    const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p);
+    const Pair MINUS1 = R::pair((P)-1, (P)-1);
+    // ---- neighbours, translated into this cell's frame and negated: -(l_j + s) = fma(l_j, -1, -s) ----
+    Pair nqx[8], nqy[8];
+#pragma unroll
+    for (int idx = 0; idx < 9; ++idx) {
+      if (idx == 4) continue;
+      const int e = idx < 4 ? idx : idx - 1;
+      const int ox = idx % 3 - 1, oy = idx / 3 - 1;
+      const P nsx = ox < 0 ? wx : ox > 0 ? -wx : (P)0;
+      const P nsy = oy < 0 ? wy : oy > 0 ? -wy : (P)0;
+      nqx[e] = R::pfma(h[idx].x, MINUS1, R::pair(nsx, nsx));
+      nqy[e] = R::pfma(h[idx].y, MINUS1, R::pair(nsy, nsy));
+    }
+    // ---- own cell in visiting order (Alg. 2 lines 8-9, L186-187) ----
+    P Ax = h[4].x.x, Ay = h[4].y.x, Bx = h[4].x.y, By = h[4].y.y;
+    const bool two = n == 2u;
+    bool flip = false;                   // true: A is slot 1
+    if (two) {                           // n = 2: Fisher-Yates is one draw, j = bounded(S0, 2); j = 0 swaps
+      uint32_t S[4];
+      philox4x32_10(w.cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
+      flip = bounded(S[0], 2u) == 0u;
+    }
+    if (flip) { P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }
+
+    // ---- NS trial moves (Alg. 2 lines 11-32, L189-230) ----
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+      const P Mx = R::add(Ax, ddx[s]), My = R::add(Ay, ddy[s]);              // D_move = l + displacement
+      const bool inside = (Mx > (P)0) && (Mx <= wx) && (My > (P)0) && (My <= wy);   // (0, w]  (A3; L79, L118)
+      const P Dbx = R::sub(Mx, Bx), Dby = R::sub(My, By);                    // the other own disk (s = 0)
+      P rmin = R::fma(Dbx, Dbx, R::mul(Dby, Dby));
+      const Pair MMx = R::pair(Mx, Mx), MMy = R::pair(My, My);
+#pragma unroll
+      for (int e = 0; e < 8; ++e) {                                          // |D_move - (D + s)|^2  (line 19, L204)
+        const Pair Dx = R::padd(MMx, nqx[e]), Dy = R::padd(MMy, nqy[e]);
+        const Pair r2 = R::pfma(Dx, Dx, R::pmul(Dy, Dy));
+        rmin = R::min3(rmin, r2.x, r2.y);
+      }
+      const bool ov = rmin < sigma2;                                         // strict (A4)
+      const bool acc = inside && !ov;
+      if (acc) { Ax = Mx; Ay = My; amask |= 1u << s; }                       // lines 24-27 (L215-222)
+      n_rb += inside ? 0u : 1u;                                              // leaves the cell: rejected
+      n_acc += acc ? 1u : 0u;
+      if (two) { const P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }   // s mod n cycling (L75)
+    }
+    // a sentinel never passes the in-cell test; empty cells (and the clamped lanes past the end) attempt nothing (A10)
+    if (n == 0u) { n_rb = 0u; n_acc = 0u; amask = 0u; }
+    else { n_ro = (uint32_t)NS - n_acc - n_rb; }
+    // ---- write back (line 34, L234): the slot pair in slot order ----
+    if (amask != 0u) {
+      if (two && (NS & 1)) flip = !flip;
+      Half<P> o;
+      o.x = flip ? R::pair(Bx, Ax) : R::pair(Ax, Bx);
+      o.y = flip ? R::pair(By, Ay) : R::pair(Ay, By);
+      st_half(posb, 2u * Q * Mqp + w.ci, o);
+    }
+  }
+  if (DEBUG && w.valid) {
+    p.mask[w.cell] = amask;
+    if (n > 0u) atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)w.cell << 32) | amask)));
+  }
+  add_counters(p, n_acc, n_rb, n_ro);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// General sub-sweep kernel: any occupancy up to n_max = 4 per cell — the paper's own regime, w up to
+// sqrt(2) sigma (L152) — and any n_s.  Same mapping and arithmetic; all four slots of the 3x3 cells are kept
+// in registers (own cell as two negated pairs, each neighbour as two translated, negated pairs; slot pair 1 is
+// loaded only where n > 2), and the disk a move acts on is chosen with select chains from the visiting
+// permutation.  NS > 0 fixes n_s at compile time (Philox blocks issued up front, move loop unrolled); NS = 0 is
+// the run-time loop.
+// ---------------------------------------------------------------------------------------------------------
+template <typename P, int NS, bool DEBUG>
+__global__ void __launch_bounds__(SUB_THREADS, SUB_MINB)
+k_sub_sweep(const __grid_constant__ Params p, const uint32_t setk) {
+  using R = Real<P>;
+  using Pair = typename R::Pair;
+  static_assert(NS % 2 == 0, "compile-time n_s must be even");
+  const Ctl* __restrict__ ctl = p.ctl;
+  const uint32_t Q = setk < 4 ? ctl->order[setk] : (setk & 3u);
+  const unsigned long long t = ctl->t;
+  const uint32_t cur = ctl->cur;
+  const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
+  const Where w = locate_active(p, Q, blockIdx.x * SUB_THREADS + threadIdx.x);
+  const uint8_t* cntb = p.cnt[cur];
+  P* posb = reinterpret_cast<P*>(p.pos[cur]);
+  const uint32_t Mqp = p.Mqp;
+
+  // ---- level-1 loads, all independent: count and slot pair 0 of the 3x3 cells (idx 4 = own cell) ----
+  uint32_t cj[9], pidx[9];
+  Half<P> h0[9];
+#pragma unroll
+  for (int idx = 0; idx < 9; ++idx) {
+    uint32_t qn, cn;
+    neighbour(w, idx % 3 - 1, idx / 3 - 1, qn, cn);
+    pidx[idx] = 2u * qn * Mqp + cn;
+    cj[idx] = ld_u8_early(cntb + (qn * Mqp + cn));
+    h0[idx] = ld_half_early(posb, pidx[idx]);
+  }
+
+  // ---- Philox words of the shuffle and of the displacements, while the loads are in flight ----
+  constexpr int NSA = NS > 0 ? NS : 2;
+  P ddx[NSA], ddy[NSA];
+  auto displacement2 = [&](uint32_t q, int at) {       // block q serves moves 2q and 2q + 1 (reading A9)
+    uint32_t Rw[4];
+    philox4x32_10(w.cell, t_lo, t_hi, q, p.seed_lo, p.seed_hi, Rw);
+    ddx[at] = R::scaled_sym(p, Rw[0]); ddy[at] = R::scaled_sym(p, Rw[1]);
+    ddx[at + 1] = R::scaled_sym(p, Rw[2]); ddy[at + 1] = R::scaled_sym(p, Rw[3]);
+  };
+  uint32_t S[4];
+  philox4x32_10(w.cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
+  if (NS > 0) {
+#pragma unroll
+    for (int q = 0; q < NS / 2; ++q) displacement2((uint32_t)q, 2 * q);
+  }
+
+  uint32_t n_acc = 0, n_rb = 0, n_ro = 0, amask = 0;
+  const uint32_t n = w.valid ? cj[4] : 0u;
+  const uint32_t nv = n > 0u ? n : 1u;                 // visiting modulus; an empty cell "visits" a sentinel
+  const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p);
+  const P FAR = R::far_away();
+  const Pair MINUS1 = R::pair((P)-1, (P)-1);
+
+  // ---- level-2 loads: slot pair 1 where n > 2 ----
+  Half<P> h1[9];
+#pragma unroll
+  for (int idx = 0; idx < 9; ++idx) {
+    h1[idx].x = R::pair(FAR, FAR); h1[idx].y = h1[idx].x;
+    if (cj[idx] > 2u) h1[idx] = ld_half(posb, pidx[idx] + Mqp);
+  }
+
+  // ---- own cell (Alg. 2 line 8, L186), negated, as pairs (slot 0,1) and (slot 2,3) ----
+  Pair nox[2], noy[2];
+  nox[0] = R::pair(-h0[4].x.x, -h0[4].x.y); nox[1] = R::pair(-h1[4].x.x, -h1[4].x.y);
+  noy[0] = R::pair(-h0[4].y.x, -h0[4].y.y); noy[1] = R::pair(-h1[4].y.x, -h1[4].y.y);
+
+  // ---- neighbours, translated into this cell's frame (s = (ox wx, oy wy), L154, L196), negated ----
+  Pair nqx[16], nqy[16];
+#pragma unroll
+  for (int idx = 0; idx < 9; ++idx) {
+    if (idx == 4) continue;
+    const int e = idx < 4 ? idx : idx - 1;
+    const int ox = idx % 3 - 1, oy = idx / 3 - 1;
+    const P nsx = ox < 0 ? wx : ox > 0 ? -wx : (P)0;
+    const P nsy = oy < 0 ? wy : oy > 0 ? -wy : (P)0;
+    nqx[2 * e] = R::pfma(h0[idx].x, MINUS1, R::pair(nsx, nsx));
+    nqy[2 * e] = R::pfma(h0[idx].y, MINUS1, R::pair(nsy, nsy));
+    nqx[2 * e + 1] = R::pfma(h1[idx].x, MINUS1, R::pair(nsx, nsx));
+    nqy[2 * e + 1] = R::pfma(h1[idx].y, MINUS1, R::pair(nsy, nsy));
+  }
+
+  const uint32_t perm = visiting_permutation(n, S);    // Alg. 2 line 9 (L187)
+
+  // ---- n_s trial moves (Alg. 2 lines 11-32, L189-230) ----
+  uint32_t vi = 0;
+  auto trial_move = [&](const uint32_t s, const P dx, const P dy) {
+    const uint32_t k = (perm >> (4u * vi)) & 3u;               // p <- particles[s mod n]  (L75)
+    vi = (vi + 1u == nv) ? 0u : vi + 1u;                       // lines 28-32 (L224-230)
+    const P nlx = k == 0 ? nox[0].x : k == 1 ? nox[0].y : k == 2 ? nox[1].x : nox[1].y;
+    const P nly = k == 0 ? noy[0].x : k == 1 ? noy[0].y : k == 2 ? noy[1].x : noy[1].y;
+    const P Mx = R::sub(dx, nlx);                              // D_move = l + displacement
+    const P My = R::sub(dy, nly);
+    const bool inside = (Mx > (P)0) && (Mx <= wx) && (My > (P)0) && (My <= wy);   // (0, w]  (A3)
+    const Pair MMx = R::pair(Mx, Mx), MMy = R::pair(My, My);
+    bool ov = false;
+    // the other disks of the own cell (line 17 skips i = j, L201); s = 0 so q = l_j
+#pragma unroll
+    for (int hh = 0; hh < 2; ++hh) {
+      const Pair Dx = R::padd(MMx, nox[hh]), Dy = R::padd(MMy, noy[hh]);
+      const Pair r2 = R::pfma(Dx, Dx, R::pmul(Dy, Dy));
+      ov |= (r2.x < sigma2) && ((uint32_t)(2 * hh) != k);
+      ov |= (r2.y < sigma2) && ((uint32_t)(2 * hh + 1) != k);
+    }
+    // neighbour disks: |D_move - (D + s)|^2 < sigma^2 (line 19, L204)
+    P rmin = FAR;
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+      const Pair Dx = R::padd(MMx, nqx[e]), Dy = R::padd(MMy, nqy[e]);
+      const Pair r2 = R::pfma(Dx, Dx, R::pmul(Dy, Dy));
+      rmin = R::min3(rmin, r2.x, r2.y);
+    }
+    ov |= rmin < sigma2;
+    if (!inside) {
+      ++n_rb;                                                  // leaves the cell: rejected (L79, L118)
+    } else if (ov) {
+      ++n_ro;
+    } else {                                                   // lines 24-27 (L215-222)
+      ++n_acc;
+      amask |= 1u << (s & 31u);
+      const P nMx = -Mx, nMy = -My;
+      if (k == 0) { nox[0].x = nMx; noy[0].x = nMy; }
+      if (k == 1) { nox[0].y = nMx; noy[0].y = nMy; }
+      if (k == 2) { nox[1].x = nMx; noy[1].x = nMy; }
+      if (k == 3) { nox[1].y = nMx; noy[1].y = nMy; }
+    }
+  };
+  if (NS > 0) {
+#pragma unroll
+    for (int s = 0; s < NS; ++s) trial_move((uint32_t)s, ddx[s], ddy[s]);
+  } else {
+    for (uint32_t s = 0; s < p.n_s; s += 2) {
+      displacement2(s >> 1, 0);
+      trial_move(s, ddx[0], ddy[0]);
+      if (s + 1 < p.n_s) trial_move(s + 1, ddx[1], ddy[1]);
+    }
+  }
+  if (n == 0u) { n_rb = 0u; n_acc = 0u; n_ro = 0u; amask = 0u; }   // empty cells attempt nothing (A10)
+
+  // ---- write back (line 34, L234) ----
+  if (amask != 0u) {
+    Half<P> o;
+    o.x = R::pair(-nox[0].x, -nox[0].y); o.y = R::pair(-noy[0].x, -noy[0].y);
+    st_half(posb, pidx[4], o);
+    if (n > 2u) {
+      o.x = R::pair(-nox[1].x, -nox[1].y); o.y = R::pair(-noy[1].x, -noy[1].y);
+      st_half(posb, pidx[4] + Mqp, o);
+    }
+  }
+  if (DEBUG && w.valid) {
+    p.mask[w.cell] = amask;
+    if (n > 0u) atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)w.cell << 32) | amask)));
+  }
+  add_counters(p, n_acc, n_rb, n_ro);
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // Cell shift (Algorithm 4, pull form).  One thread per NEW cell (L350): its own old disks that stay, in slot
 // order, then the disks of the one old neighbour in direction f that left it.  l' = rn(l - f*delta) is the
 // same single operation on both sides, and the +-w translation of an entrant is a separate operation after
-// the test (L352), so no disk is lost or duplicated.  Writes the other buffer (L350).  The last block to
-// finish flips the buffer, advances the sweep index, moves the grid origin and draws the next sweep's set
-// order and shift, so a sweep needs no host involvement.
+// the test (L352), so no disk is lost or duplicated.  Writes the other buffer (L350).  Both old cells are one
+// slot-pair load each (+ ids), the new cell is compacted in registers and written as one slot pair (sentinel in
+// the empty slots); cells with more than 2 disks take a rolled generic path.  The last block to finish flips
+// the buffer, advances the sweep index, moves the grid origin and draws the next sweep's set order and shift,
+// so a sweep needs no host involvement.
 // ovr: 0 = use Ctl's draws and advance the sweep; 1 = test hook (explicit dir/delta, sweep index unchanged).
 // ---------------------------------------------------------------------------------------------------------
+template <typename P> struct Disk { P x, y; uint32_t id; };
+template <typename P> __device__ __forceinline__ Disk<P> pick(bool c, const Disk<P>& a, const Disk<P>& b) {
+  Disk<P> r; r.x = c ? a.x : b.x; r.y = c ? a.y : b.y; r.id = c ? a.id : b.id; return r;
+}
+
 // one new cell; ALONG_X and POSITIVE are uniform across the grid, so the caller branches once
 template <typename P, bool ALONG_X, bool POSITIVE>
 __device__ __forceinline__ void shift_cell(const Params& p, Ctl* ctl, const uint32_t cur, const uint32_t Q,
                                            const uint32_t ci, const P delta) {
   using R = Real<P>;
-  using P2 = typename R::T2;
   const uint32_t nxt = cur ^ 1u, Mqp = p.Mqp;
   const uint8_t* __restrict__ cntc = p.cnt[cur];
-  const P2* __restrict__ posc = reinterpret_cast<const P2*>(p.pos[cur]);
-  const uint32_t* __restrict__ idsc = p.ids[cur];
-  P2* __restrict__ posn = reinterpret_cast<P2*>(p.pos[nxt]);
-  uint32_t* __restrict__ idsn = p.ids[nxt];
+  const P* __restrict__ posc = reinterpret_cast<const P*>(p.pos[cur]);
+  const uint2* __restrict__ idsc = reinterpret_cast<const uint2*>(p.ids[cur]);
+  P* __restrict__ posn = reinterpret_cast<P*>(p.pos[nxt]);
+  uint2* __restrict__ idsn = reinterpret_cast<uint2*>(p.ids[nxt]);
   const P w = ALONG_X ? R::wx(p) : R::wy(p);
   const P step = POSITIVE ? -delta : delta;     // l' = l - f*delta   (L303)
   const P back = POSITIVE ? w : -w;             // entrant translation (L332)
+  const P FAR = R::far_away();
   const uint32_t offx = Q & 1u, offy = Q >> 1;
   // the old neighbour in direction f (lines 15-16, L314-317)
   uint32_t qn, cn;
@@ -311,39 +471,73 @@ __device__ __forceinline__ void shift_cell(const Params& p, Ctl* ctl, const uint
     if (POSITIVE) cn = offy ? (ci + p.hx >= p.Mq ? ci + p.hx - p.Mq : ci + p.hx) : ci;
     else          cn = offy ? ci : (ci < p.hx ? ci + p.Mq - p.hx : ci - p.hx);
   }
-  const uint32_t own0 = Q * NMAX * Mqp + ci, nb0 = qn * NMAX * Mqp + cn;
+  const uint32_t own = 2u * Q * Mqp + ci, nb = 2u * qn * Mqp + cn;       // slot-pair indices (half 0)
   const uint32_t n0 = cntc[Q * Mqp + ci], n1 = cntc[qn * Mqp + cn];
-  uint32_t nn = 0;
-  // lines 7-14 (L299-312): own disks that stay, in slot order
-#pragma unroll
-  for (int i = 0; i < NMAX; ++i) {
-    if ((uint32_t)i < n0) {
-      P2 v = posc[own0 + i * Mqp];
-      const uint32_t id = idsc[own0 + i * Mqp];
-      const P a = R::add(ALONG_X ? v.x : v.y, step);
-      if (a > (P)0 && a <= w) {
-        if (ALONG_X) v.x = a; else v.y = a;
-        posn[own0 + nn * Mqp] = v;
-        idsn[own0 + nn * Mqp] = id;
-        ++nn;
-      }
+  const Half<P> a = ld_half(posc, own), b = ld_half(posc, nb);
+  const uint2 ia = idsc[own], ib = idsc[nb];
+  uint32_t nn;
+  if (n0 <= 2u && n1 <= 2u) {
+    // lines 7-14 (L299-312): own disks that stay; a sentinel stays a sentinel and fails the test
+    Disk<P> o0 = {a.x.x, a.y.x, ia.x}, o1 = {a.x.y, a.y.y, ia.y};
+    const P a0 = R::add(ALONG_X ? o0.x : o0.y, step), a1 = R::add(ALONG_X ? o1.x : o1.y, step);
+    if (ALONG_X) { o0.x = a0; o1.x = a1; } else { o0.y = a0; o1.y = a1; }
+    const bool k0 = a0 > (P)0 && a0 <= w, k1 = a1 > (P)0 && a1 <= w;
+    // lines 17-27 (L319-339): disks of the neighbour that left it enter here; L332 is a separate operation
+    Disk<P> e0 = {b.x.x, b.y.x, ib.x}, e1 = {b.x.y, b.y.y, ib.y};
+    const P b0 = R::add(ALONG_X ? e0.x : e0.y, step), b1 = R::add(ALONG_X ? e1.x : e1.y, step);
+    const bool g0 = n1 > 0u && !(b0 > (P)0 && b0 <= w), g1 = n1 > 1u && !(b1 > (P)0 && b1 <= w);
+    const P c0 = R::add(b0, back), c1 = R::add(b1, back);
+    if (ALONG_X) { e0.x = c0; e1.x = c1; } else { e0.y = c0; e1.y = c1; }
+    // compaction: stayers in slot order, then entrants in slot order (reading A13)
+    const Disk<P> none = {FAR, FAR, 0xFFFFFFFFu};
+    const uint32_t ns = (k0 ? 1u : 0u) + (k1 ? 1u : 0u), ne = (g0 ? 1u : 0u) + (g1 ? 1u : 0u);
+    const Disk<P> s0 = pick(k0, o0, o1);
+    const Disk<P> t0 = pick(ne > 0u, pick(g0, e0, e1), none), t1 = pick(ne > 1u, e1, none);
+    const Disk<P> r0 = pick(ns > 0u, s0, t0);
+    const Disk<P> r1 = pick(ns == 2u, o1, pick(ns == 1u, t0, t1));
+    nn = ns + ne;
+    Half<P> o;
+    o.x = R::pair(r0.x, r1.x); o.y = R::pair(r0.y, r1.y);
+    st_half(posn, own, o);
+    idsn[own] = make_uint2(r0.id, r1.id);
+    if (nn > 2u) {
+      const Disk<P> r2 = pick(ns == 2u, t0, pick(ns == 1u, t1, none));
+      const Disk<P> r3 = pick(ns == 2u, t1, none);
+      o.x = R::pair(r2.x, r3.x); o.y = R::pair(r2.y, r3.y);
+      st_half(posn, own + Mqp, o);
+      idsn[own + Mqp] = make_uint2(r2.id, r3.id);
     }
-  }
-  // lines 17-27 (L319-339): disks of the neighbour that left it enter here
-#pragma unroll
-  for (int i = 0; i < NMAX; ++i) {
-    if ((uint32_t)i < n1) {
-      P2 v = posc[nb0 + i * Mqp];
-      const P a = R::add(ALONG_X ? v.x : v.y, step);
-      if (!(a > (P)0 && a <= w)) {              // else: stays in the neighbour (L326-328)
-        const P b = R::add(a, back);            // L332: a separate operation after the test (L352)
+  } else {
+    // generic: any occupancy, rolled loops, scalar accesses
+    nn = 0;
+    P* on = posn + (size_t)own * 4;                  // new cell: slot s at on[(s>>1)*4*Mqp + (s&1)], y at +2
+    uint32_t* idn = p.ids[nxt] + (size_t)own * 2;
+    const uint32_t* idc = p.ids[cur];
+#pragma unroll 1
+    for (uint32_t pass = 0; pass < 2u; ++pass) {
+      const uint32_t src = pass ? nb : own, cnt = pass ? n1 : n0;
+#pragma unroll 1
+      for (uint32_t i = 0; i < cnt; ++i) {
+        const size_t e = (size_t)(src + (i >> 1) * Mqp);
+        P x = posc[e * 4 + (i & 1u)], y = posc[e * 4 + 2 + (i & 1u)];
+        P m = R::add(ALONG_X ? x : y, step);
+        const bool in = m > (P)0 && m <= w;
+        if (pass ? in : !in) continue;               // own: leavers go elsewhere; neighbour: stayers stay (L326-328)
+        if (pass) m = R::add(m, back);               // L332, after the test (L352)
+        if (ALONG_X) x = m; else y = m;
         if (nn < (uint32_t)NMAX) {
-          if (ALONG_X) v.x = b; else v.y = b;
-          posn[own0 + nn * Mqp] = v;
-          idsn[own0 + nn * Mqp] = idsc[nb0 + i * Mqp];
+          const size_t d = (size_t)(nn >> 1) * Mqp;
+          on[d * 4 + (nn & 1u)] = x; on[d * 4 + 2 + (nn & 1u)] = y;
+          idn[d * 2 + (nn & 1u)] = idc[e * 2 + (i & 1u)];
         }
         ++nn;
       }
+    }
+    const uint32_t fill_to = nn > 2u ? (uint32_t)NMAX : 2u;     // sentinel in the empty slots of the halves in use
+    for (uint32_t s = nn; s < fill_to; ++s) {
+      const size_t d = (size_t)(s >> 1) * Mqp;
+      on[d * 4 + (s & 1u)] = FAR; on[d * 4 + 2 + (s & 1u)] = FAR;
+      idn[d * 2 + (s & 1u)] = 0xFFFFFFFFu;
     }
   }
   if (nn > (uint32_t)NMAX) { atomicOr(&ctl->err, ERRBIT_OVERFLOW); nn = NMAX; }
