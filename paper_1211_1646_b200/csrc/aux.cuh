@@ -8,17 +8,16 @@ namespace mpmc {
 constexpr int AUX_THREADS = 256;
 
 __global__ void k_reset(const __grid_constant__ Params p) {
-  // clear the u32 build counters and the control block; draw sweep 0
+  // clear the u32 build counters and the control block
   const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
   const uint32_t total = 4u * p.Mqp;
   for (uint32_t i = g; i < total; i += gridDim.x * blockDim.x) p.cnt32[i] = 0;
   if (g == 0) {
     Ctl* c = p.ctl;
-    c->t = 0; c->cur = 0; c->err = 0; c->ticket = 0; c->pad0 = 0;
+    c->t = 0; c->cur = 0; c->err = 0; c->bar = 0; c->pad0 = 0;
     c->origin[0] = 0.0; c->origin[1] = 0.0;
     c->digest = 0;
     for (uint32_t r = 0; r < CTR_SLOTS; ++r) c->counters[r][0] = c->counters[r][1] = c->counters[r][2] = c->counters[r][3] = 0;
-    draw_sweep(p, 0ull, c);
   }
 }
 

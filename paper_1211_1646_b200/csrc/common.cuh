@@ -36,16 +36,13 @@ constexpr uint32_t ERRBIT_RANGE = 2u;     // loaded coordinate NaN or outside [0
 constexpr uint32_t ERRBIT_OVERLAP = 4u;   // loaded positions overlap
 constexpr uint32_t CTR_SLOTS = 64;        // rows of move counters (summed on read)
 
-// Device-resident control block: everything that changes from sweep to sweep, so that a captured CUDA graph
-// can be replayed with no host-side argument updates (mpmc.h, mpmc_sweep).
+// Device-resident control block: the state that survives between launches.  Inside a launch the sweep index,
+// buffer parity, grid origin and per-sweep draws live in registers / shared memory (sweep.cuh, k_sweeps).
 struct Ctl {
   unsigned long long t;            // sweep index
-  uint32_t order[4];               // checkerboard sets in the order they run this sweep (Alg. 1 line 2, L64)
-  uint32_t dir;                    // shift direction 0:+x 1:-x 2:+y 3:-y (Alg. 1 line 16, L91)
-  uint32_t dist_word;              // random word the shift distance is made of (Alg. 1 line 15, L90)
   uint32_t cur;                    // which buffer holds the current state
   uint32_t err;                    // sticky error bits
-  uint32_t ticket;                 // blocks-done counter of the shift kernel
+  uint32_t bar;                    // arrival counter of the grid barrier (zeroed by the host before a launch)
   uint32_t pad0;
   double origin[2];                // grid origin: X = origin + cell * w + local
   unsigned long long digest;       // accept-sequence digest (MPMC_DEBUG)
@@ -152,8 +149,10 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 __device__ __forceinline__ uint32_t bounded(uint32_t word, uint32_t bound) { return __umulhi(word, bound); }
 
 // Per-sweep draws (Alg. 1 lines 2, 15, 16; reading A9): Fisher-Yates of the four sets with
-// words G0..G2, direction from the top two bits of G3, distance word from a second counter.
-__device__ __forceinline__ void draw_sweep(const Params& p, unsigned long long t, Ctl* ctl) {
+// words G0..G2, direction from the top two bits of G3, distance word from a second counter.  A pure function of
+// (seed, sweep index), so every block computes it for itself.
+struct Draws { uint32_t order[4]; uint32_t dir; uint32_t dist_word; };
+__device__ __forceinline__ Draws draw_sweep(const Params& p, unsigned long long t) {
   uint32_t G[4], H[4];
   philox4x32_10(CELL_GLOBAL, (uint32_t)t, (uint32_t)(t >> 32), SLOT_ORDER, p.seed_lo, p.seed_hi, G);
   uint32_t o[4] = {0, 1, 2, 3};
@@ -167,9 +166,11 @@ __device__ __forceinline__ void draw_sweep(const Params& p, unsigned long long t
     o[i] = b;
   }
   philox4x32_10(CELL_GLOBAL, (uint32_t)t, (uint32_t)(t >> 32), SLOT_DIST, p.seed_lo, p.seed_hi, H);
-  ctl->order[0] = o[0]; ctl->order[1] = o[1]; ctl->order[2] = o[2]; ctl->order[3] = o[3];
-  ctl->dir = G[3] >> 30;
-  ctl->dist_word = H[0];
+  Draws d;
+  d.order[0] = o[0]; d.order[1] = o[1]; d.order[2] = o[2]; d.order[3] = o[3];
+  d.dir = G[3] >> 30;
+  d.dist_word = H[0];
+  return d;
 }
 
 // ya = ci / hx, xa = ci - ya * hx with the precomputed magic numbers of Params
@@ -182,7 +183,7 @@ __device__ __forceinline__ uint32_t div_hx(const Params& p, uint32_t ci) {
 // so they are issued up front and their latency overlaps the Philox arithmetic (sweep.cuh, level-1 loads).
 __device__ __forceinline__ uint32_t ld_u8_early(const uint8_t* ptr) {
   uint32_t v;
-  asm volatile("ld.global.u8 %0, [%1];" : "=r"(v) : "l"(ptr));
+  asm volatile("ld.global.u8 %0, [%1];" : "=r"(v) : "l"(ptr) : "memory");
   return v;
 }
 
@@ -193,14 +194,14 @@ template <typename P> struct Half { typename Real<P>::Pair x, y; };   // (x_a, x
 __device__ __forceinline__ Half<float> ld_half_early(const float* pos, uint32_t i) {
   Half<float> h;
   asm volatile("ld.global.v4.f32 {%0, %1, %2, %3}, [%4];"
-               : "=f"(h.x.x), "=f"(h.x.y), "=f"(h.y.x), "=f"(h.y.y) : "l"(reinterpret_cast<const float4*>(pos) + i));
+               : "=f"(h.x.x), "=f"(h.x.y), "=f"(h.y.x), "=f"(h.y.y) : "l"(reinterpret_cast<const float4*>(pos) + i) : "memory");
   return h;
 }
 __device__ __forceinline__ Half<double> ld_half_early(const double* pos, uint32_t i) {
   Half<double> h;
   const double2* q = reinterpret_cast<const double2*>(pos) + 2 * (size_t)i;
-  asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(h.x.x), "=d"(h.x.y) : "l"(q));
-  asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(h.y.x), "=d"(h.y.y) : "l"(q + 1));
+  asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(h.x.x), "=d"(h.x.y) : "l"(q) : "memory");
+  asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(h.y.x), "=d"(h.y.y) : "l"(q + 1) : "memory");
   return h;
 }
 __device__ __forceinline__ Half<float> ld_half(const float* pos, uint32_t i) {

@@ -21,14 +21,14 @@ struct mpmc_ctx {
   bool fp32, debug, loaded;
   int nf;                  // 2: w < 1.15 sigma, cells hold 0/1/2 disks -> fast sub-sweep kernel; 4: general kernel
   cudaStream_t stream;
-  cudaGraphExec_t graph1;  // one sweep
-  cudaGraphExec_t graphK;  // GRAPH_BATCH sweeps
+  const void* kernel;      // the k_sweeps instantiation for this context
+  uint32_t grid;           // co-resident blocks of the persistent kernel
   int sticky;
 };
 
 namespace {
 
-constexpr uint32_t GRAPH_BATCH = 16;
+constexpr uint32_t MAX_SWEEPS_PER_LAUNCH = 1u << 16;
 constexpr size_t ALIGN = 256;
 constexpr uint32_t MAX_BINS = 4096;
 
@@ -107,41 +107,27 @@ int cuda_fail(cudaError_t e) {
 
 dim3 cell_grid(const mpmc_ctx* c, int threads) { return dim3((c->p.Mq + threads - 1) / threads, 4, 1); }
 
-// ---- kernel launchers ----------------------------------------------------------------------------------
-// fast = the w ~ sigma kernel (occupancy 0/1/2, compile-time n_s in {4, 8}); otherwise the general kernel
+// ---- the persistent sweep kernel ------------------------------------------------------------------------
+// fast = the w ~ sigma cell update (occupancy 0/1/2, compile-time n_s in {4, 8}); otherwise the general one
 template <typename P, bool DEBUG>
-void launch_sub_t(const mpmc_ctx* c, uint32_t setk) {
-  const dim3 grid((c->p.Mq + SUB_THREADS - 1) / SUB_THREADS);
-  if (c->nf == 2 && c->p.n_s == 4) { k_sub_fast<P, 4, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); return; }
-  if (c->nf == 2 && c->p.n_s == 8) { k_sub_fast<P, 8, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); return; }
-  switch (c->p.n_s) {      // n_s = 4 and 8 are compile-time instantiations
-    case 4: k_sub_sweep<P, 4, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); break;
-    case 8: k_sub_sweep<P, 8, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); break;
-    default: k_sub_sweep<P, 0, DEBUG><<<grid, SUB_THREADS, 0, c->stream>>>(c->p, setk); break;
-  }
+const void* pick_kernel_t(bool fast, uint32_t n_s) {
+  if (fast && n_s == 4) return (const void*)k_sweeps<P, 4, DEBUG, true>;
+  if (fast && n_s == 8) return (const void*)k_sweeps<P, 8, DEBUG, true>;
+  if (n_s == 4) return (const void*)k_sweeps<P, 4, DEBUG, false>;
+  if (n_s == 8) return (const void*)k_sweeps<P, 8, DEBUG, false>;
+  return (const void*)k_sweeps<P, 0, DEBUG, false>;
 }
-void launch_sub(const mpmc_ctx* c, uint32_t setk) {
-  if (c->fp32) { if (c->debug) launch_sub_t<float, true>(c, setk); else launch_sub_t<float, false>(c, setk); }
-  else         { if (c->debug) launch_sub_t<double, true>(c, setk); else launch_sub_t<double, false>(c, setk); }
-}
-void launch_shift(const mpmc_ctx* c, uint32_t ovr, uint32_t dir, double delta) {
-  const dim3 grid = cell_grid(c, SHIFT_THREADS);
-  if (c->fp32) k_shift<float><<<grid, SHIFT_THREADS, 0, c->stream>>>(c->p, ovr, dir, delta);
-  else         k_shift<double><<<grid, SHIFT_THREADS, 0, c->stream>>>(c->p, ovr, dir, delta);
-}
-void enqueue_sweep(const mpmc_ctx* c) {       // Algorithm 1: 4 sub-sweeps + shift
-  for (uint32_t k = 0; k < 4; ++k) launch_sub(c, k);
-  launch_shift(c, 0, 0, 0.0);
+const void* pick_kernel(bool fp32, bool debug, bool fast, uint32_t n_s) {
+  if (fp32) return debug ? pick_kernel_t<float, true>(fast, n_s) : pick_kernel_t<float, false>(fast, n_s);
+  return debug ? pick_kernel_t<double, true>(fast, n_s) : pick_kernel_t<double, false>(fast, n_s);
 }
 
-int build_graph(mpmc_ctx* c, uint32_t sweeps, cudaGraphExec_t* out) {
-  cudaGraph_t g = nullptr;
-  CU(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
-  for (uint32_t i = 0; i < sweeps; ++i) enqueue_sweep(c);
-  CU(cudaStreamEndCapture(c->stream, &g));
-  cudaError_t e = cudaGraphInstantiate(out, g, 0);
-  cudaGraphDestroy(g);
-  return cuda_fail(e);
+// one cooperative launch: k sweeps, or one piece of a sweep (test hooks)
+int launch_sweeps(mpmc_ctx* c, uint32_t k, uint32_t op, uint32_t arg, double delta) {
+  CU(cudaMemsetAsync(&c->p.ctl->bar, 0, sizeof(uint32_t), c->stream));
+  void* args[] = {(void*)&c->p, (void*)&k, (void*)&op, (void*)&arg, (void*)&delta};
+  CU(cudaLaunchCooperativeKernel(c->kernel, dim3(c->grid), dim3(SUB_THREADS), args, 0, c->stream));
+  return MPMC_OK;
 }
 
 int read_ctl(mpmc_ctx* c, Ctl* h) {
@@ -224,7 +210,7 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   if (!c) return MPMC_ERR_ARG;
   std::memset(&c->p, 0, sizeof(Params));
   c->N = N; c->flags = flags; c->fp32 = fp32; c->debug = debug; c->loaded = false; c->sticky = MPMC_OK;
-  c->stream = (cudaStream_t)cuda_stream; c->graph1 = nullptr; c->graphK = nullptr;
+  c->stream = (cudaStream_t)cuda_stream;
   Params& p = c->p;
   p.mx = g.m[0]; p.my = g.m[1]; p.hx = g.m[0] / 2; p.hy = g.m[1] / 2;
   p.Mq = L.Mq; p.Mqp = L.Mqp; p.n_s = n_s; p.N = (uint32_t)N;
@@ -252,6 +238,16 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   // path); general kernel in the paper's regime (w up to sqrt(2) sigma, L152).
   const double wmax = g.wp[0] > g.wp[1] ? g.wp[0] : g.wp[1];
   c->nf = (wmax < 1.15 * sigma) ? 2 : 4;
+  c->kernel = pick_kernel(fp32, debug, c->nf == 2 && (n_s == 4 || n_s == 8), n_s);
+  // grid of the persistent kernel: every block co-resident (cooperative launch), no more blocks than chunks
+  int dev = 0, sms = 0, occ = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->kernel, SUB_THREADS, 0) != cudaSuccess || occ < 1) {
+    cudaGetLastError(); delete c; return MPMC_ERR_CUDA;
+  }
+  const uint32_t chunks = (L.Mq + SUB_THREADS - 1) / SUB_THREADS;
+  c->grid = (uint32_t)sms * (uint32_t)occ;
+  if (c->grid > chunks) c->grid = chunks;
   *out = c;
   return MPMC_OK;
 }
@@ -263,8 +259,6 @@ int mpmc_create(mpmc_ctx** out, uint64_t N, const double box[2], double sigma, d
 
 int mpmc_destroy(mpmc_ctx* c) {
   if (!c) return MPMC_OK;
-  if (c->graph1) cudaGraphExecDestroy(c->graph1);
-  if (c->graphK) cudaGraphExecDestroy(c->graphK);
   delete c;
   return MPMC_OK;
 }
@@ -304,20 +298,12 @@ int mpmc_load_positions(mpmc_ctx* c, const double* xy) {
 int mpmc_sweep(mpmc_ctx* c, uint64_t k) {
   if (!c) return MPMC_ERR_ARG;
   if (!c->loaded) return MPMC_ERR_STATE;
-  if (c->stream == nullptr) {
-    // the legacy default stream cannot be captured: plain launches (same kernels, same order)
-    for (; k > 0; --k) enqueue_sweep(c);
-    CU(cudaGetLastError());
-    return c->sticky;
-  }
-  if (!c->graph1) {
-    int st = build_graph(c, 1, &c->graph1);
+  while (k > 0) {
+    const uint32_t kk = k > MAX_SWEEPS_PER_LAUNCH ? MAX_SWEEPS_PER_LAUNCH : (uint32_t)k;
+    const int st = launch_sweeps(c, kk, OP_SWEEPS, 0, 0.0);
     if (st != MPMC_OK) return st;
-    st = build_graph(c, GRAPH_BATCH, &c->graphK);
-    if (st != MPMC_OK) return st;
+    k -= kk;
   }
-  while (k >= GRAPH_BATCH) { CU(cudaGraphLaunch(c->graphK, c->stream)); k -= GRAPH_BATCH; }
-  while (k > 0) { CU(cudaGraphLaunch(c->graph1, c->stream)); --k; }
   return c->sticky;
 }
 
@@ -383,17 +369,15 @@ int mpmc_pressure_contact(mpmc_ctx* c, double dr, uint32_t nbins, uint32_t degre
 int mpmc_debug_sub_sweep(mpmc_ctx* c, uint32_t set) {
   if (!c || set > 3) return MPMC_ERR_ARG;
   if (!c->loaded) return MPMC_ERR_STATE;
-  launch_sub(c, 4u + set);
-  CU(cudaGetLastError());
-  return c->sticky;
+  const int st = launch_sweeps(c, 0, OP_SUB_SWEEP, set, 0.0);
+  return st != MPMC_OK ? st : c->sticky;
 }
 
 int mpmc_debug_shift(mpmc_ctx* c, uint32_t direction, double delta) {
   if (!c || direction > 3 || !(delta >= 0)) return MPMC_ERR_ARG;
   if (!c->loaded) return MPMC_ERR_STATE;
-  launch_shift(c, 1, direction, delta);
-  CU(cudaGetLastError());
-  return c->sticky;
+  const int st = launch_sweeps(c, 0, OP_SHIFT, direction, delta);
+  return st != MPMC_OK ? st : c->sticky;
 }
 
 int mpmc_debug_state(mpmc_ctx* c, void* counts, void* slab, void* ids, void* accept_mask, double origin[2],
