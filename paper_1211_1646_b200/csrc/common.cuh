@@ -43,7 +43,9 @@ struct Ctl {
   uint32_t cur;                    // which buffer holds the current state
   uint32_t err;                    // sticky error bits
   uint32_t bar;                    // arrival counter of the grid barrier (zeroed by the host before a launch)
-  uint32_t pad0;
+  uint32_t ticket;                 // blocks-done counter of the tile kernel
+  uint32_t crowded[4];             // crowded[t & 3] != 0: at sweep t some cell holds more than 2 disks (tile.cuh)
+  uint32_t pad0[2];
   double origin[2];                // grid origin: X = origin + cell * w + local
   unsigned long long digest;       // accept-sequence digest (MPMC_DEBUG)
   unsigned long long counters[CTR_SLOTS][4];  // per row: accepted, rejected_boundary, rejected_overlap, -
@@ -55,6 +57,8 @@ struct Params {
   uint32_t Mq, Mqp;          // cells per colour; plane stride (Mq rounded up to 64)
   uint32_t n_s, N;
   uint32_t hx_magic, hx_sh1, hx_sh2;  // ci / hx without a divide (Granlund-Montgomery; host: div_magic)
+  uint32_t tl_ntx, tl_nty, tl_PS, tl_single;  // tile kernel: tiles per axis, shared-memory plane stride (cells),
+                                              // 1 if a loaded region wraps around the box at most once
   uint32_t seed_lo, seed_hi;
   float wx_f, wy_f, sigma2_f, d_f;      // working-precision constants (fp32 mode)
   double wx_p, wy_p, sigma2_p, d_p;     // working-precision constants (fp64 mode)

@@ -4,6 +4,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -11,6 +12,7 @@
 #include "aux.cuh"
 #include "common.cuh"
 #include "sweep.cuh"
+#include "tile.cuh"
 
 using namespace mpmc;
 
@@ -23,12 +25,15 @@ struct mpmc_ctx {
   cudaStream_t stream;
   const void* kernel;      // the k_sweeps instantiation for this context
   uint32_t grid;           // co-resident blocks of the persistent kernel
+  const void* tile_kernel; // the k_tile_sweep instantiation, or nullptr when the tile path does not apply
+  uint32_t tile_grid;      // tiles = CTAs of the tile kernel
+  size_t tile_smem;        // its dynamic shared memory
+  uint64_t t_host;         // sweeps requested since the last load (the sweep index the device will reach)
   int sticky;
 };
 
 namespace {
 
-constexpr uint32_t MAX_SWEEPS_PER_LAUNCH = 1u << 16;
 constexpr size_t ALIGN = 256;
 constexpr uint32_t MAX_BINS = 4096;
 
@@ -122,12 +127,41 @@ const void* pick_kernel(bool fp32, bool debug, bool fast, uint32_t n_s) {
   return debug ? pick_kernel_t<double, true>(fast, n_s) : pick_kernel_t<double, false>(fast, n_s);
 }
 
-// one cooperative launch: k sweeps, or one piece of a sweep (test hooks)
-int launch_sweeps(mpmc_ctx* c, uint32_t k, uint32_t op, uint32_t arg, double delta) {
+// one cooperative launch: sweeps up to sweep index t_end, or one piece of a sweep (test hooks)
+int launch_sweeps(mpmc_ctx* c, unsigned long long t_end, uint32_t op, uint32_t arg, double delta) {
   CU(cudaMemsetAsync(&c->p.ctl->bar, 0, sizeof(uint32_t), c->stream));
-  void* args[] = {(void*)&c->p, (void*)&k, (void*)&op, (void*)&arg, (void*)&delta};
+  void* args[] = {(void*)&c->p, (void*)&t_end, (void*)&op, (void*)&arg, (void*)&delta};
   CU(cudaLaunchCooperativeKernel(c->kernel, dim3(c->grid), dim3(SUB_THREADS), args, 0, c->stream));
   return MPMC_OK;
+}
+
+const void* pick_tile_kernel(bool fp32, bool debug, uint32_t n_s) {
+  if (n_s == 4) return fp32 ? (debug ? (const void*)k_tile_sweep<float, 4, true> : (const void*)k_tile_sweep<float, 4, false>)
+                            : (debug ? (const void*)k_tile_sweep<double, 4, true> : (const void*)k_tile_sweep<double, 4, false>);
+  if (n_s == 8) return fp32 ? (debug ? (const void*)k_tile_sweep<float, 8, true> : (const void*)k_tile_sweep<float, 8, false>)
+                            : (debug ? (const void*)k_tile_sweep<double, 8, true> : (const void*)k_tile_sweep<double, 8, false>);
+  return nullptr;
+}
+
+// Tiling of the tile kernel: ntx x nty tiles of (nearly) equal even size whose loaded region (tile + 2 HALO) fits
+// the shared memory of one SM; among those, the one with the least work on the busiest SM:
+// waves * cells of the largest region.  Returns false if not even a 2 x 2 tile fits.
+bool choose_tiling(uint32_t hx, uint32_t hy, size_t cell_bytes, size_t smem_max, uint32_t sms, uint32_t* ntx, uint32_t* nty,
+                   uint32_t* PS) {
+  double best = 0; bool found = false;
+  const uint32_t lim = 1024;
+  for (uint32_t ax = 1; ax <= hx && ax <= lim; ++ax) {
+    const uint32_t TX = 2 * ((hx + ax - 1) / ax), pw = (TX + 2 * HALO) / 2;
+    for (uint32_t ay = 1; ay <= hy && ay <= lim; ++ay) {
+      const uint32_t TY = 2 * ((hy + ay - 1) / ay), ph = (TY + 2 * HALO) / 2;
+      const size_t bytes = (size_t)4 * pw * ph * cell_bytes;
+      if (bytes > smem_max || pw * ph >= 16384u) continue;
+      const double waves = std::ceil((double)ax * ay / sms);
+      const double cost = waves * (double)(TX + 2 * HALO) * (TY + 2 * HALO) + 1e-6 * ax * ay;
+      if (!found || cost < best) { best = cost; found = true; *ntx = ax; *nty = ay; *PS = pw * ph; }
+    }
+  }
+  return found;
 }
 
 int read_ctl(mpmc_ctx* c, Ctl* h) {
@@ -248,6 +282,28 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   const uint32_t chunks = (L.Mq + SUB_THREADS - 1) / SUB_THREADS;
   c->grid = (uint32_t)sms * (uint32_t)occ;
   if (c->grid > chunks) c->grid = chunks;
+  // the tile kernel (tile.cuh) where cells hold 0/1/2 disks and n_s is a compile-time instantiation
+  c->tile_kernel = nullptr; c->tile_grid = 0; c->tile_smem = 0; c->t_host = 0;
+  if (c->nf == 2 && (n_s == 4 || n_s == 8)) {
+    int smem_optin = 0;
+    cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    const size_t cell_bytes = fp32 ? sizeof(SmemCell<float>) : sizeof(SmemCell<double>);
+    const size_t smem_max = smem_optin > 2048 ? (size_t)smem_optin - 1024 : 0;   // static shared memory: draws, flags
+    uint32_t ntx = 0, nty = 0, PS = 0;
+    if (choose_tiling(p.hx, p.hy, cell_bytes, smem_max, (uint32_t)sms, &ntx, &nty, &PS)) {
+      c->tile_kernel = pick_tile_kernel(fp32, debug, n_s);
+      c->tile_grid = ntx * nty;
+      c->tile_smem = (size_t)4 * PS * cell_bytes;
+      p.tl_ntx = ntx; p.tl_nty = nty; p.tl_PS = PS;
+      p.tl_single = (p.mx >= 6 && p.my >= 6) ? 1u : 0u;
+      if (std::getenv("MPMC_VERBOSE"))
+        std::fprintf(stderr, "[mpmc] tile kernel: %u x %u tiles, plane stride %u cells, %zu B shared memory, grid %u; general grid %u\n",
+                     ntx, nty, PS, c->tile_smem, c->tile_grid, c->grid);
+      if (cudaFuncSetAttribute(c->tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tile_smem) != cudaSuccess) {
+        cudaGetLastError(); delete c; return MPMC_ERR_CUDA;
+      }
+    }
+  }
   *out = c;
   return MPMC_OK;
 }
@@ -275,6 +331,7 @@ int mpmc_load_positions(mpmc_ctx* c, const double* xy) {
   if (!c || !xy) return MPMC_ERR_ARG;
   c->loaded = false;
   c->sticky = MPMC_OK;
+  c->t_host = 0;
   k_reset<<<148 * 4, 256, 0, c->stream>>>(c->p);
   const dim3 gN((c->p.N + AUX_THREADS - 1) / AUX_THREADS), gC = cell_grid(c, AUX_THREADS);
   if (c->fp32) {
@@ -298,13 +355,17 @@ int mpmc_load_positions(mpmc_ctx* c, const double* xy) {
 int mpmc_sweep(mpmc_ctx* c, uint64_t k) {
   if (!c) return MPMC_ERR_ARG;
   if (!c->loaded) return MPMC_ERR_STATE;
-  while (k > 0) {
-    const uint32_t kk = k > MAX_SWEEPS_PER_LAUNCH ? MAX_SWEEPS_PER_LAUNCH : (uint32_t)k;
-    const int st = launch_sweeps(c, kk, OP_SWEEPS, 0, 0.0);
-    if (st != MPMC_OK) return st;
-    k -= kk;
+  if (k == 0) return c->sticky;
+  c->t_host += k;
+  if (c->tile_kernel) {
+    // one tile-kernel launch per sweep; each returns at once if the state has become crowded (tile.cuh) ...
+    void* args[] = {(void*)&c->p};
+    for (uint64_t i = 0; i < k; ++i)
+      CU(cudaLaunchKernel(c->tile_kernel, dim3(c->tile_grid), dim3(c->fp32 ? TileThreads<float>::value : TileThreads<double>::value), args, c->tile_smem, c->stream));
   }
-  return c->sticky;
+  // ... and the general kernel runs whatever is left up to the target sweep index (normally nothing)
+  const int st = launch_sweeps(c, c->t_host, OP_SWEEPS, 0, 0.0);
+  return st != MPMC_OK ? st : c->sticky;
 }
 
 int mpmc_get_positions(mpmc_ctx* c, double* xy_out) {

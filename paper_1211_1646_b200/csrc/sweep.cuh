@@ -435,10 +435,45 @@ template <typename P> __device__ __forceinline__ Disk<P> pick(bool c, const Disk
   Disk<P> r; r.x = c ? a.x : b.x; r.y = c ? a.y : b.y; r.id = c ? a.id : b.id; return r;
 }
 
+// The new cell from the slot pairs of its own old cell (a, ids ia) and of the old neighbour in direction f (b, ib),
+// both holding at most 2 disks (empty slot = sentinel): stayers in slot order, then entrants in slot order
+// (reading A13), compacted in registers.  Returns the new count; o01/i01 = slots 0, 1; o23/i23 = slots 2, 3
+// (meaningful when the count exceeds 2), empty slots = sentinel.
+template <typename P, bool ALONG_X>
+__device__ __forceinline__ uint32_t shift_pair(const Half<P>& a, const Half<P>& b, const uint2 ia, const uint2 ib,
+                                               const P step, const P back, const P w, Half<P>& o01, uint2& i01,
+                                               Half<P>& o23, uint2& i23) {
+  using R = Real<P>;
+  const P FAR = R::far_away(), HALF_FAR = FAR * (P)0.5;
+  // lines 7-14 (L299-312): own disks that stay; a sentinel stays a sentinel and fails the test
+  Disk<P> o0 = {a.x.x, a.y.x, ia.x}, o1 = {a.x.y, a.y.y, ia.y};
+  const P a0 = R::add(ALONG_X ? o0.x : o0.y, step), a1 = R::add(ALONG_X ? o1.x : o1.y, step);
+  if (ALONG_X) { o0.x = a0; o1.x = a1; } else { o0.y = a0; o1.y = a1; }
+  const bool k0 = a0 > (P)0 && a0 <= w, k1 = a1 > (P)0 && a1 <= w;
+  // lines 17-27 (L319-339): disks of the neighbour that left it enter here; L332 is a separate operation
+  Disk<P> e0 = {b.x.x, b.y.x, ib.x}, e1 = {b.x.y, b.y.y, ib.y};
+  const bool v0 = e0.x < HALF_FAR, v1 = e1.x < HALF_FAR;          // occupied slots of the neighbour
+  const P b0 = R::add(ALONG_X ? e0.x : e0.y, step), b1 = R::add(ALONG_X ? e1.x : e1.y, step);
+  const bool g0 = v0 && !(b0 > (P)0 && b0 <= w), g1 = v1 && !(b1 > (P)0 && b1 <= w);
+  const P c0 = R::add(b0, back), c1 = R::add(b1, back);
+  if (ALONG_X) { e0.x = c0; e1.x = c1; } else { e0.y = c0; e1.y = c1; }
+  const Disk<P> none = {FAR, FAR, 0xFFFFFFFFu};
+  const uint32_t ns = (k0 ? 1u : 0u) + (k1 ? 1u : 0u), ne = (g0 ? 1u : 0u) + (g1 ? 1u : 0u);
+  const Disk<P> s0 = pick(k0, o0, o1);
+  const Disk<P> t0 = pick(ne > 0u, pick(g0, e0, e1), none), t1 = pick(ne > 1u, e1, none);
+  const Disk<P> r0 = pick(ns > 0u, s0, t0);
+  const Disk<P> r1 = pick(ns == 2u, o1, pick(ns == 1u, t0, t1));
+  const Disk<P> r2 = pick(ns == 2u, t0, pick(ns == 1u, t1, none));
+  const Disk<P> r3 = pick(ns == 2u, t1, none);
+  o01.x = R::pair(r0.x, r1.x); o01.y = R::pair(r0.y, r1.y); i01 = make_uint2(r0.id, r1.id);
+  o23.x = R::pair(r2.x, r3.x); o23.y = R::pair(r2.y, r3.y); i23 = make_uint2(r2.id, r3.id);
+  return ns + ne;
+}
+
 // one new cell; ALONG_X and POSITIVE are uniform across the grid, so the caller branches once
 template <typename P, bool ALONG_X, bool POSITIVE>
 __device__ __forceinline__ void shift_cell(const Params& p, Ctl* ctl, const uint32_t cur, const uint32_t Q,
-                                           const uint32_t ci, const P delta) {
+                                           const uint32_t ci, const P delta, uint32_t* crowded) {
   using R = Real<P>;
   const uint32_t nxt = cur ^ 1u, Mqp = p.Mqp;
   const uint8_t* cntc = p.cnt[cur];
@@ -471,36 +506,11 @@ __device__ __forceinline__ void shift_cell(const Params& p, Ctl* ctl, const uint
   const uint2 ia = idsc[own], ib = idsc[nb];
   uint32_t nn;
   if (n0 <= 2u && n1 <= 2u) {
-    // lines 7-14 (L299-312): own disks that stay; a sentinel stays a sentinel and fails the test
-    Disk<P> o0 = {a.x.x, a.y.x, ia.x}, o1 = {a.x.y, a.y.y, ia.y};
-    const P a0 = R::add(ALONG_X ? o0.x : o0.y, step), a1 = R::add(ALONG_X ? o1.x : o1.y, step);
-    if (ALONG_X) { o0.x = a0; o1.x = a1; } else { o0.y = a0; o1.y = a1; }
-    const bool k0 = a0 > (P)0 && a0 <= w, k1 = a1 > (P)0 && a1 <= w;
-    // lines 17-27 (L319-339): disks of the neighbour that left it enter here; L332 is a separate operation
-    Disk<P> e0 = {b.x.x, b.y.x, ib.x}, e1 = {b.x.y, b.y.y, ib.y};
-    const P b0 = R::add(ALONG_X ? e0.x : e0.y, step), b1 = R::add(ALONG_X ? e1.x : e1.y, step);
-    const bool g0 = n1 > 0u && !(b0 > (P)0 && b0 <= w), g1 = n1 > 1u && !(b1 > (P)0 && b1 <= w);
-    const P c0 = R::add(b0, back), c1 = R::add(b1, back);
-    if (ALONG_X) { e0.x = c0; e1.x = c1; } else { e0.y = c0; e1.y = c1; }
-    // compaction: stayers in slot order, then entrants in slot order (reading A13)
-    const Disk<P> none = {FAR, FAR, 0xFFFFFFFFu};
-    const uint32_t ns = (k0 ? 1u : 0u) + (k1 ? 1u : 0u), ne = (g0 ? 1u : 0u) + (g1 ? 1u : 0u);
-    const Disk<P> s0 = pick(k0, o0, o1);
-    const Disk<P> t0 = pick(ne > 0u, pick(g0, e0, e1), none), t1 = pick(ne > 1u, e1, none);
-    const Disk<P> r0 = pick(ns > 0u, s0, t0);
-    const Disk<P> r1 = pick(ns == 2u, o1, pick(ns == 1u, t0, t1));
-    nn = ns + ne;
-    Half<P> o;
-    o.x = R::pair(r0.x, r1.x); o.y = R::pair(r0.y, r1.y);
-    st_half(posn, own, o);
-    idsn[own] = make_uint2(r0.id, r1.id);
-    if (nn > 2u) {
-      const Disk<P> r2 = pick(ns == 2u, t0, pick(ns == 1u, t1, none));
-      const Disk<P> r3 = pick(ns == 2u, t1, none);
-      o.x = R::pair(r2.x, r3.x); o.y = R::pair(r2.y, r3.y);
-      st_half(posn, own + Mqp, o);
-      idsn[own + Mqp] = make_uint2(r2.id, r3.id);
-    }
+    Half<P> o01, o23; uint2 i01, i23;
+    nn = shift_pair<P, ALONG_X>(a, b, ia, ib, step, back, w, o01, i01, o23, i23);
+    st_half(posn, own, o01);
+    idsn[own] = i01;
+    if (nn > 2u) { st_half(posn, own + Mqp, o23); idsn[own + Mqp] = i23; }
   } else {
     // generic: any occupancy, rolled loops, scalar accesses
     nn = 0;
@@ -535,6 +545,7 @@ __device__ __forceinline__ void shift_cell(const Params& p, Ctl* ctl, const uint
     }
   }
   if (nn > (uint32_t)NMAX) { atomicOr(&ctl->err, ERRBIT_OVERFLOW); nn = NMAX; }
+  if (nn > 2u) *crowded = 1u;                    // the new state needs the general kernel (tile.cuh)
   p.cnt[nxt][Q * Mqp + ci] = (uint8_t)nn;        // L280, L342
 }
 
@@ -564,19 +575,19 @@ __device__ __forceinline__ void grid_barrier(uint32_t* bar, uint32_t& target) {
 constexpr uint32_t OP_SWEEPS = 0, OP_SUB_SWEEP = 1, OP_SHIFT = 2;
 
 // ---------------------------------------------------------------------------------------------------------
-// The persistent sweep kernel: k sweeps of Algorithm 1 (L60-93) in ONE cooperative launch.  Each sweep is four
+// The persistent sweep kernel: any number of sweeps of Algorithm 1 (L60-93) in ONE cooperative launch.  Each sweep is four
 // sub-sweep phases (the sets in the order drawn for this sweep, Alg. 1 line 2) and the shift phase (lines
 // 15-17), separated by grid barriers.  Every block owns a contiguous range of the active plane per phase (equal
 // shares, so the SMs finish together) and walks it blockDim.x cells at a time; the draws of a sweep are a pure
 // function of (seed, sweep index) and are recomputed by every block, so nothing but the barrier counter is
 // shared between blocks during the launch.  Block 0 writes the control block back at the end.
-//   op = OP_SWEEPS: k sweeps.  OP_SUB_SWEEP (test hook): one sub-sweep of set `arg` at the current sweep index.
+//   op = OP_SWEEPS: sweeps until the sweep index reaches t_end (none if it already has).  OP_SUB_SWEEP (test hook): one sub-sweep of set `arg` at the current sweep index.
 //   OP_SHIFT (test hook): one shift with direction `arg` and distance `delta_in`; the sweep index stays.
 // FAST selects update_cell_fast (w ~ sigma) or update_cell_general.
 // ---------------------------------------------------------------------------------------------------------
 template <typename P, int NS, bool DEBUG, bool FAST>
 __global__ void __launch_bounds__(SUB_THREADS, FAST ? (sizeof(P) == 4 ? FAST_MINB : FAST_MINB / 2) : SUB_MINB)
-k_sweeps(const __grid_constant__ Params p, const uint32_t k, const uint32_t op, const uint32_t arg,
+k_sweeps(const __grid_constant__ Params p, const unsigned long long t_end, const uint32_t op, const uint32_t arg,
          const double delta_in) {
   using R = Real<P>;
   __shared__ Draws sdraw;
@@ -601,16 +612,16 @@ k_sweeps(const __grid_constant__ Params p, const uint32_t k, const uint32_t op, 
       else                update_cell_general<P, NS, DEBUG>(p, Q, t, cur, ci, ci < sub_hi, tally);
     }
   };
-  auto shift_phase = [&](const uint32_t dir, const P delta) {
+  auto shift_phase = [&](const uint32_t dir, const P delta, uint32_t* crowded) {
     const bool along_x = dir < 2, positive = (dir & 1u) == 0;
     for (uint32_t g = all_lo + threadIdx.x; g < all_hi; g += SUB_THREADS) {
       const uint32_t Q = g / p.Mq, ci = g - Q * p.Mq;
       if (along_x) {
-        if (positive) shift_cell<P, true, true>(p, ctl, cur, Q, ci, delta);
-        else          shift_cell<P, true, false>(p, ctl, cur, Q, ci, delta);
+        if (positive) shift_cell<P, true, true>(p, ctl, cur, Q, ci, delta, crowded);
+        else          shift_cell<P, true, false>(p, ctl, cur, Q, ci, delta, crowded);
       } else {
-        if (positive) shift_cell<P, false, true>(p, ctl, cur, Q, ci, delta);
-        else          shift_cell<P, false, false>(p, ctl, cur, Q, ci, delta);
+        if (positive) shift_cell<P, false, true>(p, ctl, cur, Q, ci, delta, crowded);
+        else          shift_cell<P, false, false>(p, ctl, cur, Q, ci, delta, crowded);
       }
     }
     // the grid origin follows the shift (X = origin + cell*w + local stays put)
@@ -626,10 +637,17 @@ k_sweeps(const __grid_constant__ Params p, const uint32_t k, const uint32_t op, 
   if (op == OP_SUB_SWEEP) {
     sub_phase(arg & 3u);
   } else if (op == OP_SHIFT) {
-    shift_phase(arg & 3u, (P)delta_in);
+    // the state changes at an unchanged sweep index: its crowded flag is recomputed from scratch
+    if (b == 0 && threadIdx.x == 0) ctl->crowded[t & 3u] = 0u;
+    grid_barrier(&ctl->bar, target);
+    shift_phase(arg & 3u, (P)delta_in, &ctl->crowded[t & 3u]);
   } else {
+    const uint32_t k = t_end > t ? (uint32_t)(t_end - t) : 0u;
     for (uint32_t it = 0; it < k; ++it) {
-      if (threadIdx.x == 0) sdraw = draw_sweep(p, t);          // Alg. 1 lines 2, 15, 16 (L64, L90-91)
+      if (threadIdx.x == 0) {
+        sdraw = draw_sweep(p, t);                              // Alg. 1 lines 2, 15, 16 (L64, L90-91)
+        if (b == 0) ctl->crowded[(t + 2ull) & 3u] = 0u;        // slot of the sweep after next: nobody uses it now
+      }
       __syncthreads();
       const uint32_t dir = sdraw.dir, dist_word = sdraw.dist_word;
 #pragma unroll 1
@@ -639,7 +657,7 @@ k_sweeps(const __grid_constant__ Params p, const uint32_t k, const uint32_t op, 
       }
       // line 15 (L90): delta = uniform(0, w/2) = rn(rn(0.5 w) * u01)
       const P w = dir < 2 ? R::wx(p) : R::wy(p);
-      shift_phase(dir, R::mul(R::mul((P)0.5, w), R::unit(dist_word)));
+      shift_phase(dir, R::mul(R::mul((P)0.5, w), R::unit(dist_word)), &ctl->crowded[(t + 1ull) & 3u]);
       t += 1ull;
       if (it + 1u < k) grid_barrier(&ctl->bar, target);
     }
