@@ -79,8 +79,8 @@ int mpmc_geometry(const mpmc_ctx* ctx, uint32_t m[2], double w[2], double L_eff[
  * counters.  Synchronises; returns MPMC_ERR_OVERLAP / MPMC_ERR_CELL_OVERFLOW for bad input. */
 int mpmc_load_positions(mpmc_ctx* ctx, const double* xy);
 
-/* k full sweeps of Algorithm 1 (each: 4 sub-sweep kernels + 1 shift kernel, replayed from a CUDA graph).
- * Asynchronous.  All random draws, including the per-sweep set order and shift, are made on the device from
+/* k full sweeps of Algorithm 1 (four sub-sweeps + shift each): one fused tile-kernel launch per sweep where cells
+ * hold 0/1/2 disks (w ~ sigma), otherwise one persistent cooperative launch for all k.  Asynchronous.  All random draws, including the per-sweep set order and shift, are made on the device from
  * (seed, sweep index), so there is no host<->device traffic inside the loop. */
 int mpmc_sweep(mpmc_ctx* ctx, uint64_t k);
 
@@ -110,6 +110,11 @@ int mpmc_debug_shift(mpmc_ctx* ctx, uint32_t direction /*0:+x 1:-x 2:+y 3:-y*/, 
  * Synchronises. */
 int mpmc_debug_state(mpmc_ctx* ctx, void* counts, void* slab, void* ids, void* accept_mask, double origin[2],
                      uint64_t* sweep, uint64_t* digest);
+
+/* Test hook: out = host, {sweeps done by the fused tile kernel, sweeps done by the general persistent kernel} since
+ * the last load (the tile kernel serves cell widths w ~ sigma and hands a sweep to the general
+ * kernel only when more cells hold 3 or 4 disks than it can carry).  Synchronises. */
+int mpmc_debug_path(mpmc_ctx* ctx, uint64_t out[2]);
 
 /* Test hook: Philox4x32-10 evaluated ON THE DEVICE by the same routine the kernels use.
  * ctr = device u32[n][4], key = host u32[2], out = device u32[n][4]; enqueued on cuda_stream and synchronised. */

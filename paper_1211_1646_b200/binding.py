@@ -32,6 +32,7 @@ SYMBOLS = {
     "mpmc_debug_sub_sweep": (C.c_int, [_vp, _u32]),
     "mpmc_debug_shift": (C.c_int, [_vp, _u32, _dbl]),
     "mpmc_debug_state": (C.c_int, [_vp, _vp, _vp, _vp, _vp, C.POINTER(_dbl), C.POINTER(_u64), C.POINTER(_u64)]),
+    "mpmc_debug_path": (C.c_int, [_vp, C.POINTER(_u64)]),
     "mpmc_debug_philox": (C.c_int, [_vp, C.POINTER(_u32), _vp, _u32, _vp]),
     "mpmc_strerror": (C.c_char_p, [C.c_int]),
     "mpmc_version": (C.c_char_p, []),
@@ -201,6 +202,15 @@ class Mpmc:
             self._enter()
             _chk(lib().mpmc_debug_shift(self._h, int(direction), float(delta)))
             self._exit()
+
+    def path_sweeps(self) -> tuple:
+        """(sweeps done by the fused tile kernel, sweeps done by the general kernel) since the last load."""
+        out = (_u64 * 2)()
+        with self.torch.cuda.device(self.device):
+            self._enter()
+            _chk(lib().mpmc_debug_path(self._h, out))
+            self._exit()
+        return int(out[0]), int(out[1])
 
     def debug_state(self) -> dict:
         t = self.torch

@@ -15,9 +15,9 @@ __global__ void k_reset(const __grid_constant__ Params p) {
   if (g == 0) {
     Ctl* c = p.ctl;
     c->t = 0; c->cur = 0; c->err = 0; c->bar = 0; c->ticket = 0; c->pad0[0] = c->pad0[1] = 0;
-    c->crowded[0] = c->crowded[1] = c->crowded[2] = c->crowded[3] = 0;
+    for (int i = 0; i < 4; ++i) { c->crowded[i] = 0; c->ccount[i] = 0; }
     c->origin[0] = 0.0; c->origin[1] = 0.0;
-    c->digest = 0;
+    c->digest = 0; c->path_sweeps[0] = c->path_sweeps[1] = 0;
     for (uint32_t r = 0; r < CTR_SLOTS; ++r) c->counters[r][0] = c->counters[r][1] = c->counters[r][2] = c->counters[r][3] = 0;
   }
 }
@@ -71,7 +71,10 @@ __global__ void __launch_bounds__(AUX_THREADS) k_load_sort(const __grid_constant
   uint32_t n = p.cnt32[Q * p.Mqp + ci];
   if (n > (uint32_t)NMAX) n = NMAX;
   cnt_plane(p, 0, Q)[ci] = (uint8_t)n;
-  if (n > 2u) p.ctl->crowded[0] = 1u;            // sweep 0 starts from a state the tile kernel cannot hold
+  if (n > 2u) {                                  // crowded cell of the state at sweep 0 (tile.cuh)
+    const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
+    note_crowded(p.ctl, 0u, (2u * ya + (Q >> 1)) * p.mx + (2u * xa + (Q & 1u)));
+  }
   uint32_t id[NMAX]; P2 v[NMAX];
 #pragma unroll
   for (int i = 0; i < NMAX; ++i) {

@@ -35,6 +35,7 @@ constexpr uint32_t ERRBIT_OVERFLOW = 1u;  // a cell would hold more than NMAX di
 constexpr uint32_t ERRBIT_RANGE = 2u;     // loaded coordinate NaN or outside [0, L]
 constexpr uint32_t ERRBIT_OVERLAP = 4u;   // loaded positions overlap
 constexpr uint32_t CTR_SLOTS = 64;        // rows of move counters (summed on read)
+constexpr uint32_t CROWD_CAP = 256;       // cells with more than 2 disks the tile kernel can carry per state
 
 // Device-resident control block: the state that survives between launches.  Inside a launch the sweep index,
 // buffer parity, grid origin and per-sweep draws live in registers / shared memory (sweep.cuh, k_sweeps).
@@ -44,10 +45,17 @@ struct Ctl {
   uint32_t err;                    // sticky error bits
   uint32_t bar;                    // arrival counter of the grid barrier (zeroed by the host before a launch)
   uint32_t ticket;                 // blocks-done counter of the tile kernel
-  uint32_t crowded[4];             // crowded[t & 3] != 0: at sweep t some cell holds more than 2 disks (tile.cuh)
+  // Cells holding more than 2 disks ("crowded") in the state at sweep t, kept per (t & 3): ccount = how many,
+  // clist = their canonical ids y*mx+x in no particular order; crowded != 0: more than CROWD_CAP of them, the
+  // list is incomplete and the tile kernel (tile.cuh) must leave this state to the general kernel.  Written by
+  // whichever kernel produces the state; a slot is cleared two sweeps ahead of its use.
+  uint32_t crowded[4];
+  uint32_t ccount[4];
   uint32_t pad0[2];
+  uint32_t clist[4][CROWD_CAP];
   double origin[2];                // grid origin: X = origin + cell * w + local
   unsigned long long digest;       // accept-sequence digest (MPMC_DEBUG)
+  unsigned long long path_sweeps[2];  // sweeps done by the tile kernel / by the general kernel since the last load
   unsigned long long counters[CTR_SLOTS][4];  // per row: accepted, rejected_boundary, rejected_overlap, -
 };
 
@@ -57,9 +65,9 @@ struct Params {
   uint32_t Mq, Mqp;          // cells per colour; plane stride (Mq rounded up to 64)
   uint32_t n_s, N;
   uint32_t hx_magic, hx_sh1, hx_sh2;  // ci / hx without a divide (Granlund-Montgomery; host: div_magic)
-  uint32_t tl_ntx, tl_nty, tl_PS, tl_single;  // tile kernel: tiles per axis, shared-memory plane stride (cells),
-                                              // 1 if a loaded region wraps around the box at most once
+  uint32_t tl_ntx, tl_nty, tl_PS;       // tile kernel: tiles per axis, shared-memory plane stride (cells)
   uint32_t seed_lo, seed_hi;
+  uint32_t rk0[10], rk1[10];            // Philox round keys seed + r * Weyl constant (philox4x32_10_rk)
   float wx_f, wy_f, sigma2_f, d_f;      // working-precision constants (fp32 mode)
   double wx_p, wy_p, sigma2_p, d_p;     // working-precision constants (fp64 mode)
   float dsc_f; double dsc_p;            // d 2^-24 (fp32) / d 2^-32 (fp64): displacement = dsc * odd integer
@@ -148,6 +156,30 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
     k1 += 0xBB67AE85u;
   }
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// The same function with the ten round keys of the run's seed taken from the kernel parameters (constant bank):
+// the key schedule costs no instruction.
+__device__ __forceinline__ void philox4x32_10_rk(const Params& p, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                 uint32_t (&out)[4]) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;
+    const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ p.rk0[r];
+    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ p.rk1[r];
+    c1 = (uint32_t)p1;
+    c3 = (uint32_t)p0;
+    c0 = n0;
+    c2 = n2;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// a kernel that writes a cell with more than 2 disks into the state of sweep slot `slot` records it here
+__device__ __forceinline__ void note_crowded(Ctl* ctl, uint32_t slot, uint32_t cell) {
+  const uint32_t i = atomicAdd(&ctl->ccount[slot], 1u);
+  if (i < CROWD_CAP) ctl->clist[slot][i] = cell; else ctl->crowded[slot] = 1u;
 }
 
 __device__ __forceinline__ uint32_t bounded(uint32_t word, uint32_t bound) { return __umulhi(word, bound); }

@@ -145,15 +145,17 @@ const void* pick_tile_kernel(bool fp32, bool debug, uint32_t n_s) {
 
 // Tiling of the tile kernel: ntx x nty tiles of (nearly) equal even size whose loaded region (tile + 2 HALO) fits
 // the shared memory of one SM; among those, the one with the least work on the busiest SM:
-// waves * cells of the largest region.  Returns false if not even a 2 x 2 tile fits.
+// waves * cells of the largest region.  Returns false if no such tiling exists (boxes under 12 cells across).
 bool choose_tiling(uint32_t hx, uint32_t hy, size_t cell_bytes, size_t smem_max, uint32_t sms, uint32_t* ntx, uint32_t* nty,
                    uint32_t* PS) {
   double best = 0; bool found = false;
   const uint32_t lim = 1024;
   for (uint32_t ax = 1; ax <= hx && ax <= lim; ++ax) {
     const uint32_t TX = 2 * ((hx + ax - 1) / ax), pw = (TX + 2 * HALO) / 2;
+    if (TX + 2 * HALO > 2 * hx) continue;           // a region must not overlap itself around the box
     for (uint32_t ay = 1; ay <= hy && ay <= lim; ++ay) {
       const uint32_t TY = 2 * ((hy + ay - 1) / ay), ph = (TY + 2 * HALO) / 2;
+      if (TY + 2 * HALO > 2 * hy) continue;
       const size_t bytes = (size_t)4 * pw * ph * cell_bytes;
       if (bytes > smem_max || pw * ph >= 16384u) continue;
       const double waves = std::ceil((double)ax * ay / sms);
@@ -250,6 +252,7 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   p.Mq = L.Mq; p.Mqp = L.Mqp; p.n_s = n_s; p.N = (uint32_t)N;
   div_magic(p.hx, &p.hx_magic, &p.hx_sh1, &p.hx_sh2);
   p.seed_lo = (uint32_t)seed; p.seed_hi = (uint32_t)(seed >> 32);
+  for (uint32_t r = 0; r < 10; ++r) { p.rk0[r] = p.seed_lo + r * 0x9E3779B9u; p.rk1[r] = p.seed_hi + r * 0xBB67AE85u; }
   p.wx_f = (float)g.w0[0]; p.wy_f = (float)g.w0[1];
   p.sigma2_f = (float)sigma * (float)sigma; p.d_f = (float)d;
   p.dsc_f = p.d_f * 0x1p-24f; p.dsc_p = d * 0x1p-32;
@@ -288,14 +291,14 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
     int smem_optin = 0;
     cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     const size_t cell_bytes = fp32 ? sizeof(SmemCell<float>) : sizeof(SmemCell<double>);
-    const size_t smem_max = smem_optin > 2048 ? (size_t)smem_optin - 1024 : 0;   // static shared memory: draws, flags
+    const size_t stat = (fp32 ? sizeof(CrowdList<float>) : sizeof(CrowdList<double>)) + 256;   // static shared memory
+    const size_t smem_max = (size_t)smem_optin > stat ? (size_t)smem_optin - stat : 0;
     uint32_t ntx = 0, nty = 0, PS = 0;
     if (choose_tiling(p.hx, p.hy, cell_bytes, smem_max, (uint32_t)sms, &ntx, &nty, &PS)) {
       c->tile_kernel = pick_tile_kernel(fp32, debug, n_s);
       c->tile_grid = ntx * nty;
       c->tile_smem = (size_t)4 * PS * cell_bytes;
       p.tl_ntx = ntx; p.tl_nty = nty; p.tl_PS = PS;
-      p.tl_single = (p.mx >= 6 && p.my >= 6) ? 1u : 0u;
       if (std::getenv("MPMC_VERBOSE"))
         std::fprintf(stderr, "[mpmc] tile kernel: %u x %u tiles, plane stride %u cells, %zu B shared memory, grid %u; general grid %u\n",
                      ntx, nty, PS, c->tile_smem, c->tile_grid, c->grid);
@@ -459,6 +462,15 @@ int mpmc_debug_state(mpmc_ctx* c, void* counts, void* slab, void* ids, void* acc
   if (origin) { origin[0] = h.origin[0]; origin[1] = h.origin[1]; }
   if (sweep) *sweep = h.t;
   if (digest) *digest = h.digest;
+  return st;
+}
+
+int mpmc_debug_path(mpmc_ctx* c, uint64_t out[2]) {
+  if (!c || !out) return MPMC_ERR_ARG;
+  if (!c->loaded) return MPMC_ERR_STATE;
+  Ctl h;
+  const int st = read_ctl(c, &h);
+  out[0] = h.path_sweeps[0]; out[1] = h.path_sweeps[1];
   return st;
 }
 

@@ -473,7 +473,7 @@ __device__ __forceinline__ uint32_t shift_pair(const Half<P>& a, const Half<P>& 
 // one new cell; ALONG_X and POSITIVE are uniform across the grid, so the caller branches once
 template <typename P, bool ALONG_X, bool POSITIVE>
 __device__ __forceinline__ void shift_cell(const Params& p, Ctl* ctl, const uint32_t cur, const uint32_t Q,
-                                           const uint32_t ci, const P delta, uint32_t* crowded) {
+                                           const uint32_t ci, const P delta, const uint32_t crowd_slot) {
   using R = Real<P>;
   const uint32_t nxt = cur ^ 1u, Mqp = p.Mqp;
   const uint8_t* cntc = p.cnt[cur];
@@ -545,7 +545,10 @@ __device__ __forceinline__ void shift_cell(const Params& p, Ctl* ctl, const uint
     }
   }
   if (nn > (uint32_t)NMAX) { atomicOr(&ctl->err, ERRBIT_OVERFLOW); nn = NMAX; }
-  if (nn > 2u) *crowded = 1u;                    // the new state needs the general kernel (tile.cuh)
+  if (nn > 2u) {                                 // crowded cell of the new state (tile.cuh)
+    const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
+    note_crowded(ctl, crowd_slot, (2u * ya + offy) * p.mx + (2u * xa + offx));
+  }
   p.cnt[nxt][Q * Mqp + ci] = (uint8_t)nn;        // L280, L342
 }
 
@@ -612,7 +615,7 @@ k_sweeps(const __grid_constant__ Params p, const unsigned long long t_end, const
       else                update_cell_general<P, NS, DEBUG>(p, Q, t, cur, ci, ci < sub_hi, tally);
     }
   };
-  auto shift_phase = [&](const uint32_t dir, const P delta, uint32_t* crowded) {
+  auto shift_phase = [&](const uint32_t dir, const P delta, const uint32_t crowded) {
     const bool along_x = dir < 2, positive = (dir & 1u) == 0;
     for (uint32_t g = all_lo + threadIdx.x; g < all_hi; g += SUB_THREADS) {
       const uint32_t Q = g / p.Mq, ci = g - Q * p.Mq;
@@ -638,15 +641,15 @@ k_sweeps(const __grid_constant__ Params p, const unsigned long long t_end, const
     sub_phase(arg & 3u);
   } else if (op == OP_SHIFT) {
     // the state changes at an unchanged sweep index: its crowded flag is recomputed from scratch
-    if (b == 0 && threadIdx.x == 0) ctl->crowded[t & 3u] = 0u;
+    if (b == 0 && threadIdx.x == 0) { ctl->crowded[t & 3u] = 0u; ctl->ccount[t & 3u] = 0u; }
     grid_barrier(&ctl->bar, target);
-    shift_phase(arg & 3u, (P)delta_in, &ctl->crowded[t & 3u]);
+    shift_phase(arg & 3u, (P)delta_in, (uint32_t)(t & 3u));
   } else {
     const uint32_t k = t_end > t ? (uint32_t)(t_end - t) : 0u;
     for (uint32_t it = 0; it < k; ++it) {
       if (threadIdx.x == 0) {
         sdraw = draw_sweep(p, t);                              // Alg. 1 lines 2, 15, 16 (L64, L90-91)
-        if (b == 0) ctl->crowded[(t + 2ull) & 3u] = 0u;        // slot of the sweep after next: nobody uses it now
+        if (b == 0) { ctl->crowded[(t + 2ull) & 3u] = 0u; ctl->ccount[(t + 2ull) & 3u] = 0u; }   // sweep after next
       }
       __syncthreads();
       const uint32_t dir = sdraw.dir, dist_word = sdraw.dist_word;
@@ -657,14 +660,17 @@ k_sweeps(const __grid_constant__ Params p, const unsigned long long t_end, const
       }
       // line 15 (L90): delta = uniform(0, w/2) = rn(rn(0.5 w) * u01)
       const P w = dir < 2 ? R::wx(p) : R::wy(p);
-      shift_phase(dir, R::mul(R::mul((P)0.5, w), R::unit(dist_word)), &ctl->crowded[(t + 1ull) & 3u]);
+      shift_phase(dir, R::mul(R::mul((P)0.5, w), R::unit(dist_word)), (uint32_t)((t + 1ull) & 3u));
       t += 1ull;
       if (it + 1u < k) grid_barrier(&ctl->bar, target);
     }
   }
   flush_tally(p, tally);
   if (op == OP_SHIFT) grid_barrier(&ctl->bar, target);   // every block has read the control block before it changes
-  if (b == 0 && threadIdx.x == 0) { ctl->t = t; ctl->cur = cur; ctl->origin[0] = ox; ctl->origin[1] = oy; }
+  if (b == 0 && threadIdx.x == 0) {
+    if (op == OP_SWEEPS) ctl->path_sweeps[1] += t - ctl->t;
+    ctl->t = t; ctl->cur = cur; ctl->origin[0] = ox; ctl->origin[1] = oy;
+  }
 }
 
 }  // namespace mpmc

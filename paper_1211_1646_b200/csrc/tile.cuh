@@ -16,11 +16,15 @@
 // identical results: the trajectory is bit-identical to the one-kernel-per-sub-sweep path and to the oracle.
 // Moves are tallied for interior cells only.
 //
-// Precondition: no cell of the system holds more than 2 disks (then slot pair 0 + sentinels is the whole state
-// and counts are implied: a slot is empty iff it holds the sentinel).  The flag Ctl::crowded[t & 3] says whether
-// the state at sweep t violates it; it is maintained by every kernel that writes cell counts.  A crowded state
-// makes this kernel return at once, and the general persistent kernel (sweep.cuh k_sweeps), which mpmc_sweep
-// always enqueues behind the tile kernels with the target sweep index, runs the remaining sweeps.
+// Cells with more than 2 disks ("crowded"; about one in a million at phi = 0.716, w ~ sigma): shared memory holds
+// slot pair 0 only, where a slot is empty iff it holds the sentinel, so counts are implied.  The few crowded cells
+// of the state are listed in the control block (Ctl::clist, maintained by every kernel that writes cell counts);
+// a CTA copies those inside its region, with their slots 2 and 3, into a small shared-memory list, and a cell whose
+// 3x3 neighbourhood (or, in the shift, whose source neighbour) touches a listed cell takes a rolled general path.
+// With more than CROWD_CAP crowded cells (Ctl::crowded) this kernel returns at once, and the general persistent
+// kernel (sweep.cuh k_sweeps), which mpmc_sweep always enqueues behind the tile kernels with the target sweep
+// index, runs the remaining sweeps.  The host only tiles boxes in which a loaded region never overlaps itself
+// (tile + 2 HALO <= box), so every cell appears at most once in a region.
 #pragma once
 #include "common.cuh"
 #include "sweep.cuh"
@@ -31,9 +35,11 @@ namespace mpmc {
 template <typename P> struct TileThreads { static constexpr int value = sizeof(P) == 4 ? 768 : 384; };
 constexpr int HALO = 5;
 
-__device__ __forceinline__ uint32_t wrap_cell(int v, uint32_t m, bool single) {
-  if (single) { if (v < 0) v += (int)m; else if (v >= (int)m) v -= (int)m; return (uint32_t)v; }
-  int r = v % (int)m; if (r < 0) r += (int)m; return (uint32_t)r;
+// v in [-m, 2m) -> [0, m)
+__device__ __forceinline__ uint32_t wrap_cell(int v, uint32_t m) {
+  if (v < 0) v += (int)m;
+  if (v >= (int)m) v -= (int)m;
+  return (uint32_t)v;
 }
 
 template <typename P> struct SmemCell;                        // slot pair 0 of a cell: {x0, x1, y0, y1}
@@ -68,41 +74,141 @@ __device__ __forceinline__ TileBox tile_box(const Params& p, uint32_t tx, uint32
   return b;
 }
 
+// A crowded cell inside the loaded region: where it is, and its slots 2 and 3 (slot pair 1 of global memory).
+template <typename P> struct CrowdEntry { uint32_t si; uint32_t lxly; Half<P> hi; };   // lxly = lx | ly << 16
+template <typename P> struct CrowdList { uint32_t n; CrowdEntry<P> e[CROWD_CAP]; };
+
+template <typename P>
+__device__ __forceinline__ int crowd_find(const CrowdList<P>& cl, uint32_t nc, uint32_t si) {
+  for (uint32_t i = 0; i < nc; ++i) if (cl.e[i].si == si) return (int)i;
+  return -1;
+}
+// does the 3x3 neighbourhood of the cell at local coordinates (lx, ly) contain a listed cell?
+template <typename P>
+__device__ __forceinline__ bool crowd_near(const CrowdList<P>& cl, uint32_t nc, uint32_t lx, uint32_t ly) {
+  bool near = false;
+  for (uint32_t i = 0; i < nc; ++i) {
+    const uint32_t v = cl.e[i].lxly;
+    near |= (lx - (v & 0xFFFFu) + 1u <= 2u) && (ly - (v >> 16) + 1u <= 2u);
+  }
+  return near;
+}
+
+// shared-memory offsets of the 3x3 cells relative to an active cell of local colour q (uniform per phase)
+__device__ __forceinline__ int neighbour_offset(uint32_t q, int ox, int oy, uint32_t PS, uint32_t pw) {
+  const int qx = (int)(q & 1u), qy = (int)(q >> 1);
+  const int qn = ((qy ^ (oy & 1)) << 1) | (qx ^ (ox & 1));
+  const int dx = ox < 0 ? qx - 1 : ox > 0 ? qx : 0, dy = oy < 0 ? qy - 1 : oy > 0 ? qy : 0;
+  return (qn - (int)q) * (int)PS + dy * (int)pw + dx;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// General cell update on the tile (rare: a crowded cell in the 3x3 neighbourhood): Algorithm 2 line by line,
+// rolled loops, up to 4 disks per cell (slots 0, 1 from the planes, slots 2, 3 from the crowd list).
+// ---------------------------------------------------------------------------------------------------------
+template <typename P, bool DEBUG>
+__device__ __noinline__ void tile_update_cell_general(const Params& p, SmemCell<P>* sm, CrowdList<P>& cl, const uint32_t nc,
+                                                      const uint32_t q, const uint32_t pw, const uint32_t si_own, const uint32_t cell,
+                                                      const bool interior, const unsigned long long t, Tally& tally) {
+  using R = Real<P>;
+  const uint32_t PS = p.tl_PS;
+  const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p);
+  const P FAR = R::far_away(), HALF_FAR = FAR * (P)0.5;
+  const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
+  // own disks (Alg. 2 line 8, L186)
+  P lx[NMAX], ly[NMAX];
+  const Half<P> h0 = lds_half(sm, si_own);
+  const int eo = crowd_find(cl, nc, si_own);
+  lx[0] = h0.x.x; lx[1] = h0.x.y; ly[0] = h0.y.x; ly[1] = h0.y.y;
+  lx[2] = lx[3] = ly[2] = ly[3] = FAR;
+  if (eo >= 0) { lx[2] = cl.e[eo].hi.x.x; lx[3] = cl.e[eo].hi.x.y; ly[2] = cl.e[eo].hi.y.x; ly[3] = cl.e[eo].hi.y.y; }
+  uint32_t n = 0;
+  while (n < (uint32_t)NMAX && lx[n] < HALF_FAR) ++n;
+  uint32_t n_acc = 0, n_rb = 0, n_ro = 0, amask = 0;
+  if (n > 0u) {
+    // the disks of the 8 neighbour cells, translated into this cell's frame once: q = l_j + s, s = (ox wx, oy wy)
+    // (L154, L196) — the moves below only read them
+    P nx[8 * NMAX], ny[8 * NMAX];
+    uint32_t nnb = 0;
+#pragma unroll 1
+    for (int idx = 0; idx < 9; ++idx) {
+      if (idx == 4) continue;
+      const int ox = idx % 3 - 1, oy = idx / 3 - 1;
+      const P sx = ox < 0 ? -wx : ox > 0 ? wx : (P)0, sy = oy < 0 ? -wy : oy > 0 ? wy : (P)0;
+      const uint32_t si = (uint32_t)((int)si_own + neighbour_offset(q, ox, oy, PS, pw));
+      const Half<P> h = lds_half(sm, si);
+      if (h.x.x < HALF_FAR) { nx[nnb] = R::add(h.x.x, sx); ny[nnb] = R::add(h.y.x, sy); ++nnb; }
+      if (h.x.y < HALF_FAR) { nx[nnb] = R::add(h.x.y, sx); ny[nnb] = R::add(h.y.y, sy); ++nnb; }
+      const int en = crowd_find(cl, nc, si);
+      if (en >= 0) {
+        const Half<P> g = cl.e[en].hi;
+        if (g.x.x < HALF_FAR) { nx[nnb] = R::add(g.x.x, sx); ny[nnb] = R::add(g.y.x, sy); ++nnb; }
+        if (g.x.y < HALF_FAR) { nx[nnb] = R::add(g.x.y, sx); ny[nnb] = R::add(g.y.y, sy); ++nnb; }
+      }
+    }
+    uint32_t perm = 0x3210u;
+    if (n >= 2u) {                                               // line 9 (L187)
+      uint32_t S[4];
+      philox4x32_10_rk(p, cell, t_lo, t_hi, SLOT_SHUFFLE, S);
+      perm = visiting_permutation(n, S);
+    }
+    uint32_t vi = 0;
+    uint32_t Rw[4] = {0, 0, 0, 0};
+#pragma unroll 1
+    for (uint32_t s = 0; s < p.n_s; ++s) {                       // lines 11-32 (L189-230)
+      if ((s & 1u) == 0u) philox4x32_10_rk(p, cell, t_lo, t_hi, s >> 1, Rw);
+      const uint32_t k = (perm >> (4u * vi)) & 3u;               // p <- particles[s mod n]  (L75)
+      vi = (vi + 1u == n) ? 0u : vi + 1u;
+      const uint32_t r0 = (s & 1u) ? Rw[2] : Rw[0], r1 = (s & 1u) ? Rw[3] : Rw[1];
+      const P Mx = R::add(lx[k], R::scaled_sym(p, r0)), My = R::add(ly[k], R::scaled_sym(p, r1));
+      if (!((Mx > (P)0) && (Mx <= wx) && (My > (P)0) && (My <= wy))) { ++n_rb; continue; }   // (0, w]  (A3)
+      bool ov = false;
+      for (uint32_t j = 0; j < n; ++j) {                         // own cell: s = 0, so q = l_j; line 17 skips j = k
+        if (j == k) continue;
+        const P Dx = R::sub(Mx, lx[j]), Dy = R::sub(My, ly[j]);
+        ov |= R::fma(Dx, Dx, R::mul(Dy, Dy)) < sigma2;
+      }
+      for (uint32_t j = 0; j < nnb; ++j) {                       // line 19 (L204), strict (A4)
+        const P Dx = R::sub(Mx, nx[j]), Dy = R::sub(My, ny[j]);
+        ov |= R::fma(Dx, Dx, R::mul(Dy, Dy)) < sigma2;
+      }
+      if (ov) { ++n_ro; }
+      else { ++n_acc; amask |= 1u << (s & 31u); lx[k] = Mx; ly[k] = My; }   // lines 24-27 (L215-222)
+    }
+    if (amask != 0u) {                                           // write back (line 34, L234)
+      Half<P> o;
+      o.x = R::pair(lx[0], lx[1]); o.y = R::pair(ly[0], ly[1]);
+      sts_half(sm, si_own, o);
+      if (eo >= 0) { cl.e[eo].hi.x = R::pair(lx[2], lx[3]); cl.e[eo].hi.y = R::pair(ly[2], ly[3]); }
+    }
+  }
+  if (interior && n > 0u) { tally.acc += n_acc; tally.rb += n_rb; tally.ro += n_ro; }
+  if (DEBUG && interior) {
+    p.mask[cell] = amask;
+    if (n > 0u) atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)cell << 32) | amask)));
+  }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // One cell update (Algorithm 2) on the tile in shared memory: the arithmetic of update_cell_fast
-// (sweep.cuh), neighbours read with one LDS.128 each.  (px, py): position in the plane of local colour q.
+// (sweep.cuh), the 3x3 cells read with one LDS.128 each at si_own + noff[idx] (offsets uniform per phase).
 // ---------------------------------------------------------------------------------------------------------
 template <typename P, int NS, bool DEBUG>
-__device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* sm, const TileBox& tb, const uint32_t q,
-                                                 const uint32_t px, const uint32_t py, const bool active,
-                                                 const unsigned long long t, const bool single, Tally& tally) {
+__device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* sm, const uint32_t si_own,
+                                                 const int (&noff)[9], const uint32_t cell, const bool interior,
+                                                 const unsigned long long t, Tally& tally) {
   using R = Real<P>;
   using Pair = typename R::Pair;
-  const uint32_t qx = q & 1u, qy = q >> 1, PS = p.tl_PS, pw = tb.pw;
-  const uint32_t lx = 2u * px + qx, ly = 2u * py + qy;
-  // ---- the 3x3 cells from shared memory (idx 4 = own) ----
   Half<P> h[9];
-  uint32_t own_idx = 0;
 #pragma unroll
-  for (int idx = 0; idx < 9; ++idx) {
-    const int ox = idx % 3 - 1, oy = idx / 3 - 1;
-    const uint32_t qn = ((qy ^ (uint32_t)(oy & 1)) << 1) | (qx ^ (uint32_t)(ox & 1));
-    const uint32_t pxn = px + (ox < 0 ? qx - 1u : ox > 0 ? qx : 0u);
-    const uint32_t pyn = py + (oy < 0 ? qy - 1u : oy > 0 ? qy : 0u);
-    const uint32_t si = qn * PS + pyn * pw + pxn;
-    if (idx == 4) own_idx = si;
-    h[idx] = lds_half(sm, si);
-  }
+  for (int idx = 0; idx < 9; ++idx) h[idx] = lds_half(sm, (uint32_t)((int)si_own + noff[idx]));
   // ---- displacements of all NS moves from the GLOBAL cell id (line 12, L190; A2, A9) ----
-  const uint32_t gx = wrap_cell((int)tb.x0 - HALO + (int)lx, p.mx, single);
-  const uint32_t gy = wrap_cell((int)tb.y0 - HALO + (int)ly, p.my, single);
-  const uint32_t cell = gy * p.mx + gx;
   const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
   P ddx[NS], ddy[NS];
 #pragma unroll
   for (int b = 0; b < NS / 2; ++b) {
     uint32_t Rw[4];
-    philox4x32_10(cell, t_lo, t_hi, (uint32_t)b, p.seed_lo, p.seed_hi, Rw);
+    philox4x32_10_rk(p, cell, t_lo, t_hi, (uint32_t)b, Rw);
     ddx[2 * b] = R::scaled_sym(p, Rw[0]); ddy[2 * b] = R::scaled_sym(p, Rw[1]);
     ddx[2 * b + 1] = R::scaled_sym(p, Rw[2]); ddy[2 * b + 1] = R::scaled_sym(p, Rw[3]);
   }
@@ -123,12 +229,12 @@ __device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* s
   }
   // ---- own cell in visiting order (Alg. 2 lines 8-9, L186-187); a slot is empty iff it holds the sentinel ----
   P Ax = h[4].x.x, Ay = h[4].y.x, Bx = h[4].x.y, By = h[4].y.y;
-  const uint32_t n = !active ? 0u : (Bx < HALF_FAR ? 2u : (Ax < HALF_FAR ? 1u : 0u));
+  const uint32_t n = Bx < HALF_FAR ? 2u : (Ax < HALF_FAR ? 1u : 0u);
   const bool two = n == 2u;
   bool flip = false;                   // true: A is slot 1
   if (two) {                           // n = 2: Fisher-Yates is one draw, j = bounded(S0, 2); j = 0 swaps
     uint32_t S[4];
-    philox4x32_10(cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
+    philox4x32_10_rk(p, cell, t_lo, t_hi, SLOT_SHUFFLE, S);
     flip = bounded(S[0], 2u) == 0u;
   }
   if (flip) { P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }
@@ -152,20 +258,19 @@ __device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* s
     n_acc += acc ? 1u : 0u;
     if (two) { const P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }   // s mod n cycling (L75)
   }
-  if (n == 0u) amask = 0u;             // empty cells (and idle lanes) attempt nothing (A10)
+  if (n == 0u) amask = 0u;             // empty cells attempt nothing (A10)
   if (amask != 0u) {                   // write back (line 34, L234): the slot pair in slot order
     if (two && (NS & 1)) flip = !flip;
     Half<P> o;
     o.x = flip ? R::pair(Bx, Ax) : R::pair(Ax, Bx);
     o.y = flip ? R::pair(By, Ay) : R::pair(Ay, By);
-    sts_half(sm, own_idx, o);
+    sts_half(sm, si_own, o);
   }
   // tallies, accept masks and the digest count every cell once: in the tile that owns it
-  const bool interior = lx >= (uint32_t)HALO && lx < tb.TX + HALO && ly >= (uint32_t)HALO && ly < tb.TY + HALO;
   if (interior && n > 0u) {
     tally.acc += n_acc; tally.rb += n_rb; tally.ro += (uint32_t)NS - n_acc - n_rb;
   }
-  if (DEBUG && interior && active) {
+  if (DEBUG && interior) {
     p.mask[cell] = amask;
     if (n > 0u) atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)cell << 32) | amask)));
   }
@@ -174,6 +279,60 @@ __device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* s
 // floor(n / d) for n < 2^16, 1 <= d < 2^16 with the per-phase constant inv = ceil(2^32 / d) (0 stands for d = 1)
 __device__ __forceinline__ uint32_t small_div_magic(uint32_t d) { return d == 1u ? 0u : (uint32_t)(0xFFFFFFFFull / d) + 1u; }
 __device__ __forceinline__ uint32_t small_div(uint32_t n, uint32_t inv) { return inv == 0u ? n : __umulhi(n, inv); }
+
+// General shift of one interior cell (rare: it or its source neighbour is crowded): Algorithm 4 line by line.
+template <typename P>
+__device__ __noinline__ void tile_shift_cell_general(const Params& p, const SmemCell<P>* sm, const CrowdList<P>& cl,
+                                                     const uint32_t nc, const uint32_t si_own, const uint32_t si_nb,
+                                                     const uint32_t own_g, const uint32_t nb_g, const uint32_t cnt_g,
+                                                     const uint32_t cell, const bool along_x, const P step, const P back,
+                                                     const P w, const uint32_t cur, const uint32_t crowd_slot) {
+  using R = Real<P>;
+  const uint32_t nxt = cur ^ 1u, Mqp = p.Mqp;
+  const P FAR = R::far_away(), HALF_FAR = FAR * (P)0.5;
+  const uint2* idsc = reinterpret_cast<const uint2*>(p.ids[cur]);
+  P ox[NMAX + 1], oy[NMAX + 1]; uint32_t oid[NMAX + 1];
+  uint32_t nn = 0;
+#pragma unroll 1
+  for (uint32_t pass = 0; pass < 2u; ++pass) {                   // own disks that stay, then the neighbour's leavers
+    const uint32_t si = pass ? si_nb : si_own, g = pass ? nb_g : own_g;
+    const Half<P> h = lds_half(sm, si);
+    P jx[NMAX] = {h.x.x, h.x.y, FAR, FAR}, jy[NMAX] = {h.y.x, h.y.y, FAR, FAR};
+    uint32_t jid[NMAX] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
+    const uint2 i01 = idsc[g];
+    jid[0] = i01.x; jid[1] = i01.y;
+    const int e = crowd_find(cl, nc, si);
+    if (e >= 0) {
+      jx[2] = cl.e[e].hi.x.x; jx[3] = cl.e[e].hi.x.y; jy[2] = cl.e[e].hi.y.x; jy[3] = cl.e[e].hi.y.y;
+      const uint2 i23 = idsc[g + Mqp];
+      jid[2] = i23.x; jid[3] = i23.y;
+    }
+    for (uint32_t i = 0; i < (uint32_t)NMAX; ++i) {
+      if (!(jx[i] < HALF_FAR)) continue;                         // empty slot
+      P x = jx[i], y = jy[i];
+      P m = R::add(along_x ? x : y, step);                       // l' = l - f*delta  (L303)
+      const bool in = m > (P)0 && m <= w;
+      if (pass ? in : !in) continue;                             // own leavers go elsewhere; neighbour's stayers stay
+      if (pass) m = R::add(m, back);                             // L332, after the test (L352)
+      if (along_x) x = m; else y = m;
+      if (nn < (uint32_t)NMAX) { ox[nn] = x; oy[nn] = y; oid[nn] = jid[i]; }
+      ++nn;
+    }
+  }
+  if (nn > (uint32_t)NMAX) { atomicOr(&p.ctl->err, ERRBIT_OVERFLOW); nn = NMAX; }
+  for (uint32_t i = nn; i < (uint32_t)NMAX; ++i) { ox[i] = FAR; oy[i] = FAR; oid[i] = 0xFFFFFFFFu; }
+  P* posn = reinterpret_cast<P*>(p.pos[nxt]);
+  uint2* idsn = reinterpret_cast<uint2*>(p.ids[nxt]);
+  Half<P> o;
+  o.x = R::pair(ox[0], ox[1]); o.y = R::pair(oy[0], oy[1]);
+  st_half(posn, own_g, o); idsn[own_g] = make_uint2(oid[0], oid[1]);
+  if (nn > 2u) {
+    o.x = R::pair(ox[2], ox[3]); o.y = R::pair(oy[2], oy[3]);
+    st_half(posn, own_g + Mqp, o); idsn[own_g + Mqp] = make_uint2(oid[2], oid[3]);
+    note_crowded(p.ctl, crowd_slot, cell);
+  }
+  p.cnt[nxt][cnt_g] = (uint8_t)nn;
+}
 
 // ---------------------------------------------------------------------------------------------------------
 // The fused sweep kernel: one CTA per tile, one launch per sweep.  See the header of this file.
@@ -186,38 +345,57 @@ k_tile_sweep(const __grid_constant__ Params p) {
   constexpr uint32_t TILE_THREADS = TileThreads<P>::value;
   extern __shared__ __align__(16) unsigned char tile_smem[];
   SmemCell<P>* sm = reinterpret_cast<SmemCell<P>*>(tile_smem);
+  __shared__ CrowdList<P> cl;
   __shared__ Draws sdraw;
   __shared__ uint32_t s_last;
   Ctl* ctl = p.ctl;
   const unsigned long long t = ctl->t;
-  if (ctl->crowded[t & 3u] != 0u) return;        // a cell with more than 2 disks: the general kernel takes over
+  const uint32_t slot = (uint32_t)(t & 3u), slot1 = (uint32_t)((t + 1ull) & 3u), slot2 = (uint32_t)((t + 2ull) & 3u);
+  if (ctl->crowded[slot] != 0u) return;          // too many crowded cells: the general kernel takes over
   const uint32_t cur = ctl->cur, nxt = cur ^ 1u;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   const uint32_t ty = blockIdx.x / p.tl_ntx, tx = blockIdx.x - ty * p.tl_ntx;
   const TileBox tb = tile_box(p, tx, ty);
-  const bool single = p.tl_single != 0u;
   const uint32_t PS = p.tl_PS, pw = tb.pw, ph = tb.ph, Mqp = p.Mqp;
+  const int gx0 = (int)tb.x0 - HALO, gy0 = (int)tb.y0 - HALO;       // global cell of the region's corner (unwrapped)
   if (tid == 0) {
     sdraw = draw_sweep(p, t);                    // Alg. 1 lines 2, 15, 16 (L64, L90-91)
-    ctl->crowded[(t + 2ull) & 3u] = 0u;          // slot of the sweep after next: nobody uses it now
+    cl.n = 0u;
+    ctl->crowded[slot2] = 0u; ctl->ccount[slot2] = 0u;   // slots of the sweep after next: nobody uses them now
   }
+  __syncthreads();
 
-  // ---- load the tile and its halo: one warp per plane row, lanes along the row (512 contiguous bytes) ----
+  // ---- load the tile and its halo: warps take plane rows, lanes run along the row (512 contiguous bytes) ----
   {
     const P* posc = reinterpret_cast<const P*>(p.pos[cur]);
-    for (uint32_t row = warp; row < 4u * ph; row += TILE_THREADS / 32) {
-      const uint32_t q = row / ph, py = row - q * ph;
-      const uint32_t gy = wrap_cell((int)tb.y0 - HALO + (int)(2u * py + (q >> 1)), p.my, single);
-      const uint32_t rowbase = (gy >> 1) * p.hx;
-      for (uint32_t px = lane; px < pw; px += 32u) {
-        const uint32_t gx = wrap_cell((int)tb.x0 - HALO + (int)(2u * px + (q & 1u)), p.mx, single);
-        const uint32_t Qg = ((gy & 1u) << 1) | (gx & 1u);
-        sts_half(sm, q * PS + py * pw + px, ld_half(posc, 2u * Qg * Mqp + rowbase + (gx >> 1)));
+#pragma unroll 1
+    for (uint32_t q = 0; q < 4u; ++q) {
+      for (uint32_t py = warp; py < ph; py += TILE_THREADS / 32) {
+        const uint32_t gy = wrap_cell(gy0 + (int)(2u * py + (q >> 1)), p.my);
+        const uint32_t gbase = 2u * ((gy & 1u) << 1) * Mqp + (gy >> 1) * p.hx, sbase = q * PS + py * pw;
+        for (uint32_t px = lane; px < pw; px += 32u) {
+          const uint32_t gx = wrap_cell(gx0 + (int)(2u * px + (q & 1u)), p.mx);
+          sts_half(sm, sbase + px, ld_half(posc, gbase + 2u * (gx & 1u) * Mqp + (gx >> 1)));
+        }
+      }
+    }
+    // the crowded cells of this state that lie in the region, with their slots 2 and 3
+    const uint32_t ng = ctl->ccount[slot];
+    for (uint32_t i = tid; i < ng; i += TILE_THREADS) {
+      const uint32_t cell = ctl->clist[slot][i];
+      const uint32_t gy = cell / p.mx, gx = cell - gy * p.mx;
+      const uint32_t lx = wrap_cell((int)gx - gx0, p.mx), ly = wrap_cell((int)gy - gy0, p.my);
+      if (lx < tb.w && ly < tb.h) {
+        const uint32_t e = atomicAdd(&cl.n, 1u);
+        cl.e[e].si = (((ly & 1u) << 1) | (lx & 1u)) * PS + (ly >> 1) * pw + (lx >> 1);
+        cl.e[e].lxly = lx | (ly << 16);
+        cl.e[e].hi = ld_half(posc, (2u * (((gy & 1u) << 1) | (gx & 1u)) + 1u) * Mqp + (gy >> 1) * p.hx + (gx >> 1));
       }
     }
   }
   __syncthreads();
   const Draws dr = sdraw;
+  const uint32_t nc = cl.n;
   Tally tally;
 
   // ---- four sub-sweeps (Alg. 1 lines 3-14, L66-88): sub-sweep k updates its colour at ring >= k ----
@@ -230,19 +408,29 @@ k_tile_sweep(const __grid_constant__ Params p) {
     const uint32_t py0 = (k - qy + 1u) >> 1, py1 = (tb.h - 1u - k - qy) >> 1;
     const uint32_t nxp = px1 - px0 + 1u, count = nxp * (py1 - py0 + 1u);
     const uint32_t inv = small_div_magic(nxp);
+    int noff[9];
+#pragma unroll
+    for (int idx = 0; idx < 9; ++idx) noff[idx] = neighbour_offset(q, idx % 3 - 1, idx / 3 - 1, PS, pw);
     for (uint32_t idx = tid; idx < count; idx += TILE_THREADS) {
       const uint32_t ry = small_div(idx, inv), rx = idx - ry * nxp;
-      tile_update_cell<P, NS, DEBUG>(p, sm, tb, q, px0 + rx, py0 + ry, true, t, single, tally);
+      const uint32_t px = px0 + rx, py = py0 + ry, lx = 2u * px + qx, ly = 2u * py + qy;
+      const uint32_t si = q * PS + py * pw + px;
+      const uint32_t cell = wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx);
+      const bool interior = lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY;
+      if (nc != 0u && crowd_near(cl, nc, lx, ly))
+        tile_update_cell_general<P, DEBUG>(p, sm, cl, nc, q, pw, si, cell, interior, t, tally);
+      else
+        tile_update_cell<P, NS, DEBUG>(p, sm, si, noff, cell, interior, t, tally);
     }
     __syncthreads();
   }
 
   // ---- cell shift (Alg. 1 lines 15-17; Algorithm 4) of the interior cells, shared memory -> other buffer ----
+  const uint32_t dir = dr.dir;
+  const bool along_x = dir < 2u, positive = (dir & 1u) == 0u;
+  const P w = along_x ? R::wx(p) : R::wy(p);
+  const P delta = R::mul(R::mul((P)0.5, w), R::unit(dr.dist_word));   // line 15 (L90)
   {
-    const uint32_t dir = dr.dir;
-    const bool along_x = dir < 2u, positive = (dir & 1u) == 0u;
-    const P w = along_x ? R::wx(p) : R::wy(p);
-    const P delta = R::mul(R::mul((P)0.5, w), R::unit(dr.dist_word));   // line 15 (L90)
     const P step = positive ? -delta : delta;     // l' = l - f*delta   (L303)
     const P back = positive ? w : -w;             // entrant translation (L332)
     const uint2* idsc = reinterpret_cast<const uint2*>(p.ids[cur]);
@@ -256,30 +444,32 @@ k_tile_sweep(const __grid_constant__ Params p) {
     for (uint32_t q = 0; q < 4u; ++q) {
       const uint32_t qx = q & 1u, qy = q >> 1;
       const uint32_t px0 = (HALO - qx + 1u) >> 1, py0 = (HALO - qy + 1u) >> 1;
+      const int nboff = neighbour_offset(q, dox, doy, PS, pw);       // the old neighbour in direction f (L314-317)
       for (uint32_t idx = tid; idx < per_plane; idx += TILE_THREADS) {
         const uint32_t ry = small_div(idx, inv), rx = idx - ry * hTX;
-        const uint32_t px = px0 + rx, py = py0 + ry;
-        // the old neighbour in direction f (Alg. 4 lines 15-16, L314-317)
-        const uint32_t qn = along_x ? (q ^ 1u) : (q ^ 2u);
-        const uint32_t pxn = px + (dox < 0 ? qx - 1u : dox > 0 ? qx : 0u);
-        const uint32_t pyn = py + (doy < 0 ? qy - 1u : doy > 0 ? qy : 0u);
-        const Half<P> a = lds_half(sm, q * PS + py * pw + px), b = lds_half(sm, qn * PS + pyn * pw + pxn);
-        const uint32_t gx = wrap_cell((int)tb.x0 - HALO + (int)(2u * px + qx), p.mx, true);   // interior: one wrap
-        const uint32_t gy = wrap_cell((int)tb.y0 - HALO + (int)(2u * py + qy), p.my, true);
-        const uint32_t gxn = wrap_cell((int)gx + dox, p.mx, true), gyn = wrap_cell((int)gy + doy, p.my, true);
+        const uint32_t px = px0 + rx, py = py0 + ry, lx = 2u * px + qx, ly = 2u * py + qy;
+        const uint32_t si = q * PS + py * pw + px, sn = (uint32_t)((int)si + nboff);
+        const uint32_t gx = (uint32_t)(gx0 + (int)lx), gy = (uint32_t)(gy0 + (int)ly);      // interior: no wrap
+        const uint32_t gxn = wrap_cell((int)gx + dox, p.mx), gyn = wrap_cell((int)gy + doy, p.my);
         const uint32_t Qg = ((gy & 1u) << 1) | (gx & 1u), Qn = ((gyn & 1u) << 1) | (gxn & 1u);
         const uint32_t cig = (gy >> 1) * p.hx + (gx >> 1), cin = (gyn >> 1) * p.hx + (gxn >> 1);
-        const uint32_t own = 2u * Qg * Mqp + cig;
-        const uint2 ia = idsc[own], ib = idsc[2u * Qn * Mqp + cin];
+        const uint32_t own = 2u * Qg * Mqp + cig, nbg = 2u * Qn * Mqp + cin;
+        if (nc != 0u && (crowd_find(cl, nc, si) >= 0 || crowd_find(cl, nc, sn) >= 0)) {
+          tile_shift_cell_general<P>(p, sm, cl, nc, si, sn, own, nbg, Qg * Mqp + cig, gy * p.mx + gx, along_x, step, back, w,
+                                     cur, slot1);
+          continue;
+        }
+        const Half<P> a = lds_half(sm, si), b = lds_half(sm, sn);
+        const uint2 ia = idsc[own], ib = idsc[nbg];
         Half<P> o01, o23; uint2 i01, i23;
         uint32_t nn;
         if (along_x) nn = shift_pair<P, true>(a, b, ia, ib, step, back, w, o01, i01, o23, i23);
         else         nn = shift_pair<P, false>(a, b, ia, ib, step, back, w, o01, i01, o23, i23);
         st_half(posn, own, o01);
         idsn[own] = i01;
-        if (nn > 2u) {                            // the next state needs the general kernel
+        if (nn > 2u) {                            // a crowded cell of the new state
           st_half(posn, own + Mqp, o23); idsn[own + Mqp] = i23;
-          ctl->crowded[(t + 1ull) & 3u] = 1u;
+          note_crowded(ctl, slot1, gy * p.mx + gx);
         }
         cntn[Qg * Mqp + cig] = (uint8_t)nn;       // L280, L342
       }
@@ -295,10 +485,6 @@ k_tile_sweep(const __grid_constant__ Params p) {
   }
   __syncthreads();
   if (s_last && tid == 0) {
-    const uint32_t dir = dr.dir;
-    const bool along_x = dir < 2u, positive = (dir & 1u) == 0u;
-    const P w = along_x ? R::wx(p) : R::wy(p);
-    const P delta = R::mul(R::mul((P)0.5, w), R::unit(dr.dist_word));
     const double L = along_x ? p.Lx_eff : p.Ly_eff;
     double o = ctl->origin[along_x ? 0 : 1];     // the grid origin follows the shift
     o = __dadd_rn(o, positive ? (double)delta : -(double)delta);
@@ -308,6 +494,7 @@ k_tile_sweep(const __grid_constant__ Params p) {
     ctl->ticket = 0u;
     ctl->cur = nxt;
     ctl->t = t + 1ull;
+    ctl->path_sweeps[0] += 1ull;
   }
 }
 
