@@ -2,8 +2,8 @@
 """bench.py — hard-disk trial moves/s of the checkerboard cell sweep (BASELINE.json metric) on B200.
 
 One "step" = one pass of the whole hot path over one batch of synthetic input:
-  cell-list build from N x 2 doubles  ->  S sweeps (4 sub-sweep kernels + shift each)  ->  contact histogram
-  ->  unpack  ->  read the move counters.
+  cell-list build from N x 2 doubles  ->  S sweeps (four sub-sweeps + shift each; one fused tile-kernel launch per
+  sweep)  ->  contact histogram  ->  unpack  ->  read the move counters.
 `value`  : inputs resident in HBM when the timed region starts (CUDA events on the library's stream).
 `e2e`    : the same step through the same C-ABI calls with HOST buffers: pinned host -> device copy of the
            positions and device -> host copy of the result inside the timed region.
@@ -90,16 +90,30 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def algorithmic_bytes_per_sub_sweep(N: int, M: int, fp32: bool) -> float:
-    """a sub-sweep reads every cell once (e bytes per disk + 1 count byte per cell) and writes
-    back the active quarter: 1.25 (e N + M)."""
-    e = 8 if fp32 else 16
-    return 1.25 * (e * N + M)
-
-
 def algorithmic_bytes_per_sweep(N: int, M: int, fp32: bool) -> float:
+    """each of the four sub-sweeps reads every cell once (e bytes per disk + 1 count byte per cell)
+    and writes back the active quarter, the shift reads and writes everything: 7 (e N + M) per sweep."""
     e = 8 if fp32 else 16
     return 7.0 * (e * N + M)          # 4 x 1.25 passes + shift read + shift write
+
+
+def fused_floor_bytes_per_sweep(N: int, M: int, fp32: bool) -> float:
+    """What a sweep fused into one pass (the tile kernel) must move: read everything once, write everything once."""
+    e = 8 if fp32 else 16
+    return 2.0 * (e * N + M)
+
+
+def aggregate(dist, dev, ms_and_moves):
+    """Whole-job figures of N independent replicas: MAX over ranks of the device times, SUM over ranks of the moves.
+    ms_and_moves = [ms, ms_e2e, moves, moves_e2e]; returns the same four, reduced (unchanged without dist)."""
+    if dist is None:
+        return list(ms_and_moves)
+    import torch
+    t = torch.tensor(ms_and_moves[:2], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    m = torch.tensor(ms_and_moves[2:], dtype=torch.float64, device=dev)
+    dist.all_reduce(m, op=dist.ReduceOp.SUM)
+    return t.tolist() + m.tolist()
 
 
 def run_reference(args, w):
@@ -147,7 +161,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C3", choices=sorted(I.CONFIGS))
-    ap.add_argument("--sweeps", type=int, default=100, help="sweeps per step (PAPER.md L421: 100 timed sweeps)")
+    ap.add_argument("--sweeps", type=int, default=1000, help="sweeps per step (BASELINE.json C3: 1,000 sweeps)")
     ap.add_argument("--ref-sweeps", type=int, default=2, help="oracle sweeps per step for --impl reference")
     ap.add_argument("--cpu-baseline-sweeps", type=int, default=15)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -232,49 +246,49 @@ def main():
         step_e2e()
     ms_e2e, moves_e2e = timed(step_e2e, args.steps)
 
-    # ---- roofline of the dominant kernel (k_sub_sweep), timed live with CUDA events on the library's stream ----
-    reps = 50
+    # ---- roofline of the dominant kernel: k_tile_sweep, one launch = one whole sweep (four sub-sweeps + shift),
+    #      timed live with CUDA events on the library's stream over S back-to-back launches ----
     sim.load_positions(xy_dev)
-    sim.sweep(20)
-    for q in range(4):
-        sim.sub_sweep(q)
+    sim.sweep(100)
+    a0 = sim.acceptance()[0]
     torch.cuda.synchronize(dev)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(reps):
-        for q in range(4):
-            sim.sub_sweep(q)
-    e1.record()
-    torch.cuda.synchronize(dev)
-    sub_ms = e0.elapsed_time(e1) / (4 * reps)
-    # whole-sweep device time (graph replay), for the kernel's share of the step
     e0.record(); sim.sweep(S); e1.record(); torch.cuda.synchronize(dev)
     sweep_ms = e0.elapsed_time(e1) / S
+    moves_per_sweep = (sim.acceptance()[0] - a0) / S
+    tile_sweeps, general_sweeps = sim.path_sweeps()
+    kernel = "k_tile_sweep" if tile_sweeps >= general_sweeps else "k_sweeps"
     peak, peak_src = peaks()
-    alg = algorithmic_bytes_per_sub_sweep(w.N, sim.M, w.fp32)
-    achieved = alg / (sub_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_sub_sweep", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    alg = algorithmic_bytes_per_sweep(w.N, sim.M, w.fp32)
+    achieved = alg / (sweep_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": alg, "launch_ms": sub_ms, "sweep_ms": sweep_ms,
-                "share_of_sweep": 4 * sub_ms / sweep_ms,
-                "sweep_algorithmic_GBps": algorithmic_bytes_per_sweep(w.N, sim.M, w.fp32) / (sweep_ms * 1e-3) / 1e9,
-                "note": "state (~10 B/cell touched) is L2-resident at this size: the kernel is issue/latency-"
-                        "bound, the HBM fraction is reported because BASELINE.json names it"}
+                "algorithmic_bytes_per_launch": alg, "launch_ms": sweep_ms,
+                "algorithmic_bytes_per_move": alg / moves_per_sweep,
+                "share_of_step": S * sweep_ms / (ms / args.steps),
+                "sweeps_on_tile_kernel": tile_sweeps, "sweeps_on_general_kernel": general_sweeps,
+                "fused_floor_bytes_per_launch": fused_floor_bytes_per_sweep(w.N, sim.M, w.fp32),
+                "note": "one launch = one sweep; the state (16 B per cell) is L2-resident at this size and the kernel is "
+                        "issue-bound on the plain ALUs (see alu), the HBM fraction is reported because BASELINE.json "
+                        "names it"}
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         try:
-            roofline["traffic"] = json.load(open(tpath)).get(f"k_sub_sweep:{w.name}")
+            tr = json.load(open(tpath))
+            roofline["traffic"] = tr.get(f"{kernel}:{w.name}")
+            ipl = tr.get(f"{kernel}:{w.name}:warp_instructions")
+            if ipl and clocks.get("sm_mhz"):
+                sms = torch.cuda.get_device_properties(dev).multi_processor_count
+                issue_peak = sms * 4 * clocks["sm_mhz"] * 1e6          # warp instructions per second, 1 per scheduler per clock
+                roofline["alu"] = {"bound": "alu", "achieved": ipl / (sweep_ms * 1e-3), "peak": issue_peak,
+                                   "unit": "warp-instructions/s", "frac": ipl / (sweep_ms * 1e-3) / issue_peak,
+                                   "warp_instructions_per_launch": ipl,
+                                   "warp_instructions_per_move": ipl / moves_per_sweep}
         except Exception:
             pass
 
     # ---- max over ranks, whole-job aggregate ----
-    if dist:
-        t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        m = torch.tensor([moves, moves_e2e], dtype=torch.float64, device=dev)
-        dist.all_reduce(m, op=dist.ReduceOp.SUM)
-        ms, ms_e2e = t.tolist()
-        moves, moves_e2e = m.tolist()
+    ms, ms_e2e, moves, moves_e2e = aggregate(dist, dev, [ms, ms_e2e, moves, moves_e2e])
     value = moves / (ms * 1e-3)
     e2e = moves_e2e / (ms_e2e * 1e-3)
 
@@ -299,12 +313,13 @@ def main():
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32" if w.fp32 else "f64", "data": "synthetic",
             "config": dict(workload_config(w, S), parallelism=f"replicas x{world}" if world > 1 else "1 GPU",
-                           l2="flushed between timed steps (256 MiB fill); state itself is L2-resident",
+                           l2="flushed between timed steps (256 MiB fill); the state itself is L2-resident",
                            step="load_positions + sweeps + contact histogram + get_positions + counters"),
             "clocks": clocks,
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(xy_pinned.numel() * 8),
                     "d2h_bytes_per_step": int(out_pinned.numel() * 8 + 20 * 8 + 64), "ms_per_step": ms_e2e / args.steps},
-            "gpu_launches": args.steps * (4 + 5 * S + 1 + 1),
+            "gpu_launches": args.steps * (4 + S + 1 + 1 + 1),   # cell-list build 4, one tile kernel per sweep, general
+                                                                # kernel (no-op), histogram, unpack
             "roofline": roofline,
             "cpu_baseline": cpu,
             "paper_context": "PAPER.md L413: 1.09e9 trial moves/s on a Tesla K20 (different cell width, proposal and RNG)",

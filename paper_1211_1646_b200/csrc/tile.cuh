@@ -103,89 +103,97 @@ __device__ __forceinline__ int neighbour_offset(uint32_t q, int ox, int oy, uint
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// General cell update on the tile (rare: a crowded cell in the 3x3 neighbourhood): Algorithm 2 line by line,
-// rolled loops, up to 4 disks per cell (slots 0, 1 from the planes, slots 2, 3 from the crowd list).
+// General cell update on the tile (rare: a crowded cell in the 3x3 neighbourhood), done by a WHOLE WARP for one
+// cell: Algorithm 2 line by line with up to 4 disks per cell (slots 0, 1 from the planes, slots 2, 3 from the crowd
+// list).  Every lane runs the move sequence (identical values in all lanes); lane idx < 9 holds the disks of
+// neighbour cell idx, tests them against the trial position, and the verdict is a warp vote — the overlap test as a
+// warp-parallel any-reduction over the neighbour list.  All arguments are warp-uniform.
 // ---------------------------------------------------------------------------------------------------------
 template <typename P, bool DEBUG>
-__device__ __noinline__ void tile_update_cell_general(const Params& p, SmemCell<P>* sm, CrowdList<P>& cl, const uint32_t nc,
-                                                      const uint32_t q, const uint32_t pw, const uint32_t si_own, const uint32_t cell,
-                                                      const bool interior, const unsigned long long t, Tally& tally) {
+__device__ __noinline__ void tile_update_cell_warp(const Params& p, SmemCell<P>* sm, CrowdList<P>& cl, const uint32_t nc,
+                                                   const uint32_t q, const uint32_t pw, const uint32_t si_own,
+                                                   const uint32_t cell, const bool interior, const unsigned long long t,
+                                                   Tally& tally) {
   using R = Real<P>;
-  const uint32_t PS = p.tl_PS;
+  const uint32_t PS = p.tl_PS, lane = threadIdx.x & 31u;
   const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p);
   const P FAR = R::far_away(), HALF_FAR = FAR * (P)0.5;
   const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
-  // own disks (Alg. 2 line 8, L186)
+  // own disks (Alg. 2 line 8, L186), in every lane
   P lx[NMAX], ly[NMAX];
   const Half<P> h0 = lds_half(sm, si_own);
   const int eo = crowd_find(cl, nc, si_own);
   lx[0] = h0.x.x; lx[1] = h0.x.y; ly[0] = h0.y.x; ly[1] = h0.y.y;
   lx[2] = lx[3] = ly[2] = ly[3] = FAR;
   if (eo >= 0) { lx[2] = cl.e[eo].hi.x.x; lx[3] = cl.e[eo].hi.x.y; ly[2] = cl.e[eo].hi.y.x; ly[3] = cl.e[eo].hi.y.y; }
-  uint32_t n = 0;
-  while (n < (uint32_t)NMAX && lx[n] < HALF_FAR) ++n;
-  uint32_t n_acc = 0, n_rb = 0, n_ro = 0, amask = 0;
-  if (n > 0u) {
-    // the disks of the 8 neighbour cells, translated into this cell's frame once: q = l_j + s, s = (ox wx, oy wy)
-    // (L154, L196) — the moves below only read them
-    P nx[8 * NMAX], ny[8 * NMAX];
-    uint32_t nnb = 0;
+  const uint32_t n = lx[0] < HALF_FAR ? (lx[1] < HALF_FAR ? (lx[2] < HALF_FAR ? (lx[3] < HALF_FAR ? 4u : 3u) : 2u) : 1u) : 0u;
+  if (n == 0u) {                                                 // lines 4-7 (L181-185)
+    if (DEBUG && interior && lane == 0u) p.mask[cell] = 0u;
+    return;
+  }
+  // lane idx < 9, idx != 4: the disks of neighbour cell idx translated into this cell's frame, q = l_j + s,
+  // s = (ox wx, oy wy) (L154, L196); empty slots keep the sentinel, which never overlaps
+  P jx[NMAX] = {FAR, FAR, FAR, FAR}, jy[NMAX] = {FAR, FAR, FAR, FAR};
+  if (lane < 9u && lane != 4u) {
+    const int ox = (int)(lane % 3u) - 1, oy = (int)(lane / 3u) - 1;
+    const P sx = ox < 0 ? -wx : ox > 0 ? wx : (P)0, sy = oy < 0 ? -wy : oy > 0 ? wy : (P)0;
+    const uint32_t si = (uint32_t)((int)si_own + neighbour_offset(q, ox, oy, PS, pw));
+    const Half<P> h = lds_half(sm, si);
+    if (h.x.x < HALF_FAR) { jx[0] = R::add(h.x.x, sx); jy[0] = R::add(h.y.x, sy); }
+    if (h.x.y < HALF_FAR) { jx[1] = R::add(h.x.y, sx); jy[1] = R::add(h.y.y, sy); }
+    const int en = crowd_find(cl, nc, si);
+    if (en >= 0) {
+      const Half<P> g = cl.e[en].hi;
+      if (g.x.x < HALF_FAR) { jx[2] = R::add(g.x.x, sx); jy[2] = R::add(g.y.x, sy); }
+      if (g.x.y < HALF_FAR) { jx[3] = R::add(g.x.y, sx); jy[3] = R::add(g.y.y, sy); }
+    }
+  }
+  uint32_t perm = 0x3210u;
+  if (n >= 2u) {                                                 // line 9 (L187)
+    uint32_t S[4];
+    philox4x32_10_rk(p, cell, t_lo, t_hi, SLOT_SHUFFLE, S);
+    perm = visiting_permutation(n, S);
+  }
+  uint32_t n_acc = 0, n_rb = 0, n_ro = 0, amask = 0, vi = 0;
+  uint32_t Rw[4] = {0, 0, 0, 0};
 #pragma unroll 1
-    for (int idx = 0; idx < 9; ++idx) {
-      if (idx == 4) continue;
-      const int ox = idx % 3 - 1, oy = idx / 3 - 1;
-      const P sx = ox < 0 ? -wx : ox > 0 ? wx : (P)0, sy = oy < 0 ? -wy : oy > 0 ? wy : (P)0;
-      const uint32_t si = (uint32_t)((int)si_own + neighbour_offset(q, ox, oy, PS, pw));
-      const Half<P> h = lds_half(sm, si);
-      if (h.x.x < HALF_FAR) { nx[nnb] = R::add(h.x.x, sx); ny[nnb] = R::add(h.y.x, sy); ++nnb; }
-      if (h.x.y < HALF_FAR) { nx[nnb] = R::add(h.x.y, sx); ny[nnb] = R::add(h.y.y, sy); ++nnb; }
-      const int en = crowd_find(cl, nc, si);
-      if (en >= 0) {
-        const Half<P> g = cl.e[en].hi;
-        if (g.x.x < HALF_FAR) { nx[nnb] = R::add(g.x.x, sx); ny[nnb] = R::add(g.y.x, sy); ++nnb; }
-        if (g.x.y < HALF_FAR) { nx[nnb] = R::add(g.x.y, sx); ny[nnb] = R::add(g.y.y, sy); ++nnb; }
-      }
+  for (uint32_t s = 0; s < p.n_s; ++s) {                         // lines 11-32 (L189-230)
+    if ((s & 1u) == 0u) philox4x32_10_rk(p, cell, t_lo, t_hi, s >> 1, Rw);
+    const uint32_t k = (perm >> (4u * vi)) & 3u;                 // p <- particles[s mod n]  (L75)
+    vi = (vi + 1u == n) ? 0u : vi + 1u;
+    const uint32_t r0 = (s & 1u) ? Rw[2] : Rw[0], r1 = (s & 1u) ? Rw[3] : Rw[1];
+    const P lkx = k == 0u ? lx[0] : k == 1u ? lx[1] : k == 2u ? lx[2] : lx[3];
+    const P lky = k == 0u ? ly[0] : k == 1u ? ly[1] : k == 2u ? ly[2] : ly[3];
+    const P Mx = R::add(lkx, R::scaled_sym(p, r0)), My = R::add(lky, R::scaled_sym(p, r1));
+    if (!((Mx > (P)0) && (Mx <= wx) && (My > (P)0) && (My <= wy))) { ++n_rb; continue; }   // (0, w]  (A3)
+    bool ov = false;
+#pragma unroll
+    for (int j = 0; j < NMAX; ++j) {
+      // lane 4 tests the other disks of the own cell (s = 0, q = l_j; line 17 skips j = k), lanes 0-3, 5-8 theirs
+      const P qx_ = lane == 4u ? ((uint32_t)j == k ? FAR : lx[j]) : jx[j];
+      const P qy_ = lane == 4u ? ((uint32_t)j == k ? FAR : ly[j]) : jy[j];
+      const P Dx = R::sub(Mx, qx_), Dy = R::sub(My, qy_);
+      ov |= R::fma(Dx, Dx, R::mul(Dy, Dy)) < sigma2;             // line 19 (L204), strict (A4)
     }
-    uint32_t perm = 0x3210u;
-    if (n >= 2u) {                                               // line 9 (L187)
-      uint32_t S[4];
-      philox4x32_10_rk(p, cell, t_lo, t_hi, SLOT_SHUFFLE, S);
-      perm = visiting_permutation(n, S);
+    if (__any_sync(0xFFFFFFFFu, ov)) { ++n_ro; }
+    else {                                                       // lines 24-27 (L215-222)
+      ++n_acc; amask |= 1u << (s & 31u);
+      if (k == 0u) { lx[0] = Mx; ly[0] = My; } else if (k == 1u) { lx[1] = Mx; ly[1] = My; }
+      else if (k == 2u) { lx[2] = Mx; ly[2] = My; } else { lx[3] = Mx; ly[3] = My; }
     }
-    uint32_t vi = 0;
-    uint32_t Rw[4] = {0, 0, 0, 0};
-#pragma unroll 1
-    for (uint32_t s = 0; s < p.n_s; ++s) {                       // lines 11-32 (L189-230)
-      if ((s & 1u) == 0u) philox4x32_10_rk(p, cell, t_lo, t_hi, s >> 1, Rw);
-      const uint32_t k = (perm >> (4u * vi)) & 3u;               // p <- particles[s mod n]  (L75)
-      vi = (vi + 1u == n) ? 0u : vi + 1u;
-      const uint32_t r0 = (s & 1u) ? Rw[2] : Rw[0], r1 = (s & 1u) ? Rw[3] : Rw[1];
-      const P Mx = R::add(lx[k], R::scaled_sym(p, r0)), My = R::add(ly[k], R::scaled_sym(p, r1));
-      if (!((Mx > (P)0) && (Mx <= wx) && (My > (P)0) && (My <= wy))) { ++n_rb; continue; }   // (0, w]  (A3)
-      bool ov = false;
-      for (uint32_t j = 0; j < n; ++j) {                         // own cell: s = 0, so q = l_j; line 17 skips j = k
-        if (j == k) continue;
-        const P Dx = R::sub(Mx, lx[j]), Dy = R::sub(My, ly[j]);
-        ov |= R::fma(Dx, Dx, R::mul(Dy, Dy)) < sigma2;
-      }
-      for (uint32_t j = 0; j < nnb; ++j) {                       // line 19 (L204), strict (A4)
-        const P Dx = R::sub(Mx, nx[j]), Dy = R::sub(My, ny[j]);
-        ov |= R::fma(Dx, Dx, R::mul(Dy, Dy)) < sigma2;
-      }
-      if (ov) { ++n_ro; }
-      else { ++n_acc; amask |= 1u << (s & 31u); lx[k] = Mx; ly[k] = My; }   // lines 24-27 (L215-222)
-    }
+  }
+  if (lane == 0u) {
     if (amask != 0u) {                                           // write back (line 34, L234)
       Half<P> o;
       o.x = R::pair(lx[0], lx[1]); o.y = R::pair(ly[0], ly[1]);
       sts_half(sm, si_own, o);
       if (eo >= 0) { cl.e[eo].hi.x = R::pair(lx[2], lx[3]); cl.e[eo].hi.y = R::pair(ly[2], ly[3]); }
     }
-  }
-  if (interior && n > 0u) { tally.acc += n_acc; tally.rb += n_rb; tally.ro += n_ro; }
-  if (DEBUG && interior) {
-    p.mask[cell] = amask;
-    if (n > 0u) atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)cell << 32) | amask)));
+    if (interior) { tally.acc += n_acc; tally.rb += n_rb; tally.ro += n_ro; }
+    if (DEBUG && interior) {
+      p.mask[cell] = amask;
+      atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)cell << 32) | amask)));
+    }
   }
 }
 
@@ -411,16 +419,34 @@ k_tile_sweep(const __grid_constant__ Params p) {
     int noff[9];
 #pragma unroll
     for (int idx = 0; idx < 9; ++idx) noff[idx] = neighbour_offset(q, idx % 3 - 1, idx / 3 - 1, PS, pw);
+    // cells of this colour next to a crowded cell: one warp each, before the warp's share of the ordinary cells
+    for (uint32_t e = warp; e < nc; e += TILE_THREADS / 32) {
+      const uint32_t elx = cl.e[e].lxly & 0xFFFFu, ely = cl.e[e].lxly >> 16;
+#pragma unroll 1
+      for (int d = 0; d < 9; ++d) {
+        const uint32_t lx = elx + (uint32_t)(d % 3) - 1u, ly = ely + (uint32_t)(d / 3) - 1u;   // may wrap below 0: fails the tests
+        if ((lx & 1u) != qx || (ly & 1u) != qy) continue;
+        if (lx < k || lx > tb.w - 1u - k || ly < k || ly > tb.h - 1u - k) continue;             // ring >= k
+        bool first = true;                                       // a cell next to two listed cells is done once
+        for (uint32_t e2 = 0; e2 < e; ++e2) {
+          const uint32_t v = cl.e[e2].lxly;
+          first &= !((lx - (v & 0xFFFFu) + 1u <= 2u) && (ly - (v >> 16) + 1u <= 2u));
+        }
+        if (!first) continue;
+        const uint32_t si = q * PS + (ly >> 1) * pw + (lx >> 1);
+        const uint32_t cell = wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx);
+        const bool interior = lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY;
+        tile_update_cell_warp<P, DEBUG>(p, sm, cl, nc, q, pw, si, cell, interior, t, tally);
+      }
+    }
     for (uint32_t idx = tid; idx < count; idx += TILE_THREADS) {
       const uint32_t ry = small_div(idx, inv), rx = idx - ry * nxp;
       const uint32_t px = px0 + rx, py = py0 + ry, lx = 2u * px + qx, ly = 2u * py + qy;
+      if (nc != 0u && crowd_near(cl, nc, lx, ly)) continue;      // done above
       const uint32_t si = q * PS + py * pw + px;
       const uint32_t cell = wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx);
       const bool interior = lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY;
-      if (nc != 0u && crowd_near(cl, nc, lx, ly))
-        tile_update_cell_general<P, DEBUG>(p, sm, cl, nc, q, pw, si, cell, interior, t, tally);
-      else
-        tile_update_cell<P, NS, DEBUG>(p, sm, si, noff, cell, interior, t, tally);
+      tile_update_cell<P, NS, DEBUG>(p, sm, si, noff, cell, interior, t, tally);
     }
     __syncthreads();
   }
