@@ -53,6 +53,11 @@ struct Ctl {
   uint32_t ccount[4];
   uint32_t pad0[2];
   uint32_t clist[4][CROWD_CAP];
+#ifdef MPMC_TILE_TIMING
+  long long dbg[8];                // experiment builds: phase boundaries (clock64) of tile 0
+  unsigned long long tmin, tmax, tspan, tspan_min, last_span, last_gap, prev_end, last_cta, last_cta_min;
+  unsigned long long ncrowd_ctas, span_sum[2], span_cnt[2], span_max[2];
+#endif
   double origin[2];                // grid origin: X = origin + cell * w + local
   unsigned long long digest;       // accept-sequence digest (MPMC_DEBUG)
   unsigned long long path_sweeps[2];  // sweeps done by the tile kernel / by the general kernel since the last load
@@ -101,7 +106,7 @@ template <> struct Real<float> {
   static __device__ __forceinline__ float unit(uint32_t R) { return __fmul_rn((float)(R >> 8), 0x1p-24f); }
   // d * sym(R) as (d 2^-24) * integer: the same real product, so the same rounded value (host checks d 2^-24 is normal)
   static __device__ __forceinline__ float scaled_sym(const Params& p, uint32_t R) {
-    return __fmul_rn((float)((int)(2u * (R >> 8) + 1u) - (1 << 24)), p.dsc_f);
+    return __fmul_rn((float)((int)((R >> 7) | 1u) - (1 << 24)), p.dsc_f);   // (R >> 7) | 1 = 2 (R >> 8) + 1
   }
   static __device__ __forceinline__ float min3(float a, float b, float c) { return fminf(fminf(a, b), c); }
   static __device__ __forceinline__ float far_away() { return 1.0e18f; }   // sentinel: never overlaps

@@ -94,6 +94,10 @@ __device__ __forceinline__ bool crowd_near(const CrowdList<P>& cl, uint32_t nc, 
   return near;
 }
 
+// floor(n / d) for n < 2^16, 1 <= d < 2^16 with the per-phase constant inv = ceil(2^32 / d) (0 stands for d = 1)
+__device__ __forceinline__ uint32_t small_div_magic(uint32_t d) { return d == 1u ? 0u : (uint32_t)(0xFFFFFFFFull / d) + 1u; }
+__device__ __forceinline__ uint32_t small_div(uint32_t n, uint32_t inv) { return inv == 0u ? n : __umulhi(n, inv); }
+
 // shared-memory offsets of the 3x3 cells relative to an active cell of local colour q (uniform per phase)
 __device__ __forceinline__ int neighbour_offset(uint32_t q, int ox, int oy, uint32_t PS, uint32_t pw) {
   const int qx = (int)(q & 1u), qy = (int)(q >> 1);
@@ -201,15 +205,16 @@ __device__ __noinline__ void tile_update_cell_warp(const Params& p, SmemCell<P>*
 // One cell update (Algorithm 2) on the tile in shared memory: the arithmetic of update_cell_fast
 // (sweep.cuh), the 3x3 cells read with one LDS.128 each at si_own + noff[idx] (offsets uniform per phase).
 // ---------------------------------------------------------------------------------------------------------
-template <typename P, int NS, bool DEBUG>
+template <typename P, int NS, bool DEBUG, uint32_t QL>
 __device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* sm, const uint32_t si_own,
-                                                 const int (&noff)[9], const uint32_t cell, const bool interior,
+                                                 const uint32_t pw, const uint32_t cell, const bool interior,
                                                  const unsigned long long t, Tally& tally) {
   using R = Real<P>;
   using Pair = typename R::Pair;
   Half<P> h[9];
+  const SmemCell<P>* own = sm + si_own;            // QL, tl_PS and pw are uniform: the nine offsets cost nothing per cell
 #pragma unroll
-  for (int idx = 0; idx < 9; ++idx) h[idx] = lds_half(sm, (uint32_t)((int)si_own + noff[idx]));
+  for (int idx = 0; idx < 9; ++idx) h[idx] = lds_half(own + neighbour_offset(QL, idx % 3 - 1, idx / 3 - 1, p.tl_PS, pw), 0u);
   // ---- displacements of all NS moves from the GLOBAL cell id (line 12, L190; A2, A9) ----
   const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
   P ddx[NS], ddy[NS];
@@ -240,11 +245,19 @@ __device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* s
   const uint32_t n = Bx < HALF_FAR ? 2u : (Ax < HALF_FAR ? 1u : 0u);
   const bool two = n == 2u;
   bool flip = false;                   // true: A is slot 1
+#ifdef MPMC_SHUFFLE_ALWAYS
+  {                                    // n = 2: Fisher-Yates is one draw, j = bounded(S0, 2); j = 0 swaps
+    uint32_t S[4];
+    philox4x32_10_rk(p, cell, t_lo, t_hi, SLOT_SHUFFLE, S);
+    flip = two && bounded(S[0], 2u) == 0u;
+  }
+#else
   if (two) {                           // n = 2: Fisher-Yates is one draw, j = bounded(S0, 2); j = 0 swaps
     uint32_t S[4];
     philox4x32_10_rk(p, cell, t_lo, t_hi, SLOT_SHUFFLE, S);
     flip = bounded(S[0], 2u) == 0u;
   }
+#endif
   if (flip) { P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }
   uint32_t n_acc = 0, n_rb = 0, amask = 0;
 #pragma unroll
@@ -283,10 +296,6 @@ __device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* s
     if (n > 0u) atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)cell << 32) | amask)));
   }
 }
-
-// floor(n / d) for n < 2^16, 1 <= d < 2^16 with the per-phase constant inv = ceil(2^32 / d) (0 stands for d = 1)
-__device__ __forceinline__ uint32_t small_div_magic(uint32_t d) { return d == 1u ? 0u : (uint32_t)(0xFFFFFFFFull / d) + 1u; }
-__device__ __forceinline__ uint32_t small_div(uint32_t n, uint32_t inv) { return inv == 0u ? n : __umulhi(n, inv); }
 
 // General shift of one interior cell (rare: it or its source neighbour is crowded): Algorithm 4 line by line.
 template <typename P>
@@ -342,6 +351,37 @@ __device__ __noinline__ void tile_shift_cell_general(const Params& p, const Smem
   p.cnt[nxt][cnt_g] = (uint8_t)nn;
 }
 
+// The ordinary cells of sub-sweep k: the cells of local colour QL at ring >= k.  Warps draw chunks of 32 cells from a
+// shared counter, so a warp that was busy with a crowded cell (or started late) simply takes fewer.
+template <typename P, int NS, bool DEBUG, uint32_t QL>
+__device__ __forceinline__ void tile_sub_sweep_cells(const Params& p, SmemCell<P>* sm, const CrowdList<P>& cl,
+                                                     const uint32_t nc, const TileBox& tb, const uint32_t k, const int gx0,
+                                                     const int gy0, const unsigned long long t, uint32_t* next,
+                                                     Tally& tally) {
+  constexpr uint32_t qx = QL & 1u, qy = QL >> 1;
+  const uint32_t PS = p.tl_PS, pw = tb.pw;
+  const uint32_t px0 = (k - qx + 1u) >> 1, px1 = (tb.w - 1u - k - qx) >> 1;
+  const uint32_t py0 = (k - qy + 1u) >> 1, py1 = (tb.h - 1u - k - qy) >> 1;
+  const uint32_t nxp = px1 - px0 + 1u, count = nxp * (py1 - py0 + 1u);
+  const uint32_t inv = small_div_magic(nxp);
+  const uint32_t lane = threadIdx.x & 31u;
+  for (;;) {                                                   // warps draw chunks of 32 cells until none is left
+    uint32_t base = 0;
+    if (lane == 0u) base = atomicAdd(next, 32u);
+    base = __shfl_sync(0xFFFFFFFFu, base, 0);
+    if (base >= count) break;
+    const uint32_t idx = base + lane;
+    if (idx >= count) continue;
+    const uint32_t ry = small_div(idx, inv), rx = idx - ry * nxp;
+    const uint32_t px = px0 + rx, py = py0 + ry, lx = 2u * px + qx, ly = 2u * py + qy;
+    if (nc != 0u && crowd_near(cl, nc, lx, ly)) continue;      // done by a warp (tile_update_cell_warp)
+    const uint32_t si = QL * PS + py * pw + px;
+    const uint32_t cell = wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx);
+    const bool interior = lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY;
+    tile_update_cell<P, NS, DEBUG, QL>(p, sm, si, pw, cell, interior, t, tally);
+  }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // The fused sweep kernel: one CTA per tile, one launch per sweep.  See the header of this file.
 // Dynamic shared memory: 4 planes x tl_PS cells x sizeof(SmemCell<P>).
@@ -356,7 +396,11 @@ k_tile_sweep(const __grid_constant__ Params p) {
   __shared__ CrowdList<P> cl;
   __shared__ Draws sdraw;
   __shared__ uint32_t s_last;
+  __shared__ uint32_t s_next[8];                 // chunk counters: sub-sweeps 1-4, shift planes 0-3
   Ctl* ctl = p.ctl;
+#ifdef MPMC_TILE_TIMING
+  unsigned long long gt0; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt0));
+#endif
   const unsigned long long t = ctl->t;
   const uint32_t slot = (uint32_t)(t & 3u), slot1 = (uint32_t)((t + 1ull) & 3u), slot2 = (uint32_t)((t + 2ull) & 3u);
   if (ctl->crowded[slot] != 0u) return;          // too many crowded cells: the general kernel takes over
@@ -369,22 +413,46 @@ k_tile_sweep(const __grid_constant__ Params p) {
   if (tid == 0) {
     sdraw = draw_sweep(p, t);                    // Alg. 1 lines 2, 15, 16 (L64, L90-91)
     cl.n = 0u;
+    for (int i = 0; i < 8; ++i) s_next[i] = 0u;
     ctl->crowded[slot2] = 0u; ctl->ccount[slot2] = 0u;   // slots of the sweep after next: nobody uses them now
   }
   __syncthreads();
+#ifdef MPMC_TILE_TIMING
+  if (blockIdx.x == 0 && tid == 0) ctl->dbg[0] = clock64();
+#endif
 
   // ---- load the tile and its halo: warps take plane rows, lanes run along the row (512 contiguous bytes) ----
   {
     const P* posc = reinterpret_cast<const P*>(p.pos[cur]);
-#pragma unroll 1
-    for (uint32_t q = 0; q < 4u; ++q) {
-      for (uint32_t py = warp; py < ph; py += TILE_THREADS / 32) {
-        const uint32_t gy = wrap_cell(gy0 + (int)(2u * py + (q >> 1)), p.my);
-        const uint32_t gbase = 2u * ((gy & 1u) << 1) * Mqp + (gy >> 1) * p.hx, sbase = q * PS + py * pw;
-        for (uint32_t px = lane; px < pw; px += 32u) {
-          const uint32_t gx = wrap_cell(gx0 + (int)(2u * px + (q & 1u)), p.mx);
-          sts_half(sm, sbase + px, ld_half(posc, gbase + 2u * (gx & 1u) * Mqp + (gx >> 1)));
+    // four plane rows x two 32-cell column blocks per warp and pass: eight independent loads in flight per lane
+    // before the first shared-memory store (a load -> store chain per row would expose the L2 latency every time)
+    constexpr uint32_t NW = TILE_THREADS / 32;
+    const uint32_t nrows = 4u * ph, inv_ph = small_div_magic(ph);
+    for (uint32_t c0 = 0; c0 < pw; c0 += 64u) {
+      for (uint32_t r0 = warp; r0 < nrows; r0 += 4u * NW) {
+        Half<P> v[4][2];
+        uint32_t sidx[4][2];
+        bool ok[4][2];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const uint32_t r = r0 + (uint32_t)j * NW, rr = r < nrows ? r : 0u;
+          const uint32_t q = small_div(rr, inv_ph), py = rr - q * ph;
+          const uint32_t gy = wrap_cell(gy0 + (int)(2u * py + (q >> 1)), p.my);
+          const uint32_t gbase = 2u * ((gy & 1u) << 1) * Mqp + (gy >> 1) * p.hx, sbase = q * PS + py * pw;
+#pragma unroll
+          for (int c = 0; c < 2; ++c) {
+            const uint32_t px = c0 + lane + 32u * (uint32_t)c;
+            ok[j][c] = r < nrows && px < pw;
+            const uint32_t gx = wrap_cell(gx0 + (int)(2u * (ok[j][c] ? px : 0u) + (q & 1u)), p.mx);
+            sidx[j][c] = sbase + px;
+            if (ok[j][c]) v[j][c] = ld_half(posc, gbase + 2u * (gx & 1u) * Mqp + (gx >> 1));
+          }
         }
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+#pragma unroll
+          for (int c = 0; c < 2; ++c)
+            if (ok[j][c]) sts_half(sm, sidx[j][c], v[j][c]);
       }
     }
     // the crowded cells of this state that lie in the region, with their slots 2 and 3
@@ -402,6 +470,9 @@ k_tile_sweep(const __grid_constant__ Params p) {
     }
   }
   __syncthreads();
+#ifdef MPMC_TILE_TIMING
+  if (blockIdx.x == 0 && tid == 0) ctl->dbg[1] = clock64();
+#endif
   const Draws dr = sdraw;
   const uint32_t nc = cl.n;
   Tally tally;
@@ -412,43 +483,37 @@ k_tile_sweep(const __grid_constant__ Params p) {
     const uint32_t Qg = k == 1u ? dr.order[0] : k == 2u ? dr.order[1] : k == 3u ? dr.order[2] : dr.order[3];
     const uint32_t q = Qg ^ 3u;                  // the region starts at an odd cell (x0 - 5, y0 - 5): colours flip
     const uint32_t qx = q & 1u, qy = q >> 1;
-    const uint32_t px0 = (k - qx + 1u) >> 1, px1 = (tb.w - 1u - k - qx) >> 1;
-    const uint32_t py0 = (k - qy + 1u) >> 1, py1 = (tb.h - 1u - k - qy) >> 1;
-    const uint32_t nxp = px1 - px0 + 1u, count = nxp * (py1 - py0 + 1u);
-    const uint32_t inv = small_div_magic(nxp);
-    int noff[9];
-#pragma unroll
-    for (int idx = 0; idx < 9; ++idx) noff[idx] = neighbour_offset(q, idx % 3 - 1, idx / 3 - 1, PS, pw);
     // cells of this colour next to a crowded cell: one warp each, before the warp's share of the ordinary cells
-    for (uint32_t e = warp; e < nc; e += TILE_THREADS / 32) {
+    for (uint32_t pi = warp; pi < 9u * nc; pi += TILE_THREADS / 32) {      // (listed cell, 3x3 position) pairs
+      const uint32_t e = pi / 9u, d = pi - 9u * e;
       const uint32_t elx = cl.e[e].lxly & 0xFFFFu, ely = cl.e[e].lxly >> 16;
-#pragma unroll 1
-      for (int d = 0; d < 9; ++d) {
-        const uint32_t lx = elx + (uint32_t)(d % 3) - 1u, ly = ely + (uint32_t)(d / 3) - 1u;   // may wrap below 0: fails the tests
-        if ((lx & 1u) != qx || (ly & 1u) != qy) continue;
-        if (lx < k || lx > tb.w - 1u - k || ly < k || ly > tb.h - 1u - k) continue;             // ring >= k
-        bool first = true;                                       // a cell next to two listed cells is done once
-        for (uint32_t e2 = 0; e2 < e; ++e2) {
-          const uint32_t v = cl.e[e2].lxly;
-          first &= !((lx - (v & 0xFFFFu) + 1u <= 2u) && (ly - (v >> 16) + 1u <= 2u));
-        }
-        if (!first) continue;
-        const uint32_t si = q * PS + (ly >> 1) * pw + (lx >> 1);
-        const uint32_t cell = wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx);
-        const bool interior = lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY;
-        tile_update_cell_warp<P, DEBUG>(p, sm, cl, nc, q, pw, si, cell, interior, t, tally);
+      const uint32_t lx = elx + d % 3u - 1u, ly = ely + d / 3u - 1u;       // may wrap below 0: fails the tests
+      if ((lx & 1u) != qx || (ly & 1u) != qy) continue;
+      if (lx < k || lx > tb.w - 1u - k || ly < k || ly > tb.h - 1u - k) continue;               // ring >= k
+      bool first = true;                                         // a cell next to two listed cells is done once
+      for (uint32_t e2 = 0; e2 < e; ++e2) {
+        const uint32_t v = cl.e[e2].lxly;
+        first &= !((lx - (v & 0xFFFFu) + 1u <= 2u) && (ly - (v >> 16) + 1u <= 2u));
       }
-    }
-    for (uint32_t idx = tid; idx < count; idx += TILE_THREADS) {
-      const uint32_t ry = small_div(idx, inv), rx = idx - ry * nxp;
-      const uint32_t px = px0 + rx, py = py0 + ry, lx = 2u * px + qx, ly = 2u * py + qy;
-      if (nc != 0u && crowd_near(cl, nc, lx, ly)) continue;      // done above
-      const uint32_t si = q * PS + py * pw + px;
+      if (!first) continue;
+      const uint32_t si = q * PS + (ly >> 1) * pw + (lx >> 1);
       const uint32_t cell = wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx);
       const bool interior = lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY;
-      tile_update_cell<P, NS, DEBUG>(p, sm, si, noff, cell, interior, t, tally);
+      tile_update_cell_warp<P, DEBUG>(p, sm, cl, nc, q, pw, si, cell, interior, t, tally);
     }
+    switch (q) {                                   // the local colour as a compile-time constant: uniform offsets
+      case 0: tile_sub_sweep_cells<P, NS, DEBUG, 0>(p, sm, cl, nc, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      case 1: tile_sub_sweep_cells<P, NS, DEBUG, 1>(p, sm, cl, nc, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      case 2: tile_sub_sweep_cells<P, NS, DEBUG, 2>(p, sm, cl, nc, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      default: tile_sub_sweep_cells<P, NS, DEBUG, 3>(p, sm, cl, nc, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
+    }
+#ifdef MPMC_TILE_TIMING
+    if (blockIdx.x == 0 && tid == 0) ctl->dbg[6] = clock64();      // this thread's own work done, before the barrier
+#endif
     __syncthreads();
+#ifdef MPMC_TILE_TIMING
+    if (blockIdx.x == 0 && tid == 0) ctl->dbg[1 + k] = clock64();
+#endif
   }
 
   // ---- cell shift (Alg. 1 lines 15-17; Algorithm 4) of the interior cells, shared memory -> other buffer ----
@@ -466,12 +531,20 @@ k_tile_sweep(const __grid_constant__ Params p) {
     const uint32_t hTX = tb.TX >> 1, per_plane = hTX * (tb.TY >> 1);
     const uint32_t inv = small_div_magic(hTX);
     const int dox = along_x ? (positive ? 1 : -1) : 0, doy = along_x ? 0 : (positive ? 1 : -1);
+    // The interior cells of the four local colour planes in chunks of 32 that the warps draw from shared counters;
+    // consecutive lanes write consecutive cells of one global colour plane.
 #pragma unroll 1
     for (uint32_t q = 0; q < 4u; ++q) {
       const uint32_t qx = q & 1u, qy = q >> 1;
       const uint32_t px0 = (HALO - qx + 1u) >> 1, py0 = (HALO - qy + 1u) >> 1;
       const int nboff = neighbour_offset(q, dox, doy, PS, pw);       // the old neighbour in direction f (L314-317)
-      for (uint32_t idx = tid; idx < per_plane; idx += TILE_THREADS) {
+      for (;;) {
+        uint32_t base = 0;
+        if (lane == 0u) base = atomicAdd(&s_next[4u + q], 32u);
+        base = __shfl_sync(0xFFFFFFFFu, base, 0);
+        if (base >= per_plane) break;
+        const uint32_t idx = base + lane;
+        if (idx >= per_plane) continue;
         const uint32_t ry = small_div(idx, inv), rx = idx - ry * hTX;
         const uint32_t px = px0 + rx, py = py0 + ry, lx = 2u * px + qx, ly = 2u * py + qy;
         const uint32_t si = q * PS + py * pw + px, sn = (uint32_t)((int)si + nboff);
@@ -485,8 +558,8 @@ k_tile_sweep(const __grid_constant__ Params p) {
                                      cur, slot1);
           continue;
         }
-        const Half<P> a = lds_half(sm, si), b = lds_half(sm, sn);
         const uint2 ia = idsc[own], ib = idsc[nbg];
+        const Half<P> a = lds_half(sm, si), b = lds_half(sm, sn);
         Half<P> o01, o23; uint2 i01, i23;
         uint32_t nn;
         if (along_x) nn = shift_pair<P, true>(a, b, ia, ib, step, back, w, o01, i01, o23, i23);
@@ -505,11 +578,26 @@ k_tile_sweep(const __grid_constant__ Params p) {
   // ---- counters; the last CTA to finish advances the control block ----
   flush_tally(p, tally);
   __syncthreads();
+#ifdef MPMC_TILE_TIMING
+  if (blockIdx.x == 0 && tid == 0) ctl->dbg[7] = clock64();
+#endif
   if (tid == 0) {
     __threadfence();
     s_last = (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1u) ? 1u : 0u;
   }
   __syncthreads();
+#ifdef MPMC_TILE_TIMING
+  if (tid == 0) {
+    unsigned long long gt1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt1));
+    atomicMin((unsigned long long*)&ctl->tmin, gt0); atomicMax((unsigned long long*)&ctl->tmax, gt1);
+    atomicMax((unsigned long long*)&ctl->tspan, gt1 - gt0); atomicMin((unsigned long long*)&ctl->tspan_min, gt1 - gt0);
+    if (nc != 0u) atomicAdd((unsigned long long*)&ctl->ncrowd_ctas, 1ull);
+    if (s_last) { { const unsigned long long sp = ctl->tmax - ctl->tmin; const int cr = ctl->ncrowd_ctas != 0; ctl->span_sum[cr] += sp; ctl->span_cnt[cr] += 1; if (sp > ctl->span_max[cr]) ctl->span_max[cr] = sp; ctl->ncrowd_ctas = 0; }
+                  ctl->last_span = ctl->tmax - ctl->tmin; ctl->last_gap = ctl->tmin - ctl->prev_end; ctl->prev_end = ctl->tmax;
+                  ctl->last_cta = ctl->tspan; ctl->last_cta_min = ctl->tspan_min;
+                  ctl->tmin = ~0ull; ctl->tmax = 0; ctl->tspan = 0; ctl->tspan_min = ~0ull; }
+  }
+#endif
   if (s_last && tid == 0) {
     const double L = along_x ? p.Lx_eff : p.Ly_eff;
     double o = ctl->origin[along_x ? 0 : 1];     // the grid origin follows the shift
