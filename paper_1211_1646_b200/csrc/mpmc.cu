@@ -362,9 +362,20 @@ int mpmc_sweep(mpmc_ctx* c, uint64_t k) {
   c->t_host += k;
   if (c->tile_kernel) {
     // one tile-kernel launch per sweep; each returns at once if the state has become crowded (tile.cuh) ...
+    // Programmatic dependent launch: the CTAs of sweep t+1 become resident as the SMs of sweep t free up and park at
+    // griddepcontrol.wait until sweep t has completed and flushed, which hides the launch latency (~4 us of ~50).
+    // MPMC_PDL=0 in the environment turns it off (A/B timing).
+    static const bool pdl = [] { const char* e = std::getenv("MPMC_PDL"); return !(e && e[0] == '0'); }();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(c->tile_grid);
+    cfg.blockDim = dim3(c->fp32 ? TileThreads<float>::value : TileThreads<double>::value);
+    cfg.dynamicSmemBytes = c->tile_smem; cfg.stream = c->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = (pdl && c->stream != nullptr) ? 1 : 0;
     void* args[] = {(void*)&c->p};
-    for (uint64_t i = 0; i < k; ++i)
-      CU(cudaLaunchKernel(c->tile_kernel, dim3(c->tile_grid), dim3(c->fp32 ? TileThreads<float>::value : TileThreads<double>::value), args, c->tile_smem, c->stream));
+    for (uint64_t i = 0; i < k; ++i) CU(cudaLaunchKernelExC(&cfg, c->tile_kernel, args));
   }
   // ... and the general kernel runs whatever is left up to the target sweep index (normally nothing)
   const int st = launch_sweeps(c, c->t_host, OP_SWEEPS, 0, 0.0);

@@ -398,6 +398,9 @@ k_tile_sweep(const __grid_constant__ Params p) {
   __shared__ uint32_t s_last;
   __shared__ uint32_t s_next[8];                 // chunk counters: sub-sweeps 1-4, shift planes 0-3
   Ctl* ctl = p.ctl;
+  // launched with programmatic stream serialisation (mpmc.cu): everything below reads what the previous sweep wrote
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 #ifdef MPMC_TILE_TIMING
   unsigned long long gt0; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt0));
 #endif
