@@ -18,10 +18,6 @@ __global__ void k_reset(const __grid_constant__ Params p) {
     for (int i = 0; i < 4; ++i) { c->crowded[i] = 0; c->ccount[i] = 0; }
     c->origin[0] = 0.0; c->origin[1] = 0.0;
     c->digest = 0; c->path_sweeps[0] = c->path_sweeps[1] = 0;
-#ifdef MPMC_TILE_TIMING
-    c->tmin = ~0ull; c->tmax = 0; c->tspan = 0; c->tspan_min = ~0ull; c->prev_end = 0; c->ncrowd_ctas = 0;
-    for (int i = 0; i < 2; ++i) { c->span_sum[i] = 0; c->span_cnt[i] = 0; c->span_max[i] = 0; }
-#endif
     for (uint32_t r = 0; r < CTR_SLOTS; ++r) c->counters[r][0] = c->counters[r][1] = c->counters[r][2] = c->counters[r][3] = 0;
   }
 }

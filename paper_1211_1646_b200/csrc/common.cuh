@@ -53,11 +53,6 @@ struct Ctl {
   uint32_t ccount[4];
   uint32_t pad0[2];
   uint32_t clist[4][CROWD_CAP];
-#ifdef MPMC_TILE_TIMING
-  long long dbg[8];                // experiment builds: phase boundaries (clock64) of tile 0
-  unsigned long long tmin, tmax, tspan, tspan_min, last_span, last_gap, prev_end, last_cta, last_cta_min;
-  unsigned long long ncrowd_ctas, span_sum[2], span_cnt[2], span_max[2];
-#endif
   double origin[2];                // grid origin: X = origin + cell * w + local
   unsigned long long digest;       // accept-sequence digest (MPMC_DEBUG)
   unsigned long long path_sweeps[2];  // sweeps done by the tile kernel / by the general kernel since the last load

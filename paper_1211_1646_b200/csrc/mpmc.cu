@@ -482,15 +482,6 @@ int mpmc_debug_path(mpmc_ctx* c, uint64_t out[2]) {
   Ctl h;
   const int st = read_ctl(c, &h);
   out[0] = h.path_sweeps[0]; out[1] = h.path_sweeps[1];
-#ifdef MPMC_TILE_TIMING
-  std::fprintf(stderr, "[mpmc] tile 0 cycles: load %lld, sub %lld %lld %lld %lld (own work of thread 0 in the last: %lld), shift %lld\n",
-               h.dbg[1] - h.dbg[0], h.dbg[2] - h.dbg[1], h.dbg[3] - h.dbg[2], h.dbg[4] - h.dbg[3], h.dbg[5] - h.dbg[4],
-               h.dbg[6] - h.dbg[4], h.dbg[7] - h.dbg[5]);
-  std::fprintf(stderr, "[mpmc] last tile kernel: span %llu ns, gap to previous %llu ns, slowest CTA %llu ns, fastest CTA %llu ns\n",
-               h.last_span, h.last_gap, h.last_cta, h.last_cta_min);
-  for (int i = 0; i < 2; ++i) std::fprintf(stderr, "[mpmc] kernels %s crowded cells: %llu, mean span %.0f ns, max %llu ns\n", i ? "with" : "without",
-               h.span_cnt[i], h.span_cnt[i] ? (double)h.span_sum[i] / h.span_cnt[i] : 0.0, h.span_max[i]);
-#endif
   return st;
 }
 

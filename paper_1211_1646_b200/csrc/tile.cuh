@@ -245,19 +245,11 @@ __device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* s
   const uint32_t n = Bx < HALF_FAR ? 2u : (Ax < HALF_FAR ? 1u : 0u);
   const bool two = n == 2u;
   bool flip = false;                   // true: A is slot 1
-#ifdef MPMC_SHUFFLE_ALWAYS
-  {                                    // n = 2: Fisher-Yates is one draw, j = bounded(S0, 2); j = 0 swaps
-    uint32_t S[4];
-    philox4x32_10_rk(p, cell, t_lo, t_hi, SLOT_SHUFFLE, S);
-    flip = two && bounded(S[0], 2u) == 0u;
-  }
-#else
   if (two) {                           // n = 2: Fisher-Yates is one draw, j = bounded(S0, 2); j = 0 swaps
     uint32_t S[4];
     philox4x32_10_rk(p, cell, t_lo, t_hi, SLOT_SHUFFLE, S);
     flip = bounded(S[0], 2u) == 0u;
   }
-#endif
   if (flip) { P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }
   uint32_t n_acc = 0, n_rb = 0, amask = 0;
 #pragma unroll
@@ -401,9 +393,6 @@ k_tile_sweep(const __grid_constant__ Params p) {
   // launched with programmatic stream serialisation (mpmc.cu): everything below reads what the previous sweep wrote
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-#ifdef MPMC_TILE_TIMING
-  unsigned long long gt0; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt0));
-#endif
   const unsigned long long t = ctl->t;
   const uint32_t slot = (uint32_t)(t & 3u), slot1 = (uint32_t)((t + 1ull) & 3u), slot2 = (uint32_t)((t + 2ull) & 3u);
   if (ctl->crowded[slot] != 0u) return;          // too many crowded cells: the general kernel takes over
@@ -420,9 +409,6 @@ k_tile_sweep(const __grid_constant__ Params p) {
     ctl->crowded[slot2] = 0u; ctl->ccount[slot2] = 0u;   // slots of the sweep after next: nobody uses them now
   }
   __syncthreads();
-#ifdef MPMC_TILE_TIMING
-  if (blockIdx.x == 0 && tid == 0) ctl->dbg[0] = clock64();
-#endif
 
   // ---- load the tile and its halo: warps take plane rows, lanes run along the row (512 contiguous bytes) ----
   {
@@ -473,9 +459,6 @@ k_tile_sweep(const __grid_constant__ Params p) {
     }
   }
   __syncthreads();
-#ifdef MPMC_TILE_TIMING
-  if (blockIdx.x == 0 && tid == 0) ctl->dbg[1] = clock64();
-#endif
   const Draws dr = sdraw;
   const uint32_t nc = cl.n;
   Tally tally;
@@ -510,13 +493,7 @@ k_tile_sweep(const __grid_constant__ Params p) {
       case 2: tile_sub_sweep_cells<P, NS, DEBUG, 2>(p, sm, cl, nc, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
       default: tile_sub_sweep_cells<P, NS, DEBUG, 3>(p, sm, cl, nc, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
     }
-#ifdef MPMC_TILE_TIMING
-    if (blockIdx.x == 0 && tid == 0) ctl->dbg[6] = clock64();      // this thread's own work done, before the barrier
-#endif
     __syncthreads();
-#ifdef MPMC_TILE_TIMING
-    if (blockIdx.x == 0 && tid == 0) ctl->dbg[1 + k] = clock64();
-#endif
   }
 
   // ---- cell shift (Alg. 1 lines 15-17; Algorithm 4) of the interior cells, shared memory -> other buffer ----
@@ -581,26 +558,11 @@ k_tile_sweep(const __grid_constant__ Params p) {
   // ---- counters; the last CTA to finish advances the control block ----
   flush_tally(p, tally);
   __syncthreads();
-#ifdef MPMC_TILE_TIMING
-  if (blockIdx.x == 0 && tid == 0) ctl->dbg[7] = clock64();
-#endif
   if (tid == 0) {
     __threadfence();
     s_last = (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1u) ? 1u : 0u;
   }
   __syncthreads();
-#ifdef MPMC_TILE_TIMING
-  if (tid == 0) {
-    unsigned long long gt1; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt1));
-    atomicMin((unsigned long long*)&ctl->tmin, gt0); atomicMax((unsigned long long*)&ctl->tmax, gt1);
-    atomicMax((unsigned long long*)&ctl->tspan, gt1 - gt0); atomicMin((unsigned long long*)&ctl->tspan_min, gt1 - gt0);
-    if (nc != 0u) atomicAdd((unsigned long long*)&ctl->ncrowd_ctas, 1ull);
-    if (s_last) { { const unsigned long long sp = ctl->tmax - ctl->tmin; const int cr = ctl->ncrowd_ctas != 0; ctl->span_sum[cr] += sp; ctl->span_cnt[cr] += 1; if (sp > ctl->span_max[cr]) ctl->span_max[cr] = sp; ctl->ncrowd_ctas = 0; }
-                  ctl->last_span = ctl->tmax - ctl->tmin; ctl->last_gap = ctl->tmin - ctl->prev_end; ctl->prev_end = ctl->tmax;
-                  ctl->last_cta = ctl->tspan; ctl->last_cta_min = ctl->tspan_min;
-                  ctl->tmin = ~0ull; ctl->tmax = 0; ctl->tspan = 0; ctl->tspan_min = ~0ull; }
-  }
-#endif
   if (s_last && tid == 0) {
     const double L = along_x ? p.Lx_eff : p.Ly_eff;
     double o = ctl->origin[along_x ? 0 : 1];     // the grid origin follows the shift
