@@ -87,10 +87,11 @@ def test_c1_100_sweeps_bit_exact(oracle_mod, torch_cuda, fp32):
     w = I.CONFIGS["C1"]
     xy, box = I.workload_inputs(w)
     o, g = make_pair(oracle_mod, torch_cuda, w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32, xy)
-    for k in (1, 1, 3, 16, 17, 62):                    # single launches, graph batches and remainders
+    for k in (1, 1, 3, 16, 17, 62):                    # several call sizes: one tile-kernel launch per sweep
         o.sweep(k); g.sweep(k)
         st = assert_same_state(o, g, fp32)
     assert st["sweep"] == 100
+    assert g.path_sweeps() == (100, 0)                 # every sweep on the fused tile kernel
     att, acc, rb, ro = g.acceptance()
     assert att == acc + rb + ro and acc > 0 and rb > 0 and ro > 0
 
@@ -123,6 +124,7 @@ def test_c3_headline_config_bench_launch_configuration(oracle_mod, torch_cuda):
     o.sweep(12); g.sweep(12)
     st = assert_same_state(o, g, True, check_mask=False)
     assert st["counts"].sum() == w.N
+    assert g.path_sweeps() == (12, 0)                  # the fused tile kernel did them all (crowded cells included)
     att = g.acceptance()[0]
     assert 11.5 * 4.0e6 < att < 12 * 4.2e6
 
@@ -175,6 +177,36 @@ def test_three_per_cell_with_two_register_slots(oracle_mod, torch_cuda, fp32):
         st = assert_same_state(o, g, fp32)
         seen3 |= st["counts"].max() >= 3
     assert seen3
+    tile, general = g.path_sweeps()
+    assert tile + general == 200 and tile > 0          # crowded cells carried by the tile kernel's shared-memory list
+
+
+@pytest.mark.parametrize("fp32", [False, True])
+def test_tile_kernel_hands_over_when_too_many_cells_are_crowded(oracle_mod, torch_cuda, fp32):
+    # a denser system at the same cell width: more than 256 cells hold 3 disks, so the tile kernel returns at once
+    # and the general persistent kernel runs the sweeps (and the tile kernel resumes if the state thins out)
+    xy, box = I.jittered_lattice(192, 0.70, seed=9)
+    o, g = make_pair(oracle_mod, torch_cuda, 192 * 192, box, 1.0, 0.2, 4, 5, fp32, xy, w_target=1.135)
+    assert 1.135 <= g.wx < 1.15 and 1.135 <= g.wy < 1.15
+    most = 0
+    for _ in range(4):
+        o.sweep(10); g.sweep(10)
+        st = assert_same_state(o, g, fp32)
+        most = max(most, int((st["counts"] >= 3).sum()))
+    tile, general = g.path_sweeps()
+    assert tile + general == 40
+    assert general > 0 and most > 256
+
+
+@pytest.mark.parametrize("n,phi", [(14, 0.5), (24, 0.6), (50, 0.7), (98, 0.65)])
+def test_tile_kernel_uneven_tilings(oracle_mod, torch_cuda, n, phi):
+    # box sizes that do not divide evenly into tiles (tiles of different widths, many tiny tiles, few large ones)
+    xy, box = I.jittered_lattice(n, phi, seed=n)
+    o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.15, 4, n, True, xy)
+    for k in (1, 2, 7):
+        o.sweep(k); g.sweep(k)
+        assert_same_state(o, g, True)
+    assert sum(g.path_sweeps()) == 10
 
 
 @pytest.mark.parametrize("fp32", [False, True])
