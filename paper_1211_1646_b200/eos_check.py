@@ -1,0 +1,85 @@
+#!/usr/bin/env python
+"""One equation-of-state point with the paper's pressure estimator (eq. 4-6): pair-distance histogram
+near contact with dr = 1e-4 sigma on (sigma, 1.02 sigma], sampled every 200 sweeps, degree-5 polynomial fit extrapolated to
+r = sigma.  Default: N = 256^2, phi = 0.698, the liquid point of Table 2 (L399: P* = 9.1709(1) MPMC, 9.1708(4) event-chain).
+Uses the CUDA library only (needs a GPU).  The box is the 2/sqrt(3) rectangle of the BASELINE configs, not the paper's
+square, and the proposal is the square of reading A2; neither changes the ensemble.
+
+  python -m paper_1211_1646_b200.eos_check [--n 256] [--phi 0.698] [--equil 400000] [--sweeps 2000000] [--d 0.12]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import time
+
+import numpy as np
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--n", type=int, default=256, help="lattice side: N = n^2 disks")
+    ap.add_argument("--phi", type=float, default=0.698)
+    ap.add_argument("--d", type=float, default=0.12, help="maximum displacement per coordinate, in sigma")
+    ap.add_argument("--n-s", type=int, default=4)
+    ap.add_argument("--equil", type=int, default=400_000, help="sweeps discarded before sampling")
+    ap.add_argument("--sweeps", type=int, default=2_000_000, help="sampled sweeps")
+    ap.add_argument("--every", type=int, default=200, help="sweeps between histogram samples (L384)")
+    ap.add_argument("--blocks", type=int, default=10, help="blocks for the error estimate")
+    ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--fp64", action="store_true")
+    args = ap.parse_args()
+
+    import torch
+    from . import inputs as I
+    from .binding import Mpmc
+    xy, box = I.jittered_lattice(args.n, args.phi, seed=args.seed)
+    N = args.n * args.n
+    sim = Mpmc(N, box, 1.0, args.d, args.n_s, args.seed, fp32=not args.fp64, device="cuda:0")
+    sim.load_positions(torch.as_tensor(xy, device="cuda:0"))
+    dr, nbins, degree = 1e-4, 200, 5                      # L382
+    t0 = time.time()
+    sim.sweep(args.equil)
+    torch.cuda.synchronize()
+    t_eq = time.time() - t0
+    a0 = sim.acceptance()
+    nsamp = args.sweeps // args.every
+    per_block = max(1, nsamp // args.blocks)
+    hist_block = np.zeros((args.blocks, nbins), dtype=np.float64)
+    t0 = time.time()
+    for i in range(per_block * args.blocks):
+        sim.sweep(args.every)
+        hist_block[i // per_block] += sim.contact_histogram(dr, nbins)
+    torch.cuda.synchronize()
+    t_run = time.time() - t0
+    a1 = sim.acceptance()
+    L = sim.L_eff
+    rho = N / (L[0] * L[1])
+
+    def p_star(hist, samples):
+        # eq. 5-6 (L374-379): g(R_i) = 2 H_i / (N rho 2 pi R_i dr) per sample; unweighted degree-5 fit; eq. 4 (L368)
+        r0 = 1.0 + dr * np.arange(nbins); r1 = r0 + dr
+        R = (2.0 / 3.0) * (r1 ** 3 - r0 ** 3) / (r1 ** 2 - r0 ** 2)
+        g = 2.0 * hist / samples / (N * rho * 2.0 * np.pi * R * dr)
+        c = np.polynomial.polynomial.polyfit((R - 1.0) / (dr * nbins), g, degree)
+        return rho * (1.0 + 0.5 * np.pi * rho * c[0]), c[0]
+
+    p_all, g_all = p_star(hist_block.sum(axis=0), per_block * args.blocks)
+    p_blocks = np.array([p_star(h, per_block)[0] for h in hist_block])
+    out = {
+        "N": N, "phi": args.phi, "box": list(L), "cells": [sim.mx, sim.my], "d": args.d, "n_s": args.n_s,
+        "dtype": "f64" if args.fp64 else "f32", "equil_sweeps": args.equil, "sampled_sweeps": per_block * args.blocks * args.every,
+        "samples": per_block * args.blocks, "P_star": p_all, "g_contact": g_all,
+        "P_star_block_mean": float(p_blocks.mean()), "P_star_stderr": float(p_blocks.std(ddof=1) / np.sqrt(args.blocks)),
+        "P_star_blocks": [float(v) for v in p_blocks],
+        "acceptance": (a1[1] - a0[1]) / max(1, a1[0] - a0[0]),
+        "paper": {"P_star_MPMC": 9.1709, "P_star_event_chain": 9.1708, "citation": "PAPER.md L399 (Table 2, phi = 0.698, N = 256^2)"}
+        if abs(args.phi - 0.698) < 1e-9 else None,
+        "moves_per_s_incl_sampling": (a1[0] - a0[0]) / t_run, "seconds": {"equilibration": t_eq, "sampling": t_run},
+        "path_sweeps": sim.path_sweeps(),
+    }
+    print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    main()
