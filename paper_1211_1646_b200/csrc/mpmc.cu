@@ -28,6 +28,7 @@ struct mpmc_ctx {
   const void* tile_kernel; // the k_tile_sweep instantiation, or nullptr when the tile path does not apply
   uint32_t tile_grid;      // tiles = CTAs of the tile kernel
   size_t tile_smem;        // its dynamic shared memory
+  uint32_t tile_threads;   // threads per CTA of the tile kernel
   uint64_t t_host;         // sweeps requested since the last load (the sweep index the device will reach)
   int sticky;
 };
@@ -294,14 +295,23 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
     const size_t stat = (fp32 ? sizeof(CrowdList<float>) : sizeof(CrowdList<double>)) + 256;   // static shared memory
     const size_t smem_max = (size_t)smem_optin > stat ? (size_t)smem_optin - stat : 0;
     uint32_t ntx = 0, nty = 0, PS = 0;
-    if (choose_tiling(p.hx, p.hy, cell_bytes, smem_max, (uint32_t)sms, &ntx, &nty, &PS)) {
+    c->tile_threads = fp32 ? TileThreads<float>::value : TileThreads<double>::value;
+    bool have = choose_tiling(p.hx, p.hy, cell_bytes, smem_max, (uint32_t)sms, &ntx, &nty, &PS);
+    if (const char* e = std::getenv("MPMC_TILE")) {        // experiments: "ntx,nty,threads"
+      unsigned a = 0, b = 0, th = 0;
+      if (std::sscanf(e, "%u,%u,%u", &a, &b, &th) == 3 && a && b && th && th <= c->tile_threads && a <= p.hx && b <= p.hy) {
+        const uint32_t pw = (2 * ((p.hx + a - 1) / a) + 2 * HALO) / 2, ph = (2 * ((p.hy + b - 1) / b) + 2 * HALO) / 2;
+        if ((size_t)4 * pw * ph * cell_bytes <= smem_max) { ntx = a; nty = b; PS = pw * ph; c->tile_threads = th; have = true; }
+      }
+    }
+    if (have) {
       c->tile_kernel = pick_tile_kernel(fp32, debug, n_s);
       c->tile_grid = ntx * nty;
       c->tile_smem = (size_t)4 * PS * cell_bytes;
       p.tl_ntx = ntx; p.tl_nty = nty; p.tl_PS = PS;
       if (std::getenv("MPMC_VERBOSE"))
-        std::fprintf(stderr, "[mpmc] tile kernel: %u x %u tiles, plane stride %u cells, %zu B shared memory, grid %u; general grid %u\n",
-                     ntx, nty, PS, c->tile_smem, c->tile_grid, c->grid);
+        std::fprintf(stderr, "[mpmc] tile kernel: %u x %u tiles, plane stride %u cells, %zu B shared memory, grid %u x %u threads; general grid %u\n",
+                     ntx, nty, PS, c->tile_smem, c->tile_grid, c->tile_threads, c->grid);
       if (cudaFuncSetAttribute(c->tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tile_smem) != cudaSuccess) {
         cudaGetLastError(); delete c; return MPMC_ERR_CUDA;
       }
@@ -368,7 +378,7 @@ int mpmc_sweep(mpmc_ctx* c, uint64_t k) {
     static const bool pdl = [] { const char* e = std::getenv("MPMC_PDL"); return !(e && e[0] == '0'); }();
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(c->tile_grid);
-    cfg.blockDim = dim3(c->fp32 ? TileThreads<float>::value : TileThreads<double>::value);
+    cfg.blockDim = dim3(c->tile_threads);
     cfg.dynamicSmemBytes = c->tile_smem; cfg.stream = c->stream;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;

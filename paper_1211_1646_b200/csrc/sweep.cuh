@@ -437,12 +437,13 @@ template <typename P> __device__ __forceinline__ Disk<P> pick(bool c, const Disk
 
 // The new cell from the slot pairs of its own old cell (a, ids ia) and of the old neighbour in direction f (b, ib),
 // both holding at most 2 disks (empty slot = sentinel): stayers in slot order, then entrants in slot order
-// (reading A13), compacted in registers.  Returns the new count; o01/i01 = slots 0, 1; o23/i23 = slots 2, 3
-// (meaningful when the count exceeds 2), empty slots = sentinel.
+// (reading A13), compacted in registers.  Returns the new count; o01/i01 = slots 0, 1 (empty slots = sentinel); `rest`
+// is what shift_pair_rest makes slots 2, 3 of when the count exceeds 2.
+template <typename P> struct ShiftRest { uint32_t ns; Disk<P> t0, t1; };   // what slots 2, 3 are made of (rarely needed)
 template <typename P, bool ALONG_X>
 __device__ __forceinline__ uint32_t shift_pair(const Half<P>& a, const Half<P>& b, const uint2 ia, const uint2 ib,
                                                const P step, const P back, const P w, Half<P>& o01, uint2& i01,
-                                               Half<P>& o23, uint2& i23) {
+                                               ShiftRest<P>& rest) {
   using R = Real<P>;
   const P FAR = R::far_away(), HALF_FAR = FAR * (P)0.5;
   // lines 7-14 (L299-312): own disks that stay; a sentinel stays a sentinel and fails the test
@@ -463,11 +464,18 @@ __device__ __forceinline__ uint32_t shift_pair(const Half<P>& a, const Half<P>& 
   const Disk<P> t0 = pick(ne > 0u, pick(g0, e0, e1), none), t1 = pick(ne > 1u, e1, none);
   const Disk<P> r0 = pick(ns > 0u, s0, t0);
   const Disk<P> r1 = pick(ns == 2u, o1, pick(ns == 1u, t0, t1));
-  const Disk<P> r2 = pick(ns == 2u, t0, pick(ns == 1u, t1, none));
-  const Disk<P> r3 = pick(ns == 2u, t1, none);
   o01.x = R::pair(r0.x, r1.x); o01.y = R::pair(r0.y, r1.y); i01 = make_uint2(r0.id, r1.id);
-  o23.x = R::pair(r2.x, r3.x); o23.y = R::pair(r2.y, r3.y); i23 = make_uint2(r2.id, r3.id);
+  rest.ns = ns; rest.t0 = t0; rest.t1 = t1;
   return ns + ne;
+}
+// slots 2, 3 of the new cell (count above 2): what is left of the entrants after slots 0, 1
+template <typename P>
+__device__ __forceinline__ void shift_pair_rest(const ShiftRest<P>& rest, Half<P>& o23, uint2& i23) {
+  using R = Real<P>;
+  const Disk<P> none = {R::far_away(), R::far_away(), 0xFFFFFFFFu};
+  const Disk<P> r2 = pick(rest.ns == 2u, rest.t0, pick(rest.ns == 1u, rest.t1, none));
+  const Disk<P> r3 = pick(rest.ns == 2u, rest.t1, none);
+  o23.x = R::pair(r2.x, r3.x); o23.y = R::pair(r2.y, r3.y); i23 = make_uint2(r2.id, r3.id);
 }
 
 // one new cell; ALONG_X and POSITIVE are uniform across the grid, so the caller branches once
@@ -506,11 +514,15 @@ __device__ __forceinline__ void shift_cell(const Params& p, Ctl* ctl, const uint
   const uint2 ia = idsc[own], ib = idsc[nb];
   uint32_t nn;
   if (n0 <= 2u && n1 <= 2u) {
-    Half<P> o01, o23; uint2 i01, i23;
-    nn = shift_pair<P, ALONG_X>(a, b, ia, ib, step, back, w, o01, i01, o23, i23);
+    Half<P> o01; uint2 i01; ShiftRest<P> rest;
+    nn = shift_pair<P, ALONG_X>(a, b, ia, ib, step, back, w, o01, i01, rest);
     st_half(posn, own, o01);
     idsn[own] = i01;
-    if (nn > 2u) { st_half(posn, own + Mqp, o23); idsn[own + Mqp] = i23; }
+    if (nn > 2u) {
+      Half<P> o23; uint2 i23;
+      shift_pair_rest<P>(rest, o23, i23);
+      st_half(posn, own + Mqp, o23); idsn[own + Mqp] = i23;
+    }
   } else {
     // generic: any occupancy, rolled loops, scalar accesses
     nn = 0;

@@ -375,6 +375,96 @@ __device__ __forceinline__ void tile_sub_sweep_cells(const Params& p, SmemCell<P
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// The shift of the interior cells of a tile (Algorithm 4, pull form: one thread per NEW cell, L350), from the
+// planes in shared memory to the other global buffer.  Warps draw chunks of 64 cells of one local colour plane
+// from shared counters, two cells per lane: the four id loads of a lane are in flight together, and consecutive
+// lanes write consecutive cells of one global colour plane.  Everything that depends only on the plane (colours,
+// the neighbour's offset, the index constants) is uniform.
+// ---------------------------------------------------------------------------------------------------------
+template <typename P, bool ALONG_X>
+__device__ __forceinline__ void tile_shift_cells(const Params& p, const SmemCell<P>* sm, const CrowdList<P>& cl,
+                                                 const uint32_t nc, const TileBox& tb, const int gx0, const int gy0,
+                                                 const bool positive, const P delta, const uint32_t cur,
+                                                 const uint32_t crowd_slot, uint32_t* next) {
+  using R = Real<P>;
+  const uint32_t nxt = cur ^ 1u, Mqp = p.Mqp, PS = p.tl_PS, pw = tb.pw, lane = threadIdx.x & 31u;
+  const P w = ALONG_X ? R::wx(p) : R::wy(p);
+  const P step = positive ? -delta : delta;     // l' = l - f*delta   (L303)
+  const P back = positive ? w : -w;             // entrant translation (L332)
+  const uint2* idsc = reinterpret_cast<const uint2*>(p.ids[cur]);
+  P* posn = reinterpret_cast<P*>(p.pos[nxt]);
+  uint2* idsn = reinterpret_cast<uint2*>(p.ids[nxt]);
+  uint8_t* cntn = p.cnt[nxt];
+  const uint32_t hTX = tb.TX >> 1, per_plane = hTX * (tb.TY >> 1);
+  const uint32_t inv = small_div_magic(hTX);
+  const int dox = ALONG_X ? (positive ? 1 : -1) : 0, doy = ALONG_X ? 0 : (positive ? 1 : -1);
+#pragma unroll 1
+  for (uint32_t q = 0; q < 4u; ++q) {
+    const uint32_t qx = q & 1u, qy = q >> 1;
+    const uint32_t px0 = (HALO - qx + 1u) >> 1, py0 = (HALO - qy + 1u) >> 1;
+    const int nboff = neighbour_offset(q, dox, doy, PS, pw);         // the old neighbour in direction f (L314-317)
+    // the region starts at an odd cell, so the global colour of local colour q is q ^ 3 and, with arithmetic shifts,
+    // gx >> 1 = px + ((gx0 + qx) >> 1): the index of an interior cell in its global plane is py*hx + px + constant
+    const uint32_t Qg = q ^ 3u, Qn = Qg ^ (ALONG_X ? 1u : 2u);
+    const int chx = (gx0 + (int)qx) >> 1, chy = (gy0 + (int)qy) >> 1;
+    const int cbase = chy * (int)p.hx + chx;
+    // the neighbour's index in ITS plane: same half-coordinate or the next/previous one, by the parity of this colour
+    const int bit = ALONG_X ? (int)(Qg & 1u) : (int)(Qg >> 1);
+    const int dh = positive ? bit : bit - 1;                         // (g + 1) >> 1 - (g >> 1) = bit; (g - 1) >> 1 - (g >> 1) = bit - 1
+    const int hn = ALONG_X ? (int)p.hx : (int)p.hy;                  // half-cells along the shift axis
+    for (;;) {
+      uint32_t base = 0;
+      if (lane == 0u) base = atomicAdd(&next[q], 64u);
+      base = __shfl_sync(0xFFFFFFFFu, base, 0);
+      if (base >= per_plane) break;
+      uint32_t si[2], sn[2], own[2], nbg[2], cell[2];
+      bool ok[2], general[2];
+      uint2 ia[2], ib[2];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const uint32_t idx = base + lane + 32u * (uint32_t)u;
+        ok[u] = idx < per_plane;
+        const uint32_t id2 = ok[u] ? idx : 0u;
+        const uint32_t ry = small_div(id2, inv), rx = id2 - ry * hTX;
+        const uint32_t px = px0 + rx, py = py0 + ry;
+        si[u] = q * PS + py * pw + px; sn[u] = (uint32_t)((int)si[u] + nboff);
+        const int hxg = (int)px + chx, hyg = (int)py + chy;            // half-coordinates in the global plane
+        const int cig = (int)(py * p.hx + px) + cbase;
+        int hnb = (ALONG_X ? hxg : hyg) + dh;                          // neighbour's half-coordinate, wrapped
+        hnb = hnb < 0 ? hnb + hn : (hnb >= hn ? hnb - hn : hnb);
+        const int cin = ALONG_X ? hyg * (int)p.hx + hnb : hnb * (int)p.hx + hxg;
+        own[u] = 2u * Qg * Mqp + (uint32_t)cig; nbg[u] = 2u * Qn * Mqp + (uint32_t)cin;
+        cell[u] = (uint32_t)(2 * hyg + (int)(Qg >> 1)) * p.mx + (uint32_t)(2 * hxg + (int)(Qg & 1u));
+        general[u] = nc != 0u && (crowd_find(cl, nc, si[u]) >= 0 || crowd_find(cl, nc, sn[u]) >= 0);
+        if (ok[u] && !general[u]) { ia[u] = idsc[own[u]]; ib[u] = idsc[nbg[u]]; }
+      }
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        if (!ok[u]) continue;
+        const uint32_t cnt_g = own[u] - Qg * Mqp;                      // Qg*Mqp + cig
+        if (general[u]) {
+          tile_shift_cell_general<P>(p, sm, cl, nc, si[u], sn[u], own[u], nbg[u], cnt_g, cell[u], ALONG_X, step, back, w, cur,
+                                     crowd_slot);
+          continue;
+        }
+        const Half<P> a = lds_half(sm, si[u]), b = lds_half(sm, sn[u]);
+        Half<P> o01; uint2 i01; ShiftRest<P> rest;
+        const uint32_t nn = shift_pair<P, ALONG_X>(a, b, ia[u], ib[u], step, back, w, o01, i01, rest);
+        st_half(posn, own[u], o01);
+        idsn[own[u]] = i01;
+        if (nn > 2u) {                            // a crowded cell of the new state
+          Half<P> o23; uint2 i23;
+          shift_pair_rest<P>(rest, o23, i23);
+          st_half(posn, own[u] + Mqp, o23); idsn[own[u] + Mqp] = i23;
+          note_crowded(p.ctl, crowd_slot, cell[u]);
+        }
+        cntn[cnt_g] = (uint8_t)nn;                // L280, L342
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // The fused sweep kernel: one CTA per tile, one launch per sweep.  See the header of this file.
 // Dynamic shared memory: 4 planes x tl_PS cells x sizeof(SmemCell<P>).
 // ---------------------------------------------------------------------------------------------------------
@@ -382,7 +472,7 @@ template <typename P, int NS, bool DEBUG>
 __global__ void __launch_bounds__(TileThreads<P>::value, 1)
 k_tile_sweep(const __grid_constant__ Params p) {
   using R = Real<P>;
-  constexpr uint32_t TILE_THREADS = TileThreads<P>::value;
+  const uint32_t TILE_THREADS = blockDim.x;           // at most TileThreads<P>::value (the host may launch fewer)
   extern __shared__ __align__(16) unsigned char tile_smem[];
   SmemCell<P>* sm = reinterpret_cast<SmemCell<P>*>(tile_smem);
   __shared__ CrowdList<P> cl;
@@ -415,7 +505,7 @@ k_tile_sweep(const __grid_constant__ Params p) {
     const P* posc = reinterpret_cast<const P*>(p.pos[cur]);
     // four plane rows x two 32-cell column blocks per warp and pass: eight independent loads in flight per lane
     // before the first shared-memory store (a load -> store chain per row would expose the L2 latency every time)
-    constexpr uint32_t NW = TILE_THREADS / 32;
+    const uint32_t NW = TILE_THREADS / 32;
     const uint32_t nrows = 4u * ph, inv_ph = small_div_magic(ph);
     for (uint32_t c0 = 0; c0 < pw; c0 += 64u) {
       for (uint32_t r0 = warp; r0 < nrows; r0 += 4u * NW) {
@@ -501,59 +591,8 @@ k_tile_sweep(const __grid_constant__ Params p) {
   const bool along_x = dir < 2u, positive = (dir & 1u) == 0u;
   const P w = along_x ? R::wx(p) : R::wy(p);
   const P delta = R::mul(R::mul((P)0.5, w), R::unit(dr.dist_word));   // line 15 (L90)
-  {
-    const P step = positive ? -delta : delta;     // l' = l - f*delta   (L303)
-    const P back = positive ? w : -w;             // entrant translation (L332)
-    const uint2* idsc = reinterpret_cast<const uint2*>(p.ids[cur]);
-    P* posn = reinterpret_cast<P*>(p.pos[nxt]);
-    uint2* idsn = reinterpret_cast<uint2*>(p.ids[nxt]);
-    uint8_t* cntn = p.cnt[nxt];
-    const uint32_t hTX = tb.TX >> 1, per_plane = hTX * (tb.TY >> 1);
-    const uint32_t inv = small_div_magic(hTX);
-    const int dox = along_x ? (positive ? 1 : -1) : 0, doy = along_x ? 0 : (positive ? 1 : -1);
-    // The interior cells of the four local colour planes in chunks of 32 that the warps draw from shared counters;
-    // consecutive lanes write consecutive cells of one global colour plane.
-#pragma unroll 1
-    for (uint32_t q = 0; q < 4u; ++q) {
-      const uint32_t qx = q & 1u, qy = q >> 1;
-      const uint32_t px0 = (HALO - qx + 1u) >> 1, py0 = (HALO - qy + 1u) >> 1;
-      const int nboff = neighbour_offset(q, dox, doy, PS, pw);       // the old neighbour in direction f (L314-317)
-      for (;;) {
-        uint32_t base = 0;
-        if (lane == 0u) base = atomicAdd(&s_next[4u + q], 32u);
-        base = __shfl_sync(0xFFFFFFFFu, base, 0);
-        if (base >= per_plane) break;
-        const uint32_t idx = base + lane;
-        if (idx >= per_plane) continue;
-        const uint32_t ry = small_div(idx, inv), rx = idx - ry * hTX;
-        const uint32_t px = px0 + rx, py = py0 + ry, lx = 2u * px + qx, ly = 2u * py + qy;
-        const uint32_t si = q * PS + py * pw + px, sn = (uint32_t)((int)si + nboff);
-        const uint32_t gx = (uint32_t)(gx0 + (int)lx), gy = (uint32_t)(gy0 + (int)ly);      // interior: no wrap
-        const uint32_t gxn = wrap_cell((int)gx + dox, p.mx), gyn = wrap_cell((int)gy + doy, p.my);
-        const uint32_t Qg = ((gy & 1u) << 1) | (gx & 1u), Qn = ((gyn & 1u) << 1) | (gxn & 1u);
-        const uint32_t cig = (gy >> 1) * p.hx + (gx >> 1), cin = (gyn >> 1) * p.hx + (gxn >> 1);
-        const uint32_t own = 2u * Qg * Mqp + cig, nbg = 2u * Qn * Mqp + cin;
-        if (nc != 0u && (crowd_find(cl, nc, si) >= 0 || crowd_find(cl, nc, sn) >= 0)) {
-          tile_shift_cell_general<P>(p, sm, cl, nc, si, sn, own, nbg, Qg * Mqp + cig, gy * p.mx + gx, along_x, step, back, w,
-                                     cur, slot1);
-          continue;
-        }
-        const uint2 ia = idsc[own], ib = idsc[nbg];
-        const Half<P> a = lds_half(sm, si), b = lds_half(sm, sn);
-        Half<P> o01, o23; uint2 i01, i23;
-        uint32_t nn;
-        if (along_x) nn = shift_pair<P, true>(a, b, ia, ib, step, back, w, o01, i01, o23, i23);
-        else         nn = shift_pair<P, false>(a, b, ia, ib, step, back, w, o01, i01, o23, i23);
-        st_half(posn, own, o01);
-        idsn[own] = i01;
-        if (nn > 2u) {                            // a crowded cell of the new state
-          st_half(posn, own + Mqp, o23); idsn[own + Mqp] = i23;
-          note_crowded(ctl, slot1, gy * p.mx + gx);
-        }
-        cntn[Qg * Mqp + cig] = (uint8_t)nn;       // L280, L342
-      }
-    }
-  }
+  if (along_x) tile_shift_cells<P, true>(p, sm, cl, nc, tb, gx0, gy0, positive, delta, cur, slot1, &s_next[4]);
+  else         tile_shift_cells<P, false>(p, sm, cl, nc, tb, gx0, gy0, positive, delta, cur, slot1, &s_next[4]);
 
   // ---- counters; the last CTA to finish advances the control block ----
   flush_tally(p, tally);
