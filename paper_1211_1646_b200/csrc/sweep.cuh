@@ -1,5 +1,7 @@
-// sweep.cuh — the hot kernels: the active-cell sub-sweep (Algorithm 2) in two forms and the
-// cell shift / re-bin (Algorithm 4), re-designed for sm_100a.  See DESIGN.md "Kernels".
+// sweep.cuh — the general path: the cell update (Algorithm 2) in two register-resident forms and
+// the cell shift / re-bin (Algorithm 4) on the colour planes in global memory, driven by the persistent
+// cooperative kernel k_sweeps (any cell width up to sqrt(2) sigma, any n_s).  The fused tile kernel for w ~ sigma
+// (tile.cuh) reuses shift_pair, the tallies and the visiting permutation from here.  See DESIGN.md "Kernels".
 #pragma once
 #include "common.cuh"
 
@@ -66,7 +68,7 @@ __device__ __forceinline__ uint32_t visiting_permutation(const uint32_t n, const
 
 // ---------------------------------------------------------------------------------------------------------
 // Generic cell update: Algorithm 2 line by line on the slots in global memory, any occupancy up to n_max.
-// Used by the fast kernel for the rare cells whose 3x3 neighbourhood holds a cell with more than 2 disks.
+// Used by update_cell_fast for the rare cells whose 3x3 neighbourhood holds a cell with more than 2 disks.
 // Deliberately compact (rolled loops, scalar arithmetic): it runs for a handful of lanes.
 // ---------------------------------------------------------------------------------------------------------
 template <typename P>
@@ -133,9 +135,9 @@ __device__ __forceinline__ void flush_tally(const Params& p, const Tally& tl) {
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Fast sub-sweep kernel for cell widths w ~ sigma (the BASELINE configs: occupancy 0/1/2 per cell).
-// One thread per cell of the active checkerboard set (the paper's mapping, L158/L260) over the dense colour
-// plane, so a warp's 32 cells are contiguous.
+// Fast cell update for cell widths w ~ sigma (occupancy 0/1/2 per cell), one thread per cell of the active
+// checkerboard set (the paper's mapping, L158/L260) over the dense colour plane in global memory, so a warp's 32 cells
+// are contiguous.  (The tile kernel's tile_update_cell is the same arithmetic on shared memory.)
 //
 //  * each of the 3x3 cells is ONE load of its slot pair {x0, x1, y0, y1} (128 bit in fp32), issued up front and
 //    unconditionally; empty slots hold the far-away sentinel (the paper's (-10,-10) trick, L295/L346), so the
@@ -262,7 +264,7 @@ __device__ __forceinline__ void update_cell_fast(const Params& p, const uint32_t
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// General sub-sweep kernel: any occupancy up to n_max = 4 per cell — the paper's own regime, w up to
+// General cell update: any occupancy up to n_max = 4 per cell — the paper's own regime, w up to
 // sqrt(2) sigma (L152) — and any n_s.  Same mapping and arithmetic; all four slots of the 3x3 cells are kept
 // in registers (own cell as two negated pairs, each neighbour as two translated, negated pairs; slot pair 1 is
 // loaded only where n > 2), and the disk a move acts on is chosen with select chains from the visiting
