@@ -289,7 +289,9 @@ __device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* s
   }
 }
 
-// General shift of one interior cell (rare: it or its source neighbour is crowded): Algorithm 4 line by line.
+// General shift of one interior cell (rare: it or its source neighbour is crowded): Algorithm 4 with up to 4 disks
+// in each of the two old cells.  Straight-line code on registers (eight candidates, four output slots filled by
+// prefix count), because the whole tile waits for the thread that runs it.
 template <typename P>
 __device__ __noinline__ void tile_shift_cell_general(const Params& p, const SmemCell<P>* sm, const CrowdList<P>& cl,
                                                      const uint32_t nc, const uint32_t si_own, const uint32_t si_nb,
@@ -300,36 +302,44 @@ __device__ __noinline__ void tile_shift_cell_general(const Params& p, const Smem
   const uint32_t nxt = cur ^ 1u, Mqp = p.Mqp;
   const P FAR = R::far_away(), HALF_FAR = FAR * (P)0.5;
   const uint2* idsc = reinterpret_cast<const uint2*>(p.ids[cur]);
-  P ox[NMAX + 1], oy[NMAX + 1]; uint32_t oid[NMAX + 1];
-  uint32_t nn = 0;
-#pragma unroll 1
-  for (uint32_t pass = 0; pass < 2u; ++pass) {                   // own disks that stay, then the neighbour's leavers
-    const uint32_t si = pass ? si_nb : si_own, g = pass ? nb_g : own_g;
-    const Half<P> h = lds_half(sm, si);
-    P jx[NMAX] = {h.x.x, h.x.y, FAR, FAR}, jy[NMAX] = {h.y.x, h.y.y, FAR, FAR};
-    uint32_t jid[NMAX] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
-    const uint2 i01 = idsc[g];
-    jid[0] = i01.x; jid[1] = i01.y;
-    const int e = crowd_find(cl, nc, si);
-    if (e >= 0) {
-      jx[2] = cl.e[e].hi.x.x; jx[3] = cl.e[e].hi.x.y; jy[2] = cl.e[e].hi.y.x; jy[3] = cl.e[e].hi.y.y;
-      const uint2 i23 = idsc[g + Mqp];
-      jid[2] = i23.x; jid[3] = i23.y;
-    }
-    for (uint32_t i = 0; i < (uint32_t)NMAX; ++i) {
-      if (!(jx[i] < HALF_FAR)) continue;                         // empty slot
-      P x = jx[i], y = jy[i];
-      P m = R::add(along_x ? x : y, step);                       // l' = l - f*delta  (L303)
-      const bool in = m > (P)0 && m <= w;
-      if (pass ? in : !in) continue;                             // own leavers go elsewhere; neighbour's stayers stay
-      if (pass) m = R::add(m, back);                             // L332, after the test (L352)
-      if (along_x) x = m; else y = m;
-      if (nn < (uint32_t)NMAX) { ox[nn] = x; oy[nn] = y; oid[nn] = jid[i]; }
-      ++nn;
+  // candidates 0-3: the own old cell (stay if still inside), 4-7: the old neighbour in direction f (enter if they left it)
+  const int eo = crowd_find(cl, nc, si_own), en = crowd_find(cl, nc, si_nb);
+  const uint2 io01 = idsc[own_g], in01 = idsc[nb_g];
+  uint2 io23 = make_uint2(0xFFFFFFFFu, 0xFFFFFFFFu), in23 = io23;
+  if (eo >= 0) io23 = idsc[own_g + Mqp];
+  if (en >= 0) in23 = idsc[nb_g + Mqp];
+  const Half<P> ho = lds_half(sm, si_own), hn = lds_half(sm, si_nb);
+  Half<P> go, gn;
+  go.x = R::pair(FAR, FAR); go.y = go.x; gn = go;
+  if (eo >= 0) go = cl.e[eo].hi;
+  if (en >= 0) gn = cl.e[en].hi;
+  P cx[8] = {ho.x.x, ho.x.y, go.x.x, go.x.y, hn.x.x, hn.x.y, gn.x.x, gn.x.y};
+  P cy[8] = {ho.y.x, ho.y.y, go.y.x, go.y.y, hn.y.x, hn.y.y, gn.y.x, gn.y.y};
+  const uint32_t cid[8] = {io01.x, io01.y, io23.x, io23.y, in01.x, in01.y, in23.x, in23.y};
+  bool take[8];
+  uint32_t pos[8], nn = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const bool occupied = cx[i] < HALF_FAR;
+    P m = R::add(along_x ? cx[i] : cy[i], step);                 // l' = l - f*delta  (L303)
+    const bool in = m > (P)0 && m <= w;
+    take[i] = occupied && (i < 4 ? in : !in);                    // own disks that stay; the neighbour's that left it (L326-328)
+    if (i >= 4) m = R::add(m, back);                             // L332, after the test (L352)
+    if (along_x) cx[i] = m; else cy[i] = m;
+    pos[i] = nn;
+    nn += take[i] ? 1u : 0u;
+  }
+  P ox[NMAX], oy[NMAX]; uint32_t oid[NMAX];
+#pragma unroll
+  for (int j = 0; j < NMAX; ++j) {
+    ox[j] = FAR; oy[j] = FAR; oid[j] = 0xFFFFFFFFu;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const bool here = take[i] && pos[i] == (uint32_t)j;
+      ox[j] = here ? cx[i] : ox[j]; oy[j] = here ? cy[i] : oy[j]; oid[j] = here ? cid[i] : oid[j];
     }
   }
   if (nn > (uint32_t)NMAX) { atomicOr(&p.ctl->err, ERRBIT_OVERFLOW); nn = NMAX; }
-  for (uint32_t i = nn; i < (uint32_t)NMAX; ++i) { ox[i] = FAR; oy[i] = FAR; oid[i] = 0xFFFFFFFFu; }
   P* posn = reinterpret_cast<P*>(p.pos[nxt]);
   uint2* idsn = reinterpret_cast<uint2*>(p.ids[nxt]);
   Half<P> o;
@@ -398,6 +408,23 @@ __device__ __forceinline__ void tile_shift_cells(const Params& p, const SmemCell
   const uint32_t hTX = tb.TX >> 1, per_plane = hTX * (tb.TY >> 1);
   const uint32_t inv = small_div_magic(hTX);
   const int dox = ALONG_X ? (positive ? 1 : -1) : 0, doy = ALONG_X ? 0 : (positive ? 1 : -1);
+  // The few interior cells that are crowded or pull from a crowded cell take the rolled general routine; they are
+  // done first, by the first threads, so that its latency overlaps the chunks the other warps draw meanwhile.
+  for (uint32_t pi = threadIdx.x; pi < 2u * nc; pi += blockDim.x) {
+    const uint32_t e = pi >> 1, role = pi & 1u;                      // role 0: the listed cell; role 1: the cell pulling from it
+    const uint32_t lx = (cl.e[e].lxly & 0xFFFFu) - (role ? (uint32_t)dox : 0u);
+    const uint32_t ly = (cl.e[e].lxly >> 16) - (role ? (uint32_t)doy : 0u);
+    if (!(lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY)) continue;      // not an interior cell of this tile
+    const uint32_t q = ((ly & 1u) << 1) | (lx & 1u);
+    const uint32_t si = q * PS + (ly >> 1) * pw + (lx >> 1), sn = (uint32_t)((int)si + neighbour_offset(q, dox, doy, PS, pw));
+    if (role && crowd_find(cl, nc, si) >= 0) continue;               // listed itself: done in its own role 0
+    const uint32_t gx = (uint32_t)(gx0 + (int)lx), gy = (uint32_t)(gy0 + (int)ly);    // interior: no wrap
+    const uint32_t gxn = wrap_cell((int)gx + dox, p.mx), gyn = wrap_cell((int)gy + doy, p.my);
+    const uint32_t Qg = ((gy & 1u) << 1) | (gx & 1u), Qn = ((gyn & 1u) << 1) | (gxn & 1u);
+    const uint32_t cig = (gy >> 1) * p.hx + (gx >> 1), cin = (gyn >> 1) * p.hx + (gxn >> 1);
+    tile_shift_cell_general<P>(p, sm, cl, nc, si, sn, 2u * Qg * Mqp + cig, 2u * Qn * Mqp + cin, Qg * Mqp + cig, gy * p.mx + gx,
+                               ALONG_X, step, back, w, cur, crowd_slot);
+  }
 #pragma unroll 1
   for (uint32_t q = 0; q < 4u; ++q) {
     const uint32_t qx = q & 1u, qy = q >> 1;
@@ -442,11 +469,7 @@ __device__ __forceinline__ void tile_shift_cells(const Params& p, const SmemCell
       for (int u = 0; u < 2; ++u) {
         if (!ok[u]) continue;
         const uint32_t cnt_g = own[u] - Qg * Mqp;                      // Qg*Mqp + cig
-        if (general[u]) {
-          tile_shift_cell_general<P>(p, sm, cl, nc, si[u], sn[u], own[u], nbg[u], cnt_g, cell[u], ALONG_X, step, back, w, cur,
-                                     crowd_slot);
-          continue;
-        }
+        if (general[u]) continue;                                      // done above
         const Half<P> a = lds_half(sm, si[u]), b = lds_half(sm, sn[u]);
         Half<P> o01; uint2 i01; ShiftRest<P> rest;
         const uint32_t nn = shift_pair<P, ALONG_X>(a, b, ia[u], ib[u], step, back, w, o01, i01, rest);
