@@ -41,7 +41,7 @@ enum {
   OR_ERR_CELL_OVERFLOW = -5,
   OR_ERR_STATE = -7,
 };
-enum { OR_FP64 = 1u, OR_FP32 = 2u };
+enum { OR_FP64 = 1u, OR_FP32 = 2u, OR_DISC = 4u };   // OR_DISC: trial displacement uniform in the disc of radius d (L190)
 
 // ---------------------------------------------------------------------------------------------
 // Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11): 10 rounds; multipliers 0xD2511F53, 0xCD9E8D57;
@@ -70,6 +70,9 @@ void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]
 // Counter layout (reading A9): counter = (cell_id, t_lo, t_hi, slot), key = (seed_lo, seed_hi).
 //   slot q in [0, ceil(n_s/2)): the displacement words of trial moves 2q (words 0, 1 = x, y) and
 //                             2q + 1 (words 2, 3 = x, y) — all four words of a Philox block are used
+//   with the disc proposal (flag OR_DISC; the paper's rng.inCircle(d), L190): block (s | j << 16), j = 0, 1, ...,
+//                             serves the candidate pairs 2j (words 0, 1) and 2j + 1 (words 2, 3) of trial move s; the
+//                             first pair inside the unit disc is taken (rejection from the square)
 //   slot 0x80000000         : the shuffle words of the cell
 //   cell 0xFFFFFFFF, slot 0xFFFFFFFF : per-sweep set order + shift direction
 //   cell 0xFFFFFFFF, slot 0xFFFFFFFE : per-sweep shift distance
@@ -208,11 +211,23 @@ struct Sim : Base {
     for (uint32_t s = 0; s < n_s; ++s) {                        // line 11 (L189)
       const uint32_t k = visit(perm, nc, s);
       uint32_t R[4];
-      draw(seed, (uint32_t)c, t, s >> 1, R);                    // reading A9: block s/2 serves moves 2q, 2q+1
-      const uint32_t h = 2u * (s & 1u);
-      // line 12 (L190); reading A2: uniform in the square [-d, d]^2
-      const P ddx = d * Variate<P>::sym(R[h]);
-      const P ddy = d * Variate<P>::sym(R[h + 1]);
+      P ddx, ddy;
+      if (!(flags & OR_DISC)) {
+        draw(seed, (uint32_t)c, t, s >> 1, R);                  // reading A9: block s/2 serves moves 2q, 2q+1
+        const uint32_t h = 2u * (s & 1u);
+        // line 12 (L190); reading A2: uniform in the square [-d, d]^2
+        ddx = d * Variate<P>::sym(R[h]);
+        ddy = d * Variate<P>::sym(R[h + 1]);
+      } else {
+        // line 12 as printed: rng.inCircle(d) (L190), uniform in the disc of radius d, by rejection from the square:
+        // candidate pairs (ux, uy) in order until rn(fma(ux, ux, rn(uy*uy))) <= 1
+        for (uint32_t j = 0;; ++j) {
+          if ((j & 1u) == 0u) draw(seed, (uint32_t)c, t, s | ((j >> 1) << 16), R);
+          const P ux = Variate<P>::sym(R[2u * (j & 1u)]), uy = Variate<P>::sym(R[2u * (j & 1u) + 1u]);
+          const P yy = uy * uy;
+          if (std::fma(ux, ux, yy) <= (P)1) { ddx = d * ux; ddy = d * uy; break; }
+        }
+      }
       const P Mx = lx[c * NMAX + k] + ddx;
       const P My = ly[c * NMAX + k] + ddy;
       counters[0] += 1;
@@ -512,6 +527,7 @@ int oracle_create(oracle_ctx** out, uint64_t N, const double box[2], double sigm
                   uint64_t seed, uint32_t flags, double w_target) {
   if (!out || !box || N == 0 || N >= 0xFFFFFFFFull || !(sigma > 0) || !(d > 0) || n_s > 32) return OR_ERR_ARG;
   const bool f64 = (flags & OR_FP64) != 0, f32 = (flags & OR_FP32) != 0;
+  if ((flags & OR_DISC) && n_s > 0xFFFFu) return OR_ERR_ARG;     // the move index shares the counter word with the attempt
   if (f64 == f32) return OR_ERR_ARG;
   Base* b = nullptr;
   const int st = f32 ? make<float>(&b, N, box, sigma, d, n_s, seed, flags, w_target)

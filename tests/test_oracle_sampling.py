@@ -32,6 +32,51 @@ def test_isolated_disk_acceptance(oracle_mod, fp32, d, box):
     assert acc / att == pytest.approx(expect, abs=0.006)
 
 
+@pytest.mark.parametrize("fp32", [False, True])
+@pytest.mark.parametrize("d,box", [(0.5, (2.6, 2.6)), (0.3, (2.2, 2.8))])
+def test_isolated_disk_acceptance_disc_proposal(oracle_mod, fp32, d, box):
+    """The paper's proposal, uniform in the disc of radius d (L190).  For a position uniform in the cell the move stays
+    with probability 1 - E|dx|/wx - E|dy|/wy + E|dx dy|/(wx wy), E|dx| = 4d/(3 pi), E|dx dy| = d^2/(2 pi) (disc
+    integrals, worked out by hand) — different from the square proposal's (1 - d/2wx)(1 - d/2wy)."""
+    o = oracle_mod.Oracle(1, box, 1.0, d, 4, 13, fp32=fp32, disc=True)
+    o.load_positions(np.array([[0.3, 0.4]]))
+    o.sweep(30000)
+    att, acc, rej_b, rej_o = o.acceptance()
+    assert att == 4 * 30000 and rej_o == 0
+    expect = 1 - 4 * d / (3 * math.pi) * (1 / o.wx + 1 / o.wy) + d * d / (2 * math.pi * o.wx * o.wy)
+    square = (1 - d / (2 * o.wx)) * (1 - d / (2 * o.wy))
+    assert acc / att == pytest.approx(expect, abs=0.006)
+    assert abs(acc / att - square) > 0.02            # the two proposals are told apart
+
+
+def test_disc_proposal_displacements_are_uniform_in_the_disc(oracle_mod):
+    """One disk in a wide cell (boundary rejections rare), n_s = 1: the displacement of every accepted move is a position
+    difference.  |delta| <= d always; r^2/d^2 uniform on [0, 1] (chi^2), mean r^2 = d^2/2 (the square would give 2d^2/3);
+    the angle uniform (chi^2 over 8 sectors)."""
+    d = 0.7
+    o = oracle_mod.Oracle(1, (60.0, 60.0), 1.0, d, 1, 5, fp32=False, w_target=30.0, disc=True)
+    assert (o.mx, o.my) == (2, 2)
+    o.load_positions(np.array([[15.0, 15.0]]))
+    prev = o.get_positions()[0].copy()
+    disp = []
+    for _ in range(6000):
+        o.sweep(1)
+        cur = o.get_positions()[0]
+        dd = cur - prev
+        dd -= np.round(dd / 60.0) * 60.0
+        if np.abs(dd).max() > 0:
+            disp.append(dd)
+        prev = cur.copy()
+    disp = np.array(disp)
+    assert len(disp) > 5000
+    r2 = (disp ** 2).sum(axis=1) / d ** 2
+    assert r2.max() <= 1.0 + 1e-12
+    assert r2.mean() == pytest.approx(0.5, abs=0.02)
+    assert stats.chisquare(np.histogram(r2, bins=10, range=(0, 1))[0]).pvalue > 1e-3
+    ang = np.arctan2(disp[:, 1], disp[:, 0])
+    assert stats.chisquare(np.histogram(ang, bins=8, range=(-math.pi, math.pi))[0]).pvalue > 1e-3
+
+
 def _excluded_disc_law(K, Le, sub=80):
     xs = (np.arange(K * sub) + 0.5) / (K * sub) * Le[0] - Le[0] / 2
     ys = (np.arange(K * sub) + 0.5) / (K * sub) * Le[1] - Le[1] / 2
@@ -40,10 +85,10 @@ def _excluded_disc_law(K, Le, sub=80):
     return ok.reshape(K, sub, K, sub).sum(axis=(1, 3)) / ok.sum()
 
 
-@pytest.mark.parametrize("fp32,seed", [(False, 1), (True, 2)])
-def test_two_disks_sample_uniform_law(oracle_mod, fp32, seed):
+@pytest.mark.parametrize("fp32,seed,disc", [(False, 1, False), (True, 2, False), (False, 3, True)])
+def test_two_disks_sample_uniform_law(oracle_mod, fp32, seed, disc):
     L = (2.6, 2.9)
-    o = oracle_mod.Oracle(2, L, 1.0, 0.4, 4, seed, fp32=fp32)
+    o = oracle_mod.Oracle(2, L, 1.0, 0.4, 4, seed, fp32=fp32, disc=disc)
     assert (o.mx, o.my) == (2, 2)          # one neighbour cell appears at two image offsets (A11)
     o.load_positions(np.array([[0.5, 0.5], [1.8, 1.9]]))
     S = 20000
