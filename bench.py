@@ -124,7 +124,7 @@ def run_reference(args, w):
     from oracle import oracle as O
     O.build()
     xy, box = I.workload_inputs(w)
-    o = O.Oracle(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=w.fp32)
+    o = O.Oracle(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=w.fp32, w_target=w.w_target, disc=w.disc)
     o.load_positions(xy)
     sample_sweeps = max(1, args.ref_sweeps)
     for _ in range(args.warmup):
@@ -150,7 +150,9 @@ def run_reference(args, w):
 
 def workload_config(w, sweeps):
     return {"workload": f"{w.name}: N={w.N} hard disks ({w.n_side}x{w.n_side} jittered triangular lattice), "
-                        f"phi={w.phi}, d={w.d} sigma, n_s={w.n_s}, {'fp32' if w.fp32 else 'fp64'} positions",
+                        f"phi={w.phi}, d={w.d} sigma, n_s={w.n_s}, {'fp32' if w.fp32 else 'fp64'} positions"
+                        + (f", cell width >= {w.w_target} sigma" if w.w_target else "")
+                        + (", disc-shaped displacement" if w.disc else ""),
             "sweeps_per_step": sweeps, "seed": w.seed}
 
 
@@ -194,7 +196,7 @@ def main():
     xy_dev = xy_pinned.to(dev)
     out_dev = torch.empty_like(xy_dev)
     out_pinned = torch.empty_like(xy_pinned).pin_memory()
-    sim = Mpmc(w.N, box, w.sigma, w.d, w.n_s, w.seed + rank, fp32=w.fp32, device=dev)   # replicas: seed per rank
+    sim = Mpmc(w.N, box, w.sigma, w.d, w.n_s, w.seed + rank, fp32=w.fp32, device=dev, w_target=w.w_target, disc=w.disc)   # replicas: seed per rank
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
 
     def step_resident():
@@ -296,7 +298,7 @@ def main():
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import oracle as O
         O.build()
-        o = O.Oracle(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=w.fp32)
+        o = O.Oracle(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=w.fp32, w_target=w.w_target, disc=w.disc)
         o.load_positions(xy_np)
         o.sweep(1)
         a0 = o.acceptance()[0]

@@ -46,6 +46,8 @@ typedef struct mpmc_ctx mpmc_ctx; /* opaque host object; owns no device memory *
 /* flags for mpmc_create: exactly one precision bit */
 #define MPMC_FP64 0x1u  /* local coordinates and all move arithmetic in double */
 #define MPMC_FP32 0x2u  /* ... in float (the paper's benchmarks, L390); pressure histogram still in double */
+#define MPMC_DISC 0x4u   /* trial moves uniform in the DISC of radius d (the paper's rng.inCircle(d), L190) instead of the
+                           square [-d, d]^2 of reading A2; runs on the general kernel */
 #define MPMC_DEBUG 0x100u /* record per-cell accept masks and the accept-sequence digest (tests only; slower) */
 
 /* Bytes of device workspace mpmc_create needs for this system (0 on invalid arguments).  Pure host arithmetic.
@@ -56,7 +58,8 @@ size_t mpmc_workspace_bytes_ex(uint64_t N, const double box[2], double sigma, do
 
 /* Create a simulation of N hard disks of diameter sigma in the periodic box [0,Lx) x [0,Ly)  (L25, L362).
  *   box      host, {Lx, Ly}
- *   d        maximum displacement per coordinate: trial moves are uniform in [-d, d]^2 (reading A2)
+ *   d        maximum displacement: trial moves are uniform in [-d, d]^2 (reading A2), or in the disc of radius d
+ *            with MPMC_DISC
  *   n_s      trial moves per non-empty active cell per sub-sweep (the paper's n_M, L95, L358); 0..32
  *   seed     user seed, fixed for the run (L170); keys the Philox4x32-10 streams (reading A9)
  *   workspace  device, 256-byte aligned, >= mpmc_workspace_bytes(...); owned by the caller

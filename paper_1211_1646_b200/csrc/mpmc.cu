@@ -116,16 +116,20 @@ dim3 cell_grid(const mpmc_ctx* c, int threads) { return dim3((c->p.Mq + threads 
 // ---- the persistent sweep kernel ------------------------------------------------------------------------
 // fast = the w ~ sigma cell update (occupancy 0/1/2, compile-time n_s in {4, 8}); otherwise the general one
 template <typename P, bool DEBUG>
-const void* pick_kernel_t(bool fast, uint32_t n_s) {
+const void* pick_kernel_t(bool fast, bool disc, uint32_t n_s) {
+  if (disc) {           // the paper's disc-shaped proposal: general cell update only
+    if (n_s == 4) return (const void*)k_sweeps<P, 4, DEBUG, false, true>;
+    return (const void*)k_sweeps<P, 0, DEBUG, false, true>;
+  }
   if (fast && n_s == 4) return (const void*)k_sweeps<P, 4, DEBUG, true>;
   if (fast && n_s == 8) return (const void*)k_sweeps<P, 8, DEBUG, true>;
   if (n_s == 4) return (const void*)k_sweeps<P, 4, DEBUG, false>;
   if (n_s == 8) return (const void*)k_sweeps<P, 8, DEBUG, false>;
   return (const void*)k_sweeps<P, 0, DEBUG, false>;
 }
-const void* pick_kernel(bool fp32, bool debug, bool fast, uint32_t n_s) {
-  if (fp32) return debug ? pick_kernel_t<float, true>(fast, n_s) : pick_kernel_t<float, false>(fast, n_s);
-  return debug ? pick_kernel_t<double, true>(fast, n_s) : pick_kernel_t<double, false>(fast, n_s);
+const void* pick_kernel(bool fp32, bool debug, bool fast, bool disc, uint32_t n_s) {
+  if (fp32) return debug ? pick_kernel_t<float, true>(fast, disc, n_s) : pick_kernel_t<float, false>(fast, disc, n_s);
+  return debug ? pick_kernel_t<double, true>(fast, disc, n_s) : pick_kernel_t<double, false>(fast, disc, n_s);
 }
 
 // one cooperative launch: sweeps up to sweep index t_end, or one piece of a sweep (test hooks)
@@ -232,7 +236,8 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
                    void* cuda_stream) {
   if (!out || !box || N == 0 || N >= 0xFFFFFFFFull || !(sigma > 0) || !(d > 0) || n_s > 32 || !precision_ok(flags))
     return MPMC_ERR_ARG;
-  const bool fp32 = (flags & MPMC_FP32) != 0, debug = (flags & MPMC_DEBUG) != 0;
+  const bool fp32 = (flags & MPMC_FP32) != 0, debug = (flags & MPMC_DEBUG) != 0, disc = (flags & MPMC_DISC) != 0;
+  if (disc && n_s > 0xFFFFu) return MPMC_ERR_ARG;
   Geom g;
   const int st = geometry(box, sigma, w_target, fp32, &g);
   if (st != MPMC_OK) return st;
@@ -276,7 +281,7 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   // path); general kernel in the paper's regime (w up to sqrt(2) sigma, L152).
   const double wmax = g.wp[0] > g.wp[1] ? g.wp[0] : g.wp[1];
   c->nf = (wmax < 1.15 * sigma) ? 2 : 4;
-  c->kernel = pick_kernel(fp32, debug, c->nf == 2 && (n_s == 4 || n_s == 8), n_s);
+  c->kernel = pick_kernel(fp32, debug, c->nf == 2 && (n_s == 4 || n_s == 8), disc, n_s);
   // grid of the persistent kernel: every block co-resident (cooperative launch), no more blocks than chunks
   int dev = 0, sms = 0, occ = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
@@ -288,7 +293,7 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   if (c->grid > chunks) c->grid = chunks;
   // the tile kernel (tile.cuh) where cells hold 0/1/2 disks and n_s is a compile-time instantiation
   c->tile_kernel = nullptr; c->tile_grid = 0; c->tile_smem = 0; c->t_host = 0;
-  if (c->nf == 2 && (n_s == 4 || n_s == 8)) {
+  if (c->nf == 2 && (n_s == 4 || n_s == 8) && !disc) {
     int smem_optin = 0;
     cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     const size_t cell_bytes = fp32 ? sizeof(SmemCell<float>) : sizeof(SmemCell<double>);

@@ -271,7 +271,7 @@ __device__ __forceinline__ void update_cell_fast(const Params& p, const uint32_t
 // permutation.  NS > 0 fixes n_s at compile time (Philox blocks issued up front, move loop unrolled); NS = 0 is
 // the run-time loop.
 // ---------------------------------------------------------------------------------------------------------
-template <typename P, int NS, bool DEBUG>
+template <typename P, int NS, bool DEBUG, bool DISC>
 __device__ __forceinline__ void update_cell_general(const Params& p, const uint32_t Q, const unsigned long long t,
                                                     const uint32_t cur, const uint32_t ci_raw, const bool valid,
                                                     Tally& tally) {
@@ -305,11 +305,27 @@ __device__ __forceinline__ void update_cell_general(const Params& p, const uint3
     ddx[at] = R::scaled_sym(p, Rw[0]); ddy[at] = R::scaled_sym(p, Rw[1]);
     ddx[at + 1] = R::scaled_sym(p, Rw[2]); ddy[at + 1] = R::scaled_sym(p, Rw[3]);
   };
+  // DISC: the paper's proposal, uniform in the disc of radius d (rng.inCircle(d), L190), by rejection from the square:
+  // block (s | j << 16) serves the candidate pairs 2j (words 0, 1) and 2j + 1 (words 2, 3) of move s; the first pair
+  // with fma(ux, ux, uy*uy) <= 1 is taken (reading A2)
+  auto displacement_disc = [&](uint32_t s, int at) {
+    uint32_t Rw[4] = {0, 0, 0, 0};
+    for (uint32_t j = 0;; ++j) {
+      if ((j & 1u) == 0u) philox4x32_10(w.cell, t_lo, t_hi, s | ((j >> 1) << 16), p.seed_lo, p.seed_hi, Rw);
+      const P ux = R::sym((j & 1u) ? Rw[2] : Rw[0]), uy = R::sym((j & 1u) ? Rw[3] : Rw[1]);
+      if (R::fma(ux, ux, R::mul(uy, uy)) <= (P)1) { ddx[at] = R::mul(R::d(p), ux); ddy[at] = R::mul(R::d(p), uy); break; }
+    }
+  };
   uint32_t S[4];
   philox4x32_10(w.cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
   if (NS > 0) {
+    if (DISC) {
 #pragma unroll
-    for (int q = 0; q < NS / 2; ++q) displacement2((uint32_t)q, 2 * q);
+      for (int s = 0; s < NS; ++s) displacement_disc((uint32_t)s, s);
+    } else {
+#pragma unroll
+      for (int q = 0; q < NS / 2; ++q) displacement2((uint32_t)q, 2 * q);
+    }
   }
 
   uint32_t n_acc = 0, n_rb = 0, n_ro = 0, amask = 0;
@@ -397,7 +413,8 @@ __device__ __forceinline__ void update_cell_general(const Params& p, const uint3
     for (int s = 0; s < NS; ++s) trial_move((uint32_t)s, ddx[s], ddy[s]);
   } else {
     for (uint32_t s = 0; s < p.n_s; s += 2) {
-      displacement2(s >> 1, 0);
+      if (DISC) { displacement_disc(s, 0); if (s + 1 < p.n_s) displacement_disc(s + 1, 1); }
+      else displacement2(s >> 1, 0);
       trial_move(s, ddx[0], ddy[0]);
       if (s + 1 < p.n_s) trial_move(s + 1, ddx[1], ddy[1]);
     }
@@ -600,9 +617,9 @@ constexpr uint32_t OP_SWEEPS = 0, OP_SUB_SWEEP = 1, OP_SHIFT = 2;
 // shared between blocks during the launch.  Block 0 writes the control block back at the end.
 //   op = OP_SWEEPS: sweeps until the sweep index reaches t_end (none if it already has).  OP_SUB_SWEEP (test hook): one sub-sweep of set `arg` at the current sweep index.
 //   OP_SHIFT (test hook): one shift with direction `arg` and distance `delta_in`; the sweep index stays.
-// FAST selects update_cell_fast (w ~ sigma) or update_cell_general.
+// FAST selects update_cell_fast (w ~ sigma) or update_cell_general; DISC (general only) the disc-shaped proposal.
 // ---------------------------------------------------------------------------------------------------------
-template <typename P, int NS, bool DEBUG, bool FAST>
+template <typename P, int NS, bool DEBUG, bool FAST, bool DISC = false>
 __global__ void __launch_bounds__(SUB_THREADS, FAST ? (sizeof(P) == 4 ? FAST_MINB : FAST_MINB / 2) : SUB_MINB)
 k_sweeps(const __grid_constant__ Params p, const unsigned long long t_end, const uint32_t op, const uint32_t arg,
          const double delta_in) {
@@ -626,7 +643,7 @@ k_sweeps(const __grid_constant__ Params p, const unsigned long long t_end, const
     for (uint32_t base = sub_lo; base + warp0 < sub_hi; base += SUB_THREADS) {    // warp-uniform trip count
       const uint32_t ci = base + threadIdx.x;
       if constexpr (FAST) update_cell_fast<P, NS, DEBUG>(p, Q, t, cur, ci, ci < sub_hi, tally);
-      else                update_cell_general<P, NS, DEBUG>(p, Q, t, cur, ci, ci < sub_hi, tally);
+      else                update_cell_general<P, NS, DEBUG, DISC>(p, Q, t, cur, ci, ci < sub_hi, tally);
     }
   };
   auto shift_phase = [&](const uint32_t dir, const P delta, const uint32_t crowded) {

@@ -35,6 +35,8 @@ class Workload:
     seed: int
     fp32: bool
     jitter: float = 0.05
+    w_target: float = 0.0   # requested minimum cell width (0: smallest width >= sigma that divides the box)
+    disc: bool = False      # trial displacement uniform in the disc of radius d instead of the square
 
     @property
     def N(self) -> int:
@@ -49,6 +51,12 @@ CONFIGS = {
     "C4": Workload("C4", 4096, 0.720, 1.0, 0.06, 8, 200, 1, fp32=True),
     "C5": Workload("C5", 1024, 0.30, 1.0, 0.5, 4, 1000, 1, fp32=True),
 }
+
+# The paper's own regime as a second workload: cell width just under sqrt(2) sigma (L152), disc-shaped
+# displacement of radius d = 0.16 sigma and n_M = 4 (L190, L358), phi = 0.698, single precision (L390), sizes next to
+# Table 4's N = 253^2 ... 3040^2 (L411).  Same jittered triangular lattice in the 2/sqrt(3) box (the paper's box is square).
+for _n in (256, 768, 1536, 3072):
+    CONFIGS[f"P{_n}"] = Workload(f"P{_n}", _n, 0.698, 1.0, 0.16, 4, 100, 1, fp32=True, w_target=1.40, disc=True)
 
 
 def lattice_constant(phi: float, sigma: float = 1.0) -> float:

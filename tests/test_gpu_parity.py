@@ -21,10 +21,10 @@ def torch_cuda():
     return torch
 
 
-def make_pair(oracle_mod, torch, N, box, sigma, d, n_s, seed, fp32, xy, debug=True, w_target=0.0):
+def make_pair(oracle_mod, torch, N, box, sigma, d, n_s, seed, fp32, xy, debug=True, w_target=0.0, disc=False):
     from paper_1211_1646_b200.binding import Mpmc
-    o = oracle_mod.Oracle(N, box, sigma, d, n_s, seed, fp32=fp32, w_target=w_target)
-    g = Mpmc(N, box, sigma, d, n_s, seed, fp32=fp32, debug=debug, w_target=w_target)
+    o = oracle_mod.Oracle(N, box, sigma, d, n_s, seed, fp32=fp32, w_target=w_target, disc=disc)
+    g = Mpmc(N, box, sigma, d, n_s, seed, fp32=fp32, debug=debug, w_target=w_target, disc=disc)
     assert (g.mx, g.my) == (o.mx, o.my) and (g.wx, g.wy) == (o.wx, o.wy) and g.L_eff == o.L_eff
     o.load_positions(xy)
     g.load_positions(torch.as_tensor(xy, device="cuda"))
@@ -218,6 +218,27 @@ def test_paper_cell_regime_w_1p4(oracle_mod, torch_cuda, fp32):
     o.sweep(25); g.sweep(25)
     st = assert_same_state(o, g, fp32)
     assert st["counts"].max() >= 3
+
+
+@pytest.mark.parametrize("fp32", [False, True])
+@pytest.mark.parametrize("n_s", [4, 3])
+def test_paper_regime_with_disc_proposal(oracle_mod, torch_cuda, fp32, n_s):
+    # SURVEY.md §8(f).1 in full: w just under sqrt(2) sigma, disc-shaped displacement of radius 0.16 sigma (L190, L358)
+    w = I.CONFIGS["P256"]
+    xy, box = I.workload_inputs(w)
+    o, g = make_pair(oracle_mod, torch_cuda, w.N, box, w.sigma, w.d, n_s, 7, fp32, xy, w_target=w.w_target, disc=True)
+    assert g.wx >= 1.40 and g.wx < math.sqrt(2)
+    o.sweep(20); g.sweep(20)
+    st = assert_same_state(o, g, fp32)
+    assert st["counts"].max() >= 3 and g.path_sweeps() == (0, 20)
+
+
+def test_disc_proposal_at_unit_cell_width_runs_on_the_general_kernel(oracle_mod, torch_cuda):
+    xy, box = I.jittered_lattice(64, 0.6, seed=3)
+    o, g = make_pair(oracle_mod, torch_cuda, 4096, box, 1.0, 0.2, 4, 9, True, xy, disc=True)
+    o.sweep(15); g.sweep(15)
+    assert_same_state(o, g, True)
+    assert g.path_sweeps() == (0, 15)
 
 
 @pytest.mark.parametrize("N,box,xy", [
