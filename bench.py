@@ -259,7 +259,8 @@ def main():
     sweep_ms = e0.elapsed_time(e1) / S
     moves_per_sweep = (sim.acceptance()[0] - a0) / S
     tile_sweeps, general_sweeps = sim.path_sweeps()
-    kernel = "k_tile_sweep" if tile_sweeps >= general_sweeps else "k_sweeps"
+    tile_name = "k_tile4_sweep" if (w.disc or w.w_target >= 1.15) else "k_tile_sweep"     # 4-slot / 2-slot tile kernel
+    kernel = tile_name if tile_sweeps >= general_sweeps else "k_sweeps"
     peak, peak_src = peaks()
     alg = algorithmic_bytes_per_sweep(w.N, sim.M, w.fp32)
     achieved = alg / (sweep_ms * 1e-3) / 1e9

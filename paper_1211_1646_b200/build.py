@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmpmc_b200.so")
 SOURCES = ["mpmc.cu"]
-DEPS = ["mpmc.cu", "common.cuh", "sweep.cuh", "tile.cuh", "aux.cuh", os.path.join("..", "..", "include", "mpmc.h")]
+DEPS = ["mpmc.cu", "common.cuh", "sweep.cuh", "tile.cuh", "tile4.cuh", "aux.cuh", os.path.join("..", "..", "include", "mpmc.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -13,6 +13,7 @@
 #include "common.cuh"
 #include "sweep.cuh"
 #include "tile.cuh"
+#include "tile4.cuh"
 
 using namespace mpmc;
 
@@ -146,6 +147,16 @@ const void* pick_tile_kernel(bool fp32, bool debug, uint32_t n_s) {
   if (n_s == 8) return fp32 ? (debug ? (const void*)k_tile_sweep<float, 8, true> : (const void*)k_tile_sweep<float, 8, false>)
                             : (debug ? (const void*)k_tile_sweep<double, 8, true> : (const void*)k_tile_sweep<double, 8, false>);
   return nullptr;
+}
+
+template <typename P, bool DEBUG>
+const void* pick_tile4_kernel_t(bool disc) {
+  return disc ? (const void*)k_tile4_sweep<P, 4, DEBUG, true> : (const void*)k_tile4_sweep<P, 4, DEBUG, false>;
+}
+const void* pick_tile4_kernel(bool fp32, bool debug, bool disc, uint32_t n_s) {
+  if (n_s != 4) return nullptr;
+  if (fp32) return debug ? pick_tile4_kernel_t<float, true>(disc) : pick_tile4_kernel_t<float, false>(disc);
+  return debug ? pick_tile4_kernel_t<double, true>(disc) : pick_tile4_kernel_t<double, false>(disc);
 }
 
 // Tiling of the tile kernel: ntx x nty tiles of (nearly) equal even size whose loaded region (tile + 2 HALO) fits
@@ -291,16 +302,20 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   const uint32_t chunks = (L.Mq + SUB_THREADS - 1) / SUB_THREADS;
   c->grid = (uint32_t)sms * (uint32_t)occ;
   if (c->grid > chunks) c->grid = chunks;
-  // the tile kernel (tile.cuh) where cells hold 0/1/2 disks and n_s is a compile-time instantiation
+  // The fused tile kernels: tile.cuh (2 slots per cell in shared memory) where cells hold 0/1/2 disks (w < 1.15 sigma),
+  // the square proposal and n_s in {4, 8}; otherwise tile4.cuh (all 4 slots; any width, both proposals) for n_s = 4.
   c->tile_kernel = nullptr; c->tile_grid = 0; c->tile_smem = 0; c->t_host = 0;
-  if (c->nf == 2 && (n_s == 4 || n_s == 8) && !disc) {
+  const bool two_slot = c->nf == 2 && (n_s == 4 || n_s == 8) && !disc;
+  const void* tk = two_slot ? pick_tile_kernel(fp32, debug, n_s) : pick_tile4_kernel(fp32, debug, disc, n_s);
+  if (tk) {
     int smem_optin = 0;
     cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    const size_t cell_bytes = fp32 ? sizeof(SmemCell<float>) : sizeof(SmemCell<double>);
-    const size_t stat = (fp32 ? sizeof(CrowdList<float>) : sizeof(CrowdList<double>)) + 256;   // static shared memory
+    const size_t cell_bytes = (fp32 ? sizeof(SmemCell<float>) : sizeof(SmemCell<double>)) * (two_slot ? 1 : 2);
+    const size_t stat = (two_slot ? (fp32 ? sizeof(CrowdList<float>) : sizeof(CrowdList<double>)) : 0) + 256;   // static shared memory
     const size_t smem_max = (size_t)smem_optin > stat ? (size_t)smem_optin - stat : 0;
     uint32_t ntx = 0, nty = 0, PS = 0;
-    c->tile_threads = fp32 ? TileThreads<float>::value : TileThreads<double>::value;
+    c->tile_threads = two_slot ? (fp32 ? TileThreads<float>::value : TileThreads<double>::value)
+                               : (fp32 ? Tile4Threads<float>::value : Tile4Threads<double>::value);
     bool have = choose_tiling(p.hx, p.hy, cell_bytes, smem_max, (uint32_t)sms, &ntx, &nty, &PS);
     if (const char* e = std::getenv("MPMC_TILE")) {        // experiments: "ntx,nty,threads"
       unsigned a = 0, b = 0, th = 0;
@@ -310,13 +325,13 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
       }
     }
     if (have) {
-      c->tile_kernel = pick_tile_kernel(fp32, debug, n_s);
+      c->tile_kernel = tk;
       c->tile_grid = ntx * nty;
       c->tile_smem = (size_t)4 * PS * cell_bytes;
       p.tl_ntx = ntx; p.tl_nty = nty; p.tl_PS = PS;
       if (std::getenv("MPMC_VERBOSE"))
-        std::fprintf(stderr, "[mpmc] tile kernel: %u x %u tiles, plane stride %u cells, %zu B shared memory, grid %u x %u threads; general grid %u\n",
-                     ntx, nty, PS, c->tile_smem, c->tile_grid, c->tile_threads, c->grid);
+        std::fprintf(stderr, "[mpmc] tile kernel (%d slots): %u x %u tiles, plane stride %u cells, %zu B shared memory, grid %u x %u threads; general grid %u\n",
+                     two_slot ? 2 : 4, ntx, nty, PS, c->tile_smem, c->tile_grid, c->tile_threads, c->grid);
       if (cudaFuncSetAttribute(c->tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tile_smem) != cudaSuccess) {
         cudaGetLastError(); delete c; return MPMC_ERR_CUDA;
       }

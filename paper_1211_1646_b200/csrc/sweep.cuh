@@ -263,45 +263,24 @@ __device__ __forceinline__ void update_cell_fast(const Params& p, const uint32_t
   tally.acc += n_acc; tally.rb += n_rb; tally.ro += n_ro;
 }
 
-// ---------------------------------------------------------------------------------------------------------
-// General cell update: any occupancy up to n_max = 4 per cell — the paper's own regime, w up to
-// sqrt(2) sigma (L152) — and any n_s.  Same mapping and arithmetic; all four slots of the 3x3 cells are kept
-// in registers (own cell as two negated pairs, each neighbour as two translated, negated pairs; slot pair 1 is
-// loaded only where n > 2), and the disk a move acts on is chosen with select chains from the visiting
-// permutation.  NS > 0 fixes n_s at compile time (Philox blocks issued up front, move loop unrolled); NS = 0 is
-// the run-time loop.
-// ---------------------------------------------------------------------------------------------------------
-template <typename P, int NS, bool DEBUG, bool DISC>
-__device__ __forceinline__ void update_cell_general(const Params& p, const uint32_t Q, const unsigned long long t,
-                                                    const uint32_t cur, const uint32_t ci_raw, const bool valid,
-                                                    Tally& tally) {
+// The moves of one cell with up to n_max = 4 disks (Algorithm 2 lines 9-32) on registers: h0 / h1 = slot pairs 0 / 1 of
+// the 3x3 cells (idx 4 = own cell; empty slots = sentinel), n = the own count, cell = canonical cell id (Philox counter).
+// Returns the own cell's slot pairs after the moves, the accept mask and the three tallies.  Shared by the general
+// kernel (operands from global memory) and the 4-slot tile kernel (operands from shared memory).
+template <typename P, int NS, bool DISC>
+__device__ __forceinline__ void cell_moves_general(const Params& p, const Half<P> (&h0)[9], const Half<P> (&h1)[9],
+                                                   const uint32_t n, const uint32_t cell, const uint32_t t_lo,
+                                                   const uint32_t t_hi, Half<P>& o0, Half<P>& o1, uint32_t& amask,
+                                                   uint32_t& n_acc, uint32_t& n_rb, uint32_t& n_ro) {
   using R = Real<P>;
   using Pair = typename R::Pair;
   static_assert(NS % 2 == 0, "compile-time n_s must be even");
-  const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
-  const Where w = locate_active(p, Q, ci_raw, valid);
-  const uint8_t* cntb = p.cnt[cur];
-  P* posb = reinterpret_cast<P*>(p.pos[cur]);
-  const uint32_t Mqp = p.Mqp;
-
-  // ---- level-1 loads, all independent: count and slot pair 0 of the 3x3 cells (idx 4 = own cell) ----
-  uint32_t cj[9], pidx[9];
-  Half<P> h0[9];
-#pragma unroll
-  for (int idx = 0; idx < 9; ++idx) {
-    uint32_t qn, cn;
-    neighbour(w, idx % 3 - 1, idx / 3 - 1, qn, cn);
-    pidx[idx] = 2u * qn * Mqp + cn;
-    cj[idx] = ld_u8_early(cntb + (qn * Mqp + cn));
-    h0[idx] = ld_half_early(posb, pidx[idx]);
-  }
-
   // ---- Philox words of the shuffle and of the displacements, while the loads are in flight ----
   constexpr int NSA = NS > 0 ? NS : 2;
   P ddx[NSA], ddy[NSA];
   auto displacement2 = [&](uint32_t q, int at) {       // block q serves moves 2q and 2q + 1 (reading A9)
     uint32_t Rw[4];
-    philox4x32_10(w.cell, t_lo, t_hi, q, p.seed_lo, p.seed_hi, Rw);
+    philox4x32_10(cell, t_lo, t_hi, q, p.seed_lo, p.seed_hi, Rw);
     ddx[at] = R::scaled_sym(p, Rw[0]); ddy[at] = R::scaled_sym(p, Rw[1]);
     ddx[at + 1] = R::scaled_sym(p, Rw[2]); ddy[at + 1] = R::scaled_sym(p, Rw[3]);
   };
@@ -309,15 +288,27 @@ __device__ __forceinline__ void update_cell_general(const Params& p, const uint3
   // block (s | j << 16) serves the candidate pairs 2j (words 0, 1) and 2j + 1 (words 2, 3) of move s; the first pair
   // with fma(ux, ux, uy*uy) <= 1 is taken (reading A2)
   auto displacement_disc = [&](uint32_t s, int at) {
-    uint32_t Rw[4] = {0, 0, 0, 0};
-    for (uint32_t j = 0;; ++j) {
-      if ((j & 1u) == 0u) philox4x32_10(w.cell, t_lo, t_hi, s | ((j >> 1) << 16), p.seed_lo, p.seed_hi, Rw);
-      const P ux = R::sym((j & 1u) ? Rw[2] : Rw[0]), uy = R::sym((j & 1u) ? Rw[3] : Rw[1]);
-      if (R::fma(ux, ux, R::mul(uy, uy)) <= (P)1) { ddx[at] = R::mul(R::d(p), ux); ddy[at] = R::mul(R::d(p), uy); break; }
+    // both pairs of the first block are evaluated without a branch (one of them is inside the disc 95 % of the time);
+    // the rare lanes that need more go through further blocks in a structured loop
+    uint32_t Rw[4];
+    philox4x32_10(cell, t_lo, t_hi, s, p.seed_lo, p.seed_hi, Rw);
+    const P ax = R::sym(Rw[0]), ay = R::sym(Rw[1]), bx = R::sym(Rw[2]), by = R::sym(Rw[3]);
+    const bool oka = R::fma(ax, ax, R::mul(ay, ay)) <= (P)1, okb = R::fma(bx, bx, R::mul(by, by)) <= (P)1;
+    P ux = oka ? ax : bx, uy = oka ? ay : by;
+    bool found = oka || okb;
+    uint32_t blk = 1;
+    while (!found) {
+      philox4x32_10(cell, t_lo, t_hi, s | (blk << 16), p.seed_lo, p.seed_hi, Rw);
+      const P cx = R::sym(Rw[0]), cy = R::sym(Rw[1]), ex = R::sym(Rw[2]), ey = R::sym(Rw[3]);
+      const bool okc = R::fma(cx, cx, R::mul(cy, cy)) <= (P)1, oke = R::fma(ex, ex, R::mul(ey, ey)) <= (P)1;
+      ux = okc ? cx : ex; uy = okc ? cy : ey;
+      found = okc || oke;
+      ++blk;
     }
+    ddx[at] = R::mul(R::d(p), ux); ddy[at] = R::mul(R::d(p), uy);
   };
   uint32_t S[4];
-  philox4x32_10(w.cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
+  philox4x32_10(cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
   if (NS > 0) {
     if (DISC) {
 #pragma unroll
@@ -328,20 +319,11 @@ __device__ __forceinline__ void update_cell_general(const Params& p, const uint3
     }
   }
 
-  uint32_t n_acc = 0, n_rb = 0, n_ro = 0, amask = 0;
-  const uint32_t n = w.valid ? cj[4] : 0u;
+  n_acc = 0; n_rb = 0; n_ro = 0; amask = 0;
   const uint32_t nv = n > 0u ? n : 1u;                 // visiting modulus; an empty cell "visits" a sentinel
   const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p);
   const P FAR = R::far_away();
   const Pair MINUS1 = R::pair((P)-1, (P)-1);
-
-  // ---- level-2 loads: slot pair 1 where n > 2 ----
-  Half<P> h1[9];
-#pragma unroll
-  for (int idx = 0; idx < 9; ++idx) {
-    h1[idx].x = R::pair(FAR, FAR); h1[idx].y = h1[idx].x;
-    if (cj[idx] > 2u) h1[idx] = ld_half(posb, pidx[idx] + Mqp);
-  }
 
   // ---- own cell (Alg. 2 line 8, L186), negated, as pairs (slot 0,1) and (slot 2,3) ----
   Pair nox[2], noy[2];
@@ -420,16 +402,58 @@ __device__ __forceinline__ void update_cell_general(const Params& p, const uint3
     }
   }
   if (n == 0u) { n_rb = 0u; n_acc = 0u; n_ro = 0u; amask = 0u; }   // empty cells attempt nothing (A10)
+  o0.x = R::pair(-nox[0].x, -nox[0].y); o0.y = R::pair(-noy[0].x, -noy[0].y);
+  o1.x = R::pair(-nox[1].x, -nox[1].y); o1.y = R::pair(-noy[1].x, -noy[1].y);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// General cell update: any occupancy up to n_max = 4 per cell — the paper's own regime, w up to
+// sqrt(2) sigma (L152) — and any n_s.  Same mapping and arithmetic; all four slots of the 3x3 cells are kept
+// in registers (own cell as two negated pairs, each neighbour as two translated, negated pairs; slot pair 1 is
+// loaded only where n > 2), and the disk a move acts on is chosen with select chains from the visiting
+// permutation.  NS > 0 fixes n_s at compile time (Philox blocks issued up front, move loop unrolled); NS = 0 is
+// the run-time loop.
+// ---------------------------------------------------------------------------------------------------------
+template <typename P, int NS, bool DEBUG, bool DISC>
+__device__ __forceinline__ void update_cell_general(const Params& p, const uint32_t Q, const unsigned long long t,
+                                                    const uint32_t cur, const uint32_t ci_raw, const bool valid,
+                                                    Tally& tally) {
+  using R = Real<P>;
+  const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
+  const Where w = locate_active(p, Q, ci_raw, valid);
+  const uint8_t* cntb = p.cnt[cur];
+  P* posb = reinterpret_cast<P*>(p.pos[cur]);
+  const uint32_t Mqp = p.Mqp;
+
+  // ---- level-1 loads, all independent: count and slot pair 0 of the 3x3 cells (idx 4 = own cell) ----
+  uint32_t cj[9], pidx[9];
+  Half<P> h0[9];
+#pragma unroll
+  for (int idx = 0; idx < 9; ++idx) {
+    uint32_t qn, cn;
+    neighbour(w, idx % 3 - 1, idx / 3 - 1, qn, cn);
+    pidx[idx] = 2u * qn * Mqp + cn;
+    cj[idx] = ld_u8_early(cntb + (qn * Mqp + cn));
+    h0[idx] = ld_half_early(posb, pidx[idx]);
+  }
+
+  // ---- slot pair 1 where n > 2 ----
+  const P FAR = R::far_away();
+  Half<P> h1[9];
+#pragma unroll
+  for (int idx = 0; idx < 9; ++idx) {
+    h1[idx].x = R::pair(FAR, FAR); h1[idx].y = h1[idx].x;
+    if (cj[idx] > 2u) h1[idx] = ld_half(posb, pidx[idx] + Mqp);
+  }
+  const uint32_t n = w.valid ? cj[4] : 0u;
+  uint32_t n_acc, n_rb, n_ro, amask;
+  Half<P> o0, o1;
+  cell_moves_general<P, NS, DISC>(p, h0, h1, n, w.cell, t_lo, t_hi, o0, o1, amask, n_acc, n_rb, n_ro);
 
   // ---- write back (line 34, L234) ----
   if (amask != 0u) {
-    Half<P> o;
-    o.x = R::pair(-nox[0].x, -nox[0].y); o.y = R::pair(-noy[0].x, -noy[0].y);
-    st_half(posb, pidx[4], o);
-    if (n > 2u) {
-      o.x = R::pair(-nox[1].x, -nox[1].y); o.y = R::pair(-noy[1].x, -noy[1].y);
-      st_half(posb, pidx[4] + Mqp, o);
-    }
+    st_half(posb, pidx[4], o0);
+    if (n > 2u) st_half(posb, pidx[4] + Mqp, o1);
   }
   if (DEBUG && w.valid) {
     p.mask[w.cell] = amask;
@@ -495,6 +519,48 @@ __device__ __forceinline__ void shift_pair_rest(const ShiftRest<P>& rest, Half<P
   const Disk<P> r2 = pick(rest.ns == 2u, rest.t0, pick(rest.ns == 1u, rest.t1, none));
   const Disk<P> r3 = pick(rest.ns == 2u, rest.t1, none);
   o23.x = R::pair(r2.x, r3.x); o23.y = R::pair(r2.y, r3.y); i23 = make_uint2(r2.id, r3.id);
+}
+
+// The new cell from ALL FOUR slots of its own old cell (slot pairs ho0, ho1, ids io01, io23) and of the old neighbour in
+// direction f (hn0, hn1, in01, in23); empty slots = sentinel.  Straight-line code on registers: eight candidates, four
+// output slots filled by prefix count (stayers in slot order, then entrants in slot order, reading A13).  Returns the
+// new count (may exceed n_max: the caller reports the overflow); o0/o1 and j01/j23 = the new slot pairs and ids.
+template <typename P>
+__device__ __forceinline__ uint32_t shift_eight(const Half<P>& ho0, const Half<P>& ho1, const Half<P>& hn0, const Half<P>& hn1,
+                                                const uint2 io01, const uint2 io23, const uint2 in01, const uint2 in23,
+                                                const bool along_x, const P step, const P back, const P w,
+                                                Half<P>& o0, Half<P>& o1, uint2& j01, uint2& j23) {
+  using R = Real<P>;
+  const P FAR = R::far_away(), HALF_FAR = FAR * (P)0.5;
+  P cx[8] = {ho0.x.x, ho0.x.y, ho1.x.x, ho1.x.y, hn0.x.x, hn0.x.y, hn1.x.x, hn1.x.y};
+  P cy[8] = {ho0.y.x, ho0.y.y, ho1.y.x, ho1.y.y, hn0.y.x, hn0.y.y, hn1.y.x, hn1.y.y};
+  const uint32_t cid[8] = {io01.x, io01.y, io23.x, io23.y, in01.x, in01.y, in23.x, in23.y};
+  bool take[8];
+  uint32_t pos[8], nn = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const bool occupied = cx[i] < HALF_FAR;
+    P m = R::add(along_x ? cx[i] : cy[i], step);                 // l' = l - f*delta  (L303)
+    const bool in = m > (P)0 && m <= w;
+    take[i] = occupied && (i < 4 ? in : !in);                    // own disks that stay; the neighbour's that left it (L326-328)
+    if (i >= 4) m = R::add(m, back);                             // L332, after the test (L352)
+    if (along_x) cx[i] = m; else cy[i] = m;
+    pos[i] = nn;
+    nn += take[i] ? 1u : 0u;
+  }
+  P ox[NMAX], oy[NMAX]; uint32_t oid[NMAX];
+#pragma unroll
+  for (int j = 0; j < NMAX; ++j) {
+    ox[j] = FAR; oy[j] = FAR; oid[j] = 0xFFFFFFFFu;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const bool here = take[i] && pos[i] == (uint32_t)j;
+      ox[j] = here ? cx[i] : ox[j]; oy[j] = here ? cy[i] : oy[j]; oid[j] = here ? cid[i] : oid[j];
+    }
+  }
+  o0.x = R::pair(ox[0], ox[1]); o0.y = R::pair(oy[0], oy[1]); j01 = make_uint2(oid[0], oid[1]);
+  o1.x = R::pair(ox[2], ox[3]); o1.y = R::pair(oy[2], oy[3]); j23 = make_uint2(oid[2], oid[3]);
+  return nn;
 }
 
 // one new cell; ALONG_X and POSITIVE are uniform across the grid, so the caller branches once

@@ -313,41 +313,14 @@ __device__ __noinline__ void tile_shift_cell_general(const Params& p, const Smem
   go.x = R::pair(FAR, FAR); go.y = go.x; gn = go;
   if (eo >= 0) go = cl.e[eo].hi;
   if (en >= 0) gn = cl.e[en].hi;
-  P cx[8] = {ho.x.x, ho.x.y, go.x.x, go.x.y, hn.x.x, hn.x.y, gn.x.x, gn.x.y};
-  P cy[8] = {ho.y.x, ho.y.y, go.y.x, go.y.y, hn.y.x, hn.y.y, gn.y.x, gn.y.y};
-  const uint32_t cid[8] = {io01.x, io01.y, io23.x, io23.y, in01.x, in01.y, in23.x, in23.y};
-  bool take[8];
-  uint32_t pos[8], nn = 0;
-#pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    const bool occupied = cx[i] < HALF_FAR;
-    P m = R::add(along_x ? cx[i] : cy[i], step);                 // l' = l - f*delta  (L303)
-    const bool in = m > (P)0 && m <= w;
-    take[i] = occupied && (i < 4 ? in : !in);                    // own disks that stay; the neighbour's that left it (L326-328)
-    if (i >= 4) m = R::add(m, back);                             // L332, after the test (L352)
-    if (along_x) cx[i] = m; else cy[i] = m;
-    pos[i] = nn;
-    nn += take[i] ? 1u : 0u;
-  }
-  P ox[NMAX], oy[NMAX]; uint32_t oid[NMAX];
-#pragma unroll
-  for (int j = 0; j < NMAX; ++j) {
-    ox[j] = FAR; oy[j] = FAR; oid[j] = 0xFFFFFFFFu;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      const bool here = take[i] && pos[i] == (uint32_t)j;
-      ox[j] = here ? cx[i] : ox[j]; oy[j] = here ? cy[i] : oy[j]; oid[j] = here ? cid[i] : oid[j];
-    }
-  }
+  Half<P> o0, o1; uint2 j01, j23;
+  uint32_t nn = shift_eight<P>(ho, go, hn, gn, io01, io23, in01, in23, along_x, step, back, w, o0, o1, j01, j23);
   if (nn > (uint32_t)NMAX) { atomicOr(&p.ctl->err, ERRBIT_OVERFLOW); nn = NMAX; }
   P* posn = reinterpret_cast<P*>(p.pos[nxt]);
   uint2* idsn = reinterpret_cast<uint2*>(p.ids[nxt]);
-  Half<P> o;
-  o.x = R::pair(ox[0], ox[1]); o.y = R::pair(oy[0], oy[1]);
-  st_half(posn, own_g, o); idsn[own_g] = make_uint2(oid[0], oid[1]);
+  st_half(posn, own_g, o0); idsn[own_g] = j01;
   if (nn > 2u) {
-    o.x = R::pair(ox[2], ox[3]); o.y = R::pair(oy[2], oy[3]);
-    st_half(posn, own_g + Mqp, o); idsn[own_g + Mqp] = make_uint2(oid[2], oid[3]);
+    st_half(posn, own_g + Mqp, o1); idsn[own_g + Mqp] = j23;
     note_crowded(p.ctl, crowd_slot, cell);
   }
   p.cnt[nxt][cnt_g] = (uint8_t)nn;

@@ -1,0 +1,225 @@
+// tile4.cuh — the fused sweep kernel for the paper's own regime: cell widths up to sqrt(2) sigma, where a cell holds up
+// to n_max = 4 disks and 3-4 disks per cell are the norm.  Same plan as tile.cuh — one launch = one
+// whole sweep of Algorithm 1 (L60-93) on a tile + halo of 5 cells held in shared memory, halo recompute, warps drawing
+// chunks of 32 cells, shift straight into the other global buffer, last CTA advances the control block — but shared
+// memory holds BOTH slot pairs of every cell (32 B in fp32; empty slots = sentinel, so counts are implied), the cell
+// update is the register-resident general one (cell_moves_general, sweep.cuh: 16 neighbour pairs + 2 own pairs per
+// move) and the shift compacts eight candidates (shift_eight).  No list of crowded cells is needed.  Serves the square
+// and the disc-shaped proposal (MPMC_DISC, L190).
+#pragma once
+#include "common.cuh"
+#include "sweep.cuh"
+#include "tile.cuh"
+
+namespace mpmc {
+
+// threads per CTA, one CTA per SM: 12 warps at <= 170 registers (fp32), 8 warps at <= 255 registers (fp64)
+template <typename P> struct Tile4Threads { static constexpr int value = sizeof(P) == 4 ? 384 : 256; };
+
+// The cells of sub-sweep k: local colour QL at ring >= k, in chunks of 32 drawn from a shared counter.
+template <typename P, int NS, bool DEBUG, bool DISC, uint32_t QL>
+__device__ __forceinline__ void tile4_sub_sweep_cells(const Params& p, SmemCell<P>* sm0, SmemCell<P>* sm1, const TileBox& tb,
+                                                      const uint32_t k, const int gx0, const int gy0,
+                                                      const unsigned long long t, uint32_t* next, Tally& tally) {
+  using R = Real<P>;
+  constexpr uint32_t qx = QL & 1u, qy = QL >> 1;
+  const uint32_t PS = p.tl_PS, pw = tb.pw;
+  const uint32_t px0 = (k - qx + 1u) >> 1, px1 = (tb.w - 1u - k - qx) >> 1;
+  const uint32_t py0 = (k - qy + 1u) >> 1, py1 = (tb.h - 1u - k - qy) >> 1;
+  const uint32_t nxp = px1 - px0 + 1u, count = nxp * (py1 - py0 + 1u);
+  const uint32_t inv = small_div_magic(nxp);
+  const uint32_t lane = threadIdx.x & 31u;
+  const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
+  const P HALF_FAR = R::far_away() * (P)0.5;
+  for (;;) {
+    uint32_t base = 0;
+    if (lane == 0u) base = atomicAdd(next, 32u);
+    base = __shfl_sync(0xFFFFFFFFu, base, 0);
+    if (base >= count) break;
+    const uint32_t idx = base + lane;
+    if (idx >= count) continue;
+    const uint32_t ry = small_div(idx, inv), rx = idx - ry * nxp;
+    const uint32_t px = px0 + rx, py = py0 + ry, lx = 2u * px + qx, ly = 2u * py + qy;
+    const uint32_t si = QL * PS + py * pw + px;
+    const uint32_t cell = wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx);
+    const bool interior = lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY;
+    Half<P> h0[9], h1[9];
+#pragma unroll
+    for (int j = 0; j < 9; ++j) {
+      const int off = neighbour_offset(QL, j % 3 - 1, j / 3 - 1, PS, pw);
+      h0[j] = lds_half(sm0 + si + off, 0u);
+      h1[j] = lds_half(sm1 + si + off, 0u);
+    }
+    // slots fill in order, so the count is the number of occupied slots
+    const uint32_t n = h0[4].x.x < HALF_FAR ? (h0[4].x.y < HALF_FAR ? (h1[4].x.x < HALF_FAR ? (h1[4].x.y < HALF_FAR ? 4u : 3u) : 2u) : 1u) : 0u;
+    uint32_t amask, n_acc, n_rb, n_ro;
+    Half<P> o0, o1;
+    cell_moves_general<P, NS, DISC>(p, h0, h1, n, cell, t_lo, t_hi, o0, o1, amask, n_acc, n_rb, n_ro);
+    if (amask != 0u) {                              // write back (Alg. 2 line 34, L234)
+      sts_half(sm0, si, o0);
+      if (n > 2u) sts_half(sm1, si, o1);
+    }
+    if (interior) { tally.acc += n_acc; tally.rb += n_rb; tally.ro += n_ro; }
+    if (DEBUG && interior) {
+      p.mask[cell] = amask;
+      if (n > 0u) atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)cell << 32) | amask)));
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// The fused sweep kernel, four slots per cell.  Dynamic shared memory: 2 slot pairs x 4 planes x tl_PS cells.
+// ---------------------------------------------------------------------------------------------------------
+template <typename P, int NS, bool DEBUG, bool DISC>
+__global__ void __launch_bounds__(Tile4Threads<P>::value, 1)
+k_tile4_sweep(const __grid_constant__ Params p) {
+  using R = Real<P>;
+  extern __shared__ __align__(16) unsigned char tile_smem[];
+  const uint32_t PS = p.tl_PS;
+  SmemCell<P>* sm0 = reinterpret_cast<SmemCell<P>*>(tile_smem);     // slot pair 0 of the four local colour planes
+  SmemCell<P>* sm1 = sm0 + 4u * PS;                                 // slot pair 1
+  __shared__ Draws sdraw;
+  __shared__ uint32_t s_last;
+  __shared__ uint32_t s_next[8];                 // chunk counters: sub-sweeps 1-4, shift planes 0-3
+  Ctl* ctl = p.ctl;
+  // launched with programmatic stream serialisation (mpmc.cu): everything below reads what the previous sweep wrote
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const unsigned long long t = ctl->t;
+  const uint32_t cur = ctl->cur, nxt = cur ^ 1u;
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, NW = blockDim.x >> 5;
+  const uint32_t ty = blockIdx.x / p.tl_ntx, tx = blockIdx.x - ty * p.tl_ntx;
+  const TileBox tb = tile_box(p, tx, ty);
+  const uint32_t pw = tb.pw, ph = tb.ph, Mqp = p.Mqp;
+  const int gx0 = (int)tb.x0 - HALO, gy0 = (int)tb.y0 - HALO;       // global cell of the region's corner (unwrapped)
+  const P FAR = R::far_away(), HALF_FAR = FAR * (P)0.5;
+  if (tid == 0) {
+    sdraw = draw_sweep(p, t);                    // Alg. 1 lines 2, 15, 16 (L64, L90-91)
+    for (int i = 0; i < 8; ++i) s_next[i] = 0u;
+  }
+  __syncthreads();
+
+  // ---- load the tile and its halo: warps take plane rows, lanes run along the row; slot pair 1 only where n > 2 ----
+  {
+    const P* posc = reinterpret_cast<const P*>(p.pos[cur]);
+    const uint8_t* cntc = p.cnt[cur];
+    const uint32_t nrows = 4u * ph, inv_ph = small_div_magic(ph);
+    for (uint32_t c0 = 0; c0 < pw; c0 += 32u) {
+      for (uint32_t r0 = warp; r0 < nrows; r0 += 4u * NW) {
+        Half<P> v[4];
+        uint32_t sidx[4], gidx[4], cnt[4];
+        bool ok[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const uint32_t r = r0 + (uint32_t)j * NW, rr = r < nrows ? r : 0u;
+          const uint32_t q = small_div(rr, inv_ph), py = rr - q * ph, px = c0 + lane;
+          ok[j] = r < nrows && px < pw;
+          const uint32_t gy = wrap_cell(gy0 + (int)(2u * py + (q >> 1)), p.my);
+          const uint32_t gx = wrap_cell(gx0 + (int)(2u * (ok[j] ? px : 0u) + (q & 1u)), p.mx);
+          const uint32_t Qg = ((gy & 1u) << 1) | (gx & 1u), cig = (gy >> 1) * p.hx + (gx >> 1);
+          sidx[j] = q * PS + py * pw + px; gidx[j] = 2u * Qg * Mqp + cig;
+          cnt[j] = 0u;
+          if (ok[j]) { cnt[j] = cntc[Qg * Mqp + cig]; v[j] = ld_half(posc, gidx[j]); }
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          if (!ok[j]) continue;
+          Half<P> hi; hi.x = R::pair(FAR, FAR); hi.y = hi.x;
+          if (cnt[j] > 2u) hi = ld_half(posc, gidx[j] + Mqp);
+          sts_half(sm0, sidx[j], v[j]);
+          sts_half(sm1, sidx[j], hi);
+        }
+      }
+    }
+  }
+  __syncthreads();
+  const Draws dr = sdraw;
+  Tally tally;
+
+  // ---- four sub-sweeps (Alg. 1 lines 3-14, L66-88): sub-sweep k updates its colour at ring >= k ----
+#pragma unroll 1
+  for (uint32_t k = 1; k <= 4u; ++k) {
+    const uint32_t Qg = k == 1u ? dr.order[0] : k == 2u ? dr.order[1] : k == 3u ? dr.order[2] : dr.order[3];
+    switch (Qg ^ 3u) {                           // the region starts at an odd cell (x0 - 5, y0 - 5): colours flip
+      case 0: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 0>(p, sm0, sm1, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      case 1: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 1>(p, sm0, sm1, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      case 2: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 2>(p, sm0, sm1, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      default: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 3>(p, sm0, sm1, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
+    }
+    __syncthreads();
+  }
+
+  // ---- cell shift (Alg. 1 lines 15-17; Algorithm 4) of the interior cells, shared memory -> other buffer ----
+  const uint32_t dir = dr.dir;
+  const bool along_x = dir < 2u, positive = (dir & 1u) == 0u;
+  const P w = along_x ? R::wx(p) : R::wy(p);
+  const P delta = R::mul(R::mul((P)0.5, w), R::unit(dr.dist_word));   // line 15 (L90)
+  {
+    const P step = positive ? -delta : delta;     // l' = l - f*delta   (L303)
+    const P back = positive ? w : -w;             // entrant translation (L332)
+    const uint2* idsc = reinterpret_cast<const uint2*>(p.ids[cur]);
+    P* posn = reinterpret_cast<P*>(p.pos[nxt]);
+    uint2* idsn = reinterpret_cast<uint2*>(p.ids[nxt]);
+    uint8_t* cntn = p.cnt[nxt];
+    const uint32_t hTX = tb.TX >> 1, per_plane = hTX * (tb.TY >> 1);
+    const uint32_t inv = small_div_magic(hTX);
+    const int dox = along_x ? (positive ? 1 : -1) : 0, doy = along_x ? 0 : (positive ? 1 : -1);
+    const uint2 none = make_uint2(0xFFFFFFFFu, 0xFFFFFFFFu);
+#pragma unroll 1
+    for (uint32_t q = 0; q < 4u; ++q) {
+      const uint32_t qx = q & 1u, qy = q >> 1;
+      const uint32_t px0 = (HALO - qx + 1u) >> 1, py0 = (HALO - qy + 1u) >> 1;
+      const int nboff = neighbour_offset(q, dox, doy, PS, pw);       // the old neighbour in direction f (L314-317)
+      for (;;) {
+        uint32_t base = 0;
+        if (lane == 0u) base = atomicAdd(&s_next[4u + q], 32u);
+        base = __shfl_sync(0xFFFFFFFFu, base, 0);
+        if (base >= per_plane) break;
+        const uint32_t idx = base + lane;
+        if (idx >= per_plane) continue;
+        const uint32_t ry = small_div(idx, inv), rx = idx - ry * hTX;
+        const uint32_t px = px0 + rx, py = py0 + ry, lx = 2u * px + qx, ly = 2u * py + qy;
+        const uint32_t si = q * PS + py * pw + px, sn = (uint32_t)((int)si + nboff);
+        const uint32_t gx = (uint32_t)(gx0 + (int)lx), gy = (uint32_t)(gy0 + (int)ly);      // interior: no wrap
+        const uint32_t gxn = wrap_cell((int)gx + dox, p.mx), gyn = wrap_cell((int)gy + doy, p.my);
+        const uint32_t Qg = ((gy & 1u) << 1) | (gx & 1u), Qn = ((gyn & 1u) << 1) | (gxn & 1u);
+        const uint32_t cig = (gy >> 1) * p.hx + (gx >> 1), cin = (gyn >> 1) * p.hx + (gxn >> 1);
+        const uint32_t own = 2u * Qg * Mqp + cig, nbg = 2u * Qn * Mqp + cin;
+        const Half<P> ho0 = lds_half(sm0, si), ho1 = lds_half(sm1, si), hn0 = lds_half(sm0, sn), hn1 = lds_half(sm1, sn);
+        const uint2 io01 = idsc[own], in01 = idsc[nbg];
+        uint2 io23 = none, in23 = none;
+        if (ho1.x.x < HALF_FAR) io23 = idsc[own + Mqp];            // slots 2, 3 in use: their ids are valid
+        if (hn1.x.x < HALF_FAR) in23 = idsc[nbg + Mqp];
+        Half<P> o0, o1; uint2 j01, j23;
+        uint32_t nn = shift_eight<P>(ho0, ho1, hn0, hn1, io01, io23, in01, in23, along_x, step, back, w, o0, o1, j01, j23);
+        if (nn > (uint32_t)NMAX) { atomicOr(&ctl->err, ERRBIT_OVERFLOW); nn = NMAX; }
+        st_half(posn, own, o0); idsn[own] = j01;
+        if (nn > 2u) { st_half(posn, own + Mqp, o1); idsn[own + Mqp] = j23; }
+        cntn[Qg * Mqp + cig] = (uint8_t)nn;       // L280, L342
+      }
+    }
+  }
+
+  // ---- counters; the last CTA to finish advances the control block ----
+  flush_tally(p, tally);
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    s_last = (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1u) ? 1u : 0u;
+  }
+  __syncthreads();
+  if (s_last && tid == 0) {
+    const double L = along_x ? p.Lx_eff : p.Ly_eff;
+    double o = ctl->origin[along_x ? 0 : 1];     // the grid origin follows the shift
+    o = __dadd_rn(o, positive ? (double)delta : -(double)delta);
+    if (o >= L) o = __dsub_rn(o, L);
+    if (o < 0.0) o = __dadd_rn(o, L);
+    ctl->origin[along_x ? 0 : 1] = o;
+    ctl->ticket = 0u;
+    ctl->cur = nxt;
+    ctl->t = t + 1ull;
+    ctl->path_sweeps[0] += 1ull;
+  }
+}
+
+}  // namespace mpmc

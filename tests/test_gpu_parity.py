@@ -211,7 +211,7 @@ def test_tile_kernel_uneven_tilings(oracle_mod, torch_cuda, n, phi):
 
 @pytest.mark.parametrize("fp32", [False, True])
 def test_paper_cell_regime_w_1p4(oracle_mod, torch_cuda, fp32):
-    # cell width just under sqrt(2) sigma, n_max = 4 fully used (L152); NF = 4 kernel
+    # cell width just under sqrt(2) sigma, n_max = 4 fully used (L152); 4-slot tile kernel
     xy, box = I.jittered_lattice(128, 0.698, seed=2)
     o, g = make_pair(oracle_mod, torch_cuda, 128 * 128, box, 1.0, 0.16, 4, 3, fp32, xy, w_target=1.40)
     assert g.wx >= 1.40 and g.wx < math.sqrt(2)
@@ -230,15 +230,16 @@ def test_paper_regime_with_disc_proposal(oracle_mod, torch_cuda, fp32, n_s):
     assert g.wx >= 1.40 and g.wx < math.sqrt(2)
     o.sweep(20); g.sweep(20)
     st = assert_same_state(o, g, fp32)
-    assert st["counts"].max() >= 3 and g.path_sweeps() == (0, 20)
+    assert st["counts"].max() >= 3
+    assert g.path_sweeps() == ((20, 0) if n_s == 4 else (0, 20))     # 4-slot tile kernel for n_s = 4, else the general kernel
 
 
-def test_disc_proposal_at_unit_cell_width_runs_on_the_general_kernel(oracle_mod, torch_cuda):
+def test_disc_proposal_at_unit_cell_width(oracle_mod, torch_cuda):
     xy, box = I.jittered_lattice(64, 0.6, seed=3)
     o, g = make_pair(oracle_mod, torch_cuda, 4096, box, 1.0, 0.2, 4, 9, True, xy, disc=True)
     o.sweep(15); g.sweep(15)
     assert_same_state(o, g, True)
-    assert g.path_sweeps() == (0, 15)
+    assert g.path_sweeps() == (15, 0)                  # the 4-slot tile kernel serves the disc proposal at any width
 
 
 @pytest.mark.parametrize("N,box,xy", [
