@@ -234,6 +234,17 @@ def test_paper_regime_with_disc_proposal(oracle_mod, torch_cuda, fp32, n_s):
     assert g.path_sweeps() == ((20, 0) if n_s == 4 else (0, 20))     # 4-slot tile kernel for n_s = 4, else the general kernel
 
 
+@pytest.mark.parametrize("n,phi,disc", [(20, 0.5, False), (34, 0.66, True), (70, 0.698, False), (126, 0.6, True)])
+def test_four_slot_tile_kernel_uneven_tilings(oracle_mod, torch_cuda, n, phi, disc):
+    # w = 1.4 sigma on boxes that do not divide evenly into tiles; both proposals
+    xy, box = I.jittered_lattice(n, phi, seed=n)
+    o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.16, 4, n + 1, True, xy, w_target=1.40, disc=disc)
+    for k in (1, 3, 6):
+        o.sweep(k); g.sweep(k)
+        assert_same_state(o, g, True)
+    assert sum(g.path_sweeps()) == 10
+
+
 def test_disc_proposal_at_unit_cell_width(oracle_mod, torch_cuda):
     xy, box = I.jittered_lattice(64, 0.6, seed=3)
     o, g = make_pair(oracle_mod, torch_cuda, 4096, box, 1.0, 0.2, 4, 9, True, xy, disc=True)
