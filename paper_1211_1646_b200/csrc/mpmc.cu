@@ -404,8 +404,9 @@ int mpmc_sweep(mpmc_ctx* c, uint64_t k) {
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = (pdl && c->stream != nullptr) ? 1 : 0;
-    void* args[] = {(void*)&c->p};
-    for (uint64_t i = 0; i < k; ++i) CU(cudaLaunchKernelExC(&cfg, c->tile_kernel, args));
+    unsigned long long t = c->t_host - k;          // sweep index of each launch (kernel argument: uniform on the device)
+    void* args[] = {(void*)&c->p, (void*)&t};
+    for (uint64_t i = 0; i < k; ++i, ++t) CU(cudaLaunchKernelExC(&cfg, c->tile_kernel, args));
   }
   // ... and the general kernel runs whatever is left up to the target sweep index (normally nothing)
   const int st = launch_sweeps(c, c->t_host, OP_SWEEPS, 0, 0.0);

@@ -8,7 +8,8 @@
 // pass over HBM/L2 per sweep instead of six, neighbour loads at shared-memory latency.
 //
 // Halo recompute: sub-sweep k (k = 1..4) updates the cells of its colour whose ring index
-// (distance to the edge of the loaded region) is >= k.  A cell of ring r reads neighbours of ring >= r-1, and
+// (distance to the edge of the loaded region) is >= k (>= k + 1 on the three sides the shift does not pull from, see
+// sub_sweep_rect).  A cell of ring r reads neighbours of ring >= r-1, and
 // colours already updated this sweep are correct from ring j <= k-1 on, the others are untouched: by induction
 // every value read is correct.  After sub-sweep 4 all cells of ring >= 4 are final; the shift of an interior
 // cell (ring >= 5) reads itself and one neighbour (ring >= 4).  Halo cells are updated redundantly by the
@@ -72,6 +73,19 @@ __device__ __forceinline__ TileBox tile_box(const Params& p, uint32_t tx, uint32
   b.w = b.TX + 2 * HALO; b.h = b.TY + 2 * HALO;
   b.pw = b.w / 2; b.ph = b.h / 2;
   return b;
+}
+
+// The cells sub-sweep k (1..4) has to update, as a rectangle of local coordinates.  The shift of the interior (ring >= 5)
+// reads one more column or row on the side the shift pulls from (direction dir), so after sub-sweep 4 the cells of
+// S4 = interior + that one line must be final; sub-sweep k then needs its colour correct on S4 grown by 4 - k, whose
+// neighbours (S4 grown by 5 - k) are correct from the earlier sub-sweeps by the same rule.  That is ring >= k on the side
+// of the shift and ring >= k + 1 on the other three.
+struct SubRect { uint32_t x_lo, x_hi, y_lo, y_hi; };
+__device__ __forceinline__ SubRect sub_sweep_rect(const TileBox& tb, uint32_t k, uint32_t dir) {
+  SubRect r;
+  r.x_lo = k + (dir == 1u ? 0u : 1u); r.x_hi = tb.w - 1u - (k + (dir == 0u ? 0u : 1u));   // dir 0: +x pulls from x+1, 1: -x
+  r.y_lo = k + (dir == 3u ? 0u : 1u); r.y_hi = tb.h - 1u - (k + (dir == 2u ? 0u : 1u));   // dir 2: +y, 3: -y
+  return r;
 }
 
 // A crowded cell inside the loaded region: where it is, and its slots 2 and 3 (slot pair 1 of global memory).
@@ -251,7 +265,7 @@ __device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* s
     flip = bounded(S[0], 2u) == 0u;
   }
   if (flip) { P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }
-  uint32_t n_acc = 0, n_rb = 0, amask = 0;
+  uint32_t amask = 0, bmask = 0;       // bit s: move s accepted / left the cell
 #pragma unroll
   for (int s = 0; s < NS; ++s) {       // Alg. 2 lines 11-32 (L189-230)
     const P Mx = R::add(Ax, ddx[s]), My = R::add(Ay, ddy[s]);              // D_move = l + displacement
@@ -267,11 +281,11 @@ __device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* s
     }
     const bool acc = inside && !(rmin < sigma2);                           // strict (A4)
     if (acc) { Ax = Mx; Ay = My; amask |= 1u << s; }                       // lines 24-27 (L215-222)
-    n_rb += inside ? 0u : 1u;
-    n_acc += acc ? 1u : 0u;
+    if (!inside) bmask |= 1u << s;                                         // leaves the cell: rejected (L79, L118)
     if (two) { const P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }   // s mod n cycling (L75)
   }
   if (n == 0u) amask = 0u;             // empty cells attempt nothing (A10)
+  const uint32_t n_acc = __popc(amask), n_rb = __popc(bmask);
   if (amask != 0u) {                   // write back (line 34, L234): the slot pair in slot order
     if (two && (NS & 1)) flip = !flip;
     Half<P> o;
@@ -330,13 +344,14 @@ __device__ __noinline__ void tile_shift_cell_general(const Params& p, const Smem
 // shared counter, so a warp that was busy with a crowded cell (or started late) simply takes fewer.
 template <typename P, int NS, bool DEBUG, uint32_t QL>
 __device__ __forceinline__ void tile_sub_sweep_cells(const Params& p, SmemCell<P>* sm, const CrowdList<P>& cl,
-                                                     const uint32_t nc, const TileBox& tb, const uint32_t k, const int gx0,
-                                                     const int gy0, const unsigned long long t, uint32_t* next,
-                                                     Tally& tally) {
+                                                     const uint32_t nc, const TileBox& tb, const uint32_t k,
+                                                     const uint32_t dir, const int gx0, const int gy0,
+                                                     const unsigned long long t, uint32_t* next, Tally& tally) {
   constexpr uint32_t qx = QL & 1u, qy = QL >> 1;
   const uint32_t PS = p.tl_PS, pw = tb.pw;
-  const uint32_t px0 = (k - qx + 1u) >> 1, px1 = (tb.w - 1u - k - qx) >> 1;
-  const uint32_t py0 = (k - qy + 1u) >> 1, py1 = (tb.h - 1u - k - qy) >> 1;
+  const SubRect rc = sub_sweep_rect(tb, k, dir);
+  const uint32_t px0 = (rc.x_lo - qx + 1u) >> 1, px1 = (rc.x_hi - qx) >> 1;
+  const uint32_t py0 = (rc.y_lo - qy + 1u) >> 1, py1 = (rc.y_hi - qy) >> 1;
   const uint32_t nxp = px1 - px0 + 1u, count = nxp * (py1 - py0 + 1u);
   const uint32_t inv = small_div_magic(nxp);
   const uint32_t lane = threadIdx.x & 31u;
@@ -466,20 +481,23 @@ __device__ __forceinline__ void tile_shift_cells(const Params& p, const SmemCell
 // ---------------------------------------------------------------------------------------------------------
 template <typename P, int NS, bool DEBUG>
 __global__ void __launch_bounds__(TileThreads<P>::value, 1)
-k_tile_sweep(const __grid_constant__ Params p) {
+k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   using R = Real<P>;
   const uint32_t TILE_THREADS = blockDim.x;           // at most TileThreads<P>::value (the host may launch fewer)
   extern __shared__ __align__(16) unsigned char tile_smem[];
   SmemCell<P>* sm = reinterpret_cast<SmemCell<P>*>(tile_smem);
   __shared__ CrowdList<P> cl;
-  __shared__ Draws sdraw;
   __shared__ uint32_t s_last;
   __shared__ uint32_t s_next[8];                 // chunk counters: sub-sweeps 1-4, shift planes 0-3
   Ctl* ctl = p.ctl;
-  // launched with programmatic stream serialisation (mpmc.cu): everything below reads what the previous sweep wrote
+  // The sweep index comes as a kernel argument (the host counts launches), so the draws of this sweep — a pure function
+  // of (seed, t), Alg. 1 lines 2, 15, 16 (L64, L90-91) — and all they decide are warp-uniform values computed before the
+  // wait.  Launched with programmatic stream serialisation (mpmc.cu): everything below the wait reads what the previous
+  // sweep wrote.  If the state is not at sweep t (an earlier launch left its sweep to the general kernel), return.
+  const Draws dr = draw_sweep(p, t);
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  const unsigned long long t = ctl->t;
+  if (ctl->t != t) return;
   const uint32_t slot = (uint32_t)(t & 3u), slot1 = (uint32_t)((t + 1ull) & 3u), slot2 = (uint32_t)((t + 2ull) & 3u);
   if (ctl->crowded[slot] != 0u) return;          // too many crowded cells: the general kernel takes over
   const uint32_t cur = ctl->cur, nxt = cur ^ 1u;
@@ -489,7 +507,6 @@ k_tile_sweep(const __grid_constant__ Params p) {
   const uint32_t PS = p.tl_PS, pw = tb.pw, ph = tb.ph, Mqp = p.Mqp;
   const int gx0 = (int)tb.x0 - HALO, gy0 = (int)tb.y0 - HALO;       // global cell of the region's corner (unwrapped)
   if (tid == 0) {
-    sdraw = draw_sweep(p, t);                    // Alg. 1 lines 2, 15, 16 (L64, L90-91)
     cl.n = 0u;
     for (int i = 0; i < 8; ++i) s_next[i] = 0u;
     ctl->crowded[slot2] = 0u; ctl->ccount[slot2] = 0u;   // slots of the sweep after next: nobody uses them now
@@ -545,7 +562,6 @@ k_tile_sweep(const __grid_constant__ Params p) {
     }
   }
   __syncthreads();
-  const Draws dr = sdraw;
   const uint32_t nc = cl.n;
   Tally tally;
 
@@ -555,13 +571,14 @@ k_tile_sweep(const __grid_constant__ Params p) {
     const uint32_t Qg = k == 1u ? dr.order[0] : k == 2u ? dr.order[1] : k == 3u ? dr.order[2] : dr.order[3];
     const uint32_t q = Qg ^ 3u;                  // the region starts at an odd cell (x0 - 5, y0 - 5): colours flip
     const uint32_t qx = q & 1u, qy = q >> 1;
+    const SubRect rc = sub_sweep_rect(tb, k, dr.dir);
     // cells of this colour next to a crowded cell: one warp each, before the warp's share of the ordinary cells
     for (uint32_t pi = warp; pi < 9u * nc; pi += TILE_THREADS / 32) {      // (listed cell, 3x3 position) pairs
       const uint32_t e = pi / 9u, d = pi - 9u * e;
       const uint32_t elx = cl.e[e].lxly & 0xFFFFu, ely = cl.e[e].lxly >> 16;
       const uint32_t lx = elx + d % 3u - 1u, ly = ely + d / 3u - 1u;       // may wrap below 0: fails the tests
       if ((lx & 1u) != qx || (ly & 1u) != qy) continue;
-      if (lx < k || lx > tb.w - 1u - k || ly < k || ly > tb.h - 1u - k) continue;               // ring >= k
+      if (lx < rc.x_lo || lx > rc.x_hi || ly < rc.y_lo || ly > rc.y_hi) continue;               // not in this sub-sweep's rectangle
       bool first = true;                                         // a cell next to two listed cells is done once
       for (uint32_t e2 = 0; e2 < e; ++e2) {
         const uint32_t v = cl.e[e2].lxly;
@@ -574,10 +591,10 @@ k_tile_sweep(const __grid_constant__ Params p) {
       tile_update_cell_warp<P, DEBUG>(p, sm, cl, nc, q, pw, si, cell, interior, t, tally);
     }
     switch (q) {                                   // the local colour as a compile-time constant: uniform offsets
-      case 0: tile_sub_sweep_cells<P, NS, DEBUG, 0>(p, sm, cl, nc, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
-      case 1: tile_sub_sweep_cells<P, NS, DEBUG, 1>(p, sm, cl, nc, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
-      case 2: tile_sub_sweep_cells<P, NS, DEBUG, 2>(p, sm, cl, nc, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
-      default: tile_sub_sweep_cells<P, NS, DEBUG, 3>(p, sm, cl, nc, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      case 0: tile_sub_sweep_cells<P, NS, DEBUG, 0>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      case 1: tile_sub_sweep_cells<P, NS, DEBUG, 1>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      case 2: tile_sub_sweep_cells<P, NS, DEBUG, 2>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      default: tile_sub_sweep_cells<P, NS, DEBUG, 3>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
     }
     __syncthreads();
   }

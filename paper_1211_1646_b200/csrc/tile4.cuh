@@ -19,13 +19,14 @@ template <typename P> struct Tile4Threads { static constexpr int value = sizeof(
 // The cells of sub-sweep k: local colour QL at ring >= k, in chunks of 32 drawn from a shared counter.
 template <typename P, int NS, bool DEBUG, bool DISC, uint32_t QL>
 __device__ __forceinline__ void tile4_sub_sweep_cells(const Params& p, SmemCell<P>* sm0, SmemCell<P>* sm1, const TileBox& tb,
-                                                      const uint32_t k, const int gx0, const int gy0,
+                                                      const uint32_t k, const uint32_t dir, const int gx0, const int gy0,
                                                       const unsigned long long t, uint32_t* next, Tally& tally) {
   using R = Real<P>;
   constexpr uint32_t qx = QL & 1u, qy = QL >> 1;
   const uint32_t PS = p.tl_PS, pw = tb.pw;
-  const uint32_t px0 = (k - qx + 1u) >> 1, px1 = (tb.w - 1u - k - qx) >> 1;
-  const uint32_t py0 = (k - qy + 1u) >> 1, py1 = (tb.h - 1u - k - qy) >> 1;
+  const SubRect rc = sub_sweep_rect(tb, k, dir);
+  const uint32_t px0 = (rc.x_lo - qx + 1u) >> 1, px1 = (rc.x_hi - qx) >> 1;
+  const uint32_t py0 = (rc.y_lo - qy + 1u) >> 1, py1 = (rc.y_hi - qy) >> 1;
   const uint32_t nxp = px1 - px0 + 1u, count = nxp * (py1 - py0 + 1u);
   const uint32_t inv = small_div_magic(nxp);
   const uint32_t lane = threadIdx.x & 31u;
@@ -72,20 +73,23 @@ __device__ __forceinline__ void tile4_sub_sweep_cells(const Params& p, SmemCell<
 // ---------------------------------------------------------------------------------------------------------
 template <typename P, int NS, bool DEBUG, bool DISC>
 __global__ void __launch_bounds__(Tile4Threads<P>::value, 1)
-k_tile4_sweep(const __grid_constant__ Params p) {
+k_tile4_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   using R = Real<P>;
   extern __shared__ __align__(16) unsigned char tile_smem[];
   const uint32_t PS = p.tl_PS;
   SmemCell<P>* sm0 = reinterpret_cast<SmemCell<P>*>(tile_smem);     // slot pair 0 of the four local colour planes
   SmemCell<P>* sm1 = sm0 + 4u * PS;                                 // slot pair 1
-  __shared__ Draws sdraw;
   __shared__ uint32_t s_last;
   __shared__ uint32_t s_next[8];                 // chunk counters: sub-sweeps 1-4, shift planes 0-3
   Ctl* ctl = p.ctl;
-  // launched with programmatic stream serialisation (mpmc.cu): everything below reads what the previous sweep wrote
+  // The sweep index comes as a kernel argument (the host counts launches), so the draws of this sweep — a pure function
+  // of (seed, t), Alg. 1 lines 2, 15, 16 (L64, L90-91) — and all they decide are warp-uniform values computed before the
+  // wait.  Launched with programmatic stream serialisation (mpmc.cu): everything below the wait reads what the previous
+  // sweep wrote.  If the state is not at sweep t (an earlier launch left its sweep to the general kernel), return.
+  const Draws dr = draw_sweep(p, t);
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  const unsigned long long t = ctl->t;
+  if (ctl->t != t) return;
   const uint32_t cur = ctl->cur, nxt = cur ^ 1u;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, NW = blockDim.x >> 5;
   const uint32_t ty = blockIdx.x / p.tl_ntx, tx = blockIdx.x - ty * p.tl_ntx;
@@ -94,7 +98,6 @@ k_tile4_sweep(const __grid_constant__ Params p) {
   const int gx0 = (int)tb.x0 - HALO, gy0 = (int)tb.y0 - HALO;       // global cell of the region's corner (unwrapped)
   const P FAR = R::far_away(), HALF_FAR = FAR * (P)0.5;
   if (tid == 0) {
-    sdraw = draw_sweep(p, t);                    // Alg. 1 lines 2, 15, 16 (L64, L90-91)
     for (int i = 0; i < 8; ++i) s_next[i] = 0u;
   }
   __syncthreads();
@@ -133,7 +136,6 @@ k_tile4_sweep(const __grid_constant__ Params p) {
     }
   }
   __syncthreads();
-  const Draws dr = sdraw;
   Tally tally;
 
   // ---- four sub-sweeps (Alg. 1 lines 3-14, L66-88): sub-sweep k updates its colour at ring >= k ----
@@ -141,10 +143,10 @@ k_tile4_sweep(const __grid_constant__ Params p) {
   for (uint32_t k = 1; k <= 4u; ++k) {
     const uint32_t Qg = k == 1u ? dr.order[0] : k == 2u ? dr.order[1] : k == 3u ? dr.order[2] : dr.order[3];
     switch (Qg ^ 3u) {                           // the region starts at an odd cell (x0 - 5, y0 - 5): colours flip
-      case 0: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 0>(p, sm0, sm1, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
-      case 1: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 1>(p, sm0, sm1, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
-      case 2: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 2>(p, sm0, sm1, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
-      default: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 3>(p, sm0, sm1, tb, k, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      case 0: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 0>(p, sm0, sm1, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      case 1: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 1>(p, sm0, sm1, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      case 2: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 2>(p, sm0, sm1, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      default: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 3>(p, sm0, sm1, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
     }
     __syncthreads();
   }
