@@ -141,7 +141,9 @@ int launch_sweeps(mpmc_ctx* c, unsigned long long t_end, uint32_t op, uint32_t a
   return MPMC_OK;
 }
 
-const void* pick_tile_kernel(bool fp32, bool debug, uint32_t n_s) {
+const void* pick_tile_kernel(bool fp32, bool debug, uint32_t n_s, bool compact) {
+  // dilute systems (most cells empty): the variant that runs the cell update on compacted warps of non-empty cells
+  if (compact && fp32 && n_s == 4) return debug ? (const void*)k_tile_sweep<float, 4, true, true> : (const void*)k_tile_sweep<float, 4, false, true>;
   if (n_s == 4) return fp32 ? (debug ? (const void*)k_tile_sweep<float, 4, true> : (const void*)k_tile_sweep<float, 4, false>)
                             : (debug ? (const void*)k_tile_sweep<double, 4, true> : (const void*)k_tile_sweep<double, 4, false>);
   if (n_s == 8) return fp32 ? (debug ? (const void*)k_tile_sweep<float, 8, true> : (const void*)k_tile_sweep<float, 8, false>)
@@ -306,12 +308,14 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   // the square proposal and n_s in {4, 8}; otherwise tile4.cuh (all 4 slots; any width, both proposals) for n_s = 4.
   c->tile_kernel = nullptr; c->tile_grid = 0; c->tile_smem = 0; c->t_host = 0;
   const bool two_slot = c->nf == 2 && (n_s == 4 || n_s == 8) && !disc;
-  const void* tk = two_slot ? pick_tile_kernel(fp32, debug, n_s) : pick_tile4_kernel(fp32, debug, disc, n_s);
+  const bool compact = (double)N < 0.6 * (double)p.mx * (double)p.my;    // fewer than 0.6 disks per cell
+  const void* tk = two_slot ? pick_tile_kernel(fp32, debug, n_s, compact) : pick_tile4_kernel(fp32, debug, disc, n_s);
   if (tk) {
     int smem_optin = 0;
     cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     const size_t cell_bytes = (fp32 ? sizeof(SmemCell<float>) : sizeof(SmemCell<double>)) * (two_slot ? 1 : 2);
-    const size_t stat = (two_slot ? (fp32 ? sizeof(CrowdList<float>) : sizeof(CrowdList<double>)) : 0) + 256;   // static shared memory
+    const size_t stat = (two_slot ? (fp32 ? sizeof(CrowdList<float>) : sizeof(CrowdList<double>)) : 0) + 256   // static shared memory
+                        + (two_slot && compact ? (TileThreads<float>::value / 32) * 64 * sizeof(uint16_t) : 0);
     const size_t smem_max = (size_t)smem_optin > stat ? (size_t)smem_optin - stat : 0;
     uint32_t ntx = 0, nty = 0, PS = 0;
     c->tile_threads = two_slot ? (fp32 ? TileThreads<float>::value : TileThreads<double>::value)

@@ -59,6 +59,9 @@ __device__ __forceinline__ void sts_half(SmemCell<double>* s, uint32_t i, const 
   s[i].a = make_double2(h.x.x, h.x.y); s[i].b = make_double2(h.y.x, h.y.y);
 }
 
+__device__ __forceinline__ float lds_x0(const SmemCell<float>* s, uint32_t i) { return s[i].v.x; }     // x of slot 0
+__device__ __forceinline__ double lds_x0(const SmemCell<double>* s, uint32_t i) { return s[i].a.x; }
+
 // Geometry of one tile: interior [x0, x0+TX) x [y0, y0+TY) in cells (all even), loaded region = interior grown
 // by HALO; shared-memory planes by LOCAL colour q = 2 (ly & 1) + (lx & 1), pw x ph cells each, stride PS.
 struct TileBox {
@@ -372,6 +375,68 @@ __device__ __forceinline__ void tile_sub_sweep_cells(const Params& p, SmemCell<P
   }
 }
 
+// The same for dilute systems (most cells empty, e.g. BASELINE config C5: 62 % at phi = 0.30): an empty cell attempts
+// nothing (A10), so running the update on it wastes the lane.  Each warp scans its chunks, queues the indices of the
+// NON-EMPTY cells in a private shared-memory queue (ballot + prefix count) and runs the update on full warps of them.
+template <typename P, int NS, bool DEBUG, uint32_t QL>
+__device__ __forceinline__ void tile_sub_sweep_cells_compact(const Params& p, SmemCell<P>* sm, const CrowdList<P>& cl,
+                                                             const uint32_t nc, const TileBox& tb, const uint32_t k,
+                                                             const uint32_t dir, const int gx0, const int gy0,
+                                                             const unsigned long long t, uint32_t* next, uint16_t* wq,
+                                                             Tally& tally) {
+  constexpr uint32_t qx = QL & 1u, qy = QL >> 1;
+  const uint32_t PS = p.tl_PS, pw = tb.pw;
+  const SubRect rc = sub_sweep_rect(tb, k, dir);
+  const uint32_t px0 = (rc.x_lo - qx + 1u) >> 1, px1 = (rc.x_hi - qx) >> 1;
+  const uint32_t py0 = (rc.y_lo - qy + 1u) >> 1, py1 = (rc.y_hi - qy) >> 1;
+  const uint32_t nxp = px1 - px0 + 1u, count = nxp * (py1 - py0 + 1u);
+  const uint32_t inv = small_div_magic(nxp);
+  const uint32_t lane = threadIdx.x & 31u;
+  const P HALF_FAR = Real<P>::far_away() * (P)0.5;
+  uint32_t qn = 0;                                             // queued cells (warp-uniform)
+  bool more = true;
+  while (more || qn > 0u) {
+    if (more) {                                                // scan one chunk of 32 cells
+      uint32_t base = 0;
+      if (lane == 0u) base = atomicAdd(next, 32u);
+      base = __shfl_sync(0xFFFFFFFFu, base, 0);
+      more = base < count;
+      const uint32_t idx = base + lane;
+      bool occ = false;
+      if (more && idx < count) {
+        const uint32_t ry = small_div(idx, inv), rx = idx - ry * nxp;
+        const uint32_t px = px0 + rx, py = py0 + ry, lx = 2u * px + qx, ly = 2u * py + qy;
+        if (!(nc != 0u && crowd_near(cl, nc, lx, ly))) {       // else: done by a warp (tile_update_cell_warp)
+          occ = lds_x0(sm, QL * PS + py * pw + px) < HALF_FAR; // slots fill in order: slot 0 empty = cell empty
+          if (DEBUG && !occ && lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY)
+            p.mask[wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx)] = 0u;
+        }
+      }
+      const uint32_t m = __ballot_sync(0xFFFFFFFFu, occ);
+      if (occ) wq[qn + __popc(m & ((1u << lane) - 1u))] = (uint16_t)idx;
+      qn += __popc(m);
+      __syncwarp();
+    }
+    if (qn >= 32u || (!more && qn > 0u)) {                     // a full warp of non-empty cells (or the last few)
+      const uint32_t take = qn < 32u ? qn : 32u;
+      const uint32_t mine = wq[lane], rest = wq[lane + 32u];
+      __syncwarp();
+      if (lane + 32u < qn) wq[lane] = (uint16_t)rest;          // keep the overflow at the front of the queue
+      qn -= take;
+      if (lane < take) {
+        const uint32_t idx = mine;
+        const uint32_t ry = small_div(idx, inv), rx = idx - ry * nxp;
+        const uint32_t px = px0 + rx, py = py0 + ry, lx = 2u * px + qx, ly = 2u * py + qy;
+        const uint32_t si = QL * PS + py * pw + px;
+        const uint32_t cell = wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx);
+        const bool interior = lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY;
+        tile_update_cell<P, NS, DEBUG, QL>(p, sm, si, pw, cell, interior, t, tally);
+      }
+      __syncwarp();
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // The shift of the interior cells of a tile (Algorithm 4, pull form: one thread per NEW cell, L350), from the
 // planes in shared memory to the other global buffer.  Warps draw chunks of 64 cells of one local colour plane
@@ -479,7 +544,7 @@ __device__ __forceinline__ void tile_shift_cells(const Params& p, const SmemCell
 // The fused sweep kernel: one CTA per tile, one launch per sweep.  See the header of this file.
 // Dynamic shared memory: 4 planes x tl_PS cells x sizeof(SmemCell<P>).
 // ---------------------------------------------------------------------------------------------------------
-template <typename P, int NS, bool DEBUG>
+template <typename P, int NS, bool DEBUG, bool COMPACT = false>
 __global__ void __launch_bounds__(TileThreads<P>::value, 1)
 k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   using R = Real<P>;
@@ -489,6 +554,7 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   __shared__ CrowdList<P> cl;
   __shared__ uint32_t s_last;
   __shared__ uint32_t s_next[8];                 // chunk counters: sub-sweeps 1-4, shift planes 0-3
+  __shared__ uint16_t s_queue[COMPACT ? (TileThreads<P>::value / 32) * 64 : 1];   // per-warp queues of non-empty cells
   Ctl* ctl = p.ctl;
   // The sweep index comes as a kernel argument (the host counts launches), so the draws of this sweep — a pure function
   // of (seed, t), Alg. 1 lines 2, 15, 16 (L64, L90-91) — and all they decide are warp-uniform values computed before the
@@ -590,11 +656,21 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
       const bool interior = lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY;
       tile_update_cell_warp<P, DEBUG>(p, sm, cl, nc, q, pw, si, cell, interior, t, tally);
     }
-    switch (q) {                                   // the local colour as a compile-time constant: uniform offsets
-      case 0: tile_sub_sweep_cells<P, NS, DEBUG, 0>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
-      case 1: tile_sub_sweep_cells<P, NS, DEBUG, 1>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
-      case 2: tile_sub_sweep_cells<P, NS, DEBUG, 2>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
-      default: tile_sub_sweep_cells<P, NS, DEBUG, 3>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
+    if (COMPACT) {
+      uint16_t* wq = &s_queue[COMPACT ? warp * 64u : 0u];
+      switch (q) {                                 // the local colour as a compile-time constant: uniform offsets
+        case 0: tile_sub_sweep_cells_compact<P, NS, DEBUG, 0>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], wq, tally); break;
+        case 1: tile_sub_sweep_cells_compact<P, NS, DEBUG, 1>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], wq, tally); break;
+        case 2: tile_sub_sweep_cells_compact<P, NS, DEBUG, 2>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], wq, tally); break;
+        default: tile_sub_sweep_cells_compact<P, NS, DEBUG, 3>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], wq, tally); break;
+      }
+    } else {
+      switch (q) {                                 // the local colour as a compile-time constant: uniform offsets
+        case 0: tile_sub_sweep_cells<P, NS, DEBUG, 0>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
+        case 1: tile_sub_sweep_cells<P, NS, DEBUG, 1>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
+        case 2: tile_sub_sweep_cells<P, NS, DEBUG, 2>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
+        default: tile_sub_sweep_cells<P, NS, DEBUG, 3>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
+      }
     }
     __syncthreads();
   }
