@@ -308,7 +308,8 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   // the square proposal and n_s in {4, 8}; otherwise tile4.cuh (all 4 slots; any width, both proposals) for n_s = 4.
   c->tile_kernel = nullptr; c->tile_grid = 0; c->tile_smem = 0; c->t_host = 0;
   const bool two_slot = c->nf == 2 && (n_s == 4 || n_s == 8) && !disc;
-  const bool compact = (double)N < 0.6 * (double)p.mx * (double)p.my;    // fewer than 0.6 disks per cell
+  bool compact = (double)N < 0.6 * (double)p.mx * (double)p.my;          // fewer than 0.6 disks per cell
+  if (const char* e = std::getenv("MPMC_COMPACT")) compact = e[0] == '1';    // experiments
   const void* tk = two_slot ? pick_tile_kernel(fp32, debug, n_s, compact) : pick_tile4_kernel(fp32, debug, disc, n_s);
   if (tk) {
     int smem_optin = 0;
