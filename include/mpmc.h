@@ -119,6 +119,13 @@ int mpmc_debug_state(mpmc_ctx* ctx, void* counts, void* slab, void* ids, void* a
  * kernel only when more cells hold 3 or 4 disks than it can carry).  Synchronises. */
 int mpmc_debug_path(mpmc_ctx* ctx, uint64_t out[2]);
 
+/* Test hook (pure host arithmetic, no device needed): the tiling the fused tile kernels would use for a grid of
+ * 2 hx x 2 hy cells when a cell takes cell_bytes of shared memory, an SM offers smem_max bytes and the device has sms
+ * SMs.  out = {tiles along x, tiles along y, shared-memory plane stride in cells}.  Every tile (rounded up to even
+ * sizes) plus a halo of 5 cells on each side fits smem_max and is no wider than the grid; MPMC_ERR_BOX if no such
+ * tiling exists (grids under 12 cells across). */
+int mpmc_debug_tiling(uint32_t hx, uint32_t hy, size_t cell_bytes, size_t smem_max, uint32_t sms, uint32_t out[3]);
+
 /* Test hook: Philox4x32-10 evaluated ON THE DEVICE by the same routine the kernels use.
  * ctr = device u32[n][4], key = host u32[2], out = device u32[n][4]; enqueued on cuda_stream and synchronised. */
 int mpmc_debug_philox(const uint32_t* ctr, const uint32_t key[2], uint32_t* out, uint32_t n, void* cuda_stream);

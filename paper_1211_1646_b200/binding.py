@@ -34,6 +34,7 @@ SYMBOLS = {
     "mpmc_debug_shift": (C.c_int, [_vp, _u32, _dbl]),
     "mpmc_debug_state": (C.c_int, [_vp, _vp, _vp, _vp, _vp, C.POINTER(_dbl), C.POINTER(_u64), C.POINTER(_u64)]),
     "mpmc_debug_path": (C.c_int, [_vp, C.POINTER(_u64)]),
+    "mpmc_debug_tiling": (C.c_int, [_u32, _u32, C.c_size_t, C.c_size_t, _u32, C.POINTER(_u32)]),
     "mpmc_debug_philox": (C.c_int, [_vp, C.POINTER(_u32), _vp, _u32, _vp]),
     "mpmc_strerror": (C.c_char_p, [C.c_int]),
     "mpmc_version": (C.c_char_p, []),
@@ -232,6 +233,17 @@ class Mpmc:
                     ids=ids.cpu().numpy().view(np.uint32),
                     accept_mask=mask.cpu().numpy().view(np.uint32) if mask is not None else None,
                     origin=(origin[0], origin[1]), sweep=int(sw.value), digest=int(dg.value))
+
+
+def tiling(hx: int, hy: int, cell_bytes: int = 16, smem_max: int = 226 * 1024, sms: int = 148):
+    """(tiles along x, tiles along y, plane stride) the tile kernels would use; host arithmetic only.  None if the grid is
+    too small to tile."""
+    out = (_u32 * 3)()
+    code = lib().mpmc_debug_tiling(int(hx), int(hy), int(cell_bytes), int(smem_max), int(sms), out)
+    if code == -2:
+        return None
+    _chk(code)
+    return int(out[0]), int(out[1]), int(out[2])
 
 
 def device_philox(ctr, key, device="cuda:0"):

@@ -521,6 +521,14 @@ int mpmc_debug_path(mpmc_ctx* c, uint64_t out[2]) {
   return st;
 }
 
+int mpmc_debug_tiling(uint32_t hx, uint32_t hy, size_t cell_bytes, size_t smem_max, uint32_t sms, uint32_t out[3]) {
+  if (!out || hx == 0 || hy == 0 || cell_bytes == 0 || sms == 0) return MPMC_ERR_ARG;
+  uint32_t ntx = 0, nty = 0, PS = 0;
+  if (!choose_tiling(hx, hy, cell_bytes, smem_max, sms, &ntx, &nty, &PS)) return MPMC_ERR_BOX;
+  out[0] = ntx; out[1] = nty; out[2] = PS;
+  return MPMC_OK;
+}
+
 int mpmc_debug_philox(const uint32_t* ctr, const uint32_t key[2], uint32_t* out, uint32_t n, void* cuda_stream) {
   if (!ctr || !key || !out) return MPMC_ERR_ARG;
   if (n == 0) return MPMC_OK;
