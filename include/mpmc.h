@@ -48,6 +48,9 @@ typedef struct mpmc_ctx mpmc_ctx; /* opaque host object; owns no device memory *
 #define MPMC_FP32 0x2u  /* ... in float (the paper's benchmarks, L390); pressure histogram still in double */
 #define MPMC_DISC 0x4u   /* trial moves uniform in the DISC of radius d (the paper's rng.inCircle(d), L190) instead of the
                            square [-d, d]^2 of reading A2; runs on the general kernel */
+/* ablations of PAPER.md section 2.4 / Table 1 (L114-142); both leave the chain valid only in the sense the paper discusses */
+#define MPMC_NO_PARTICLE_SHUFFLE 0x8u  /* visit the disks of a cell in slot order (the paper shows a pressure bias) */
+#define MPMC_NO_SET_SHUFFLE 0x10u     /* run the checkerboard sets in the fixed order a, b, c, d (harmless per the paper) */
 #define MPMC_DEBUG 0x100u /* record per-cell accept masks and the accept-sequence digest (tests only; slower) */
 
 /* Bytes of device workspace mpmc_create needs for this system (0 on invalid arguments).  Pure host arithmetic.

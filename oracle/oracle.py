@@ -26,6 +26,8 @@ _LIB = os.path.join(_HERE, "liboracle_mpmc.so")
 
 FP64 = 1
 FP32 = 2
+NO_PARTICLE_SHUFFLE = 8     # ablations of PAPER.md section 2.4 / Table 1 (L114-142)
+NO_SET_SHUFFLE = 16
 DISC = 4      # trial displacement uniform in the disc of radius d instead of the square of reading A2
 
 ERR = {0: "ok", -1: "bad argument", -2: "box too small", -4: "overlap or out-of-box input",
@@ -121,13 +123,14 @@ class Oracle:
     """oracle_* calls with numpy host arrays.  Same call list as the product's `Mpmc` binding."""
 
     def __init__(self, N: int, box, sigma: float, d: float, n_s: int, seed: int, fp32: bool = False,
-                 w_target: float = 0.0, disc: bool = False):
+                 w_target: float = 0.0, disc: bool = False, particle_shuffle: bool = True, set_shuffle: bool = True):
         self._h = C.c_void_p()
         self.N = int(N)
         self.fp32 = bool(fp32)
         self.sigma = float(sigma)
         b = (C.c_double * 2)(float(box[0]), float(box[1]))
-        _chk(lib().oracle_create(C.byref(self._h), self.N, b, sigma, d, n_s, seed, (FP32 if fp32 else FP64) | (DISC if disc else 0),
+        _chk(lib().oracle_create(C.byref(self._h), self.N, b, sigma, d, n_s, seed, (FP32 if fp32 else FP64) | (DISC if disc else 0)
+                                 | (0 if particle_shuffle else NO_PARTICLE_SHUFFLE) | (0 if set_shuffle else NO_SET_SHUFFLE),
                                  float(w_target)))
         m = (C.c_uint32 * 2)()
         w = (C.c_double * 2)()

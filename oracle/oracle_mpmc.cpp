@@ -41,7 +41,9 @@ enum {
   OR_ERR_CELL_OVERFLOW = -5,
   OR_ERR_STATE = -7,
 };
-enum { OR_FP64 = 1u, OR_FP32 = 2u, OR_DISC = 4u };   // OR_DISC: trial displacement uniform in the disc of radius d (L190)
+enum { OR_FP64 = 1u, OR_FP32 = 2u, OR_DISC = 4u,
+       // ablations of PAPER.md section 2.4 / Table 1 (L114-142): leave out the particle shuffle / the checkerboard-set shuffle
+       OR_NO_PARTICLE_SHUFFLE = 8u, OR_NO_SET_SHUFFLE = 16u };   // OR_DISC: trial displacement uniform in the disc of radius d (L190)
 
 // ---------------------------------------------------------------------------------------------
 // Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11): 10 rounds; multipliers 0xD2511F53, 0xCD9E8D57;
@@ -130,12 +132,12 @@ struct SweepDraws {
   uint32_t dist_word; // the word the shift distance is made of (Alg. 1 line 15, L90)
 };
 
-SweepDraws sweep_draws(uint64_t seed, uint64_t t) {
+SweepDraws sweep_draws(uint64_t seed, uint64_t t, bool shuffle_sets = true) {
   SweepDraws D;
   uint32_t G[4], H[4];
   draw(seed, CELL_GLOBAL, t, SLOT_ORDER, G);
   for (uint32_t q = 0; q < 4; ++q) D.order[q] = q;
-  fisher_yates(D.order, 4, G);            // uses G[0], G[1], G[2]   (Alg. 1 line 2, L64)
+  if (shuffle_sets) fisher_yates(D.order, 4, G);   // uses G[0], G[1], G[2]   (Alg. 1 line 2, L64)
   D.dir = G[3] >> 30;
   draw(seed, CELL_GLOBAL, t, SLOT_DIST, H);
   D.dist_word = H[0];
@@ -202,7 +204,7 @@ struct Sim : Base {
     mask[c] = 0;
     if (nc == 0) return;                                        // lines 4-7 (L181-185); reading A10
     uint32_t perm[NMAX] = {0, 1, 2, 3};
-    if (nc >= 2) {                                              // line 9 (L187): rng.shuffle
+    if (nc >= 2 && !(flags & OR_NO_PARTICLE_SHUFFLE)) {          // line 9 (L187): rng.shuffle
       uint32_t S[4];
       draw(seed, (uint32_t)c, t, SLOT_SHUFFLE, S);
       fisher_yates(perm, nc, S);
@@ -330,7 +332,7 @@ struct Sim : Base {
   int sweep(uint64_t k) override {
     if (!loaded) return OR_ERR_STATE;
     for (uint64_t it = 0; it < k; ++it) {
-      const SweepDraws D = sweep_draws(seed, t);
+      const SweepDraws D = sweep_draws(seed, t, !(flags & OR_NO_SET_SHUFFLE));
       for (uint32_t q = 0; q < 4; ++q) sub_sweep(D.order[q]);            // lines 3-14
       const bool along_x = D.dir < 2;
       const P half = (P)0.5 * (along_x ? wx : wy);                        // line 15: uniform(0, w/2)

@@ -13,6 +13,8 @@ from . import build as _build
 FP64 = 0x1
 FP32 = 0x2
 DISC = 0x4
+NO_PARTICLE_SHUFFLE = 0x8
+NO_SET_SHUFFLE = 0x10
 DEBUG = 0x100
 
 _u32, _u64, _dbl, _vp, _sz = C.c_uint32, C.c_uint64, C.c_double, C.c_void_p, C.c_size_t
@@ -85,14 +87,16 @@ class Mpmc:
     """mpmc_* calls on torch CUDA tensors.  Same call list as the C ABI."""
 
     def __init__(self, N: int, box, sigma: float, d: float, n_s: int, seed: int, fp32: bool = False,
-                 debug: bool = False, w_target: float = 0.0, device="cuda:0", stream=None, disc: bool = False):
+                 debug: bool = False, w_target: float = 0.0, device="cuda:0", stream=None, disc: bool = False,
+                 particle_shuffle: bool = True, set_shuffle: bool = True):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1211_1646_b200 needs a CUDA device; there is no CPU fallback")
         self.torch = torch
         self.device = torch.device(device)
         self.N, self.fp32, self.debug, self.sigma = int(N), bool(fp32), bool(debug), float(sigma)
-        self.flags = (FP32 if fp32 else FP64) | (DEBUG if debug else 0) | (DISC if disc else 0)
+        self.flags = ((FP32 if fp32 else FP64) | (DEBUG if debug else 0) | (DISC if disc else 0)
+                      | (0 if particle_shuffle else NO_PARTICLE_SHUFFLE) | (0 if set_shuffle else NO_SET_SHUFFLE))
         nbytes = workspace_bytes(N, box, sigma, fp32, debug, w_target)
         if nbytes == 0:
             # let mpmc_create report the precise error code

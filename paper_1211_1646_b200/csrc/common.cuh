@@ -34,6 +34,7 @@ constexpr uint32_t SLOT_DIST = 0xFFFFFFFEu;     // shift distance
 constexpr uint32_t ERRBIT_OVERFLOW = 1u;  // a cell would hold more than NMAX disks
 constexpr uint32_t ERRBIT_RANGE = 2u;     // loaded coordinate NaN or outside [0, L]
 constexpr uint32_t ERRBIT_OVERLAP = 4u;   // loaded positions overlap
+constexpr uint32_t FLAG_NO_PARTICLE_SHUFFLE = 8u, FLAG_NO_SET_SHUFFLE = 16u;   // = MPMC_NO_* of mpmc.h
 constexpr uint32_t CTR_SLOTS = 64;        // rows of move counters (summed on read)
 constexpr uint32_t CROWD_CAP = 256;       // cells with more than 2 disks the tile kernel can carry per state
 
@@ -64,6 +65,7 @@ struct Params {
   uint32_t mx, my, hx, hy;   // cells; hx = mx/2, hy = my/2
   uint32_t Mq, Mqp;          // cells per colour; plane stride (Mq rounded up to 64)
   uint32_t n_s, N;
+  uint32_t flags;            // MPMC_* creation flags (the ablation switches are read on the device)
   uint32_t hx_magic, hx_sh1, hx_sh2;  // ci / hx without a divide (Granlund-Montgomery; host: div_magic)
   uint32_t tl_ntx, tl_nty, tl_PS;       // tile kernel: tiles per axis, shared-memory plane stride (cells)
   uint32_t seed_lo, seed_hi;
@@ -193,7 +195,7 @@ __device__ __forceinline__ Draws draw_sweep(const Params& p, unsigned long long 
   philox4x32_10(CELL_GLOBAL, (uint32_t)t, (uint32_t)(t >> 32), SLOT_ORDER, p.seed_lo, p.seed_hi, G);
   uint32_t o[4] = {0, 1, 2, 3};
 #pragma unroll
-  for (int i = 3; i >= 1; --i) {
+  for (int i = 3; i >= 1 && !(p.flags & FLAG_NO_SET_SHUFFLE); --i) {
     const uint32_t j = bounded(G[3 - i], (uint32_t)i + 1u);
     const uint32_t a = o[i];
     // o[j] with j dynamic: select chain keeps o[] in registers

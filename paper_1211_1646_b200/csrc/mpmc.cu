@@ -268,7 +268,7 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   c->stream = (cudaStream_t)cuda_stream;
   Params& p = c->p;
   p.mx = g.m[0]; p.my = g.m[1]; p.hx = g.m[0] / 2; p.hy = g.m[1] / 2;
-  p.Mq = L.Mq; p.Mqp = L.Mqp; p.n_s = n_s; p.N = (uint32_t)N;
+  p.Mq = L.Mq; p.Mqp = L.Mqp; p.n_s = n_s; p.N = (uint32_t)N; p.flags = flags;
   div_magic(p.hx, &p.hx_magic, &p.hx_sh1, &p.hx_sh2);
   p.seed_lo = (uint32_t)seed; p.seed_hi = (uint32_t)(seed >> 32);
   for (uint32_t r = 0; r < 10; ++r) { p.rk0[r] = p.seed_lo + r * 0x9E3779B9u; p.rk1[r] = p.seed_hi + r * 0xBB67AE85u; }

@@ -51,8 +51,9 @@ __device__ __forceinline__ void neighbour(const Where& w, int ox, int oy, uint32
 }
 
 // Fisher-Yates of the cell's n disks (Alg. 2 line 9, L187) as a visiting permutation packed in nibbles
-__device__ __forceinline__ uint32_t visiting_permutation(const uint32_t n, const uint32_t (&S)[4]) {
+__device__ __forceinline__ uint32_t visiting_permutation(const Params& p, const uint32_t n, const uint32_t (&S)[4]) {
   uint32_t perm = 0x3210u;
+  if (p.flags & FLAG_NO_PARTICLE_SHUFFLE) return perm;        // ablation (Table 1): slot order
 #pragma unroll
   for (int step = 0; step < NMAX - 1; ++step) {
     if ((uint32_t)step + 1u < n) {
@@ -83,7 +84,7 @@ __device__ __forceinline__ void cell_update_generic(const Params& p, const Where
   if (n >= 2u) {
     uint32_t S[4];
     philox4x32_10(w.cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
-    perm = visiting_permutation(n, S);
+    perm = visiting_permutation(p, n, S);
   }
   const uint32_t own = 2u * w.Q * Mqp + w.ci;           // half-0 index of the own cell
   uint32_t vi = 0;
@@ -219,7 +220,7 @@ __device__ __forceinline__ void update_cell_fast(const Params& p, const uint32_t
     if (two) {                           // n = 2: Fisher-Yates is one draw, j = bounded(S0, 2); j = 0 swaps
       uint32_t S[4];
       philox4x32_10(w.cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
-      flip = bounded(S[0], 2u) == 0u;
+      flip = bounded(S[0], 2u) == 0u && !(p.flags & FLAG_NO_PARTICLE_SHUFFLE);
     }
     if (flip) { P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }
 
@@ -345,7 +346,7 @@ __device__ __forceinline__ void cell_moves_general(const Params& p, const Half<P
     nqy[2 * e + 1] = R::pfma(h1[idx].y, MINUS1, R::pair(nsy, nsy));
   }
 
-  const uint32_t perm = visiting_permutation(n, S);    // Alg. 2 line 9 (L187)
+  const uint32_t perm = visiting_permutation(p, n, S);    // Alg. 2 line 9 (L187)
 
   // ---- n_s trial moves (Alg. 2 lines 11-32, L189-230) ----
   uint32_t vi = 0;

@@ -173,7 +173,7 @@ __device__ __noinline__ void tile_update_cell_warp(const Params& p, SmemCell<P>*
   if (n >= 2u) {                                                 // line 9 (L187)
     uint32_t S[4];
     philox4x32_10_rk(p, cell, t_lo, t_hi, SLOT_SHUFFLE, S);
-    perm = visiting_permutation(n, S);
+    perm = visiting_permutation(p, n, S);
   }
   uint32_t n_acc = 0, n_rb = 0, n_ro = 0, amask = 0, vi = 0;
   uint32_t Rw[4] = {0, 0, 0, 0};
@@ -265,7 +265,7 @@ __device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* s
   if (two) {                           // n = 2: Fisher-Yates is one draw, j = bounded(S0, 2); j = 0 swaps
     uint32_t S[4];
     philox4x32_10_rk(p, cell, t_lo, t_hi, SLOT_SHUFFLE, S);
-    flip = bounded(S[0], 2u) == 0u;
+    flip = bounded(S[0], 2u) == 0u && !(p.flags & FLAG_NO_PARTICLE_SHUFFLE);
   }
   if (flip) { P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }
   uint32_t amask = 0, bmask = 0;       // bit s: move s accepted / left the cell

@@ -28,6 +28,10 @@ def main():
     ap.add_argument("--blocks", type=int, default=10, help="blocks for the error estimate")
     ap.add_argument("--seed", type=int, default=1)
     ap.add_argument("--fp64", action="store_true")
+    ap.add_argument("--w-target", type=float, default=0.0, help="minimum cell width (1.40: the paper's regime, L152)")
+    ap.add_argument("--disc", action="store_true", help="disc-shaped displacement (the paper's, L190)")
+    ap.add_argument("--no-particle-shuffle", action="store_true", help="ablation of Table 1 (L134-142)")
+    ap.add_argument("--no-set-shuffle", action="store_true", help="ablation of Table 1 (L134-142)")
     args = ap.parse_args()
 
     import torch
@@ -35,7 +39,8 @@ def main():
     from .binding import Mpmc
     xy, box = I.jittered_lattice(args.n, args.phi, seed=args.seed)
     N = args.n * args.n
-    sim = Mpmc(N, box, 1.0, args.d, args.n_s, args.seed, fp32=not args.fp64, device="cuda:0")
+    sim = Mpmc(N, box, 1.0, args.d, args.n_s, args.seed, fp32=not args.fp64, device="cuda:0", w_target=args.w_target,
+               disc=args.disc, particle_shuffle=not args.no_particle_shuffle, set_shuffle=not args.no_set_shuffle)
     sim.load_positions(torch.as_tensor(xy, device="cuda:0"))
     dr, nbins, degree = 1e-4, 200, 5                      # L382
     t0 = time.time()
@@ -68,7 +73,8 @@ def main():
     p_blocks = np.array([p_star(h, per_block)[0] for h in hist_block])
     out = {
         "N": N, "phi": args.phi, "box": list(L), "cells": [sim.mx, sim.my], "d": args.d, "n_s": args.n_s,
-        "dtype": "f64" if args.fp64 else "f32", "equil_sweeps": args.equil, "sampled_sweeps": per_block * args.blocks * args.every,
+        "dtype": "f64" if args.fp64 else "f32", "w_target": args.w_target, "disc": args.disc,
+        "particle_shuffle": not args.no_particle_shuffle, "set_shuffle": not args.no_set_shuffle, "equil_sweeps": args.equil, "sampled_sweeps": per_block * args.blocks * args.every,
         "samples": per_block * args.blocks, "P_star": p_all, "g_contact": g_all,
         "P_star_block_mean": float(p_blocks.mean()), "P_star_stderr": float(p_blocks.std(ddof=1) / np.sqrt(args.blocks)),
         "P_star_blocks": [float(v) for v in p_blocks],

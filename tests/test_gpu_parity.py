@@ -21,10 +21,10 @@ def torch_cuda():
     return torch
 
 
-def make_pair(oracle_mod, torch, N, box, sigma, d, n_s, seed, fp32, xy, debug=True, w_target=0.0, disc=False):
+def make_pair(oracle_mod, torch, N, box, sigma, d, n_s, seed, fp32, xy, debug=True, w_target=0.0, disc=False, **ablate):
     from paper_1211_1646_b200.binding import Mpmc
-    o = oracle_mod.Oracle(N, box, sigma, d, n_s, seed, fp32=fp32, w_target=w_target, disc=disc)
-    g = Mpmc(N, box, sigma, d, n_s, seed, fp32=fp32, debug=debug, w_target=w_target, disc=disc)
+    o = oracle_mod.Oracle(N, box, sigma, d, n_s, seed, fp32=fp32, w_target=w_target, disc=disc, **ablate)
+    g = Mpmc(N, box, sigma, d, n_s, seed, fp32=fp32, debug=debug, w_target=w_target, disc=disc, **ablate)
     assert (g.mx, g.my) == (o.mx, o.my) and (g.wx, g.wy) == (o.wx, o.wy) and g.L_eff == o.L_eff
     o.load_positions(xy)
     g.load_positions(torch.as_tensor(xy, device="cuda"))
@@ -243,6 +243,17 @@ def test_four_slot_tile_kernel_uneven_tilings(oracle_mod, torch_cuda, n, phi, di
         o.sweep(k); g.sweep(k)
         assert_same_state(o, g, True)
     assert sum(g.path_sweeps()) == 10
+
+
+@pytest.mark.parametrize("pshuf,sshuf", [(False, True), (True, False), (False, False)])
+@pytest.mark.parametrize("w_target,n_s", [(0.0, 4), (1.40, 4), (1.40, 6)])      # 2-slot tile, 4-slot tile, general kernel
+def test_ablation_switches(oracle_mod, torch_cuda, pshuf, sshuf, w_target, n_s):
+    # PAPER.md section 2.4 / Table 1: particle shuffle and checkerboard-set shuffle switched off
+    xy, box = I.jittered_lattice(64, 0.66, seed=12)
+    o, g = make_pair(oracle_mod, torch_cuda, 4096, box, 1.0, 0.2, n_s, 3, True, xy, w_target=w_target,
+                     particle_shuffle=pshuf, set_shuffle=sshuf)
+    o.sweep(12); g.sweep(12)
+    assert_same_state(o, g, True)
 
 
 def test_disc_proposal_at_unit_cell_width(oracle_mod, torch_cuda):

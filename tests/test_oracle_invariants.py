@@ -220,3 +220,47 @@ def test_deterministic_and_seed_dependent(oracle_mod):
     for _ in range(5):
         o.sweep(1)
     assert np.array_equal(o.get_positions(), runs[0][0])
+
+
+# ---- ablation switches of PAPER.md section 2.4 / Table 1 (L114-142) -------------------------------------------------
+def test_without_particle_shuffle_the_first_move_acts_on_slot_zero(oracle_mod):
+    """Two disks in one cell, n_s = 1: without the particle shuffle (L187 left out) the single move of a sub-sweep always
+    acts on slot 0 = the lower id (slots ascend by id at load, A13); with it, slot 1 goes first about half the time."""
+    box, xy = (2.6, 2.6), np.array([[0.25, 0.30], [1.20, 1.25]])          # w = 1.3: both in cell (0, 0)
+    moved_second = {True: 0, False: 0}
+    for shuffle in (False, True):
+        for seed in range(200):
+            o = oracle_mod.Oracle(2, box, 1.0, 0.05, 1, seed, w_target=1.3, particle_shuffle=shuffle)
+            assert (o.mx, o.my) == (2, 2)
+            o.load_positions(xy)
+            o.sub_sweep(0)                                                    # set a holds cell (0, 0)
+            p = o.get_positions()
+            assert np.all(o.debug_state()["counts"].reshape(2, 2) == [[2, 0], [0, 0]])
+            if not np.array_equal(p[1], xy[1]):
+                moved_second[shuffle] += 1
+    assert moved_second[False] == 0
+    assert 50 < moved_second[True] < 150          # about half of the accepted first moves (acceptance < 1)
+
+
+def test_without_set_shuffle_the_sets_run_in_order_abcd(oracle_mod):
+    """set_shuffle = False: a sweep equals sub-sweeps a, b, c, d in that order followed by the drawn shift (composed from
+    the single-piece hooks); with the shuffle some sweep differs from that composition."""
+    xy, box = I.jittered_lattice(12, 0.55, seed=3)
+    differs = False
+    for shuffle in (False, True):
+        # compose sweep 0 by hand on a fresh copy
+        a = oracle_mod.Oracle(144, box, 1.0, 0.2, 4, 5, set_shuffle=shuffle)
+        b = oracle_mod.Oracle(144, box, 1.0, 0.2, 4, 5, set_shuffle=shuffle)
+        a.load_positions(xy); b.load_positions(xy)
+        a.sweep(1)
+        order, direction, word = oracle_mod.sweep_draws(5, 0)
+        for q in (0, 1, 2, 3):
+            b.sub_sweep(q)
+        w_axis = b.wx if direction < 2 else b.wy
+        b.shift(direction, (0.5 * w_axis) * (word * 2.0 ** -32))
+        same = np.array_equal(a.get_positions(), b.get_positions())
+        if shuffle:
+            differs |= (order != [0, 1, 2, 3]) and not same
+        else:
+            assert same
+    assert differs or oracle_mod.sweep_draws(5, 0)[0] == [0, 1, 2, 3]
