@@ -17,11 +17,16 @@
 // P.  Build with -ffp-contract=off so the compiler contracts nothing; the one FMA of the method (the
 // squared distance) is written std::fma.
 //
+// Options beside the default reading: the paper's disc-shaped displacement (OR_DISC, L190) and the two ablations of
+// Table 1 (OR_NO_PARTICLE_SHUFFLE, OR_NO_SET_SHUFFLE, L134-142).
+//
 // Pins (tests/test_oracle_*.py, all `-m "not gpu"`): Philox known answers; the visiting-order example
 // of PAPER.md L112; bookkeeping invariants (L152, L354); overlap-free configurations checked
 // independently in numpy; isolated-disk acceptance closed form; N=2 / N=3 sampling law (chi^2);
 // agreement with a separately written serial MC (Fig. 1); virial-series pressure;
-// the polynomial fit on the paper's model distribution (L382).  No function here is "parity unpinned".
+// the polynomial fit on the paper's model distribution (L382); for the disc proposal the isolated-disk closed form of
+// the disc, the displacement law and the two-disk law; for the ablations the slot-order and set-order behaviour.
+// No function here is "parity unpinned".
 
 #include <cmath>
 #include <cstdint>
