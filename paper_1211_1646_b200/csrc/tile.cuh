@@ -5,7 +5,9 @@
 // HALO = 5 cells into shared memory (slot pair 0 of every cell: 16 B in fp32), runs the four sub-sweeps there
 // with __syncthreads() between them — where separate kernels cost a dependent launch (~3.3 us measured) or a
 // grid barrier each — then performs the shift from shared memory straight into the other global buffer.  One
-// pass over HBM/L2 per sweep instead of six, neighbour loads at shared-memory latency.
+// pass over HBM/L2 per sweep instead of six, neighbour loads at shared-memory latency.  Within a phase the warps
+// draw chunks of cells from shared counters (dynamic balance); dilute systems use a variant that compacts the
+// non-empty cells into full warps.
 //
 // Halo recompute: sub-sweep k (k = 1..4) updates the cells of its colour whose ring index
 // (distance to the edge of the loaded region) is >= k (>= k + 1 on the three sides the shift does not pull from, see
@@ -20,8 +22,9 @@
 // Cells with more than 2 disks ("crowded"; about one in a million at phi = 0.716, w ~ sigma): shared memory holds
 // slot pair 0 only, where a slot is empty iff it holds the sentinel, so counts are implied.  The few crowded cells
 // of the state are listed in the control block (Ctl::clist, maintained by every kernel that writes cell counts);
-// a CTA copies those inside its region, with their slots 2 and 3, into a small shared-memory list, and a cell whose
-// 3x3 neighbourhood (or, in the shift, whose source neighbour) touches a listed cell takes a rolled general path.
+// a CTA copies those inside its region, with their slots 2 and 3, into a small shared-memory list; a cell whose 3x3
+// neighbourhood touches a listed cell is updated by a whole warp (tile_update_cell_warp), and in the shift a cell that is
+// listed or pulls from a listed cell goes through the eight-candidate routine (tile_shift_cell_general).
 // With more than CROWD_CAP crowded cells (Ctl::crowded) this kernel returns at once, and the general persistent
 // kernel (sweep.cuh k_sweeps), which mpmc_sweep always enqueues behind the tile kernels with the target sweep
 // index, runs the remaining sweeps.  The host only tiles boxes in which a loaded region never overlaps itself
