@@ -145,6 +145,18 @@ def test_c4_shape_reduced_and_ns8(oracle_mod, torch_cuda):
     assert_same_state(o, g, True)
 
 
+def test_c4_full_size_bit_exact(oracle_mod, torch_cuda):
+    """BASELINE config C4 at full size (N = 2^24, n_s = 8, fp32, 18.3 M cells, 2538 tiles in 18 waves), NO debug flag:
+    two sweeps against the oracle, state compared cell by cell."""
+    w = I.CONFIGS["C4"]
+    xy, box = I.workload_inputs(w)
+    o, g = make_pair(oracle_mod, torch_cuda, w.N, box, w.sigma, w.d, w.n_s, w.seed, True, xy, debug=False)
+    assert (g.mx, g.my) == (4596, 3980)
+    o.sweep(2); g.sweep(2)
+    st = assert_same_state(o, g, True, check_mask=False)
+    assert st["counts"].sum() == w.N and g.path_sweeps() == (2, 0)
+
+
 def test_c5_dilute_fluid_with_three_per_cell(oracle_mod, torch_cuda):
     # C5's parameters (phi 0.30, d 0.5, w = sigma) on 256^2 disks; melted by the ORACLE (reading A15), then
     # both sides run from the melted configuration.
