@@ -38,6 +38,10 @@ namespace mpmc {
 // threads per CTA, one CTA per SM: 24 warps at <= 85 registers (fp32), 12 warps at <= 170 registers (fp64)
 template <typename P> struct TileThreads { static constexpr int value = sizeof(P) == 4 ? 768 : 384; };
 constexpr int HALO = 5;
+#ifndef MPMC_SHIFT_U
+#define MPMC_SHIFT_U 4
+#endif
+constexpr int SHIFT_U = MPMC_SHIFT_U;   // cells per lane and chunk in the shift (their id loads are in flight together)
 
 // v in [-m, 2m) -> [0, m)
 __device__ __forceinline__ uint32_t wrap_cell(int v, uint32_t m) {
@@ -497,14 +501,14 @@ __device__ __forceinline__ void tile_shift_cells(const Params& p, const SmemCell
     const int hn = ALONG_X ? (int)p.hx : (int)p.hy;                  // half-cells along the shift axis
     for (;;) {
       uint32_t base = 0;
-      if (lane == 0u) base = atomicAdd(&next[q], 64u);
+      if (lane == 0u) base = atomicAdd(&next[q], 32u * SHIFT_U);
       base = __shfl_sync(0xFFFFFFFFu, base, 0);
       if (base >= per_plane) break;
-      uint32_t si[2], sn[2], own[2], nbg[2], cell[2];
-      bool ok[2], general[2];
-      uint2 ia[2], ib[2];
+      uint32_t si[SHIFT_U], sn[SHIFT_U], own[SHIFT_U], nbg[SHIFT_U], cell[SHIFT_U];
+      bool ok[SHIFT_U], general[SHIFT_U];
+      uint2 ia[SHIFT_U], ib[SHIFT_U];
 #pragma unroll
-      for (int u = 0; u < 2; ++u) {
+      for (int u = 0; u < SHIFT_U; ++u) {
         const uint32_t idx = base + lane + 32u * (uint32_t)u;
         ok[u] = idx < per_plane;
         const uint32_t id2 = ok[u] ? idx : 0u;
@@ -522,7 +526,7 @@ __device__ __forceinline__ void tile_shift_cells(const Params& p, const SmemCell
         if (ok[u] && !general[u]) { ia[u] = idsc[own[u]]; ib[u] = idsc[nbg[u]]; }
       }
 #pragma unroll
-      for (int u = 0; u < 2; ++u) {
+      for (int u = 0; u < SHIFT_U; ++u) {
         if (!ok[u]) continue;
         const uint32_t cnt_g = own[u] - Qg * Mqp;                      // Qg*Mqp + cig
         if (general[u]) continue;                                      // done above
