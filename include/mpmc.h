@@ -47,7 +47,8 @@ typedef struct mpmc_ctx mpmc_ctx; /* opaque host object; owns no device memory *
 #define MPMC_FP64 0x1u  /* local coordinates and all move arithmetic in double */
 #define MPMC_FP32 0x2u  /* ... in float (the paper's benchmarks, L390); pressure histogram still in double */
 #define MPMC_DISC 0x4u   /* trial moves uniform in the DISC of radius d (the paper's rng.inCircle(d), L190) instead of the
-                           square [-d, d]^2 of reading A2; runs on the general kernel */
+                           square [-d, d]^2 of reading A2; runs on the 4-slot fused tile kernel for n_s = 4, otherwise on
+                           the general persistent kernel */
 /* ablations of PAPER.md section 2.4 / Table 1 (L114-142); both leave the chain valid only in the sense the paper discusses */
 #define MPMC_NO_PARTICLE_SHUFFLE 0x8u  /* visit the disks of a cell in slot order (the paper shows a pressure bias) */
 #define MPMC_NO_SET_SHUFFLE 0x10u     /* run the checkerboard sets in the fixed order a, b, c, d (harmless per the paper) */
@@ -107,6 +108,8 @@ int mpmc_pressure_contact(mpmc_ctx* ctx, double dr, uint32_t nbins, uint32_t deg
 
 /* Test hooks: single pieces of Algorithm 1 at the current sweep index (do not advance it). */
 int mpmc_debug_sub_sweep(mpmc_ctx* ctx, uint32_t checkerboard_set /*0=a(0,0) 1=b(1,0) 2=c(0,1) 3=d(1,1)*/);
+/* delta in [0, w) of the chosen axis (Algorithm 1 draws it from [0, w/2), L90; the pull form of Algorithm 4 takes
+ * entrants from one neighbour only, so a larger delta is MPMC_ERR_ARG). */
 int mpmc_debug_shift(mpmc_ctx* ctx, uint32_t direction /*0:+x 1:-x 2:+y 3:-y*/, double delta);
 
 /* Test hook: the state in a layout-independent canonical form, cell c = y*mx + x.  Device out-pointers (any may
@@ -121,6 +124,13 @@ int mpmc_debug_state(mpmc_ctx* ctx, void* counts, void* slab, void* ids, void* a
  * the last load (the tile kernel serves cell widths w ~ sigma and hands a sweep to the general
  * kernel only when more cells hold 3 or 4 disks than it can carry).  Synchronises. */
 int mpmc_debug_path(mpmc_ctx* ctx, uint64_t out[2]);
+
+/* Test hook (host values only): how mpmc_sweep will run this context.  out = host, {slots per cell of the fused tile
+ * kernel: 2 (tile.cuh, w ~ sigma), 4 (tile4.cuh) or 0 (no tile kernel: every sweep on the general persistent kernel);
+ * 1 if the tile kernel is the variant for dilute systems that compacts non-empty cells into full warps; tiles along x;
+ * tiles along y; threads per tile CTA; dynamic shared memory per tile CTA in bytes; CTAs of the general kernel; threads
+ * per CTA of the general kernel}. */
+int mpmc_debug_config(const mpmc_ctx* ctx, uint32_t out[8]);
 
 /* Test hook (pure host arithmetic, no device needed): the tiling the fused tile kernels would use for a grid of
  * 2 hx x 2 hy cells when a cell takes cell_bytes of shared memory, an SM offers smem_max bytes and the device has sms

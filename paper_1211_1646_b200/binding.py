@@ -36,6 +36,7 @@ SYMBOLS = {
     "mpmc_debug_shift": (C.c_int, [_vp, _u32, _dbl]),
     "mpmc_debug_state": (C.c_int, [_vp, _vp, _vp, _vp, _vp, C.POINTER(_dbl), C.POINTER(_u64), C.POINTER(_u64)]),
     "mpmc_debug_path": (C.c_int, [_vp, C.POINTER(_u64)]),
+    "mpmc_debug_config": (C.c_int, [_vp, C.POINTER(_u32)]),
     "mpmc_debug_tiling": (C.c_int, [_u32, _u32, C.c_size_t, C.c_size_t, _u32, C.POINTER(_u32)]),
     "mpmc_debug_philox": (C.c_int, [_vp, C.POINTER(_u32), _vp, _u32, _vp]),
     "mpmc_strerror": (C.c_char_p, [C.c_int]),
@@ -217,6 +218,13 @@ class Mpmc:
             _chk(lib().mpmc_debug_path(self._h, out))
             self._exit()
         return int(out[0]), int(out[1])
+
+    def config(self) -> dict:
+        """How mpmc_sweep runs this context (mpmc_debug_config; host values only)."""
+        out = (_u32 * 8)()
+        _chk(lib().mpmc_debug_config(self._h, out))
+        keys = ("tile_slots", "compact", "ntx", "nty", "tile_threads", "tile_smem", "general_grid", "general_threads")
+        return dict(zip(keys, (int(v) for v in out)))
 
     def debug_state(self) -> dict:
         t = self.torch

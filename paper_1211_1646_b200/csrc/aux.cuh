@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(AUX_THREADS) k_load_sort(const __grid_constant
   uint32_t n = p.cnt32[Q * p.Mqp + ci];
   if (n > (uint32_t)NMAX) n = NMAX;
   cnt_plane(p, 0, Q)[ci] = (uint8_t)n;
-  if (n > 2u) {                                  // crowded cell of the state at sweep 0 (tile.cuh)
+  if (n > 2u && p.track_crowded) {               // crowded cell of the state at sweep 0 (tile.cuh)
     const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
     note_crowded(p.ctl, 0u, (2u * ya + (Q >> 1)) * p.mx + (2u * xa + (Q & 1u)));
   }

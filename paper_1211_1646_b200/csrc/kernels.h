@@ -1,0 +1,19 @@
+// kernels.h — the per-sweep kernels are compiled in translation units of their own (one per kernel family and
+// precision, so the library builds in parallel); the host code in mpmc.cu picks an instantiation through these.
+#pragma once
+#include <stdint.h>
+
+namespace mpmc {
+
+// k_sweeps<P, NS, DEBUG, FAST, DISC> (sweep.cuh): fast = the w ~ sigma cell update (occupancy 0/1/2, compile-time
+// n_s in {4, 8}); otherwise the general one
+const void* pick_kernel_f32(bool debug, bool fast, bool disc, uint32_t n_s);
+const void* pick_kernel_f64(bool debug, bool fast, bool disc, uint32_t n_s);
+// k_tile_sweep<P, NS, DEBUG, COMPACT> (tile.cuh); nullptr if there is no instantiation for n_s
+const void* pick_tile_kernel_f32(bool debug, uint32_t n_s, bool compact);
+const void* pick_tile_kernel_f64(bool debug, uint32_t n_s, bool compact);
+// k_tile4_sweep<P, 4, DEBUG, DISC> (tile4.cuh); nullptr unless n_s = 4
+const void* pick_tile4_kernel_f32(bool debug, bool disc, uint32_t n_s);
+const void* pick_tile4_kernel_f64(bool debug, bool disc, uint32_t n_s);
+
+}  // namespace mpmc

@@ -14,6 +14,7 @@
 #include "sweep.cuh"
 #include "tile.cuh"
 #include "tile4.cuh"
+#include "kernels.h"
 
 using namespace mpmc;
 
@@ -30,6 +31,9 @@ struct mpmc_ctx {
   uint32_t tile_grid;      // tiles = CTAs of the tile kernel
   size_t tile_smem;        // its dynamic shared memory
   uint32_t tile_threads;   // threads per CTA of the tile kernel
+  bool tile_compact;       // ... in its variant for dilute systems (non-empty cells compacted into full warps)
+  bool tile_two_slot;      // the tile kernel is the 2-slot one (tile.cuh), which may hand a crowded state to the general kernel
+  uint32_t sms;            // SMs of the device
   uint64_t t_host;         // sweeps requested since the last load (the sweep index the device will reach)
   int sticky;
 };
@@ -114,51 +118,12 @@ int cuda_fail(cudaError_t e) {
 
 dim3 cell_grid(const mpmc_ctx* c, int threads) { return dim3((c->p.Mq + threads - 1) / threads, 4, 1); }
 
-// ---- the persistent sweep kernel ------------------------------------------------------------------------
-// fast = the w ~ sigma cell update (occupancy 0/1/2, compile-time n_s in {4, 8}); otherwise the general one
-template <typename P, bool DEBUG>
-const void* pick_kernel_t(bool fast, bool disc, uint32_t n_s) {
-  if (disc) {           // the paper's disc-shaped proposal: general cell update only
-    if (n_s == 4) return (const void*)k_sweeps<P, 4, DEBUG, false, true>;
-    return (const void*)k_sweeps<P, 0, DEBUG, false, true>;
-  }
-  if (fast && n_s == 4) return (const void*)k_sweeps<P, 4, DEBUG, true>;
-  if (fast && n_s == 8) return (const void*)k_sweeps<P, 8, DEBUG, true>;
-  if (n_s == 4) return (const void*)k_sweeps<P, 4, DEBUG, false>;
-  if (n_s == 8) return (const void*)k_sweeps<P, 8, DEBUG, false>;
-  return (const void*)k_sweeps<P, 0, DEBUG, false>;
-}
-const void* pick_kernel(bool fp32, bool debug, bool fast, bool disc, uint32_t n_s) {
-  if (fp32) return debug ? pick_kernel_t<float, true>(fast, disc, n_s) : pick_kernel_t<float, false>(fast, disc, n_s);
-  return debug ? pick_kernel_t<double, true>(fast, disc, n_s) : pick_kernel_t<double, false>(fast, disc, n_s);
-}
-
 // one cooperative launch: sweeps up to sweep index t_end, or one piece of a sweep (test hooks)
 int launch_sweeps(mpmc_ctx* c, unsigned long long t_end, uint32_t op, uint32_t arg, double delta) {
   CU(cudaMemsetAsync(&c->p.ctl->bar, 0, sizeof(uint32_t), c->stream));
   void* args[] = {(void*)&c->p, (void*)&t_end, (void*)&op, (void*)&arg, (void*)&delta};
   CU(cudaLaunchCooperativeKernel(c->kernel, dim3(c->grid), dim3(SUB_THREADS), args, 0, c->stream));
   return MPMC_OK;
-}
-
-const void* pick_tile_kernel(bool fp32, bool debug, uint32_t n_s, bool compact) {
-  // dilute systems (most cells empty): the variant that runs the cell update on compacted warps of non-empty cells
-  if (compact && fp32 && n_s == 4) return debug ? (const void*)k_tile_sweep<float, 4, true, true> : (const void*)k_tile_sweep<float, 4, false, true>;
-  if (n_s == 4) return fp32 ? (debug ? (const void*)k_tile_sweep<float, 4, true> : (const void*)k_tile_sweep<float, 4, false>)
-                            : (debug ? (const void*)k_tile_sweep<double, 4, true> : (const void*)k_tile_sweep<double, 4, false>);
-  if (n_s == 8) return fp32 ? (debug ? (const void*)k_tile_sweep<float, 8, true> : (const void*)k_tile_sweep<float, 8, false>)
-                            : (debug ? (const void*)k_tile_sweep<double, 8, true> : (const void*)k_tile_sweep<double, 8, false>);
-  return nullptr;
-}
-
-template <typename P, bool DEBUG>
-const void* pick_tile4_kernel_t(bool disc) {
-  return disc ? (const void*)k_tile4_sweep<P, 4, DEBUG, true> : (const void*)k_tile4_sweep<P, 4, DEBUG, false>;
-}
-const void* pick_tile4_kernel(bool fp32, bool debug, bool disc, uint32_t n_s) {
-  if (n_s != 4) return nullptr;
-  if (fp32) return debug ? pick_tile4_kernel_t<float, true>(disc) : pick_tile4_kernel_t<float, false>(disc);
-  return debug ? pick_tile4_kernel_t<double, true>(disc) : pick_tile4_kernel_t<double, false>(disc);
 }
 
 // Tiling of the tile kernel: ntx x nty tiles of (nearly) equal even size whose loaded region (tile + 2 HALO) fits
@@ -250,7 +215,6 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   if (!out || !box || N == 0 || N >= 0xFFFFFFFFull || !(sigma > 0) || !(d > 0) || n_s > 32 || !precision_ok(flags))
     return MPMC_ERR_ARG;
   const bool fp32 = (flags & MPMC_FP32) != 0, debug = (flags & MPMC_DEBUG) != 0, disc = (flags & MPMC_DISC) != 0;
-  if (disc && n_s > 0xFFFFu) return MPMC_ERR_ARG;
   Geom g;
   const int st = geometry(box, sigma, w_target, fp32, &g);
   if (st != MPMC_OK) return st;
@@ -294,7 +258,10 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   // path); general kernel in the paper's regime (w up to sqrt(2) sigma, L152).
   const double wmax = g.wp[0] > g.wp[1] ? g.wp[0] : g.wp[1];
   c->nf = (wmax < 1.15 * sigma) ? 2 : 4;
-  c->kernel = pick_kernel(fp32, debug, c->nf == 2 && (n_s == 4 || n_s == 8), disc, n_s);
+  {
+    const bool fast = c->nf == 2 && (n_s == 4 || n_s == 8);
+    c->kernel = fp32 ? pick_kernel_f32(debug, fast, disc, n_s) : pick_kernel_f64(debug, fast, disc, n_s);
+  }
   // grid of the persistent kernel: every block co-resident (cooperative launch), no more blocks than chunks
   int dev = 0, sms = 0, occ = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
@@ -302,42 +269,55 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
     cudaGetLastError(); delete c; return MPMC_ERR_CUDA;
   }
   const uint32_t chunks = (L.Mq + SUB_THREADS - 1) / SUB_THREADS;
+  c->sms = (uint32_t)sms;
   c->grid = (uint32_t)sms * (uint32_t)occ;
   if (c->grid > chunks) c->grid = chunks;
   // The fused tile kernels: tile.cuh (2 slots per cell in shared memory) where cells hold 0/1/2 disks (w < 1.15 sigma),
   // the square proposal and n_s in {4, 8}; otherwise tile4.cuh (all 4 slots; any width, both proposals) for n_s = 4.
-  c->tile_kernel = nullptr; c->tile_grid = 0; c->tile_smem = 0; c->t_host = 0;
+  c->tile_kernel = nullptr; c->tile_grid = 0; c->tile_smem = 0; c->t_host = 0; c->tile_compact = false; c->tile_threads = 0;
   const bool two_slot = c->nf == 2 && (n_s == 4 || n_s == 8) && !disc;
+  c->tile_two_slot = two_slot;
+  p.track_crowded = two_slot ? 1u : 0u;      // only the 2-slot tile kernel reads the list of crowded cells
   bool compact = (double)N < 0.6 * (double)p.mx * (double)p.my;          // fewer than 0.6 disks per cell
-  if (const char* e = std::getenv("MPMC_COMPACT")) compact = e[0] == '1';    // experiments
-  const void* tk = two_slot ? pick_tile_kernel(fp32, debug, n_s, compact) : pick_tile4_kernel(fp32, debug, disc, n_s);
+#ifdef MPMC_EXPERIMENT
+  if (const char* e = std::getenv("MPMC_COMPACT")) compact = e[0] == '1';
+#endif
+  const void* tk = two_slot ? (fp32 ? pick_tile_kernel_f32(debug, n_s, compact) : pick_tile_kernel_f64(debug, n_s, compact))
+                            : (fp32 ? pick_tile4_kernel_f32(debug, disc, n_s) : pick_tile4_kernel_f64(debug, disc, n_s));
   if (tk) {
     int smem_optin = 0;
     cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     const size_t cell_bytes = (fp32 ? sizeof(SmemCell<float>) : sizeof(SmemCell<double>)) * (two_slot ? 1 : 2);
     const size_t stat = (two_slot ? (fp32 ? sizeof(CrowdList<float>) : sizeof(CrowdList<double>)) : 0) + 256   // static shared memory
-                        + (two_slot && compact ? (TileThreads<float>::value / 32) * 64 * sizeof(uint16_t) : 0);
+                        + (two_slot && compact ? ((fp32 ? TileThreads<float>::value : TileThreads<double>::value) / 32) * 64 * sizeof(uint16_t) : 0);
     const size_t smem_max = (size_t)smem_optin > stat ? (size_t)smem_optin - stat : 0;
     uint32_t ntx = 0, nty = 0, PS = 0;
     c->tile_threads = two_slot ? (fp32 ? TileThreads<float>::value : TileThreads<double>::value)
                                : (fp32 ? Tile4Threads<float>::value : Tile4Threads<double>::value);
     bool have = choose_tiling(p.hx, p.hy, cell_bytes, smem_max, (uint32_t)sms, &ntx, &nty, &PS);
-    if (const char* e = std::getenv("MPMC_TILE")) {        // experiments: "ntx,nty,threads"
+#ifdef MPMC_EXPERIMENT
+    if (const char* e = std::getenv("MPMC_TILE")) {        // "ntx,nty,threads" (whole warps)
       unsigned a = 0, b = 0, th = 0;
-      if (std::sscanf(e, "%u,%u,%u", &a, &b, &th) == 3 && a && b && th && th <= c->tile_threads && a <= p.hx && b <= p.hy) {
+      if (std::sscanf(e, "%u,%u,%u", &a, &b, &th) == 3 && a && b && th >= 32 && th % 32 == 0 && th <= c->tile_threads && a <= p.hx && b <= p.hy) {
         const uint32_t pw = (2 * ((p.hx + a - 1) / a) + 2 * HALO) / 2, ph = (2 * ((p.hy + b - 1) / b) + 2 * HALO) / 2;
         if ((size_t)4 * pw * ph * cell_bytes <= smem_max) { ntx = a; nty = b; PS = pw * ph; c->tile_threads = th; have = true; }
       }
     }
+#endif
     if (have) {
       c->tile_kernel = tk;
       c->tile_grid = ntx * nty;
       c->tile_smem = (size_t)4 * PS * cell_bytes;
       p.tl_ntx = ntx; p.tl_nty = nty; p.tl_PS = PS;
-      if (std::getenv("MPMC_VERBOSE"))
-        std::fprintf(stderr, "[mpmc] tile kernel (%d slots): %u x %u tiles, plane stride %u cells, %zu B shared memory, grid %u x %u threads; general grid %u\n",
-                     two_slot ? 2 : 4, ntx, nty, PS, c->tile_smem, c->tile_grid, c->tile_threads, c->grid);
-      if (cudaFuncSetAttribute(c->tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tile_smem) != cudaSuccess) {
+      c->tile_compact = two_slot && compact;
+      // The attribute belongs to the kernel function, not to this context: set it to the most any tiling can ask for
+      // (the opt-in maximum minus the kernel's static shared memory), so that live contexts with different tilings
+      // of the same instantiation do not undo each other's setting.
+      cudaFuncAttributes fa;
+      if (cudaFuncGetAttributes(&fa, c->tile_kernel) != cudaSuccess ||
+          (size_t)smem_optin < fa.sharedSizeBytes + c->tile_smem ||
+          cudaFuncSetAttribute(c->tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               smem_optin - (int)fa.sharedSizeBytes) != cudaSuccess) {
         cudaGetLastError(); delete c; return MPMC_ERR_CUDA;
       }
     }
@@ -370,7 +350,7 @@ int mpmc_load_positions(mpmc_ctx* c, const double* xy) {
   c->loaded = false;
   c->sticky = MPMC_OK;
   c->t_host = 0;
-  k_reset<<<148 * 4, 256, 0, c->stream>>>(c->p);
+  k_reset<<<c->sms * 4, 256, 0, c->stream>>>(c->p);
   const dim3 gN((c->p.N + AUX_THREADS - 1) / AUX_THREADS), gC = cell_grid(c, AUX_THREADS);
   if (c->fp32) {
     k_load_bin<float><<<gN, AUX_THREADS, 0, c->stream>>>(c->p, xy);
@@ -394,13 +374,14 @@ int mpmc_sweep(mpmc_ctx* c, uint64_t k) {
   if (!c) return MPMC_ERR_ARG;
   if (!c->loaded) return MPMC_ERR_STATE;
   if (k == 0) return c->sticky;
-  c->t_host += k;
   if (c->tile_kernel) {
     // one tile-kernel launch per sweep; each returns at once if the state has become crowded (tile.cuh) ...
     // Programmatic dependent launch: the CTAs of sweep t+1 become resident as the SMs of sweep t free up and park at
     // griddepcontrol.wait until sweep t has completed and flushed, which hides the launch latency (~4 us of ~50).
-    // MPMC_PDL=0 in the environment turns it off (A/B timing).
-    static const bool pdl = [] { const char* e = std::getenv("MPMC_PDL"); return !(e && e[0] == '0'); }();
+    bool pdl = c->stream != nullptr;
+#ifdef MPMC_EXPERIMENT
+    if (const char* e = std::getenv("MPMC_PDL")) pdl = pdl && e[0] != '0';      // A/B timing
+#endif
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(c->tile_grid);
     cfg.blockDim = dim3(c->tile_threads);
@@ -408,12 +389,22 @@ int mpmc_sweep(mpmc_ctx* c, uint64_t k) {
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = (pdl && c->stream != nullptr) ? 1 : 0;
-    unsigned long long t = c->t_host - k;          // sweep index of each launch (kernel argument: uniform on the device)
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    unsigned long long t = c->t_host;              // sweep index of each launch (kernel argument: uniform on the device)
     void* args[] = {(void*)&c->p, (void*)&t};
-    for (uint64_t i = 0; i < k; ++i, ++t) CU(cudaLaunchKernelExC(&cfg, c->tile_kernel, args));
+    for (uint64_t i = 0; i < k; ++i, ++t) {
+      const cudaError_t e = cudaLaunchKernelExC(&cfg, c->tile_kernel, args);
+      if (e != cudaSuccess) {                      // the device stays at the sweeps launched so far
+        c->t_host += i;
+        return cuda_fail(e);
+      }
+    }
   }
-  // ... and the general kernel runs whatever is left up to the target sweep index (normally nothing)
+  c->t_host += k;
+  // ... and the general kernel runs whatever is left up to the target sweep index: everything without a tile kernel,
+  // normally nothing behind the 2-slot tile kernel (it hands over only a state with too many crowded cells), never
+  // anything behind the 4-slot tile kernel, which takes every state
+  if (c->tile_kernel && !c->tile_two_slot) return c->sticky;
   const int st = launch_sweeps(c, c->t_host, OP_SWEEPS, 0, 0.0);
   return st != MPMC_OK ? st : c->sticky;
 }
@@ -486,6 +477,8 @@ int mpmc_debug_sub_sweep(mpmc_ctx* c, uint32_t set) {
 
 int mpmc_debug_shift(mpmc_ctx* c, uint32_t direction, double delta) {
   if (!c || direction > 3 || !(delta >= 0)) return MPMC_ERR_ARG;
+  // Algorithm 1 draws delta from [0, w/2) (L90); the pull form takes entrants from ONE neighbour, so delta must stay below w
+  if (!(delta < (direction < 2 ? c->p.wx_d : c->p.wy_d))) return MPMC_ERR_ARG;
   if (!c->loaded) return MPMC_ERR_STATE;
   const int st = launch_sweeps(c, 0, OP_SHIFT, direction, delta);
   return st != MPMC_OK ? st : c->sticky;
@@ -519,6 +512,17 @@ int mpmc_debug_path(mpmc_ctx* c, uint64_t out[2]) {
   const int st = read_ctl(c, &h);
   out[0] = h.path_sweeps[0]; out[1] = h.path_sweeps[1];
   return st;
+}
+
+int mpmc_debug_config(const mpmc_ctx* c, uint32_t out[8]) {
+  if (!c || !out) return MPMC_ERR_ARG;
+  out[0] = c->tile_kernel ? (c->tile_two_slot ? 2u : 4u) : 0u;
+  out[1] = c->tile_kernel && c->tile_compact ? 1u : 0u;
+  out[2] = c->p.tl_ntx; out[3] = c->p.tl_nty;
+  out[4] = c->tile_kernel ? c->tile_threads : 0u;
+  out[5] = (uint32_t)c->tile_smem;
+  out[6] = c->grid; out[7] = (uint32_t)SUB_THREADS;
+  return MPMC_OK;
 }
 
 int mpmc_debug_tiling(uint32_t hx, uint32_t hy, size_t cell_bytes, size_t smem_max, uint32_t sms, uint32_t out[3]) {

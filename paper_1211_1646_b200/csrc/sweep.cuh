@@ -7,18 +7,9 @@
 
 namespace mpmc {
 
-#ifndef MPMC_SUB_THREADS
-#define MPMC_SUB_THREADS 128
-#endif
-#ifndef MPMC_SUB_MINB
-#define MPMC_SUB_MINB 1
-#endif
-#ifndef MPMC_FAST_MINB
-#define MPMC_FAST_MINB 6
-#endif
-constexpr int SUB_THREADS = MPMC_SUB_THREADS;
-constexpr int SUB_MINB = MPMC_SUB_MINB;      // minimum resident blocks per SM asked of ptxas (register cap)
-constexpr int FAST_MINB = MPMC_FAST_MINB;
+constexpr int SUB_THREADS = 128;
+constexpr int SUB_MINB = 1;                  // minimum resident blocks per SM asked of ptxas (register cap)
+constexpr int FAST_MINB = 6;
 constexpr int SHIFT_THREADS = 256;
 
 // ---------------------------------------------------------------------------------------------------------
@@ -643,7 +634,7 @@ __device__ __forceinline__ void shift_cell(const Params& p, Ctl* ctl, const uint
     }
   }
   if (nn > (uint32_t)NMAX) { atomicOr(&ctl->err, ERRBIT_OVERFLOW); nn = NMAX; }
-  if (nn > 2u) {                                 // crowded cell of the new state (tile.cuh)
+  if (nn > 2u && p.track_crowded) {              // crowded cell of the new state (read by the 2-slot tile kernel only)
     const uint32_t ya = div_hx(p, ci), xa = ci - ya * p.hx;
     note_crowded(ctl, crowd_slot, (2u * ya + offy) * p.mx + (2u * xa + offx));
   }

@@ -38,10 +38,7 @@ namespace mpmc {
 // threads per CTA, one CTA per SM: 24 warps at <= 85 registers (fp32), 12 warps at <= 170 registers (fp64)
 template <typename P> struct TileThreads { static constexpr int value = sizeof(P) == 4 ? 768 : 384; };
 constexpr int HALO = 5;
-#ifndef MPMC_SHIFT_U
-#define MPMC_SHIFT_U 4
-#endif
-constexpr int SHIFT_U = MPMC_SHIFT_U;   // cells per lane and chunk in the shift (their id loads are in flight together)
+constexpr int SHIFT_U = 4;              // cells per lane and chunk in the shift (their id loads are in flight together)
 
 // v in [-m, 2m) -> [0, m)
 __device__ __forceinline__ uint32_t wrap_cell(int v, uint32_t m) {

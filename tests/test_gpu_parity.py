@@ -137,12 +137,17 @@ def test_c3_debug_digest(oracle_mod, torch_cuda):
     assert_same_state(o, g, True)
 
 
-def test_c4_shape_reduced_and_ns8(oracle_mod, torch_cuda):
-    # C4's parameters (phi 0.720, d 0.06, n_s 8) on a 512^2 lattice the oracle finishes in seconds
-    xy, box = I.jittered_lattice(512, 0.720, seed=1)
-    o, g = make_pair(oracle_mod, torch_cuda, 512 * 512, box, 1.0, 0.06, 8, 1, True, xy)
+@pytest.mark.parametrize("fp32,n", [(True, 512), (False, 256)])
+def test_c4_shape_reduced_and_ns8(oracle_mod, torch_cuda, fp32, n):
+    # C4's parameters (phi 0.720, d 0.06, n_s 8) on a lattice the oracle finishes in seconds; both precisions
+    # (k_tile_sweep<float, 8> and k_tile_sweep<double, 8>)
+    xy, box = I.jittered_lattice(n, 0.720, seed=1)
+    o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.06, 8, 1, fp32, xy)
+    cfg = g.config()
+    assert cfg["tile_slots"] == 2 and cfg["compact"] == 0
     o.sweep(8); g.sweep(8)
-    assert_same_state(o, g, True)
+    assert_same_state(o, g, fp32)
+    assert g.path_sweeps() == (8, 0)
 
 
 def test_c4_full_size_bit_exact(oracle_mod, torch_cuda):
@@ -157,23 +162,66 @@ def test_c4_full_size_bit_exact(oracle_mod, torch_cuda):
     assert st["counts"].sum() == w.N and g.path_sweeps() == (2, 0)
 
 
-def test_c5_dilute_fluid_with_three_per_cell(oracle_mod, torch_cuda):
-    # C5's parameters (phi 0.30, d 0.5, w = sigma) on 256^2 disks; melted by the ORACLE (reading A15), then
-    # both sides run from the melted configuration.
-    n = 256
-    xy0, box = I.jittered_lattice(n, 0.30, seed=1)
-    pre = oracle_mod.Oracle(n * n, box, 1.0, 0.5, 4, 999, fp32=True)
+def melted_by_the_oracle(oracle_mod, n, phi, d, w_target=0.0, fp32=True):
+    """Reading A15: the method itself with a fixed preparation seed until attempted >= 100 N.  The ORACLE melts: no
+    oracle input ever comes from the CUDA path."""
+    xy0, box = I.jittered_lattice(n, phi, seed=1)
+    pre = oracle_mod.Oracle(n * n, box, 1.0, d, 4, 999, fp32=fp32, w_target=w_target)
     pre.load_positions(xy0)
     while pre.acceptance()[0] < 100 * n * n:
         pre.sweep(10)
-    xy = pre.get_positions()
+    return pre.get_positions(), box
+
+
+def test_c5_dilute_fluid_reduced(oracle_mod, torch_cuda):
+    # C5's parameters (phi 0.30, d 0.5, w = sigma) on 256^2 disks, 60 sweeps with the accept masks compared
+    n = 256
+    xy, box = melted_by_the_oracle(oracle_mod, n, 0.30, 0.5)
     o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.5, 4, 1, True, xy)
+    assert g.config()["compact"] == 1                  # the dilute-system variant of the tile kernel
     for _ in range(6):
         o.sweep(10); g.sweep(10)
         st = assert_same_state(o, g, True)
     assert st["counts"].max() >= 2 and (st["counts"] == 0).mean() > 0.5
+    assert g.path_sweeps() == (60, 0)
     att, acc, rb, ro = g.acceptance()
     assert rb / att > 0.3           # boundary-crossing rejections dominate at d = 0.5 (config C5)
+
+
+def test_c5_full_size(oracle_mod, torch_cuda):
+    """BASELINE config C5 at its configured size (N = 2^20, phi = 0.30, 1780 x 1540 cells), NO debug flag: the launch
+    configuration bench.py --workload C5 times (compacting variant of the tile kernel)."""
+    w = I.CONFIGS["C5"]
+    xy, box = melted_by_the_oracle(oracle_mod, w.n_side, w.phi, w.d)
+    o, g = make_pair(oracle_mod, torch_cuda, w.N, box, w.sigma, w.d, w.n_s, w.seed, True, xy, debug=False)
+    assert (g.mx, g.my) == (1780, 1540)
+    cfg = g.config()
+    assert cfg["tile_slots"] == 2 and cfg["compact"] == 1
+    o.sweep(10); g.sweep(10)
+    st = assert_same_state(o, g, True, check_mask=False)
+    assert g.path_sweeps() == (10, 0)
+    assert st["counts"].sum() == w.N and (st["counts"] == 0).mean() > 0.6 and st["counts"].max() >= 2
+    att, acc, rb, ro = g.acceptance()
+    assert rb / att > 0.3
+
+
+@pytest.mark.parametrize("fp32", [True, False])
+def test_dilute_fluid_with_three_per_cell(oracle_mod, torch_cuda, fp32):
+    # C5's density and displacement at a cell width just under 1.15 sigma: still the 2-slot tile kernel in its compacting
+    # variant (0.48 disks per cell), and cells with THREE disks do occur — compacted warps x the list of crowded cells
+    n = 256
+    xy, box = melted_by_the_oracle(oracle_mod, n, 0.30, 0.5, w_target=1.12, fp32=fp32)
+    o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.5, 4, 1, fp32, xy, w_target=1.12)
+    cfg = g.config()
+    assert cfg["tile_slots"] == 2 and cfg["compact"] == 1
+    seen3, sweeps_with3 = False, 0
+    for _ in range(8):
+        o.sweep(5); g.sweep(5)
+        st = assert_same_state(o, g, fp32)
+        has3 = st["counts"].max() >= 3
+        seen3 |= has3; sweeps_with3 += int(has3)
+    assert seen3 and sweeps_with3 >= 2
+    assert g.path_sweeps() == (40, 0)                  # the tile kernel carried the crowded cells itself
 
 
 @pytest.mark.parametrize("fp32", [False, True])
@@ -210,15 +258,28 @@ def test_tile_kernel_hands_over_when_too_many_cells_are_crowded(oracle_mod, torc
     assert general > 0 and most > 256
 
 
-@pytest.mark.parametrize("n,phi", [(14, 0.5), (24, 0.6), (50, 0.7), (98, 0.65)])
+@pytest.mark.parametrize("n,phi", [(14, 0.5), (24, 0.6), (50, 0.7), (98, 0.65),
+                                   (14, 0.3), (26, 0.38), (50, 0.33), (98, 0.4), (150, 0.25)])    # dilute: compacting variant
 def test_tile_kernel_uneven_tilings(oracle_mod, torch_cuda, n, phi):
     # box sizes that do not divide evenly into tiles (tiles of different widths, many tiny tiles, few large ones)
     xy, box = I.jittered_lattice(n, phi, seed=n)
-    o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.15, 4, n, True, xy)
+    o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.15 if phi >= 0.5 else 0.4, 4, n, True, xy)
+    cfg = g.config()
+    assert cfg["tile_slots"] == 2 and cfg["compact"] == (1 if n * n < 0.6 * g.M else 0) == (1 if phi < 0.5 else 0)
     for k in (1, 2, 7):
         o.sweep(k); g.sweep(k)
         assert_same_state(o, g, True)
-    assert sum(g.path_sweeps()) == 10
+    assert g.path_sweeps() == (10, 0)
+
+
+@pytest.mark.parametrize("n_s", [4, 8])
+def test_compacting_variant_fp64(oracle_mod, torch_cuda, n_s):
+    xy, box = I.jittered_lattice(60, 0.35, seed=8)
+    o, g = make_pair(oracle_mod, torch_cuda, 3600, box, 1.0, 0.4, n_s, 2, False, xy)
+    assert g.config()["compact"] == 1
+    o.sweep(12); g.sweep(12)
+    assert_same_state(o, g, False)
+    assert g.path_sweeps() == (12, 0)
 
 
 @pytest.mark.parametrize("fp32", [False, True])
@@ -309,6 +370,33 @@ def test_seed_and_high_sweep_words(oracle_mod, torch_cuda):
     assert_same_state(o, g, True)
 
 
+def test_two_live_contexts_with_different_tilings(oracle_mod, torch_cuda):
+    """Two contexts of the SAME kernel instantiation with different tilings and shared-memory sizes, sweeps interleaved:
+    the dynamic shared-memory limit is a property of the kernel function, so the second create must not undo the first."""
+    big = I.jittered_lattice(256, 0.70, seed=1)
+    small = I.jittered_lattice(32, 0.6, seed=4)
+    ob, gb = make_pair(oracle_mod, torch_cuda, 256 * 256, big[1], 1.0, 0.1, 4, 1, True, big[0])
+    os_, gs = make_pair(oracle_mod, torch_cuda, 1024, small[1], 1.0, 0.2, 4, 5, True, small[0])
+    assert gb.config()["tile_smem"] > 4 * gs.config()["tile_smem"] > 0
+    for k in (1, 3, 2):
+        gb.sweep(k); gs.sweep(k); ob.sweep(k); os_.sweep(k)
+        gs.sweep(1); gb.sweep(1); os_.sweep(1); ob.sweep(1)
+    assert_same_state(ob, gb, True)
+    assert_same_state(os_, gs, True)
+    assert gb.path_sweeps() == (9, 0) and gs.path_sweeps() == (9, 0)
+
+
+def test_debug_shift_rejects_a_shift_of_a_cell_width(oracle_mod, torch_cuda):
+    from paper_1211_1646_b200.binding import MpmcError
+    xy, box = I.jittered_lattice(32, 0.6, seed=4)
+    o, g = make_pair(oracle_mod, torch_cuda, 1024, box, 1.0, 0.2, 4, 5, True, xy)
+    with pytest.raises(MpmcError) as e:
+        g.shift(0, g.wx)               # the pull form takes entrants from one neighbour only: delta < w
+    assert e.value.code == -1
+    g.shift(0, 0.49 * g.wx); o.shift(0, 0.49 * o.wx)
+    assert_same_state(o, g, True)
+
+
 def test_errors_on_device(oracle_mod, torch_cuda):
     torch = torch_cuda
     from paper_1211_1646_b200.binding import Mpmc, MpmcError
@@ -353,7 +441,9 @@ def test_overlap_free_and_conserved_at_full_size(torch_cuda):
     assert (p >= 0).all() and (p < Le).all()
     tree = cKDTree(np.minimum(p, np.nextafter(Le, 0)), boxsize=Le)
     dmin = tree.query(p, k=2)[0][:, 1].min()
-    assert dmin >= 1.0 - 1e-4          # fp32 locals: two cells' frames differ by an ulp of w (~1e-7) at most
+    # fp32 locals: the overlap test is made in the mover's frame and two cells' frames differ by an ulp, so seen from
+    # the unpacked doubles r^2 >= sigma^2 (1 - 4 eps_P), eps_P = 2^-23
+    assert dmin >= math.sqrt(1.0 - 4 * float(np.finfo(np.float32).eps)) and dmin < 1.001
     st = g.debug_state()
     assert st["counts"].sum() == w.N and st["counts"].max() <= 4 and st["sweep"] == 200
     used = np.arange(4)[None, :] < st["counts"][:, None]

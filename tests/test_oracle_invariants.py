@@ -50,7 +50,7 @@ def test_c1_invariants_every_sweep(oracle_mod, fp32):
     assert (o.mx, o.my) == (86, 74)
     assert o.wx >= w.sigma and o.wy >= w.sigma
     o.load_positions(xy)
-    eps = 6e-8 if fp32 else 1.2e-16
+    eps = float(np.finfo(np.float32 if fp32 else np.float64).eps)     # r^2 >= sigma^2 (1 - 4 eps_P)
     got = o.get_positions()
     assert np.abs(periodic_delta(got, xy, o.L_eff)).max() < (2e-4 if fp32 else 1e-12)
     last = o.acceptance()
@@ -66,8 +66,23 @@ def test_c1_invariants_every_sweep(oracle_mod, fp32):
         last = a
         pos = o.get_positions()
         assert np.all(pos >= 0) and np.all(pos[:, 0] < o.L_eff[0]) and np.all(pos[:, 1] < o.L_eff[1])
-        assert min_pair_distance(pos, o.L_eff) >= w.sigma * (1 - 4 * eps) - (1e-4 if fp32 else 0)
+        # (the unpacked doubles carry their own rounding, ~1e-14 at X ~ 90, which only matters in fp64)
+        assert min_pair_distance(pos, o.L_eff) >= w.sigma * math.sqrt(1 - 4 * eps) - (0 if fp32 else 1e-12)
     assert last[1] > 0 and last[2] > 0 and last[3] > 0
+
+
+def test_dense_fp32_hard_core_within_four_eps(oracle_mod):
+    """The same pin where it bites: phi = 0.716 (config C3's density), fp32, where many pairs sit at r ~ sigma.  The
+    overlap test is made in the mover's cell frame in fp32; seen from unpacked double coordinates the frames of two
+    cells differ by an ulp, hence r^2 >= sigma^2 (1 - 4 eps_P) and not r >= sigma."""
+    xy, box = I.jittered_lattice(64, 0.716, seed=3)
+    o = oracle_mod.Oracle(4096, box, 1.0, 0.08, 4, 3, fp32=True)
+    o.load_positions(xy)
+    eps = float(np.finfo(np.float32).eps)
+    for _ in range(20):
+        o.sweep(5)
+        d = min_pair_distance(o.get_positions(), o.L_eff)
+        assert d >= math.sqrt(1 - 4 * eps) and d < 1.001          # close pairs do exist: the pin is not vacuous
 
 
 def test_attempted_counts_nonempty_active_cells(oracle_mod):
