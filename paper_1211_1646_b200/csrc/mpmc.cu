@@ -440,10 +440,30 @@ int mpmc_pressure_contact(mpmc_ctx* c, double dr, uint32_t nbins, uint32_t degre
   const double wmin = p.wx_d < p.wy_d ? p.wx_d : p.wy_d;
   const int Rc = (int)std::ceil(rmax / wmin);
   CU(cudaMemsetAsync(p.hist, 0, (size_t)nbins * 8, c->stream));
-  const dim3 gC = cell_grid(c, AUX_THREADS);
+  if (Rc > 120) return MPMC_ERR_ARG;                     // the range must stay within a few cells (offsets are packed in 8 bits)
+  // offsets of the half neighbourhood whose cells can hold a pair closer than rmax (radius 1 and 2: compile-time loops)
+  unsigned long long keep = 0;
+  const double rmax2 = rmax * rmax * 1.000001;
+  if (Rc <= 2)
+    for (int oy = 0; oy <= Rc; ++oy)
+      for (int ox = -Rc; ox <= Rc; ++ox) {
+        if (oy == 0 && ox <= 0) continue;
+        const int gi = (ox < 0 ? -ox : ox) - 1, gj = oy - 1;
+        const double gx = (gi > 0 ? gi : 0) * p.wx_d, gy = (gj > 0 ? gj : 0) * p.wy_d;
+        if (gx * gx + gy * gy < rmax2) keep |= 1ull << hist_offset_index(ox, oy, Rc);
+      }
   const size_t sh = (size_t)nbins * 4;
-  if (c->fp32) k_contact_hist<float><<<gC, AUX_THREADS, sh, c->stream>>>(p, dr, nbins, Rc);
-  else         k_contact_hist<double><<<gC, AUX_THREADS, sh, c->stream>>>(p, dr, nbins, Rc);
+  if (Rc <= 2) {                     // tiles staged in shared memory
+    const dim3 gT((p.mx + HT_W - 1) / HT_W, (p.my + HT_H - 1) / HT_H);
+#define MPMC_HIST(P, RC) k_contact_hist_tile<P, RC><<<gT, HT_THREADS, sh, c->stream>>>(p, dr, nbins, rmax, keep)
+    if (c->fp32) { if (Rc == 1) MPMC_HIST(float, 1); else MPMC_HIST(float, 2); }
+    else         { if (Rc == 1) MPMC_HIST(double, 1); else MPMC_HIST(double, 2); }
+#undef MPMC_HIST
+  } else {
+    const dim3 gC = cell_grid(c, HIST_THREADS);
+    if (c->fp32) k_contact_hist<float, 0><<<gC, HIST_THREADS, sh, c->stream>>>(p, dr, nbins, Rc, rmax, keep);
+    else         k_contact_hist<double, 0><<<gC, HIST_THREADS, sh, c->stream>>>(p, dr, nbins, Rc, rmax, keep);
+  }
   CU(cudaGetLastError());
   std::vector<uint64_t> H(nbins);
   CU(cudaMemcpyAsync(H.data(), p.hist, (size_t)nbins * 8, cudaMemcpyDeviceToHost, c->stream));

@@ -115,6 +115,38 @@ def test_c2_dense_fluid(oracle_mod, torch_cuda, fp32):
     assert np.array_equal(hg, o.contact_histogram(1e-4, 200))
 
 
+@pytest.mark.parametrize("fp32", [False, True])
+@pytest.mark.parametrize("w_target", [0.0, 1.12, 1.40])
+def test_contact_histogram_ranges(oracle_mod, torch_cuda, fp32, w_target):
+    """a4 on its own: neighbourhood radius 1 and 2 (tiles in shared memory) and 3, 4 (general kernel), cells with 0..4
+    disks, bins from the paper's 1e-4 sigma (L382) to coarse ones; counts identical to the oracle's."""
+    xy, box = I.jittered_lattice(64, 0.55, seed=21)
+    o, g = make_pair(oracle_mod, torch_cuda, 4096, box, 1.0, 0.3, 4, 6, fp32, xy, w_target=w_target)
+    o.sweep(30); g.sweep(30)
+    st = assert_same_state(o, g, fp32)
+    if w_target > 1.0:
+        assert st["counts"].max() >= 3
+    for dr, nbins in [(0.005, 20), (1e-4, 200), (0.0004, 1000), (0.01, 250), (0.001, 4096), (0.6, 3)]:
+        ho, hg = o.contact_histogram(dr, nbins), g.contact_histogram(dr, nbins)
+        assert np.array_equal(ho, hg), (dr, nbins, int(ho.sum()), int(hg.sum()))
+        assert ho.sum() > 0
+
+
+@pytest.mark.parametrize("N,box,xy", [
+    (2, (2.6, 2.9), [[0.5, 0.5], [1.8, 1.9]]),                 # mx = my = 2: every cell is met at several image offsets
+    (3, (4.3, 4.5), [[0.5, 0.5], [2.0, 2.0], [3.5, 0.9]]),
+    (5, (6.4, 3.3), [[0.4, 0.4], [1.6, 0.5], [2.9, 0.6], [4.3, 2.2], [5.5, 1.0]]),
+])
+@pytest.mark.parametrize("fp32", [False, True])
+def test_contact_histogram_of_tiny_boxes(oracle_mod, torch_cuda, N, box, xy, fp32):
+    xy = np.array(xy, dtype=np.float64)
+    o, g = make_pair(oracle_mod, torch_cuda, N, box, 1.0, 0.4, 4, 9, fp32, xy)
+    for _ in range(3):
+        o.sweep(7); g.sweep(7)
+        for dr, nbins in [(0.005, 20), (0.05, 20), (0.1, 25), (0.25, 20)]:    # radius 2, 2, 3-4, 5-6 cells: images of images
+            assert np.array_equal(o.contact_histogram(dr, nbins), g.contact_histogram(dr, nbins)), (dr, nbins)
+
+
 def test_c3_headline_config_bench_launch_configuration(oracle_mod, torch_cuda):
     """Full size N = 2^20, fp32, NO debug flag: exactly the kernels bench.py times."""
     w = I.CONFIGS["C3"]
@@ -127,6 +159,9 @@ def test_c3_headline_config_bench_launch_configuration(oracle_mod, torch_cuda):
     assert g.path_sweeps() == (12, 0)                  # the fused tile kernel did them all (crowded cells included)
     att = g.acceptance()[0]
     assert 11.5 * 4.0e6 < att < 12 * 4.2e6
+    # a4 at the headline size: C2's bins and the paper's (L382)
+    for dr, nbins in [(0.005, 20), (1e-4, 200)]:
+        assert np.array_equal(o.contact_histogram(dr, nbins), g.contact_histogram(dr, nbins))
 
 
 def test_c3_debug_digest(oracle_mod, torch_cuda):
