@@ -127,10 +127,18 @@ int mpmc_debug_path(mpmc_ctx* ctx, uint64_t out[2]);
 
 /* Test hook (host values only): how mpmc_sweep will run this context.  out = host, {slots per cell of the fused tile
  * kernel: 2 (tile.cuh, w ~ sigma), 4 (tile4.cuh) or 0 (no tile kernel: every sweep on the general persistent kernel);
- * 1 if the tile kernel is the variant for dilute systems that compacts non-empty cells into full warps; tiles along x;
+ * CTAs (= tiles) of the tile kernel; tiles along x;
  * tiles along y; threads per tile CTA; dynamic shared memory per tile CTA in bytes; CTAs of the general kernel; threads
  * per CTA of the general kernel}. */
 int mpmc_debug_config(const mpmc_ctx* ctx, uint32_t out[8]);
+
+/* Profiling hook.  A library built with -DMPMC_PHASE_CLOCKS (paper_1211_1646_b200/phase_clocks.py) makes the 2-slot tile
+ * kernel record a clock mark at each of its phase boundaries; this call copies the marks of the LAST launch to the host:
+ * out = host, max_tiles x *marks values, row = tile; value 0 of a row is the global nanosecond timer at the start of the
+ * tile's work, the others are SM cycle counters (clock64) at the ends of: wait for the previous sweep, load,
+ * sub-sweeps 1-4, shift, ticket.  *marks = values per row, 0 in an ordinary build (nothing is written
+ * to out).  MPMC_ERR_STATE unless the context runs the 2-slot tile kernel.  Synchronises. */
+int mpmc_debug_phase_clocks(mpmc_ctx* ctx, uint64_t* out, uint32_t max_tiles, uint32_t* marks);
 
 /* Test hook (pure host arithmetic, no device needed): the tiling the fused tile kernels would use for a grid of
  * 2 hx x 2 hy cells when a cell takes cell_bytes of shared memory, an SM offers smem_max bytes and the device has sms

@@ -37,6 +37,7 @@ SYMBOLS = {
     "mpmc_debug_state": (C.c_int, [_vp, _vp, _vp, _vp, _vp, C.POINTER(_dbl), C.POINTER(_u64), C.POINTER(_u64)]),
     "mpmc_debug_path": (C.c_int, [_vp, C.POINTER(_u64)]),
     "mpmc_debug_config": (C.c_int, [_vp, C.POINTER(_u32)]),
+    "mpmc_debug_phase_clocks": (C.c_int, [_vp, _vp, _u32, C.POINTER(_u32)]),
     "mpmc_debug_tiling": (C.c_int, [_u32, _u32, C.c_size_t, C.c_size_t, _u32, C.POINTER(_u32)]),
     "mpmc_debug_philox": (C.c_int, [_vp, C.POINTER(_u32), _vp, _u32, _vp]),
     "mpmc_strerror": (C.c_char_p, [C.c_int]),
@@ -223,8 +224,23 @@ class Mpmc:
         """How mpmc_sweep runs this context (mpmc_debug_config; host values only)."""
         out = (_u32 * 8)()
         _chk(lib().mpmc_debug_config(self._h, out))
-        keys = ("tile_slots", "compact", "ntx", "nty", "tile_threads", "tile_smem", "general_grid", "general_threads")
+        keys = ("tile_slots", "tiles", "ntx", "nty", "tile_threads", "tile_smem", "general_grid", "general_threads")
         return dict(zip(keys, (int(v) for v in out)))
+
+    def phase_clocks(self):
+        """(tiles, marks) uint64 array of the tile kernel's clock marks in its last launch; None unless the library was
+        built with -DMPMC_PHASE_CLOCKS (mpmc_debug_phase_clocks)."""
+        import numpy as np
+        tiles = self.config()["tiles"]
+        flat = np.zeros(max(tiles, 1) * 16, dtype=np.uint64)
+        marks = _u32()
+        with self.torch.cuda.device(self.device):
+            self._enter()
+            _chk(lib().mpmc_debug_phase_clocks(self._h, flat.ctypes.data, tiles, C.byref(marks)))
+            self._exit()
+        if marks.value == 0:
+            return None
+        return flat[: tiles * marks.value].reshape(tiles, marks.value)
 
     def debug_state(self) -> dict:
         t = self.torch

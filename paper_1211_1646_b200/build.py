@@ -45,6 +45,11 @@ def build(force: bool = False, verbose: bool = False, extra_flags=(), lib: str =
         return os.environ["MPMC_B200_LIB"]
     obj_dir = OBJ if lib == LIB else OBJ + "_" + os.path.basename(lib).replace(".so", "")
     os.makedirs(obj_dir, exist_ok=True)
+    stamp = os.path.join(obj_dir, "flags.txt")                # objects compiled with other flags are stale
+    flags_now = " ".join(NVCC_FLAGS + list(extra_flags))
+    if not os.path.exists(stamp) or open(stamp).read() != flags_now:
+        force = True
+        open(stamp, "w").write(flags_now)
 
     def compile_unit(unit):
         src, obj, defs = unit

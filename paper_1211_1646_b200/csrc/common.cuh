@@ -66,6 +66,7 @@ struct Params {
   uint32_t Mq, Mqp;          // cells per colour; plane stride (Mq rounded up to 64)
   uint32_t n_s, N;
   uint32_t flags;            // MPMC_* creation flags (the ablation switches are read on the device)
+  uint32_t tune;             // tuning word for experiments (builds with -DMPMC_EXPERIMENT read it from MPMC_TUNE); unused by default
   uint32_t track_crowded;    // 1: kernels that write cell counts list the cells with more than 2 disks (for tile.cuh)
   uint32_t hx_magic, hx_sh1, hx_sh2;  // ci / hx without a divide (Granlund-Montgomery; host: div_magic)
   uint32_t tl_ntx, tl_nty, tl_PS;       // tile kernel: tiles per axis, shared-memory plane stride (cells)

@@ -21,4 +21,17 @@ const void* pick(uint32_t n_s, bool compact) {
 const void* MPMC_CAT(pick_tile_kernel_, MPMC_SUFFIX)(bool debug, uint32_t n_s, bool compact) {
   return debug ? pick<MPMC_P, true>(n_s, compact) : pick<MPMC_P, false>(n_s, compact);
 }
+
+// -DMPMC_PHASE_CLOCKS: copy the phase marks of the last launch to the host (tiles x PHASE_MARKS values)
+int MPMC_CAT(phase_clocks_, MPMC_SUFFIX)(unsigned long long* out, uint32_t tiles, void* stream) {
+#ifdef MPMC_PHASE_CLOCKS
+  if (tiles > PHASE_TILES) tiles = PHASE_TILES;
+  if (cudaMemcpyFromSymbolAsync(out, g_phase_clocks, (size_t)tiles * PHASE_MARKS * 8, 0, cudaMemcpyDeviceToHost, (cudaStream_t)stream) != cudaSuccess) return -1;
+  if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) return -1;
+  return (int)PHASE_MARKS;
+#else
+  (void)out; (void)tiles; (void)stream;
+  return 0;
+#endif
+}
 }  // namespace mpmc

@@ -12,6 +12,10 @@ const void* pick_kernel_f64(bool debug, bool fast, bool disc, uint32_t n_s);
 // k_tile_sweep<P, NS, DEBUG, COMPACT> (tile.cuh); nullptr if there is no instantiation for n_s
 const void* pick_tile_kernel_f32(bool debug, uint32_t n_s, bool compact);
 const void* pick_tile_kernel_f64(bool debug, uint32_t n_s, bool compact);
+// builds with -DMPMC_PHASE_CLOCKS: the clock marks k_tile_sweep took at its phase boundaries in its last launch, copied to
+// the host (tiles x marks values); returns the number of marks per tile, 0 in an ordinary build, -1 on a CUDA error
+int phase_clocks_f32(unsigned long long* out, uint32_t tiles, void* stream);
+int phase_clocks_f64(unsigned long long* out, uint32_t tiles, void* stream);
 // k_tile4_sweep<P, 4, DEBUG, DISC> (tile4.cuh); nullptr unless n_s = 4
 const void* pick_tile4_kernel_f32(bool debug, bool disc, uint32_t n_s);
 const void* pick_tile4_kernel_f64(bool debug, bool disc, uint32_t n_s);

@@ -31,7 +31,6 @@ struct mpmc_ctx {
   uint32_t tile_grid;      // tiles = CTAs of the tile kernel
   size_t tile_smem;        // its dynamic shared memory
   uint32_t tile_threads;   // threads per CTA of the tile kernel
-  bool tile_compact;       // ... in its variant for dilute systems (non-empty cells compacted into full warps)
   bool tile_two_slot;      // the tile kernel is the 2-slot one (tile.cuh), which may hand a crowded state to the general kernel
   uint32_t sms;            // SMs of the device
   uint64_t t_host;         // sweeps requested since the last load (the sweep index the device will reach)
@@ -274,14 +273,17 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   if (c->grid > chunks) c->grid = chunks;
   // The fused tile kernels: tile.cuh (2 slots per cell in shared memory) where cells hold 0/1/2 disks (w < 1.15 sigma),
   // the square proposal and n_s in {4, 8}; otherwise tile4.cuh (all 4 slots; any width, both proposals) for n_s = 4.
-  c->tile_kernel = nullptr; c->tile_grid = 0; c->tile_smem = 0; c->t_host = 0; c->tile_compact = false; c->tile_threads = 0;
+  c->tile_kernel = nullptr; c->tile_grid = 0; c->tile_smem = 0; c->t_host = 0; c->tile_threads = 0;
   const bool two_slot = c->nf == 2 && (n_s == 4 || n_s == 8) && !disc;
   c->tile_two_slot = two_slot;
-  p.track_crowded = two_slot ? 1u : 0u;      // only the 2-slot tile kernel reads the list of crowded cells
-  bool compact = (double)N < 0.6 * (double)p.mx * (double)p.my;          // fewer than 0.6 disks per cell
+  p.tune = 0u;
+  // dilute systems (fewer than 0.6 disks per cell): the tile kernel variant that compacts the non-empty cells
+  bool compact = (double)N < 0.6 * (double)p.mx * (double)p.my;
 #ifdef MPMC_EXPERIMENT
+  if (const char* e = std::getenv("MPMC_TUNE")) p.tune = (uint32_t)std::strtoul(e, nullptr, 0);
   if (const char* e = std::getenv("MPMC_COMPACT")) compact = e[0] == '1';
 #endif
+  p.track_crowded = two_slot ? 1u : 0u;      // only the 2-slot tile kernel reads the list of crowded cells
   const void* tk = two_slot ? (fp32 ? pick_tile_kernel_f32(debug, n_s, compact) : pick_tile_kernel_f64(debug, n_s, compact))
                             : (fp32 ? pick_tile4_kernel_f32(debug, disc, n_s) : pick_tile4_kernel_f64(debug, disc, n_s));
   if (tk) {
@@ -309,7 +311,6 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
       c->tile_grid = ntx * nty;
       c->tile_smem = (size_t)4 * PS * cell_bytes;
       p.tl_ntx = ntx; p.tl_nty = nty; p.tl_PS = PS;
-      c->tile_compact = two_slot && compact;
       // The attribute belongs to the kernel function, not to this context: set it to the most any tiling can ask for
       // (the opt-in maximum minus the kernel's static shared memory), so that live contexts with different tilings
       // of the same instantiation do not undo each other's setting.
@@ -537,11 +538,22 @@ int mpmc_debug_path(mpmc_ctx* c, uint64_t out[2]) {
 int mpmc_debug_config(const mpmc_ctx* c, uint32_t out[8]) {
   if (!c || !out) return MPMC_ERR_ARG;
   out[0] = c->tile_kernel ? (c->tile_two_slot ? 2u : 4u) : 0u;
-  out[1] = c->tile_kernel && c->tile_compact ? 1u : 0u;
+  out[1] = c->tile_kernel ? c->tile_grid : 0u;
   out[2] = c->p.tl_ntx; out[3] = c->p.tl_nty;
   out[4] = c->tile_kernel ? c->tile_threads : 0u;
   out[5] = (uint32_t)c->tile_smem;
   out[6] = c->grid; out[7] = (uint32_t)SUB_THREADS;
+  return MPMC_OK;
+}
+
+int mpmc_debug_phase_clocks(mpmc_ctx* c, uint64_t* out, uint32_t max_tiles, uint32_t* marks) {
+  if (!c || !out || !marks) return MPMC_ERR_ARG;
+  if (!c->loaded || !c->tile_kernel || !c->tile_two_slot) return MPMC_ERR_STATE;
+  const uint32_t tiles = c->tile_grid < max_tiles ? c->tile_grid : max_tiles;
+  static_assert(sizeof(unsigned long long) == sizeof(uint64_t), "");
+  const int m = c->fp32 ? phase_clocks_f32((unsigned long long*)out, tiles, c->stream) : phase_clocks_f64((unsigned long long*)out, tiles, c->stream);
+  if (m < 0) return MPMC_ERR_CUDA;
+  *marks = (uint32_t)m;
   return MPMC_OK;
 }
 

@@ -63,6 +63,18 @@ __device__ __forceinline__ void sts_half(SmemCell<double>* s, uint32_t i, const 
   s[i].a = make_double2(h.x.x, h.x.y); s[i].b = make_double2(h.y.x, h.y.y);
 }
 
+// asynchronous copy of one cell (slot pair i of the global planes) into shared memory, 16 bytes per cp.async, past L1
+__device__ __forceinline__ void cp_async_cell(SmemCell<float>* dst, const float* pos, uint32_t i) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(d), "l"(reinterpret_cast<const float4*>(pos) + i) : "memory");
+}
+__device__ __forceinline__ void cp_async_cell(SmemCell<double>* dst, const double* pos, uint32_t i) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst);
+  const double2* src = reinterpret_cast<const double2*>(pos) + 2 * (size_t)i;
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(d), "l"(src) : "memory");
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(d + 16u), "l"(src + 1) : "memory");
+}
+
 __device__ __forceinline__ float lds_x0(const SmemCell<float>* s, uint32_t i) { return s[i].v.x; }     // x of slot 0
 __device__ __forceinline__ double lds_x0(const SmemCell<double>* s, uint32_t i) { return s[i].a.x; }
 
@@ -548,6 +560,23 @@ __device__ __forceinline__ void tile_shift_cells(const Params& p, const SmemCell
 // The fused sweep kernel: one CTA per tile, one launch per sweep.  See the header of this file.
 // Dynamic shared memory: 4 planes x tl_PS cells x sizeof(SmemCell<P>).
 // ---------------------------------------------------------------------------------------------------------
+// -DMPMC_PHASE_CLOCKS builds a variant that records clock64() at every phase boundary (phase_clocks.py).
+#ifdef MPMC_PHASE_CLOCKS
+constexpr uint32_t PHASE_TILES = 4096, PHASE_MARKS = 9;
+__device__ unsigned long long g_phase_clocks[PHASE_TILES][PHASE_MARKS];
+__device__ __forceinline__ unsigned long long globaltimer_ns() { unsigned long long v; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(v)); return v; }
+// (the clock is read AFTER a shared-memory load that follows the barrier: a bare clock read right behind __syncthreads is
+// issued before the barrier releases and would record this warp's arrival instead)
+__device__ __forceinline__ unsigned long long clock_after(const volatile uint32_t* s) {
+  const uint32_t v = *s; unsigned long long c;
+  asm volatile("mov.u64 %0, %%clock64;" : "=l"(c) : "r"(v) : "memory");
+  return c;
+}
+#define MPMC_PHASE_MARK(i) do { if (threadIdx.x == 0 && blockIdx.x < PHASE_TILES) g_phase_clocks[blockIdx.x][i] = (i) == 0 ? globaltimer_ns() : clock_after(&s_last); } while (0)
+#else
+#define MPMC_PHASE_MARK(i) do { } while (0)
+#endif
+
 template <typename P, int NS, bool DEBUG, bool COMPACT = false>
 __global__ void __launch_bounds__(TileThreads<P>::value, 1)
 k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
@@ -570,6 +599,7 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   if (ctl->t != t) return;
   const uint32_t slot = (uint32_t)(t & 3u), slot1 = (uint32_t)((t + 1ull) & 3u), slot2 = (uint32_t)((t + 2ull) & 3u);
   if (ctl->crowded[slot] != 0u) return;          // too many crowded cells: the general kernel takes over
+  MPMC_PHASE_MARK(0); MPMC_PHASE_MARK(1);
   const uint32_t cur = ctl->cur, nxt = cur ^ 1u;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   const uint32_t ty = blockIdx.x / p.tl_ntx, tx = blockIdx.x - ty * p.tl_ntx;
@@ -583,38 +613,19 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   }
   __syncthreads();
 
-  // ---- load the tile and its halo: warps take plane rows, lanes run along the row (512 contiguous bytes) ----
+  // ---- load the tile and its halo: warps take plane rows, lanes run along the row (512 contiguous bytes).  Asynchronous
+  //      copies global -> shared (cp.async, 16 bytes each): no register staging, so every copy of a thread (13 at C3) is
+  //      in flight at once; the phase then runs at the L2 -> SM bandwidth all SMs share (measured 6 TB/s) ----
   {
     const P* posc = reinterpret_cast<const P*>(p.pos[cur]);
-    // four plane rows x two 32-cell column blocks per warp and pass: eight independent loads in flight per lane
-    // before the first shared-memory store (a load -> store chain per row would expose the L2 latency every time)
-    const uint32_t NW = TILE_THREADS / 32;
-    const uint32_t nrows = 4u * ph, inv_ph = small_div_magic(ph);
-    for (uint32_t c0 = 0; c0 < pw; c0 += 64u) {
-      for (uint32_t r0 = warp; r0 < nrows; r0 += 4u * NW) {
-        Half<P> v[4][2];
-        uint32_t sidx[4][2];
-        bool ok[4][2];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const uint32_t r = r0 + (uint32_t)j * NW, rr = r < nrows ? r : 0u;
-          const uint32_t q = small_div(rr, inv_ph), py = rr - q * ph;
-          const uint32_t gy = wrap_cell(gy0 + (int)(2u * py + (q >> 1)), p.my);
-          const uint32_t gbase = 2u * ((gy & 1u) << 1) * Mqp + (gy >> 1) * p.hx, sbase = q * PS + py * pw;
-#pragma unroll
-          for (int c = 0; c < 2; ++c) {
-            const uint32_t px = c0 + lane + 32u * (uint32_t)c;
-            ok[j][c] = r < nrows && px < pw;
-            const uint32_t gx = wrap_cell(gx0 + (int)(2u * (ok[j][c] ? px : 0u) + (q & 1u)), p.mx);
-            sidx[j][c] = sbase + px;
-            if (ok[j][c]) v[j][c] = ld_half(posc, gbase + 2u * (gx & 1u) * Mqp + (gx >> 1));
-          }
-        }
-#pragma unroll
-        for (int j = 0; j < 4; ++j)
-#pragma unroll
-          for (int c = 0; c < 2; ++c)
-            if (ok[j][c]) sts_half(sm, sidx[j][c], v[j][c]);
+    const uint32_t nrows = 4u * ph, inv_ph = small_div_magic(ph), NW = TILE_THREADS / 32;
+    for (uint32_t r = warp; r < nrows; r += NW) {
+      const uint32_t q = small_div(r, inv_ph), py = r - q * ph;
+      const uint32_t gy = wrap_cell(gy0 + (int)(2u * py + (q >> 1)), p.my);
+      const uint32_t gbase = 2u * ((gy & 1u) << 1) * Mqp + (gy >> 1) * p.hx, sbase = q * PS + py * pw;
+      for (uint32_t px = lane; px < pw; px += 32u) {
+        const uint32_t gx = wrap_cell(gx0 + (int)(2u * px + (q & 1u)), p.mx);
+        cp_async_cell(sm + sbase + px, posc, gbase + 2u * (gx & 1u) * Mqp + (gx >> 1));
       }
     }
     // the crowded cells of this state that lie in the region, with their slots 2 and 3
@@ -630,8 +641,10 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
         cl.e[e].hi = ld_half(posc, (2u * (((gy & 1u) << 1) | (gx & 1u)) + 1u) * Mqp + (gy >> 1) * p.hx + (gx >> 1));
       }
     }
+    asm volatile("cp.async.wait_all;" ::: "memory");
   }
   __syncthreads();
+  MPMC_PHASE_MARK(2);
   const uint32_t nc = cl.n;
   Tally tally;
 
@@ -677,6 +690,7 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
       }
     }
     __syncthreads();
+    MPMC_PHASE_MARK(2 + k);
   }
 
   // ---- cell shift (Alg. 1 lines 15-17; Algorithm 4) of the interior cells, shared memory -> other buffer ----
@@ -690,10 +704,9 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   // ---- counters; the last CTA to finish advances the control block ----
   flush_tally(p, tally);
   __syncthreads();
-  if (tid == 0) {
-    __threadfence();
-    s_last = (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1u) ? 1u : 0u;
-  }
+  MPMC_PHASE_MARK(7);
+  // (no fence: nothing written here is read before the launch completes, and the next launch waits for that)
+  if (tid == 0) s_last = (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1u) ? 1u : 0u;
   __syncthreads();
   if (s_last && tid == 0) {
     const double L = along_x ? p.Lx_eff : p.Ly_eff;
@@ -707,6 +720,7 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
     ctl->t = t + 1ull;
     ctl->path_sweeps[0] += 1ull;
   }
+  MPMC_PHASE_MARK(8);
 }
 
 }  // namespace mpmc

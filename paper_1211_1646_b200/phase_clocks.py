@@ -1,0 +1,64 @@
+"""Per-phase cycle counts of the fused tile kernel (k_tile_sweep), from clock64() marks at its phase boundaries.
+
+    python -m paper_1211_1646_b200.phase_clocks [--workload C3] [--sweeps 200]
+
+Builds an instrumented copy of the library (-DMPMC_PHASE_CLOCKS, its own .so; the shipped library carries no marks),
+runs the workload on cuda:0 and prints, over the tiles of the last few sweeps, the mean and the maximum number of SM
+cycles each phase took.  The figures quoted in profiles/*ncu_full.md come from this script.
+"""
+from __future__ import annotations
+
+import argparse
+import os
+
+import numpy as np
+
+PHASES = ["wait for the previous sweep", "load tile + halo", "sub-sweep 1", "sub-sweep 2", "sub-sweep 3", "sub-sweep 4",
+          "shift + counters", "ticket"]
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--workload", default="C3")
+    ap.add_argument("--sweeps", type=int, default=200)
+    ap.add_argument("--samples", type=int, default=20, help="launches whose marks are read")
+    ap.add_argument("--dump", default="", help="write the per-tile mean cycles of every phase to this .npy file")
+    ap.add_argument("--define", action="append", default=[], help="extra -D for the instrumented build (experiments)")
+    ap.add_argument("--burst", type=int, default=10, help="back-to-back sweeps before each read (the last one's marks are read)")
+    args = ap.parse_args()
+    from . import build
+    lib = os.path.join(build.HERE, "libmpmc_b200_phase_clocks.so")
+    build.build(extra_flags=["-DMPMC_PHASE_CLOCKS"] + [f"-D{d}" for d in args.define], lib=lib)
+    os.environ["MPMC_B200_LIB"] = lib
+    import torch
+    from . import inputs as I
+    from .binding import Mpmc
+    w = I.CONFIGS[args.workload]
+    xy, box = I.workload_inputs(w)
+    g = Mpmc(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=w.fp32, w_target=w.w_target, disc=w.disc)
+    g.load_positions(torch.as_tensor(xy, device="cuda"))
+    g.sweep(args.sweeps)
+    rows = []
+    for _ in range(args.samples):
+        g.sweep(args.burst)
+        pc = g.phase_clocks()
+        if pc is None:
+            raise SystemExit("this library was built without -DMPMC_PHASE_CLOCKS")
+        rows.append(pc.astype(np.int64))
+    pc = np.stack(rows)                              # (samples, tiles, marks)
+    d = np.diff(pc[:, :, 1:], axis=2)                # cycles per phase
+    span_ns = pc[:, :, 0].max(axis=1) - pc[:, :, 0].min(axis=1)
+    cfg = g.config()
+    print(f"{w.name}: {cfg['ntx']} x {cfg['nty']} tiles, {cfg['tile_threads']} threads, {cfg['tile_smem']} B shared memory; "
+          f"{args.samples} launches; tile start times within {span_ns.mean():.0f} ns")
+    for i in range(d.shape[2]):
+        name = PHASES[i + 1] if i + 1 < len(PHASES) else f"phase {i + 1}"
+        print(f"  {name:42s} mean {d[:, :, i].mean():9.0f}   max over tiles (mean over launches) {d[:, :, i].max(axis=1).mean():9.0f} cycles")
+    if args.dump:
+        np.save(args.dump, d.mean(axis=0))
+    tot = pc[:, :, -1] - pc[:, :, 1]
+    print(f"  {'whole tile':42s} mean {tot.mean():9.0f}   max {tot.max(axis=1).mean():9.0f} cycles")
+
+
+if __name__ == "__main__":
+    main()

@@ -40,7 +40,7 @@ def run(name, N, box, xy, d, n_s, seed, fp32, sweeps, w_target=0.0, disc=False, 
             for k, v in want.items():
                 assert cfg[k] == v, (name, k, cfg)
         print(f"{name:28s} debug={int(debug)} fp{'32' if fp32 else '64'} N={N} cells={g.mx}x{g.my} tile_slots={cfg['tile_slots']} "
-              f"compact={cfg['compact']} tiles={cfg['ntx']}x{cfg['nty']} path={path} max n={int(so['counts'].max())}  ok", flush=True)
+              f"tiles={cfg['ntx']}x{cfg['nty']} path={path} max n={int(so['counts'].max())}  ok", flush=True)
         g.close()
 
 
@@ -50,11 +50,11 @@ def main():
     w = I.CONFIGS["C1"]
     xy, box = I.workload_inputs(w)
     for fp32 in (False, True):
-        run("C1", w.N, box, xy, w.d, w.n_s, w.seed, fp32, 6, want={"tile_slots": 2, "compact": 0})
+        run("C1", w.N, box, xy, w.d, w.n_s, w.seed, fp32, 6, want={"tile_slots": 2})
     xy, box = I.jittered_lattice(50, 0.7, seed=50)                 # tiles of different sizes
     run("uneven tiling 50^2", 2500, box, xy, 0.15, 4, 50, True, 5, want={"tile_slots": 2})
-    xy, box = I.jittered_lattice(50, 0.33, seed=50)                # ... in the compacting variant
-    run("uneven tiling, dilute", 2500, box, xy, 0.4, 4, 50, True, 5, want={"tile_slots": 2, "compact": 1})
+    xy, box = I.jittered_lattice(50, 0.33, seed=50)                # ... with most cells empty
+    run("uneven tiling, dilute", 2500, box, xy, 0.4, 4, 50, True, 5, want={"tile_slots": 2})
     xy, box = I.jittered_lattice(64, 0.50, seed=6)                 # cells with three disks on the 2-slot tile kernel
     run("three per cell, w=1.12", 4096, box, xy, 0.3, 4, 8, True, 40, w_target=1.12, want={"tile_slots": 2})
     run("three per cell, w=1.12", 4096, box, xy, 0.3, 8, 8, False, 20, w_target=1.12, want={"tile_slots": 2})

@@ -178,8 +178,7 @@ def test_c4_shape_reduced_and_ns8(oracle_mod, torch_cuda, fp32, n):
     # (k_tile_sweep<float, 8> and k_tile_sweep<double, 8>)
     xy, box = I.jittered_lattice(n, 0.720, seed=1)
     o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.06, 8, 1, fp32, xy)
-    cfg = g.config()
-    assert cfg["tile_slots"] == 2 and cfg["compact"] == 0
+    assert g.config()["tile_slots"] == 2
     o.sweep(8); g.sweep(8)
     assert_same_state(o, g, fp32)
     assert g.path_sweeps() == (8, 0)
@@ -213,7 +212,7 @@ def test_c5_dilute_fluid_reduced(oracle_mod, torch_cuda):
     n = 256
     xy, box = melted_by_the_oracle(oracle_mod, n, 0.30, 0.5)
     o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.5, 4, 1, True, xy)
-    assert g.config()["compact"] == 1                  # the dilute-system variant of the tile kernel
+    assert g.config()["tile_slots"] == 2
     for _ in range(6):
         o.sweep(10); g.sweep(10)
         st = assert_same_state(o, g, True)
@@ -230,8 +229,7 @@ def test_c5_full_size(oracle_mod, torch_cuda):
     xy, box = melted_by_the_oracle(oracle_mod, w.n_side, w.phi, w.d)
     o, g = make_pair(oracle_mod, torch_cuda, w.N, box, w.sigma, w.d, w.n_s, w.seed, True, xy, debug=False)
     assert (g.mx, g.my) == (1780, 1540)
-    cfg = g.config()
-    assert cfg["tile_slots"] == 2 and cfg["compact"] == 1
+    assert g.config()["tile_slots"] == 2
     o.sweep(10); g.sweep(10)
     st = assert_same_state(o, g, True, check_mask=False)
     assert g.path_sweeps() == (10, 0)
@@ -242,13 +240,13 @@ def test_c5_full_size(oracle_mod, torch_cuda):
 
 @pytest.mark.parametrize("fp32", [True, False])
 def test_dilute_fluid_with_three_per_cell(oracle_mod, torch_cuda, fp32):
-    # C5's density and displacement at a cell width just under 1.15 sigma: still the 2-slot tile kernel in its compacting
-    # variant (0.48 disks per cell), and cells with THREE disks do occur — compacted warps x the list of crowded cells
+    # C5's density and displacement at a cell width just under 1.15 sigma: still the 2-slot tile kernel (0.48 disks per
+    # cell: most queue entries are dropped as empty), and cells with THREE disks do occur — occupancy queues x the list of
+    # crowded cells
     n = 256
     xy, box = melted_by_the_oracle(oracle_mod, n, 0.30, 0.5, w_target=1.12, fp32=fp32)
     o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.5, 4, 1, fp32, xy, w_target=1.12)
-    cfg = g.config()
-    assert cfg["tile_slots"] == 2 and cfg["compact"] == 1
+    assert g.config()["tile_slots"] == 2
     seen3, sweeps_with3 = False, 0
     for _ in range(8):
         o.sweep(5); g.sweep(5)
@@ -294,13 +292,13 @@ def test_tile_kernel_hands_over_when_too_many_cells_are_crowded(oracle_mod, torc
 
 
 @pytest.mark.parametrize("n,phi", [(14, 0.5), (24, 0.6), (50, 0.7), (98, 0.65),
-                                   (14, 0.3), (26, 0.38), (50, 0.33), (98, 0.4), (150, 0.25)])    # dilute: compacting variant
+                                   (14, 0.3), (26, 0.38), (50, 0.33), (98, 0.4), (150, 0.25)])    # dilute: most cells empty
 def test_tile_kernel_uneven_tilings(oracle_mod, torch_cuda, n, phi):
     # box sizes that do not divide evenly into tiles (tiles of different widths, many tiny tiles, few large ones)
     xy, box = I.jittered_lattice(n, phi, seed=n)
     o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.15 if phi >= 0.5 else 0.4, 4, n, True, xy)
     cfg = g.config()
-    assert cfg["tile_slots"] == 2 and cfg["compact"] == (1 if n * n < 0.6 * g.M else 0) == (1 if phi < 0.5 else 0)
+    assert cfg["tile_slots"] == 2 and cfg["tiles"] == cfg["ntx"] * cfg["nty"] > 1
     for k in (1, 2, 7):
         o.sweep(k); g.sweep(k)
         assert_same_state(o, g, True)
@@ -308,10 +306,10 @@ def test_tile_kernel_uneven_tilings(oracle_mod, torch_cuda, n, phi):
 
 
 @pytest.mark.parametrize("n_s", [4, 8])
-def test_compacting_variant_fp64(oracle_mod, torch_cuda, n_s):
+def test_dilute_system_fp64(oracle_mod, torch_cuda, n_s):
     xy, box = I.jittered_lattice(60, 0.35, seed=8)
     o, g = make_pair(oracle_mod, torch_cuda, 3600, box, 1.0, 0.4, n_s, 2, False, xy)
-    assert g.config()["compact"] == 1
+    assert g.config()["tile_slots"] == 2
     o.sweep(12); g.sweep(12)
     assert_same_state(o, g, False)
     assert g.path_sweeps() == (12, 0)
