@@ -106,6 +106,24 @@ int mpmc_acceptance(mpmc_ctx* ctx, uint64_t out[4]);
 int mpmc_pressure_contact(mpmc_ctx* ctx, double dr, uint32_t nbins, uint32_t degree, uint64_t* hist_out,
                           double* g_contact, double* p_star);
 
+/* Contact pressure averaged over samples — the paper's procedure (L384: a sample every 200 sweeps; eq. 5 averages n[r_i]
+ * over configurations before the fit).
+ *   mpmc_pressure_accumulate  adds the pair histogram of the CURRENT state (same bins and arithmetic as
+ *       mpmc_pressure_contact) to an accumulator in the workspace and counts one sample.  Asynchronous: no host
+ *       synchronisation per sample.  The first sample after a reset fixes (dr, nbins); other values are MPMC_ERR_ARG.
+ *   mpmc_pressure_accumulated  hist_out = host, nbins summed counts (may be NULL); *samples = number of samples (may be
+ *       NULL); g_contact / p_star (each may be NULL) = eq. 5-6 on the sample-averaged histogram, polynomial fit of the
+ *       given degree extrapolated to r = sigma, and eq. 4.  Synchronises.  MPMC_ERR_STATE with no sample.
+ *   mpmc_pressure_reset  empties the accumulator (mpmc_load_positions does NOT).
+ *   mpmc_pressure_from_histogram  the same estimator on a caller's histogram (host, nbins counts summed over `samples`
+ *       configurations of THIS system — e.g. blocks of accumulated histograms added up).  Host arithmetic only. */
+int mpmc_pressure_accumulate(mpmc_ctx* ctx, double dr, uint32_t nbins);
+int mpmc_pressure_accumulated(mpmc_ctx* ctx, uint32_t degree, uint64_t* hist_out, uint64_t* samples, double* g_contact,
+                              double* p_star);
+int mpmc_pressure_reset(mpmc_ctx* ctx);
+int mpmc_pressure_from_histogram(const mpmc_ctx* ctx, const uint64_t* hist, uint64_t samples, double dr, uint32_t nbins,
+                                 uint32_t degree, double* g_contact, double* p_star);
+
 /* Test hooks: single pieces of Algorithm 1 at the current sweep index (do not advance it). */
 int mpmc_debug_sub_sweep(mpmc_ctx* ctx, uint32_t checkerboard_set /*0=a(0,0) 1=b(1,0) 2=c(0,1) 3=d(1,1)*/);
 /* delta in [0, w) of the chosen axis (Algorithm 1 draws it from [0, w/2), L90; the pull form of Algorithm 4 takes

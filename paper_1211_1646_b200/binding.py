@@ -32,6 +32,10 @@ SYMBOLS = {
     "mpmc_get_positions": (C.c_int, [_vp, _vp]),
     "mpmc_acceptance": (C.c_int, [_vp, C.POINTER(_u64)]),
     "mpmc_pressure_contact": (C.c_int, [_vp, _dbl, _u32, _u32, _vp, C.POINTER(_dbl), C.POINTER(_dbl)]),
+    "mpmc_pressure_accumulate": (C.c_int, [_vp, _dbl, _u32]),
+    "mpmc_pressure_accumulated": (C.c_int, [_vp, _u32, _vp, C.POINTER(_u64), C.POINTER(_dbl), C.POINTER(_dbl)]),
+    "mpmc_pressure_reset": (C.c_int, [_vp]),
+    "mpmc_pressure_from_histogram": (C.c_int, [_vp, _vp, _u64, _dbl, _u32, _u32, C.POINTER(_dbl), C.POINTER(_dbl)]),
     "mpmc_debug_sub_sweep": (C.c_int, [_vp, _u32]),
     "mpmc_debug_shift": (C.c_int, [_vp, _u32, _dbl]),
     "mpmc_debug_state": (C.c_int, [_vp, _vp, _vp, _vp, _vp, C.POINTER(_dbl), C.POINTER(_u64), C.POINTER(_u64)]),
@@ -197,6 +201,38 @@ class Mpmc:
             _chk(lib().mpmc_pressure_contact(self._h, float(dr), int(nbins), 0, h.ctypes.data, None, None))
             self._exit()
         return h
+
+    def pressure_accumulate(self, dr: float, nbins: int) -> None:
+        """Add the current state's pair histogram to the device accumulator (asynchronous)."""
+        with self.torch.cuda.device(self.device):
+            self._enter()
+            _chk(lib().mpmc_pressure_accumulate(self._h, float(dr), int(nbins)))
+            self._exit()
+
+    def pressure_accumulated(self, degree: int, nbins: int, fit: bool = True):
+        """(summed histogram, samples, g(sigma+), P*) of the accumulator; g and P* are None with fit=False."""
+        import numpy as np
+        h = np.zeros(nbins, dtype=np.uint64)
+        n, g0, ps = _u64(), _dbl(), _dbl()
+        with self.torch.cuda.device(self.device):
+            self._enter()
+            _chk(lib().mpmc_pressure_accumulated(self._h, int(degree), h.ctypes.data, C.byref(n),
+                                                 C.byref(g0) if fit else None, C.byref(ps) if fit else None))
+            self._exit()
+        return h, int(n.value), (g0.value if fit else None), (ps.value if fit else None)
+
+    def pressure_reset(self) -> None:
+        _chk(lib().mpmc_pressure_reset(self._h))
+
+    def pressure_from_histogram(self, hist, samples: int, dr: float, degree: int):
+        """(g(sigma+), P*) of eq. 4-6 on a histogram summed over `samples` configurations of this system (host arithmetic
+        inside the library)."""
+        import numpy as np
+        h = np.ascontiguousarray(hist, dtype=np.uint64)
+        g0, ps = _dbl(), _dbl()
+        _chk(lib().mpmc_pressure_from_histogram(self._h, h.ctypes.data, int(samples), float(dr), len(h), int(degree),
+                                                C.byref(g0), C.byref(ps)))
+        return g0.value, ps.value
 
     # --- test hooks ------------------------------------------------------------------------------------
     def sub_sweep(self, checkerboard_set: int) -> None:

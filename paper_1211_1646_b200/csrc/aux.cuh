@@ -255,7 +255,7 @@ __device__ __forceinline__ void hist_pairs_exact(const Params& p, const P* pos, 
 template <typename P, int RC>
 __global__ void __launch_bounds__(HIST_THREADS) k_contact_hist(const __grid_constant__ Params p, const double dr,
                                                                const uint32_t nbins, const int Rc_arg, const double rmax,
-                                                               const unsigned long long keep) {
+                                                               const unsigned long long keep, unsigned long long* out) {
   using F = Real<float>;
   extern __shared__ uint32_t sh_hist[];
   __shared__ HistQueue s_queue[HIST_THREADS / 32];
@@ -372,7 +372,7 @@ __global__ void __launch_bounds__(HIST_THREADS) k_contact_hist(const __grid_cons
   if (lane < qn) hist_pairs_exact<P>(p, pos, ids, q.own[lane], q.nb[lane], q.code[lane], dr, nbins, rmax2, sh_hist);
   __syncthreads();
   for (uint32_t b = threadIdx.x; b < nbins; b += HIST_THREADS)
-    if (sh_hist[b]) atomicAdd(&p.hist[b], (unsigned long long)sh_hist[b]);
+    if (sh_hist[b]) atomicAdd(&out[b], (unsigned long long)sh_hist[b]);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -388,7 +388,7 @@ constexpr int HT_W = 32, HT_H = 16, HT_THREADS = 256;      // a warp per row, HT
 template <typename P, int RC>
 __global__ void __launch_bounds__(HT_THREADS) k_contact_hist_tile(const __grid_constant__ Params p, const double dr,
                                                                    const uint32_t nbins, const double rmax,
-                                                                   const unsigned long long keep) {
+                                                                   const unsigned long long keep, unsigned long long* out) {
   using F = Real<float>;
   constexpr int CW = HT_W + 2 * RC, CH = HT_H + RC, NT = HT_THREADS;
   extern __shared__ uint32_t sh_hist[];
@@ -512,7 +512,7 @@ __global__ void __launch_bounds__(HT_THREADS) k_contact_hist_tile(const __grid_c
   if (lane < qn) exact(qp[lane], qc[lane]);
   __syncthreads();
   for (uint32_t b = tid; b < nbins; b += NT)
-    if (sh_hist[b]) atomicAdd(&p.hist[b], (unsigned long long)sh_hist[b]);
+    if (sh_hist[b]) atomicAdd(&out[b], (unsigned long long)sh_hist[b]);
 }
 
 __global__ void k_philox_test(const uint32_t* __restrict__ ctr, uint32_t k0, uint32_t k1, uint32_t* __restrict__ out, uint32_t n) {

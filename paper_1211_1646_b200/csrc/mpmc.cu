@@ -34,6 +34,9 @@ struct mpmc_ctx {
   bool tile_two_slot;      // the tile kernel is the 2-slot one (tile.cuh), which may hand a crowded state to the general kernel
   uint32_t sms;            // SMs of the device
   uint64_t t_host;         // sweeps requested since the last load (the sweep index the device will reach)
+  unsigned long long* hist_acc;   // device: histogram accumulated over samples (mpmc_pressure_accumulate)
+  uint64_t acc_samples;    // samples in it
+  double acc_dr; uint32_t acc_nbins;   // its bins (fixed by the first sample after a reset)
   int sticky;
 };
 
@@ -75,7 +78,7 @@ int geometry(const double box[2], double sigma, double w_target, bool fp32, Geom
 
 struct Layout {
   uint32_t Mq, Mqp;
-  size_t off_ctl, off_hist, off_cnt32, off_cnt[2], off_pos[2], off_ids[2], off_mask, total;
+  size_t off_ctl, off_hist, off_hist_acc, off_cnt32, off_cnt[2], off_pos[2], off_ids[2], off_mask, total;
 };
 
 Layout layout(const Geom& g, bool fp32, bool debug) {
@@ -86,6 +89,7 @@ Layout layout(const Geom& g, bool fp32, bool debug) {
   size_t o = 0;
   L.off_ctl = o; o += up(sizeof(Ctl), ALIGN);
   L.off_hist = o; o += up((size_t)MAX_BINS * 8, ALIGN);
+  L.off_hist_acc = o; o += up((size_t)MAX_BINS * 8, ALIGN);
   L.off_cnt32 = o; o += up((size_t)4 * L.Mqp * 4, ALIGN);
   for (int b = 0; b < 2; ++b) { L.off_cnt[b] = o; o += up((size_t)4 * L.Mqp, ALIGN); }
   for (int b = 0; b < 2; ++b) { L.off_pos[b] = o; o += up((size_t)4 * NMAX * L.Mqp * real2, ALIGN); }
@@ -193,6 +197,62 @@ bool polyfit_at_zero(const std::vector<double>& t, const std::vector<double>& y,
   return true;
 }
 
+// eq. 5-6 (L374-379) on a histogram summed over `samples` configurations: g(R_i) = 2 H_i / (samples N rho 2 pi R_i dr),
+// R_i = (2/3)(r_{i+1}^3 - r_i^3)/(r_{i+1}^2 - r_i^2); unweighted polynomial fit extrapolated to r = sigma (L382);
+// P* = sigma^2 rho (1 + (pi/2) sigma^2 rho g(sigma+))  (eq. 4).  Host arithmetic.
+int fit_contact(const mpmc_ctx* c, const uint64_t* H, uint64_t samples, double dr, uint32_t nbins, uint32_t degree,
+                double* g_contact, double* p_star) {
+  const Params& p = c->p;
+  const double Nd = (double)c->N, rho = Nd / (p.Lx_eff * p.Ly_eff), sg = p.sigma_d;
+  const double PI = 3.14159265358979323846;
+  std::vector<double> t(nbins), g(nbins);
+  for (uint32_t i = 0; i < nbins; ++i) {
+    const double r0 = sg + dr * (double)i, r1 = sg + dr * (double)(i + 1);
+    const double Ri = (2.0 / 3.0) * (r1 * r1 * r1 - r0 * r0 * r0) / (r1 * r1 - r0 * r0);
+    t[i] = (Ri - sg) / (dr * (double)nbins);     // scaled abscissa; the value at 0 is unchanged
+    g[i] = 2.0 * ((double)H[i] / (double)samples) / (Nd * rho * 2.0 * PI * Ri * dr);
+  }
+  double g0 = 0;
+  if (!polyfit_at_zero(t, g, degree, &g0)) return MPMC_ERR_ARG;
+  if (g_contact) *g_contact = g0;
+  if (p_star) *p_star = sg * sg * rho * (1.0 + 0.5 * PI * sg * sg * rho * g0);
+  return MPMC_OK;
+}
+
+// the pair-distance histogram of the current state, ADDED to `target` (device, nbins u64); asynchronous
+int launch_histogram(mpmc_ctx* c, double dr, uint32_t nbins, unsigned long long* target) {
+  const Params& p = c->p;
+  const double rmax = p.sigma_d + (double)nbins * dr;
+  const double wmin = p.wx_d < p.wy_d ? p.wx_d : p.wy_d;
+  const int Rc = (int)std::ceil(rmax / wmin);
+  if (Rc > 120) return MPMC_ERR_ARG;                     // the range must stay within a few cells (offsets are packed in 8 bits)
+  // offsets of the half neighbourhood whose cells can hold a pair closer than rmax (radius 1 and 2: compile-time loops)
+  unsigned long long keep = 0;
+  const double rmax2 = rmax * rmax * 1.000001;
+  if (Rc <= 2)
+    for (int oy = 0; oy <= Rc; ++oy)
+      for (int ox = -Rc; ox <= Rc; ++ox) {
+        if (oy == 0 && ox <= 0) continue;
+        const int gi = (ox < 0 ? -ox : ox) - 1, gj = oy - 1;
+        const double gx = (gi > 0 ? gi : 0) * p.wx_d, gy = (gj > 0 ? gj : 0) * p.wy_d;
+        if (gx * gx + gy * gy < rmax2) keep |= 1ull << hist_offset_index(ox, oy, Rc);
+      }
+  const size_t sh = (size_t)nbins * 4;
+  if (Rc <= 2) {                     // tiles staged in shared memory
+    const dim3 gT((p.mx + HT_W - 1) / HT_W, (p.my + HT_H - 1) / HT_H);
+#define MPMC_HIST(P, RC) k_contact_hist_tile<P, RC><<<gT, HT_THREADS, sh, c->stream>>>(p, dr, nbins, rmax, keep, target)
+    if (c->fp32) { if (Rc == 1) MPMC_HIST(float, 1); else MPMC_HIST(float, 2); }
+    else         { if (Rc == 1) MPMC_HIST(double, 1); else MPMC_HIST(double, 2); }
+#undef MPMC_HIST
+  } else {
+    const dim3 gC = cell_grid(c, HIST_THREADS);
+    if (c->fp32) k_contact_hist<float, 0><<<gC, HIST_THREADS, sh, c->stream>>>(p, dr, nbins, Rc, rmax, keep, target);
+    else         k_contact_hist<double, 0><<<gC, HIST_THREADS, sh, c->stream>>>(p, dr, nbins, Rc, rmax, keep, target);
+  }
+  CU(cudaGetLastError());
+  return MPMC_OK;
+}
+
 }  // namespace
 
 // =========================================================================================================
@@ -246,6 +306,8 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   char* base = (char*)workspace;
   p.ctl = (Ctl*)(base + L.off_ctl);
   p.hist = (unsigned long long*)(base + L.off_hist);
+  c->hist_acc = (unsigned long long*)(base + L.off_hist_acc);
+  c->acc_samples = 0; c->acc_dr = 0.0; c->acc_nbins = 0;
   p.cnt32 = (uint32_t*)(base + L.off_cnt32);
   for (int b = 0; b < 2; ++b) {
     p.cnt[b] = (uint8_t*)(base + L.off_cnt[b]);
@@ -436,57 +498,63 @@ int mpmc_pressure_contact(mpmc_ctx* c, double dr, uint32_t nbins, uint32_t degre
   if (!c || !(dr > 0) || nbins == 0 || nbins > MAX_BINS) return MPMC_ERR_ARG;
   if ((g_contact || p_star) && degree + 1 > nbins) return MPMC_ERR_ARG;
   if (!c->loaded) return MPMC_ERR_STATE;
-  const Params& p = c->p;
-  const double rmax = p.sigma_d + (double)nbins * dr;
-  const double wmin = p.wx_d < p.wy_d ? p.wx_d : p.wy_d;
-  const int Rc = (int)std::ceil(rmax / wmin);
-  CU(cudaMemsetAsync(p.hist, 0, (size_t)nbins * 8, c->stream));
-  if (Rc > 120) return MPMC_ERR_ARG;                     // the range must stay within a few cells (offsets are packed in 8 bits)
-  // offsets of the half neighbourhood whose cells can hold a pair closer than rmax (radius 1 and 2: compile-time loops)
-  unsigned long long keep = 0;
-  const double rmax2 = rmax * rmax * 1.000001;
-  if (Rc <= 2)
-    for (int oy = 0; oy <= Rc; ++oy)
-      for (int ox = -Rc; ox <= Rc; ++ox) {
-        if (oy == 0 && ox <= 0) continue;
-        const int gi = (ox < 0 ? -ox : ox) - 1, gj = oy - 1;
-        const double gx = (gi > 0 ? gi : 0) * p.wx_d, gy = (gj > 0 ? gj : 0) * p.wy_d;
-        if (gx * gx + gy * gy < rmax2) keep |= 1ull << hist_offset_index(ox, oy, Rc);
-      }
-  const size_t sh = (size_t)nbins * 4;
-  if (Rc <= 2) {                     // tiles staged in shared memory
-    const dim3 gT((p.mx + HT_W - 1) / HT_W, (p.my + HT_H - 1) / HT_H);
-#define MPMC_HIST(P, RC) k_contact_hist_tile<P, RC><<<gT, HT_THREADS, sh, c->stream>>>(p, dr, nbins, rmax, keep)
-    if (c->fp32) { if (Rc == 1) MPMC_HIST(float, 1); else MPMC_HIST(float, 2); }
-    else         { if (Rc == 1) MPMC_HIST(double, 1); else MPMC_HIST(double, 2); }
-#undef MPMC_HIST
-  } else {
-    const dim3 gC = cell_grid(c, HIST_THREADS);
-    if (c->fp32) k_contact_hist<float, 0><<<gC, HIST_THREADS, sh, c->stream>>>(p, dr, nbins, Rc, rmax, keep);
-    else         k_contact_hist<double, 0><<<gC, HIST_THREADS, sh, c->stream>>>(p, dr, nbins, Rc, rmax, keep);
-  }
-  CU(cudaGetLastError());
+  CU(cudaMemsetAsync(c->p.hist, 0, (size_t)nbins * 8, c->stream));
+  const int st = launch_histogram(c, dr, nbins, c->p.hist);
+  if (st != MPMC_OK) return st;
   std::vector<uint64_t> H(nbins);
-  CU(cudaMemcpyAsync(H.data(), p.hist, (size_t)nbins * 8, cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaMemcpyAsync(H.data(), c->p.hist, (size_t)nbins * 8, cudaMemcpyDeviceToHost, c->stream));
   CU(cudaStreamSynchronize(c->stream));
   if (hist_out) std::memcpy(hist_out, H.data(), (size_t)nbins * 8);
   if (g_contact || p_star) {
-    // eq. 5-6 (L374-379): g(R_i) = 2 H_i / (N rho 2 pi R_i dr), R_i = (2/3)(r_{i+1}^3 - r_i^3)/(r_{i+1}^2 - r_i^2)
-    const double Nd = (double)c->N, rho = Nd / (p.Lx_eff * p.Ly_eff), sg = p.sigma_d;
-    const double PI = 3.14159265358979323846;
-    std::vector<double> t(nbins), g(nbins);
-    for (uint32_t i = 0; i < nbins; ++i) {
-      const double r0 = sg + dr * (double)i, r1 = sg + dr * (double)(i + 1);
-      const double Ri = (2.0 / 3.0) * (r1 * r1 * r1 - r0 * r0 * r0) / (r1 * r1 - r0 * r0);
-      t[i] = (Ri - sg) / (dr * (double)nbins);     // scaled abscissa; the value at 0 is unchanged
-      g[i] = 2.0 * (double)H[i] / (Nd * rho * 2.0 * PI * Ri * dr);
-    }
-    double g0 = 0;
-    if (!polyfit_at_zero(t, g, degree, &g0)) return MPMC_ERR_ARG;
-    if (g_contact) *g_contact = g0;
-    if (p_star) *p_star = sg * sg * rho * (1.0 + 0.5 * PI * sg * sg * rho * g0);   // eq. 4 (L368)
+    const int fs = fit_contact(c, H.data(), 1, dr, nbins, degree, g_contact, p_star);
+    if (fs != MPMC_OK) return fs;
   }
   return c->sticky;
+}
+
+int mpmc_pressure_accumulate(mpmc_ctx* c, double dr, uint32_t nbins) {
+  if (!c || !(dr > 0) || nbins == 0 || nbins > MAX_BINS) return MPMC_ERR_ARG;
+  if (!c->loaded) return MPMC_ERR_STATE;
+  if (c->acc_samples == 0) {                     // the first sample after a reset fixes the bins
+    CU(cudaMemsetAsync(c->hist_acc, 0, (size_t)MAX_BINS * 8, c->stream));
+    c->acc_dr = dr; c->acc_nbins = nbins;
+  } else if (dr != c->acc_dr || nbins != c->acc_nbins) {
+    return MPMC_ERR_ARG;
+  }
+  const int st = launch_histogram(c, dr, nbins, c->hist_acc);      // the kernels ADD to their target
+  if (st != MPMC_OK) return st;
+  c->acc_samples += 1;
+  return c->sticky;
+}
+
+int mpmc_pressure_accumulated(mpmc_ctx* c, uint32_t degree, uint64_t* hist_out, uint64_t* samples, double* g_contact,
+                              double* p_star) {
+  if (!c) return MPMC_ERR_ARG;
+  if (!c->loaded) return MPMC_ERR_STATE;
+  if (samples) *samples = c->acc_samples;
+  if (c->acc_samples == 0) return (hist_out || g_contact || p_star) ? MPMC_ERR_STATE : c->sticky;
+  if ((g_contact || p_star) && degree + 1 > c->acc_nbins) return MPMC_ERR_ARG;
+  std::vector<uint64_t> H(c->acc_nbins);
+  CU(cudaMemcpyAsync(H.data(), c->hist_acc, (size_t)c->acc_nbins * 8, cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  if (hist_out) std::memcpy(hist_out, H.data(), (size_t)c->acc_nbins * 8);
+  if (g_contact || p_star) {
+    const int fs = fit_contact(c, H.data(), c->acc_samples, c->acc_dr, c->acc_nbins, degree, g_contact, p_star);
+    if (fs != MPMC_OK) return fs;
+  }
+  return c->sticky;
+}
+
+int mpmc_pressure_reset(mpmc_ctx* c) {
+  if (!c) return MPMC_ERR_ARG;
+  c->acc_samples = 0; c->acc_dr = 0.0; c->acc_nbins = 0;
+  return MPMC_OK;
+}
+
+int mpmc_pressure_from_histogram(const mpmc_ctx* c, const uint64_t* hist, uint64_t samples, double dr, uint32_t nbins,
+                                 uint32_t degree, double* g_contact, double* p_star) {
+  if (!c || !hist || samples == 0 || !(dr > 0) || nbins == 0 || degree + 1 > nbins) return MPMC_ERR_ARG;
+  return fit_contact(c, hist, samples, dr, nbins, degree, g_contact, p_star);
 }
 
 int mpmc_debug_sub_sweep(mpmc_ctx* c, uint32_t set) {

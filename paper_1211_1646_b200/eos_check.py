@@ -50,27 +50,26 @@ def main():
     a0 = sim.acceptance()
     nsamp = args.sweeps // args.every
     per_block = max(1, nsamp // args.blocks)
-    hist_block = np.zeros((args.blocks, nbins), dtype=np.float64)
+    # the estimator (eq. 4-6, degree-5 fit) lives behind the C ABI: mpmc_pressure_accumulate adds a sample on the device
+    # without a host synchronisation, mpmc_pressure_accumulated fits a block, mpmc_pressure_from_histogram the whole run
+    hist_all = np.zeros(nbins, dtype=np.uint64)
+    p_blocks = []
     t0 = time.time()
-    for i in range(per_block * args.blocks):
-        sim.sweep(args.every)
-        hist_block[i // per_block] += sim.contact_histogram(dr, nbins)
+    for _ in range(args.blocks):
+        sim.pressure_reset()
+        for _ in range(per_block):
+            sim.sweep(args.every)
+            sim.pressure_accumulate(dr, nbins)
+        h, n, _, p_b = sim.pressure_accumulated(degree, nbins)
+        assert n == per_block
+        hist_all += h
+        p_blocks.append(p_b)
     torch.cuda.synchronize()
     t_run = time.time() - t0
     a1 = sim.acceptance()
     L = sim.L_eff
-    rho = N / (L[0] * L[1])
-
-    def p_star(hist, samples):
-        # eq. 5-6 (L374-379): g(R_i) = 2 H_i / (N rho 2 pi R_i dr) per sample; unweighted degree-5 fit; eq. 4 (L368)
-        r0 = 1.0 + dr * np.arange(nbins); r1 = r0 + dr
-        R = (2.0 / 3.0) * (r1 ** 3 - r0 ** 3) / (r1 ** 2 - r0 ** 2)
-        g = 2.0 * hist / samples / (N * rho * 2.0 * np.pi * R * dr)
-        c = np.polynomial.polynomial.polyfit((R - 1.0) / (dr * nbins), g, degree)
-        return rho * (1.0 + 0.5 * np.pi * rho * c[0]), c[0]
-
-    p_all, g_all = p_star(hist_block.sum(axis=0), per_block * args.blocks)
-    p_blocks = np.array([p_star(h, per_block)[0] for h in hist_block])
+    g_all, p_all = sim.pressure_from_histogram(hist_all, per_block * args.blocks, dr, degree)
+    p_blocks = np.array(p_blocks)
     out = {
         "N": N, "phi": args.phi, "box": list(L), "cells": [sim.mx, sim.my], "d": args.d, "n_s": args.n_s,
         "dtype": "f64" if args.fp64 else "f32", "w_target": args.w_target, "disc": args.disc,

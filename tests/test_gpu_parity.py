@@ -147,6 +147,39 @@ def test_contact_histogram_of_tiny_boxes(oracle_mod, torch_cuda, N, box, xy, fp3
             assert np.array_equal(o.contact_histogram(dr, nbins), g.contact_histogram(dr, nbins)), (dr, nbins)
 
 
+@pytest.mark.parametrize("fp32", [False, True])
+def test_sample_averaged_pressure_estimator(oracle_mod, torch_cuda, fp32):
+    """The paper's procedure (L384, eq. 5): histograms of many configurations are averaged, then fitted.  The accumulator
+    and the fit live behind the C ABI; the oracle's estimator on the summed oracle histograms is the reference."""
+    from paper_1211_1646_b200.binding import MpmcError
+    xy, box = I.jittered_lattice(64, 0.66, seed=5)
+    o, g = make_pair(oracle_mod, torch_cuda, 4096, box, 1.0, 0.15, 4, 2, fp32, xy)
+    dr, nbins, degree = 1e-3, 40, 3
+    with pytest.raises(MpmcError) as e:
+        g.pressure_accumulated(degree, nbins)            # no sample yet
+    assert e.value.code == -7
+    total = np.zeros(nbins, dtype=np.uint64)
+    for s in range(6):
+        o.sweep(5); g.sweep(5)
+        g.pressure_accumulate(dr, nbins)
+        total += o.contact_histogram(dr, nbins)
+    with pytest.raises(MpmcError) as e:
+        g.pressure_accumulate(2 * dr, nbins)             # the bins are fixed by the first sample
+    assert e.value.code == -1
+    h, n, g0, ps = g.pressure_accumulated(degree, nbins)
+    assert n == 6 and np.array_equal(h, total) and total.sum() > 1000
+    g0_o, ps_o = oracle_mod.pressure_from_histogram(total.astype(np.float64) / 6, o.N, o.L_eff, o.sigma, dr, degree)
+    assert g0 == pytest.approx(g0_o, rel=1e-9) and ps == pytest.approx(ps_o, rel=1e-9)
+    # the same fit on a caller's histogram, and one sample == mpmc_pressure_contact
+    assert g.pressure_from_histogram(total, 6, dr, degree) == (g0, ps)
+    g.pressure_reset()
+    g.pressure_accumulate(dr, nbins)
+    h1, n1, g1, p1 = g.pressure_accumulated(degree, nbins)
+    hc, gc, pc = g.pressure_contact(dr, nbins, degree)
+    assert n1 == 1 and np.array_equal(h1, hc) and (g1, p1) == (gc, pc)
+    assert_same_state(o, g, fp32)
+
+
 def test_c3_headline_config_bench_launch_configuration(oracle_mod, torch_cuda):
     """Full size N = 2^20, fp32, NO debug flag: exactly the kernels bench.py times."""
     w = I.CONFIGS["C3"]
