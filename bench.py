@@ -159,7 +159,7 @@ def workload_config(w, sweeps):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=11, help="timed steps (11: the paper's protocol, median of 11 runs, PAPER.md L421)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C3", choices=sorted(I.CONFIGS))
@@ -216,7 +216,8 @@ def main():
         return sim.acceptance()[0], hist
 
     def timed(fn, K, sampler=None):
-        total_ms, moves = 0.0, 0
+        """K timed steps; returns (sum of the step times in ms, sum of the trial moves, per-step rates in moves/s)."""
+        total_ms, moves, rates = 0.0, 0, []
         for _ in range(K):
             flush.fill_(1)                            # L2 flush between timed iterations (not timed)
             torch.cuda.synchronize(dev)
@@ -225,9 +226,15 @@ def main():
             att, _ = fn()
             e1.record()
             torch.cuda.synchronize(dev)
-            total_ms += e0.elapsed_time(e1)
+            ms_step = e0.elapsed_time(e1)
+            total_ms += ms_step
             moves += att
-        return total_ms, moves
+            rates.append(att / (ms_step * 1e-3))
+        return total_ms, moves, rates
+
+    def spread(rates):
+        """median with min / max over the timed steps (the paper reports the median of 11 runs)"""
+        return {"median": float(np.median(rates)), "min": float(np.min(rates)), "max": float(np.max(rates)), "steps": len(rates)}
 
     # everything below is enqueued on the library's own stream, so torch.cuda.Event times that stream
     torch.cuda.synchronize(dev)
@@ -239,14 +246,14 @@ def main():
     torch.cuda.synchronize(dev)
     sampler = ClockSampler(local)
     sampler.start()
-    ms, moves = timed(step_resident, args.steps)
+    ms, moves, rates = timed(step_resident, args.steps)
     clocks = sampler.stop()
     torch.cuda.synchronize(dev)
     if dist:
         dist.barrier()
     for _ in range(max(1, args.warmup // 3)):
         step_e2e()
-    ms_e2e, moves_e2e = timed(step_e2e, args.steps)
+    ms_e2e, moves_e2e, rates_e2e = timed(step_e2e, args.steps)
 
     # ---- roofline of the dominant kernel: k_tile_sweep, one launch = one whole sweep (four sub-sweeps + shift),
     #      timed live with CUDA events on the library's stream over S back-to-back launches ----
@@ -259,6 +266,10 @@ def main():
     sweep_ms = e0.elapsed_time(e1) / S
     moves_per_sweep = (sim.acceptance()[0] - a0) / S
     tile_sweeps, general_sweeps = sim.path_sweeps()
+    cfg = sim.config()
+    e = 8 if w.fp32 else 16
+    state_bytes = sim.M * (2 * e + 8 + 1)              # slot pair 0 + its ids + count of every cell, one buffer
+    l2_bytes = torch.cuda.get_device_properties(dev).L2_cache_size
     tile_name = "k_tile4_sweep" if (w.disc or w.w_target >= 1.15) else "k_tile_sweep"     # 4-slot / 2-slot tile kernel
     kernel = tile_name if tile_sweeps >= general_sweeps else "k_sweeps"
     peak, peak_src = peaks()
@@ -271,9 +282,14 @@ def main():
                 "share_of_step": S * sweep_ms / (ms / args.steps),
                 "sweeps_on_tile_kernel": tile_sweeps, "sweeps_on_general_kernel": general_sweeps,
                 "fused_floor_bytes_per_launch": fused_floor_bytes_per_sweep(w.N, sim.M, w.fp32),
-                "note": "one launch = one sweep; the state (16 B per cell) is L2-resident at this size and the kernel is "
-                        "issue-bound on the plain ALUs (see alu), the HBM fraction is reported because BASELINE.json "
-                        "names it"}
+                "state_bytes": state_bytes, "l2_bytes": l2_bytes,
+                "note": ("one launch = one sweep; the state is L2-resident at this size (2 buffers x state_bytes < L2): the "
+                         "load and shift phases run at the L2 bandwidth the SMs share, the sub-sweeps are bound by the FMA-class "
+                         "pipes (see alu); the HBM fraction is reported because BASELINE.json names it")
+                if 2 * state_bytes < l2_bytes else
+                        ("one launch = one sweep; the state does not fit L2 (2 buffers x state_bytes > L2), so every sweep "
+                         "streams it from and to HBM: `traffic` (ncu dram bytes per launch) against the fused floor "
+                         "2 (e N + M) is the HBM figure")}
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         try:
@@ -295,7 +311,7 @@ def main():
     value = moves / (ms * 1e-3)
     e2e = moves_e2e / (ms_e2e * 1e-3)
 
-    cpu = None
+    cpu, cpu_strips = None, None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import oracle as O
         O.build()
@@ -309,22 +325,39 @@ def main():
         cpu = {"value": (o.acceptance()[0] - a0) / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"{args.cpu_baseline_sweeps} sweeps of {w.name} (N={w.N}) after 1 warm-up sweep, "
                          f"single thread of {os.cpu_count()} host cores, {dt:.1f} s"}
+        # the paper's multi-core CPU program: OpenMP, one horizontal strip of cells per thread, same
+        # trajectory as the oracle bit for bit (checked here on the sample)
+        O.build_strip()
+        sb = O.StripBaseline(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=w.fp32, w_target=w.w_target, disc=w.disc)
+        sb.load_positions(xy_np)
+        sb.sweep(1)
+        b0 = sb.acceptance()[0]
+        t0 = time.perf_counter()
+        sb.sweep(args.cpu_baseline_sweeps)
+        dts = time.perf_counter() - t0
+        cpu_strips = {"value": (sb.acceptance()[0] - b0) / dts, "unit": UNIT, "cores": sb.threads, "kind": "openmp-strips",
+                      "identical_to_oracle": sb.acceptance() == o.acceptance(),
+                      "sample": f"the same {args.cpu_baseline_sweeps} sweeps, {sb.threads} OpenMP threads, {dts:.1f} s"}
 
     if rank == 0:
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32" if w.fp32 else "f64", "data": "synthetic",
+            "per_step": dict(spread(rates), unit=UNIT, note="this rank's steps; `value` is all steps' moves / all steps' time"),
             "config": dict(workload_config(w, S), parallelism=f"replicas x{world}" if world > 1 else "1 GPU",
                            l2="flushed between timed steps (256 MiB fill); the state itself is L2-resident",
                            step="load_positions + sweeps + contact histogram + get_positions + counters"),
             "clocks": clocks,
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": int(xy_pinned.numel() * 8),
-                    "d2h_bytes_per_step": int(out_pinned.numel() * 8 + 20 * 8 + 64), "ms_per_step": ms_e2e / args.steps},
-            "gpu_launches": args.steps * (4 + S + 1 + 1 + 1),   # cell-list build 4, one tile kernel per sweep, general
-                                                                # kernel (no-op), histogram, unpack
+                    "d2h_bytes_per_step": int(out_pinned.numel() * 8 + 20 * 8 + 64), "ms_per_step": ms_e2e / args.steps,
+                    "per_step": spread(rates_e2e)},
+            # cell-list build 4; one tile kernel per sweep (+ the general kernel's pass behind the 2-slot tile kernel: a
+            # no-op unless a state was handed over), or one persistent launch without a tile kernel; histogram; unpack
+            "gpu_launches": args.steps * (4 + (S + (1 if cfg["tile_slots"] == 2 else 0) if cfg["tile_slots"] else 1) + 1 + 1),
             "roofline": roofline,
             "cpu_baseline": cpu,
+            "cpu_baseline_strips": cpu_strips,
             "paper_context": "PAPER.md L413: 1.09e9 trial moves/s on a Tesla K20 (different cell width, proposal and RNG)",
         }))
     if dist:

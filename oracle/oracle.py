@@ -43,13 +43,25 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
+_STRIP_SRC = os.path.join(_HERE, "strip_omp.cpp")
+_STRIP_LIB = os.path.join(_HERE, "liboracle_strip_omp.so")
+
+
+def build_strip(force: bool = False) -> str:
+    """The OpenMP strip baseline of PAPER.md L390 (strip_omp.cpp, which includes oracle_mpmc.cpp): g++ -O2 -fopenmp."""
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_STRIP_SRC))
+    if force or not os.path.exists(_STRIP_LIB) or os.path.getmtime(_STRIP_LIB) < newest:
+        cmd = ["g++", "-O2", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared",
+               "-o", _STRIP_LIB, _STRIP_SRC]
+        subprocess.run(cmd, check=True)
+    return _STRIP_LIB
+
+
 _lib = None
+_strip_lib = None
 
 
-def lib():
-    global _lib
-    if _lib is None:
-        L = C.CDLL(build())
+def _declare(L):
         u32, u64, dbl, vp = C.c_uint32, C.c_uint64, C.c_double, C.c_void_p
         L.oracle_create.argtypes = [C.POINTER(vp), u64, C.POINTER(dbl), dbl, dbl, u32, u64, u32, dbl]
         L.oracle_destroy.argtypes = [vp]
@@ -74,8 +86,25 @@ def lib():
         L.oracle_variate_sym_f64.argtypes = [u32]; L.oracle_variate_sym_f64.restype = C.c_double
         L.oracle_variate_unit_f32.argtypes = [u32]; L.oracle_variate_unit_f32.restype = C.c_float
         L.oracle_variate_unit_f64.argtypes = [u32]; L.oracle_variate_unit_f64.restype = C.c_double
-        _lib = L
+        return L
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = _declare(C.CDLL(build()))
     return _lib
+
+
+def strip_lib():
+    global _strip_lib
+    if _strip_lib is None:
+        L = _declare(C.CDLL(build_strip()))
+        L.strip_create.argtypes = [C.POINTER(C.c_void_p), C.c_uint64, C.POINTER(C.c_double), C.c_double, C.c_double,
+                                   C.c_uint32, C.c_uint64, C.c_uint32, C.c_double, C.c_int]
+        L.strip_threads.restype = C.c_int
+        _strip_lib = L
+    return _strip_lib
 
 
 class OracleError(RuntimeError):
@@ -129,23 +158,27 @@ class Oracle:
         self.fp32 = bool(fp32)
         self.sigma = float(sigma)
         b = (C.c_double * 2)(float(box[0]), float(box[1]))
-        _chk(lib().oracle_create(C.byref(self._h), self.N, b, sigma, d, n_s, seed, (FP32 if fp32 else FP64) | (DISC if disc else 0)
-                                 | (0 if particle_shuffle else NO_PARTICLE_SHUFFLE) | (0 if set_shuffle else NO_SET_SHUFFLE),
-                                 float(w_target)))
+        flags = ((FP32 if fp32 else FP64) | (DISC if disc else 0) | (0 if particle_shuffle else NO_PARTICLE_SHUFFLE)
+                 | (0 if set_shuffle else NO_SET_SHUFFLE))
+        self._create(b, sigma, d, n_s, seed, flags, float(w_target))
         m = (C.c_uint32 * 2)()
         w = (C.c_double * 2)()
         Le = (C.c_double * 2)()
-        lib().oracle_geometry(self._h, m, w, Le)
+        self._L.oracle_geometry(self._h, m, w, Le)
         self.mx, self.my = int(m[0]), int(m[1])
         self.wx, self.wy = float(w[0]), float(w[1])
         self.L_eff = (float(Le[0]), float(Le[1]))
         self.M = self.mx * self.my
         self.real = np.float32 if fp32 else np.float64
 
+    def _create(self, b, sigma, d, n_s, seed, flags, w_target):
+        self._L = lib()
+        _chk(self._L.oracle_create(C.byref(self._h), self.N, b, sigma, d, n_s, seed, flags, w_target))
+
     def __del__(self):
         try:
             if self._h:
-                lib().oracle_destroy(self._h)
+                self._L.oracle_destroy(self._h)
                 self._h = None
         except Exception:
             pass
@@ -153,30 +186,30 @@ class Oracle:
     def load_positions(self, xy: np.ndarray) -> None:
         xy = np.ascontiguousarray(xy, dtype=np.float64)
         assert xy.shape == (self.N, 2)
-        _chk(lib().oracle_load_positions(self._h, xy.ctypes.data))
+        _chk(self._L.oracle_load_positions(self._h, xy.ctypes.data))
 
     def sweep(self, k: int = 1) -> None:
-        _chk(lib().oracle_sweep(self._h, int(k)))
+        _chk(self._L.oracle_sweep(self._h, int(k)))
 
     def sub_sweep(self, checkerboard_set: int) -> None:
-        _chk(lib().oracle_sub_sweep(self._h, int(checkerboard_set)))
+        _chk(self._L.oracle_sub_sweep(self._h, int(checkerboard_set)))
 
     def shift(self, direction: int, delta: float) -> None:
-        _chk(lib().oracle_shift(self._h, int(direction), float(delta)))
+        _chk(self._L.oracle_shift(self._h, int(direction), float(delta)))
 
     def get_positions(self) -> np.ndarray:
         out = np.full((self.N, 2), np.nan, dtype=np.float64)
-        _chk(lib().oracle_get_positions(self._h, out.ctypes.data))
+        _chk(self._L.oracle_get_positions(self._h, out.ctypes.data))
         return out
 
     def acceptance(self):
         o = (C.c_uint64 * 4)()
-        _chk(lib().oracle_acceptance(self._h, o))
+        _chk(self._L.oracle_acceptance(self._h, o))
         return tuple(int(v) for v in o)  # attempted, accepted, rej_boundary, rej_overlap
 
     def contact_histogram(self, dr: float, nbins: int) -> np.ndarray:
         h = np.zeros(nbins, dtype=np.uint64)
-        _chk(lib().oracle_contact_histogram(self._h, float(dr), int(nbins), h.ctypes.data))
+        _chk(self._L.oracle_contact_histogram(self._h, float(dr), int(nbins), h.ctypes.data))
         return h
 
     def pressure_contact(self, dr: float, nbins: int, degree: int):
@@ -192,10 +225,24 @@ class Oracle:
         origin = (C.c_double * 2)()
         t = C.c_uint64()
         dg = C.c_uint64()
-        _chk(lib().oracle_debug_state(self._h, counts.ctypes.data, slab.ctypes.data, ids.ctypes.data,
+        _chk(self._L.oracle_debug_state(self._h, counts.ctypes.data, slab.ctypes.data, ids.ctypes.data,
                                       mask.ctypes.data, origin, C.byref(t), C.byref(dg)))
         return dict(counts=counts, slab=slab, ids=ids, accept_mask=mask, origin=(origin[0], origin[1]),
                     sweep=int(t.value), digest=int(dg.value))
+
+
+class StripBaseline(Oracle):
+    """The OpenMP strip implementation of PAPER.md L390 (strip_omp.cpp): the oracle's Algorithms 2 and 4, one horizontal
+    strip of cells per thread.  Same calls, same trajectory bit for bit; `threads` = OpenMP threads (0: all cores)."""
+
+    def __init__(self, *args, threads: int = 0, **kw):
+        self._threads = int(threads)
+        super().__init__(*args, **kw)
+
+    def _create(self, b, sigma, d, n_s, seed, flags, w_target):
+        self._L = strip_lib()
+        _chk(self._L.strip_create(C.byref(self._h), self.N, b, sigma, d, n_s, seed, flags, w_target, self._threads))
+        self.threads = int(self._L.strip_threads())
 
 
 def g_of_r(hist: np.ndarray, N: int, L_eff, sigma: float, dr: float):

@@ -203,7 +203,18 @@ struct Sim : Base {
   }
 
   // ---- Algorithm 2: update of one active cell ------------------------------
+  // The move counters and the digest go to an accumulator the caller names (the cells of a set are independent, L48: the
+  // OpenMP strip baseline of L390, strip_omp.cpp, gives every thread its own); the plain form adds to the members.
+  struct Acc { uint64_t counters[4] = {0, 0, 0, 0}; uint64_t digest = 0; };
   void cell_update(uint32_t x, uint32_t y) {
+    Acc a;
+    cell_update(x, y, a);
+    for (int i = 0; i < 4; ++i) counters[i] += a.counters[i];
+    digest += a.digest;
+  }
+  void cell_update(uint32_t x, uint32_t y, Acc& acc) {
+    uint64_t (&counters)[4] = acc.counters;
+    uint64_t& digest = acc.digest;
     const size_t c = cell(x, y);
     const uint32_t nc = n[c];
     mask[c] = 0;
@@ -490,10 +501,10 @@ struct Sim : Base {
   double wx_d0 = 0, wy_d0 = 0;   // Lx/mx, Ly/my before rounding to P
 };
 
-template <typename P>
+template <typename P, typename SimT = Sim<P>>
 int make(Base** out, uint64_t N, const double box[2], double sigma, double d, uint32_t n_s, uint64_t seed,
          uint32_t flags, double w_target) {
-  Sim<P>* S = new (std::nothrow) Sim<P>();
+  SimT* S = new (std::nothrow) SimT();
   if (!S) return OR_ERR_ARG;
   S->N = N; S->n_s = n_s; S->seed = seed; S->flags = flags; S->sigma_d = sigma; S->d_d = d;
   S->sigma = (P)sigma; S->sigma2 = S->sigma * S->sigma; S->d = (P)d;
