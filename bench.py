@@ -116,6 +116,19 @@ def aggregate(dist, dev, ms_and_moves):
     return t.tolist() + m.tolist()
 
 
+def oracle_inputs(O, w):
+    """The workload's input for the CPU legs: no oracle input ever comes from the CUDA path, so a workload that starts
+    from a melted lattice (reading A15) is melted here by the oracle itself."""
+    xy, box = I.workload_inputs(w)
+    if w.melt:
+        prep = O.Oracle(w.N, box, w.sigma, w.d, w.n_s, 999, fp32=w.fp32, w_target=w.w_target, disc=w.disc)
+        prep.load_positions(xy)
+        while prep.acceptance()[0] < w.melt * w.N:
+            prep.sweep(10)
+        xy = prep.get_positions()
+    return xy, box
+
+
 def run_reference(args, w):
     """--impl reference: the oracle as it stands, single thread, on a bounded sample of the same workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -123,7 +136,7 @@ def run_reference(args, w):
         return
     from oracle import oracle as O
     O.build()
-    xy, box = I.workload_inputs(w)
+    xy, box = oracle_inputs(O, w)
     o = O.Oracle(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=w.fp32, w_target=w.w_target, disc=w.disc)
     o.load_positions(xy)
     sample_sweeps = max(1, args.ref_sweeps)
@@ -163,7 +176,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C3", choices=sorted(I.CONFIGS))
-    ap.add_argument("--sweeps", type=int, default=1000, help="sweeps per step (BASELINE.json C3: 1,000 sweeps)")
+    ap.add_argument("--sweeps", type=int, default=0, help="sweeps per step (0: the workload's own count; C3: 1,000)")
     ap.add_argument("--ref-sweeps", type=int, default=2, help="oracle sweeps per step for --impl reference")
     ap.add_argument("--cpu-baseline-sweeps", type=int, default=15)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -190,8 +203,15 @@ def main():
         dist = dist_mod
         dist.init_process_group("nccl", device_id=dev)
 
-    S = args.sweeps
+    S = args.sweeps if args.sweeps > 0 else w.sweeps
     xy_np, box = I.workload_inputs(w)
+    if w.melt:                                     # reading A15: the product melts the lattice (preparation seed 999)
+        prep = Mpmc(w.N, box, w.sigma, w.d, w.n_s, 999, fp32=w.fp32, device=dev, w_target=w.w_target, disc=w.disc)
+        prep.load_positions(torch.from_numpy(xy_np).to(dev))
+        while prep.acceptance()[0] < w.melt * w.N:
+            prep.sweep(10)
+        xy_np = prep.get_positions().cpu().numpy()
+        prep.close()
     xy_pinned = torch.from_numpy(xy_np).pin_memory()
     xy_dev = xy_pinned.to(dev)
     out_dev = torch.empty_like(xy_dev)
@@ -315,8 +335,9 @@ def main():
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import oracle as O
         O.build()
+        xy_cpu, _ = oracle_inputs(O, w)
         o = O.Oracle(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=w.fp32, w_target=w.w_target, disc=w.disc)
-        o.load_positions(xy_np)
+        o.load_positions(xy_cpu)
         o.sweep(1)
         a0 = o.acceptance()[0]
         t0 = time.perf_counter()
@@ -329,7 +350,7 @@ def main():
         # trajectory as the oracle bit for bit (checked here on the sample)
         O.build_strip()
         sb = O.StripBaseline(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=w.fp32, w_target=w.w_target, disc=w.disc)
-        sb.load_positions(xy_np)
+        sb.load_positions(xy_cpu)
         sb.sweep(1)
         b0 = sb.acceptance()[0]
         t0 = time.perf_counter()

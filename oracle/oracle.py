@@ -28,6 +28,7 @@ FP64 = 1
 FP32 = 2
 NO_PARTICLE_SHUFFLE = 8     # ablations of PAPER.md section 2.4 / Table 1 (L114-142)
 NO_SET_SHUFFLE = 16
+LEAVE_CELL = 32   # ablation of PAPER.md section 2.4 pitfall 1 (L118-122): disks may leave their cell during a sub-sweep (oracle only)
 DISC = 4      # trial displacement uniform in the disc of radius d instead of the square of reading A2
 
 ERR = {0: "ok", -1: "bad argument", -2: "box too small", -4: "overlap or out-of-box input",
@@ -152,14 +153,15 @@ class Oracle:
     """oracle_* calls with numpy host arrays.  Same call list as the product's `Mpmc` binding."""
 
     def __init__(self, N: int, box, sigma: float, d: float, n_s: int, seed: int, fp32: bool = False,
-                 w_target: float = 0.0, disc: bool = False, particle_shuffle: bool = True, set_shuffle: bool = True):
+                 w_target: float = 0.0, disc: bool = False, particle_shuffle: bool = True, set_shuffle: bool = True,
+                 leave_cell: bool = False):
         self._h = C.c_void_p()
         self.N = int(N)
         self.fp32 = bool(fp32)
         self.sigma = float(sigma)
         b = (C.c_double * 2)(float(box[0]), float(box[1]))
         flags = ((FP32 if fp32 else FP64) | (DISC if disc else 0) | (0 if particle_shuffle else NO_PARTICLE_SHUFFLE)
-                 | (0 if set_shuffle else NO_SET_SHUFFLE))
+                 | (0 if set_shuffle else NO_SET_SHUFFLE) | (LEAVE_CELL if leave_cell else 0))
         self._create(b, sigma, d, n_s, seed, flags, float(w_target))
         m = (C.c_uint32 * 2)()
         w = (C.c_double * 2)()

@@ -48,7 +48,11 @@ enum {
 };
 enum { OR_FP64 = 1u, OR_FP32 = 2u, OR_DISC = 4u,
        // ablations of PAPER.md section 2.4 / Table 1 (L114-142): leave out the particle shuffle / the checkerboard-set shuffle
-       OR_NO_PARTICLE_SHUFFLE = 8u, OR_NO_SET_SHUFFLE = 16u };   // OR_DISC: trial displacement uniform in the disc of radius d (L190)
+       OR_NO_PARTICLE_SHUFFLE = 8u, OR_NO_SET_SHUFFLE = 16u,
+       // pitfall 1 of section 2.4 (L118-122): a trial move whose centre leaves the cell is NOT rejected for that; the disk
+       // is handed to the cell it lands in (appended to that cell's list, L123).  The paper reports that this breaks
+       // detailed balance (the reverse sequence of moves cannot be generated); oracle-only ablation, see cell_update
+       OR_LEAVE_CELL = 32u };   // OR_DISC: trial displacement uniform in the disc of radius d (L190)
 
 // ---------------------------------------------------------------------------------------------
 // Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11): 10 rounds; multipliers 0xD2511F53, 0xCD9E8D57;
@@ -226,8 +230,14 @@ struct Sim : Base {
       fisher_yates(perm, nc, S);
     }
     uint32_t m = 0;
+    // OR_LEAVE_CELL only: where the disk that started in slot i sits now (slots close up behind a disk that left), -1 = left
+    int cur[NMAX] = {0, 1, 2, 3};
     for (uint32_t s = 0; s < n_s; ++s) {                        // line 11 (L189)
-      const uint32_t k = visit(perm, nc, s);
+      uint32_t k = visit(perm, nc, s);
+      if (flags & OR_LEAVE_CELL) {
+        if (cur[k] < 0) continue;                               // this disk has left the cell: nothing to move
+        k = (uint32_t)cur[k];
+      }
       uint32_t R[4];
       P ddx, ddy;
       if (!(flags & OR_DISC)) {
@@ -250,7 +260,41 @@ struct Sim : Base {
       const P My = ly[c * NMAX + k] + ddy;
       counters[0] += 1;
       if (!(inside(Mx, wx) && inside(My, wy))) {                // line 25 (L217), L79, L118
-        counters[2] += 1;
+        if (!(flags & OR_LEAVE_CELL)) {
+          counters[2] += 1;
+          continue;
+        }
+        // ---- ablation (L118-122): the disk may leave.  It lands in the adjacent cell (d < w), at N = M - e w in that
+        //      cell's frame; the Metropolis test is made there, against the 3x3 cells around the cell it lands in ----
+        const int ex = Mx > wx ? 1 : (Mx > (P)0 ? 0 : -1), ey = My > wy ? 1 : (My > (P)0 ? 0 : -1);
+        const P Nx = Mx - (P)ex * wx, Ny = My - (P)ey * wy;
+        const uint32_t xd = (uint32_t)(((int64_t)x + ex + mx) % mx), yd = (uint32_t)(((int64_t)y + ey + my) % my);
+        const size_t cd = cell(xd, yd);
+        const uint32_t nk = n[c];
+        if (n[cd] >= (uint32_t)NMAX || !(inside(Nx, wx) && inside(Ny, wy))) { counters[2] += 1; continue; }   // no room there
+        bool ov = false;
+        for (int oy = -1; oy <= 1; ++oy)
+          for (int ox = -1; ox <= 1; ++ox) {
+            const uint32_t xn = (uint32_t)(((int64_t)xd + ox + mx) % mx), yn = (uint32_t)(((int64_t)yd + oy + my) % my);
+            const size_t cn = cell(xn, yn);
+            const P sx = (P)ox * wx, sy = (P)oy * wy;
+            for (uint32_t j = 0; j < n[cn]; ++j) {
+              if (cn == c && j == k && (int)xn == (int)x && (int)yn == (int)y && ox == -ex && oy == -ey) continue;   // itself
+              if (overlaps(Nx, Ny, lx[cn * NMAX + j], ly[cn * NMAX + j], sx, sy)) ov = true;
+            }
+          }
+        if (ov) { counters[3] += 1; continue; }
+        const uint32_t moved_id = id[c * NMAX + k];
+        for (uint32_t j = k; j + 1 < nk; ++j) {                 // the list of the cell it leaves closes up
+          lx[c * NMAX + j] = lx[c * NMAX + j + 1]; ly[c * NMAX + j] = ly[c * NMAX + j + 1]; id[c * NMAX + j] = id[c * NMAX + j + 1];
+        }
+        lx[c * NMAX + nk - 1] = (P)0; ly[c * NMAX + nk - 1] = (P)0; id[c * NMAX + nk - 1] = 0xFFFFFFFFu;
+        n[c] = nk - 1;
+        for (int i = 0; i < NMAX; ++i) { if (cur[i] == (int)k) cur[i] = -1; else if (cur[i] > (int)k) cur[i] -= 1; }
+        lx[cd * NMAX + n[cd]] = Nx; ly[cd * NMAX + n[cd]] = Ny; id[cd * NMAX + n[cd]] = moved_id;   // added at the end (L123)
+        n[cd] += 1;
+        counters[1] += 1;
+        m |= (1u << (s & 31));
         continue;
       }
       bool overlap = false;                                     // line 13 (L193)

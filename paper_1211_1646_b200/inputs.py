@@ -37,6 +37,8 @@ class Workload:
     jitter: float = 0.05
     w_target: float = 0.0   # requested minimum cell width (0: smallest width >= sigma that divides the box)
     disc: bool = False      # trial displacement uniform in the disc of radius d instead of the square
+    melt: int = 0           # "melted for `melt` serial-equivalent sweeps" (BASELINE C5, reading A15): the caller runs the
+                            # method with preparation seed 999 until attempted >= melt * N before the measured run
 
     @property
     def N(self) -> int:
@@ -49,7 +51,7 @@ CONFIGS = {
     "C2": Workload("C2", 256, 0.70, 1.0, 0.10, 4, 1000, 1, fp32=False),
     "C3": Workload("C3", 1024, 0.716, 1.0, 0.08, 4, 1000, 1, fp32=True),
     "C4": Workload("C4", 4096, 0.720, 1.0, 0.06, 8, 200, 1, fp32=True),
-    "C5": Workload("C5", 1024, 0.30, 1.0, 0.5, 4, 1000, 1, fp32=True),
+    "C5": Workload("C5", 1024, 0.30, 1.0, 0.5, 4, 1000, 1, fp32=True, melt=100),
 }
 
 # The paper's own regime as a second workload: cell width just under sqrt(2) sigma (L152), disc-shaped

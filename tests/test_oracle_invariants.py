@@ -279,3 +279,67 @@ def test_without_set_shuffle_the_sets_run_in_order_abcd(oracle_mod):
         else:
             assert same
     assert differs or oracle_mod.sweep_draws(5, 0)[0] == [0, 1, 2, 3]
+
+
+# ---- ablation "disks may leave their cell" (section 2.4 pitfall 1, L118-122; oracle only) ----------------------
+def test_leave_cell_ablation_keeps_the_books_and_the_hard_core(oracle_mod):
+    """With the restriction of L118 lifted a move is never rejected for leaving the cell: the disk is handed to the cell
+    it lands in (appended to that list, L123) after a Metropolis test made THERE.  Fixed from outside: the disk count and
+    the ids are conserved, every local lies in (0, w], no overlap ever appears (independent KD-tree), no boundary
+    rejection is counted, and more moves are accepted than with the restriction."""
+    xy, box = I.jittered_lattice(64, 0.6, seed=4)
+    for fp32 in (False, True):
+        o = oracle_mod.Oracle(4096, box, 1.0, 0.3, 4, 9, fp32=fp32, leave_cell=True)
+        ref = oracle_mod.Oracle(4096, box, 1.0, 0.3, 4, 9, fp32=fp32)
+        o.load_positions(xy); ref.load_positions(xy)
+        eps = float(np.finfo(np.float32 if fp32 else np.float64).eps)
+        for _ in range(10):
+            o.sweep(4); ref.sweep(4)
+            check_state(o, o.debug_state())
+            assert min_pair_distance(o.get_positions(), o.L_eff) >= math.sqrt(1 - 4 * eps) - (0 if fp32 else 1e-12)
+        a, b = o.acceptance(), ref.acceptance()
+        assert a[0] == a[1] + a[3] and a[2] == 0 and b[2] > 0
+        assert a[1] / a[0] > b[1] / b[0] + 0.03
+        moved = np.abs(periodic_delta(o.get_positions(), xy, o.L_eff)).max()
+        assert moved > 1.0                                 # disks do travel across cells
+
+
+def test_leave_cell_ablation_isolated_disk_walks_freely(oracle_mod):
+    """N = 1: nothing to overlap with and no boundary to stop at, so every move is accepted and the disk performs a free
+    random walk: <|dr|^2> = T * 2 d^2 / 3 after T moves of U[-d, d]^2.  A wrong translation when the disk changes cell (a
+    lost or doubled +-w) would add jumps of a cell width and inflate this several-fold."""
+    L, d, n_s, sweeps = (6.4, 6.6), 0.4, 4, 30
+    msd, moves = [], []
+    for seed in range(120):
+        o = oracle_mod.Oracle(1, L, 1.0, d, n_s, 1000 + seed, leave_cell=True)
+        o.load_positions(np.array([[3.1, 3.3]]))
+        prev, total = o.get_positions()[0], np.zeros(2)
+        for _ in range(sweeps):
+            o.sweep(1)
+            p = o.get_positions()[0]
+            total += periodic_delta(p, prev, o.L_eff)          # at most n_s d = 1.6 per sweep, under L/2
+            prev = p
+        a = o.acceptance()
+        # every attempt is accepted; their number per sweep is no longer n_s: a cell update ends when its disk has left, and
+        # a disk that lands in a cell whose set runs later in the sweep is moved again (the state-dependent schedule the
+        # paper warns of, L118-122)
+        assert a[0] == a[1] and 0.5 * sweeps * n_s < a[0] < 2 * sweeps * n_s
+        msd.append((total ** 2).sum()); moves.append(a[1])
+    want = np.mean(moves) * 2 * d * d / 3
+    assert abs(np.mean(msd) / want - 1) < 0.25, (np.mean(msd), want)
+
+
+def test_leave_cell_ablation_coincides_with_the_method_until_a_disk_leaves(oracle_mod):
+    # same seed: the two chains are the same move for move until the first move that leaves its cell
+    o = oracle_mod.Oracle(1, (6.4, 6.6), 1.0, 0.05, 4, 5, leave_cell=True)
+    ref = oracle_mod.Oracle(1, (6.4, 6.6), 1.0, 0.05, 4, 5)
+    for s in (o, ref):
+        s.load_positions(np.array([[3.7, 3.8]]))
+    same = 0
+    for _ in range(400):
+        o.sub_sweep(0); ref.sub_sweep(0); o.sub_sweep(1); ref.sub_sweep(1); o.sub_sweep(2); ref.sub_sweep(2); o.sub_sweep(3); ref.sub_sweep(3)
+        if ref.acceptance()[2] > 0:
+            break
+        assert np.array_equal(o.get_positions(), ref.get_positions())
+        same += 1
+    assert same >= 3 and ref.acceptance()[2] > 0 and o.acceptance()[2] == 0
