@@ -70,6 +70,7 @@ struct Params {
   uint32_t track_crowded;    // 1: kernels that write cell counts list the cells with more than 2 disks (for tile.cuh)
   uint32_t hx_magic, hx_sh1, hx_sh2;  // ci / hx without a divide (Granlund-Montgomery; host: div_magic)
   uint32_t tl_ntx, tl_nty, tl_PS;       // tile kernel: tiles per axis, shared-memory plane stride (cells)
+  uint32_t tl_PH;                       // ... rows of the tallest tile's planes (sorted variant: stride of its row tables)
   uint32_t seed_lo, seed_hi;
   uint32_t rk0[10], rk1[10];            // Philox round keys seed + r * Weyl constant (philox4x32_10_rk)
   float wx_f, wy_f, sigma2_f, d_f;      // working-precision constants (fp32 mode)

@@ -44,6 +44,7 @@ namespace {
 
 constexpr size_t ALIGN = 256;
 constexpr uint32_t MAX_BINS = 4096;
+constexpr uint32_t SORT_MIN_PLANE = 1000;   // cells per shared-memory colour plane from which the sorted tile kernel is used
 
 inline size_t up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -132,8 +133,10 @@ int launch_sweeps(mpmc_ctx* c, unsigned long long t_end, uint32_t op, uint32_t a
 // Tiling of the tile kernel: ntx x nty tiles of (nearly) equal even size whose loaded region (tile + 2 HALO) fits
 // the shared memory of one SM; among those, the one with the least work on the busiest SM:
 // waves * cells of the largest region.  Returns false if no such tiling exists (boxes under 12 cells across).
+// row_bytes / pw_max: the sorted variant of the 2-slot kernel also needs row_bytes of shared memory per plane row and
+// plane rows of at most pw_max cells.
 bool choose_tiling(uint32_t hx, uint32_t hy, size_t cell_bytes, size_t smem_max, uint32_t sms, uint32_t* ntx, uint32_t* nty,
-                   uint32_t* PS) {
+                   uint32_t* PS, size_t row_bytes = 0, uint32_t pw_max = 0xFFFFFFFFu, uint32_t* PH = nullptr) {
   double best = 0; bool found = false;
   const uint32_t lim = 1024;
   for (uint32_t ax = 1; ax <= hx && ax <= lim; ++ax) {
@@ -142,11 +145,11 @@ bool choose_tiling(uint32_t hx, uint32_t hy, size_t cell_bytes, size_t smem_max,
     for (uint32_t ay = 1; ay <= hy && ay <= lim; ++ay) {
       const uint32_t TY = 2 * ((hy + ay - 1) / ay), ph = (TY + 2 * HALO) / 2;
       if (TY + 2 * HALO > 2 * hy) continue;
-      const size_t bytes = (size_t)4 * pw * ph * cell_bytes;
-      if (bytes > smem_max || pw * ph >= 16384u) continue;
+      const size_t bytes = (size_t)4 * pw * ph * cell_bytes + (size_t)4 * ph * row_bytes;
+      if (bytes > smem_max || pw * ph >= 16384u || pw > pw_max) continue;
       const double waves = std::ceil((double)ax * ay / sms);
       const double cost = waves * (double)(TX + 2 * HALO) * (TY + 2 * HALO) + 1e-6 * ax * ay;
-      if (!found || cost < best) { best = cost; found = true; *ntx = ax; *nty = ay; *PS = pw * ph; }
+      if (!found || cost < best) { best = cost; found = true; *ntx = ax; *nty = ay; *PS = pw * ph; if (PH) *PH = ph; }
     }
   }
   return found;
@@ -339,26 +342,35 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   const bool two_slot = c->nf == 2 && (n_s == 4 || n_s == 8) && !disc;
   c->tile_two_slot = two_slot;
   p.tune = 0u;
-  // dilute systems (fewer than 0.6 disks per cell): the tile kernel variant that compacts the non-empty cells
-  bool compact = (double)N < 0.6 * (double)p.mx * (double)p.my;
+  // the tile kernel variant that sorts the cells of a sweep into empty / simple / general ones (tile.cuh, SORTED)
+  bool compact = true;
 #ifdef MPMC_EXPERIMENT
   if (const char* e = std::getenv("MPMC_TUNE")) p.tune = (uint32_t)std::strtoul(e, nullptr, 0);
   if (const char* e = std::getenv("MPMC_COMPACT")) compact = e[0] == '1';
 #endif
   p.track_crowded = two_slot ? 1u : 0u;      // only the 2-slot tile kernel reads the list of crowded cells
-  const void* tk = two_slot ? (fp32 ? pick_tile_kernel_f32(debug, n_s, compact) : pick_tile_kernel_f64(debug, n_s, compact))
-                            : (fp32 ? pick_tile4_kernel_f32(debug, disc, n_s) : pick_tile4_kernel_f64(debug, disc, n_s));
-  if (tk) {
+  // the sorted variant of the 2-slot kernel first; the plain one if no tiling with plane rows of <= 64 cells fits
+  for (int attempt = 0; attempt < 2 && !c->tile_kernel; ++attempt) {
+    const bool sorted = two_slot && compact && attempt == 0;
+    if (attempt == 1 && !(two_slot && compact)) break;
+    const void* tk = two_slot ? (fp32 ? pick_tile_kernel_f32(debug, n_s, sorted) : pick_tile_kernel_f64(debug, n_s, sorted))
+                              : (fp32 ? pick_tile4_kernel_f32(debug, disc, n_s) : pick_tile4_kernel_f64(debug, disc, n_s));
+    if (!tk) break;
     int smem_optin = 0;
     cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    const size_t cell_bytes = (fp32 ? sizeof(SmemCell<float>) : sizeof(SmemCell<double>)) * (two_slot ? 1 : 2);
-    const size_t stat = (two_slot ? (fp32 ? sizeof(CrowdList<float>) : sizeof(CrowdList<double>)) : 0) + 256   // static shared memory
-                        + (two_slot && compact ? ((fp32 ? TileThreads<float>::value : TileThreads<double>::value) / 32) * 64 * sizeof(uint16_t) : 0);
+    // per cell of a shared-memory plane: the slot pair(s), and in the sorted 2-slot kernel one u16 queue entry
+    const size_t cell_bytes = (fp32 ? sizeof(SmemCell<float>) : sizeof(SmemCell<double>)) * (two_slot ? 1 : 2)
+                              + (sorted ? sizeof(uint16_t) : 0);
+    const size_t stat = (two_slot ? (fp32 ? sizeof(CrowdList<float>) : sizeof(CrowdList<double>)) : 0) + 512;   // static shared memory
     const size_t smem_max = (size_t)smem_optin > stat ? (size_t)smem_optin - stat : 0;
-    uint32_t ntx = 0, nty = 0, PS = 0;
+    uint32_t ntx = 0, nty = 0, PS = 0, PH = 0;
+    const size_t row_bytes = sorted ? SORT_ROW_BYTES : 0;
     c->tile_threads = two_slot ? (fp32 ? TileThreads<float>::value : TileThreads<double>::value)
                                : (fp32 ? Tile4Threads<float>::value : Tile4Threads<double>::value);
-    bool have = choose_tiling(p.hx, p.hy, cell_bytes, smem_max, (uint32_t)sms, &ntx, &nty, &PS);
+    bool have = choose_tiling(p.hx, p.hy, cell_bytes, smem_max, (uint32_t)sms, &ntx, &nty, &PS, row_bytes, sorted ? 64u : 0xFFFFFFFFu, &PH);
+    // the sort is a fixed cost of ~8 000 cycles per tile and sweep (measured, phase_clocks.py): it pays from about a
+    // thousand cells per colour plane on; smaller tiles (systems below ~2e5 cells) keep the plain variant
+    if (sorted && have && PS < SORT_MIN_PLANE) have = false;
 #ifdef MPMC_EXPERIMENT
     if (const char* e = std::getenv("MPMC_TILE")) {        // "ntx,nty,threads" (whole warps)
       unsigned a = 0, b = 0, th = 0;
@@ -371,8 +383,8 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
     if (have) {
       c->tile_kernel = tk;
       c->tile_grid = ntx * nty;
-      c->tile_smem = (size_t)4 * PS * cell_bytes;
-      p.tl_ntx = ntx; p.tl_nty = nty; p.tl_PS = PS;
+      c->tile_smem = (size_t)4 * PS * cell_bytes + (size_t)4 * PH * row_bytes;
+      p.tl_ntx = ntx; p.tl_nty = nty; p.tl_PS = PS; p.tl_PH = PH;
       // The attribute belongs to the kernel function, not to this context: set it to the most any tiling can ask for
       // (the opt-in maximum minus the kernel's static shared memory), so that live contexts with different tilings
       // of the same instantiation do not undo each other's setting.

@@ -40,6 +40,25 @@ template <typename P> struct TileThreads { static constexpr int value = sizeof(P
 constexpr int HALO = 5;
 constexpr int SHIFT_U = 4;              // cells per lane and chunk in the shift (their id loads are in flight together)
 
+// -DMPMC_PHASE_CLOCKS builds a variant that records clock64() at every phase boundary (phase_clocks.py).
+#ifdef MPMC_PHASE_CLOCKS
+constexpr uint32_t PHASE_TILES = 4096, PHASE_MARKS = 13;
+__device__ unsigned long long g_phase_clocks[PHASE_TILES][PHASE_MARKS];
+__device__ __forceinline__ unsigned long long globaltimer_ns() { unsigned long long v; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(v)); return v; }
+// (the clock is read AFTER a shared-memory load that follows the barrier: a bare clock read right behind __syncthreads is
+// issued before the barrier releases and would record this warp's arrival instead)
+__device__ __forceinline__ unsigned long long clock_after(const volatile uint32_t* s) {
+  const uint32_t v = *s; unsigned long long c;
+  asm volatile("mov.u64 %0, %%clock64;" : "=l"(c) : "r"(v) : "memory");
+  return c;
+}
+#define MPMC_PHASE_MARK_AT(i, mark_word) do { if (threadIdx.x == 0 && blockIdx.x < PHASE_TILES) g_phase_clocks[blockIdx.x][i] = (i) == 0 ? globaltimer_ns() : clock_after(mark_word); } while (0)
+#else
+#define MPMC_PHASE_MARK_AT(i, mark_word) do { } while (0)
+#endif
+
+#define MPMC_PHASE_MARK(i) MPMC_PHASE_MARK_AT(i, &s_last)
+
 // v in [-m, 2m) -> [0, m)
 __device__ __forceinline__ uint32_t wrap_cell(int v, uint32_t m) {
   if (v < 0) v += (int)m;
@@ -77,6 +96,8 @@ __device__ __forceinline__ void cp_async_cell(SmemCell<double>* dst, const doubl
 
 __device__ __forceinline__ float lds_x0(const SmemCell<float>* s, uint32_t i) { return s[i].v.x; }     // x of slot 0
 __device__ __forceinline__ double lds_x0(const SmemCell<double>* s, uint32_t i) { return s[i].a.x; }
+__device__ __forceinline__ float lds_x1(const SmemCell<float>* s, uint32_t i) { return s[i].v.y; }     // x of slot 1
+__device__ __forceinline__ double lds_x1(const SmemCell<double>* s, uint32_t i) { return s[i].a.y; }
 
 // Geometry of one tile: interior [x0, x0+TX) x [y0, y0+TY) in cells (all even), loaded region = interior grown
 // by HALO; shared-memory planes by LOCAL colour q = 2 (ly & 1) + (lx & 1), pw x ph cells each, stride PS.
@@ -322,6 +343,92 @@ __device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* s
   }
 }
 
+// The same with the local colour as a run-time value (the nine offsets computed once per sub-sweep): one copy serves the
+// four sub-sweeps of the SORTED variant.
+template <typename P, int NS, bool DEBUG>
+__device__ __forceinline__ void tile_update_cell_rt(const Params& p, SmemCell<P>* sm, const uint32_t si_own,
+                                                    const int (&noff)[9], const uint32_t cell, const bool interior,
+                                                 const unsigned long long t, Tally& tally) {
+  using R = Real<P>;
+  using Pair = typename R::Pair;
+  Half<P> h[9];
+  const SmemCell<P>* own = sm + si_own;            // the nine offsets are uniform per sub-sweep
+#pragma unroll
+  for (int idx = 0; idx < 9; ++idx) h[idx] = lds_half(own + noff[idx], 0u);
+  // ---- displacements of all NS moves from the GLOBAL cell id (line 12, L190; A2, A9) ----
+  const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
+  P ddx[NS], ddy[NS];
+#pragma unroll
+  for (int b = 0; b < NS / 2; ++b) {
+    uint32_t Rw[4];
+    philox4x32_10_rk(p, cell, t_lo, t_hi, (uint32_t)b, Rw);
+    ddx[2 * b] = R::scaled_sym(p, Rw[0]); ddy[2 * b] = R::scaled_sym(p, Rw[1]);
+    ddx[2 * b + 1] = R::scaled_sym(p, Rw[2]); ddy[2 * b + 1] = R::scaled_sym(p, Rw[3]);
+  }
+  const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p);
+  const P HALF_FAR = R::far_away() * (P)0.5;
+  const Pair MINUS1 = R::pair((P)-1, (P)-1);
+  // ---- neighbours, translated into this cell's frame and negated: -(l_j + s) = fma(l_j, -1, -s) ----
+  Pair nqx[8], nqy[8];
+#pragma unroll
+  for (int idx = 0; idx < 9; ++idx) {
+    if (idx == 4) continue;
+    const int e = idx < 4 ? idx : idx - 1;
+    const int ox = idx % 3 - 1, oy = idx / 3 - 1;
+    const P nsx = ox < 0 ? wx : ox > 0 ? -wx : (P)0;
+    const P nsy = oy < 0 ? wy : oy > 0 ? -wy : (P)0;
+    nqx[e] = R::pfma(h[idx].x, MINUS1, R::pair(nsx, nsx));
+    nqy[e] = R::pfma(h[idx].y, MINUS1, R::pair(nsy, nsy));
+  }
+  // ---- own cell in visiting order (Alg. 2 lines 8-9, L186-187); a slot is empty iff it holds the sentinel ----
+  P Ax = h[4].x.x, Ay = h[4].y.x, Bx = h[4].x.y, By = h[4].y.y;
+  const uint32_t n = Bx < HALF_FAR ? 2u : (Ax < HALF_FAR ? 1u : 0u);
+  const bool two = n == 2u;
+  bool flip = false;                   // true: A is slot 1
+  if (two) {                           // n = 2: Fisher-Yates is one draw, j = bounded(S0, 2); j = 0 swaps
+    uint32_t S[4];
+    philox4x32_10_rk(p, cell, t_lo, t_hi, SLOT_SHUFFLE, S);
+    flip = bounded(S[0], 2u) == 0u && !(p.flags & FLAG_NO_PARTICLE_SHUFFLE);
+  }
+  if (flip) { P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }
+  uint32_t amask = 0, bmask = 0;       // bit s: move s accepted / left the cell
+#pragma unroll
+  for (int s = 0; s < NS; ++s) {       // Alg. 2 lines 11-32 (L189-230)
+    const P Mx = R::add(Ax, ddx[s]), My = R::add(Ay, ddy[s]);              // D_move = l + displacement
+    const bool inside = (Mx > (P)0) && (Mx <= wx) && (My > (P)0) && (My <= wy);   // (0, w]  (A3; L79, L118)
+    const P Dbx = R::sub(Mx, Bx), Dby = R::sub(My, By);                    // the other own disk (s = 0)
+    P rmin = R::fma(Dbx, Dbx, R::mul(Dby, Dby));
+    const Pair MMx = R::pair(Mx, Mx), MMy = R::pair(My, My);
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {                                          // |D_move - (D + s)|^2  (line 19, L204)
+      const Pair Dx = R::padd(MMx, nqx[e]), Dy = R::padd(MMy, nqy[e]);
+      const Pair r2 = R::pfma(Dx, Dx, R::pmul(Dy, Dy));
+      rmin = R::min3(rmin, r2.x, r2.y);
+    }
+    const bool acc = inside && !(rmin < sigma2);                           // strict (A4)
+    if (acc) { Ax = Mx; Ay = My; amask |= 1u << s; }                       // lines 24-27 (L215-222)
+    if (!inside) bmask |= 1u << s;                                         // leaves the cell: rejected (L79, L118)
+    if (two) { const P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }   // s mod n cycling (L75)
+  }
+  if (n == 0u) amask = 0u;             // empty cells attempt nothing (A10)
+  const uint32_t n_acc = __popc(amask), n_rb = __popc(bmask);
+  if (amask != 0u) {                   // write back (line 34, L234): the slot pair in slot order
+    if (two && (NS & 1)) flip = !flip;
+    Half<P> o;
+    o.x = flip ? R::pair(Bx, Ax) : R::pair(Ax, Bx);
+    o.y = flip ? R::pair(By, Ay) : R::pair(Ay, By);
+    sts_half(sm, si_own, o);
+  }
+  // tallies, accept masks and the digest count every cell once: in the tile that owns it
+  if (interior && n > 0u) {
+    tally.acc += n_acc; tally.rb += n_rb; tally.ro += (uint32_t)NS - n_acc - n_rb;
+  }
+  if (DEBUG && interior) {
+    p.mask[cell] = amask;
+    if (n > 0u) atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)cell << 32) | amask)));
+  }
+}
+
 // General shift of one interior cell (rare: it or its source neighbour is crowded): Algorithm 4 with up to 4 disks
 // in each of the two old cells.  Straight-line code on registers (eight candidates, four output slots filled by
 // prefix count), because the whole tile waits for the thread that runs it.
@@ -391,65 +498,257 @@ __device__ __forceinline__ void tile_sub_sweep_cells(const Params& p, SmemCell<P
   }
 }
 
-// The same for dilute systems (most cells empty, e.g. BASELINE config C5: 62 % at phi = 0.30): an empty cell attempts
-// nothing (A10), so running the update on it wastes the lane.  Each warp scans its chunks, queues the indices of the
-// NON-EMPTY cells in a private shared-memory queue (ballot + prefix count) and runs the update on full warps of them.
-template <typename P, int NS, bool DEBUG, uint32_t QL>
-__device__ __forceinline__ void tile_sub_sweep_cells_compact(const Params& p, SmemCell<P>* sm, const CrowdList<P>& cl,
-                                                             const uint32_t nc, const TileBox& tb, const uint32_t k,
-                                                             const uint32_t dir, const int gx0, const int gy0,
-                                                             const unsigned long long t, uint32_t* next, uint16_t* wq,
-                                                             Tally& tally) {
-  constexpr uint32_t qx = QL & 1u, qy = QL >> 1;
-  const uint32_t PS = p.tl_PS, pw = tb.pw;
+// ---------------------------------------------------------------------------------------------------------
+// SORTED variant of the sub-sweeps.  The packed overlap test of tile_update_cell spends half of its lanes on slot 1 of
+// the neighbour cells, which is empty in 96.5 % of them (w ~ sigma, phi = 0.716), and every warp pays the shuffle's
+// Philox block as soon as one of its 32 cells holds two disks.  Occupancies do not change during the sub-sweeps (a move
+// never leaves its cell), so ONCE per sweep, right after the load, the cells of the four sub-sweeps are sorted into
+// three classes:
+//   empty                       attempt nothing (A10): dropped — 11 % of the cells at phi = 0.716, 62 % at phi = 0.30;
+//   simple  (61 % at C3)        one disk, and no cell of the 3x3 neighbourhood holds two: tile_update_simple tests the
+//                               eight neighbour disks as FOUR packed pairs (slot 0 of two cells per pair), draws no shuffle
+//                               word (Fisher-Yates of one element draws nothing, L187) and has no second own disk;
+//   general (28 %)              everything else with at most two disks per cell: tile_update_cell as before.
+// Cells next to a crowded cell stay with tile_update_cell_warp.  Each sub-sweep then runs on FULL warps of like cells.
+// The sort has no atomics: the warps are dealt (sub-sweep, segment) jobs, a segment being a contiguous run of 32-cell
+// chunks of the sub-sweep's rectangle; a job writes the plane indices of its simple cells upward from the start of its
+// stretch of the sub-sweep's queue and of its general cells downward from the end, and leaves its two counts in shared
+// memory.  A sub-sweep hands out batches of 32 entries, the general ones first, from one shared counter.
+// ---------------------------------------------------------------------------------------------------------
+// How the sort works (no per-cell arithmetic, no contended atomics): a plane row is at most 64 cells wide (the host sorts
+// only such tilings), so the occupancy of a row is two 64-bit masks — bit px of occ / two: the cell holds >= 1 / 2 disks —
+// taken with two ballots per row (phase A).  "A cell of the 3x3 neighbourhood holds two disks" is then nine shifted
+// ORs of row masks, evaluated once per ROW of a sub-sweep's rectangle (phase B), which yields the row's simple and
+// general masks; a prefix sum over the rows (phase C) places every row in the sub-sweep's queue, simple cells from the
+// front, general cells from the back, and phase D writes the plane indices.  Phases end at __syncthreads().
+struct QueueRect { uint32_t px_lo, px_hi, py_lo, py_hi; };     // plane coordinates of a sub-sweep's rectangle (inclusive)
+__device__ __forceinline__ QueueRect queue_rect(const TileBox& tb, const uint32_t k, const uint32_t dir, const uint32_t q) {
+  const uint32_t qx = q & 1u, qy = q >> 1;
   const SubRect rc = sub_sweep_rect(tb, k, dir);
-  const uint32_t px0 = (rc.x_lo - qx + 1u) >> 1, px1 = (rc.x_hi - qx) >> 1;
-  const uint32_t py0 = (rc.y_lo - qy + 1u) >> 1, py1 = (rc.y_hi - qy) >> 1;
-  const uint32_t nxp = px1 - px0 + 1u, count = nxp * (py1 - py0 + 1u);
-  const uint32_t inv = small_div_magic(nxp);
-  const uint32_t lane = threadIdx.x & 31u;
+  QueueRect g;
+  g.px_lo = (rc.x_lo - qx + 1u) >> 1; g.py_lo = (rc.y_lo - qy + 1u) >> 1;
+  g.px_hi = (rc.x_hi - qx) >> 1; g.py_hi = (rc.y_hi - qy) >> 1;
+  return g;
+}
+// shared-memory work area of the sort, behind the queues: per plane row (q or sub-sweep k, row py) at index 4 * PH
+struct SortArea {
+  unsigned long long *occ, *two, *simple, *general;   // [4][PH]
+  uint16_t *base1, *base2;                            // [4][PH]: queue position of the row's first simple / general cell
+};
+__device__ __forceinline__ SortArea sort_area(void* mem, const uint32_t PH) {
+  SortArea a;
+  a.occ = reinterpret_cast<unsigned long long*>(mem); a.two = a.occ + 4u * PH; a.simple = a.two + 4u * PH; a.general = a.simple + 4u * PH;
+  a.base1 = reinterpret_cast<uint16_t*>(a.general + 4u * PH); a.base2 = a.base1 + 4u * PH;
+  return a;
+}
+constexpr uint32_t SORT_ROW_BYTES = 4u * 8u + 2u * 2u;   // per plane row: four masks and two bases
+
+__device__ __forceinline__ float2 lds_x01(const SmemCell<float>* s, uint32_t i) { return make_float2(s[i].v.x, s[i].v.y); }
+__device__ __forceinline__ double2 lds_x01(const SmemCell<double>* s, uint32_t i) { return s[i].a; }
+// T[px + a] as a mask over px, a in {-1, 0, +1}
+__device__ __forceinline__ unsigned long long mask_shift(const unsigned long long T, const int a) { return a < 0 ? T << 1 : a > 0 ? T >> 1 : T; }
+
+template <typename P, bool DEBUG>
+__device__ __forceinline__ void tile_sort_cells(const Params& p, const SmemCell<P>* sm, const CrowdList<P>& cl, const uint32_t nc,
+                                                const TileBox& tb, const Draws& dr, const int gx0, const int gy0,
+                                                uint16_t* queues, const SortArea sa, uint32_t (*s_cnt)[2]) {
+  const uint32_t PS = p.tl_PS, PH = p.tl_PH, pw = tb.pw, ph = tb.ph;
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, NW = blockDim.x >> 5;
   const P HALF_FAR = Real<P>::far_away() * (P)0.5;
-  uint32_t qn = 0;                                             // queued cells (warp-uniform)
-  bool more = true;
-  while (more || qn > 0u) {
-    if (more) {                                                // scan one chunk of 32 cells
-      uint32_t base = 0;
-      if (lane == 0u) base = atomicAdd(next, 32u);
-      base = __shfl_sync(0xFFFFFFFFu, base, 0);
-      more = base < count;
-      const uint32_t idx = base + lane;
-      bool occ = false;
-      if (more && idx < count) {
-        const uint32_t ry = small_div(idx, inv), rx = idx - ry * nxp;
-        const uint32_t px = px0 + rx, py = py0 + ry, lx = 2u * px + qx, ly = 2u * py + qy;
-        if (!(nc != 0u && crowd_near(cl, nc, lx, ly))) {       // else: done by a warp (tile_update_cell_warp)
-          occ = lds_x0(sm, QL * PS + py * pw + px) < HALF_FAR; // slots fill in order: slot 0 empty = cell empty
-          if (DEBUG && !occ && lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY)
+  const uint32_t inv_ph = small_div_magic(ph);
+  // ---- A: occupancy masks of every plane row ----
+  for (uint32_t r = warp; r < 4u * ph; r += NW) {
+    const uint32_t q = small_div(r, inv_ph), py = r - q * ph;
+    unsigned long long occ = 0ull, two = 0ull;
+#pragma unroll
+    for (uint32_t half = 0; half < 2u; ++half) {
+      const uint32_t px = lane + 32u * half;
+      bool o = false, w2 = false;
+      if (px < pw) {
+        const auto x = lds_x01(sm, q * PS + py * pw + px);     // slots fill in order
+        o = x.x < HALF_FAR; w2 = x.y < HALF_FAR;
+        if (DEBUG && !o) {                                       // an empty cell of the tile: nothing accepted
+          const uint32_t lx = 2u * px + (q & 1u), ly = 2u * py + (q >> 1);
+          if (lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY)
             p.mask[wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx)] = 0u;
         }
       }
-      const uint32_t m = __ballot_sync(0xFFFFFFFFu, occ);
-      if (occ) wq[qn + __popc(m & ((1u << lane) - 1u))] = (uint16_t)idx;
-      qn += __popc(m);
-      __syncwarp();
+      occ |= (unsigned long long)__ballot_sync(0xFFFFFFFFu, o) << (32u * half);
+      two |= (unsigned long long)__ballot_sync(0xFFFFFFFFu, w2) << (32u * half);
     }
-    if (qn >= 32u || (!more && qn > 0u)) {                     // a full warp of non-empty cells (or the last few)
-      const uint32_t take = qn < 32u ? qn : 32u;
-      const uint32_t mine = wq[lane], rest = wq[lane + 32u];
-      __syncwarp();
-      if (lane + 32u < qn) wq[lane] = (uint16_t)rest;          // keep the overflow at the front of the queue
-      qn -= take;
-      if (lane < take) {
-        const uint32_t idx = mine;
-        const uint32_t ry = small_div(idx, inv), rx = idx - ry * nxp;
-        const uint32_t px = px0 + rx, py = py0 + ry, lx = 2u * px + qx, ly = 2u * py + qy;
-        const uint32_t si = QL * PS + py * pw + px;
-        const uint32_t cell = wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx);
-        const bool interior = lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY;
-        tile_update_cell<P, NS, DEBUG, QL>(p, sm, si, pw, cell, interior, t, tally);
+    if (lane == 0u) { sa.occ[q * PH + py] = occ; sa.two[q * PH + py] = two; }
+  }
+  __syncthreads();
+  MPMC_PHASE_MARK_AT(9, &s_cnt[0][0]);
+  // cells next to a crowded cell are nobody's here: a whole warp does them (tile_update_cell_warp)
+  for (uint32_t i = tid; i < 9u * nc; i += blockDim.x) {
+    const uint32_t e = i / 9u, d = i - 9u * e;
+    const uint32_t lx = (cl.e[e].lxly & 0xFFFFu) + d % 3u - 1u, ly = (cl.e[e].lxly >> 16) + d / 3u - 1u;   // may wrap below 0
+    if (lx < tb.w && ly < tb.h)
+      atomicAnd(&sa.occ[(((ly & 1u) << 1) | (lx & 1u)) * PH + (ly >> 1)], ~(1ull << (lx >> 1)));
+  }
+  __syncthreads();
+  // ---- B + C: one warp per sub-sweep, one LANE per row: the row's simple and general cells (nine shifted ORs of row
+  //      masks), then the exclusive prefix sums over the rows that place every row in the sub-sweep's queue ----
+  if (warp < 4u) {
+    const uint32_t k = warp;
+    const uint32_t Qg = k == 0u ? dr.order[0] : k == 1u ? dr.order[1] : k == 2u ? dr.order[2] : dr.order[3];
+    const uint32_t q = Qg ^ 3u;                          // the region starts at an odd cell: colours flip
+    const int qx = (int)(q & 1u), qy = (int)(q >> 1);
+    const QueueRect g = queue_rect(tb, k + 1u, dr.dir, q);
+    const unsigned long long in = (~0ull >> (63u - g.px_hi)) & (~0ull << g.px_lo);
+    const unsigned long long* T = sa.two;
+    const uint32_t q1 = q ^ 1u, q2 = q ^ 2u, q3 = q ^ 3u;
+    uint32_t run1 = 0, run2 = 0;
+    for (uint32_t r0 = 0; r0 < ph; r0 += 32u) {
+      const uint32_t py = r0 + lane;
+      unsigned long long simple = 0ull, general = 0ull;
+      if (py >= g.py_lo && py <= g.py_hi) {
+        const uint32_t ra = py + (uint32_t)qy - 1u, rb = py + (uint32_t)qy;   // the plane rows of the cells below / above
+        unsigned long long c = T[q * PH + py];
+        c |= mask_shift(T[q1 * PH + py], qx - 1) | mask_shift(T[q1 * PH + py], qx);
+        c |= T[q2 * PH + ra] | T[q2 * PH + rb];
+        c |= mask_shift(T[q3 * PH + ra], qx - 1) | mask_shift(T[q3 * PH + ra], qx);
+        c |= mask_shift(T[q3 * PH + rb], qx - 1) | mask_shift(T[q3 * PH + rb], qx);
+        const unsigned long long o = sa.occ[q * PH + py] & in;
+        simple = o & ~c; general = o & c;
       }
-      __syncwarp();
+      const uint32_t n1 = (uint32_t)__popcll(simple), n2 = (uint32_t)__popcll(general);
+      uint32_t i1 = n1, i2 = n2;
+#pragma unroll
+      for (uint32_t d = 1; d < 32u; d <<= 1) {
+        const uint32_t v1 = __shfl_up_sync(0xFFFFFFFFu, i1, d), v2 = __shfl_up_sync(0xFFFFFFFFu, i2, d);
+        if (lane >= d) { i1 += v1; i2 += v2; }
+      }
+      if (py < ph) {
+        sa.simple[k * PH + py] = simple; sa.general[k * PH + py] = general;
+        sa.base1[k * PH + py] = (uint16_t)(run1 + i1 - n1); sa.base2[k * PH + py] = (uint16_t)(run2 + i2 - n2);
+      }
+      run1 += __shfl_sync(0xFFFFFFFFu, i1, 31); run2 += __shfl_sync(0xFFFFFFFFu, i2, 31);
     }
+    if (lane == 0u) { s_cnt[k][0] = run1; s_cnt[k][1] = run2; }
+  }
+  __syncthreads();
+  MPMC_PHASE_MARK_AT(10, &s_cnt[0][0]);
+  // ---- D: the plane indices, a warp per row, a lane per cell: simple cells from the front of the sub-sweep's queue,
+  //      general cells from its back ----
+  for (uint32_t r = warp; r < 4u * ph; r += NW) {
+    const uint32_t k = small_div(r, inv_ph), py = r - k * ph;
+    const unsigned long long m1 = sa.simple[k * PH + py], m2 = sa.general[k * PH + py];
+    if ((m1 | m2) == 0ull) continue;
+    uint16_t* qk = queues + k * PS;
+    uint32_t at1 = sa.base1[k * PH + py], at2 = PS - 1u - sa.base2[k * PH + py];
+    const uint32_t below = (1u << lane) - 1u;
+#pragma unroll
+    for (uint32_t half = 0; half < 2u; ++half) {
+      const uint32_t w1 = (uint32_t)(m1 >> (32u * half)), w2 = (uint32_t)(m2 >> (32u * half));
+      const uint32_t v = py * pw + lane + 32u * half;
+      if ((w1 >> lane) & 1u) qk[at1 + (uint32_t)__popc(w1 & below)] = (uint16_t)v;
+      if ((w2 >> lane) & 1u) qk[at2 - (uint32_t)__popc(w2 & below)] = (uint16_t)v;
+      at1 += (uint32_t)__popc(w1); at2 -= (uint32_t)__popc(w2);
+    }
+  }
+  __syncthreads();
+}
+
+// A simple cell (see above): one disk, no second disk anywhere in the 3x3 cells.  Same arithmetic per disk as
+// tile_update_cell — q = fma(l_j, -1, -s), D = M + (-q), r^2 = fma(Dx, Dx, Dy Dy), overlap iff r^2 < sigma^2 — on half as
+// many packed instructions: the two lanes of a pair are slot 0 of two different neighbour cells.  The slots left out
+// hold the sentinel, whose r^2 ~ 1e36 never decides the minimum.
+template <typename P, int NS, bool DEBUG>
+__device__ __forceinline__ void tile_update_simple(const Params& p, SmemCell<P>* sm, const uint32_t si_own, const int (&noff)[9],
+                                                   const uint32_t cell, const bool interior, const unsigned long long t,
+                                                   Tally& tally) {
+  using R = Real<P>;
+  using Pair = typename R::Pair;
+  Half<P> h[9];
+  const SmemCell<P>* own = sm + si_own;
+#pragma unroll
+  for (int idx = 0; idx < 9; ++idx) h[idx] = lds_half(own + noff[idx], 0u);
+  const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
+  P ddx[NS], ddy[NS];
+#pragma unroll
+  for (int b = 0; b < NS / 2; ++b) {                   // displacements of all NS moves (line 12, L190; A2, A9)
+    uint32_t Rw[4];
+    philox4x32_10_rk(p, cell, t_lo, t_hi, (uint32_t)b, Rw);
+    ddx[2 * b] = R::scaled_sym(p, Rw[0]); ddy[2 * b] = R::scaled_sym(p, Rw[1]);
+    ddx[2 * b + 1] = R::scaled_sym(p, Rw[2]); ddy[2 * b + 1] = R::scaled_sym(p, Rw[3]);
+  }
+  const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p);
+  // slot 0 of the eight neighbour cells, translated into this cell's frame and negated, two cells per pair
+  Pair nqx[4], nqy[4];
+  {
+    P qx[8], qy[8];
+#pragma unroll
+    for (int idx = 0; idx < 9; ++idx) {
+      if (idx == 4) continue;
+      const int e = idx < 4 ? idx : idx - 1;
+      const int ox = idx % 3 - 1, oy = idx / 3 - 1;
+      const P nsx = ox < 0 ? wx : ox > 0 ? -wx : (P)0;
+      const P nsy = oy < 0 ? wy : oy > 0 ? -wy : (P)0;
+      qx[e] = R::fma(h[idx].x.x, (P)-1, nsx);          // -(l_j + s) = fma(l_j, -1, -s): one rn operation (L154, L196)
+      qy[e] = R::fma(h[idx].y.x, (P)-1, nsy);
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { nqx[j] = R::pair(qx[2 * j], qx[2 * j + 1]); nqy[j] = R::pair(qy[2 * j], qy[2 * j + 1]); }
+  }
+  P Ax = h[4].x.x, Ay = h[4].y.x;
+  uint32_t amask = 0, bmask = 0;
+#pragma unroll
+  for (int s = 0; s < NS; ++s) {                       // Alg. 2 lines 11-32 (L189-230) with n = 1
+    const P Mx = R::add(Ax, ddx[s]), My = R::add(Ay, ddy[s]);
+    const bool inside = (Mx > (P)0) && (Mx <= wx) && (My > (P)0) && (My <= wy);   // (0, w]  (A3; L79, L118)
+    const Pair MMx = R::pair(Mx, Mx), MMy = R::pair(My, My);
+    P rmin = R::far_away();
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {                      // |D_move - (D + s)|^2  (line 19, L204)
+      const Pair Dx = R::padd(MMx, nqx[j]), Dy = R::padd(MMy, nqy[j]);
+      const Pair r2 = R::pfma(Dx, Dx, R::pmul(Dy, Dy));
+      rmin = R::min3(rmin, r2.x, r2.y);
+    }
+    const bool acc = inside && !(rmin < sigma2);       // strict (A4)
+    if (acc) { Ax = Mx; Ay = My; amask |= 1u << s; }
+    if (!inside) bmask |= 1u << s;
+  }
+  const uint32_t n_acc = __popc(amask), n_rb = __popc(bmask);
+  if (amask != 0u) {                                   // write back (line 34, L234); slot 1 keeps its sentinel
+    Half<P> o;
+    o.x = R::pair(Ax, h[4].x.y); o.y = R::pair(Ay, h[4].y.y);
+    sts_half(sm, si_own, o);
+  }
+  if (interior) { tally.acc += n_acc; tally.rb += n_rb; tally.ro += (uint32_t)NS - n_acc - n_rb; }
+  if (DEBUG && interior) {
+    p.mask[cell] = amask;
+    atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)cell << 32) | amask)));
+  }
+}
+
+// One sub-sweep of the SORTED variant: batches of 32 queued cells, the general ones first (they take longer).
+template <typename P, int NS, bool DEBUG>
+__device__ __forceinline__ void tile_run_sorted(const Params& p, SmemCell<P>* sm, const TileBox& tb, const uint32_t q,
+                                                const int gx0, const int gy0, const unsigned long long t,
+                                                const uint16_t* qk, const uint32_t n_simple, const uint32_t n_general,
+                                                uint32_t* next, Tally& tally) {
+  const uint32_t PS = p.tl_PS, pw = tb.pw, lane = threadIdx.x & 31u;
+  const uint32_t qx = q & 1u, qy = q >> 1, inv_pw = small_div_magic(pw);
+  int noff[9];
+#pragma unroll
+  for (int idx = 0; idx < 9; ++idx) noff[idx] = neighbour_offset(q, idx % 3 - 1, idx / 3 - 1, PS, pw);
+  const uint32_t total2 = (n_general + 31u) >> 5, total = total2 + ((n_simple + 31u) >> 5);
+  for (;;) {
+    uint32_t b = 0;
+    if (lane == 0u) b = atomicAdd(next, 1u);
+    b = __shfl_sync(0xFFFFFFFFu, b, 0);
+    if (b >= total) break;
+    const bool general = b < total2;
+    const uint32_t e = 32u * (general ? b : b - total2) + lane;
+    if (e >= (general ? n_general : n_simple)) continue;
+    const uint32_t v = general ? qk[PS - 1u - e] : qk[e];
+    const uint32_t py = small_div(v, inv_pw), px = v - py * pw, lx = 2u * px + qx, ly = 2u * py + qy;
+    const uint32_t cell = wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx);
+    const bool interior = lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY;
+    if (general) tile_update_cell_rt<P, NS, DEBUG>(p, sm, q * PS + v, noff, cell, interior, t, tally);
+    else         tile_update_simple<P, NS, DEBUG>(p, sm, q * PS + v, noff, cell, interior, t, tally);
   }
 }
 
@@ -560,24 +859,7 @@ __device__ __forceinline__ void tile_shift_cells(const Params& p, const SmemCell
 // The fused sweep kernel: one CTA per tile, one launch per sweep.  See the header of this file.
 // Dynamic shared memory: 4 planes x tl_PS cells x sizeof(SmemCell<P>).
 // ---------------------------------------------------------------------------------------------------------
-// -DMPMC_PHASE_CLOCKS builds a variant that records clock64() at every phase boundary (phase_clocks.py).
-#ifdef MPMC_PHASE_CLOCKS
-constexpr uint32_t PHASE_TILES = 4096, PHASE_MARKS = 9;
-__device__ unsigned long long g_phase_clocks[PHASE_TILES][PHASE_MARKS];
-__device__ __forceinline__ unsigned long long globaltimer_ns() { unsigned long long v; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(v)); return v; }
-// (the clock is read AFTER a shared-memory load that follows the barrier: a bare clock read right behind __syncthreads is
-// issued before the barrier releases and would record this warp's arrival instead)
-__device__ __forceinline__ unsigned long long clock_after(const volatile uint32_t* s) {
-  const uint32_t v = *s; unsigned long long c;
-  asm volatile("mov.u64 %0, %%clock64;" : "=l"(c) : "r"(v) : "memory");
-  return c;
-}
-#define MPMC_PHASE_MARK(i) do { if (threadIdx.x == 0 && blockIdx.x < PHASE_TILES) g_phase_clocks[blockIdx.x][i] = (i) == 0 ? globaltimer_ns() : clock_after(&s_last); } while (0)
-#else
-#define MPMC_PHASE_MARK(i) do { } while (0)
-#endif
-
-template <typename P, int NS, bool DEBUG, bool COMPACT = false>
+template <typename P, int NS, bool DEBUG, bool SORTED = false>
 __global__ void __launch_bounds__(TileThreads<P>::value, 1)
 k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   using R = Real<P>;
@@ -587,7 +869,7 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   __shared__ CrowdList<P> cl;
   __shared__ uint32_t s_last;
   __shared__ uint32_t s_next[8];                 // chunk counters: sub-sweeps 1-4, shift planes 0-3
-  __shared__ uint16_t s_queue[COMPACT ? (TileThreads<P>::value / 32) * 64 : 1];   // per-warp queues of non-empty cells
+  __shared__ uint32_t s_cnt[4][2];               // SORTED: simple / general cells queued per sub-sweep
   Ctl* ctl = p.ctl;
   // The sweep index comes as a kernel argument (the host counts launches), so the draws of this sweep — a pure function
   // of (seed, t), Alg. 1 lines 2, 15, 16 (L64, L90-91) — and all they decide are warp-uniform values computed before the
@@ -644,8 +926,11 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
     asm volatile("cp.async.wait_all;" ::: "memory");
   }
   __syncthreads();
-  MPMC_PHASE_MARK(2);
   const uint32_t nc = cl.n;
+  // SORTED: the queues of the four sub-sweeps (behind the planes in dynamic shared memory, one plane's worth of u16 each)
+  uint16_t* queues = reinterpret_cast<uint16_t*>(sm + 4u * PS);
+  if (SORTED) tile_sort_cells<P, DEBUG>(p, sm, cl, nc, tb, dr, gx0, gy0, queues, sort_area(queues + 4u * PS, p.tl_PH), s_cnt);
+  MPMC_PHASE_MARK(2);
   Tally tally;
 
   // ---- four sub-sweeps (Alg. 1 lines 3-14, L66-88): sub-sweep k updates its colour at ring >= k ----
@@ -673,14 +958,9 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
       const bool interior = lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY;
       tile_update_cell_warp<P, DEBUG>(p, sm, cl, nc, q, pw, si, cell, interior, t, tally);
     }
-    if (COMPACT) {
-      uint16_t* wq = &s_queue[COMPACT ? warp * 64u : 0u];
-      switch (q) {                                 // the local colour as a compile-time constant: uniform offsets
-        case 0: tile_sub_sweep_cells_compact<P, NS, DEBUG, 0>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], wq, tally); break;
-        case 1: tile_sub_sweep_cells_compact<P, NS, DEBUG, 1>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], wq, tally); break;
-        case 2: tile_sub_sweep_cells_compact<P, NS, DEBUG, 2>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], wq, tally); break;
-        default: tile_sub_sweep_cells_compact<P, NS, DEBUG, 3>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], wq, tally); break;
-      }
+    if (SORTED) {
+      tile_run_sorted<P, NS, DEBUG>(p, sm, tb, q, gx0, gy0, t, queues + (k - 1u) * PS, s_cnt[k - 1u][0], s_cnt[k - 1u][1],
+                                    &s_next[k - 1u], tally);
     } else {
       switch (q) {                                 // the local colour as a compile-time constant: uniform offsets
         case 0: tile_sub_sweep_cells<P, NS, DEBUG, 0>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;

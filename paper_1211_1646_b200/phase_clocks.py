@@ -46,6 +46,8 @@ def main():
             raise SystemExit("this library was built without -DMPMC_PHASE_CLOCKS")
         rows.append(pc.astype(np.int64))
     pc = np.stack(rows)                              # (samples, tiles, marks)
+    extra = pc[:, :, 9:] if pc.shape[2] > 9 else None   # marks inside the sort of the sorted variant (0 if unused)
+    pc = pc[:, :, :9]
     d = np.diff(pc[:, :, 1:], axis=2)                # cycles per phase
     span_ns = pc[:, :, 0].max(axis=1) - pc[:, :, 0].min(axis=1)
     cfg = g.config()
@@ -54,6 +56,12 @@ def main():
     for i in range(d.shape[2]):
         name = PHASES[i + 1] if i + 1 < len(PHASES) else f"phase {i + 1}"
         print(f"  {name:42s} mean {d[:, :, i].mean():9.0f}   max over tiles (mean over launches) {d[:, :, i].max(axis=1).mean():9.0f} cycles")
+    if extra is not None and extra[:, :, 0].min() > 0:
+        t_load_end = pc[:, :, 2]
+        names = ["row occupancy masks", "simple / general masks + prefix sums"]
+        ends = [extra[:, :, i] for i in range(2)]
+        print("  inside 'load': the sort ends " + ", ".join(f"{n} {(t_load_end - e).mean():.0f}" for n, e in zip(names, ends))
+              + " cycles before the end of the phase")
     if args.dump:
         np.save(args.dump, d.mean(axis=0))
     tot = pc[:, :, -1] - pc[:, :, 1]
