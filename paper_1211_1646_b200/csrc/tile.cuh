@@ -38,7 +38,7 @@ namespace mpmc {
 // threads per CTA, one CTA per SM: 24 warps at <= 85 registers (fp32), 12 warps at <= 170 registers (fp64)
 template <typename P> struct TileThreads { static constexpr int value = sizeof(P) == 4 ? 768 : 384; };
 constexpr int HALO = 5;
-constexpr int SHIFT_U = 4;              // cells per lane and chunk in the shift (their id loads are in flight together)
+constexpr int SHIFT_U = 2;              // cells per lane and chunk in the shift (their id loads are in flight together)
 
 // -DMPMC_PHASE_CLOCKS builds a variant that records clock64() at every phase boundary (phase_clocks.py).
 #ifdef MPMC_PHASE_CLOCKS
@@ -58,6 +58,11 @@ __device__ __forceinline__ unsigned long long clock_after(const volatile uint32_
 #endif
 
 #define MPMC_PHASE_MARK(i) MPMC_PHASE_MARK_AT(i, &s_last)
+#ifdef MPMC_PHASE_CLOCKS
+#define MPMC_PHASE_VALUE(i, v) do { if (threadIdx.x == 0 && blockIdx.x < PHASE_TILES) g_phase_clocks[blockIdx.x][i] = (unsigned long long)(v); } while (0)
+#else
+#define MPMC_PHASE_VALUE(i, v) do { } while (0)
+#endif
 
 // v in [-m, 2m) -> [0, m)
 __device__ __forceinline__ uint32_t wrap_cell(int v, uint32_t m) {
@@ -580,14 +585,15 @@ __device__ __forceinline__ void tile_sort_cells(const Params& p, const SmemCell<
   }
   __syncthreads();
   MPMC_PHASE_MARK_AT(9, &s_cnt[0][0]);
-  // cells next to a crowded cell are nobody's here: a whole warp does them (tile_update_cell_warp)
-  for (uint32_t i = tid; i < 9u * nc; i += blockDim.x) {
-    const uint32_t e = i / 9u, d = i - 9u * e;
-    const uint32_t lx = (cl.e[e].lxly & 0xFFFFu) + d % 3u - 1u, ly = (cl.e[e].lxly >> 16) + d / 3u - 1u;   // may wrap below 0
-    if (lx < tb.w && ly < tb.h)
-      atomicAnd(&sa.occ[(((ly & 1u) << 1) | (lx & 1u)) * PH + (ly >> 1)], ~(1ull << (lx >> 1)));
+  if (nc != 0u) {                                        // (uniform) cells next to a crowded cell are nobody's here: a
+    for (uint32_t i = tid; i < 9u * nc; i += blockDim.x) {   // whole warp does them (tile_update_cell_warp)
+      const uint32_t e = i / 9u, d = i - 9u * e;
+      const uint32_t lx = (cl.e[e].lxly & 0xFFFFu) + d % 3u - 1u, ly = (cl.e[e].lxly >> 16) + d / 3u - 1u;   // may wrap below 0
+      if (lx < tb.w && ly < tb.h)
+        atomicAnd(&sa.occ[(((ly & 1u) << 1) | (lx & 1u)) * PH + (ly >> 1)], ~(1ull << (lx >> 1)));
+    }
+    __syncthreads();
   }
-  __syncthreads();
   // ---- B + C: one warp per sub-sweep, one LANE per row: the row's simple and general cells (nine shifted ORs of row
   //      masks), then the exclusive prefix sums over the rows that place every row in the sub-sweep's queue ----
   if (warp < 4u) {
@@ -807,6 +813,20 @@ __device__ __forceinline__ void tile_shift_cells(const Params& p, const SmemCell
     const int bit = ALONG_X ? (int)(Qg & 1u) : (int)(Qg >> 1);
     const int dh = positive ? bit : bit - 1;                         // (g + 1) >> 1 - (g >> 1) = bit; (g - 1) >> 1 - (g >> 1) = bit - 1
     const int hn = ALONG_X ? (int)p.hx : (int)p.hy;                  // half-cells along the shift axis
+    // The cells of this plane that take the general routine above: the listed cells of the plane and the cells that pull
+    // from a listed cell of the plane they pull from.  Normally none, or one or two plane indices kept in registers
+    // (a per-cell search of the list cost 2 900 cycles per tile with a crowded cell, measured); more: search the list.
+    uint32_t sp0 = 0xFFFFFFFFu, sp1 = 0xFFFFFFFFu, nsp = 0u;
+    for (uint32_t e = 0; e < nc; ++e) {
+      const uint32_t v = cl.e[e].si;
+      const uint32_t pe = (v >= 2u * PS ? 2u : 0u) + ((v >= 3u * PS || (v >= PS && v < 2u * PS)) ? 1u : 0u);
+      if (pe == q) { if (nsp == 0u) sp0 = v; else if (nsp == 1u) sp1 = v; ++nsp; }
+      if (pe == (q ^ (ALONG_X ? 1u : 2u))) {
+        const uint32_t w = (uint32_t)((int)v - nboff);
+        if (nsp == 0u) sp0 = w; else if (nsp == 1u) sp1 = w;
+        ++nsp;
+      }
+    }
     for (;;) {
       uint32_t base = 0;
       if (lane == 0u) base = atomicAdd(&next[q], 32u * SHIFT_U);
@@ -830,7 +850,8 @@ __device__ __forceinline__ void tile_shift_cells(const Params& p, const SmemCell
         const int cin = ALONG_X ? hyg * (int)p.hx + hnb : hnb * (int)p.hx + hxg;
         own[u] = 2u * Qg * Mqp + (uint32_t)cig; nbg[u] = 2u * Qn * Mqp + (uint32_t)cin;
         cell[u] = (uint32_t)(2 * hyg + (int)(Qg >> 1)) * p.mx + (uint32_t)(2 * hxg + (int)(Qg & 1u));
-        general[u] = nc != 0u && (crowd_find(cl, nc, si[u]) >= 0 || crowd_find(cl, nc, sn[u]) >= 0);
+        general[u] = nsp <= 2u ? (si[u] == sp0 || si[u] == sp1)
+                               : (crowd_find(cl, nc, si[u]) >= 0 || crowd_find(cl, nc, sn[u]) >= 0);
         if (ok[u] && !general[u]) { ia[u] = idsc[own[u]]; ib[u] = idsc[nbg[u]]; }
       }
 #pragma unroll
@@ -931,6 +952,7 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   uint16_t* queues = reinterpret_cast<uint16_t*>(sm + 4u * PS);
   if (SORTED) tile_sort_cells<P, DEBUG>(p, sm, cl, nc, tb, dr, gx0, gy0, queues, sort_area(queues + 4u * PS, p.tl_PH), s_cnt);
   MPMC_PHASE_MARK(2);
+  MPMC_PHASE_VALUE(12, nc);                      // crowded cells in this tile's region
   Tally tally;
 
   // ---- four sub-sweeps (Alg. 1 lines 3-14, L66-88): sub-sweep k updates its colour at ring >= k ----
