@@ -553,6 +553,47 @@ __device__ __forceinline__ double2 lds_x01(const SmemCell<double>* s, uint32_t i
 // T[px + a] as a mask over px, a in {-1, 0, +1}
 __device__ __forceinline__ unsigned long long mask_shift(const unsigned long long T, const int a) { return a < 0 ? T << 1 : a > 0 ? T >> 1 : T; }
 
+// Phase A of the sort for one plane row r (= q * ph + py): bit px of occ / two = the cell holds >= 1 / >= 2 disks.  Called by
+// the warp that copied the row, as soon as its copies have landed (the load phase waits on L2 bandwidth with idle issue
+// slots; the masks of the early rows are taken under the copies of the late ones).
+template <typename P, bool DEBUG>
+__device__ __forceinline__ void sort_row_masks(const Params& p, const SmemCell<P>* sm, const TileBox& tb, const int gx0, const int gy0,
+                                               const SortArea sa, const uint32_t q, const uint32_t py) {
+  const uint32_t PS = p.tl_PS, PH = p.tl_PH, pw = tb.pw, lane = threadIdx.x & 31u;
+  const P HALF_FAR = Real<P>::far_away() * (P)0.5;
+  unsigned long long occ = 0ull, two = 0ull;
+#pragma unroll
+  for (uint32_t half = 0; half < 2u; ++half) {
+    const uint32_t px = lane + 32u * half;
+    bool o = false, w2 = false;
+    if (px < pw) {
+      const auto x = lds_x01(sm, q * PS + py * pw + px);     // slots fill in order
+      o = x.x < HALF_FAR; w2 = x.y < HALF_FAR;
+      if (DEBUG && !o) {                                       // an empty cell of the tile: nothing accepted
+        const uint32_t lx = 2u * px + (q & 1u), ly = 2u * py + (q >> 1);
+        if (lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY)
+          p.mask[wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx)] = 0u;
+      }
+    }
+    occ |= (unsigned long long)__ballot_sync(0xFFFFFFFFu, o) << (32u * half);
+    two |= (unsigned long long)__ballot_sync(0xFFFFFFFFu, w2) << (32u * half);
+  }
+  if (lane == 0u) { sa.occ[q * PH + py] = occ; sa.two[q * PH + py] = two; }
+}
+// cp.async.wait_group with a run-time count (the instruction takes an immediate)
+__device__ __forceinline__ void cp_async_wait_pending(const uint32_t n) {
+  switch (n) {
+    case 0: asm volatile("cp.async.wait_group 0;" ::: "memory"); break;
+    case 1: asm volatile("cp.async.wait_group 1;" ::: "memory"); break;
+    case 2: asm volatile("cp.async.wait_group 2;" ::: "memory"); break;
+    case 3: asm volatile("cp.async.wait_group 3;" ::: "memory"); break;
+    case 4: asm volatile("cp.async.wait_group 4;" ::: "memory"); break;
+    case 5: asm volatile("cp.async.wait_group 5;" ::: "memory"); break;
+    case 6: asm volatile("cp.async.wait_group 6;" ::: "memory"); break;
+    default: asm volatile("cp.async.wait_group 7;" ::: "memory"); break;
+  }
+}
+
 template <typename P, bool DEBUG>
 __device__ __forceinline__ void tile_sort_cells(const Params& p, const SmemCell<P>* sm, const CrowdList<P>& cl, const uint32_t nc,
                                                 const TileBox& tb, const Draws& dr, const int gx0, const int gy0,
@@ -561,29 +602,7 @@ __device__ __forceinline__ void tile_sort_cells(const Params& p, const SmemCell<
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, NW = blockDim.x >> 5;
   const P HALF_FAR = Real<P>::far_away() * (P)0.5;
   const uint32_t inv_ph = small_div_magic(ph);
-  // ---- A: occupancy masks of every plane row ----
-  for (uint32_t r = warp; r < 4u * ph; r += NW) {
-    const uint32_t q = small_div(r, inv_ph), py = r - q * ph;
-    unsigned long long occ = 0ull, two = 0ull;
-#pragma unroll
-    for (uint32_t half = 0; half < 2u; ++half) {
-      const uint32_t px = lane + 32u * half;
-      bool o = false, w2 = false;
-      if (px < pw) {
-        const auto x = lds_x01(sm, q * PS + py * pw + px);     // slots fill in order
-        o = x.x < HALF_FAR; w2 = x.y < HALF_FAR;
-        if (DEBUG && !o) {                                       // an empty cell of the tile: nothing accepted
-          const uint32_t lx = 2u * px + (q & 1u), ly = 2u * py + (q >> 1);
-          if (lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY)
-            p.mask[wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx)] = 0u;
-        }
-      }
-      occ |= (unsigned long long)__ballot_sync(0xFFFFFFFFu, o) << (32u * half);
-      two |= (unsigned long long)__ballot_sync(0xFFFFFFFFu, w2) << (32u * half);
-    }
-    if (lane == 0u) { sa.occ[q * PH + py] = occ; sa.two[q * PH + py] = two; }
-  }
-  __syncthreads();
+  // (phase A — the occupancy masks of every plane row, sort_row_masks — ran with the load, row by row as the copies landed)
   MPMC_PHASE_MARK_AT(9, &s_cnt[0][0]);
   if (nc != 0u) {                                        // (uniform) cells next to a crowded cell are nobody's here: a
     for (uint32_t i = tid; i < 9u * nc; i += blockDim.x) {   // whole warp does them (tile_update_cell_warp)
@@ -922,13 +941,32 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   {
     const P* posc = reinterpret_cast<const P*>(p.pos[cur]);
     const uint32_t nrows = 4u * ph, inv_ph = small_div_magic(ph), NW = TILE_THREADS / 32;
-    for (uint32_t r = warp; r < nrows; r += NW) {
-      const uint32_t q = small_div(r, inv_ph), py = r - q * ph;
-      const uint32_t gy = wrap_cell(gy0 + (int)(2u * py + (q >> 1)), p.my);
-      const uint32_t gbase = 2u * ((gy & 1u) << 1) * Mqp + (gy >> 1) * p.hx, sbase = q * PS + py * pw;
-      for (uint32_t px = lane; px < pw; px += 32u) {
-        const uint32_t gx = wrap_cell(gx0 + (int)(2u * px + (q & 1u)), p.mx);
-        cp_async_cell(sm + sbase + px, posc, gbase + 2u * (gx & 1u) * Mqp + (gx >> 1));
+    const SortArea sa_load = sort_area(reinterpret_cast<uint16_t*>(sm + 4u * PS) + 4u * PS, p.tl_PH);
+    // a warp's rows in groups of eight: one cp.async group per row, so that (SORTED) the occupancy masks of a row can be
+    // taken as soon as ITS copies have landed, under the copies of the rows behind it
+    for (uint32_t r8 = warp; r8 < nrows; r8 += 8u * NW) {
+#pragma unroll
+      for (uint32_t j = 0; j < 8u; ++j) {
+        const uint32_t r = r8 + j * NW;
+        if (r < nrows) {
+          const uint32_t q = small_div(r, inv_ph), py = r - q * ph;
+          const uint32_t gy = wrap_cell(gy0 + (int)(2u * py + (q >> 1)), p.my);
+          const uint32_t gbase = 2u * ((gy & 1u) << 1) * Mqp + (gy >> 1) * p.hx, sbase = q * PS + py * pw;
+          for (uint32_t px = lane; px < pw; px += 32u) {
+            const uint32_t gx = wrap_cell(gx0 + (int)(2u * px + (q & 1u)), p.mx);
+            cp_async_cell(sm + sbase + px, posc, gbase + 2u * (gx & 1u) * Mqp + (gx >> 1));
+          }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+      }
+      if (SORTED) {
+#pragma unroll
+        for (uint32_t j = 0; j < 8u; ++j) {
+          const uint32_t r = r8 + j * NW;
+          cp_async_wait_pending(7u - j);
+          __syncwarp();
+          if (r < nrows) { const uint32_t q = small_div(r, inv_ph); sort_row_masks<P, DEBUG>(p, sm, tb, gx0, gy0, sa_load, q, r - q * ph); }
+        }
       }
     }
     // the crowded cells of this state that lie in the region, with their slots 2 and 3
