@@ -145,7 +145,7 @@ int mpmc_debug_path(mpmc_ctx* ctx, uint64_t out[2]);
 
 /* Test hook (host values only): how mpmc_sweep will run this context.  out = host, {slots per cell of the fused tile
  * kernel: 2 (tile.cuh, w ~ sigma), 4 (tile4.cuh) or 0 (no tile kernel: every sweep on the general persistent kernel);
- * CTAs (= tiles) of the tile kernel; tiles along x;
+ * CTAs (= tiles) of the tile kernel; tiles per row of tiles (first group of rows, see mpmc_debug_tiling);
  * tiles along y; threads per tile CTA; dynamic shared memory per tile CTA in bytes; CTAs of the general kernel; threads
  * per CTA of the general kernel}. */
 int mpmc_debug_config(const mpmc_ctx* ctx, uint32_t out[8]);
@@ -160,10 +160,11 @@ int mpmc_debug_phase_clocks(mpmc_ctx* ctx, uint64_t* out, uint32_t max_tiles, ui
 
 /* Test hook (pure host arithmetic, no device needed): the tiling the fused tile kernels would use for a grid of
  * 2 hx x 2 hy cells when a cell takes cell_bytes of shared memory, an SM offers smem_max bytes and the device has sms
- * SMs.  out = {tiles along x, tiles along y, shared-memory plane stride in cells}.  Every tile (rounded up to even
- * sizes) plus a halo of 5 cells on each side fits smem_max and is no wider than the grid; MPMC_ERR_BOX if no such
- * tiling exists (grids under 12 cells across). */
-int mpmc_debug_tiling(uint32_t hx, uint32_t hy, size_t cell_bytes, size_t smem_max, uint32_t sms, uint32_t out[3]);
+ * SMs.  out = {a, rows, plane stride in cells, na, hyA, tiles}: the tiles form `rows` rows; the first na rows hold a tiles
+ * each and share the half-rows [0, hyA) evenly, the other rows hold a + 1 tiles each and share the rest (a uniform
+ * a x rows grid has na = rows, hyA = hy).  Every tile (rounded up to even sizes) plus a halo of 5 cells on each side fits
+ * smem_max and is no wider than the grid; MPMC_ERR_BOX if no such tiling exists (grids under 12 cells across). */
+int mpmc_debug_tiling(uint32_t hx, uint32_t hy, size_t cell_bytes, size_t smem_max, uint32_t sms, uint32_t out[6]);
 
 /* Test hook: Philox4x32-10 evaluated ON THE DEVICE by the same routine the kernels use.
  * ctr = device u32[n][4], key = host u32[2], out = device u32[n][4]; enqueued on cuda_stream and synchronised. */

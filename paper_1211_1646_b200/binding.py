@@ -300,14 +300,14 @@ class Mpmc:
 
 
 def tiling(hx: int, hy: int, cell_bytes: int = 16, smem_max: int = 226 * 1024, sms: int = 148):
-    """(tiles along x, tiles along y, plane stride) the tile kernels would use; host arithmetic only.  None if the grid is
-    too small to tile."""
-    out = (_u32 * 3)()
+    """(a, rows, plane stride, na, hyA, tiles) of the tiling the tile kernels would use (mpmc_debug_tiling); host
+    arithmetic only.  None if the grid is too small to tile."""
+    out = (_u32 * 6)()
     code = lib().mpmc_debug_tiling(int(hx), int(hy), int(cell_bytes), int(smem_max), int(sms), out)
     if code == -2:
         return None
     _chk(code)
-    return int(out[0]), int(out[1]), int(out[2])
+    return tuple(int(v) for v in out)
 
 
 def device_philox(ctr, key, device="cuda:0"):

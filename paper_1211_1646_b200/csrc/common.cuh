@@ -69,7 +69,9 @@ struct Params {
   uint32_t tune;             // tuning word for experiments (builds with -DMPMC_EXPERIMENT read it from MPMC_TUNE); unused by default
   uint32_t track_crowded;    // 1: kernels that write cell counts list the cells with more than 2 disks (for tile.cuh)
   uint32_t hx_magic, hx_sh1, hx_sh2;  // ci / hx without a divide (Granlund-Montgomery; host: div_magic)
-  uint32_t tl_ntx, tl_nty, tl_PS;       // tile kernel: tiles per axis, shared-memory plane stride (cells)
+  uint32_t tl_ntx, tl_nty, tl_PS;       // tile kernel: tiles per row (first tl_na rows), rows of tiles, shared-memory plane stride (cells)
+  uint32_t tl_na, tl_hyA;               // the first tl_na rows of tiles cover the half-rows [0, tl_hyA) with tl_ntx tiles each, the
+                                        // other rows the rest with tl_ntx + 1 tiles each (uniform tiling: tl_na = tl_nty, tl_hyA = hy)
   uint32_t tl_PH;                       // ... rows of the tallest tile's planes (sorted variant: stride of its row tables)
   uint32_t seed_lo, seed_hi;
   uint32_t rk0[10], rk1[10];            // Philox round keys seed + r * Weyl constant (philox4x32_10_rk)

@@ -130,26 +130,64 @@ int launch_sweeps(mpmc_ctx* c, unsigned long long t_end, uint32_t op, uint32_t a
   return MPMC_OK;
 }
 
-// Tiling of the tile kernel: ntx x nty tiles of (nearly) equal even size whose loaded region (tile + 2 HALO) fits
-// the shared memory of one SM; among those, the one with the least work on the busiest SM:
-// waves * cells of the largest region.  Returns false if no such tiling exists (boxes under 12 cells across).
-// row_bytes / pw_max: the sorted variant of the 2-slot kernel also needs row_bytes of shared memory per plane row and
-// plane rows of at most pw_max cells.
-bool choose_tiling(uint32_t hx, uint32_t hy, size_t cell_bytes, size_t smem_max, uint32_t sms, uint32_t* ntx, uint32_t* nty,
-                   uint32_t* PS, size_t row_bytes = 0, uint32_t pw_max = 0xFFFFFFFFu, uint32_t* PH = nullptr) {
+// Tiling of the tile kernels.  Tiles form rows of (nearly) equal even size; every loaded region (tile + 2 HALO) must fit
+// the shared memory of one SM and must not overlap itself around the box.  Two families are searched for the least work
+// on the busiest SM = waves * cells of the largest region: uniform ntx x nty grids, and — while the whole grid is one wave
+// — MIXED tilings: na rows of a tiles over the half-rows [0, hyA) and nb rows of a + 1 narrower, taller tiles over the rest,
+// hyA placed so that both shapes load the same area (C3 on 148 SMs: 8 x 12 + 4 x 13 = 148 tiles instead of 12 x 12 = 144).
+// row_bytes / pw_max: the sorted variant of the 2-slot kernel also needs row_bytes of shared memory per plane row and plane
+// rows of at most pw_max cells.  Returns false if no tiling exists (boxes under 12 cells across).
+struct Tiling { uint32_t ntx, nty, na, hyA, PS, PH, tiles; };
+
+bool choose_tiling(uint32_t hx, uint32_t hy, size_t cell_bytes, size_t smem_max, uint32_t sms, Tiling* out,
+                   size_t row_bytes = 0, uint32_t pw_max = 0xFFFFFFFFu) {
   double best = 0; bool found = false;
   const uint32_t lim = 1024;
+  auto fits = [&](uint32_t TX, uint32_t TY) {
+    const uint32_t pw = (TX + 2 * HALO) / 2, ph = (TY + 2 * HALO) / 2;
+    if (TX + 2 * HALO > 2 * hx || TY + 2 * HALO > 2 * hy) return false;     // a region must not overlap itself around the box
+    const size_t bytes = (size_t)4 * pw * ph * cell_bytes + (size_t)4 * ph * row_bytes;
+    return bytes <= smem_max && pw * ph < 16384u && pw <= pw_max;
+  };
   for (uint32_t ax = 1; ax <= hx && ax <= lim; ++ax) {
-    const uint32_t TX = 2 * ((hx + ax - 1) / ax), pw = (TX + 2 * HALO) / 2;
-    if (TX + 2 * HALO > 2 * hx) continue;           // a region must not overlap itself around the box
+    const uint32_t TX = 2 * ((hx + ax - 1) / ax);
     for (uint32_t ay = 1; ay <= hy && ay <= lim; ++ay) {
-      const uint32_t TY = 2 * ((hy + ay - 1) / ay), ph = (TY + 2 * HALO) / 2;
-      if (TY + 2 * HALO > 2 * hy) continue;
-      const size_t bytes = (size_t)4 * pw * ph * cell_bytes + (size_t)4 * ph * row_bytes;
-      if (bytes > smem_max || pw * ph >= 16384u || pw > pw_max) continue;
+      const uint32_t TY = 2 * ((hy + ay - 1) / ay);
+      if (!fits(TX, TY)) continue;
       const double waves = std::ceil((double)ax * ay / sms);
       const double cost = waves * (double)(TX + 2 * HALO) * (TY + 2 * HALO) + 1e-6 * ax * ay;
-      if (!found || cost < best) { best = cost; found = true; *ntx = ax; *nty = ay; *PS = pw * ph; if (PH) *PH = ph; }
+      if (!found || cost < best) {
+        best = cost; found = true;
+        *out = Tiling{ax, ay, ay, hy, ((TX + 2 * HALO) / 2) * ((TY + 2 * HALO) / 2), (TY + 2 * HALO) / 2, ax * ay};
+      }
+    }
+  }
+  // mixed tilings of at most one wave
+  for (uint32_t a = 1; a + 1 <= hx && a < sms; ++a) {
+    const uint32_t TXa = 2 * ((hx + a - 1) / a), TXb = 2 * ((hx + a) / (a + 1));
+    for (uint32_t na = 1; na * a < sms; ++na) {
+      for (uint32_t nb = 1; na * a + nb * (a + 1) <= sms; ++nb) {
+        if (na + nb > hy) break;
+        // equal loaded areas: (TXa + 10)(2 hyA / na + 10) = (TXb + 10)(2 (hy - hyA) / nb + 10)
+        const double A = TXa + 2.0 * HALO, B = TXb + 2.0 * HALO;
+        const double hA = (B * (2.0 * hy / nb + 2.0 * HALO) - 2.0 * HALO * A) / (2.0 * A / na + 2.0 * B / nb);
+        for (int d = -1; d <= 1; ++d) {
+          const long long h = (long long)std::floor(hA + 0.5) + d;
+          if (h < (long long)na || h > (long long)hy - (long long)nb) continue;
+          const uint32_t hyA = (uint32_t)h;
+          const uint32_t TYa = 2 * ((hyA + na - 1) / na), TYb = 2 * ((hy - hyA + nb - 1) / nb);
+          if (!fits(TXa, TYa) || !fits(TXb, TYb)) continue;
+          const double ra = (double)(TXa + 2 * HALO) * (TYa + 2 * HALO), rb = (double)(TXb + 2 * HALO) * (TYb + 2 * HALO);
+          const uint32_t tiles = na * a + nb * (a + 1);
+          const double cost = (ra > rb ? ra : rb) + 1e-6 * tiles;
+          if (!found || cost < best * (1.0 - 1e-3)) {            // (a uniform tiling wins ties: simpler index arithmetic)
+            best = cost; found = true;
+            const uint32_t psa = ((TXa + 2 * HALO) / 2) * ((TYa + 2 * HALO) / 2), psb = ((TXb + 2 * HALO) / 2) * ((TYb + 2 * HALO) / 2);
+            const uint32_t pha = (TYa + 2 * HALO) / 2, phb = (TYb + 2 * HALO) / 2;
+            *out = Tiling{a, na + nb, na, hyA, psa > psb ? psa : psb, pha > phb ? pha : phb, tiles};
+          }
+        }
+      }
     }
   }
   return found;
@@ -363,28 +401,28 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
                               + (sorted ? sizeof(uint16_t) : 0);
     const size_t stat = (two_slot ? (fp32 ? sizeof(CrowdList<float>) : sizeof(CrowdList<double>)) : 0) + 512;   // static shared memory
     const size_t smem_max = (size_t)smem_optin > stat ? (size_t)smem_optin - stat : 0;
-    uint32_t ntx = 0, nty = 0, PS = 0, PH = 0;
+    Tiling tl = {};
     const size_t row_bytes = sorted ? SORT_ROW_BYTES : 0;
     c->tile_threads = two_slot ? (fp32 ? TileThreads<float>::value : TileThreads<double>::value)
                                : (fp32 ? Tile4Threads<float>::value : Tile4Threads<double>::value);
-    bool have = choose_tiling(p.hx, p.hy, cell_bytes, smem_max, (uint32_t)sms, &ntx, &nty, &PS, row_bytes, sorted ? 64u : 0xFFFFFFFFu, &PH);
+    bool have = choose_tiling(p.hx, p.hy, cell_bytes, smem_max, (uint32_t)sms, &tl, row_bytes, sorted ? 64u : 0xFFFFFFFFu);
     // the sort is a fixed cost of ~8 000 cycles per tile and sweep (measured, phase_clocks.py): it pays from about a
     // thousand cells per colour plane on; smaller tiles (systems below ~2e5 cells) keep the plain variant
-    if (sorted && have && PS < SORT_MIN_PLANE) have = false;
+    if (sorted && have && tl.PS < SORT_MIN_PLANE) have = false;
 #ifdef MPMC_EXPERIMENT
     if (const char* e = std::getenv("MPMC_TILE")) {        // "ntx,nty,threads" (whole warps)
       unsigned a = 0, b = 0, th = 0;
       if (std::sscanf(e, "%u,%u,%u", &a, &b, &th) == 3 && a && b && th >= 32 && th % 32 == 0 && th <= c->tile_threads && a <= p.hx && b <= p.hy) {
         const uint32_t pw = (2 * ((p.hx + a - 1) / a) + 2 * HALO) / 2, ph = (2 * ((p.hy + b - 1) / b) + 2 * HALO) / 2;
-        if ((size_t)4 * pw * ph * cell_bytes <= smem_max) { ntx = a; nty = b; PS = pw * ph; c->tile_threads = th; have = true; }
+        if ((size_t)4 * pw * ph * cell_bytes + (size_t)4 * ph * row_bytes <= smem_max) { tl = Tiling{a, b, b, p.hy, pw * ph, ph, a * b}; c->tile_threads = th; have = true; }
       }
     }
 #endif
     if (have) {
       c->tile_kernel = tk;
-      c->tile_grid = ntx * nty;
-      c->tile_smem = (size_t)4 * PS * cell_bytes + (size_t)4 * PH * row_bytes;
-      p.tl_ntx = ntx; p.tl_nty = nty; p.tl_PS = PS; p.tl_PH = PH;
+      c->tile_grid = tl.tiles;
+      c->tile_smem = (size_t)4 * tl.PS * cell_bytes + (size_t)4 * tl.PH * row_bytes;
+      p.tl_ntx = tl.ntx; p.tl_nty = tl.nty; p.tl_PS = tl.PS; p.tl_PH = tl.PH; p.tl_na = tl.na; p.tl_hyA = tl.hyA;
       // The attribute belongs to the kernel function, not to this context: set it to the most any tiling can ask for
       // (the opt-in maximum minus the kernel's static shared memory), so that live contexts with different tilings
       // of the same instantiation do not undo each other's setting.
@@ -637,11 +675,11 @@ int mpmc_debug_phase_clocks(mpmc_ctx* c, uint64_t* out, uint32_t max_tiles, uint
   return MPMC_OK;
 }
 
-int mpmc_debug_tiling(uint32_t hx, uint32_t hy, size_t cell_bytes, size_t smem_max, uint32_t sms, uint32_t out[3]) {
+int mpmc_debug_tiling(uint32_t hx, uint32_t hy, size_t cell_bytes, size_t smem_max, uint32_t sms, uint32_t out[6]) {
   if (!out || hx == 0 || hy == 0 || cell_bytes == 0 || sms == 0) return MPMC_ERR_ARG;
-  uint32_t ntx = 0, nty = 0, PS = 0;
-  if (!choose_tiling(hx, hy, cell_bytes, smem_max, sms, &ntx, &nty, &PS)) return MPMC_ERR_BOX;
-  out[0] = ntx; out[1] = nty; out[2] = PS;
+  Tiling tl = {};
+  if (!choose_tiling(hx, hy, cell_bytes, smem_max, sms, &tl)) return MPMC_ERR_BOX;
+  out[0] = tl.ntx; out[1] = tl.nty; out[2] = tl.PS; out[3] = tl.na; out[4] = tl.hyA; out[5] = tl.tiles;
   return MPMC_OK;
 }
 

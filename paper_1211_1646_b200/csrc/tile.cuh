@@ -109,15 +109,32 @@ __device__ __forceinline__ double lds_x1(const SmemCell<double>* s, uint32_t i) 
 struct TileBox {
   uint32_t x0, y0, TX, TY, w, h, pw, ph;
 };
-__device__ __forceinline__ TileBox tile_box(const Params& p, uint32_t tx, uint32_t ty) {
-  TileBox b;
-  b.x0 = 2u * (uint32_t)((unsigned long long)p.hx * tx / p.tl_ntx);
-  b.y0 = 2u * (uint32_t)((unsigned long long)p.hy * ty / p.tl_nty);
-  b.TX = 2u * (uint32_t)((unsigned long long)p.hx * (tx + 1) / p.tl_ntx) - b.x0;
-  b.TY = 2u * (uint32_t)((unsigned long long)p.hy * (ty + 1) / p.tl_nty) - b.y0;
-  b.w = b.TX + 2 * HALO; b.h = b.TY + 2 * HALO;
-  b.pw = b.w / 2; b.ph = b.h / 2;
-  return b;
+// Tile number b (= blockIdx.x).  The tiles form rows; the first tl_na rows hold tl_ntx tiles each and share the half-rows
+// [0, tl_hyA) evenly, the remaining rows hold tl_ntx + 1 (narrower, taller) tiles each: with two tile shapes of equal
+// loaded area the tile count can match the SM count (C3: 8 x 12 + 4 x 13 = 148) where a rectangular ntx x nty grid leaves
+// SMs idle (12 x 12 = 144).
+__device__ __forceinline__ TileBox tile_box(const Params& p, const uint32_t b) {
+  TileBox t;
+  const uint32_t nA = p.tl_na * p.tl_ntx;
+  uint32_t tx, ntx, h0, h1;
+  if (b < nA) {
+    const uint32_t r = b / p.tl_ntx;
+    tx = b - r * p.tl_ntx; ntx = p.tl_ntx;
+    h0 = (uint32_t)((unsigned long long)p.tl_hyA * r / p.tl_na);
+    h1 = (uint32_t)((unsigned long long)p.tl_hyA * (r + 1u) / p.tl_na);
+  } else {
+    const uint32_t b2 = b - nA, nb = p.tl_nty - p.tl_na, hyB = p.hy - p.tl_hyA;
+    const uint32_t r = b2 / (p.tl_ntx + 1u);
+    tx = b2 - r * (p.tl_ntx + 1u); ntx = p.tl_ntx + 1u;
+    h0 = p.tl_hyA + (uint32_t)((unsigned long long)hyB * r / nb);
+    h1 = p.tl_hyA + (uint32_t)((unsigned long long)hyB * (r + 1u) / nb);
+  }
+  t.x0 = 2u * (uint32_t)((unsigned long long)p.hx * tx / ntx);
+  t.TX = 2u * (uint32_t)((unsigned long long)p.hx * (tx + 1u) / ntx) - t.x0;
+  t.y0 = 2u * h0; t.TY = 2u * (h1 - h0);
+  t.w = t.TX + 2 * HALO; t.h = t.TY + 2 * HALO;
+  t.pw = t.w / 2; t.ph = t.h / 2;
+  return t;
 }
 
 // The cells sub-sweep k (1..4) has to update, as a rectangle of local coordinates.  The shift of the interior (ring >= 5)
@@ -924,8 +941,7 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   MPMC_PHASE_MARK(0); MPMC_PHASE_MARK(1);
   const uint32_t cur = ctl->cur, nxt = cur ^ 1u;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-  const uint32_t ty = blockIdx.x / p.tl_ntx, tx = blockIdx.x - ty * p.tl_ntx;
-  const TileBox tb = tile_box(p, tx, ty);
+  const TileBox tb = tile_box(p, blockIdx.x);
   const uint32_t PS = p.tl_PS, pw = tb.pw, ph = tb.ph, Mqp = p.Mqp;
   const int gx0 = (int)tb.x0 - HALO, gy0 = (int)tb.y0 - HALO;       // global cell of the region's corner (unwrapped)
   if (tid == 0) {

@@ -92,8 +92,7 @@ k_tile4_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   if (ctl->t != t) return;
   const uint32_t cur = ctl->cur, nxt = cur ^ 1u;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, NW = blockDim.x >> 5;
-  const uint32_t ty = blockIdx.x / p.tl_ntx, tx = blockIdx.x - ty * p.tl_ntx;
-  const TileBox tb = tile_box(p, tx, ty);
+  const TileBox tb = tile_box(p, blockIdx.x);
   const uint32_t pw = tb.pw, ph = tb.ph, Mqp = p.Mqp;
   const int gx0 = (int)tb.x0 - HALO, gy0 = (int)tb.y0 - HALO;       // global cell of the region's corner (unwrapped)
   const P FAR = R::far_away(), HALF_FAR = FAR * (P)0.5;

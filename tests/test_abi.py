@@ -104,29 +104,43 @@ def test_product_does_not_import_oracle():
 
 
 def test_tiling_of_the_tile_kernels_host_logic():
-    """choose_tiling (csrc/mpmc.cu) through the mpmc_debug_tiling hook, no device: every tile plus its halo of 5 fits the
-    shared memory and is no wider than the grid (a loaded region must not overlap itself), the tiles cover the grid, and
-    the busiest SM's work (waves x largest region) is not worse than a few obvious alternatives."""
+    """choose_tiling (csrc/mpmc.cu) through the mpmc_debug_tiling hook, no device: the tiles cover the grid exactly, every
+    tile plus its halo of 5 fits the shared memory and is no wider than the grid (a loaded region must not overlap itself),
+    and the busiest SM's work (waves x largest region) is not worse than a few obvious uniform alternatives."""
     import math
     from paper_1211_1646_b200 import binding as B
     smem, sms = 226 * 1024, 148
     for hx, hy, cb in [(576, 499, 16), (145, 126, 16), (43, 37, 32), (2298, 1990, 16), (618, 534, 32), (9, 7, 16), (6, 6, 16),
-                       (1000, 8, 16), (8, 1000, 64)]:
+                       (1000, 8, 16), (8, 1000, 64), (576, 499, 18), (890, 770, 18)]:
         t = B.tiling(hx, hy, cb, smem, sms)
         assert t is not None, (hx, hy)
-        ntx, nty, PS = t
-        assert 1 <= ntx <= hx and 1 <= nty <= hy
-        TX, TY = 2 * math.ceil(hx / ntx), 2 * math.ceil(hy / nty)          # largest tile, even sizes
-        pw, ph = (TX + 10) // 2, (TY + 10) // 2
-        assert PS == pw * ph and 4 * PS * cb <= smem                        # four colour planes fit
-        assert TX + 10 <= 2 * hx and TY + 10 <= 2 * hy                      # region no wider than the grid
-        cost = math.ceil(ntx * nty / sms) * (TX + 10) * (TY + 10)
-        for ax, ay in [(1, 1), (ntx + 1, nty), (ntx, nty + 1), (max(1, ntx - 1), nty), (ntx, max(1, nty - 1)), (12, 12), (sms, 1)]:
+        a, rows, PS, na, hyA, tiles = t
+        nb = rows - na
+        assert 1 <= a <= hx and 1 <= na <= rows <= hy and tiles == na * a + nb * (a + 1)
+        assert (nb == 0 and hyA == hy) or (0 < hyA < hy and tiles <= sms)          # mixed tilings only within one wave
+        # the tiles as the kernel derives them (tile_box): rows of group A then of group B, each row split along x
+        cells, worst, ps_max = 0, 0, 0
+        groups = [(na, a, 0, hyA)] + ([(nb, a + 1, hyA, hy)] if nb else [])
+        for nrow, ntx, h_lo, h_hi in groups:
+            for r in range(nrow):
+                h0, h1 = h_lo + (h_hi - h_lo) * r // nrow, h_lo + (h_hi - h_lo) * (r + 1) // nrow
+                for tx in range(ntx):
+                    TX, TY = 2 * (hx * (tx + 1) // ntx - hx * tx // ntx), 2 * (h1 - h0)
+                    assert TX >= 2 and TY >= 2 and TX + 10 <= 2 * hx and TY + 10 <= 2 * hy
+                    cells += TX * TY
+                    worst = max(worst, (TX + 10) * (TY + 10))
+                    ps_max = max(ps_max, ((TX + 10) // 2) * ((TY + 10) // 2))
+        assert cells == 4 * hx * hy                                          # an exact cover
+        assert ps_max <= PS and 4 * PS * cb <= smem                          # four colour planes of the largest tile fit
+        cost = math.ceil(tiles / sms) * worst
+        for ax, ay in [(1, 1), (a + 1, rows), (a, rows + 1), (max(1, a - 1), rows), (a, max(1, rows - 1)), (12, 12), (sms, 1)]:
             if ax > hx or ay > hy:
                 continue
             ux, uy = 2 * math.ceil(hx / ax), 2 * math.ceil(hy / ay)
             if ux + 10 > 2 * hx or uy + 10 > 2 * hy or 4 * ((ux + 10) // 2) * ((uy + 10) // 2) * cb > smem:
                 continue
-            assert cost <= math.ceil(ax * ay / sms) * (ux + 10) * (uy + 10) * (1 + 1e-9)
+            assert cost <= math.ceil(ax * ay / sms) * (ux + 10) * (uy + 10) * (1 + 1e-9), (hx, hy, t, ax, ay)
+    a, rows, PS, na, hyA, tiles = B.tiling(576, 499, 18, smem, sms)          # the headline grid: all 148 SMs get a tile
+    assert tiles == 148 and na < rows
     assert B.tiling(5, 40, 16, smem, sms) is None and B.tiling(40, 4, 16, smem, sms) is None   # under 12 cells across
     assert B.tiling(100, 100, 16, 4 * 36 * 16 - 1, sms) is None                                # not even a 2 x 2 tile fits

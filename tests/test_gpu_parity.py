@@ -186,6 +186,8 @@ def test_c3_headline_config_bench_launch_configuration(oracle_mod, torch_cuda):
     xy, box = I.workload_inputs(w)
     o, g = make_pair(oracle_mod, torch_cuda, w.N, box, w.sigma, w.d, w.n_s, w.seed, True, xy, debug=False)
     assert (g.mx, g.my) == (1152, 998)
+    cfg = g.config()
+    assert cfg["tiles"] == 148 > cfg["ntx"] * cfg["nty"]       # a mixed tiling: every SM of a B200 gets a tile
     o.sweep(12); g.sweep(12)
     st = assert_same_state(o, g, True, check_mask=False)
     assert st["counts"].sum() == w.N
@@ -331,11 +333,24 @@ def test_tile_kernel_uneven_tilings(oracle_mod, torch_cuda, n, phi):
     xy, box = I.jittered_lattice(n, phi, seed=n)
     o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.15 if phi >= 0.5 else 0.4, 4, n, True, xy)
     cfg = g.config()
-    assert cfg["tile_slots"] == 2 and cfg["tiles"] == cfg["ntx"] * cfg["nty"] > 1
+    assert cfg["tile_slots"] == 2 and cfg["tiles"] >= cfg["ntx"] * cfg["nty"] > 1      # (mixed tilings: some rows hold ntx + 1)
     for k in (1, 2, 7):
         o.sweep(k); g.sweep(k)
         assert_same_state(o, g, True)
     assert g.path_sweeps() == (10, 0)
+
+
+@pytest.mark.parametrize("fp32", [False, True])
+def test_mixed_tiling_two_tile_shapes(oracle_mod, torch_cuda, fp32):
+    # a grid whose best tiling has rows of a and rows of a + 1 tiles (tile_box): accept masks compared over 15 sweeps
+    xy, box = I.jittered_lattice(200, 0.68, seed=31)
+    o, g = make_pair(oracle_mod, torch_cuda, 200 * 200, box, 1.0, 0.12, 4, 4, fp32, xy)
+    cfg = g.config()
+    assert cfg["tile_slots"] == 2 and cfg["tiles"] > cfg["ntx"] * cfg["nty"]
+    for k in (1, 4, 10):
+        o.sweep(k); g.sweep(k)
+        assert_same_state(o, g, fp32)
+    assert g.path_sweeps() == (15, 0)
 
 
 @pytest.mark.parametrize("n_s", [4, 8])
