@@ -941,6 +941,10 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   MPMC_PHASE_MARK(0); MPMC_PHASE_MARK(1);
   const uint32_t cur = ctl->cur, nxt = cur ^ 1u;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+  // the list of crowded cells of this state: its first TILE_THREADS entries are fetched NOW (the chain count -> cell ->
+  // slots 2, 3 is three trips to L2; started here it ends under the tile load instead of behind it)
+  const uint32_t ng = ctl->ccount[slot];
+  const uint32_t my_listed = tid < ng ? ctl->clist[slot][tid] : 0xFFFFFFFFu;
   const TileBox tb = tile_box(p, blockIdx.x);
   const uint32_t PS = p.tl_PS, pw = tb.pw, ph = tb.ph, Mqp = p.Mqp;
   const int gx0 = (int)tb.x0 - HALO, gy0 = (int)tb.y0 - HALO;       // global cell of the region's corner (unwrapped)
@@ -956,6 +960,20 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   //      in flight at once; the phase then runs at the L2 -> SM bandwidth all SMs share (measured 6 TB/s) ----
   {
     const P* posc = reinterpret_cast<const P*>(p.pos[cur]);
+    // the crowded cells of this state that lie in the region, with their slots 2 and 3: entry tid was fetched at the top;
+    // the load of its slots 2, 3 is issued here and stored behind the tile's copies
+    uint32_t my_entry = 0xFFFFFFFFu;
+    Half<P> my_hi;
+    if (my_listed != 0xFFFFFFFFu) {
+      const uint32_t gy = my_listed / p.mx, gx = my_listed - gy * p.mx;
+      const uint32_t lx = wrap_cell((int)gx - gx0, p.mx), ly = wrap_cell((int)gy - gy0, p.my);
+      if (lx < tb.w && ly < tb.h) {
+        my_entry = atomicAdd(&cl.n, 1u);
+        cl.e[my_entry].si = (((ly & 1u) << 1) | (lx & 1u)) * PS + (ly >> 1) * pw + (lx >> 1);
+        cl.e[my_entry].lxly = lx | (ly << 16);
+        my_hi = ld_half(posc, (2u * (((gy & 1u) << 1) | (gx & 1u)) + 1u) * Mqp + (gy >> 1) * p.hx + (gx >> 1));
+      }
+    }
     const uint32_t nrows = 4u * ph, inv_ph = small_div_magic(ph), NW = TILE_THREADS / 32;
     const SortArea sa_load = sort_area(reinterpret_cast<uint16_t*>(sm + 4u * PS) + 4u * PS, p.tl_PH);
     // a warp's rows in groups of eight: one cp.async group per row, so that (SORTED) the occupancy masks of a row can be
@@ -985,9 +1003,8 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
         }
       }
     }
-    // the crowded cells of this state that lie in the region, with their slots 2 and 3
-    const uint32_t ng = ctl->ccount[slot];
-    for (uint32_t i = tid; i < ng; i += TILE_THREADS) {
+    if (my_entry != 0xFFFFFFFFu) cl.e[my_entry].hi = my_hi;
+    for (uint32_t i = tid + TILE_THREADS; i < ng; i += TILE_THREADS) {        // (more listed cells than threads: never at w ~ sigma)
       const uint32_t cell = ctl->clist[slot][i];
       const uint32_t gy = cell / p.mx, gx = cell - gy * p.mx;
       const uint32_t lx = wrap_cell((int)gx - gx0, p.mx), ly = wrap_cell((int)gy - gy0, p.my);

@@ -67,8 +67,6 @@ def main():
         whole = pc[:, :, -1] - pc[:, :, 1]
         has = ncrowd > 0
         if has.any() and (~has).any():
-            gen = extra[:, :, 2] - pc[:, :, 6]          # thread 0: from the end of sub-sweep 4 to the end of its crowded shift cells
-            print(f"  thread 0 reaches the chunk loop of the shift {gen[has].mean():.0f} cycles after sub-sweep 4 with a crowded cell, {gen[~has].mean():.0f} without")
             print(f"  tiles with a crowded cell in their region: {has.mean() * 100:.1f} % of (launch, tile) pairs; whole tile "
                   f"{whole[has].mean():.0f} cycles against {whole[~has].mean():.0f} without; per phase "
                   + ", ".join(f"{d[:, :, i][has].mean() - d[:, :, i][~has].mean():+.0f}" for i in range(d.shape[2])))
