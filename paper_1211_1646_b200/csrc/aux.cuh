@@ -395,7 +395,7 @@ __global__ void __launch_bounds__(HT_THREADS) k_contact_hist_tile(const __grid_c
   __shared__ float4 s01[CH * CW], s23[CH * CW];      // fp32 images of slots 0, 1 and 2, 3 (empty slot: +FAR)
   __shared__ uint32_t sg[CH * CW];                   // global index of the cell's slot pair 0
   __shared__ uint8_t sn[CH * CW];                    // its count
-  __shared__ uint32_t q_pair[NT / 32][HIST_QUEUE], q_code[NT / 32][HIST_QUEUE];
+  __shared__ uint32_t q_pair[NT / 32][96], q_code[NT / 32][96];    // per warp: fewer than 32 records left over + at most 64 new ones
   const uint32_t tid = threadIdx.x, lane = tid & 31u, ty = tid >> 5;
   for (uint32_t b = tid; b < nbins; b += NT) sh_hist[b] = 0;
   const uint32_t cur = p.ctl->cur;
@@ -436,78 +436,115 @@ __global__ void __launch_bounds__(HT_THREADS) k_contact_hist_tile(const __grid_c
   auto exact = [&](const uint32_t pair, const uint32_t code) {
     hist_pairs_exact<P>(p, pos, ids, sg[pair >> 16], sg[pair & 0xFFFFu], code, dr, nbins, rmax2, sh_hist);
   };
-#pragma unroll 1
-  for (uint32_t row = ty; row < (uint32_t)HT_H; row += NT / 32) {
-  const uint32_t own = row * CW + lane + RC;
-  const bool valid = x0 + lane < p.mx && y0 + row < p.my;
-  const uint32_t n = valid ? sn[own] : 0u;
-  const float4 a01 = s01[own], a23 = s23[own];
-  // negated own slots; an empty own slot goes to -FAR (empty neighbour slots sit at +FAR): no pair with an empty slot
-  // ever passes the filter
-  const F::Pair nax01 = F::pair(n > 0u ? -a01.x : FARF, n > 1u ? -a01.y : FARF), nay01 = F::pair(-a01.z, -a01.w);
-  const F::Pair nax23 = F::pair(n > 2u ? -a23.x : FARF, n > 3u ? -a23.y : FARF), nay23 = F::pair(-a23.z, -a23.w);
-  const bool own4 = n > 2u;
-  const uint32_t own_rows = 0x1111u & ((1u << (4u * n)) - 1u);    // bit 4 i for every own slot i < n
-  auto enqueue = [&](const bool has, const uint32_t nb, const int ox, const int oy, const bool self) {
-    const uint32_t m = __ballot_sync(0xFFFFFFFFu, has);
-    if (m == 0u) return;
-    if (has) {
-      const uint32_t at = qn + __popc(m & ((1u << lane) - 1u));
-      uint32_t cm = own_rows * ((1u << sn[nb]) - 1u);             // every pair of occupied slots; stage 2 filters exactly
-      if (self) cm &= 0x08CEu;                                    // inside a cell: each pair once (j > i)
-      qp[at] = (own << 16) | nb;
-      qc[at] = (uint32_t)(ox + 128) | ((uint32_t)(oy + 128) << 8) | (cm << 16);
-    }
-    qn += __popc(m);
+  // A thread owns TWO cells, one in each of its warp's rows (row, row + NT / 32): the per-offset work of a visit (the
+  // neighbour's index offset, its translation, the loop and the queue bookkeeping) is shared by both, and their
+  // arithmetic interleaves.
+  constexpr uint32_t NR = 2u, WARPS = NT / 32;
+  static_assert(HT_H % (NR * WARPS) == 0, "rows per warp");
+  struct OwnCell { uint32_t idx, rows; bool own4; F::Pair nax01, nay01, nax23, nay23; };
+  auto drain = [&]() {                                            // a full warp of records
+    exact(qp[lane], qc[lane]);
+    uint32_t a[2], c[2];
+#pragma unroll
+    for (uint32_t j = 0; j < 2u; ++j) { a[j] = qp[lane + 32u * (j + 1u)]; c[j] = qc[lane + 32u * (j + 1u)]; }
     __syncwarp();
-    if (qn >= 32u) {                                              // a full warp of records
-      exact(qp[lane], qc[lane]);
-      const uint32_t a = qp[lane + 32u], c = qc[lane + 32u];
-      __syncwarp();
-      if (lane + 32u < qn) { qp[lane] = a; qc[lane] = c; }        // the rest moves to the front
-      qn -= 32u;
-      __syncwarp();
-    }
+#pragma unroll
+    for (uint32_t j = 0; j < 2u; ++j)
+      if (lane + 32u * (j + 1u) < qn) { qp[lane + 32u * j] = a[j]; qc[lane + 32u * j] = c[j]; }   // the rest moves to the front
+    qn -= 32u;
+    __syncwarp();
   };
-  auto visit = [&](const int ox, const int oy) {
-    const uint32_t nb = (uint32_t)((int)own + oy * CW + ox);
-    const float4 b01 = s01[nb];
-    const float sx = (float)ox * wxf, sy = (float)oy * wyf;
-    const F::Pair Bx = F::padd(F::pair(b01.x, b01.y), F::pair(sx, sx)), By = F::padd(F::pair(b01.z, b01.w), F::pair(sy, sy));
-    const F::Pair r0 = r2_two(nax01.x, nay01.x, Bx, By), r1 = r2_two(nax01.y, nay01.y, Bx, By);
-    float rmin = fminf(F::min3(r0.x, r0.y, r1.x), r1.y);
-    if (crowded) {
-      const float4 b23 = s23[nb];
-      const F::Pair Cx = F::padd(F::pair(b23.x, b23.y), F::pair(sx, sx)), Cy = F::padd(F::pair(b23.z, b23.w), F::pair(sy, sy));
-      const F::Pair r2 = r2_two(nax01.x, nay01.x, Cx, Cy), r3 = r2_two(nax01.y, nay01.y, Cx, Cy);
-      const F::Pair r4 = r2_two(nax23.x, nay23.x, Bx, By), r5 = r2_two(nax23.y, nay23.y, Bx, By);
-      const F::Pair r6 = r2_two(nax23.x, nay23.x, Cx, Cy), r7 = r2_two(nax23.y, nay23.y, Cx, Cy);
-      rmin = fminf(rmin, fminf(fminf(F::min3(r2.x, r2.y, r3.x), F::min3(r3.y, r4.x, r4.y)),
-                               fminf(F::min3(r5.x, r5.y, r6.x), F::min3(r6.y, r7.x, r7.y))));
+#pragma unroll 1
+  for (uint32_t row0 = ty; row0 < (uint32_t)HT_H; row0 += NR * WARPS) {
+    OwnCell o[NR];
+#pragma unroll
+    for (uint32_t c = 0; c < NR; ++c) {
+      const uint32_t row = row0 + c * WARPS;
+      const uint32_t own = row * CW + lane + RC;
+      const bool valid = x0 + lane < p.mx && y0 + row < p.my;
+      const uint32_t n = valid ? sn[own] : 0u;
+      const float4 a01 = s01[own], a23 = s23[own];
+      // negated own slots; an empty own slot goes to -FAR (empty neighbour slots sit at +FAR): no pair with an empty
+      // slot ever passes the filter
+      o[c].idx = own; o[c].own4 = n > 2u;
+      o[c].nax01 = F::pair(n > 0u ? -a01.x : FARF, n > 1u ? -a01.y : FARF); o[c].nay01 = F::pair(-a01.z, -a01.w);
+      o[c].nax23 = F::pair(n > 2u ? -a23.x : FARF, n > 3u ? -a23.y : FARF); o[c].nay23 = F::pair(-a23.z, -a23.w);
+      o[c].rows = 0x1111u & ((1u << (4u * n)) - 1u);              // bit 4 i for every own slot i < n
     }
-    enqueue(rmin < thr2, nb, ox, oy, false);
-  };
+    // both cells' candidates of one offset go into the queue in one round (at most 64 new records on top of < 32)
+    auto enqueue = [&](const bool (&has)[NR], const uint32_t (&nb)[NR], const int ox, const int oy, const bool self) {
+      uint32_t m[NR];
+#pragma unroll
+      for (uint32_t c = 0; c < NR; ++c) m[c] = __ballot_sync(0xFFFFFFFFu, has[c]);
+      if ((m[0] | m[1]) == 0u) return;
+      uint32_t at = qn + __popc(m[0] & ((1u << lane) - 1u));
+#pragma unroll
+      for (uint32_t c = 0; c < NR; ++c) {
+        if (has[c]) {
+          uint32_t cm = o[c].rows * ((1u << sn[nb[c]]) - 1u);     // every pair of occupied slots; stage 2 filters exactly
+          if (self) cm &= 0x08CEu;                                // inside a cell: each pair once (j > i)
+          qp[at] = (o[c].idx << 16) | nb[c];
+          qc[at] = (uint32_t)(ox + 128) | ((uint32_t)(oy + 128) << 8) | (cm << 16);
+        }
+        if (c == 0u) at = qn + __popc(m[0]) + __popc(m[1] & ((1u << lane) - 1u));
+      }
+      qn += __popc(m[0]) + __popc(m[1]);
+      __syncwarp();
+      while (qn >= 32u) drain();
+    };
+    auto visit = [&](const int ox, const int oy) {
+      const int dnb = oy * CW + ox;
+      const float sx = (float)ox * wxf, sy = (float)oy * wyf;
+      bool has[NR]; uint32_t nb[NR];
+#pragma unroll
+      for (uint32_t c = 0; c < NR; ++c) {
+        nb[c] = (uint32_t)((int)o[c].idx + dnb);
+        const float4 b01 = s01[nb[c]];
+        const F::Pair Bx = F::padd(F::pair(b01.x, b01.y), F::pair(sx, sx)), By = F::padd(F::pair(b01.z, b01.w), F::pair(sy, sy));
+        const F::Pair r0 = r2_two(o[c].nax01.x, o[c].nay01.x, Bx, By), r1 = r2_two(o[c].nax01.y, o[c].nay01.y, Bx, By);
+        float rmin = fminf(F::min3(r0.x, r0.y, r1.x), r1.y);
+        if (crowded) {
+          const float4 b23 = s23[nb[c]];
+          const F::Pair Cx = F::padd(F::pair(b23.x, b23.y), F::pair(sx, sx)), Cy = F::padd(F::pair(b23.z, b23.w), F::pair(sy, sy));
+          const F::Pair r2 = r2_two(o[c].nax01.x, o[c].nay01.x, Cx, Cy), r3 = r2_two(o[c].nax01.y, o[c].nay01.y, Cx, Cy);
+          const F::Pair r4 = r2_two(o[c].nax23.x, o[c].nay23.x, Bx, By), r5 = r2_two(o[c].nax23.y, o[c].nay23.y, Bx, By);
+          const F::Pair r6 = r2_two(o[c].nax23.x, o[c].nay23.x, Cx, Cy), r7 = r2_two(o[c].nax23.y, o[c].nay23.y, Cx, Cy);
+          rmin = fminf(rmin, fminf(fminf(F::min3(r2.x, r2.y, r3.x), F::min3(r3.y, r4.x, r4.y)),
+                                   fminf(F::min3(r5.x, r5.y, r6.x), F::min3(r6.y, r7.x, r7.y))));
+        }
+        has[c] = rmin < thr2;
+      }
+      enqueue(has, nb, ox, oy, false);
+    };
 
-  // the pairs inside the cell, each once
-  {
-    const F::Pair Bx = F::pair(a01.y, a23.x), By = F::pair(a01.w, a23.z);       // own slots 1 and 2 as points
-    const F::Pair r0 = r2_two(nax01.x, nay01.x, Bx, By);                       // (0, 1), (0, 2)
-    float rmin = n >= 2u ? r0.x : FARF;
-    if (crowded) {
-      const F::Pair r1 = r2_two(nax01.y, nay01.y, Bx, By);                     // (1, 1) = 0, (1, 2)
-      const F::Pair Cx = F::pair(a23.y, a23.y), Cy = F::pair(a23.w, a23.w);     // own slot 3
-      const F::Pair r3 = r2_two(nax01.x, nay01.x, Cx, Cy), r4 = r2_two(nax01.y, nay01.y, Cx, Cy), r5 = r2_two(nax23.x, nay23.x, Cx, Cy);
-      if (own4) rmin = fminf(fminf(fminf(rmin, r0.y), fminf(r1.y, r3.x)), fminf(r4.x, r5.x));
+    // the pairs inside the cells, each once
+    {
+      bool has[NR]; uint32_t nb[NR];
+#pragma unroll
+      for (uint32_t c = 0; c < NR; ++c) {
+        nb[c] = o[c].idx;
+        // own slots 1, 2, 3 as points (un-negated); an empty one sits at -FAR
+        const F::Pair Bx = F::pair(-o[c].nax01.y, -o[c].nax23.x), By = F::pair(-o[c].nay01.y, -o[c].nay23.x);
+        const F::Pair r0 = r2_two(o[c].nax01.x, o[c].nay01.x, Bx, By);                     // (0, 1), (0, 2)
+        float rmin = r0.x;                                        // huge unless slots 0 and 1 are both occupied
+        if (crowded) {
+          const F::Pair r1 = r2_two(o[c].nax01.y, o[c].nay01.y, Bx, By);                   // (1, 1) = 0, (1, 2)
+          const F::Pair Cx = F::pair(-o[c].nax23.y, -o[c].nax23.y), Cy = F::pair(-o[c].nay23.y, -o[c].nay23.y);   // own slot 3
+          const F::Pair r3 = r2_two(o[c].nax01.x, o[c].nay01.x, Cx, Cy), r4 = r2_two(o[c].nax01.y, o[c].nay01.y, Cx, Cy),
+                        r5 = r2_two(o[c].nax23.x, o[c].nay23.x, Cx, Cy);
+          if (o[c].own4) rmin = fminf(fminf(fminf(rmin, r0.y), fminf(r1.y, r3.x)), fminf(r4.x, r5.x));
+        }
+        has[c] = rmin < thr2 && (o[c].rows & 0x10u) != 0u;         // (at least two disks in the cell)
+      }
+      enqueue(has, nb, 0, 0, true);
     }
-    enqueue(rmin < thr2, own, 0, 0, true);
-  }
-  // (rolled: one copy of the visit keeps the loop inside the instruction cache; the unrolled form stalled 30 % of its
-  // cycles on instruction fetch)
+    // (rolled: one copy of the visit keeps the loop inside the instruction cache; the unrolled form stalled 30 % of its
+    // cycles on instruction fetch)
 #pragma unroll 1
-  for (int oy = 0; oy <= RC; ++oy)
+    for (int oy = 0; oy <= RC; ++oy)
 #pragma unroll 1
-    for (int ox = (oy == 0 ? 1 : -RC); ox <= RC; ++ox)
-      if ((keep >> hist_offset_index(ox, oy, RC)) & 1ull) visit(ox, oy);
+      for (int ox = (oy == 0 ? 1 : -RC); ox <= RC; ++ox)
+        if ((keep >> hist_offset_index(ox, oy, RC)) & 1ull) visit(ox, oy);
   }
   if (lane < qn) exact(qp[lane], qc[lane]);
   __syncthreads();
