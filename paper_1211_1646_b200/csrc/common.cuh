@@ -21,6 +21,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <cstddef>
 
 namespace mpmc {
 
@@ -41,17 +42,18 @@ constexpr uint32_t CROWD_CAP = 256;       // cells with more than 2 disks the ti
 // Device-resident control block: the state that survives between launches.  Inside a launch the sweep index,
 // buffer parity, grid origin and per-sweep draws live in registers / shared memory (sweep.cuh, k_sweeps).
 struct Ctl {
+  // ---- the first 32 bytes are what a tile-kernel launch reads before it does anything: two 16-byte loads (ctl_header) ----
   unsigned long long t;            // sweep index
   uint32_t cur;                    // which buffer holds the current state
   uint32_t err;                    // sticky error bits
-  uint32_t bar;                    // arrival counter of the grid barrier (zeroed by the host before a launch)
-  uint32_t ticket;                 // blocks-done counter of the tile kernel
   // Cells holding more than 2 disks ("crowded") in the state at sweep t, kept per (t & 3): ccount = how many,
   // clist = their canonical ids y*mx+x in no particular order; crowded != 0: more than CROWD_CAP of them, the
   // list is incomplete and the tile kernel (tile.cuh) must leave this state to the general kernel.  Written by
   // whichever kernel produces the state; a slot is cleared two sweeps ahead of its use.
   uint32_t crowded[4];
   uint32_t ccount[4];
+  uint32_t bar;                    // arrival counter of the grid barrier (zeroed by the host before a launch)
+  uint32_t ticket;                 // blocks-started counter of the tile kernels
   uint32_t pad0[2];
   uint32_t clist[4][CROWD_CAP];
   double origin[2];                // grid origin: X = origin + cell * w + local
@@ -182,6 +184,20 @@ __device__ __forceinline__ void philox4x32_10_rk(const Params& p, uint32_t c0, u
   }
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
+
+// The head of the control block as two independent 16-byte loads, issued together: {t, cur, err} and crowded[0..3].
+struct CtlHeader { unsigned long long t; uint32_t cur, err; uint32_t crowded[4]; };
+__device__ __forceinline__ CtlHeader ctl_header(const Ctl* ctl) {
+  uint32_t a0, a1, a2, a3, b0, b1, b2, b3;
+  asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a0), "=r"(a1), "=r"(a2), "=r"(a3) : "l"(ctl) : "memory");
+  asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(b0), "=r"(b1), "=r"(b2), "=r"(b3)
+               : "l"(reinterpret_cast<const unsigned char*>(ctl) + 16) : "memory");
+  CtlHeader h;
+  h.t = ((unsigned long long)a1 << 32) | a0; h.cur = a2; h.err = a3;
+  h.crowded[0] = b0; h.crowded[1] = b1; h.crowded[2] = b2; h.crowded[3] = b3;
+  return h;
+}
+static_assert(offsetof(Ctl, cur) == 8 && offsetof(Ctl, crowded) == 16 && offsetof(Ctl, ccount) == 32, "ctl_header reads this layout");
 
 // a kernel that writes a cell with more than 2 disks into the state of sweep slot `slot` records it here
 __device__ __forceinline__ void note_crowded(Ctl* ctl, uint32_t slot, uint32_t cell) {

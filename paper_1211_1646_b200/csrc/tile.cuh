@@ -42,7 +42,7 @@ constexpr int SHIFT_U = 2;              // cells per lane and chunk in the shift
 
 // -DMPMC_PHASE_CLOCKS builds a variant that records clock64() at every phase boundary (phase_clocks.py).
 #ifdef MPMC_PHASE_CLOCKS
-constexpr uint32_t PHASE_TILES = 4096, PHASE_MARKS = 13;
+constexpr uint32_t PHASE_TILES = 4096, PHASE_MARKS = 16;
 __device__ unsigned long long g_phase_clocks[PHASE_TILES][PHASE_MARKS];
 __device__ __forceinline__ unsigned long long globaltimer_ns() { unsigned long long v; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(v)); return v; }
 // (the clock is read AFTER a shared-memory load that follows the barrier: a bare clock read right behind __syncthreads is
@@ -58,6 +58,12 @@ __device__ __forceinline__ unsigned long long clock_after(const volatile uint32_
 #endif
 
 #define MPMC_PHASE_MARK(i) MPMC_PHASE_MARK_AT(i, &s_last)
+// thread 0's own clock, no barrier implied (marks 11, 13-15: inside the load phase)
+#ifdef MPMC_PHASE_CLOCKS
+#define MPMC_PHASE_NOW(i) do { if (threadIdx.x == 0 && blockIdx.x < PHASE_TILES) g_phase_clocks[blockIdx.x][i] = clock_after(&s_last); } while (0)
+#else
+#define MPMC_PHASE_NOW(i) do { } while (0)
+#endif
 #ifdef MPMC_PHASE_CLOCKS
 #define MPMC_PHASE_VALUE(i, v) do { if (threadIdx.x == 0 && blockIdx.x < PHASE_TILES) g_phase_clocks[blockIdx.x][i] = (unsigned long long)(v); } while (0)
 #else
@@ -87,16 +93,25 @@ __device__ __forceinline__ void sts_half(SmemCell<double>* s, uint32_t i, const 
   s[i].a = make_double2(h.x.x, h.x.y); s[i].b = make_double2(h.y.x, h.y.y);
 }
 
-// asynchronous copy of one cell (slot pair i of the global planes) into shared memory, 16 bytes per cp.async, past L1
-__device__ __forceinline__ void cp_async_cell(SmemCell<float>* dst, const float* pos, uint32_t i) {
-  const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(d), "l"(reinterpret_cast<const float4*>(pos) + i) : "memory");
+// Bulk asynchronous copies global -> shared (cp.async.bulk, the TMA unit; SASS UBLKCP) that report to an mbarrier: ONE
+// instruction moves a whole plane row of the tile (up to 1 KB), so the tile load costs a few hundred instructions per
+// CTA instead of 13 LDGSTS per thread, and every warp is free for the sort while the bytes arrive.
+__device__ __forceinline__ uint32_t smem_addr(const void* ptr) { return (uint32_t)__cvta_generic_to_shared(ptr); }
+__device__ __forceinline__ void mbar_init_expect(const uint32_t mbar, const uint32_t bytes) {   // one thread, one phase
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(mbar) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(mbar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void cp_async_cell(SmemCell<double>* dst, const double* pos, uint32_t i) {
-  const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst);
-  const double2* src = reinterpret_cast<const double2*>(pos) + 2 * (size_t)i;
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(d), "l"(src) : "memory");
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(d + 16u), "l"(src + 1) : "memory");
+__device__ __forceinline__ void bulk_copy_g2s(const uint32_t dst, const void* src, const uint32_t bytes, const uint32_t mbar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               :: "r"(dst), "l"(src), "r"(bytes), "r"(mbar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(const uint32_t mbar, const uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(done) : "r"(mbar), "r"(parity) : "memory");
+  } while (done == 0u);
 }
 
 __device__ __forceinline__ float lds_x0(const SmemCell<float>* s, uint32_t i) { return s[i].v.x; }     // x of slot 0
@@ -114,23 +129,23 @@ struct TileBox {
 // loaded area the tile count can match the SM count (C3: 8 x 12 + 4 x 13 = 148) where a rectangular ntx x nty grid leaves
 // SMs idle (12 x 12 = 144).
 __device__ __forceinline__ TileBox tile_box(const Params& p, const uint32_t b) {
-  TileBox t;
+  TileBox t;                                     // (32-bit products: the host tiles boxes of fewer than 2^16 half-rows only)
   const uint32_t nA = p.tl_na * p.tl_ntx;
   uint32_t tx, ntx, h0, h1;
   if (b < nA) {
     const uint32_t r = b / p.tl_ntx;
     tx = b - r * p.tl_ntx; ntx = p.tl_ntx;
-    h0 = (uint32_t)((unsigned long long)p.tl_hyA * r / p.tl_na);
-    h1 = (uint32_t)((unsigned long long)p.tl_hyA * (r + 1u) / p.tl_na);
+    h0 = p.tl_hyA * r / p.tl_na;
+    h1 = p.tl_hyA * (r + 1u) / p.tl_na;
   } else {
     const uint32_t b2 = b - nA, nb = p.tl_nty - p.tl_na, hyB = p.hy - p.tl_hyA;
     const uint32_t r = b2 / (p.tl_ntx + 1u);
     tx = b2 - r * (p.tl_ntx + 1u); ntx = p.tl_ntx + 1u;
-    h0 = p.tl_hyA + (uint32_t)((unsigned long long)hyB * r / nb);
-    h1 = p.tl_hyA + (uint32_t)((unsigned long long)hyB * (r + 1u) / nb);
+    h0 = p.tl_hyA + hyB * r / nb;
+    h1 = p.tl_hyA + hyB * (r + 1u) / nb;
   }
-  t.x0 = 2u * (uint32_t)((unsigned long long)p.hx * tx / ntx);
-  t.TX = 2u * (uint32_t)((unsigned long long)p.hx * (tx + 1u) / ntx) - t.x0;
+  t.x0 = 2u * (p.hx * tx / ntx);
+  t.TX = 2u * (p.hx * (tx + 1u) / ntx) - t.x0;
   t.y0 = 2u * h0; t.TY = 2u * (h1 - h0);
   t.w = t.TX + 2 * HALO; t.h = t.TY + 2 * HALO;
   t.pw = t.w / 2; t.ph = t.h / 2;
@@ -171,7 +186,7 @@ __device__ __forceinline__ bool crowd_near(const CrowdList<P>& cl, uint32_t nc, 
 }
 
 // floor(n / d) for n < 2^16, 1 <= d < 2^16 with the per-phase constant inv = ceil(2^32 / d) (0 stands for d = 1)
-__device__ __forceinline__ uint32_t small_div_magic(uint32_t d) { return d == 1u ? 0u : (uint32_t)(0xFFFFFFFFull / d) + 1u; }
+__device__ __forceinline__ uint32_t small_div_magic(uint32_t d) { return d == 1u ? 0u : 0xFFFFFFFFu / d + 1u; }
 __device__ __forceinline__ uint32_t small_div(uint32_t n, uint32_t inv) { return inv == 0u ? n : __umulhi(n, inv); }
 
 // shared-memory offsets of the 3x3 cells relative to an active cell of local colour q (uniform per phase)
@@ -564,71 +579,34 @@ __device__ __forceinline__ SortArea sort_area(void* mem, const uint32_t PH) {
   return a;
 }
 constexpr uint32_t SORT_ROW_BYTES = 4u * 8u + 2u * 2u;   // per plane row: four masks and two bases
+constexpr uint32_t SORT_ROWS = 10;                       // plane rows a warp takes the count bytes of at a time (all of its rows up to 240 rows per tile)
 
 __device__ __forceinline__ float2 lds_x01(const SmemCell<float>* s, uint32_t i) { return make_float2(s[i].v.x, s[i].v.y); }
 __device__ __forceinline__ double2 lds_x01(const SmemCell<double>* s, uint32_t i) { return s[i].a; }
 // T[px + a] as a mask over px, a in {-1, 0, +1}
 __device__ __forceinline__ unsigned long long mask_shift(const unsigned long long T, const int a) { return a < 0 ? T << 1 : a > 0 ? T >> 1 : T; }
 
-// Phase A of the sort for one plane row r (= q * ph + py): bit px of occ / two = the cell holds >= 1 / >= 2 disks.  Called by
-// the warp that copied the row, as soon as its copies have landed (the load phase waits on L2 bandwidth with idle issue
-// slots; the masks of the early rows are taken under the copies of the late ones).
-template <typename P, bool DEBUG>
-__device__ __forceinline__ void sort_row_masks(const Params& p, const SmemCell<P>* sm, const TileBox& tb, const int gx0, const int gy0,
-                                               const SortArea sa, const uint32_t q, const uint32_t py) {
-  const uint32_t PS = p.tl_PS, PH = p.tl_PH, pw = tb.pw, lane = threadIdx.x & 31u;
-  const P HALF_FAR = Real<P>::far_away() * (P)0.5;
-  unsigned long long occ = 0ull, two = 0ull;
-#pragma unroll
-  for (uint32_t half = 0; half < 2u; ++half) {
-    const uint32_t px = lane + 32u * half;
-    bool o = false, w2 = false;
-    if (px < pw) {
-      const auto x = lds_x01(sm, q * PS + py * pw + px);     // slots fill in order
-      o = x.x < HALF_FAR; w2 = x.y < HALF_FAR;
-      if (DEBUG && !o) {                                       // an empty cell of the tile: nothing accepted
-        const uint32_t lx = 2u * px + (q & 1u), ly = 2u * py + (q >> 1);
-        if (lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY)
-          p.mask[wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx)] = 0u;
-      }
-    }
-    occ |= (unsigned long long)__ballot_sync(0xFFFFFFFFu, o) << (32u * half);
-    two |= (unsigned long long)__ballot_sync(0xFFFFFFFFu, w2) << (32u * half);
-  }
-  if (lane == 0u) { sa.occ[q * PH + py] = occ; sa.two[q * PH + py] = two; }
-}
-// cp.async.wait_group with a run-time count (the instruction takes an immediate)
-__device__ __forceinline__ void cp_async_wait_pending(const uint32_t n) {
-  switch (n) {
-    case 0: asm volatile("cp.async.wait_group 0;" ::: "memory"); break;
-    case 1: asm volatile("cp.async.wait_group 1;" ::: "memory"); break;
-    case 2: asm volatile("cp.async.wait_group 2;" ::: "memory"); break;
-    case 3: asm volatile("cp.async.wait_group 3;" ::: "memory"); break;
-    case 4: asm volatile("cp.async.wait_group 4;" ::: "memory"); break;
-    case 5: asm volatile("cp.async.wait_group 5;" ::: "memory"); break;
-    case 6: asm volatile("cp.async.wait_group 6;" ::: "memory"); break;
-    default: asm volatile("cp.async.wait_group 7;" ::: "memory"); break;
-  }
-}
+// barrier among the first `threads` threads of the CTA (the warps that sort while the others issue the tile's copies)
+__device__ __forceinline__ void sort_barrier(const uint32_t threads) { asm volatile("bar.sync 1, %0;" :: "r"(threads) : "memory"); }
 
+// Called by the first nws warps of the CTA (all of their threads).
 template <typename P, bool DEBUG>
 __device__ __forceinline__ void tile_sort_cells(const Params& p, const SmemCell<P>* sm, const CrowdList<P>& cl, const uint32_t nc,
                                                 const TileBox& tb, const Draws& dr, const int gx0, const int gy0,
-                                                uint16_t* queues, const SortArea sa, uint32_t (*s_cnt)[2]) {
+                                                uint16_t* queues, const SortArea sa, uint32_t (*s_cnt)[2], const uint32_t nws) {
   const uint32_t PS = p.tl_PS, PH = p.tl_PH, pw = tb.pw, ph = tb.ph;
-  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, NW = blockDim.x >> 5;
-  const P HALF_FAR = Real<P>::far_away() * (P)0.5;
+  const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, NW = nws;
   const uint32_t inv_ph = small_div_magic(ph);
-  // (phase A — the occupancy masks of every plane row, sort_row_masks — ran with the load, row by row as the copies landed)
+  // (phase A — the occupancy masks of every plane row — was taken from the count bytes by the warps that copy the rows)
   MPMC_PHASE_MARK_AT(9, &s_cnt[0][0]);
   if (nc != 0u) {                                        // (uniform) cells next to a crowded cell are nobody's here: a
-    for (uint32_t i = tid; i < 9u * nc; i += blockDim.x) {   // whole warp does them (tile_update_cell_warp)
+    for (uint32_t i = tid; i < 9u * nc; i += 32u * NW) {   // whole warp does them (tile_update_cell_warp)
       const uint32_t e = i / 9u, d = i - 9u * e;
       const uint32_t lx = (cl.e[e].lxly & 0xFFFFu) + d % 3u - 1u, ly = (cl.e[e].lxly >> 16) + d / 3u - 1u;   // may wrap below 0
       if (lx < tb.w && ly < tb.h)
         atomicAnd(&sa.occ[(((ly & 1u) << 1) | (lx & 1u)) * PH + (ly >> 1)], ~(1ull << (lx >> 1)));
     }
-    __syncthreads();
+    sort_barrier(32u * NW);
   }
   // ---- B + C: one warp per sub-sweep, one LANE per row: the row's simple and general cells (nine shifted ORs of row
   //      masks), then the exclusive prefix sums over the rows that place every row in the sub-sweep's queue ----
@@ -670,7 +648,7 @@ __device__ __forceinline__ void tile_sort_cells(const Params& p, const SmemCell<
     }
     if (lane == 0u) { s_cnt[k][0] = run1; s_cnt[k][1] = run2; }
   }
-  __syncthreads();
+  sort_barrier(32u * NW);
   MPMC_PHASE_MARK_AT(10, &s_cnt[0][0]);
   // ---- D: the plane indices, a warp per row, a lane per cell: simple cells from the front of the sub-sweep's queue,
   //      general cells from its back ----
@@ -682,15 +660,15 @@ __device__ __forceinline__ void tile_sort_cells(const Params& p, const SmemCell<
     uint32_t at1 = sa.base1[k * PH + py], at2 = PS - 1u - sa.base2[k * PH + py];
     const uint32_t below = (1u << lane) - 1u;
 #pragma unroll
-    for (uint32_t half = 0; half < 2u; ++half) {
+    for (uint32_t half = 0; half < 2u; ++half) {          // a cell is in at most one of the two classes: one store
       const uint32_t w1 = (uint32_t)(m1 >> (32u * half)), w2 = (uint32_t)(m2 >> (32u * half));
-      const uint32_t v = py * pw + lane + 32u * half;
-      if ((w1 >> lane) & 1u) qk[at1 + (uint32_t)__popc(w1 & below)] = (uint16_t)v;
-      if ((w2 >> lane) & 1u) qk[at2 - (uint32_t)__popc(w2 & below)] = (uint16_t)v;
-      at1 += (uint32_t)__popc(w1); at2 -= (uint32_t)__popc(w2);
+      const bool is1 = (w1 >> lane) & 1u, is2 = (w2 >> lane) & 1u;
+      const uint32_t c = (uint32_t)__popc((is1 ? w1 : w2) & below);
+      if (is1 || is2) qk[is1 ? at1 + c : at2 - c] = (uint16_t)(py * pw + lane + 32u * half);
+      if (half == 0u) { at1 += (uint32_t)__popc(w1); at2 -= (uint32_t)__popc(w2); }
     }
   }
-  __syncthreads();
+  sort_barrier(32u * NW);
 }
 
 // A simple cell (see above): one disk, no second disk anywhere in the 3x3 cells.  Same arithmetic per disk as
@@ -924,7 +902,10 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   extern __shared__ __align__(16) unsigned char tile_smem[];
   SmemCell<P>* sm = reinterpret_cast<SmemCell<P>*>(tile_smem);
   __shared__ CrowdList<P> cl;
-  __shared__ uint32_t s_last;
+#ifdef MPMC_PHASE_CLOCKS
+  __shared__ uint32_t s_last;                    // (the word the phase marks read behind a barrier)
+#endif
+  __shared__ __align__(8) unsigned long long s_mbar;   // completion of the tile load (bulk copies)
   __shared__ uint32_t s_next[8];                 // chunk counters: sub-sweeps 1-4, shift planes 0-3
   __shared__ uint32_t s_cnt[4][2];               // SORTED: simple / general cells queued per sub-sweep
   Ctl* ctl = p.ctl;
@@ -933,33 +914,150 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   // wait.  Launched with programmatic stream serialisation (mpmc.cu): everything below the wait reads what the previous
   // sweep wrote.  If the state is not at sweep t (an earlier launch left its sweep to the general kernel), return.
   const Draws dr = draw_sweep(p, t);
-  asm volatile("griddepcontrol.wait;" ::: "memory");
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  if (ctl->t != t) return;
-  const uint32_t slot = (uint32_t)(t & 3u), slot1 = (uint32_t)((t + 1ull) & 3u), slot2 = (uint32_t)((t + 2ull) & 3u);
-  if (ctl->crowded[slot] != 0u) return;          // too many crowded cells: the general kernel takes over
-  MPMC_PHASE_MARK(0); MPMC_PHASE_MARK(1);
-  const uint32_t cur = ctl->cur, nxt = cur ^ 1u;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-  // the list of crowded cells of this state: its first TILE_THREADS entries are fetched NOW (the chain count -> cell ->
-  // slots 2, 3 is three trips to L2; started here it ends under the tile load instead of behind it)
-  const uint32_t ng = ctl->ccount[slot];
-  const uint32_t my_listed = tid < ng ? ctl->clist[slot][tid] : 0xFFFFFFFFu;
   const TileBox tb = tile_box(p, blockIdx.x);
   const uint32_t PS = p.tl_PS, pw = tb.pw, ph = tb.ph, Mqp = p.Mqp;
   const int gx0 = (int)tb.x0 - HALO, gy0 = (int)tb.y0 - HALO;       // global cell of the region's corner (unwrapped)
+  const uint32_t nrows = 4u * ph, inv_ph = small_div_magic(ph), NW = TILE_THREADS / 32;
+  const uint32_t mbar = smem_addr(&s_mbar);
+  const uint32_t NPROD = NW >= 12u ? NW / 6u : 1u, NWS = NW - NPROD;   // SORTED: warps that issue the copies / that sort
+  // SORTED: where this lane's cells px = lane (.x) and lane + 32 (.y) of a plane row sit in the row's global colour planes,
+  // for rows of local colours with qx = 0 (col0) and qx = 1 (col1)
+  uint2 col0 = make_uint2(0u, 0u), col1 = col0;
+  if (SORTED) {
+    const uint32_t g00 = wrap_cell(gx0 + (int)(2u * lane), p.mx), g01 = wrap_cell(gx0 + (int)(2u * (lane + 32u)), p.mx);
+    const uint32_t g10 = wrap_cell(gx0 + (int)(2u * lane + 1u), p.mx), g11 = wrap_cell(gx0 + (int)(2u * (lane + 32u) + 1u), p.mx);
+    col0 = make_uint2((g00 & 1u) * Mqp + (g00 >> 1), (g01 & 1u) * Mqp + (g01 >> 1));
+    col1 = make_uint2((g10 & 1u) * Mqp + (g10 >> 1), (g11 & 1u) * Mqp + (g11 >> 1));
+  }
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const CtlHeader ch = ctl_header(ctl);          // sweep index, buffer parity, "too many crowded cells": one trip to L2
+  if (ch.t != t) return;
+  const uint32_t slot = (uint32_t)(t & 3u), slot1 = (uint32_t)((t + 1ull) & 3u), slot2 = (uint32_t)((t + 2ull) & 3u);
+  if ((slot == 0u ? ch.crowded[0] : slot == 1u ? ch.crowded[1] : slot == 2u ? ch.crowded[2] : ch.crowded[3]) != 0u)
+    return;                                      // too many crowded cells: the general kernel takes over
+  MPMC_PHASE_MARK(0); MPMC_PHASE_MARK(1);
+  const uint32_t cur = ch.cur, nxt = cur ^ 1u;
+  // plain variant: the list of crowded cells of this state, its first TILE_THREADS entries fetched NOW (the chain count ->
+  // cell -> slots 2, 3 is three trips to L2; started here it ends under the tile load instead of behind it).  The sorted
+  // variant finds the crowded cells of its region in the count bytes it reads anyway.
+  uint32_t ng = 0u, my_listed = 0xFFFFFFFFu;
+  if (!SORTED) {
+    ng = ctl->ccount[slot];
+    if (tid < ng) my_listed = ctl->clist[slot][tid];
+  }
   if (tid == 0) {
     cl.n = 0u;
     for (int i = 0; i < 8; ++i) s_next[i] = 0u;
     ctl->crowded[slot2] = 0u; ctl->ccount[slot2] = 0u;   // slots of the sweep after next: nobody uses them now
+    mbar_init_expect(mbar, nrows * pw * (uint32_t)sizeof(SmemCell<P>));   // the bytes of the whole region
   }
   __syncthreads();
+  MPMC_PHASE_NOW(11);
 
-  // ---- load the tile and its halo: warps take plane rows, lanes run along the row (512 contiguous bytes).  Asynchronous
-  //      copies global -> shared (cp.async, 16 bytes each): no register staging, so every copy of a thread (13 at C3) is
-  //      in flight at once; the phase then runs at the L2 -> SM bandwidth all SMs share (measured 6 TB/s) ----
-  {
-    const P* posc = reinterpret_cast<const P*>(p.pos[cur]);
+  // ---- load the tile and its halo: a plane row of the region is contiguous in its global colour plane (two pieces where
+  //      it wraps around the box), so a row is ONE bulk copy global -> shared, issued by one thread and reported to the
+  //      CTA's mbarrier; the phase runs at the L2 -> SM bandwidth all SMs share (measured 6 TB/s) with the issue slots free ----
+  const P* posc = reinterpret_cast<const P*>(p.pos[cur]);
+  // one bulk copy (two where the row wraps around the box) for plane row (q, py); called by ONE lane
+  auto copy_row = [&](const uint32_t q, const uint32_t py) {
+    const uint32_t gy = wrap_cell(gy0 + (int)(2u * py + (q >> 1)), p.my), gx = wrap_cell(gx0 + (int)(q & 1u), p.mx);
+    const uint32_t first = gx >> 1, n1 = min(pw, p.hx - first);                // the box has an even number of cells: the
+    const size_t row = (size_t)(2u * (((gy & 1u) << 1) | (gx & 1u))) * Mqp + (size_t)(gy >> 1) * p.hx;   // colour holds along the row
+    const unsigned char* src = reinterpret_cast<const unsigned char*>(posc);
+    const uint32_t dst = smem_addr(sm + q * PS + py * pw);
+    bulk_copy_g2s(dst, src + (row + first) * sizeof(SmemCell<P>), n1 * (uint32_t)sizeof(SmemCell<P>), mbar);
+    if (n1 < pw) bulk_copy_g2s(dst + n1 * (uint32_t)sizeof(SmemCell<P>), src + row * sizeof(SmemCell<P>), (pw - n1) * (uint32_t)sizeof(SmemCell<P>), mbar);
+  };
+  uint16_t* queues = reinterpret_cast<uint16_t*>(sm + 4u * PS);   // SORTED: the queues of the four sub-sweeps (behind the planes)
+  if (SORTED) {
+    // The sort needs occupancies, not positions: it works from the count bytes of the region (1 byte per cell against 16),
+    // so the whole sort — row masks, classes, prefix sums, queues — runs under the copies of the positions, whose phase is
+    // bound by L2 bandwidth and leaves the issue slots idle.  A count above 2 is a crowded cell of the region.
+    // A warp takes a block of consecutive plane rows (row arithmetic by increments); lanes run along the row.
+    const uint8_t* cntc = p.cnt[cur];
+    const SortArea sa_load = sort_area(queues + 4u * PS, p.tl_PH);
+    // Warp roles: the last NPROD warps only ISSUE the copies (a thread that issues bulk copies stalls while the copy
+    // queue is full, i.e. for most of the load: measured), the other NWS warps sort.
+    const uint32_t rpw = min(SORT_ROWS, (nrows + NWS - 1u) / NWS);             // rows per sorting warp and round
+    if (warp >= NWS) {
+      asm volatile("bar.sync 2, %0;" :: "r"(TILE_THREADS) : "memory");   // (see below)
+      const uint32_t share = (nrows + NPROD - 1u) / NPROD, first = (warp - NWS) * share, last = min(nrows, first + share);
+      for (uint32_t r = first + lane; r < last; r += 32u) { const uint32_t q = small_div(r, inv_ph); copy_row(q, r - q * ph); }
+    }
+    bool told = warp >= NWS;
+    const bool has0 = lane < pw, has1 = lane + 32u < pw;
+    for (uint32_t r0 = warp * rpw; warp < NWS && r0 < nrows; r0 += rpw * NWS) {
+      const uint32_t nr = min(rpw, nrows - r0);
+      // lane j works out where row j of the block lies; the loops below fetch that with a shuffle
+      uint32_t my_off = 0u, my_q = 0u, my_py = 0u;
+      if (lane < nr) {
+        my_q = small_div(r0 + lane, inv_ph); my_py = r0 + lane - my_q * ph;
+        const uint32_t gy = wrap_cell(gy0 + (int)(2u * my_py + (my_q >> 1)), p.my);
+        my_off = ((gy & 1u) << 1) * Mqp + (gy >> 1) * p.hx;
+      }
+      uint32_t c0[SORT_ROWS], c1[SORT_ROWS];     // counts of the cells px = lane, lane + 32 of the warp's rows
+#pragma unroll
+      for (uint32_t j = 0; j < SORT_ROWS; ++j) {
+        c0[j] = 0u; c1[j] = 0u;
+        if (j < nr) {                            // (warp-uniform)
+          const uint32_t off = __shfl_sync(0xFFFFFFFFu, my_off, j), qx = __shfl_sync(0xFFFFFFFFu, my_q, j) & 1u;
+          if (has0) c0[j] = ld_u8_early(cntc + (off + (qx ? col1.x : col0.x)));
+          if (has1) c1[j] = ld_u8_early(cntc + (off + (qx ? col1.y : col0.y)));
+        }
+      }
+      // the copies start once the count bytes have been REQUESTED: behind the copies' requests in the SM's queue to L2 they
+      // would arrive with the last rows (measured)
+      if (!told) { asm volatile("bar.arrive 2, %0;" :: "r"(TILE_THREADS) : "memory"); told = true; }
+      MPMC_PHASE_NOW(13);
+      // phase A of the sort: the occupancy masks of these rows (lane j ends up with the masks of row j and stores them)
+      uint2 m_occ = make_uint2(0u, 0u), m_two = m_occ;
+      uint32_t most = 0u;
+#pragma unroll
+      for (uint32_t j = 0; j < SORT_ROWS; ++j) {
+        if (j < nr) {
+          const uint32_t b1a = __ballot_sync(0xFFFFFFFFu, c0[j] >= 1u), b1b = __ballot_sync(0xFFFFFFFFu, c1[j] >= 1u);
+          const uint32_t b2a = __ballot_sync(0xFFFFFFFFu, c0[j] >= 2u), b2b = __ballot_sync(0xFFFFFFFFu, c1[j] >= 2u);
+          if (lane == j) { m_occ = make_uint2(b1a, b1b); m_two = make_uint2(b2a, b2b); }
+          most = max(most, max(c0[j], c1[j]));
+        }
+      }
+      if (lane < nr) {
+        reinterpret_cast<uint2*>(sa_load.occ)[my_q * p.tl_PH + my_py] = m_occ;
+        reinterpret_cast<uint2*>(sa_load.two)[my_q * p.tl_PH + my_py] = m_two;
+      }
+      if (__any_sync(0xFFFFFFFFu, most > 2u)) {  // (rare) crowded cells: into the tile's list
+#pragma unroll
+        for (uint32_t j = 0; j < SORT_ROWS; ++j) {
+          const uint32_t q = __shfl_sync(0xFFFFFFFFu, my_q, j), py = __shfl_sync(0xFFFFFFFFu, my_py, j);
+#pragma unroll
+          for (uint32_t half = 0; half < 2u; ++half) {
+            if (j < nr && (half == 0u ? c0[j] : c1[j]) > 2u) {
+              const uint32_t px = lane + 32u * half, e = atomicAdd(&cl.n, 1u);
+              cl.e[e].si = q * PS + py * pw + px;
+              cl.e[e].lxly = (2u * px + (q & 1u)) | ((2u * py + (q >> 1)) << 16);
+            }
+          }
+        }
+      }
+      if (DEBUG) {                               // an empty cell of the tile: nothing accepted
+#pragma unroll
+        for (uint32_t j = 0; j < SORT_ROWS; ++j) {
+          const uint32_t q = __shfl_sync(0xFFFFFFFFu, my_q, j), py = __shfl_sync(0xFFFFFFFFu, my_py, j);
+#pragma unroll
+          for (uint32_t half = 0; half < 2u; ++half) {
+            const uint32_t px = lane + 32u * half, lx = 2u * px + (q & 1u), ly = 2u * py + (q >> 1);
+            if (j < nr && px < pw && (half == 0u ? c0[j] : c1[j]) == 0u && lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY)
+              p.mask[wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx)] = 0u;
+          }
+        }
+      }
+    }
+    if (!told) asm volatile("bar.arrive 2, %0;" :: "r"(TILE_THREADS) : "memory");
+  } else {
+    for (uint32_t r = warp; r < nrows; r += NW)
+      if (lane == 0u) { const uint32_t q = small_div(r, inv_ph); copy_row(q, r - q * ph); }
     // the crowded cells of this state that lie in the region, with their slots 2 and 3: entry tid was fetched at the top;
     // the load of its slots 2, 3 is issued here and stored behind the tile's copies
     uint32_t my_entry = 0xFFFFFFFFu;
@@ -974,35 +1072,6 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
         my_hi = ld_half(posc, (2u * (((gy & 1u) << 1) | (gx & 1u)) + 1u) * Mqp + (gy >> 1) * p.hx + (gx >> 1));
       }
     }
-    const uint32_t nrows = 4u * ph, inv_ph = small_div_magic(ph), NW = TILE_THREADS / 32;
-    const SortArea sa_load = sort_area(reinterpret_cast<uint16_t*>(sm + 4u * PS) + 4u * PS, p.tl_PH);
-    // a warp's rows in groups of eight: one cp.async group per row, so that (SORTED) the occupancy masks of a row can be
-    // taken as soon as ITS copies have landed, under the copies of the rows behind it
-    for (uint32_t r8 = warp; r8 < nrows; r8 += 8u * NW) {
-#pragma unroll
-      for (uint32_t j = 0; j < 8u; ++j) {
-        const uint32_t r = r8 + j * NW;
-        if (r < nrows) {
-          const uint32_t q = small_div(r, inv_ph), py = r - q * ph;
-          const uint32_t gy = wrap_cell(gy0 + (int)(2u * py + (q >> 1)), p.my);
-          const uint32_t gbase = 2u * ((gy & 1u) << 1) * Mqp + (gy >> 1) * p.hx, sbase = q * PS + py * pw;
-          for (uint32_t px = lane; px < pw; px += 32u) {
-            const uint32_t gx = wrap_cell(gx0 + (int)(2u * px + (q & 1u)), p.mx);
-            cp_async_cell(sm + sbase + px, posc, gbase + 2u * (gx & 1u) * Mqp + (gx >> 1));
-          }
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-      }
-      if (SORTED) {
-#pragma unroll
-        for (uint32_t j = 0; j < 8u; ++j) {
-          const uint32_t r = r8 + j * NW;
-          cp_async_wait_pending(7u - j);
-          __syncwarp();
-          if (r < nrows) { const uint32_t q = small_div(r, inv_ph); sort_row_masks<P, DEBUG>(p, sm, tb, gx0, gy0, sa_load, q, r - q * ph); }
-        }
-      }
-    }
     if (my_entry != 0xFFFFFFFFu) cl.e[my_entry].hi = my_hi;
     for (uint32_t i = tid + TILE_THREADS; i < ng; i += TILE_THREADS) {        // (more listed cells than threads: never at w ~ sigma)
       const uint32_t cell = ctl->clist[slot][i];
@@ -1015,13 +1084,48 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
         cl.e[e].hi = ld_half(posc, (2u * (((gy & 1u) << 1) | (gx & 1u)) + 1u) * Mqp + (gy >> 1) * p.hx + (gx >> 1));
       }
     }
-    asm volatile("cp.async.wait_all;" ::: "memory");
   }
-  __syncthreads();
-  const uint32_t nc = cl.n;
-  // SORTED: the queues of the four sub-sweeps (behind the planes in dynamic shared memory, one plane's worth of u16 each)
-  uint16_t* queues = reinterpret_cast<uint16_t*>(sm + 4u * PS);
-  if (SORTED) tile_sort_cells<P, DEBUG>(p, sm, cl, nc, tb, dr, gx0, gy0, queues, sort_area(queues + 4u * PS, p.tl_PH), s_cnt);
+  MPMC_PHASE_NOW(14);
+  // ---- the control block of the next sweep.  Every CTA takes a ticket once it has read the block (above); the one that
+  //      draws the last ticket knows that all have, and advances it right away — nothing below reads it, and the next
+  //      launch waits for this one to complete — so no CTA waits for a counter at its end. ----
+  const uint32_t dir = dr.dir;
+  const bool along_x = dir < 2u, positive = (dir & 1u) == 0u;
+  const P w = along_x ? R::wx(p) : R::wy(p);
+  const P delta = R::mul(R::mul((P)0.5, w), R::unit(dr.dist_word));   // line 15 (L90)
+  if (tid == TILE_THREADS - 32u && atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1u) {   // (a warp that does not sort)
+    const double L = along_x ? p.Lx_eff : p.Ly_eff;
+    double o = ctl->origin[along_x ? 0 : 1];     // the grid origin follows the shift
+    o = __dadd_rn(o, positive ? (double)delta : -(double)delta);
+    if (o >= L) o = __dsub_rn(o, L);
+    if (o < 0.0) o = __dadd_rn(o, L);
+    ctl->origin[along_x ? 0 : 1] = o;
+    ctl->ticket = 0u;
+    ctl->cur = nxt;
+    ctl->t = t + 1ull;
+    ctl->path_sweeps[0] += 1ull;
+  }
+  uint32_t nc;
+  if (SORTED) {
+    if (warp < NWS) {
+      sort_barrier(32u * NWS);                   // row masks and the list of crowded cells are complete
+      const uint32_t ncs = cl.n;
+      tile_sort_cells<P, DEBUG>(p, sm, cl, ncs, tb, dr, gx0, gy0, queues, sort_area(queues + 4u * PS, p.tl_PH), s_cnt, NWS);
+      for (uint32_t i = tid; i < ncs; i += 32u * NWS) {              // slots 2 and 3 of the crowded cells
+        const uint32_t v = cl.e[i].lxly;
+        const uint32_t gx = wrap_cell(gx0 + (int)(v & 0xFFFFu), p.mx), gy = wrap_cell(gy0 + (int)(v >> 16), p.my);
+        cl.e[i].hi = ld_half(posc, (2u * (((gy & 1u) << 1) | (gx & 1u)) + 1u) * Mqp + (gy >> 1) * p.hx + (gx >> 1));
+      }
+    }
+    MPMC_PHASE_NOW(15);
+    mbar_wait(mbar, 0u);                         // the region has arrived
+    __syncthreads();                             // ... the queues are written and the list is complete
+    nc = cl.n;
+  } else {
+    mbar_wait(mbar, 0u);
+    __syncthreads();
+    nc = cl.n;
+  }
   MPMC_PHASE_MARK(2);
   MPMC_PHASE_VALUE(12, nc);                      // crowded cells in this tile's region
   Tally tally;
@@ -1067,33 +1171,14 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   }
 
   // ---- cell shift (Alg. 1 lines 15-17; Algorithm 4) of the interior cells, shared memory -> other buffer ----
-  const uint32_t dir = dr.dir;
-  const bool along_x = dir < 2u, positive = (dir & 1u) == 0u;
-  const P w = along_x ? R::wx(p) : R::wy(p);
-  const P delta = R::mul(R::mul((P)0.5, w), R::unit(dr.dist_word));   // line 15 (L90)
   if (along_x) tile_shift_cells<P, true>(p, sm, cl, nc, tb, gx0, gy0, positive, delta, cur, slot1, &s_next[4]);
   else         tile_shift_cells<P, false>(p, sm, cl, nc, tb, gx0, gy0, positive, delta, cur, slot1, &s_next[4]);
-
-  // ---- counters; the last CTA to finish advances the control block ----
-  flush_tally(p, tally);
+  flush_tally(p, tally);                         // counters
+#ifdef MPMC_PHASE_CLOCKS
   __syncthreads();
   MPMC_PHASE_MARK(7);
-  // (no fence: nothing written here is read before the launch completes, and the next launch waits for that)
-  if (tid == 0) s_last = (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1u) ? 1u : 0u;
-  __syncthreads();
-  if (s_last && tid == 0) {
-    const double L = along_x ? p.Lx_eff : p.Ly_eff;
-    double o = ctl->origin[along_x ? 0 : 1];     // the grid origin follows the shift
-    o = __dadd_rn(o, positive ? (double)delta : -(double)delta);
-    if (o >= L) o = __dsub_rn(o, L);
-    if (o < 0.0) o = __dadd_rn(o, L);
-    ctl->origin[along_x ? 0 : 1] = o;
-    ctl->ticket = 0u;
-    ctl->cur = nxt;
-    ctl->t = t + 1ull;
-    ctl->path_sweeps[0] += 1ull;
-  }
   MPMC_PHASE_MARK(8);
+#endif
 }
 
 }  // namespace mpmc

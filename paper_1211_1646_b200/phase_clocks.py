@@ -62,6 +62,12 @@ def main():
         ends = [extra[:, :, i] for i in range(2)]
         print("  inside 'load': the sort ends " + ", ".join(f"{n} {(t_load_end - e).mean():.0f}" for n, e in zip(names, ends))
               + " cycles before the end of the phase")
+    if extra is not None and extra.shape[2] >= 7 and extra[:, :, 4].min() > 0:
+        t1 = pc[:, :, 1]
+        pts = [("first barrier", extra[:, :, 2]), ("count bytes requested, copies issued (warp 0)", extra[:, :, 4]),
+               ("count bytes arrived (warp 0)", extra[:, :, 5]), ("row masks of all warps (barrier)", extra[:, :, 0]),
+               ("classes + prefix sums", extra[:, :, 1]), ("region arrived, queues written", extra[:, :, 6])]
+        print("  inside 'load', cycles after its start: " + "; ".join(f"{n} {(e - t1).mean():.0f}" for n, e in pts))
     if extra is not None and extra.shape[2] >= 4:
         ncrowd = extra[:, :, 3]
         whole = pc[:, :, -1] - pc[:, :, 1]
