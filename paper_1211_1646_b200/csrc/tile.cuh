@@ -930,6 +930,26 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
     col0 = make_uint2((g00 & 1u) * Mqp + (g00 >> 1), (g01 & 1u) * Mqp + (g01 >> 1));
     col1 = make_uint2((g10 & 1u) * Mqp + (g10 >> 1), (g11 & 1u) * Mqp + (g11 >> 1));
   }
+  if (tid == 0) {
+    cl.n = 0u;
+    for (int i = 0; i < 8; ++i) s_next[i] = 0u;
+    mbar_init_expect(mbar, nrows * pw * (uint32_t)sizeof(SmemCell<P>));   // the bytes of the whole region
+  }
+  // SORTED: a sorting warp takes blocks of rpw consecutive plane rows; lane j works out where row j of the block lies (the
+  // loops of the load phase fetch that with a shuffle).  The first block is set up here, ahead of the wait.
+  const uint32_t rpw = min(SORT_ROWS, (nrows + NWS - 1u) / NWS);
+  uint32_t my_off = 0u, my_q = 0u, my_py = 0u;
+  auto row_setup = [&](const uint32_t r0) {
+    my_off = 0u; my_q = 0u; my_py = 0u;
+    if (r0 + lane < nrows && lane < rpw) {
+      my_q = small_div(r0 + lane, inv_ph); my_py = r0 + lane - my_q * ph;
+      const uint32_t gy = wrap_cell(gy0 + (int)(2u * my_py + (my_q >> 1)), p.my);
+      my_off = ((gy & 1u) << 1) * Mqp + (gy >> 1) * p.hx;
+    }
+  };
+  if (SORTED) row_setup(warp * rpw);
+  __syncthreads();
+  // ---- everything above is a function of the launch parameters; what follows reads what the previous sweep wrote ----
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const CtlHeader ch = ctl_header(ctl);          // sweep index, buffer parity, "too many crowded cells": one trip to L2
@@ -947,13 +967,6 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
     ng = ctl->ccount[slot];
     if (tid < ng) my_listed = ctl->clist[slot][tid];
   }
-  if (tid == 0) {
-    cl.n = 0u;
-    for (int i = 0; i < 8; ++i) s_next[i] = 0u;
-    ctl->crowded[slot2] = 0u; ctl->ccount[slot2] = 0u;   // slots of the sweep after next: nobody uses them now
-    mbar_init_expect(mbar, nrows * pw * (uint32_t)sizeof(SmemCell<P>));   // the bytes of the whole region
-  }
-  __syncthreads();
   MPMC_PHASE_NOW(11);
 
   // ---- load the tile and its halo: a plane row of the region is contiguous in its global colour plane (two pieces where
@@ -980,7 +993,6 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
     const SortArea sa_load = sort_area(queues + 4u * PS, p.tl_PH);
     // Warp roles: the last NPROD warps only ISSUE the copies (a thread that issues bulk copies stalls while the copy
     // queue is full, i.e. for most of the load: measured), the other NWS warps sort.
-    const uint32_t rpw = min(SORT_ROWS, (nrows + NWS - 1u) / NWS);             // rows per sorting warp and round
     if (warp >= NWS) {
       asm volatile("bar.sync 2, %0;" :: "r"(TILE_THREADS) : "memory");   // (see below)
       const uint32_t share = (nrows + NPROD - 1u) / NPROD, first = (warp - NWS) * share, last = min(nrows, first + share);
@@ -990,13 +1002,7 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
     const bool has0 = lane < pw, has1 = lane + 32u < pw;
     for (uint32_t r0 = warp * rpw; warp < NWS && r0 < nrows; r0 += rpw * NWS) {
       const uint32_t nr = min(rpw, nrows - r0);
-      // lane j works out where row j of the block lies; the loops below fetch that with a shuffle
-      uint32_t my_off = 0u, my_q = 0u, my_py = 0u;
-      if (lane < nr) {
-        my_q = small_div(r0 + lane, inv_ph); my_py = r0 + lane - my_q * ph;
-        const uint32_t gy = wrap_cell(gy0 + (int)(2u * my_py + (my_q >> 1)), p.my);
-        my_off = ((gy & 1u) << 1) * Mqp + (gy >> 1) * p.hx;
-      }
+      if (r0 != warp * rpw) row_setup(r0);
       uint32_t c0[SORT_ROWS], c1[SORT_ROWS];     // counts of the cells px = lane, lane + 32 of the warp's rows
 #pragma unroll
       for (uint32_t j = 0; j < SORT_ROWS; ++j) {
@@ -1093,7 +1099,10 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   const bool along_x = dir < 2u, positive = (dir & 1u) == 0u;
   const P w = along_x ? R::wx(p) : R::wy(p);
   const P delta = R::mul(R::mul((P)0.5, w), R::unit(dr.dist_word));   // line 15 (L90)
-  if (tid == TILE_THREADS - 32u && atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1u) {   // (a warp that does not sort)
+  if (tid == TILE_THREADS - 32u) {               // (a thread of a warp that does not sort)
+    ctl->crowded[slot2] = 0u; ctl->ccount[slot2] = 0u;   // slots of the sweep after next: nobody uses them now
+  }
+  if (tid == TILE_THREADS - 32u && atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1u) {
     const double L = along_x ? p.Lx_eff : p.Ly_eff;
     double o = ctl->origin[along_x ? 0 : 1];     // the grid origin follows the shift
     o = __dadd_rn(o, positive ? (double)delta : -(double)delta);
@@ -1109,9 +1118,12 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   if (SORTED) {
     if (warp < NWS) {
       sort_barrier(32u * NWS);                   // row masks and the list of crowded cells are complete
+      asm volatile("bar.arrive 3, %0;" :: "r"(TILE_THREADS) : "memory");
+      tile_sort_cells<P, DEBUG>(p, sm, cl, cl.n, tb, dr, gx0, gy0, queues, sort_area(queues + 4u * PS, p.tl_PH), s_cnt, NWS);
+    } else {                                     // the warps that issued the copies fetch slots 2 and 3 of the crowded cells
+      asm volatile("bar.sync 3, %0;" :: "r"(TILE_THREADS) : "memory");
       const uint32_t ncs = cl.n;
-      tile_sort_cells<P, DEBUG>(p, sm, cl, ncs, tb, dr, gx0, gy0, queues, sort_area(queues + 4u * PS, p.tl_PH), s_cnt, NWS);
-      for (uint32_t i = tid; i < ncs; i += 32u * NWS) {              // slots 2 and 3 of the crowded cells
+      for (uint32_t i = tid - 32u * NWS; i < ncs; i += 32u * NPROD) {
         const uint32_t v = cl.e[i].lxly;
         const uint32_t gx = wrap_cell(gx0 + (int)(v & 0xFFFFu), p.mx), gy = wrap_cell(gy0 + (int)(v >> 16), p.my);
         cl.e[i].hi = ld_half(posc, (2u * (((gy & 1u) << 1) | (gx & 1u)) + 1u) * Mqp + (gy >> 1) * p.hx + (gx >> 1));
@@ -1137,7 +1149,9 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
     const uint32_t q = Qg ^ 3u;                  // the region starts at an odd cell (x0 - 5, y0 - 5): colours flip
     const uint32_t qx = q & 1u, qy = q >> 1;
     const SubRect rc = sub_sweep_rect(tb, k, dr.dir);
-    // cells of this colour next to a crowded cell: one warp each, before the warp's share of the ordinary cells
+    // cells of this colour next to a crowded cell: one warp each, before the warp's share of the ordinary cells (a warp
+    // update takes about as long as a batch of ordinary cells, so its warp simply draws one batch fewer; done at the
+    // end of the sub-sweep instead, it delayed the barrier by its full length: measured)
     for (uint32_t pi = warp; pi < 9u * nc; pi += TILE_THREADS / 32) {      // (listed cell, 3x3 position) pairs
       const uint32_t e = pi / 9u, d = pi - 9u * e;
       const uint32_t elx = cl.e[e].lxly & 0xFFFFu, ely = cl.e[e].lxly >> 16;
