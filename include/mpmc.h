@@ -152,10 +152,11 @@ int mpmc_debug_config(const mpmc_ctx* ctx, uint32_t out[8]);
 
 /* Profiling hook.  A library built with -DMPMC_PHASE_CLOCKS (paper_1211_1646_b200/phase_clocks.py) makes the 2-slot tile
  * kernel record a clock mark at each of its phase boundaries; this call copies the marks of the LAST launch to the host:
- * out = host, max_tiles x *marks values, row = tile; value 0 of a row is the global nanosecond timer at the start of the
- * tile's work, the others are SM cycle counters (clock64) at the ends of: wait for the previous sweep, load,
- * sub-sweeps 1-4, shift, ticket.  *marks = values per row, 0 in an ordinary build (nothing is written
- * to out).  MPMC_ERR_STATE unless the context runs the 2-slot tile kernel.  Synchronises. */
+ * out = host, room for max_tiles x 32 values; max_tiles x *marks are written, row = tile; value 0 of a row is the global
+ * nanosecond timer at the start of the tile's work, values 1-8 are SM cycle counters (clock64) at the ends of: wait for
+ * the previous sweep, load, sub-sweeps 1-4, shift, (unused); the rest are marks inside the load phase and before it
+ * (paper_1211_1646_b200/phase_clocks.py names them).  *marks = values per row (at most 32), 0 in an ordinary build
+ * (nothing is written to out).  MPMC_ERR_STATE unless the context runs the 2-slot tile kernel.  Synchronises. */
 int mpmc_debug_phase_clocks(mpmc_ctx* ctx, uint64_t* out, uint32_t max_tiles, uint32_t* marks);
 
 /* Test hook (pure host arithmetic, no device needed): the tiling the fused tile kernels would use for a grid of

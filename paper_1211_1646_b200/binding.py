@@ -268,7 +268,7 @@ class Mpmc:
         built with -DMPMC_PHASE_CLOCKS (mpmc_debug_phase_clocks)."""
         import numpy as np
         tiles = self.config()["tiles"]
-        flat = np.zeros(max(tiles, 1) * 16, dtype=np.uint64)
+        flat = np.zeros(max(tiles, 1) * 32, dtype=np.uint64)
         marks = _u32()
         with self.torch.cuda.device(self.device):
             self._enter()

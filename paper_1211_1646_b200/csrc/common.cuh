@@ -35,6 +35,7 @@ constexpr uint32_t SLOT_DIST = 0xFFFFFFFEu;     // shift distance
 constexpr uint32_t ERRBIT_OVERFLOW = 1u;  // a cell would hold more than NMAX disks
 constexpr uint32_t ERRBIT_RANGE = 2u;     // loaded coordinate NaN or outside [0, L]
 constexpr uint32_t ERRBIT_OVERLAP = 4u;   // loaded positions overlap
+constexpr uint32_t ERRBIT_STATE = 8u;     // internal: a launch was given the wrong buffer parity for its sweep index
 constexpr uint32_t FLAG_NO_PARTICLE_SHUFFLE = 8u, FLAG_NO_SET_SHUFFLE = 16u;   // = MPMC_NO_* of mpmc.h
 constexpr uint32_t CTR_SLOTS = 64;        // rows of move counters (summed on read)
 constexpr uint32_t CROWD_CAP = 256;       // cells with more than 2 disks the tile kernel can carry per state
@@ -75,6 +76,7 @@ struct Params {
   uint32_t tl_na, tl_hyA;               // the first tl_na rows of tiles cover the half-rows [0, tl_hyA) with tl_ntx tiles each, the
                                         // other rows the rest with tl_ntx + 1 tiles each (uniform tiling: tl_na = tl_nty, tl_hyA = hy)
   uint32_t tl_PH;                       // ... rows of the tallest tile's planes (sorted variant: stride of its row tables)
+  uint32_t tl_div[4][3];                // n / d without a divide (host: div_magic) for d = tl_ntx, tl_ntx + 1, tl_na, tl_nty - tl_na
   uint32_t seed_lo, seed_hi;
   uint32_t rk0[10], rk1[10];            // Philox round keys seed + r * Weyl constant (philox4x32_10_rk)
   float wx_f, wy_f, sigma2_f, d_f;      // working-precision constants (fp32 mode)
@@ -149,7 +151,7 @@ template <> struct Real<double> {
 
 // Philox4x32-10 (Salmon et al., SC'11).  Ten rounds of two 32x32->64 multiplies and xors; the key schedule
 // adds the Weyl constants.  counter = (c0..c3), key = (k0, k1).
-__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+__host__ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
                                               uint32_t k1, uint32_t (&out)[4]) {
 #pragma unroll
   for (int r = 0; r < 10; ++r) {
@@ -185,16 +187,14 @@ __device__ __forceinline__ void philox4x32_10_rk(const Params& p, uint32_t c0, u
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// The head of the control block as two independent 16-byte loads, issued together: {t, cur, err} and crowded[0..3].
-struct CtlHeader { unsigned long long t; uint32_t cur, err; uint32_t crowded[4]; };
-__device__ __forceinline__ CtlHeader ctl_header(const Ctl* ctl) {
-  uint32_t a0, a1, a2, a3, b0, b1, b2, b3;
+// The head of the control block as two independent loads, issued together: {t, cur, err} (16 bytes) and crowded[slot].
+struct CtlHeader { unsigned long long t; uint32_t cur, err, crowded; };
+__device__ __forceinline__ CtlHeader ctl_header(const Ctl* ctl, const uint32_t slot) {
+  uint32_t a0, a1, a2, a3, b;
   asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a0), "=r"(a1), "=r"(a2), "=r"(a3) : "l"(ctl) : "memory");
-  asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(b0), "=r"(b1), "=r"(b2), "=r"(b3)
-               : "l"(reinterpret_cast<const unsigned char*>(ctl) + 16) : "memory");
+  asm volatile("ld.global.u32 %0, [%1];" : "=r"(b) : "l"(reinterpret_cast<const unsigned char*>(ctl) + 16 + 4 * slot) : "memory");
   CtlHeader h;
-  h.t = ((unsigned long long)a1 << 32) | a0; h.cur = a2; h.err = a3;
-  h.crowded[0] = b0; h.crowded[1] = b1; h.crowded[2] = b2; h.crowded[3] = b3;
+  h.t = ((unsigned long long)a1 << 32) | a0; h.cur = a2; h.err = a3; h.crowded = b;
   return h;
 }
 static_assert(offsetof(Ctl, cur) == 8 && offsetof(Ctl, crowded) == 16 && offsetof(Ctl, ccount) == 32, "ctl_header reads this layout");
@@ -205,18 +205,21 @@ __device__ __forceinline__ void note_crowded(Ctl* ctl, uint32_t slot, uint32_t c
   if (i < CROWD_CAP) ctl->clist[slot][i] = cell; else ctl->crowded[slot] = 1u;
 }
 
-__device__ __forceinline__ uint32_t bounded(uint32_t word, uint32_t bound) { return __umulhi(word, bound); }
+__host__ __device__ __forceinline__ uint32_t bounded(uint32_t word, uint32_t bound) {
+  return (uint32_t)(((unsigned long long)word * bound) >> 32);
+}
 
 // Per-sweep draws (Alg. 1 lines 2, 15, 16; reading A9): Fisher-Yates of the four sets with
 // words G0..G2, direction from the top two bits of G3, distance word from a second counter.  A pure function of
 // (seed, sweep index), so every block computes it for itself.
 struct Draws { uint32_t order[4]; uint32_t dir; uint32_t dist_word; };
-__device__ __forceinline__ Draws draw_sweep(const Params& p, unsigned long long t) {
+__host__ __device__ __forceinline__ Draws draw_sweep(const uint32_t seed_lo, const uint32_t seed_hi, const uint32_t flags,
+                                                     const unsigned long long t) {
   uint32_t G[4], H[4];
-  philox4x32_10(CELL_GLOBAL, (uint32_t)t, (uint32_t)(t >> 32), SLOT_ORDER, p.seed_lo, p.seed_hi, G);
+  philox4x32_10(CELL_GLOBAL, (uint32_t)t, (uint32_t)(t >> 32), SLOT_ORDER, seed_lo, seed_hi, G);
   uint32_t o[4] = {0, 1, 2, 3};
 #pragma unroll
-  for (int i = 3; i >= 1 && !(p.flags & FLAG_NO_SET_SHUFFLE); --i) {
+  for (int i = 3; i >= 1 && !(flags & FLAG_NO_SET_SHUFFLE); --i) {
     const uint32_t j = bounded(G[3 - i], (uint32_t)i + 1u);
     const uint32_t a = o[i];
     // o[j] with j dynamic: select chain keeps o[] in registers
@@ -224,14 +227,20 @@ __device__ __forceinline__ Draws draw_sweep(const Params& p, unsigned long long 
     if (j == 0) o[0] = a; else if (j == 1) o[1] = a; else if (j == 2) o[2] = a; else o[3] = a;
     o[i] = b;
   }
-  philox4x32_10(CELL_GLOBAL, (uint32_t)t, (uint32_t)(t >> 32), SLOT_DIST, p.seed_lo, p.seed_hi, H);
+  philox4x32_10(CELL_GLOBAL, (uint32_t)t, (uint32_t)(t >> 32), SLOT_DIST, seed_lo, seed_hi, H);
   Draws d;
   d.order[0] = o[0]; d.order[1] = o[1]; d.order[2] = o[2]; d.order[3] = o[3];
   d.dir = G[3] >> 30;
   d.dist_word = H[0];
   return d;
 }
+__device__ __forceinline__ Draws draw_sweep(const Params& p, unsigned long long t) { return draw_sweep(p.seed_lo, p.seed_hi, p.flags, t); }
 
+// n / d for any 32-bit n with the numbers div_magic (mpmc.cu) made for d
+__device__ __forceinline__ uint32_t magic_div(const uint32_t n, const uint32_t (&m)[3]) {
+  const uint32_t t = __umulhi(m[0], n);
+  return (t + ((n - t) >> m[1])) >> m[2];
+}
 // ya = ci / hx, xa = ci - ya * hx with the precomputed magic numbers of Params
 __device__ __forceinline__ uint32_t div_hx(const Params& p, uint32_t ci) {
   const uint32_t t = __umulhi(p.hx_magic, ci);

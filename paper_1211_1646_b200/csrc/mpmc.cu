@@ -34,6 +34,7 @@ struct mpmc_ctx {
   bool tile_two_slot;      // the tile kernel is the 2-slot one (tile.cuh), which may hand a crowded state to the general kernel
   uint32_t sms;            // SMs of the device
   uint64_t t_host;         // sweeps requested since the last load (the sweep index the device will reach)
+  uint32_t cur_host;       // ... and the buffer that will hold that state (every sweep and every test-hook shift flips it)
   unsigned long long* hist_acc;   // device: histogram accumulated over samples (mpmc_pressure_accumulate)
   uint64_t acc_samples;    // samples in it
   double acc_dr; uint32_t acc_nbins;   // its bins (fixed by the first sample after a reset)
@@ -198,6 +199,7 @@ int read_ctl(mpmc_ctx* c, Ctl* h) {
   CU(cudaStreamSynchronize(c->stream));
   if (h->err & ERRBIT_OVERFLOW) c->sticky = MPMC_ERR_CELL_OVERFLOW;
   else if (h->err & (ERRBIT_OVERLAP | ERRBIT_RANGE)) c->sticky = MPMC_ERR_OVERLAP;
+  else if (h->err & ERRBIT_STATE) c->sticky = MPMC_ERR_STATE;
   return c->sticky;
 }
 
@@ -376,7 +378,7 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
   if (c->grid > chunks) c->grid = chunks;
   // The fused tile kernels: tile.cuh (2 slots per cell in shared memory) where cells hold 0/1/2 disks (w < 1.15 sigma),
   // the square proposal and n_s in {4, 8}; otherwise tile4.cuh (all 4 slots; any width, both proposals) for n_s = 4.
-  c->tile_kernel = nullptr; c->tile_grid = 0; c->tile_smem = 0; c->t_host = 0; c->tile_threads = 0;
+  c->tile_kernel = nullptr; c->tile_grid = 0; c->tile_smem = 0; c->t_host = 0; c->cur_host = 0; c->tile_threads = 0;
   const bool two_slot = c->nf == 2 && (n_s == 4 || n_s == 8) && !disc;
   c->tile_two_slot = two_slot;
   p.tune = 0u;
@@ -423,6 +425,10 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
       c->tile_grid = tl.tiles;
       c->tile_smem = (size_t)4 * tl.PS * cell_bytes + (size_t)4 * tl.PH * row_bytes;
       p.tl_ntx = tl.ntx; p.tl_nty = tl.nty; p.tl_PS = tl.PS; p.tl_PH = tl.PH; p.tl_na = tl.na; p.tl_hyA = tl.hyA;
+      {
+        const uint32_t dv[4] = {tl.ntx, tl.ntx + 1u, tl.na, tl.nty > tl.na ? tl.nty - tl.na : 1u};
+        for (int i = 0; i < 4; ++i) div_magic(dv[i], &p.tl_div[i][0], &p.tl_div[i][1], &p.tl_div[i][2]);
+      }
       // The attribute belongs to the kernel function, not to this context: set it to the most any tiling can ask for
       // (the opt-in maximum minus the kernel's static shared memory), so that live contexts with different tilings
       // of the same instantiation do not undo each other's setting.
@@ -462,7 +468,7 @@ int mpmc_load_positions(mpmc_ctx* c, const double* xy) {
   if (!c || !xy) return MPMC_ERR_ARG;
   c->loaded = false;
   c->sticky = MPMC_OK;
-  c->t_host = 0;
+  c->t_host = 0; c->cur_host = 0;
   k_reset<<<c->sms * 4, 256, 0, c->stream>>>(c->p);
   const dim3 gN((c->p.N + AUX_THREADS - 1) / AUX_THREADS), gC = cell_grid(c, AUX_THREADS);
   if (c->fp32) {
@@ -504,16 +510,19 @@ int mpmc_sweep(mpmc_ctx* c, uint64_t k) {
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
     unsigned long long t = c->t_host;              // sweep index of each launch (kernel argument: uniform on the device)
-    void* args[] = {(void*)&c->p, (void*)&t};
-    for (uint64_t i = 0; i < k; ++i, ++t) {
+    Draws dr;                                      // ... and its draws (read by the 2-slot kernel; the 4-slot kernel makes its own)
+    uint32_t cur = c->cur_host;                    // ... and the buffer its state is in
+    void* args[] = {(void*)&c->p, (void*)&t, (void*)&dr, (void*)&cur};
+    for (uint64_t i = 0; i < k; ++i, ++t, cur ^= 1u) {
+      dr = draw_sweep(c->p.seed_lo, c->p.seed_hi, c->p.flags, t);
       const cudaError_t e = cudaLaunchKernelExC(&cfg, c->tile_kernel, args);
       if (e != cudaSuccess) {                      // the device stays at the sweeps launched so far
-        c->t_host += i;
+        c->t_host += i; c->cur_host ^= (uint32_t)(i & 1u);
         return cuda_fail(e);
       }
     }
   }
-  c->t_host += k;
+  c->t_host += k; c->cur_host ^= (uint32_t)(k & 1u);
   // ... and the general kernel runs whatever is left up to the target sweep index: everything without a tile kernel,
   // normally nothing behind the 2-slot tile kernel (it hands over only a state with too many crowded cells), never
   // anything behind the 4-slot tile kernel, which takes every state
@@ -620,6 +629,7 @@ int mpmc_debug_shift(mpmc_ctx* c, uint32_t direction, double delta) {
   if (!(delta < (direction < 2 ? c->p.wx_d : c->p.wy_d))) return MPMC_ERR_ARG;
   if (!c->loaded) return MPMC_ERR_STATE;
   const int st = launch_sweeps(c, 0, OP_SHIFT, direction, delta);
+  if (st == MPMC_OK) c->cur_host ^= 1u;            // the shifted state is in the other buffer
   return st != MPMC_OK ? st : c->sticky;
 }
 

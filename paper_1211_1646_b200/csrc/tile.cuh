@@ -42,7 +42,7 @@ constexpr int SHIFT_U = 2;              // cells per lane and chunk in the shift
 
 // -DMPMC_PHASE_CLOCKS builds a variant that records clock64() at every phase boundary (phase_clocks.py).
 #ifdef MPMC_PHASE_CLOCKS
-constexpr uint32_t PHASE_TILES = 4096, PHASE_MARKS = 16;
+constexpr uint32_t PHASE_TILES = 4096, PHASE_MARKS = 20;
 __device__ unsigned long long g_phase_clocks[PHASE_TILES][PHASE_MARKS];
 __device__ __forceinline__ unsigned long long globaltimer_ns() { unsigned long long v; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(v)); return v; }
 // (the clock is read AFTER a shared-memory load that follows the barrier: a bare clock read right behind __syncthreads is
@@ -52,7 +52,7 @@ __device__ __forceinline__ unsigned long long clock_after(const volatile uint32_
   asm volatile("mov.u64 %0, %%clock64;" : "=l"(c) : "r"(v) : "memory");
   return c;
 }
-#define MPMC_PHASE_MARK_AT(i, mark_word) do { if (threadIdx.x == 0 && blockIdx.x < PHASE_TILES) g_phase_clocks[blockIdx.x][i] = (i) == 0 ? globaltimer_ns() : clock_after(mark_word); } while (0)
+#define MPMC_PHASE_MARK_AT(i, mark_word) do { if (threadIdx.x == 0 && blockIdx.x < PHASE_TILES) g_phase_clocks[blockIdx.x][i] = ((i) == 0 || (i) == 8) ? globaltimer_ns() : clock_after(mark_word); } while (0)
 #else
 #define MPMC_PHASE_MARK_AT(i, mark_word) do { } while (0)
 #endif
@@ -63,6 +63,12 @@ __device__ __forceinline__ unsigned long long clock_after(const volatile uint32_
 #define MPMC_PHASE_NOW(i) do { if (threadIdx.x == 0 && blockIdx.x < PHASE_TILES) g_phase_clocks[blockIdx.x][i] = clock_after(&s_last); } while (0)
 #else
 #define MPMC_PHASE_NOW(i) do { } while (0)
+#endif
+// thread 0's clock where no barrier precedes (marks 16-18: kernel entry, before and after the dependency wait)
+#ifdef MPMC_PHASE_CLOCKS
+#define MPMC_PHASE_RAW(i) do { if (threadIdx.x == 0 && blockIdx.x < PHASE_TILES) g_phase_clocks[blockIdx.x][i] = clock64(); } while (0)
+#else
+#define MPMC_PHASE_RAW(i) do { } while (0)
 #endif
 #ifdef MPMC_PHASE_CLOCKS
 #define MPMC_PHASE_VALUE(i, v) do { if (threadIdx.x == 0 && blockIdx.x < PHASE_TILES) g_phase_clocks[blockIdx.x][i] = (unsigned long long)(v); } while (0)
@@ -129,23 +135,25 @@ struct TileBox {
 // loaded area the tile count can match the SM count (C3: 8 x 12 + 4 x 13 = 148) where a rectangular ntx x nty grid leaves
 // SMs idle (12 x 12 = 144).
 __device__ __forceinline__ TileBox tile_box(const Params& p, const uint32_t b) {
-  TileBox t;                                     // (32-bit products: the host tiles boxes of fewer than 2^16 half-rows only)
+  TileBox t;                                     // (32-bit products, divisions by the host's magic numbers)
   const uint32_t nA = p.tl_na * p.tl_ntx;
-  uint32_t tx, ntx, h0, h1;
+  uint32_t tx, ntx, h0, h1, x0, x1;
   if (b < nA) {
-    const uint32_t r = b / p.tl_ntx;
+    const uint32_t r = magic_div(b, p.tl_div[0]);
     tx = b - r * p.tl_ntx; ntx = p.tl_ntx;
-    h0 = p.tl_hyA * r / p.tl_na;
-    h1 = p.tl_hyA * (r + 1u) / p.tl_na;
+    h0 = magic_div(p.tl_hyA * r, p.tl_div[2]);
+    h1 = magic_div(p.tl_hyA * (r + 1u), p.tl_div[2]);
+    x0 = magic_div(p.hx * tx, p.tl_div[0]); x1 = magic_div(p.hx * (tx + 1u), p.tl_div[0]);
   } else {
-    const uint32_t b2 = b - nA, nb = p.tl_nty - p.tl_na, hyB = p.hy - p.tl_hyA;
-    const uint32_t r = b2 / (p.tl_ntx + 1u);
+    const uint32_t b2 = b - nA, hyB = p.hy - p.tl_hyA;
+    const uint32_t r = magic_div(b2, p.tl_div[1]);
     tx = b2 - r * (p.tl_ntx + 1u); ntx = p.tl_ntx + 1u;
-    h0 = p.tl_hyA + hyB * r / nb;
-    h1 = p.tl_hyA + hyB * (r + 1u) / nb;
+    h0 = p.tl_hyA + magic_div(hyB * r, p.tl_div[3]);
+    h1 = p.tl_hyA + magic_div(hyB * (r + 1u), p.tl_div[3]);
+    x0 = magic_div(p.hx * tx, p.tl_div[1]); x1 = magic_div(p.hx * (tx + 1u), p.tl_div[1]);
   }
-  t.x0 = 2u * (p.hx * tx / ntx);
-  t.TX = 2u * (p.hx * (tx + 1u) / ntx) - t.x0;
+  (void)ntx;
+  t.x0 = 2u * x0; t.TX = 2u * x1 - t.x0;
   t.y0 = 2u * h0; t.TY = 2u * (h1 - h0);
   t.w = t.TX + 2 * HALO; t.h = t.TY + 2 * HALO;
   t.pw = t.w / 2; t.ph = t.h / 2;
@@ -619,32 +627,46 @@ __device__ __forceinline__ void tile_sort_cells(const Params& p, const SmemCell<
     const unsigned long long in = (~0ull >> (63u - g.px_hi)) & (~0ull << g.px_lo);
     const unsigned long long* T = sa.two;
     const uint32_t q1 = q ^ 1u, q2 = q ^ 2u, q3 = q ^ 3u;
+    // a lane takes the rows py = lane and lane + 32 (a plane has at most 64 rows... of interest: rows beyond hold no cell
+    // of the rectangle), both in flight together
     uint32_t run1 = 0, run2 = 0;
-    for (uint32_t r0 = 0; r0 < ph; r0 += 32u) {
-      const uint32_t py = r0 + lane;
-      unsigned long long simple = 0ull, general = 0ull;
-      if (py >= g.py_lo && py <= g.py_hi) {
-        const uint32_t ra = py + (uint32_t)qy - 1u, rb = py + (uint32_t)qy;   // the plane rows of the cells below / above
-        unsigned long long c = T[q * PH + py];
-        c |= mask_shift(T[q1 * PH + py], qx - 1) | mask_shift(T[q1 * PH + py], qx);
-        c |= T[q2 * PH + ra] | T[q2 * PH + rb];
-        c |= mask_shift(T[q3 * PH + ra], qx - 1) | mask_shift(T[q3 * PH + ra], qx);
-        c |= mask_shift(T[q3 * PH + rb], qx - 1) | mask_shift(T[q3 * PH + rb], qx);
-        const unsigned long long o = sa.occ[q * PH + py] & in;
-        simple = o & ~c; general = o & c;
-      }
-      const uint32_t n1 = (uint32_t)__popcll(simple), n2 = (uint32_t)__popcll(general);
-      uint32_t i1 = n1, i2 = n2;
+    for (uint32_t r0 = 0; r0 < ph; r0 += 64u) {
+      unsigned long long simple[2], general[2];
+      uint32_t n1[2], n2[2], i1[2], i2[2];
 #pragma unroll
-      for (uint32_t d = 1; d < 32u; d <<= 1) {
-        const uint32_t v1 = __shfl_up_sync(0xFFFFFFFFu, i1, d), v2 = __shfl_up_sync(0xFFFFFFFFu, i2, d);
-        if (lane >= d) { i1 += v1; i2 += v2; }
+      for (uint32_t h = 0; h < 2u; ++h) {
+        const uint32_t py = r0 + lane + 32u * h;
+        simple[h] = 0ull; general[h] = 0ull;
+        if (py >= g.py_lo && py <= g.py_hi) {
+          const uint32_t ra = py + (uint32_t)qy - 1u, rb = py + (uint32_t)qy;   // the plane rows of the cells below / above
+          unsigned long long c = T[q * PH + py];
+          c |= mask_shift(T[q1 * PH + py], qx - 1) | mask_shift(T[q1 * PH + py], qx);
+          c |= T[q2 * PH + ra] | T[q2 * PH + rb];
+          c |= mask_shift(T[q3 * PH + ra], qx - 1) | mask_shift(T[q3 * PH + ra], qx);
+          c |= mask_shift(T[q3 * PH + rb], qx - 1) | mask_shift(T[q3 * PH + rb], qx);
+          const unsigned long long o = sa.occ[q * PH + py] & in;
+          simple[h] = o & ~c; general[h] = o & c;
+        }
+        n1[h] = (uint32_t)__popcll(simple[h]); n2[h] = (uint32_t)__popcll(general[h]);
+        i1[h] = n1[h]; i2[h] = n2[h];
       }
-      if (py < ph) {
-        sa.simple[k * PH + py] = simple; sa.general[k * PH + py] = general;
-        sa.base1[k * PH + py] = (uint16_t)(run1 + i1 - n1); sa.base2[k * PH + py] = (uint16_t)(run2 + i2 - n2);
+#pragma unroll
+      for (uint32_t d = 1; d < 32u; d <<= 1) {       // inclusive prefix sums over the lanes, the two halves side by side
+        const uint32_t a0 = __shfl_up_sync(0xFFFFFFFFu, i1[0], d), b0 = __shfl_up_sync(0xFFFFFFFFu, i2[0], d);
+        const uint32_t a1 = __shfl_up_sync(0xFFFFFFFFu, i1[1], d), b1 = __shfl_up_sync(0xFFFFFFFFu, i2[1], d);
+        if (lane >= d) { i1[0] += a0; i2[0] += b0; i1[1] += a1; i2[1] += b1; }
       }
-      run1 += __shfl_sync(0xFFFFFFFFu, i1, 31); run2 += __shfl_sync(0xFFFFFFFFu, i2, 31);
+      const uint32_t t1 = __shfl_sync(0xFFFFFFFFu, i1[0], 31), t2 = __shfl_sync(0xFFFFFFFFu, i2[0], 31);
+#pragma unroll
+      for (uint32_t h = 0; h < 2u; ++h) {
+        const uint32_t py = r0 + lane + 32u * h;
+        if (py < ph) {
+          sa.simple[k * PH + py] = simple[h]; sa.general[k * PH + py] = general[h];
+          sa.base1[k * PH + py] = (uint16_t)(run1 + (h ? t1 : 0u) + i1[h] - n1[h]);
+          sa.base2[k * PH + py] = (uint16_t)(run2 + (h ? t2 : 0u) + i2[h] - n2[h]);
+        }
+      }
+      run1 += t1 + __shfl_sync(0xFFFFFFFFu, i1[1], 31); run2 += t2 + __shfl_sync(0xFFFFFFFFu, i2[1], 31);
     }
     if (lane == 0u) { s_cnt[k][0] = run1; s_cnt[k][1] = run2; }
   }
@@ -652,20 +674,29 @@ __device__ __forceinline__ void tile_sort_cells(const Params& p, const SmemCell<
   MPMC_PHASE_MARK_AT(10, &s_cnt[0][0]);
   // ---- D: the plane indices, a warp per row, a lane per cell: simple cells from the front of the sub-sweep's queue,
   //      general cells from its back ----
-  for (uint32_t r = warp; r < 4u * ph; r += NW) {
-    const uint32_t k = small_div(r, inv_ph), py = r - k * ph;
-    const unsigned long long m1 = sa.simple[k * PH + py], m2 = sa.general[k * PH + py];
-    if ((m1 | m2) == 0ull) continue;
-    uint16_t* qk = queues + k * PS;
-    uint32_t at1 = sa.base1[k * PH + py], at2 = PS - 1u - sa.base2[k * PH + py];
-    const uint32_t below = (1u << lane) - 1u;
+  const uint32_t below = (1u << lane) - 1u;
+  for (uint32_t r = warp; r < 4u * ph; r += 2u * NW) {           // two rows per round: their loads are in flight together
+    uint32_t k[2], py[2], at1[2], at2[2];
+    unsigned long long m1[2], m2[2];
 #pragma unroll
-    for (uint32_t half = 0; half < 2u; ++half) {          // a cell is in at most one of the two classes: one store
-      const uint32_t w1 = (uint32_t)(m1 >> (32u * half)), w2 = (uint32_t)(m2 >> (32u * half));
-      const bool is1 = (w1 >> lane) & 1u, is2 = (w2 >> lane) & 1u;
-      const uint32_t c = (uint32_t)__popc((is1 ? w1 : w2) & below);
-      if (is1 || is2) qk[is1 ? at1 + c : at2 - c] = (uint16_t)(py * pw + lane + 32u * half);
-      if (half == 0u) { at1 += (uint32_t)__popc(w1); at2 -= (uint32_t)__popc(w2); }
+    for (uint32_t h = 0; h < 2u; ++h) {
+      const uint32_t rr = min(r + h * NW, 4u * ph - 1u);
+      const bool live = r + h * NW < 4u * ph;
+      k[h] = small_div(rr, inv_ph); py[h] = rr - k[h] * ph;
+      m1[h] = live ? sa.simple[k[h] * PH + py[h]] : 0ull; m2[h] = live ? sa.general[k[h] * PH + py[h]] : 0ull;
+      at1[h] = sa.base1[k[h] * PH + py[h]]; at2[h] = PS - 1u - sa.base2[k[h] * PH + py[h]];
+    }
+#pragma unroll
+    for (uint32_t h = 0; h < 2u; ++h) {
+      uint16_t* qk = queues + k[h] * PS;
+#pragma unroll
+      for (uint32_t half = 0; half < 2u; ++half) {        // a cell is in at most one of the two classes: one store
+        const uint32_t w1 = (uint32_t)(m1[h] >> (32u * half)), w2 = (uint32_t)(m2[h] >> (32u * half));
+        const bool is1 = (w1 >> lane) & 1u, is2 = (w2 >> lane) & 1u;
+        const uint32_t c = (uint32_t)__popc((is1 ? w1 : w2) & below);
+        if (is1 || is2) qk[is1 ? at1[h] + c : at2[h] - c] = (uint16_t)(py[h] * pw + lane + 32u * half);
+        if (half == 0u) { at1[h] += (uint32_t)__popc(w1); at2[h] -= (uint32_t)__popc(w2); }
+      }
     }
   }
   sort_barrier(32u * NW);
@@ -896,7 +927,7 @@ __device__ __forceinline__ void tile_shift_cells(const Params& p, const SmemCell
 // ---------------------------------------------------------------------------------------------------------
 template <typename P, int NS, bool DEBUG, bool SORTED = false>
 __global__ void __launch_bounds__(TileThreads<P>::value, 1)
-k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
+k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t, const Draws dr_host, const uint32_t cur) {
   using R = Real<P>;
   const uint32_t TILE_THREADS = blockDim.x;           // at most TileThreads<P>::value (the host may launch fewer)
   extern __shared__ __align__(16) unsigned char tile_smem[];
@@ -909,11 +940,16 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   __shared__ uint32_t s_next[8];                 // chunk counters: sub-sweeps 1-4, shift planes 0-3
   __shared__ uint32_t s_cnt[4][2];               // SORTED: simple / general cells queued per sub-sweep
   Ctl* ctl = p.ctl;
-  // The sweep index comes as a kernel argument (the host counts launches), so the draws of this sweep — a pure function
-  // of (seed, t), Alg. 1 lines 2, 15, 16 (L64, L90-91) — and all they decide are warp-uniform values computed before the
-  // wait.  Launched with programmatic stream serialisation (mpmc.cu): everything below the wait reads what the previous
+  // The sweep index comes as a kernel argument (the host counts launches), and with it the draws of this sweep — a pure
+  // function of (seed, t), Alg. 1 lines 2, 15, 16 (L64, L90-91), evaluated by the host with the same draw_sweep (common.cuh)
+  // — so all they decide are uniform values from the constant bank.  The code ahead of the wait is on the critical path of
+  // the SM that finished the previous sweep last (24 warps computing the same uniform values took 3 400 cycles there:
+  // measured), hence host-made draws, divisions by magic numbers and nothing done twice.  Launched with programmatic stream serialisation (mpmc.cu): everything below the wait reads what the previous
   // sweep wrote.  If the state is not at sweep t (an earlier launch left its sweep to the general kernel), return.
-  const Draws dr = draw_sweep(p, t);
+  MPMC_PHASE_RAW(16);
+  Draws dr;                                      // (a copy in registers: a parameter whose address is taken lives in local memory)
+  dr.order[0] = dr_host.order[0]; dr.order[1] = dr_host.order[1]; dr.order[2] = dr_host.order[2]; dr.order[3] = dr_host.order[3];
+  dr.dir = dr_host.dir; dr.dist_word = dr_host.dist_word;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
   const TileBox tb = tile_box(p, blockIdx.x);
   const uint32_t PS = p.tl_PS, pw = tb.pw, ph = tb.ph, Mqp = p.Mqp;
@@ -944,21 +980,32 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
     if (r0 + lane < nrows && lane < rpw) {
       my_q = small_div(r0 + lane, inv_ph); my_py = r0 + lane - my_q * ph;
       const uint32_t gy = wrap_cell(gy0 + (int)(2u * my_py + (my_q >> 1)), p.my);
-      my_off = ((gy & 1u) << 1) * Mqp + (gy >> 1) * p.hx;
+      my_off = 2u * (((gy & 1u) << 1) * Mqp + (gy >> 1) * p.hx) + (my_q & 1u);     // (bit 0: the row's qx; the host tiles grids
+                                                                                 // of fewer than 2^30 cells only)
     }
   };
   if (SORTED) row_setup(warp * rpw);
   __syncthreads();
   // ---- everything above is a function of the launch parameters; what follows reads what the previous sweep wrote ----
+  MPMC_PHASE_RAW(17);
   asm volatile("griddepcontrol.wait;" ::: "memory");
+  MPMC_PHASE_RAW(18);
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  const CtlHeader ch = ctl_header(ctl);          // sweep index, buffer parity, "too many crowded cells": one trip to L2
-  if (ch.t != t) return;
+  // The head of the control block — sweep index, buffer parity, "too many crowded cells" — is one trip to L2 (~900 cycles).
+  // The host knows which buffer holds the state of sweep t (every sweep flips it) and passes it as `cur`, so the sorted
+  // variant requests the count bytes of its region at once and looks at the head when it has arrived (stale_launch below,
+  // before anything is written or copied).  A head at sweep t with another parity cannot happen; it is reported.
   const uint32_t slot = (uint32_t)(t & 3u), slot1 = (uint32_t)((t + 1ull) & 3u), slot2 = (uint32_t)((t + 2ull) & 3u);
-  if ((slot == 0u ? ch.crowded[0] : slot == 1u ? ch.crowded[1] : slot == 2u ? ch.crowded[2] : ch.crowded[3]) != 0u)
-    return;                                      // too many crowded cells: the general kernel takes over
+  const CtlHeader ch = ctl_header(ctl, slot);
+  const uint32_t nxt = cur ^ 1u;
+  auto stale_launch = [&]() -> bool {
+    // the state is not at sweep t (an earlier launch left its sweep to the general kernel), or it has too many crowded
+    // cells and the general kernel takes over
+    if (ch.t == t && ch.cur != cur && threadIdx.x == 0) atomicOr(&ctl->err, ERRBIT_STATE);
+    return ch.t != t || ch.crowded != 0u || ch.cur != cur;
+  };
+  if (!SORTED && stale_launch()) return;
   MPMC_PHASE_MARK(0); MPMC_PHASE_MARK(1);
-  const uint32_t cur = ch.cur, nxt = cur ^ 1u;
   // plain variant: the list of crowded cells of this state, its first TILE_THREADS entries fetched NOW (the chain count ->
   // cell -> slots 2, 3 is three trips to L2; started here it ends under the tile load instead of behind it).  The sorted
   // variant finds the crowded cells of its region in the count bytes it reads anyway.
@@ -995,6 +1042,7 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
     // queue is full, i.e. for most of the load: measured), the other NWS warps sort.
     if (warp >= NWS) {
       asm volatile("bar.sync 2, %0;" :: "r"(TILE_THREADS) : "memory");   // (see below)
+      if (stale_launch()) return;
       const uint32_t share = (nrows + NPROD - 1u) / NPROD, first = (warp - NWS) * share, last = min(nrows, first + share);
       for (uint32_t r = first + lane; r < last; r += 32u) { const uint32_t q = small_div(r, inv_ph); copy_row(q, r - q * ph); }
     }
@@ -1008,14 +1056,17 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
       for (uint32_t j = 0; j < SORT_ROWS; ++j) {
         c0[j] = 0u; c1[j] = 0u;
         if (j < nr) {                            // (warp-uniform)
-          const uint32_t off = __shfl_sync(0xFFFFFFFFu, my_off, j), qx = __shfl_sync(0xFFFFFFFFu, my_q, j) & 1u;
-          if (has0) c0[j] = ld_u8_early(cntc + (off + (qx ? col1.x : col0.x)));
-          if (has1) c1[j] = ld_u8_early(cntc + (off + (qx ? col1.y : col0.y)));
+          const uint32_t w = __shfl_sync(0xFFFFFFFFu, my_off, j), off = w >> 1;
+          if (has0) c0[j] = ld_u8_early(cntc + (off + ((w & 1u) ? col1.x : col0.x)));
+          if (has1) c1[j] = ld_u8_early(cntc + (off + ((w & 1u) ? col1.y : col0.y)));
         }
       }
       // the copies start once the count bytes have been REQUESTED: behind the copies' requests in the SM's queue to L2 they
       // would arrive with the last rows (measured)
-      if (!told) { asm volatile("bar.arrive 2, %0;" :: "r"(TILE_THREADS) : "memory"); told = true; }
+      if (!told) {
+        asm volatile("bar.arrive 2, %0;" :: "r"(TILE_THREADS) : "memory"); told = true;
+        if (stale_launch()) return;              // (every thread of the CTA takes the same decision)
+      }
       MPMC_PHASE_NOW(13);
       // phase A of the sort: the occupancy masks of these rows (lane j ends up with the masks of row j and stores them)
       uint2 m_occ = make_uint2(0u, 0u), m_two = m_occ;
@@ -1060,7 +1111,7 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t) {
         }
       }
     }
-    if (!told) asm volatile("bar.arrive 2, %0;" :: "r"(TILE_THREADS) : "memory");
+    if (!told) { asm volatile("bar.arrive 2, %0;" :: "r"(TILE_THREADS) : "memory"); if (stale_launch()) return; }
   } else {
     for (uint32_t r = warp; r < nrows; r += NW)
       if (lane == 0u) { const uint32_t q = small_div(r, inv_ph); copy_row(q, r - q * ph); }

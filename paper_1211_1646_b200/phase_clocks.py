@@ -14,7 +14,7 @@ import os
 import numpy as np
 
 PHASES = ["wait for the previous sweep", "load tile + halo", "sub-sweep 1", "sub-sweep 2", "sub-sweep 3", "sub-sweep 4",
-          "shift + counters", "ticket"]
+          "shift + counters"]
 
 
 def main():
@@ -48,7 +48,9 @@ def main():
     pc = np.stack(rows)                              # (samples, tiles, marks)
     extra = pc[:, :, 9:] if pc.shape[2] > 9 else None   # marks inside the sort of the sorted variant (0 if unused)
     pc = pc[:, :, :9]
-    d = np.diff(pc[:, :, 1:], axis=2)                # cycles per phase
+    d = np.diff(pc[:, :, 1:8], axis=2)               # cycles per phase
+    t_ns = (pc[:, :, 8] - pc[:, :, 0])               # mark 8 is the nanosecond timer at the end of the tile's work
+    launch_ns = pc[:, :, 8].max(axis=1) - pc[:, :, 0].min(axis=1)
     span_ns = pc[:, :, 0].max(axis=1) - pc[:, :, 0].min(axis=1)
     cfg = g.config()
     print(f"{w.name}: {cfg['ntx']} x {cfg['nty']} tiles, {cfg['tile_threads']} threads, {cfg['tile_smem']} B shared memory; "
@@ -68,9 +70,13 @@ def main():
                ("count bytes arrived (warp 0)", extra[:, :, 5]), ("row masks of all warps (barrier)", extra[:, :, 0]),
                ("classes + prefix sums", extra[:, :, 1]), ("region arrived, queues written", extra[:, :, 6])]
         print("  inside 'load', cycles after its start: " + "; ".join(f"{n} {(e - t1).mean():.0f}" for n, e in pts))
+    if extra is not None and extra.shape[2] >= 10 and extra[:, :, 7].min() > 0:
+        e, b, a = extra[:, :, 7], extra[:, :, 8], extra[:, :, 9]
+        print(f"  before 'load': kernel entry -> dependency wait {(b - e).mean():.0f} cycles (set-up), in the wait {(a - b).mean():.0f} "
+              f"(min over tiles {(a - b).min(axis=1).mean():.0f}), wait -> start of 'load' {(pc[:, :, 1] - a).mean():.0f} (control block)")
     if extra is not None and extra.shape[2] >= 4:
         ncrowd = extra[:, :, 3]
-        whole = pc[:, :, -1] - pc[:, :, 1]
+        whole = pc[:, :, 7] - pc[:, :, 1]
         has = ncrowd > 0
         if has.any() and (~has).any():
             print(f"  tiles with a crowded cell in their region: {has.mean() * 100:.1f} % of (launch, tile) pairs; whole tile "
@@ -78,8 +84,10 @@ def main():
                   + ", ".join(f"{d[:, :, i][has].mean() - d[:, :, i][~has].mean():+.0f}" for i in range(d.shape[2])))
     if args.dump:
         np.save(args.dump, d.mean(axis=0))
-    tot = pc[:, :, -1] - pc[:, :, 1]
+    tot = pc[:, :, 7] - pc[:, :, 1]
     print(f"  {'whole tile':42s} mean {tot.mean():9.0f}   max {tot.max(axis=1).mean():9.0f} cycles")
+    print(f"  in nanoseconds: a tile takes {t_ns.mean():.0f} (slowest {t_ns.max(axis=1).mean():.0f}); first start to last end of a launch "
+          f"{launch_ns.mean():.0f}; the launch period less that is the hand-over between sweeps")
 
 
 if __name__ == "__main__":

@@ -82,6 +82,34 @@ def test_pieces_load_subsweeps_shift(oracle_mod, torch_cuda, fp32):
     assert_same_state(o, g, fp32)
 
 
+@pytest.mark.parametrize("workload", ["C1", "C3s"])
+def test_sweeps_after_test_hook_shifts(oracle_mod, torch_cuda, workload):
+    """The host tells every tile-kernel launch which buffer holds its sweep's state; a shift made through the test hook
+    flips the buffer at an unchanged sweep index, an odd number of sweeps flips it too.  C3s: a system large enough for
+    the sorted variant, which starts from that hint before it has seen the control block."""
+    if workload == "C1":
+        w = I.CONFIGS["C1"]
+        N, sigma, d, n_s, seed, fp32 = w.N, w.sigma, w.d, w.n_s, w.seed, w.fp32
+        xy, box = I.workload_inputs(w)
+    else:
+        n = 704                                        # ~3 700 cells per tile region: the sorted variant
+        N, sigma, d, n_s, seed, fp32 = n * n, 1.0, 0.08, 4, 11, True
+        xy, box = I.jittered_lattice(n, 0.716, sigma, seed=seed)
+    o, g = make_pair(oracle_mod, torch_cuda, N, box, sigma, d, n_s, seed, fp32, xy)
+    done = 0
+    for k, direction in ((3, 1), (2, 2), (1, 0), (4, 3)):
+        o.sweep(k); g.sweep(k); done += k
+        assert_same_state(o, g, fp32)
+        delta = 0.27 * (o.wx if direction < 2 else o.wy)
+        o.shift(direction, delta); g.shift(direction, delta)
+        assert_same_state(o, g, fp32)
+    o.sweep(5); g.sweep(5); done += 5
+    assert_same_state(o, g, fp32)
+    assert g.path_sweeps() == (done, 0)                # every sweep on the fused tile kernel, none refused
+    if workload == "C3s":
+        assert g.config()["tile_slots"] == 2
+
+
 @pytest.mark.parametrize("fp32", [False, True])
 def test_c1_100_sweeps_bit_exact(oracle_mod, torch_cuda, fp32):
     w = I.CONFIGS["C1"]
