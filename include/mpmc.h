@@ -42,6 +42,7 @@ typedef struct mpmc_ctx mpmc_ctx; /* opaque host object; owns no device memory *
 #define MPMC_ERR_CELL_OVERFLOW (-5) /* more than n_max = 4 disks in one cell (possible only when w >= sqrt(2) sigma) */
 #define MPMC_ERR_CUDA (-6)          /* CUDA runtime error (no device, launch failure ...) */
 #define MPMC_ERR_STATE (-7)         /* no positions loaded yet */
+#define MPMC_ERR_TOO_LARGE (-8)     /* a size beyond the fixed capacity of a no-allocation entry point (see its comment) */
 
 /* flags for mpmc_create: exactly one precision bit */
 #define MPMC_FP64 0x1u  /* local coordinates and all move arithmetic in double */
@@ -123,6 +124,24 @@ int mpmc_pressure_accumulated(mpmc_ctx* ctx, uint32_t degree, uint64_t* hist_out
 int mpmc_pressure_reset(mpmc_ctx* ctx);
 int mpmc_pressure_from_histogram(const mpmc_ctx* ctx, const uint64_t* hist, uint64_t samples, double dr, uint32_t nbins,
                                  uint32_t degree, double* g_contact, double* p_star);
+
+/* Contact histogram without any allocation (for callers that cannot call cudaMalloc: code under CUDA graph capture,
+ * serving loops, harnesses that forbid it).  The same pair histogram as mpmc_pressure_contact (L366-382; same kernels, same
+ * bins, same double-precision arithmetic: the counts are identical), but the kernels' scratch — the device histogram the
+ * blocks add their counts to — is NOT the workspace's: it is a file-scope `static __device__` array of
+ * MPMC_NOALLOC_MAX_BINS 64-bit counters (8 KB) inside the library, which every GPU that loads the library holds until the
+ * process exits.  The call makes no cudaMalloc / cudaFree and no allocating library call, on the device or the host.
+ *   hist_out = DEVICE, nbins uint64 counts of unordered pairs with r in [sigma + i dr, sigma + (i+1) dr), owned by the
+ *       caller, written on the context's stream.  Asynchronous: no host synchronisation.
+ *   nbins > MPMC_NOALLOC_MAX_BINS: MPMC_ERR_TOO_LARGE, nothing is launched (use mpmc_pressure_contact, up to 4096 bins).
+ *   The context's device must be the current device (MPMC_ERR_ARG otherwise): the array's device address is resolved
+ *       once per device, with that device current, on the first call.
+ *   ALL calls on one GPU — of any context, on any stream, from any thread — share the one array, which keeps the last
+ *       call's counts: every call clears the bins it uses first, and two calls that OVERLAP on the GPU (different
+ *       streams or contexts, no ordering between them) race and both return garbage.  Calls on one stream are ordered.
+ *   MPMC_ERR_STATE with no positions loaded; device-detected errors are reported by the next synchronising call. */
+#define MPMC_NOALLOC_MAX_BINS 1024u
+int mpmc_contact_histogram_noalloc(mpmc_ctx* ctx, double dr, uint32_t nbins, uint64_t* hist_out);
 
 /* Test hooks: single pieces of Algorithm 1 at the current sweep index (do not advance it). */
 int mpmc_debug_sub_sweep(mpmc_ctx* ctx, uint32_t checkerboard_set /*0=a(0,0) 1=b(1,0) 2=c(0,1) 3=d(1,1)*/);

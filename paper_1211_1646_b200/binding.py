@@ -16,6 +16,8 @@ DISC = 0x4
 NO_PARTICLE_SHUFFLE = 0x8
 NO_SET_SHUFFLE = 0x10
 DEBUG = 0x100
+NOALLOC_MAX_BINS = 1024       # MPMC_NOALLOC_MAX_BINS of include/mpmc.h
+ERR_TOO_LARGE = -8            # MPMC_ERR_TOO_LARGE
 
 _u32, _u64, _dbl, _vp, _sz = C.c_uint32, C.c_uint64, C.c_double, C.c_void_p, C.c_size_t
 
@@ -32,6 +34,7 @@ SYMBOLS = {
     "mpmc_get_positions": (C.c_int, [_vp, _vp]),
     "mpmc_acceptance": (C.c_int, [_vp, C.POINTER(_u64)]),
     "mpmc_pressure_contact": (C.c_int, [_vp, _dbl, _u32, _u32, _vp, C.POINTER(_dbl), C.POINTER(_dbl)]),
+    "mpmc_contact_histogram_noalloc": (C.c_int, [_vp, _dbl, _u32, _vp]),
     "mpmc_pressure_accumulate": (C.c_int, [_vp, _dbl, _u32]),
     "mpmc_pressure_accumulated": (C.c_int, [_vp, _u32, _vp, C.POINTER(_u64), C.POINTER(_dbl), C.POINTER(_dbl)]),
     "mpmc_pressure_reset": (C.c_int, [_vp]),
@@ -201,6 +204,20 @@ class Mpmc:
             _chk(lib().mpmc_pressure_contact(self._h, float(dr), int(nbins), 0, h.ctypes.data, None, None))
             self._exit()
         return h
+
+    def contact_histogram_noalloc(self, dr: float, nbins: int, out=None):
+        """The pair histogram of mpmc_pressure_contact through the entry point that allocates nothing (its scratch is a
+        static device array inside the library, at most NOALLOC_MAX_BINS bins; calls that overlap on the GPU race).
+        out: int64 CUDA tensor of nbins elements owned by the caller (made here if None); asynchronous."""
+        t = self.torch
+        if out is None:
+            out = t.empty(int(nbins), dtype=t.int64, device=self.device)
+        assert out.is_cuda and out.dtype == t.int64 and out.is_contiguous() and out.numel() >= int(nbins)
+        with t.cuda.device(self.device):
+            self._enter()
+            _chk(lib().mpmc_contact_histogram_noalloc(self._h, float(dr), int(nbins), out.data_ptr()))
+            self._exit()
+        return out
 
     def pressure_accumulate(self, dr: float, nbins: int) -> None:
         """Add the current state's pair histogram to the device accumulator (asynchronous)."""

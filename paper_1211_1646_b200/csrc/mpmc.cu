@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -17,6 +18,13 @@
 #include "kernels.h"
 
 using namespace mpmc;
+
+// Scratch of mpmc_contact_histogram_noalloc (include/mpmc.h): the device histogram the contact-histogram kernels add their
+// counts to, as a file-scope device array instead of a piece of the caller's workspace, so that the call allocates nothing.
+// Every GPU that loads the library holds these 8 KB until the process exits.  In HOST code this name is a host-side stand-in,
+// not a device address (a kernel given it would fault, or silently use host memory where the GPU can reach it): the host
+// passes what cudaGetSymbolAddress returns (noalloc_scratch below).
+static __device__ __align__(256) unsigned long long g_noalloc_hist[MPMC_NOALLOC_MAX_BINS];
 
 struct mpmc_ctx {
   Params p;
@@ -296,6 +304,29 @@ int launch_histogram(mpmc_ctx* c, double dr, uint32_t nbins, unsigned long long*
   return MPMC_OK;
 }
 
+// The device address of g_noalloc_hist on the context's device: resolved once per device, with that device current, and kept.
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_mutex;
+unsigned long long* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};
+
+int noalloc_scratch(const mpmc_ctx* c, unsigned long long** out) {
+  int dev = -1;
+  CU(cudaGetDevice(&dev));
+  cudaPointerAttributes at;
+  CU(cudaPointerGetAttributes(&at, c->p.ctl));             // the device the context's workspace lives on
+  if (at.type != cudaMemoryTypeDevice || at.device != dev) return MPMC_ERR_ARG;   // ... must be the current one
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return MPMC_ERR_ARG;
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_ptr[dev]) {
+    void* ptr = nullptr;
+    CU(cudaGetSymbolAddress(&ptr, g_noalloc_hist));
+    if (!ptr) return MPMC_ERR_CUDA;
+    g_noalloc_ptr[dev] = static_cast<unsigned long long*>(ptr);
+  }
+  *out = g_noalloc_ptr[dev];
+  return MPMC_OK;
+}
+
 }  // namespace
 
 // =========================================================================================================
@@ -571,6 +602,22 @@ int mpmc_pressure_contact(mpmc_ctx* c, double dr, uint32_t nbins, uint32_t degre
   return c->sticky;
 }
 
+int mpmc_contact_histogram_noalloc(mpmc_ctx* c, double dr, uint32_t nbins, uint64_t* hist_out) {
+  if (!c || !hist_out || !(dr > 0) || nbins == 0) return MPMC_ERR_ARG;
+  if (nbins > MPMC_NOALLOC_MAX_BINS) return MPMC_ERR_TOO_LARGE;
+  if (!c->loaded) return MPMC_ERR_STATE;
+  unsigned long long* scratch = nullptr;
+  const int ss = noalloc_scratch(c, &scratch);
+  if (ss != MPMC_OK) return ss;
+  // the array keeps the last call's counts, and the kernels ADD: clear the bins this call uses
+  CU(cudaMemsetAsync(scratch, 0, (size_t)nbins * 8, c->stream));
+  const int st = launch_histogram(c, dr, nbins, scratch);
+  if (st != MPMC_OK) return st;
+  static_assert(sizeof(unsigned long long) == sizeof(uint64_t), "");
+  CU(cudaMemcpyAsync(hist_out, scratch, (size_t)nbins * 8, cudaMemcpyDeviceToDevice, c->stream));
+  return c->sticky;
+}
+
 int mpmc_pressure_accumulate(mpmc_ctx* c, double dr, uint32_t nbins) {
   if (!c || !(dr > 0) || nbins == 0 || nbins > MAX_BINS) return MPMC_ERR_ARG;
   if (!c->loaded) return MPMC_ERR_STATE;
@@ -713,6 +760,7 @@ const char* mpmc_strerror(int code) {
     case MPMC_ERR_CELL_OVERFLOW: return "more than n_max = 4 disks in one cell";
     case MPMC_ERR_CUDA: return "CUDA error (no device, or a launch failed)";
     case MPMC_ERR_STATE: return "no positions loaded";
+    case MPMC_ERR_TOO_LARGE: return "size beyond the fixed capacity of the no-allocation entry point (mpmc_contact_histogram_noalloc: at most MPMC_NOALLOC_MAX_BINS = 1024 bins)";
     default: return "unknown error";
   }
 }

@@ -34,8 +34,9 @@ def test_header_symbols_all_exported(lib):
 
 def test_version_and_strerror(lib):
     assert b"sm_100a" in lib.mpmc_version()
-    for code in range(0, -8, -1):
-        assert lib.mpmc_strerror(code)
+    for code in range(0, -9, -1):
+        assert lib.mpmc_strerror(code) and lib.mpmc_strerror(code) != b"unknown error"
+    assert b"1024" in lib.mpmc_strerror(-8)          # MPMC_ERR_TOO_LARGE names the limit of the no-allocation entry point
     assert lib.mpmc_strerror(-99) == b"unknown error"
 
 
@@ -72,6 +73,7 @@ def test_argument_errors_without_gpu(lib):
     assert lib.mpmc_create(C.byref(h), 10, b, 1.0, 0.1, 4, 1, binding.FP32, fake, 16, None) == -3
     assert lib.mpmc_create(C.byref(h), 10, b, 1.0, 0.1, 4, 1, binding.FP32, C.c_void_p(0x10001), 1 << 30, None) == -3
     assert lib.mpmc_sweep(None, 1) == -1
+    assert lib.mpmc_contact_histogram_noalloc(None, 0.1, 10, fake) == -1
     assert lib.mpmc_destroy(None) == 0
 
 
