@@ -180,6 +180,8 @@ def main():
     ap.add_argument("--ref-sweeps", type=int, default=2, help="oracle sweeps per step for --impl reference")
     ap.add_argument("--cpu-baseline-sweeps", type=int, default=15)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-resident", action="store_true",
+                    help="small systems on the fused tile kernels instead of the cluster-resident kernel (MPMC_NO_RESIDENT): A/B")
     args = ap.parse_args()
     w = I.CONFIGS[args.workload]
     if args.impl == "reference":
@@ -216,7 +218,8 @@ def main():
     xy_dev = xy_pinned.to(dev)
     out_dev = torch.empty_like(xy_dev)
     out_pinned = torch.empty_like(xy_pinned).pin_memory()
-    sim = Mpmc(w.N, box, w.sigma, w.d, w.n_s, w.seed + rank, fp32=w.fp32, device=dev, w_target=w.w_target, disc=w.disc)   # replicas: seed per rank
+    sim = Mpmc(w.N, box, w.sigma, w.d, w.n_s, w.seed + rank, fp32=w.fp32, device=dev, w_target=w.w_target, disc=w.disc,
+               resident=not args.no_resident)   # replicas: seed per rank
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
 
     def step_resident():
@@ -292,6 +295,9 @@ def main():
     l2_bytes = torch.cuda.get_device_properties(dev).L2_cache_size
     tile_name = "k_tile4_sweep" if (w.disc or w.w_target >= 1.15) else "k_tile_sweep"     # 4-slot / 2-slot tile kernel
     kernel = tile_name if tile_sweeps >= general_sweeps else "k_sweeps"
+    resident = cfg["resident_ctas"] > 0                # small system: ONE launch of one cluster runs all S sweeps (cluster.cuh)
+    if resident:
+        kernel = "k_cluster_sweeps"
     peak, peak_src = peaks()
     alg = algorithmic_bytes_per_sweep(w.N, sim.M, w.fp32)
     achieved = alg / (sweep_ms * 1e-3) / 1e9
@@ -310,6 +316,16 @@ def main():
                         ("one launch = one sweep; the state does not fit L2 (2 buffers x state_bytes > L2), so every sweep "
                          "streams it from and to HBM: `traffic` (ncu dram bytes per launch) against the fused floor "
                          "2 (e N + M) is the HBM figure")}
+    if resident:
+        roofline["launch_ms"] = sweep_ms * S
+        roofline["sweep_ms"] = sweep_ms
+        roofline["resident_ctas"] = cfg["resident_ctas"]
+        roofline["algorithmic_bytes_per_launch"] = alg * S
+        roofline["fused_floor_bytes_per_launch"] = 2.0 * state_bytes      # one launch reads the state once and writes it once
+        roofline["note"] = (f"one launch of one cluster of {cfg['resident_ctas']} CTAs = all {S} sweeps of a step on the state "
+                            "resident in shared memory: no HBM or L2 traffic inside the loop, the time is the latency of four "
+                            "sub-sweeps + shift + six cluster barriers per sweep; `achieved` = the 7-pass algorithmic bytes of "
+                            "those sweeps / launch time, reported because BASELINE.json names the HBM roofline")
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         try:
@@ -375,7 +391,9 @@ def main():
                     "per_step": spread(rates_e2e)},
             # cell-list build 4; one tile kernel per sweep (+ the general kernel's pass behind the 2-slot tile kernel: a
             # no-op unless a state was handed over), or one persistent launch without a tile kernel; histogram; unpack
-            "gpu_launches": args.steps * (4 + (S + (1 if cfg["tile_slots"] == 2 else 0) if cfg["tile_slots"] else 1) + 1 + 1),
+            # (small systems: one launch of the cluster-resident kernel for all sweeps of a step)
+            "gpu_launches": args.steps * (4 + (1 if cfg["resident_ctas"] else
+                                               (S + (1 if cfg["tile_slots"] == 2 else 0) if cfg["tile_slots"] else 1)) + 1 + 1),
             "roofline": roofline,
             "cpu_baseline": cpu,
             "cpu_baseline_strips": cpu_strips,

@@ -53,6 +53,9 @@ typedef struct mpmc_ctx mpmc_ctx; /* opaque host object; owns no device memory *
 /* ablations of PAPER.md section 2.4 / Table 1 (L114-142); both leave the chain valid only in the sense the paper discusses */
 #define MPMC_NO_PARTICLE_SHUFFLE 0x8u  /* visit the disks of a cell in slot order (the paper shows a pressure bias) */
 #define MPMC_NO_SET_SHUFFLE 0x10u     /* run the checkerboard sets in the fixed order a, b, c, d (harmless per the paper) */
+#define MPMC_NO_RESIDENT 0x20u        /* do not use the cluster-resident kernel for small systems (below): every sweep on the
+                                      * fused tile kernels or the general kernel, as for large systems.  Same trajectory; for
+                                      * tests of those kernels on small inputs and for A/B timing */
 #define MPMC_DEBUG 0x100u /* record per-cell accept masks and the accept-sequence digest (tests only; slower) */
 
 /* Bytes of device workspace mpmc_create needs for this system (0 on invalid arguments).  Pure host arithmetic.
@@ -166,8 +169,11 @@ int mpmc_debug_path(mpmc_ctx* ctx, uint64_t out[2]);
  * kernel: 2 (tile.cuh, w ~ sigma), 4 (tile4.cuh) or 0 (no tile kernel: every sweep on the general persistent kernel);
  * CTAs (= tiles) of the tile kernel; tiles per row of tiles (first group of rows, see mpmc_debug_tiling);
  * tiles along y; threads per tile CTA; dynamic shared memory per tile CTA in bytes; CTAs of the general kernel; threads
- * per CTA of the general kernel}. */
-int mpmc_debug_config(const mpmc_ctx* ctx, uint32_t out[8]);
+ * per CTA of the general kernel; CTAs of the cluster-resident kernel (cluster.cuh; 0 = not used: the system is too large
+ * for one cluster's shared memory, n_s != 4, or MPMC_NO_RESIDENT) — when non-zero, mpmc_sweep(k) is ONE launch of that
+ * kernel and the tile kernel's entries describe what MPMC_NO_RESIDENT would use; its tiles along x; along y; its dynamic
+ * shared memory per CTA in bytes}. */
+int mpmc_debug_config(const mpmc_ctx* ctx, uint32_t out[12]);
 
 /* Profiling hook.  A library built with -DMPMC_PHASE_CLOCKS (paper_1211_1646_b200/phase_clocks.py) makes the 2-slot tile
  * kernel record a clock mark at each of its phase boundaries; this call copies the marks of the LAST launch to the host:

@@ -15,6 +15,7 @@ FP32 = 0x2
 DISC = 0x4
 NO_PARTICLE_SHUFFLE = 0x8
 NO_SET_SHUFFLE = 0x10
+NO_RESIDENT = 0x20
 DEBUG = 0x100
 NOALLOC_MAX_BINS = 1024       # MPMC_NOALLOC_MAX_BINS of include/mpmc.h
 ERR_TOO_LARGE = -8            # MPMC_ERR_TOO_LARGE
@@ -97,7 +98,8 @@ class Mpmc:
 
     def __init__(self, N: int, box, sigma: float, d: float, n_s: int, seed: int, fp32: bool = False,
                  debug: bool = False, w_target: float = 0.0, device="cuda:0", stream=None, disc: bool = False,
-                 particle_shuffle: bool = True, set_shuffle: bool = True):
+                 particle_shuffle: bool = True, set_shuffle: bool = True, resident: bool = True):
+        """resident=False: MPMC_NO_RESIDENT (small systems on the tile / general kernels instead of the cluster-resident one)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1211_1646_b200 needs a CUDA device; there is no CPU fallback")
@@ -105,7 +107,8 @@ class Mpmc:
         self.device = torch.device(device)
         self.N, self.fp32, self.debug, self.sigma = int(N), bool(fp32), bool(debug), float(sigma)
         self.flags = ((FP32 if fp32 else FP64) | (DEBUG if debug else 0) | (DISC if disc else 0)
-                      | (0 if particle_shuffle else NO_PARTICLE_SHUFFLE) | (0 if set_shuffle else NO_SET_SHUFFLE))
+                      | (0 if particle_shuffle else NO_PARTICLE_SHUFFLE) | (0 if set_shuffle else NO_SET_SHUFFLE)
+                      | (0 if resident else NO_RESIDENT))
         nbytes = workspace_bytes(N, box, sigma, fp32, debug, w_target)
         if nbytes == 0:
             # let mpmc_create report the precise error code
@@ -275,9 +278,10 @@ class Mpmc:
 
     def config(self) -> dict:
         """How mpmc_sweep runs this context (mpmc_debug_config; host values only)."""
-        out = (_u32 * 8)()
+        out = (_u32 * 12)()
         _chk(lib().mpmc_debug_config(self._h, out))
-        keys = ("tile_slots", "tiles", "ntx", "nty", "tile_threads", "tile_smem", "general_grid", "general_threads")
+        keys = ("tile_slots", "tiles", "ntx", "nty", "tile_threads", "tile_smem", "general_grid", "general_threads",
+                "resident_ctas", "resident_cx", "resident_cy", "resident_smem")
         return dict(zip(keys, (int(v) for v in out)))
 
     def phase_clocks(self):

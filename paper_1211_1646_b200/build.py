@@ -15,17 +15,18 @@ OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libmpmc_b200.so")
 # headers each source includes (directly or not)
 HEADERS = {
-    "mpmc.cu": ["common.cuh", "sweep.cuh", "tile.cuh", "tile4.cuh", "aux.cuh", "kernels.h",
+    "mpmc.cu": ["common.cuh", "sweep.cuh", "tile.cuh", "tile4.cuh", "cluster.cuh", "aux.cuh", "kernels.h",
                 os.path.join("..", "..", "include", "mpmc.h")],
     "k_general.cu": ["common.cuh", "sweep.cuh", "kernels.h"],
     "k_tile2.cu": ["common.cuh", "sweep.cuh", "tile.cuh", "kernels.h"],
     "k_tile4.cu": ["common.cuh", "sweep.cuh", "tile.cuh", "tile4.cuh", "kernels.h"],
+    "k_cluster.cu": ["common.cuh", "sweep.cuh", "tile.cuh", "cluster.cuh", "kernels.h"],
 }
 # (source, object name, extra defines)
 _PREC = [("f32", "float"), ("f64", "double")]
 UNITS = [("mpmc.cu", "mpmc.o", [])] + [
     (src, f"{src[:-3]}_{sfx}.o", [f"-DMPMC_P={typ}", f"-DMPMC_SUFFIX={sfx}"])
-    for src in ("k_general.cu", "k_tile2.cu", "k_tile4.cu") for sfx, typ in _PREC]
+    for src in ("k_general.cu", "k_tile2.cu", "k_tile4.cu", "k_cluster.cu") for sfx, typ in _PREC]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -77,6 +77,8 @@ struct Params {
                                         // other rows the rest with tl_ntx + 1 tiles each (uniform tiling: tl_na = tl_nty, tl_hyA = hy)
   uint32_t tl_PH;                       // ... rows of the tallest tile's planes (sorted variant: stride of its row tables)
   uint32_t tl_div[4][3];                // n / d without a divide (host: div_magic) for d = tl_ntx, tl_ntx + 1, tl_na, tl_nty - tl_na
+  uint32_t cl_cx, cl_cy, cl_cap, cl_stride;   // cluster-resident kernel (cluster.cuh): tiles per row / column = CTAs of the cluster, cells a CTA
+                                        // has room for, row stride of a CTA's cell arrays (the widest tile)
   uint32_t seed_lo, seed_hi;
   uint32_t rk0[10], rk1[10];            // Philox round keys seed + r * Weyl constant (philox4x32_10_rk)
   float wx_f, wy_f, sigma2_f, d_f;      // working-precision constants (fp32 mode)

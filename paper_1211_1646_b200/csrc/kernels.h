@@ -20,4 +20,9 @@ int phase_clocks_f64(unsigned long long* out, uint32_t tiles, void* stream);
 const void* pick_tile4_kernel_f32(bool debug, bool disc, uint32_t n_s);
 const void* pick_tile4_kernel_f64(bool debug, bool disc, uint32_t n_s);
 
+// k_cluster_sweeps<P, 4, DEBUG, DISC, FAST> (cluster.cuh): the whole state resident in one cluster's shared memory; fast = the
+// w ~ sigma cell update (square proposal only); nullptr unless n_s = 4
+const void* pick_cluster_kernel_f32(bool debug, bool disc, bool fast, uint32_t n_s);
+const void* pick_cluster_kernel_f64(bool debug, bool disc, bool fast, uint32_t n_s);
+
 }  // namespace mpmc

@@ -15,6 +15,7 @@
 #include "sweep.cuh"
 #include "tile.cuh"
 #include "tile4.cuh"
+#include "cluster.cuh"
 #include "kernels.h"
 
 using namespace mpmc;
@@ -41,6 +42,10 @@ struct mpmc_ctx {
   uint32_t tile_threads;   // threads per CTA of the tile kernel
   bool tile_two_slot;      // the tile kernel is the 2-slot one (tile.cuh), which may hand a crowded state to the general kernel
   uint32_t sms;            // SMs of the device
+  const void* cluster_kernel;  // the k_cluster_sweeps instantiation when the system is small enough to live in one cluster's
+  uint32_t cl_ctas;            // shared memory (cluster.cuh), else nullptr; its CTAs (= cluster size), threads per CTA and
+  uint32_t cl_threads;         // dynamic shared memory per CTA
+  size_t cl_smem;
   uint64_t t_host;         // sweeps requested since the last load (the sweep index the device will reach)
   uint32_t cur_host;       // ... and the buffer that will hold that state (every sweep and every test-hook shift flips it)
   unsigned long long* hist_acc;   // device: histogram accumulated over samples (mpmc_pressure_accumulate)
@@ -472,6 +477,53 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
       }
     }
   }
+  // Small systems: the whole state resident in the shared memory of ONE cluster of up to 16 CTAs (cluster.cuh), all sweeps
+  // of a call in one launch.  Chosen while a CTA's tile stays within cluster_max_cells_per_cta (beyond that the fused tile
+  // kernels, which use all SMs, are faster: measured, cluster.cuh).  MPMC_NO_RESIDENT turns it off.
+  c->cluster_kernel = nullptr; c->cl_ctas = 0; c->cl_threads = 0; c->cl_smem = 0;
+  p.cl_cx = p.cl_cy = p.cl_cap = p.cl_stride = 0;
+  if (!(flags & MPMC_NO_RESIDENT)) {
+    const bool cfast = c->nf == 2 && !disc;
+    const void* ck = fp32 ? pick_cluster_kernel_f32(debug, disc, cfast, n_s) : pick_cluster_kernel_f64(debug, disc, cfast, n_s);
+    const uint32_t threads = fp32 ? ClThreads<float>::value : ClThreads<double>::value;
+    const size_t cell_bytes = fp32 ? cluster_cell_bytes<float>() : cluster_cell_bytes<double>();
+    const uint32_t cap_max = fp32 ? cluster_max_cells_per_cta<float>(cfast) : cluster_max_cells_per_cta<double>(cfast);
+    int smem_optin = 0, cluster_ok = 0;
+    cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    cudaDeviceGetAttribute(&cluster_ok, cudaDevAttrClusterLaunch, dev);
+    // the largest cluster (most SMs), then the squarest tiles, whose tiles fit; sizes above 8 are "non-portable" and
+    // depend on the GPU's partitioning, so every candidate is checked with the occupancy query
+    for (uint32_t nc = CL_MAX_CTAS; ck && cluster_ok && nc >= 1 && !c->cluster_kernel; nc >>= 1) {
+      uint32_t best_cx = 0, best_cap = 0, best_stride = 0; double best_aspect = 0;
+      for (uint32_t cx = 1; cx <= nc; ++cx) {
+        if (nc % cx) continue;
+        const uint32_t cy = nc / cx;
+        if (cx > p.mx || cy > p.my) continue;
+        const uint32_t tw = (p.mx + cx - 1) / cx, th = (p.my + cy - 1) / cy, cap = tw * th;
+        if (cap > cap_max || cap * cell_bytes + 1024 > (size_t)smem_optin) continue;
+        const double aspect = tw > th ? (double)tw / th : (double)th / tw;
+        if (!best_cx || aspect < best_aspect) { best_cx = cx; best_cap = cap; best_stride = tw; best_aspect = aspect; }
+      }
+      if (!best_cx) continue;
+      const size_t smem = (size_t)best_cap * cell_bytes;
+      cudaFuncAttributes fa;                      // (a per-function attribute: set to the most any context can ask for)
+      if (cudaFuncGetAttributes(&fa, ck) != cudaSuccess || (size_t)smem_optin < fa.sharedSizeBytes + smem ||
+          cudaFuncSetAttribute(ck, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - (int)fa.sharedSizeBytes) != cudaSuccess ||
+          (nc > 8 && cudaFuncSetAttribute(ck, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess)) {
+        cudaGetLastError(); continue;
+      }
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3(nc); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = smem;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = nc; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      int nclusters = 0;
+      if (cudaOccupancyMaxActiveClusters(&nclusters, ck, &cfg) != cudaSuccess || nclusters < 1) { cudaGetLastError(); continue; }
+      c->cluster_kernel = ck; c->cl_ctas = nc; c->cl_threads = threads; c->cl_smem = smem;
+      p.cl_cx = best_cx; p.cl_cy = nc / best_cx; p.cl_cap = best_cap; p.cl_stride = best_stride;
+    }
+  }
   *out = c;
   return MPMC_OK;
 }
@@ -524,6 +576,22 @@ int mpmc_sweep(mpmc_ctx* c, uint64_t k) {
   if (!c) return MPMC_ERR_ARG;
   if (!c->loaded) return MPMC_ERR_STATE;
   if (k == 0) return c->sticky;
+  if (c->cluster_kernel) {
+    // small systems: ONE launch of one cluster runs all k sweeps on the state resident in its shared memory (cluster.cuh);
+    // the state returns to the buffer it came from, so the buffer parity does not change
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(c->cl_ctas); cfg.blockDim = dim3(c->cl_threads);
+    cfg.dynamicSmemBytes = c->cl_smem; cfg.stream = c->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = c->cl_ctas; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    unsigned long long t_end = c->t_host + k;
+    void* args[] = {(void*)&c->p, (void*)&t_end};
+    CU(cudaLaunchKernelExC(&cfg, c->cluster_kernel, args));
+    c->t_host += k;
+    return c->sticky;
+  }
   if (c->tile_kernel) {
     // one tile-kernel launch per sweep; each returns at once if the state has become crowded (tile.cuh) ...
     // Programmatic dependent launch: the CTAs of sweep t+1 become resident as the SMs of sweep t free up and park at
@@ -710,7 +778,7 @@ int mpmc_debug_path(mpmc_ctx* c, uint64_t out[2]) {
   return st;
 }
 
-int mpmc_debug_config(const mpmc_ctx* c, uint32_t out[8]) {
+int mpmc_debug_config(const mpmc_ctx* c, uint32_t out[12]) {
   if (!c || !out) return MPMC_ERR_ARG;
   out[0] = c->tile_kernel ? (c->tile_two_slot ? 2u : 4u) : 0u;
   out[1] = c->tile_kernel ? c->tile_grid : 0u;
@@ -718,6 +786,7 @@ int mpmc_debug_config(const mpmc_ctx* c, uint32_t out[8]) {
   out[4] = c->tile_kernel ? c->tile_threads : 0u;
   out[5] = (uint32_t)c->tile_smem;
   out[6] = c->grid; out[7] = (uint32_t)SUB_THREADS;
+  out[8] = c->cluster_kernel ? c->cl_ctas : 0u; out[9] = c->p.cl_cx; out[10] = c->p.cl_cy; out[11] = (uint32_t)c->cl_smem;
   return MPMC_OK;
 }
 

@@ -21,10 +21,13 @@ def torch_cuda():
     return torch
 
 
-def make_pair(oracle_mod, torch, N, box, sigma, d, n_s, seed, fp32, xy, debug=True, w_target=0.0, disc=False, **ablate):
+def make_pair(oracle_mod, torch, N, box, sigma, d, n_s, seed, fp32, xy, debug=True, w_target=0.0, disc=False,
+              resident=False, **ablate):
+    """resident=False keeps small systems on the tile / general kernels (MPMC_NO_RESIDENT), which is what most tests here
+    are about; the cluster-resident kernel has its own tests below (test_resident_*)."""
     from paper_1211_1646_b200.binding import Mpmc
     o = oracle_mod.Oracle(N, box, sigma, d, n_s, seed, fp32=fp32, w_target=w_target, disc=disc, **ablate)
-    g = Mpmc(N, box, sigma, d, n_s, seed, fp32=fp32, debug=debug, w_target=w_target, disc=disc, **ablate)
+    g = Mpmc(N, box, sigma, d, n_s, seed, fp32=fp32, debug=debug, w_target=w_target, disc=disc, resident=resident, **ablate)
     assert (g.mx, g.my) == (o.mx, o.my) and (g.wx, g.wy) == (o.wx, o.wy) and g.L_eff == o.L_eff
     o.load_positions(xy)
     g.load_positions(torch.as_tensor(xy, device="cuda"))
@@ -122,6 +125,98 @@ def test_c1_100_sweeps_bit_exact(oracle_mod, torch_cuda, fp32):
     assert g.path_sweeps() == (100, 0)                 # every sweep on the fused tile kernel
     att, acc, rb, ro = g.acceptance()
     assert att == acc + rb + ro and acc > 0 and rb > 0 and ro > 0
+
+
+# ---- the cluster-resident kernel for small systems (cluster.cuh): all sweeps of a call in one launch of one cluster ----
+@pytest.mark.parametrize("fp32", [False, True])
+def test_resident_c1_100_sweeps_bit_exact(oracle_mod, torch_cuda, fp32):
+    w = I.CONFIGS["C1"]
+    xy, box = I.workload_inputs(w)
+    o, g = make_pair(oracle_mod, torch_cuda, w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32, xy, resident=True)
+    cfg = g.config()
+    assert cfg["resident_ctas"] == cfg["resident_cx"] * cfg["resident_cy"] >= 1
+    for k in (1, 1, 3, 16, 17, 62):                    # several call sizes: one launch per call
+        o.sweep(k); g.sweep(k)
+        st = assert_same_state(o, g, fp32)
+    assert st["sweep"] == 100 and g.path_sweeps() == (100, 0)
+    # pieces through the test hooks (general kernel on the global state) between resident calls
+    o.sub_sweep(2); g.sub_sweep(2)
+    o.shift(1, 0.3 * o.wx); g.shift(1, 0.3 * o.wx)
+    o.sweep(5); g.sweep(5)
+    assert_same_state(o, g, fp32)
+    ho, _, _ = o.pressure_contact(0.005, 20, 2)
+    assert np.array_equal(ho, g.contact_histogram(0.005, 20))
+
+
+@pytest.mark.parametrize("n,phi,w_target,disc,fp32", [(26, 0.6, 0.0, False, True), (50, 0.716, 0.0, False, False),
+                                                      (34, 0.3, 0.0, False, True), (64, 0.698, 1.4, True, True),
+                                                      (46, 0.698, 1.4, False, False), (90, 0.716, 0.0, False, True),
+                                                      (120, 0.65, 1.4, True, True)])
+def test_resident_uneven_tiles_widths_and_proposals(oracle_mod, torch_cuda, n, phi, w_target, disc, fp32):
+    """Grids that do not divide evenly among the cluster's CTAs, both cell regimes (cells of up to 4 disks), both
+    proposals, dilute and dense."""
+    xy, box = I.jittered_lattice(n, phi, 1.0, seed=3)
+    o, g = make_pair(oracle_mod, torch_cuda, n * n, box, 1.0, 0.12, 4, 77, fp32, xy, w_target=w_target, disc=disc, resident=True)
+    assert g.config()["resident_ctas"] >= 1
+    for k in (1, 2, 9):
+        o.sweep(k); g.sweep(k)
+        assert_same_state(o, g, fp32)
+    assert g.path_sweeps() == (12, 0)
+
+
+@pytest.mark.parametrize("fp32", [False, True])
+def test_resident_cells_with_three_disks_at_unit_width(oracle_mod, torch_cuda, fp32):
+    # w ~ 1.13 sigma keeps the fast cell update (w < 1.15 sigma) while cells with THREE disks do occur: next to such a cell
+    # the update takes the general routine, the shift the eight-candidate one (the recipe of
+    # test_three_per_cell_with_two_register_slots, on the resident kernel)
+    xy, box = I.jittered_lattice(64, 0.50, seed=6)
+    o, g = make_pair(oracle_mod, torch_cuda, 4096, box, 1.0, 0.3, 4, 8, fp32, xy, w_target=1.12, resident=True)
+    assert g.config()["resident_ctas"] >= 1 and g.config()["tile_slots"] == 2
+    seen3 = False
+    for _ in range(10):
+        o.sweep(20); g.sweep(20)
+        st = assert_same_state(o, g, fp32)
+        seen3 |= st["counts"].max() >= 3
+    assert seen3 and g.path_sweeps() == (200, 0)
+
+
+@pytest.mark.parametrize("N,box,xy", [
+    (1, (2.6, 2.6), [[0.3, 0.4]]),
+    (2, (2.6, 2.9), [[0.5, 0.5], [1.8, 1.9]]),                 # mx = my = 2: neighbour at two image offsets
+    (3, (4.3, 4.5), [[0.5, 0.5], [2.0, 2.0], [3.5, 0.9]]),
+    (5, (9.7, 2.4), [[0.5, 0.5], [2.0, 1.9], [3.5, 0.9], [6.1, 1.2], [8.3, 0.4]]),     # 8 x 2 cells: tiles one cell high
+])
+@pytest.mark.parametrize("fp32", [False, True])
+def test_resident_tiny_systems(oracle_mod, torch_cuda, N, box, xy, fp32):
+    xy = np.array(xy, dtype=np.float64)
+    o, g = make_pair(oracle_mod, torch_cuda, N, box, 1.0, 0.4, 4, 9, fp32, xy, resident=True)
+    assert g.config()["resident_ctas"] >= 1
+    for _ in range(5):
+        o.sweep(40); g.sweep(40)
+        assert_same_state(o, g, fp32)
+
+
+@pytest.mark.parametrize("pshuf,sshuf", [(False, True), (True, False), (False, False)])
+@pytest.mark.parametrize("w_target", [0.0, 1.40])
+def test_resident_ablation_switches(oracle_mod, torch_cuda, pshuf, sshuf, w_target):
+    xy, box = I.jittered_lattice(64, 0.66, seed=12)
+    o, g = make_pair(oracle_mod, torch_cuda, 4096, box, 1.0, 0.2, 4, 3, True, xy, w_target=w_target,
+                     particle_shuffle=pshuf, set_shuffle=sshuf, resident=True)
+    assert g.config()["resident_ctas"] >= 1
+    o.sweep(12); g.sweep(12)
+    assert_same_state(o, g, True)
+
+
+def test_resident_is_not_used_beyond_its_capacity_or_when_switched_off(oracle_mod, torch_cuda):
+    from paper_1211_1646_b200.binding import Mpmc
+    w = I.CONFIGS["C2"]                                # 73 080 cells: too many for one cluster
+    xy, box = I.workload_inputs(w)
+    assert Mpmc(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=True).config()["resident_ctas"] == 0
+    w = I.CONFIGS["C1"]
+    xy, box = I.workload_inputs(w)
+    assert Mpmc(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=True, resident=False).config()["resident_ctas"] == 0
+    assert Mpmc(w.N, box, w.sigma, w.d, 8, w.seed, fp32=True).config()["resident_ctas"] == 0      # n_s = 4 only
+    assert Mpmc(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=True).config()["resident_ctas"] >= 1
 
 
 @pytest.mark.parametrize("fp32", [False, True])
