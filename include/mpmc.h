@@ -181,7 +181,9 @@ int mpmc_debug_config(const mpmc_ctx* ctx, uint32_t out[12]);
  * nanosecond timer at the start of the tile's work, values 1-8 are SM cycle counters (clock64) at the ends of: wait for
  * the previous sweep, load, sub-sweeps 1-4, shift, (unused); the rest are marks inside the load phase and before it
  * (paper_1211_1646_b200/phase_clocks.py names them).  *marks = values per row (at most 32), 0 in an ordinary build
- * (nothing is written to out).  MPMC_ERR_STATE unless the context runs the 2-slot tile kernel.  Synchronises. */
+ * (nothing is written to out).  A context on the cluster-resident kernel gets one row per CTA of the cluster instead:
+ * {sweeps of the last call, SM cycles thread 0 spent in the sub-sweeps, at the cluster barriers, in the shift, in the whole
+ * loop}.  MPMC_ERR_STATE unless the context runs the 2-slot tile kernel or the cluster-resident kernel.  Synchronises. */
 int mpmc_debug_phase_clocks(mpmc_ctx* ctx, uint64_t* out, uint32_t max_tiles, uint32_t* marks);
 
 /* Test hook (pure host arithmetic, no device needed): the tiling the fused tile kernels would use for a grid of

@@ -285,10 +285,12 @@ class Mpmc:
         return dict(zip(keys, (int(v) for v in out)))
 
     def phase_clocks(self):
-        """(tiles, marks) uint64 array of the tile kernel's clock marks in its last launch; None unless the library was
-        built with -DMPMC_PHASE_CLOCKS (mpmc_debug_phase_clocks)."""
+        """(tiles, marks) uint64 array of the tile kernel's clock marks in its last launch — for a context on the
+        cluster-resident kernel (CTAs, 5): {sweeps, cycles in sub-sweeps, at barriers, in the shift, in the whole loop} of
+        the last call; None unless the library was built with -DMPMC_PHASE_CLOCKS (mpmc_debug_phase_clocks)."""
         import numpy as np
-        tiles = self.config()["tiles"]
+        cfg = self.config()
+        tiles = cfg["resident_ctas"] or cfg["tiles"]   # the cluster-resident kernel reports one row per CTA
         flat = np.zeros(max(tiles, 1) * 32, dtype=np.uint64)
         marks = _u32()
         with self.torch.cuda.device(self.device):

@@ -64,26 +64,53 @@ __device__ __forceinline__ ClTile<P> cl_tile(unsigned char* base, const uint32_t
   return t;
 }
 
-// The moves of one cell whose 3 x 3 cells hold at most 2 disks each (w ~ sigma), on registers: h = slot pair 0 of the 3 x 3
-// cells (idx 4 = own), n = the own count.  The arithmetic of update_cell_fast (sweep.cuh) / tile_update_cell (tile.cuh),
-// step for step: neighbours translated into this cell's frame and negated with one fma, -(l_j + s) = fma(l_j, -1, -s)
-// (L154, L196); the two own disks in visiting order, swapped iff n = 2 (L75, L187); verdict of a move = in the cell and
-// min r^2 >= sigma^2 (L79, L118, L194-204).  Returns the new slot pair in slot order, the accept mask and the tallies.
+// -DMPMC_PHASE_CLOCKS (phase_clocks.py --resident): thread 0 of every CTA adds up the SM cycles it spends in the sub-sweeps,
+// at the cluster barriers and in the shift; row = CTA, values = {sweeps, sub-sweeps, barriers, shift, whole loop}
+#ifdef MPMC_PHASE_CLOCKS
+constexpr uint32_t CL_CLOCK_MARKS = 5;
+__device__ unsigned long long g_cluster_clocks[CL_MAX_CTAS][CL_CLOCK_MARKS];
+#define MPMC_CL_CLOCK_START() long long ck_sub = 0, ck_bar = 0, ck_shift = 0, ck_a = clock64(); const long long ck_t0 = ck_a
+#define MPMC_CL_CLOCK_ADD(v) do { const long long n_ = clock64(); v += n_ - ck_a; ck_a = n_; } while (0)
+#else
+#define MPMC_CL_CLOCK_START() do { } while (0)
+#define MPMC_CL_CLOCK_ADD(v) do { } while (0)
+#endif
+
+// The random numbers of one cell's moves in the fast update: the NS displacements (Alg. 2 line 12, L190; A2, A9) and
+// whether the shuffle of TWO disks swaps them (line 9, L187: Fisher-Yates of two is one draw, j = bounded(S0, 2); j = 0
+// swaps; made only for a cell of two).  The displacement blocks depend on nothing loaded: they run under the loads.
+template <typename P, int NS> struct ClDraws { P ddx[NS], ddy[NS]; bool swap2; };
 template <typename P, int NS>
-__device__ __forceinline__ void cl_moves_fast(const Params& p, const Half<P> (&h)[9], const uint32_t n, const uint32_t cell,
-                                              const uint32_t t_lo, const uint32_t t_hi, Half<P>& o, uint32_t& amask,
-                                              uint32_t& n_acc, uint32_t& n_rb, uint32_t& n_ro) {
+__device__ __forceinline__ void cl_draws_fast(const Params& p, const uint32_t cell, const uint32_t t_lo, const uint32_t t_hi,
+                                              const bool two, ClDraws<P, NS>& d) {
   using R = Real<P>;
-  using Pair = typename R::Pair;
   static_assert(NS > 0 && NS % 2 == 0, "compile-time n_s must be even");
-  P ddx[NS], ddy[NS];
 #pragma unroll
-  for (int q = 0; q < NS / 2; ++q) {               // displacements of all NS moves (line 12, L190; A2, A9)
+  for (int q = 0; q < NS / 2; ++q) {
     uint32_t Rw[4];
     philox4x32_10(cell, t_lo, t_hi, (uint32_t)q, p.seed_lo, p.seed_hi, Rw);
-    ddx[2 * q] = R::scaled_sym(p, Rw[0]); ddy[2 * q] = R::scaled_sym(p, Rw[1]);
-    ddx[2 * q + 1] = R::scaled_sym(p, Rw[2]); ddy[2 * q + 1] = R::scaled_sym(p, Rw[3]);
+    d.ddx[2 * q] = R::scaled_sym(p, Rw[0]); d.ddy[2 * q] = R::scaled_sym(p, Rw[1]);
+    d.ddx[2 * q + 1] = R::scaled_sym(p, Rw[2]); d.ddy[2 * q + 1] = R::scaled_sym(p, Rw[3]);
   }
+  d.swap2 = false;
+  if (two) {                                       // (a single disk is not shuffled: no draw is made)
+    uint32_t S[4];
+    philox4x32_10(cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
+    d.swap2 = bounded(S[0], 2u) == 0u && !(p.flags & FLAG_NO_PARTICLE_SHUFFLE);
+  }
+}
+
+// The moves of one cell whose 3 x 3 cells hold at most 2 disks each (w ~ sigma), on registers: h = slot pair 0 of the 3 x 3
+// cells (idx 4 = own), n = the own count, d = the cell's draws.  The arithmetic of update_cell_fast (sweep.cuh) /
+// tile_update_cell (tile.cuh), step for step: neighbours translated into this cell's frame and negated with one fma,
+// -(l_j + s) = fma(l_j, -1, -s) (L154, L196); the two own disks in visiting order, swapped iff n = 2 (L75, L187); verdict of
+// a move = in the cell and min r^2 >= sigma^2 (L79, L118, L194-204).  Returns the new slot pair in slot order, the accept
+// mask and the tallies.
+template <typename P, int NS>
+__device__ __forceinline__ void cl_moves_fast(const Params& p, const Half<P> (&h)[9], const uint32_t n, const ClDraws<P, NS>& d,
+                                              Half<P>& o, uint32_t& amask, uint32_t& n_acc, uint32_t& n_rb, uint32_t& n_ro) {
+  using R = Real<P>;
+  using Pair = typename R::Pair;
   n_acc = 0; n_rb = 0; n_ro = 0; amask = 0;
   const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p);
   const Pair MINUS1 = R::pair((P)-1, (P)-1);
@@ -100,16 +127,11 @@ __device__ __forceinline__ void cl_moves_fast(const Params& p, const Half<P> (&h
   }
   P Ax = h[4].x.x, Ay = h[4].y.x, Bx = h[4].x.y, By = h[4].y.y;      // own cell in visiting order (Alg. 2 lines 8-9)
   const bool two = n == 2u;
-  bool flip = false;                               // true: A is slot 1
-  if (two) {                                       // n = 2: Fisher-Yates is one draw, j = bounded(S0, 2); j = 0 swaps
-    uint32_t S[4];
-    philox4x32_10(cell, t_lo, t_hi, SLOT_SHUFFLE, p.seed_lo, p.seed_hi, S);
-    flip = bounded(S[0], 2u) == 0u && !(p.flags & FLAG_NO_PARTICLE_SHUFFLE);
-  }
+  bool flip = two && d.swap2;                      // true: A is slot 1 (a single disk is not shuffled: no draw is used)
   if (flip) { const P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }
 #pragma unroll
   for (int s = 0; s < NS; ++s) {                   // NS trial moves (Alg. 2 lines 11-32, L189-230)
-    const P Mx = R::add(Ax, ddx[s]), My = R::add(Ay, ddy[s]);
+    const P Mx = R::add(Ax, d.ddx[s]), My = R::add(Ay, d.ddy[s]);
     const bool inside = (Mx > (P)0) && (Mx <= wx) && (My > (P)0) && (My <= wy);   // (0, w]  (A3; L79, L118)
     const P Dbx = R::sub(Mx, Bx), Dby = R::sub(My, By);                          // the other own disk
     P rmin = R::fma(Dbx, Dbx, R::mul(Dby, Dby));
@@ -248,25 +270,37 @@ k_cluster_sweeps(const __grid_constant__ Params p, const unsigned long long t_en
   }
   cluster.sync();                                // every CTA of the cluster runs and has loaded its tile
   Tally tally;
+  MPMC_CL_CLOCK_START();
+
+  // The cells of checkerboard set Q in this tile: every second column from ax0, every second row from ay0.
+  struct ActiveSet { uint32_t ax0, ay0, nax, na, inv_a; };
+  auto active_set = [&](const uint32_t Q) {
+    ActiveSet a;
+    const uint32_t qx = Q & 1u, qy = Q >> 1;
+    a.ax0 = x0 + ((x0 ^ qx) & 1u); a.ay0 = y0 + ((y0 ^ qy) & 1u);
+    a.nax = a.ax0 < x1 ? (x1 - a.ax0 + 1u) >> 1 : 0u;
+    const uint32_t nay = a.ay0 < y1 ? (y1 - a.ay0 + 1u) >> 1 : 0u;
+    a.na = a.nax * nay; a.inv_a = small_div_magic(a.nax == 0u ? 1u : a.nax);
+    return a;
+  };
+  auto set_of = [](const Draws& d, const uint32_t k) { return k == 0u ? d.order[0] : k == 1u ? d.order[1] : k == 2u ? d.order[2] : d.order[3]; };
+  // (Making a cell's draws while its thread waits at the barrier BEFORE the sub-sweep was tried: the Philox rounds already
+  // run under the latency of the sub-sweep's loads, so nothing left the critical path and the barriers grew: C1 +3-7 %.)
+  Draws dr = draw_sweep(p, t_start);             // Alg. 1 lines 2, 15, 16 (L64, L90-91): a pure function of (seed, t)
 
 #pragma unroll 1
   for (unsigned long long t = t_start; t < t_end; ++t) {
-    const Draws dr = draw_sweep(p, t);           // Alg. 1 lines 2, 15, 16 (L64, L90-91): a pure function of (seed, t)
     const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
     const ClTile<P> me = cl_tile<P>(cl_smem, cap, b);
     // ---- four sub-sweeps (Alg. 1 lines 3-14, L66-88): a sub-sweep writes cells of its set only and reads, besides the
     //      own cell, cells of the other sets only, so there is nothing to order inside it ----
 #pragma unroll 1
     for (uint32_t k = 0; k < 4u; ++k) {
-      const uint32_t Q = k == 0u ? dr.order[0] : k == 1u ? dr.order[1] : k == 2u ? dr.order[2] : dr.order[3];
-      const uint32_t qx = Q & 1u, qy = Q >> 1;
-      // the cells of set Q in this tile: every second column from ax0, every second row from ay0
-      const uint32_t ax0 = x0 + ((x0 ^ qx) & 1u), ay0 = y0 + ((y0 ^ qy) & 1u);
-      const uint32_t nax = ax0 < x1 ? (x1 - ax0 + 1u) >> 1 : 0u, nay = ay0 < y1 ? (y1 - ay0 + 1u) >> 1 : 0u;
-      const uint32_t na = nax * nay, inv_a = small_div_magic(nax == 0u ? 1u : nax);
-      for (uint32_t idx = tid; idx < na; idx += T) {
-        const uint32_t iy = small_div(idx, inv_a), ix = idx - iy * nax;
-        const uint32_t gx = ax0 + 2u * ix, gy = ay0 + 2u * iy, lx = gx - x0, ly = gy - y0;
+      const ActiveSet as = active_set(set_of(dr, k));
+      MPMC_CL_CLOCK_ADD(ck_shift);                 // (set-up of the sub-sweep: counted with the shift)
+      for (uint32_t idx = tid; idx < as.na; idx += T) {
+        const uint32_t iy = small_div(idx, as.inv_a), ix = idx - iy * as.nax;
+        const uint32_t gx = as.ax0 + 2u * ix, gy = as.ay0 + 2u * iy, lx = gx - x0, ly = gy - y0;
         const uint32_t cell = gy * p.mx + gx;
         uint32_t amask, n_acc, n_rb, n_ro, n;
         if constexpr (FAST) {
@@ -289,8 +323,10 @@ k_cluster_sweeps(const __grid_constant__ Params p, const unsigned long long t_en
             if (n > 0u) cl_update_general_rare<P, NS>(p, s_base, g, b, lx, ly, cell, t_lo, t_hi, r4);
             amask = r4[0]; n_acc = r4[1]; n_rb = r4[2]; n_ro = r4[3];
           } else {
+            ClDraws<P, NS> pre;
+            cl_draws_fast<P, NS>(p, cell, t_lo, t_hi, n == 2u, pre);
             Half<P> o;
-            cl_moves_fast<P, NS>(p, h, n, cell, t_lo, t_hi, o, amask, n_acc, n_rb, n_ro);
+            cl_moves_fast<P, NS>(p, h, n, pre, o, amask, n_acc, n_rb, n_ro);
             if (amask != 0u) sts_half(me.s0, ly * g.stride + lx, o);       // write back (Alg. 2 line 34, L234)
           }
         } else {
@@ -303,7 +339,9 @@ k_cluster_sweeps(const __grid_constant__ Params p, const unsigned long long t_en
           if (n > 0u) atomicAdd(&ctl->digest, mix64(mix64(t) ^ (((unsigned long long)cell << 32) | amask)));
         }
       }
+      MPMC_CL_CLOCK_ADD(ck_sub);
       cluster.sync();
+      MPMC_CL_CLOCK_ADD(ck_bar);
     }
 
     // ---- cell shift (Alg. 1 lines 15-17; Algorithm 4, pull form): new cell = stayers of the old own cell, then the disks
@@ -316,32 +354,48 @@ k_cluster_sweeps(const __grid_constant__ Params p, const unsigned long long t_en
     const P back = positive ? w : -w;             // entrant translation (L332)
     const int dox = along_x ? (positive ? 1 : -1) : 0, doy = along_x ? 0 : (positive ? 1 : -1);
     const ClTile<P> to = cl_tile<P>(cl_smem, cap, b ^ 1u);
-    for (uint32_t idx = tid; idx < ncell; idx += T) {
-      const uint32_t ly = small_div(idx, inv_w), lx = idx - ly * g.wme, li = ly * g.stride + lx;
-      uint32_t which, ni;
-      cl_neighbour(g, lx, ly, dox, doy, which, ni);
-      const ClTile<P> nt = cl_tile<P>(s_base[which], cap, b);
-      const uint32_t c_own = me.cnt[li], c_nb = nt.cnt[ni];
-      const Half<P> a0 = lds_half(me.s0, li), b0 = lds_half(nt.s0, ni);
-      const uint2 ia = me.i01[li], ib = nt.i01[ni];
+    // two cells per thread and round (tiles of more cells than threads): the loads of both are in flight together
+    struct ShiftIn { Half<P> a0, b0; uint2 ia, ib; uint32_t c_own, c_nb, li, ni, which; };
+    auto shift_load = [&](const uint32_t idx) {
+      ShiftIn in;
+      const uint32_t ly = small_div(idx, inv_w), lx = idx - ly * g.wme;
+      in.li = ly * g.stride + lx;
+      cl_neighbour(g, lx, ly, dox, doy, in.which, in.ni);
+      const ClTile<P> nt = cl_tile<P>(s_base[in.which], cap, b);
+      in.c_own = me.cnt[in.li]; in.c_nb = nt.cnt[in.ni];
+      in.a0 = lds_half(me.s0, in.li); in.b0 = lds_half(nt.s0, in.ni);
+      in.ia = me.i01[in.li]; in.ib = nt.i01[in.ni];
+      return in;
+    };
+    auto shift_store = [&](const ShiftIn& in) {
       Half<P> o0, o1; uint2 j01, j23;
       uint32_t nn;
-      if (c_own <= 2u && c_nb <= 2u) {
+      if (in.c_own <= 2u && in.c_nb <= 2u) {
         ShiftRest<P> rest;
-        nn = along_x ? shift_pair<P, true>(a0, b0, ia, ib, step, back, w, o0, j01, rest)
-                     : shift_pair<P, false>(a0, b0, ia, ib, step, back, w, o0, j01, rest);
+        nn = along_x ? shift_pair<P, true>(in.a0, in.b0, in.ia, in.ib, step, back, w, o0, j01, rest)
+                     : shift_pair<P, false>(in.a0, in.b0, in.ia, in.ib, step, back, w, o0, j01, rest);
         o1.x = R::pair(FAR, FAR); o1.y = o1.x; j23 = none;
         if (nn > 2u) shift_pair_rest<P>(rest, o1, j23);
       } else {
-        nn = shift_eight<P>(a0, lds_half(me.s1, li), b0, lds_half(nt.s1, ni), ia, me.i23[li], ib, nt.i23[ni], along_x, step, back,
-                            w, o0, o1, j01, j23);
+        const ClTile<P> nt = cl_tile<P>(s_base[in.which], cap, b);
+        nn = shift_eight<P>(in.a0, lds_half(me.s1, in.li), in.b0, lds_half(nt.s1, in.ni), in.ia, me.i23[in.li], in.ib,
+                            nt.i23[in.ni], along_x, step, back, w, o0, o1, j01, j23);
         if (nn > (uint32_t)NMAX) { atomicOr(&ctl->err, ERRBIT_OVERFLOW); nn = NMAX; }
       }
-      sts_half(to.s0, li, o0); sts_half(to.s1, li, o1);
-      to.i01[li] = j01; to.i23[li] = j23; to.cnt[li] = (uint8_t)nn;     // L280, L342
+      sts_half(to.s0, in.li, o0); sts_half(to.s1, in.li, o1);
+      to.i01[in.li] = j01; to.i23[in.li] = j23; to.cnt[in.li] = (uint8_t)nn;     // L280, L342
+    };
+    for (uint32_t idx = tid; idx < ncell; idx += 2u * T) {
+      const bool second = idx + T < ncell;
+      const ShiftIn in0 = shift_load(idx);
+      ShiftIn in1 = in0;
+      if (second) in1 = shift_load(idx + T);
+      shift_store(in0);
+      if (second) shift_store(in1);
     }
     b ^= 1u;
-    cluster.sync();
+    MPMC_CL_CLOCK_ADD(ck_shift);
+    cluster.barrier_arrive();
     {                                             // the grid origin follows the shift (X = origin + cell*w + local stays put)
       const double L = along_x ? p.Lx_eff : p.Ly_eff;
       double o = along_x ? org_x : org_y;
@@ -350,8 +404,18 @@ k_cluster_sweeps(const __grid_constant__ Params p, const unsigned long long t_en
       if (o < 0.0) o = __dadd_rn(o, L);
       if (along_x) org_x = o; else org_y = o;
     }
+    if (t + 1ull < t_end) dr = draw_sweep(p, t + 1ull);     // the draws of the next sweep, under the barrier
+    cluster.barrier_wait();
+    MPMC_CL_CLOCK_ADD(ck_bar);
   }
 
+#ifdef MPMC_PHASE_CLOCKS
+  if (tid == 0u && rank < CL_MAX_CTAS) {
+    g_cluster_clocks[rank][0] = t_end - t_start; g_cluster_clocks[rank][1] = (unsigned long long)ck_sub;
+    g_cluster_clocks[rank][2] = (unsigned long long)ck_bar; g_cluster_clocks[rank][3] = (unsigned long long)ck_shift;
+    g_cluster_clocks[rank][4] = (unsigned long long)(clock64() - ck_t0);
+  }
+#endif
   // ---- write the tile back to the global buffer it came from; rank 0 advances the control block ----
   {
     const ClTile<P> me = cl_tile<P>(cl_smem, cap, b);

@@ -18,4 +18,17 @@ const void* MPMC_CAT(pick_cluster_kernel_, MPMC_SUFFIX)(bool debug, bool disc, b
   if (n_s != 4) return nullptr;
   return debug ? pick<true>(disc, fast) : pick<false>(disc, fast);
 }
+
+// -DMPMC_PHASE_CLOCKS: the cycle sums k_cluster_sweeps took in its last launch, copied to the host (ctas x marks values)
+int MPMC_CAT(cluster_clocks_, MPMC_SUFFIX)(unsigned long long* out, uint32_t ctas, void* stream) {
+#ifdef MPMC_PHASE_CLOCKS
+  if (ctas > CL_MAX_CTAS) ctas = CL_MAX_CTAS;
+  if (cudaMemcpyFromSymbolAsync(out, g_cluster_clocks, (size_t)ctas * CL_CLOCK_MARKS * 8, 0, cudaMemcpyDeviceToHost, (cudaStream_t)stream) != cudaSuccess) return -1;
+  if (cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) return -1;
+  return (int)CL_CLOCK_MARKS;
+#else
+  (void)out; (void)ctas; (void)stream;
+  return 0;
+#endif
+}
 }  // namespace mpmc

@@ -24,5 +24,8 @@ const void* pick_tile4_kernel_f64(bool debug, bool disc, uint32_t n_s);
 // w ~ sigma cell update (square proposal only); nullptr unless n_s = 4
 const void* pick_cluster_kernel_f32(bool debug, bool disc, bool fast, uint32_t n_s);
 const void* pick_cluster_kernel_f64(bool debug, bool disc, bool fast, uint32_t n_s);
+// builds with -DMPMC_PHASE_CLOCKS: cycle sums of the last k_cluster_sweeps launch (ctas x marks); marks per CTA, 0, or -1
+int cluster_clocks_f32(unsigned long long* out, uint32_t ctas, void* stream);
+int cluster_clocks_f64(unsigned long long* out, uint32_t ctas, void* stream);
 
 }  // namespace mpmc

@@ -792,6 +792,13 @@ int mpmc_debug_config(const mpmc_ctx* c, uint32_t out[12]) {
 
 int mpmc_debug_phase_clocks(mpmc_ctx* c, uint64_t* out, uint32_t max_tiles, uint32_t* marks) {
   if (!c || !out || !marks) return MPMC_ERR_ARG;
+  if (c->loaded && c->cluster_kernel) {               // the cluster-resident kernel: one row per CTA (cluster.cuh)
+    const uint32_t ctas = c->cl_ctas < max_tiles ? c->cl_ctas : max_tiles;
+    const int m = c->fp32 ? cluster_clocks_f32((unsigned long long*)out, ctas, c->stream) : cluster_clocks_f64((unsigned long long*)out, ctas, c->stream);
+    if (m < 0) return MPMC_ERR_CUDA;
+    *marks = (uint32_t)m;
+    return MPMC_OK;
+  }
   if (!c->loaded || !c->tile_kernel || !c->tile_two_slot) return MPMC_ERR_STATE;
   const uint32_t tiles = c->tile_grid < max_tiles ? c->tile_grid : max_tiles;
   static_assert(sizeof(unsigned long long) == sizeof(uint64_t), "");

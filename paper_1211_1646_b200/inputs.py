@@ -160,3 +160,12 @@ def random_dilute(N: int, L: tuple[float, float], sigma: float, seed: int) -> np
         if ok:
             pts.append((px, py))
     return np.asarray(pts, dtype=np.float64).reshape(N, 2)
+
+# Small systems ("launch overhead" below N ~ 1e5): C3's parameters at N = 32^2 and 64^2, and
+# the paper's regime at N = 64^2 and 128^2 — sizes at which the state lives in one thread-block cluster's shared memory
+# (csrc/cluster.cuh).  bench.py --workload S64 [--no-resident] times both mappings.
+for _n in (32, 64):
+    CONFIGS[f"S{_n}"] = Workload(f"S{_n}", _n, 0.716, 1.0, 0.08, 4, 1000, 1, fp32=True)
+for _n in (64, 128):
+    CONFIGS[f"P{_n}"] = Workload(f"P{_n}", _n, 0.698, 1.0, 0.16, 4, 1000, 1, fp32=True, w_target=1.40, disc=True)
+

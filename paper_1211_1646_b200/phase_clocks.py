@@ -25,6 +25,9 @@ def main():
     ap.add_argument("--dump", default="", help="write the per-tile mean cycles of every phase to this .npy file")
     ap.add_argument("--define", action="append", default=[], help="extra -D for the instrumented build (experiments)")
     ap.add_argument("--burst", type=int, default=10, help="back-to-back sweeps before each read (the last one's marks are read)")
+    ap.add_argument("--resident", action="store_true",
+                    help="small systems: the cluster-resident kernel's cycle sums (sub-sweeps, barriers, shift) instead of the tile kernel's marks")
+    ap.add_argument("--fp32", action="store_true", help="run the workload in fp32 whatever its own precision (with --resident)")
     args = ap.parse_args()
     from . import build
     lib = os.path.join(build.HERE, "libmpmc_b200_phase_clocks.so")
@@ -35,7 +38,28 @@ def main():
     from .binding import Mpmc
     w = I.CONFIGS[args.workload]
     xy, box = I.workload_inputs(w)
-    g = Mpmc(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=w.fp32, w_target=w.w_target, disc=w.disc)
+    if args.resident:
+        g = Mpmc(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=w.fp32 or args.fp32, w_target=w.w_target, disc=w.disc)
+        cfg = g.config()
+        if not cfg["resident_ctas"]:
+            raise SystemExit(f"{w.name} does not run on the cluster-resident kernel (too large, or n_s != 4)")
+        g.load_positions(torch.as_tensor(xy, device="cuda"))
+        g.sweep(args.sweeps)
+        g.sweep(args.sweeps)
+        pc = g.phase_clocks()
+        if pc is None:
+            raise SystemExit("this library was built without -DMPMC_PHASE_CLOCKS")
+        pc = pc.astype(np.float64)
+        per = pc[:, 1:] / pc[:, :1]                  # cycles per sweep
+        print(f"{w.name} ({'fp32' if (w.fp32 or args.fp32) else 'fp64'}): cluster of {cfg['resident_ctas']} CTAs ({cfg['resident_cx']} x "
+              f"{cfg['resident_cy']} tiles of ~{g.M // cfg['resident_ctas']} cells), {cfg['resident_smem']} B shared memory per CTA; one launch "
+              f"of {int(pc[0, 0])} sweeps; SM cycles per sweep, thread 0 of every CTA (mean, max over CTAs):")
+        for i, name in enumerate(["four sub-sweeps", "five cluster barriers (incl. waiting for the slowest CTA)", "shift + set-up",
+                                  "whole sweep"]):
+            print(f"  {name:56s} {per[:, i].mean():9.0f} {per[:, i].max():9.0f}")
+        return
+    g = Mpmc(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=w.fp32, w_target=w.w_target, disc=w.disc,
+             resident=False)                         # the marks are the TILE kernel's: keep small systems on it
     g.load_positions(torch.as_tensor(xy, device="cuda"))
     g.sweep(args.sweeps)
     rows = []

@@ -22,10 +22,10 @@ from paper_1211_1646_b200 import build, inputs as I  # noqa: E402
 from paper_1211_1646_b200.binding import Mpmc  # noqa: E402
 
 
-def run(name, N, box, xy, d, n_s, seed, fp32, sweeps, w_target=0.0, disc=False, want=None):
+def run(name, N, box, xy, d, n_s, seed, fp32, sweeps, w_target=0.0, disc=False, want=None, resident=False):
     for debug in (True, False):
         o = O.Oracle(N, box, 1.0, d, n_s, seed, fp32=fp32, w_target=w_target, disc=disc)
-        g = Mpmc(N, box, 1.0, d, n_s, seed, fp32=fp32, debug=debug, w_target=w_target, disc=disc)
+        g = Mpmc(N, box, 1.0, d, n_s, seed, fp32=fp32, debug=debug, w_target=w_target, disc=disc, resident=resident)
         o.load_positions(xy)
         g.load_positions(torch.as_tensor(xy, device="cuda"))
         o.sweep(sweeps); g.sweep(sweeps)
@@ -40,7 +40,8 @@ def run(name, N, box, xy, d, n_s, seed, fp32, sweeps, w_target=0.0, disc=False, 
             for k, v in want.items():
                 assert cfg[k] == v, (name, k, cfg)
         print(f"{name:28s} debug={int(debug)} fp{'32' if fp32 else '64'} N={N} cells={g.mx}x{g.my} tile_slots={cfg['tile_slots']} "
-              f"tiles={cfg['ntx']}x{cfg['nty']} path={path} max n={int(so['counts'].max())}  ok", flush=True)
+              f"tiles={cfg['ntx']}x{cfg['nty']} resident_ctas={cfg['resident_ctas'] if resident else 0} path={path} "
+              f"max n={int(so['counts'].max())}  ok", flush=True)
         g.close()
 
 
@@ -51,6 +52,7 @@ def main():
     xy, box = I.workload_inputs(w)
     for fp32 in (False, True):
         run("C1", w.N, box, xy, w.d, w.n_s, w.seed, fp32, 6, want={"tile_slots": 2})
+        run("C1, cluster-resident", w.N, box, xy, w.d, w.n_s, w.seed, fp32, 6, resident=True)
     xy, box = I.jittered_lattice(50, 0.7, seed=50)                 # tiles of different sizes
     run("uneven tiling 50^2", 2500, box, xy, 0.15, 4, 50, True, 5, want={"tile_slots": 2})
     xy, box = I.jittered_lattice(50, 0.33, seed=50)                # ... with most cells empty
