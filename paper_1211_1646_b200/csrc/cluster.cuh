@@ -18,10 +18,10 @@
 // needs no barrier inside; the shift reads the old own cell and one old neighbour from one buffer and writes the new cell
 // to the other (two buffers per CTA), so it needs none either.
 //
-// Measured (B200, us per sweep, this kernel / fused tile kernel): N = 1024-4096 fp32 w ~ sigma 6.2-6.3 / 11.7-12.0; C1
-// (N = 4096, fp64) 10.5-11.3 / 15.2; N = 4096 at w = 1.4 sigma with the disc proposal, fp32 15.7 / 19.5.  What a sweep costs
-// here is latency: one warp per scheduler runs a dependent chain of ~700 (fp32) to ~900 (fp64) instructions per sub-sweep
-// at ~0.3 instructions per cycle (C1: 3 650 cycles), five barriers of ~800 cycles, a shift of 2 200.
+// Measured (B200, us per sweep, this kernel / fused tile kernel): N = 1024-4096 fp32 w ~ sigma 4.9-5.2 / 11.7; C1 (N = 4096,
+// fp64) 9.7 / 15.2; N = 4096 at w = 1.4 sigma with the disc proposal, fp32 14.7 / 19.5.  What a sweep costs here is latency:
+// one warp per scheduler runs a dependent chain of ~700 (fp32) to ~900 (fp64) instructions per sub-sweep at ~0.3-0.4
+// instructions per cycle (fp32 1 650 cycles, fp64 3 500), five barriers of ~400 cycles, a shift of 1 900-2 500.
 #pragma once
 #include <cooperative_groups.h>
 #include <cstdio>
@@ -155,6 +155,30 @@ __device__ __forceinline__ void cl_moves_fast(const Params& p, const Half<P> (&h
   o.y = flip ? R::pair(By, Ay) : R::pair(Ay, By);
 }
 
+// The barrier between the phases of a sweep.  What it has to order is SHARED memory only: a CTA's stores into its own tile
+// before the other CTAs' loads from it (and their loads before its next stores).  cluster.sync() is a release at cluster
+// scope, which this GPU implements as MEMBAR.ALL.GPU + ERRBAR (SASS; ~470 cycles per barrier, 18 % of a sweep at N = 4096:
+// ncu).  A tile lives in ONE place, the shared memory of its SM, and remote loads are served there, uncached; so a fence at
+// CTA scope (MEMBAR.ALL.CTA: this thread's stores are performed in that memory) followed by the relaxed arrive puts the
+// stores before every load a CTA issues after its wait, and a thread has consumed its own loads before it arrives.  The
+// PTX memory model asks for cluster scope here; -DMPMC_CLUSTER_SYNC_STRICT builds that version.  (Global memory is not
+// ordered by this barrier: the kernel writes global memory only at its end, and the launch boundary orders that.)
+__device__ __forceinline__ void cl_sync() {
+#ifdef MPMC_CLUSTER_SYNC_STRICT
+  cooperative_groups::this_cluster().sync();
+#else
+  asm volatile("fence.acq_rel.cta;\n\tbarrier.cluster.arrive.relaxed.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+#endif
+}
+__device__ __forceinline__ void cl_sync_arrive() {
+#ifdef MPMC_CLUSTER_SYNC_STRICT
+  cooperative_groups::this_cluster().barrier_arrive();
+#else
+  asm volatile("fence.acq_rel.cta;\n\tbarrier.cluster.arrive.relaxed.aligned;" ::: "memory");
+#endif
+}
+__device__ __forceinline__ void cl_sync_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+
 // A CTA's tile and what it needs to know of its periodic neighbours (balanced split of the mx x my cells, every tile non-empty)
 struct ClGeom { uint32_t wme, hme, wl, hb, stride, cap; };   // own width / height; width of the tile to the left, height of the
                                                              // tile below; row stride and capacity of every CTA's arrays
@@ -272,17 +296,21 @@ k_cluster_sweeps(const __grid_constant__ Params p, const unsigned long long t_en
   Tally tally;
   MPMC_CL_CLOCK_START();
 
-  // The cells of checkerboard set Q in this tile: every second column from ax0, every second row from ay0.
+  // The cells of checkerboard set Q in this tile: every second column from ax0, every second row from ay0.  The four sets'
+  // figures are made once (a division each) and kept in shared memory.
   struct ActiveSet { uint32_t ax0, ay0, nax, na, inv_a; };
-  auto active_set = [&](const uint32_t Q) {
+  __shared__ ActiveSet s_set[4];
+  if (tid < 4u) {
     ActiveSet a;
-    const uint32_t qx = Q & 1u, qy = Q >> 1;
+    const uint32_t qx = tid & 1u, qy = tid >> 1;
     a.ax0 = x0 + ((x0 ^ qx) & 1u); a.ay0 = y0 + ((y0 ^ qy) & 1u);
     a.nax = a.ax0 < x1 ? (x1 - a.ax0 + 1u) >> 1 : 0u;
     const uint32_t nay = a.ay0 < y1 ? (y1 - a.ay0 + 1u) >> 1 : 0u;
     a.na = a.nax * nay; a.inv_a = small_div_magic(a.nax == 0u ? 1u : a.nax);
-    return a;
-  };
+    s_set[tid] = a;
+  }
+  __syncthreads();
+  auto active_set = [&](const uint32_t Q) { return s_set[Q]; };
   auto set_of = [](const Draws& d, const uint32_t k) { return k == 0u ? d.order[0] : k == 1u ? d.order[1] : k == 2u ? d.order[2] : d.order[3]; };
   // (Making a cell's draws while its thread waits at the barrier BEFORE the sub-sweep was tried: the Philox rounds already
   // run under the latency of the sub-sweep's loads, so nothing left the critical path and the barriers grew: C1 +3-7 %.)
@@ -340,7 +368,7 @@ k_cluster_sweeps(const __grid_constant__ Params p, const unsigned long long t_en
         }
       }
       MPMC_CL_CLOCK_ADD(ck_sub);
-      cluster.sync();
+      cl_sync();
       MPMC_CL_CLOCK_ADD(ck_bar);
     }
 
@@ -395,7 +423,7 @@ k_cluster_sweeps(const __grid_constant__ Params p, const unsigned long long t_en
     }
     b ^= 1u;
     MPMC_CL_CLOCK_ADD(ck_shift);
-    cluster.barrier_arrive();
+    cl_sync_arrive();
     {                                             // the grid origin follows the shift (X = origin + cell*w + local stays put)
       const double L = along_x ? p.Lx_eff : p.Ly_eff;
       double o = along_x ? org_x : org_y;
@@ -405,7 +433,7 @@ k_cluster_sweeps(const __grid_constant__ Params p, const unsigned long long t_en
       if (along_x) org_x = o; else org_y = o;
     }
     if (t + 1ull < t_end) dr = draw_sweep(p, t + 1ull);     // the draws of the next sweep, under the barrier
-    cluster.barrier_wait();
+    cl_sync_wait();
     MPMC_CL_CLOCK_ADD(ck_bar);
   }
 
