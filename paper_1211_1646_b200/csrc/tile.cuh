@@ -137,22 +137,21 @@ struct TileBox {
 __device__ __forceinline__ TileBox tile_box(const Params& p, const uint32_t b) {
   TileBox t;                                     // (32-bit products, divisions by the host's magic numbers)
   const uint32_t nA = p.tl_na * p.tl_ntx;
-  uint32_t tx, ntx, h0, h1, x0, x1;
+  uint32_t tx, h0, h1, x0, x1;
   if (b < nA) {
     const uint32_t r = magic_div(b, p.tl_div[0]);
-    tx = b - r * p.tl_ntx; ntx = p.tl_ntx;
+    tx = b - r * p.tl_ntx;
     h0 = magic_div(p.tl_hyA * r, p.tl_div[2]);
     h1 = magic_div(p.tl_hyA * (r + 1u), p.tl_div[2]);
     x0 = magic_div(p.hx * tx, p.tl_div[0]); x1 = magic_div(p.hx * (tx + 1u), p.tl_div[0]);
   } else {
     const uint32_t b2 = b - nA, hyB = p.hy - p.tl_hyA;
     const uint32_t r = magic_div(b2, p.tl_div[1]);
-    tx = b2 - r * (p.tl_ntx + 1u); ntx = p.tl_ntx + 1u;
+    tx = b2 - r * (p.tl_ntx + 1u);
     h0 = p.tl_hyA + magic_div(hyB * r, p.tl_div[3]);
     h1 = p.tl_hyA + magic_div(hyB * (r + 1u), p.tl_div[3]);
     x0 = magic_div(p.hx * tx, p.tl_div[1]); x1 = magic_div(p.hx * (tx + 1u), p.tl_div[1]);
   }
-  (void)ntx;
   t.x0 = 2u * x0; t.TX = 2u * x1 - t.x0;
   t.y0 = 2u * h0; t.TY = 2u * (h1 - h0);
   t.w = t.TX + 2 * HALO; t.h = t.TY + 2 * HALO;
