@@ -207,6 +207,21 @@ def test_resident_ablation_switches(oracle_mod, torch_cuda, pshuf, sshuf, w_targ
     assert_same_state(o, g, True)
 
 
+@pytest.mark.parametrize("name,fp32", [("S64", True), ("C1", False), ("P64", True)])
+def test_resident_long_runs_in_one_launch(oracle_mod, torch_cuda, name, fp32):
+    """2 000 sweeps in ONE launch (10 000 barriers between CTAs that read each other's shared memory): any ordering slip of
+    the kernel's barrier (a CTA-scope fence and a relaxed arrive, cluster.cuh cl_sync) would change the trajectory."""
+    w = I.CONFIGS[name]
+    xy, box = I.workload_inputs(w)
+    o, g = make_pair(oracle_mod, torch_cuda, w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32, xy, debug=False, w_target=w.w_target,
+                     disc=w.disc, resident=True)
+    assert g.config()["resident_ctas"] == 16
+    for k in (2000, 1):
+        o.sweep(k); g.sweep(k)
+        assert_same_state(o, g, fp32)
+    assert g.path_sweeps() == (2001, 0)
+
+
 def test_resident_is_not_used_beyond_its_capacity_or_when_switched_off(oracle_mod, torch_cuda):
     from paper_1211_1646_b200.binding import Mpmc
     w = I.CONFIGS["C2"]                                # 73 080 cells: too many for one cluster
