@@ -90,9 +90,13 @@ int mpmc_geometry(const mpmc_ctx* ctx, uint32_t m[2], double w[2], double L_eff[
  * counters.  Synchronises; returns MPMC_ERR_OVERLAP / MPMC_ERR_CELL_OVERFLOW for bad input. */
 int mpmc_load_positions(mpmc_ctx* ctx, const double* xy);
 
-/* k full sweeps of Algorithm 1 (four sub-sweeps + shift each): one fused tile-kernel launch per sweep where cells
- * hold 0/1/2 disks (w ~ sigma), otherwise one persistent cooperative launch for all k.  Asynchronous.  All random draws, including the per-sweep set order and shift, are made on the device from
- * (seed, sweep index), so there is no host<->device traffic inside the loop. */
+/* k full sweeps of Algorithm 1 (four sub-sweeps + shift each).  How they run is chosen at creation
+ * (mpmc_debug_config tells): a small system (n_s = 4, up to ~1e4 - 2e4 cells) in ONE launch of the cluster-resident kernel for
+ * all k; otherwise one fused tile-kernel launch per sweep (n_s = 4, or n_s = 8 at w ~ sigma with the square proposal),
+ * otherwise one persistent cooperative launch for all k.  Every path gives the same trajectory bit for bit.
+ * Asynchronous.  All random draws are functions of (seed, sweep index, cell): the per-sweep set order and shift are
+ * evaluated on the device, or by the host at launch time and passed as kernel arguments; there is no device->host traffic
+ * inside the loop. */
 int mpmc_sweep(mpmc_ctx* ctx, uint64_t k);
 
 /* Unpack (L154): xy_out = device, N x 2 doubles, written in the original disk order;
