@@ -605,6 +605,25 @@ def test_two_live_contexts_with_different_tilings(oracle_mod, torch_cuda):
     assert gb.path_sweeps() == (9, 0) and gs.path_sweeps() == (9, 0)
 
 
+def test_two_live_resident_contexts_and_a_tiled_one(oracle_mod, torch_cuda):
+    """Two contexts on the SAME instantiation of the cluster-resident kernel with different tile sizes (hence different
+    dynamic shared memory: a property of the kernel function) and one on the tile kernel, sweeps interleaved on their own
+    streams."""
+    a = I.jittered_lattice(96, 0.70, seed=1)
+    b = I.jittered_lattice(32, 0.6, seed=4)
+    c = I.jittered_lattice(64, 0.65, seed=9)
+    oa, ga = make_pair(oracle_mod, torch_cuda, 96 * 96, a[1], 1.0, 0.1, 4, 1, True, a[0], resident=True)
+    ob, gb = make_pair(oracle_mod, torch_cuda, 1024, b[1], 1.0, 0.2, 4, 5, True, b[0], resident=True)
+    oc, gc = make_pair(oracle_mod, torch_cuda, 4096, c[1], 1.0, 0.15, 4, 6, True, c[0], resident=False)
+    assert ga.config()["resident_smem"] > 4 * gb.config()["resident_smem"] > 0 and gc.config()["resident_ctas"] == 0
+    for k in (1, 3, 2):
+        ga.sweep(k); gb.sweep(k); gc.sweep(k); oa.sweep(k); ob.sweep(k); oc.sweep(k)
+        gb.sweep(1); gc.sweep(1); ga.sweep(1); ob.sweep(1); oc.sweep(1); oa.sweep(1)
+    for o, g in ((oa, ga), (ob, gb), (oc, gc)):
+        assert_same_state(o, g, True)
+        assert g.path_sweeps() == (9, 0)
+
+
 def test_debug_shift_rejects_a_shift_of_a_cell_width(oracle_mod, torch_cuda):
     from paper_1211_1646_b200.binding import MpmcError
     xy, box = I.jittered_lattice(32, 0.6, seed=4)
