@@ -134,15 +134,15 @@ __device__ __forceinline__ void cl_moves_fast(const Params& p, const Half<P> (&h
     const P Mx = R::add(Ax, d.ddx[s]), My = R::add(Ay, d.ddy[s]);
     const bool inside = (Mx > (P)0) && (Mx <= wx) && (My > (P)0) && (My <= wy);   // (0, w]  (A3; L79, L118)
     const P Dbx = R::sub(Mx, Bx), Dby = R::sub(My, By);                          // the other own disk
-    P rmin = R::fma(Dbx, Dbx, R::mul(Dby, Dby));
+    OverlapAcc<P> ov(sigma2, R::fma(Dbx, Dbx, R::mul(Dby, Dby)));
     const Pair MMx = R::pair(Mx, Mx), MMy = R::pair(My, My);
 #pragma unroll
     for (int e = 0; e < 8; ++e) {                  // |D_move - (D + s)|^2  (line 19, L204)
       const Pair Dx = R::padd(MMx, nqx[e]), Dy = R::padd(MMy, nqy[e]);
       const Pair r2 = R::pfma(Dx, Dx, R::pmul(Dy, Dy));
-      rmin = R::min3(rmin, r2.x, r2.y);
+      if (e & 1) ov.template pair<1>(r2); else ov.template pair<0>(r2);
     }
-    const bool acc = inside && !(rmin < sigma2);   // strict (A4)
+    const bool acc = inside && !ov.overlap(sigma2);   // strict (A4)
     if (acc) { Ax = Mx; Ay = My; amask |= 1u << s; }
     n_rb += inside ? 0u : 1u;
     n_acc += acc ? 1u : 0u;

@@ -151,6 +151,29 @@ template <> struct Real<double> {
   static __device__ __forceinline__ Pair pfma(Pair a, Pair b, Pair c) { return pair(__fma_rn(a.x, b.x, c.x), __fma_rn(a.y, b.y, c.y)); }
 };
 
+// "Does the trial position overlap one of these disks": min r^2 < sigma^2 over the distances fed in (L194-204, strict: A4).
+// fp32 keeps a running minimum (one 3-input FMNMX per pair of distances).  In fp64 a minimum is DSETP.MIN + two FSEL and the
+// running minimum of 17 values a dependent chain of 16 of them per move (~900 cycles of a 3 500-cycle sub-sweep pass at
+// N = 4096: measured); min r^2 < s is the same verdict as "some r^2 < s" (no NaN occurs: every operand is finite), so fp64
+// compares each distance and ORs the predicates, on two independent accumulators.  Used where a sub-sweep is ONE pass of
+// one warp per scheduler (cluster.cuh: C1 14 020 -> 13 390 cycles); on the tile kernels, whose fp64 sub-sweeps are bound by
+// the DP pipe's throughput rather than by the chain, the running minimum is faster (C2: 18.9 against 20.0 us per sweep).
+template <typename P> struct OverlapAcc;
+template <> struct OverlapAcc<float> {
+  float rmin;
+  __device__ __forceinline__ OverlapAcc(float, float first) : rmin(first) {}      // first = the first distance
+  template <int E> __device__ __forceinline__ void pair(float2 r2) { rmin = fminf(fminf(rmin, r2.x), r2.y); }
+  __device__ __forceinline__ bool overlap(float sigma2) const { return rmin < sigma2; }
+};
+template <> struct OverlapAcc<double> {
+  double s2; bool a, b;
+  __device__ __forceinline__ OverlapAcc(double sigma2, double first) : s2(sigma2), a(first < sigma2), b(false) {}
+  template <int E> __device__ __forceinline__ void pair(Real<double>::Pair r2) {      // E: which accumulator (parity)
+    if (E & 1) b |= (r2.x < s2) | (r2.y < s2); else a |= (r2.x < s2) | (r2.y < s2);
+  }
+  __device__ __forceinline__ bool overlap(double) const { return a | b; }
+};
+
 // Philox4x32-10 (Salmon et al., SC'11).  Ten rounds of two 32x32->64 multiplies and xors; the key schedule
 // adds the Weyl constants.  counter = (c0..c3), key = (k0, k1).
 __host__ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
