@@ -337,6 +337,24 @@ def test_c3_headline_config_bench_launch_configuration(oracle_mod, torch_cuda):
         assert np.array_equal(o.contact_histogram(dr, nbins), g.contact_histogram(dr, nbins))
 
 
+def test_c3_the_config_s_1000_sweeps(oracle_mod, torch_cuda):
+    """C3 as BASELINE.json states it — N = 2^20, 1 000 sweeps — on the kernels bench.py times, against the oracle's strip
+    program (oracle/strip_omp.cpp: the same Algorithms 2 and 4 on all host cores, identical to the single-thread oracle bit
+    for bit: tests/test_strip_baseline.py), which makes 4e9 trial moves affordable."""
+    w = I.CONFIGS["C3"]
+    xy, box = I.workload_inputs(w)
+    from paper_1211_1646_b200.binding import Mpmc
+    o = oracle_mod.StripBaseline(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=True)
+    g = Mpmc(w.N, box, w.sigma, w.d, w.n_s, w.seed, fp32=True)
+    o.load_positions(xy)
+    g.load_positions(torch_cuda.as_tensor(xy, device="cuda"))
+    g.sweep(w.sweeps)
+    o.sweep(w.sweeps)
+    st = assert_same_state(o, g, True, check_mask=False)
+    assert st["sweep"] == 1000 and st["counts"].sum() == w.N
+    assert g.path_sweeps() == (1000, 0) and g.acceptance()[0] > 3.9e9      # ~4e9 trial moves, all compared through the counters
+
+
 def test_c3_debug_digest(oracle_mod, torch_cuda):
     w = I.CONFIGS["C3"]
     xy, box = I.workload_inputs(w)
