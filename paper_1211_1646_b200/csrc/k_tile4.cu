@@ -7,9 +7,17 @@
 #define MPMC_CAT(a, b) MPMC_CAT2(a, b)
 
 namespace mpmc {
-const void* MPMC_CAT(pick_tile4_kernel_, MPMC_SUFFIX)(bool debug, bool disc, uint32_t n_s) {
+namespace {
+template <bool DEBUG, bool WIDE>
+const void* pick(bool disc) {
+  return disc ? (const void*)k_tile4_sweep<MPMC_P, 4, DEBUG, true, WIDE> : (const void*)k_tile4_sweep<MPMC_P, 4, DEBUG, false, WIDE>;
+}
+}  // namespace
+const void* MPMC_CAT(pick_tile4_kernel_, MPMC_SUFFIX)(bool debug, bool disc, bool wide, uint32_t n_s) {
   if (n_s != 4) return nullptr;
-  if (debug) return disc ? (const void*)k_tile4_sweep<MPMC_P, 4, true, true> : (const void*)k_tile4_sweep<MPMC_P, 4, true, false>;
-  return disc ? (const void*)k_tile4_sweep<MPMC_P, 4, false, true> : (const void*)k_tile4_sweep<MPMC_P, 4, false, false>;
+  if constexpr (sizeof(MPMC_P) == 4) {         // (fp64 has one thread count: no second instantiation)
+    if (wide) return debug ? pick<true, true>(disc) : pick<false, true>(disc);
+  }
+  return debug ? pick<true, false>(disc) : pick<false, false>(disc);
 }
 }  // namespace mpmc

@@ -16,9 +16,9 @@ const void* pick_tile_kernel_f64(bool debug, uint32_t n_s, bool compact);
 // the host (tiles x marks values); returns the number of marks per tile, 0 in an ordinary build, -1 on a CUDA error
 int phase_clocks_f32(unsigned long long* out, uint32_t tiles, void* stream);
 int phase_clocks_f64(unsigned long long* out, uint32_t tiles, void* stream);
-// k_tile4_sweep<P, 4, DEBUG, DISC> (tile4.cuh); nullptr unless n_s = 4
-const void* pick_tile4_kernel_f32(bool debug, bool disc, uint32_t n_s);
-const void* pick_tile4_kernel_f64(bool debug, bool disc, uint32_t n_s);
+// k_tile4_sweep<P, 4, DEBUG, DISC, WIDE> (tile4.cuh); wide = the 512-thread instantiation (fp32 only); nullptr unless n_s = 4
+const void* pick_tile4_kernel_f32(bool debug, bool disc, bool wide, uint32_t n_s);
+const void* pick_tile4_kernel_f64(bool debug, bool disc, bool wide, uint32_t n_s);
 
 // k_cluster_sweeps<P, 4, DEBUG, DISC, FAST> (cluster.cuh): the whole state resident in one cluster's shared memory; fast = the
 // w ~ sigma cell update (square proposal only); nullptr unless n_s = 4

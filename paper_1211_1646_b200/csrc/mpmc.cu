@@ -430,7 +430,7 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
     const bool sorted = two_slot && compact && attempt == 0;
     if (attempt == 1 && !(two_slot && compact)) break;
     const void* tk = two_slot ? (fp32 ? pick_tile_kernel_f32(debug, n_s, sorted) : pick_tile_kernel_f64(debug, n_s, sorted))
-                              : (fp32 ? pick_tile4_kernel_f32(debug, disc, n_s) : pick_tile4_kernel_f64(debug, disc, n_s));
+                              : (fp32 ? pick_tile4_kernel_f32(debug, disc, false, n_s) : pick_tile4_kernel_f64(debug, disc, false, n_s));
     if (!tk) break;
     int smem_optin = 0;
     cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
@@ -442,7 +442,7 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
     Tiling tl = {};
     const size_t row_bytes = sorted ? SORT_ROW_BYTES : 0;
     c->tile_threads = two_slot ? (fp32 ? TileThreads<float>::value : TileThreads<double>::value)
-                               : (fp32 ? Tile4Threads<float>::value : Tile4Threads<double>::value);
+                               : (fp32 ? Tile4Threads<float, false>::value : Tile4Threads<double, false>::value);
     bool have = choose_tiling(p.hx, p.hy, cell_bytes, smem_max, (uint32_t)sms, &tl, row_bytes, sorted ? 64u : 0xFFFFFFFFu);
     // the sort is a fixed cost of ~8 000 cycles per tile and sweep (measured, phase_clocks.py): it pays from about a
     // thousand cells per colour plane on; smaller tiles (systems below ~2e5 cells) keep the plain variant
@@ -456,6 +456,10 @@ int mpmc_create_ex(mpmc_ctx** out, uint64_t N, const double box[2], double sigma
       }
     }
 #endif
+    if (have && !two_slot && fp32 && tl.PS >= TILE4_WIDE_MIN_PLANE) {      // large tiles: the 512-thread instantiation (tile4.cuh)
+      tk = pick_tile4_kernel_f32(debug, disc, true, n_s);
+      c->tile_threads = Tile4Threads<float, true>::value;
+    }
     if (have) {
       c->tile_kernel = tk;
       c->tile_grid = tl.tiles;

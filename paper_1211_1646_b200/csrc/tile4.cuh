@@ -13,8 +13,14 @@
 
 namespace mpmc {
 
-// threads per CTA, one CTA per SM: 12 warps at <= 170 registers (fp32), 8 warps at <= 255 registers (fp64)
-template <typename P> struct Tile4Threads { static constexpr int value = sizeof(P) == 4 ? 384 : 256; };
+// Threads per CTA, one CTA per SM.  fp32: the update needs ~150 registers; 12 warps at <= 170 leave three warps per
+// scheduler to hide a long dependent chain behind (ncu at P1536: issue slots 43 % busy, wait 22 %, long_scoreboard 16 %), 16
+// warps at <= 128 registers spill 4 bytes and run P1536 / P3072 12-13 % faster (measured; 20 warps at 96 registers spill 700
+// bytes and lose) — so tiles with more cells of a set than 384 take the WIDE instantiation, small tiles (one pass either
+// way: latency, where the tighter register budget costs 3 %) the narrow one.  fp64: 8 warps at <= 255 registers (12 at 168
+// spill 836 bytes).
+template <typename P, bool WIDE> struct Tile4Threads { static constexpr int value = sizeof(P) == 4 ? (WIDE ? 512 : 384) : 256; };
+constexpr uint32_t TILE4_WIDE_MIN_PLANE = 385;   // cells per colour plane of a tile region from which the wide instantiation is used
 
 // The cells of sub-sweep k: local colour QL at ring >= k, in chunks of 32 drawn from a shared counter.
 template <typename P, int NS, bool DEBUG, bool DISC, uint32_t QL>
@@ -71,8 +77,8 @@ __device__ __forceinline__ void tile4_sub_sweep_cells(const Params& p, SmemCell<
 // ---------------------------------------------------------------------------------------------------------
 // The fused sweep kernel, four slots per cell.  Dynamic shared memory: 2 slot pairs x 4 planes x tl_PS cells.
 // ---------------------------------------------------------------------------------------------------------
-template <typename P, int NS, bool DEBUG, bool DISC>
-__global__ void __launch_bounds__(Tile4Threads<P>::value, 1)
+template <typename P, int NS, bool DEBUG, bool DISC, bool WIDE = false>
+__global__ void __launch_bounds__(Tile4Threads<P, WIDE>::value, 1)
 k_tile4_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   using R = Real<P>;
   extern __shared__ __align__(16) unsigned char tile_smem[];
