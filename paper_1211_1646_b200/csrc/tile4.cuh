@@ -79,33 +79,60 @@ __device__ __forceinline__ void tile4_sub_sweep_cells(const Params& p, SmemCell<
 // ---------------------------------------------------------------------------------------------------------
 template <typename P, int NS, bool DEBUG, bool DISC, bool WIDE = false>
 __global__ void __launch_bounds__(Tile4Threads<P, WIDE>::value, 1)
-k_tile4_sweep(const __grid_constant__ Params p, const unsigned long long t) {
+k_tile4_sweep(const __grid_constant__ Params p, const unsigned long long t, const Draws dr_host, const uint32_t cur) {
   using R = Real<P>;
   extern __shared__ __align__(16) unsigned char tile_smem[];
   const uint32_t PS = p.tl_PS;
   SmemCell<P>* sm0 = reinterpret_cast<SmemCell<P>*>(tile_smem);     // slot pair 0 of the four local colour planes
   SmemCell<P>* sm1 = sm0 + 4u * PS;                                 // slot pair 1
-  __shared__ uint32_t s_last;
   __shared__ uint32_t s_next[8];                 // chunk counters: sub-sweeps 1-4, shift planes 0-3
   Ctl* ctl = p.ctl;
-  // The sweep index comes as a kernel argument (the host counts launches), so the draws of this sweep — a pure function
-  // of (seed, t), Alg. 1 lines 2, 15, 16 (L64, L90-91) — and all they decide are warp-uniform values computed before the
-  // wait.  Launched with programmatic stream serialisation (mpmc.cu): everything below the wait reads what the previous
-  // sweep wrote.  If the state is not at sweep t (an earlier launch left its sweep to the general kernel), return.
-  const Draws dr = draw_sweep(p, t);
-  asm volatile("griddepcontrol.wait;" ::: "memory");
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  if (ctl->t != t) return;
-  const uint32_t cur = ctl->cur, nxt = cur ^ 1u;
+  // The sweep index comes as a kernel argument (the host counts launches), and with it the draws of this sweep — a pure
+  // function of (seed, t), Alg. 1 lines 2, 15, 16 (L64, L90-91), evaluated by the host with the same draw_sweep — and the
+  // buffer that holds the sweep's state (every sweep flips it): uniform values, so the tile's geometry and the counters are
+  // set up before the wait.  Launched with programmatic stream serialisation (mpmc.cu): everything below the wait reads
+  // what the previous sweep wrote.
+  Draws dr;                                      // (a copy in registers: a parameter whose address is taken lives in local memory)
+  dr.order[0] = dr_host.order[0]; dr.order[1] = dr_host.order[1]; dr.order[2] = dr_host.order[2]; dr.order[3] = dr_host.order[3];
+  dr.dir = dr_host.dir; dr.dist_word = dr_host.dist_word;
+  const uint32_t nxt = cur ^ 1u;
   const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, NW = blockDim.x >> 5;
   const TileBox tb = tile_box(p, blockIdx.x);
   const uint32_t pw = tb.pw, ph = tb.ph, Mqp = p.Mqp;
   const int gx0 = (int)tb.x0 - HALO, gy0 = (int)tb.y0 - HALO;       // global cell of the region's corner (unwrapped)
   const P FAR = R::far_away(), HALF_FAR = FAR * (P)0.5;
+  const uint32_t dir = dr.dir;
+  const bool along_x = dir < 2u, positive = (dir & 1u) == 0u;
+  const P w = along_x ? R::wx(p) : R::wy(p);
+  const P delta = R::mul(R::mul((P)0.5, w), R::unit(dr.dist_word));   // line 15 (L90)
   if (tid == 0) {
     for (int i = 0; i < 8; ++i) s_next[i] = 0u;
   }
   __syncthreads();
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  // the head of the control block, one trip to L2: a launch whose sweep index is not the state's returns (nothing has been
+  // written); the state's buffer is the one the host named (anything else cannot happen and is reported)
+  {
+    const CtlHeader ch = ctl_header(ctl, (uint32_t)(t & 3u));
+    if (ch.t == t && ch.cur != cur && tid == 0) atomicOr(&ctl->err, ERRBIT_STATE);
+    if (ch.t != t || ch.cur != cur) return;
+  }
+  // Every CTA takes a ticket once it has read the control block; the one that draws the last ticket knows that all have,
+  // and advances the block right away — nothing below reads it, and the next launch waits for this one to complete — so no
+  // CTA waits for a counter at its end.
+  if (tid == 0 && atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1u) {
+    const double L = along_x ? p.Lx_eff : p.Ly_eff;
+    double o = ctl->origin[along_x ? 0 : 1];     // the grid origin follows the shift
+    o = __dadd_rn(o, positive ? (double)delta : -(double)delta);
+    if (o >= L) o = __dsub_rn(o, L);
+    if (o < 0.0) o = __dadd_rn(o, L);
+    ctl->origin[along_x ? 0 : 1] = o;
+    ctl->ticket = 0u;
+    ctl->cur = nxt;
+    ctl->t = t + 1ull;
+    ctl->path_sweeps[0] += 1ull;
+  }
 
   // ---- load the tile and its halo: warps take plane rows, lanes run along the row; slot pair 1 only where n > 2 ----
   {
@@ -157,10 +184,6 @@ k_tile4_sweep(const __grid_constant__ Params p, const unsigned long long t) {
   }
 
   // ---- cell shift (Alg. 1 lines 15-17; Algorithm 4) of the interior cells, shared memory -> other buffer ----
-  const uint32_t dir = dr.dir;
-  const bool along_x = dir < 2u, positive = (dir & 1u) == 0u;
-  const P w = along_x ? R::wx(p) : R::wy(p);
-  const P delta = R::mul(R::mul((P)0.5, w), R::unit(dr.dist_word));   // line 15 (L90)
   {
     const P step = positive ? -delta : delta;     // l' = l - f*delta   (L303)
     const P back = positive ? w : -w;             // entrant translation (L332)
@@ -207,26 +230,7 @@ k_tile4_sweep(const __grid_constant__ Params p, const unsigned long long t) {
     }
   }
 
-  // ---- counters; the last CTA to finish advances the control block ----
-  flush_tally(p, tally);
-  __syncthreads();
-  if (tid == 0) {
-    __threadfence();
-    s_last = (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1u) ? 1u : 0u;
-  }
-  __syncthreads();
-  if (s_last && tid == 0) {
-    const double L = along_x ? p.Lx_eff : p.Ly_eff;
-    double o = ctl->origin[along_x ? 0 : 1];     // the grid origin follows the shift
-    o = __dadd_rn(o, positive ? (double)delta : -(double)delta);
-    if (o >= L) o = __dsub_rn(o, L);
-    if (o < 0.0) o = __dadd_rn(o, L);
-    ctl->origin[along_x ? 0 : 1] = o;
-    ctl->ticket = 0u;
-    ctl->cur = nxt;
-    ctl->t = t + 1ull;
-    ctl->path_sweeps[0] += 1ull;
-  }
+  flush_tally(p, tally);                         // counters
 }
 
 }  // namespace mpmc
