@@ -23,12 +23,12 @@ template <typename P, bool WIDE> struct Tile4Threads { static constexpr int valu
 constexpr uint32_t TILE4_WIDE_MIN_PLANE = 385;   // cells per colour plane of a tile region from which the wide instantiation is used
 
 // The cells of sub-sweep k: local colour QL at ring >= k, in chunks of 32 drawn from a shared counter.
-template <typename P, int NS, bool DEBUG, bool DISC, uint32_t QL>
+template <typename P, int NS, bool DEBUG, bool DISC>
 __device__ __forceinline__ void tile4_sub_sweep_cells(const Params& p, SmemCell<P>* sm0, SmemCell<P>* sm1, const TileBox& tb,
-                                                      const uint32_t k, const uint32_t dir, const int gx0, const int gy0,
-                                                      const unsigned long long t, uint32_t* next, Tally& tally) {
+                                                      const uint32_t QL, const uint32_t k, const uint32_t dir, const int gx0,
+                                                      const int gy0, const unsigned long long t, uint32_t* next, Tally& tally) {
   using R = Real<P>;
-  constexpr uint32_t qx = QL & 1u, qy = QL >> 1;
+  const uint32_t qx = QL & 1u, qy = QL >> 1;
   const uint32_t PS = p.tl_PS, pw = tb.pw;
   const SubRect rc = sub_sweep_rect(tb, k, dir);
   const uint32_t px0 = (rc.x_lo - qx + 1u) >> 1, px1 = (rc.x_hi - qx) >> 1;
@@ -38,6 +38,9 @@ __device__ __forceinline__ void tile4_sub_sweep_cells(const Params& p, SmemCell<
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
   const P HALF_FAR = R::far_away() * (P)0.5;
+  int noff[9];                                   // the 3 x 3 cells relative to a cell of this colour (uniform)
+#pragma unroll
+  for (int j = 0; j < 9; ++j) noff[j] = neighbour_offset(QL, j % 3 - 1, j / 3 - 1, PS, pw);
   for (;;) {
     uint32_t base = 0;
     if (lane == 0u) base = atomicAdd(next, 32u);
@@ -53,9 +56,8 @@ __device__ __forceinline__ void tile4_sub_sweep_cells(const Params& p, SmemCell<
     Half<P> h0[9], h1[9];
 #pragma unroll
     for (int j = 0; j < 9; ++j) {
-      const int off = neighbour_offset(QL, j % 3 - 1, j / 3 - 1, PS, pw);
-      h0[j] = lds_half(sm0 + si + off, 0u);
-      h1[j] = lds_half(sm1 + si + off, 0u);
+      h0[j] = lds_half(sm0 + si + noff[j], 0u);
+      h1[j] = lds_half(sm1 + si + noff[j], 0u);
     }
     // slots fill in order, so the count is the number of occupied slots
     const uint32_t n = h0[4].x.x < HALF_FAR ? (h0[4].x.y < HALF_FAR ? (h1[4].x.x < HALF_FAR ? (h1[4].x.y < HALF_FAR ? 4u : 3u) : 2u) : 1u) : 0u;
@@ -174,12 +176,9 @@ k_tile4_sweep(const __grid_constant__ Params p, const unsigned long long t, cons
 #pragma unroll 1
   for (uint32_t k = 1; k <= 4u; ++k) {
     const uint32_t Qg = k == 1u ? dr.order[0] : k == 2u ? dr.order[1] : k == 3u ? dr.order[2] : dr.order[3];
-    switch (Qg ^ 3u) {                           // the region starts at an odd cell (x0 - 5, y0 - 5): colours flip
-      case 0: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 0>(p, sm0, sm1, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
-      case 1: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 1>(p, sm0, sm1, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
-      case 2: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 2>(p, sm0, sm1, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
-      default: tile4_sub_sweep_cells<P, NS, DEBUG, DISC, 3>(p, sm0, sm1, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
-    }
+    // the region starts at an odd cell (x0 - 5, y0 - 5): colours flip.  ONE copy of the update for the four colours (the
+    // local colour is a run-time value): a quarter of the code for the instruction cache
+    tile4_sub_sweep_cells<P, NS, DEBUG, DISC>(p, sm0, sm1, tb, Qg ^ 3u, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally);
     __syncthreads();
   }
 
