@@ -19,7 +19,7 @@
 // to the other (two buffers per CTA), so it needs none either.
 //
 // Measured (B200, us per sweep, this kernel / fused tile kernel): N = 1024-4096 fp32 w ~ sigma 4.9-5.2 / 11.7; C1 (N = 4096,
-// fp64) 9.5 / 15.2; N = 4096 at w = 1.4 sigma with the disc proposal, fp32 14.7 / 19.5.  What a sweep costs here is latency:
+// fp64) 9.5 / 15.2; N = 4096 at w = 1.4 sigma with the disc proposal, fp32 13.1 / 16.1.  What a sweep costs here is latency:
 // one warp per scheduler runs a dependent chain of ~700 (fp32) to ~900 (fp64) instructions per sub-sweep at ~0.3-0.4
 // instructions per cycle (fp32 1 650 cycles, fp64 3 500), five barriers of ~400 cycles, a shift of 1 900-2 500.
 #pragma once
