@@ -301,96 +301,12 @@ __device__ __noinline__ void tile_update_cell_warp(const Params& p, SmemCell<P>*
 
 // ---------------------------------------------------------------------------------------------------------
 // One cell update (Algorithm 2) on the tile in shared memory: the arithmetic of update_cell_fast
-// (sweep.cuh), the 3x3 cells read with one LDS.128 each at si_own + noff[idx] (offsets uniform per phase).
+// (sweep.cuh), the 3x3 cells read with one LDS.128 each at si_own + noff[idx].  The local colour is a run-time value
+// (the nine offsets are computed once per sub-sweep and are uniform): one copy serves the four sub-sweeps of both
+// variants of the kernel.
 // ---------------------------------------------------------------------------------------------------------
-template <typename P, int NS, bool DEBUG, uint32_t QL>
-__device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* sm, const uint32_t si_own,
-                                                 const uint32_t pw, const uint32_t cell, const bool interior,
-                                                 const unsigned long long t, Tally& tally) {
-  using R = Real<P>;
-  using Pair = typename R::Pair;
-  Half<P> h[9];
-  const SmemCell<P>* own = sm + si_own;            // QL, tl_PS and pw are uniform: the nine offsets cost nothing per cell
-#pragma unroll
-  for (int idx = 0; idx < 9; ++idx) h[idx] = lds_half(own + neighbour_offset(QL, idx % 3 - 1, idx / 3 - 1, p.tl_PS, pw), 0u);
-  // ---- displacements of all NS moves from the GLOBAL cell id (line 12, L190; A2, A9) ----
-  const uint32_t t_lo = (uint32_t)t, t_hi = (uint32_t)(t >> 32);
-  P ddx[NS], ddy[NS];
-#pragma unroll
-  for (int b = 0; b < NS / 2; ++b) {
-    uint32_t Rw[4];
-    philox4x32_10_rk(p, cell, t_lo, t_hi, (uint32_t)b, Rw);
-    ddx[2 * b] = R::scaled_sym(p, Rw[0]); ddy[2 * b] = R::scaled_sym(p, Rw[1]);
-    ddx[2 * b + 1] = R::scaled_sym(p, Rw[2]); ddy[2 * b + 1] = R::scaled_sym(p, Rw[3]);
-  }
-  const P wx = R::wx(p), wy = R::wy(p), sigma2 = R::sigma2(p);
-  const P HALF_FAR = R::far_away() * (P)0.5;
-  const Pair MINUS1 = R::pair((P)-1, (P)-1);
-  // ---- neighbours, translated into this cell's frame and negated: -(l_j + s) = fma(l_j, -1, -s) ----
-  Pair nqx[8], nqy[8];
-#pragma unroll
-  for (int idx = 0; idx < 9; ++idx) {
-    if (idx == 4) continue;
-    const int e = idx < 4 ? idx : idx - 1;
-    const int ox = idx % 3 - 1, oy = idx / 3 - 1;
-    const P nsx = ox < 0 ? wx : ox > 0 ? -wx : (P)0;
-    const P nsy = oy < 0 ? wy : oy > 0 ? -wy : (P)0;
-    nqx[e] = R::pfma(h[idx].x, MINUS1, R::pair(nsx, nsx));
-    nqy[e] = R::pfma(h[idx].y, MINUS1, R::pair(nsy, nsy));
-  }
-  // ---- own cell in visiting order (Alg. 2 lines 8-9, L186-187); a slot is empty iff it holds the sentinel ----
-  P Ax = h[4].x.x, Ay = h[4].y.x, Bx = h[4].x.y, By = h[4].y.y;
-  const uint32_t n = Bx < HALF_FAR ? 2u : (Ax < HALF_FAR ? 1u : 0u);
-  const bool two = n == 2u;
-  bool flip = false;                   // true: A is slot 1
-  if (two) {                           // n = 2: Fisher-Yates is one draw, j = bounded(S0, 2); j = 0 swaps
-    uint32_t S[4];
-    philox4x32_10_rk(p, cell, t_lo, t_hi, SLOT_SHUFFLE, S);
-    flip = bounded(S[0], 2u) == 0u && !(p.flags & FLAG_NO_PARTICLE_SHUFFLE);
-  }
-  if (flip) { P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }
-  uint32_t amask = 0, bmask = 0;       // bit s: move s accepted / left the cell
-#pragma unroll
-  for (int s = 0; s < NS; ++s) {       // Alg. 2 lines 11-32 (L189-230)
-    const P Mx = R::add(Ax, ddx[s]), My = R::add(Ay, ddy[s]);              // D_move = l + displacement
-    const bool inside = (Mx > (P)0) && (Mx <= wx) && (My > (P)0) && (My <= wy);   // (0, w]  (A3; L79, L118)
-    const P Dbx = R::sub(Mx, Bx), Dby = R::sub(My, By);                    // the other own disk (s = 0)
-    P rmin = R::fma(Dbx, Dbx, R::mul(Dby, Dby));
-    const Pair MMx = R::pair(Mx, Mx), MMy = R::pair(My, My);
-#pragma unroll
-    for (int e = 0; e < 8; ++e) {                                          // |D_move - (D + s)|^2  (line 19, L204)
-      const Pair Dx = R::padd(MMx, nqx[e]), Dy = R::padd(MMy, nqy[e]);
-      const Pair r2 = R::pfma(Dx, Dx, R::pmul(Dy, Dy));
-      rmin = R::min3(rmin, r2.x, r2.y);
-    }
-    const bool acc = inside && !(rmin < sigma2);                           // strict (A4)
-    if (acc) { Ax = Mx; Ay = My; amask |= 1u << s; }                       // lines 24-27 (L215-222)
-    if (!inside) bmask |= 1u << s;                                         // leaves the cell: rejected (L79, L118)
-    if (two) { const P tx = Ax, ty = Ay; Ax = Bx; Ay = By; Bx = tx; By = ty; }   // s mod n cycling (L75)
-  }
-  if (n == 0u) amask = 0u;             // empty cells attempt nothing (A10)
-  const uint32_t n_acc = __popc(amask), n_rb = __popc(bmask);
-  if (amask != 0u) {                   // write back (line 34, L234): the slot pair in slot order
-    if (two && (NS & 1)) flip = !flip;
-    Half<P> o;
-    o.x = flip ? R::pair(Bx, Ax) : R::pair(Ax, Bx);
-    o.y = flip ? R::pair(By, Ay) : R::pair(Ay, By);
-    sts_half(sm, si_own, o);
-  }
-  // tallies, accept masks and the digest count every cell once: in the tile that owns it
-  if (interior && n > 0u) {
-    tally.acc += n_acc; tally.rb += n_rb; tally.ro += (uint32_t)NS - n_acc - n_rb;
-  }
-  if (DEBUG && interior) {
-    p.mask[cell] = amask;
-    if (n > 0u) atomicAdd(&p.ctl->digest, mix64(mix64(t) ^ (((unsigned long long)cell << 32) | amask)));
-  }
-}
-
-// The same with the local colour as a run-time value (the nine offsets computed once per sub-sweep): one copy serves the
-// four sub-sweeps of the SORTED variant.
 template <typename P, int NS, bool DEBUG>
-__device__ __forceinline__ void tile_update_cell_rt(const Params& p, SmemCell<P>* sm, const uint32_t si_own,
+__device__ __forceinline__ void tile_update_cell(const Params& p, SmemCell<P>* sm, const uint32_t si_own,
                                                     const int (&noff)[9], const uint32_t cell, const bool interior,
                                                  const unsigned long long t, Tally& tally) {
   using R = Real<P>;
@@ -512,13 +428,19 @@ __device__ __noinline__ void tile_shift_cell_general(const Params& p, const Smem
 
 // The ordinary cells of sub-sweep k: the cells of local colour QL at ring >= k.  Warps draw chunks of 32 cells from a
 // shared counter, so a warp that was busy with a crowded cell (or started late) simply takes fewer.
-template <typename P, int NS, bool DEBUG, uint32_t QL>
+// The local colour QL is a run-time value and ONE copy of the update serves the four sub-sweeps: this variant runs the
+// small and middle-sized systems, whose sub-sweeps are a single batch per warp — every phase a cold start — and with four
+// specialised copies 30 % of the working warps' stall samples were instruction fetch (ncu at C2).
+template <typename P, int NS, bool DEBUG>
 __device__ __forceinline__ void tile_sub_sweep_cells(const Params& p, SmemCell<P>* sm, const CrowdList<P>& cl,
-                                                     const uint32_t nc, const TileBox& tb, const uint32_t k,
+                                                     const uint32_t nc, const TileBox& tb, const uint32_t QL, const uint32_t k,
                                                      const uint32_t dir, const int gx0, const int gy0,
                                                      const unsigned long long t, uint32_t* next, Tally& tally) {
-  constexpr uint32_t qx = QL & 1u, qy = QL >> 1;
+  const uint32_t qx = QL & 1u, qy = QL >> 1;
   const uint32_t PS = p.tl_PS, pw = tb.pw;
+  int noff[9];
+#pragma unroll
+  for (int idx = 0; idx < 9; ++idx) noff[idx] = neighbour_offset(QL, idx % 3 - 1, idx / 3 - 1, PS, pw);
   const SubRect rc = sub_sweep_rect(tb, k, dir);
   const uint32_t px0 = (rc.x_lo - qx + 1u) >> 1, px1 = (rc.x_hi - qx) >> 1;
   const uint32_t py0 = (rc.y_lo - qy + 1u) >> 1, py1 = (rc.y_hi - qy) >> 1;
@@ -538,7 +460,7 @@ __device__ __forceinline__ void tile_sub_sweep_cells(const Params& p, SmemCell<P
     const uint32_t si = QL * PS + py * pw + px;
     const uint32_t cell = wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx);
     const bool interior = lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY;
-    tile_update_cell<P, NS, DEBUG, QL>(p, sm, si, pw, cell, interior, t, tally);
+    tile_update_cell<P, NS, DEBUG>(p, sm, si, noff, cell, interior, t, tally);
   }
 }
 
@@ -797,7 +719,7 @@ __device__ __forceinline__ void tile_run_sorted(const Params& p, SmemCell<P>* sm
     const uint32_t py = small_div(v, inv_pw), px = v - py * pw, lx = 2u * px + qx, ly = 2u * py + qy;
     const uint32_t cell = wrap_cell(gy0 + (int)ly, p.my) * p.mx + wrap_cell(gx0 + (int)lx, p.mx);
     const bool interior = lx - (uint32_t)HALO < tb.TX && ly - (uint32_t)HALO < tb.TY;
-    if (general) tile_update_cell_rt<P, NS, DEBUG>(p, sm, q * PS + v, noff, cell, interior, t, tally);
+    if (general) tile_update_cell<P, NS, DEBUG>(p, sm, q * PS + v, noff, cell, interior, t, tally);
     else         tile_update_simple<P, NS, DEBUG>(p, sm, q * PS + v, noff, cell, interior, t, tally);
   }
 }
@@ -1223,12 +1145,7 @@ k_tile_sweep(const __grid_constant__ Params p, const unsigned long long t, const
       tile_run_sorted<P, NS, DEBUG>(p, sm, tb, q, gx0, gy0, t, queues + (k - 1u) * PS, s_cnt[k - 1u][0], s_cnt[k - 1u][1],
                                     &s_next[k - 1u], tally);
     } else {
-      switch (q) {                                 // the local colour as a compile-time constant: uniform offsets
-        case 0: tile_sub_sweep_cells<P, NS, DEBUG, 0>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
-        case 1: tile_sub_sweep_cells<P, NS, DEBUG, 1>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
-        case 2: tile_sub_sweep_cells<P, NS, DEBUG, 2>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
-        default: tile_sub_sweep_cells<P, NS, DEBUG, 3>(p, sm, cl, nc, tb, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally); break;
-      }
+      tile_sub_sweep_cells<P, NS, DEBUG>(p, sm, cl, nc, tb, q, k, dr.dir, gx0, gy0, t, &s_next[k - 1u], tally);
     }
     __syncthreads();
     MPMC_PHASE_MARK(2 + k);
